@@ -1,0 +1,169 @@
+/*
+ * ttdft.h -- C ABI of the B200-native Chebyshev filter of ChFSI (TTDFT, arXiv 2110.15853).
+ *
+ * The library implements ONE thing: step 1 of Algorithm 1, the degree-m scaled
+ * three-term Chebyshev recurrence whose every step multiplies the sparse symmetric Kohn-Sham
+ * Hamiltonian H (M x M, localized Tucker tensor basis) by a dense block of
+ * wavefunctions X (M x N_orb), plus the bare product it is made of.
+ *
+ * Conventions (all calls):
+ *   - All matrices are fp64.  X, Y, ... are ROW-MAJOR M x ncols with a leading dimension (in
+ *     elements) ld >= ncols.  Indices are 0-based int32.
+ *   - Unless a parameter is documented as HOST, every data pointer is a DEVICE pointer owned by the
+ *     caller.  The library allocates no device memory: the converted H lives in the caller's
+ *     `dev_storage`, scratch panels in the caller's `work`.
+ *   - `stream` is a CUDA stream handle (cudaStream_t / CUstream) passed as void*; NULL = the legacy
+ *     default stream.  Work is enqueued on it and the call returns without synchronising, except
+ *     where stated.
+ *   - Every call returns a ttdft_status.  On a non-OK status no output has been modified, and
+ *     ttdft_last_error() returns a thread-local message.  Nothing throws or aborts.
+ *   - H is used AS STORED (both triangles present); symmetry is a promise that is only checked on
+ *     request, and results are defined for a non-symmetric H too.
+ */
+#ifndef TTDFT_H
+#define TTDFT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ttdft_h_s* ttdft_h_t; /* opaque handle, host object owned by the library */
+
+typedef enum {
+  TTDFT_OK = 0,
+  TTDFT_ERR_INVALID_ARG = 1,
+  TTDFT_ERR_UNSUPPORTED = 2,
+  TTDFT_ERR_WORKSPACE_TOO_SMALL = 3,
+  TTDFT_ERR_NOT_SYMMETRIC = 4,
+  TTDFT_ERR_CUDA = 5
+} ttdft_status;
+
+typedef enum { TTDFT_FMT_CSR = 0, TTDFT_FMT_BSR = 1 } ttdft_format;
+
+/* flags for ttdft_h_desc.flags */
+#define TTDFT_CHECK_SORTED 1u   /* verify indices in range, ascending and unique per row (synchronises) */
+#define TTDFT_CHECK_SYMMETRY 2u /* verify H == H^T bit for bit (synchronises; needs sorted columns)      */
+#define TTDFT_FORCE_GENERIC 4u  /* keep the input format and use the generic row-per-warp kernel          */
+
+/*
+ * Description of the input Hamiltonian (PAPER.md:L199-205 H^L; L250-252 block structure: "the
+ * diagonal blocks are much denser compared to the off-diagonal blocks").
+ *   CSR: row_ptr[M+1], col_idx[nnz] ascending and unique per row, values[nnz]; explicit zeros are
+ *        allowed and treated as values.  nnz < 2^31.
+ *   BSR: row_ptr[M/block+1], col_idx[nblocks] block columns ascending per block row,
+ *        values[nblocks*block*block], each block a row-major block x block tile.  M % block == 0.
+ *   subdomain_of_row (CSR only, optional, may be NULL): subdomain label of every row.  If the labels
+ *        are non-decreasing and every subdomain owns the same number b of rows, with b in
+ *        {32, 64, 96, 128}, the builder groups each localized subdomain's basis functions into b x b
+ *        tiles (block-sparse storage); otherwise the CSR is kept as is.
+ * All four arrays are DEVICE pointers; the struct itself is a HOST object.
+ */
+typedef struct {
+  ttdft_format fmt;
+  int64_t M;
+  int32_t block;
+  const int32_t* row_ptr;
+  const int32_t* col_idx;
+  const double* values;
+  const int32_t* subdomain_of_row;
+  uint32_t flags;
+} ttdft_h_desc;
+
+/* read-back description of a built handle (all HOST values) */
+typedef struct {
+  int64_t M;
+  int64_t nnz_stored;     /* stored scalar entries incl. explicit zeros (BSR: nblocks*b*b) */
+  int32_t block;          /* tile size of the device format, 0 if CSR                       */
+  int32_t kernel;         /* 1 = block-sparse TMA + fp64 tensor-core kernel, 0 = generic    */
+  int64_t nblocks;
+  size_t storage_bytes;
+} ttdft_h_info_t;
+
+/* A0 -- storage builder (north_star "BSR/CSR storage builder"). */
+
+/* Bytes of device storage ttdft_h_build needs for this description.  Reads row_ptr's last entry
+ * from the device (synchronises `stream`-less: uses a blocking 4-byte copy). */
+ttdft_status ttdft_h_storage_bytes(const ttdft_h_desc* desc, size_t* bytes);
+
+/* Validate and convert H into the device format inside dev_storage (>= the bytes reported above,
+ * 1024-byte aligned).  The input arrays may be freed once `stream` has passed this call; the handle
+ * only points into dev_storage, is immutable afterwards, and may be used from several streams.
+ * With a CHECK flag the call synchronises `stream` and reports TTDFT_ERR_INVALID_ARG (unsorted /
+ * out-of-range indices) or TTDFT_ERR_NOT_SYMMETRIC. */
+ttdft_status ttdft_h_build(const ttdft_h_desc* desc, void* dev_storage, size_t bytes, void* stream,
+                           ttdft_h_t* out);
+ttdft_status ttdft_h_info(ttdft_h_t h, ttdft_h_info_t* info);
+ttdft_status ttdft_h_destroy(ttdft_h_t h);
+
+/*
+ * Y = alpha * H * X + beta * Y         (the kernel of every filter step)
+ * X, Y: M x ncols, ncols >= 1.  X must not overlap Y.  beta == 0 does not read Y (NaN-safe);
+ * alpha == 0 does not read H or X.
+ */
+ttdft_status ttdft_spmm(ttdft_h_t h, double alpha, const double* X, int64_t ldx, double beta, double* Y,
+                        int64_t ldy, int64_t ncols, void* stream);
+
+/*
+ * One fused recurrence step:
+ *     Yout = alpha * (H * Yk - c * Yk) + beta * Ykm1
+ * in ONE pass over H, Yk and Ykm1 (scale, shift and axpby live in the product's epilogue).
+ * Ykm1 == NULL means the beta term is absent (the first step).  Ykm1 may be the
+ * same matrix as Yout (it is only read at the output position); Yk must not overlap Yout.
+ */
+ttdft_status ttdft_cheb_step(ttdft_h_t h, double alpha, double c, double beta, const double* Yk, int64_t ldk,
+                             const double* Ykm1, int64_t ldm, double* Yout, int64_t ldo, int64_t ncols,
+                             void* stream);
+
+/*
+ * A1 -- the scalars of Algorithm 1, HOST arrays of length m:
+ *   e = (b-a)/2, c = (b+a)/2, sigma_1 = e/(a0-c), gamma = 2/sigma_1, sigma_{k+1} = 1/(gamma-sigma_k)
+ *   alpha[0] = sigma_1/e, beta[0] = 0;   alpha[k] = 2*sigma_{k+1}/e, beta[k] = -sigma_k*sigma_{k+1}
+ * so that step k (0-based) is  Y_{k+1} = alpha[k]*(H*Y_k - c*Y_k) + beta[k]*Y_{k-1},  Y_0 = X.
+ * a = eps_ub^w, b = eps_ub^uw, a0 = eps_0.  Requires m >= 0, a0 < a < b.
+ */
+ttdft_status ttdft_cheb_scalars(int32_t m, double a, double b, double a0, double* c_out, double* alpha,
+                                double* beta);
+
+/* Bytes of scratch ttdft_cheb_filter needs: one compact M x panel panel (panel_cols == 0: the
+ * library's default panel width for this ncols). */
+ttdft_status ttdft_cheb_filter_work_bytes(ttdft_h_t h, int64_t ncols, int64_t panel_cols, size_t* bytes);
+
+/*
+ * Y = p_m(H) X,  p_m(t) = T_m((t-c)/e) / T_m((a0-c)/e)      (Algorithm 1, step 1)
+ * computed as m fused steps per column panel of width panel_cols (0 = default), the iterates
+ * rotating between the X panel, the Y panel and one scratch panel on `stream`.  m == 0 copies X
+ * to Y.  Y may be X exactly (in place) but must not partially overlap it.  The result of every
+ * column is independent of panel_cols.  Requires ncols >= 1, m >= 0, a0 < a < b.
+ */
+ttdft_status ttdft_cheb_filter(ttdft_h_t h, const double* X, int64_t ldx, double* Y, int64_t ldy, int64_t ncols,
+                               int32_t m, double a, double b, double a0, int64_t panel_cols, void* work,
+                               size_t work_bytes, void* stream);
+
+/*
+ * The same filter with X and Y in HOST memory (pinned for full speed): column panels are copied
+ * host->device, filtered, and copied device->host, the copies of neighbouring panels overlapping
+ * the arithmetic.  `work` is DEVICE scratch of at least ttdft_cheb_filter_host_work_bytes.  The call
+ * returns after the last panel has reached Y (it synchronises).
+ */
+ttdft_status ttdft_cheb_filter_host_work_bytes(ttdft_h_t h, int64_t ncols, int64_t panel_cols, size_t* bytes);
+ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* X_host, int64_t ldx, double* Y_host, int64_t ldy,
+                                    int64_t ncols, int32_t m, double a, double b, double a0, int64_t panel_cols,
+                                    void* work, size_t work_bytes, void* stream);
+
+/* Measured fp64 rate of this GPU: kind 0 = scalar DFMA loop, 1 = DMMA (mma.sync m8n8k4.f64) loop;
+ * runs for about `millis` ms on `stream`, synchronises, returns TFLOP/s in *tflops. */
+ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, double* tflops);
+
+/* Number of kernels this library has launched since load (all threads). */
+int64_t ttdft_launch_count(void);
+
+/* Thread-local message describing the last non-OK status returned on this thread ("" if none). */
+const char* ttdft_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TTDFT_H */

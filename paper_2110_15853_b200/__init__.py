@@ -1,0 +1,29 @@
+"""B200-native Chebyshev filter of ChFSI (TTDFT, arXiv 2110.15853, Algorithm 1 step 1).
+
+Thin Python binding over the C-ABI library ``libttdft.so`` (``include/ttdft.h``).  PyTorch is used
+for device memory and streams only; every step of the path runs in the library's CUDA kernels.
+There is no CPU fallback: if the library is missing or no CUDA device is present, calls fail.
+"""
+from .api import (  # noqa: F401
+    TTDFTError,
+    Hamiltonian,
+    h_storage_bytes,
+    h_build,
+    h_build_bsr,
+    h_build_csr,
+    spmm,
+    cheb_step,
+    cheb_scalars,
+    cheb_filter,
+    cheb_filter_work_bytes,
+    cheb_filter_host,
+    cheb_filter_host_work_bytes,
+    probe_fp64_peak,
+    launch_count,
+    last_error,
+    library_path,
+    exported_symbols,
+    CHECK_SORTED,
+    CHECK_SYMMETRY,
+    FORCE_GENERIC,
+)

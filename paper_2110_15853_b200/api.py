@@ -1,0 +1,288 @@
+"""ctypes binding of include/ttdft.h -- argument marshalling only (same names as the C calls)."""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, byref, c_char_p, c_double, c_int32, c_int64, c_size_t, c_uint32, c_void_p
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_PKG, "libttdft.so")
+
+CHECK_SORTED, CHECK_SYMMETRY, FORCE_GENERIC = 1, 2, 4
+FMT_CSR, FMT_BSR = 0, 1
+_STATUS = {0: "OK", 1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "NOT_SYMMETRIC", 5: "CUDA"}
+
+# every symbol include/ttdft.h declares
+exported_symbols = [
+    "ttdft_h_storage_bytes", "ttdft_h_build", "ttdft_h_info", "ttdft_h_destroy", "ttdft_spmm", "ttdft_cheb_step",
+    "ttdft_cheb_scalars", "ttdft_cheb_filter_work_bytes", "ttdft_cheb_filter", "ttdft_cheb_filter_host_work_bytes",
+    "ttdft_cheb_filter_host", "ttdft_probe_fp64_peak", "ttdft_launch_count", "ttdft_last_error",
+]
+
+
+class TTDFTError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"TTDFT_ERR_{_STATUS.get(status, status)}: {message}")
+        self.status = status
+        self.status_name = _STATUS.get(status, str(status))
+
+
+class _Desc(ctypes.Structure):
+    _fields_ = [("fmt", c_int32), ("M", c_int64), ("block", c_int32), ("row_ptr", c_void_p), ("col_idx", c_void_p),
+                ("values", c_void_p), ("subdomain_of_row", c_void_p), ("flags", c_uint32)]
+
+
+class _Info(ctypes.Structure):
+    _fields_ = [("M", c_int64), ("nnz_stored", c_int64), ("block", c_int32), ("kernel", c_int32), ("nblocks", c_int64),
+                ("storage_bytes", c_size_t)]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def _load() -> ctypes.CDLL:
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} is missing: build it with `python -m paper_2110_15853_b200.build` "
+                          "(there is no CPU fallback)")
+    L = ctypes.CDLL(_LIB_PATH)
+    st = c_int32
+    L.ttdft_h_storage_bytes.restype = st
+    L.ttdft_h_storage_bytes.argtypes = [POINTER(_Desc), POINTER(c_size_t)]
+    L.ttdft_h_build.restype = st
+    L.ttdft_h_build.argtypes = [POINTER(_Desc), c_void_p, c_size_t, c_void_p, POINTER(c_void_p)]
+    L.ttdft_h_info.restype = st
+    L.ttdft_h_info.argtypes = [c_void_p, POINTER(_Info)]
+    L.ttdft_h_destroy.restype = st
+    L.ttdft_h_destroy.argtypes = [c_void_p]
+    L.ttdft_spmm.restype = st
+    L.ttdft_spmm.argtypes = [c_void_p, c_double, c_void_p, c_int64, c_double, c_void_p, c_int64, c_int64, c_void_p]
+    L.ttdft_cheb_step.restype = st
+    L.ttdft_cheb_step.argtypes = [c_void_p, c_double, c_double, c_double, c_void_p, c_int64, c_void_p, c_int64, c_void_p,
+                                  c_int64, c_int64, c_void_p]
+    L.ttdft_cheb_scalars.restype = st
+    L.ttdft_cheb_scalars.argtypes = [c_int32, c_double, c_double, c_double, POINTER(c_double), POINTER(c_double),
+                                     POINTER(c_double)]
+    L.ttdft_cheb_filter_work_bytes.restype = st
+    L.ttdft_cheb_filter_work_bytes.argtypes = [c_void_p, c_int64, c_int64, POINTER(c_size_t)]
+    L.ttdft_cheb_filter_host_work_bytes.restype = st
+    L.ttdft_cheb_filter_host_work_bytes.argtypes = [c_void_p, c_int64, c_int64, POINTER(c_size_t)]
+    for name in ("ttdft_cheb_filter", "ttdft_cheb_filter_host"):
+        fn = getattr(L, name)
+        fn.restype = st
+        fn.argtypes = [c_void_p, c_void_p, c_int64, c_void_p, c_int64, c_int64, c_int32, c_double, c_double, c_double,
+                       c_int64, c_void_p, c_size_t, c_void_p]
+    L.ttdft_probe_fp64_peak.restype = st
+    L.ttdft_probe_fp64_peak.argtypes = [c_int32, c_int32, c_void_p, POINTER(c_double)]
+    L.ttdft_launch_count.restype = c_int64
+    L.ttdft_launch_count.argtypes = []
+    L.ttdft_last_error.restype = c_char_p
+    L.ttdft_last_error.argtypes = []
+    _lib = L
+    return L
+
+
+def last_error() -> str:
+    return _load().ttdft_last_error().decode()
+
+
+def launch_count() -> int:
+    return int(_load().ttdft_launch_count())
+
+
+def _check(status: int):
+    if status != 0:
+        raise TTDFTError(status, last_error())
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2110_15853_b200 needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+def _stream(stream=None) -> int:
+    torch = _torch()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def _mat(t, name="matrix"):
+    """(device pointer, leading dimension) of a row-major fp64 CUDA matrix view."""
+    torch = _torch()
+    if t.dtype != torch.float64 or not t.is_cuda or t.dim() != 2:
+        raise TypeError(f"{name} must be a 2-D float64 CUDA tensor")
+    if t.shape[1] > 1 and t.stride(1) != 1:
+        raise ValueError(f"{name} must be row-major with unit column stride")
+    ld = t.stride(0) if t.shape[0] > 1 else max(t.shape[1], t.stride(0))
+    return t.data_ptr(), int(ld)
+
+
+class Hamiltonian:
+    """A built H: owns the device storage tensor and the library handle (ttdft_h_t)."""
+
+    def __init__(self, handle: int, storage, M: int):
+        self._h = c_void_p(handle)
+        self.storage = storage
+        self.M = M
+
+    @property
+    def handle(self) -> c_void_p:
+        if self._h is None:
+            raise RuntimeError("Hamiltonian was destroyed")
+        return self._h
+
+    def info(self) -> dict:
+        inf = _Info()
+        _check(_load().ttdft_h_info(self.handle, byref(inf)))
+        return {k: getattr(inf, k) for k, _ in _Info._fields_}
+
+    def destroy(self):
+        if self._h is not None:
+            _load().ttdft_h_destroy(self._h)
+            self._h = None
+            self.storage = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def _desc(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row, flags) -> _Desc:
+    torch = _torch()
+    for t, dt, nm in ((row_ptr, torch.int32, "row_ptr"), (col_idx, torch.int32, "col_idx"), (values, torch.float64, "values")):
+        if t is not None and (t.dtype != dt or not t.is_cuda or not t.is_contiguous()):
+            raise TypeError(f"{nm} must be a contiguous {dt} CUDA tensor")
+    d = _Desc()
+    d.fmt, d.M, d.block, d.flags = fmt, M, block, flags
+    d.row_ptr = row_ptr.data_ptr() if row_ptr is not None else None
+    d.col_idx = col_idx.data_ptr() if col_idx is not None and col_idx.numel() else None
+    d.values = values.data_ptr() if values is not None and values.numel() else None
+    d.subdomain_of_row = subdomain_of_row.data_ptr() if subdomain_of_row is not None else None
+    return d
+
+
+def h_storage_bytes(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row=None, flags=0) -> int:
+    d = _desc(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row, flags)
+    n = c_size_t()
+    _check(_load().ttdft_h_storage_bytes(byref(d), byref(n)))
+    return int(n.value)
+
+
+def h_build(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row=None, flags=0, stream=None) -> Hamiltonian:
+    """ttdft_h_build: validate + convert H into library-format device storage (allocated here by torch)."""
+    torch = _torch()
+    d = _desc(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row, flags)
+    n = c_size_t()
+    L = _load()
+    _check(L.ttdft_h_storage_bytes(byref(d), byref(n)))
+    storage = torch.empty(max(int(n.value), 1024) + 1024, dtype=torch.uint8, device=values.device if values is not None else "cuda")
+    base = storage.data_ptr()
+    aligned = (base + 1023) // 1024 * 1024
+    h = c_void_p()
+    _check(L.ttdft_h_build(byref(d), c_void_p(aligned), c_size_t(int(n.value)), c_void_p(_stream(stream)), byref(h)))
+    return Hamiltonian(h.value, storage, M)
+
+
+def h_build_bsr(M, block, row_ptr, col_idx, values, flags=0, stream=None) -> Hamiltonian:
+    return h_build(FMT_BSR, M, block, row_ptr, col_idx, values.reshape(-1), None, flags, stream)
+
+
+def h_build_csr(M, row_ptr, col_idx, values, subdomain_of_row=None, flags=0, stream=None) -> Hamiltonian:
+    return h_build(FMT_CSR, M, 0, row_ptr, col_idx, values, subdomain_of_row, flags, stream)
+
+
+def spmm(H: Hamiltonian, alpha: float, X, beta: float, Y, stream=None):
+    """Y = alpha*H*X + beta*Y (ttdft_spmm)."""
+    xp, ldx = _mat(X, "X")
+    yp, ldy = _mat(Y, "Y")
+    if X.shape != Y.shape or X.shape[0] != H.M:
+        raise ValueError("shape mismatch")
+    _check(_load().ttdft_spmm(H.handle, alpha, xp, ldx, beta, yp, ldy, X.shape[1], _stream(stream)))
+    return Y
+
+
+def cheb_step(H: Hamiltonian, alpha: float, c: float, beta: float, Yk, Ykm1, Yout, stream=None):
+    """Yout = alpha*(H*Yk - c*Yk) + beta*Ykm1 (ttdft_cheb_step); Ykm1 None = beta term absent."""
+    kp, ldk = _mat(Yk, "Yk")
+    op, ldo = _mat(Yout, "Yout")
+    mp, ldm = (None, 0) if Ykm1 is None else _mat(Ykm1, "Ykm1")
+    if Yk.shape != Yout.shape or Yk.shape[0] != H.M or (Ykm1 is not None and Ykm1.shape != Yk.shape):
+        raise ValueError("shape mismatch")
+    _check(_load().ttdft_cheb_step(H.handle, alpha, c, beta, kp, ldk, mp, ldm, op, ldo, Yk.shape[1], _stream(stream)))
+    return Yout
+
+
+def cheb_scalars(m: int, a: float, b: float, a0: float):
+    """(c, alpha[m], beta[m]) of Algorithm 1 (ttdft_cheb_scalars); host-only, needs no GPU."""
+    n = max(m, 1)
+    al = (c_double * n)()
+    be = (c_double * n)()
+    c = c_double()
+    _check(_load().ttdft_cheb_scalars(m, a, b, a0, byref(c), al, be))
+    return c.value, list(al)[:max(m, 0)], list(be)[:max(m, 0)]
+
+
+def cheb_filter_work_bytes(H: Hamiltonian, ncols: int, panel_cols: int = 0) -> int:
+    n = c_size_t()
+    _check(_load().ttdft_cheb_filter_work_bytes(H.handle, ncols, panel_cols, byref(n)))
+    return int(n.value)
+
+
+def cheb_filter(H: Hamiltonian, X, Y, m: int, a: float, b: float, a0: float, panel_cols: int = 0, work=None, stream=None):
+    """Y = p_m(H) X (ttdft_cheb_filter).  `work`: uint8/float64 CUDA tensor of >= cheb_filter_work_bytes."""
+    torch = _torch()
+    xp, ldx = _mat(X, "X")
+    yp, ldy = _mat(Y, "Y")
+    if X.shape != Y.shape or X.shape[0] != H.M:
+        raise ValueError("shape mismatch")
+    ncols = X.shape[1]
+    if work is None:
+        work = torch.empty(cheb_filter_work_bytes(H, ncols, panel_cols) + 16, dtype=torch.uint8, device=X.device)
+    wp = (work.data_ptr() + 15) // 16 * 16
+    wbytes = work.numel() * work.element_size() - (wp - work.data_ptr())
+    _check(_load().ttdft_cheb_filter(H.handle, xp, ldx, yp, ldy, ncols, m, a, b, a0, panel_cols, wp, wbytes, _stream(stream)))
+    return Y
+
+
+def cheb_filter_host_work_bytes(H: Hamiltonian, ncols: int, panel_cols: int = 0) -> int:
+    n = c_size_t()
+    _check(_load().ttdft_cheb_filter_host_work_bytes(H.handle, ncols, panel_cols, byref(n)))
+    return int(n.value)
+
+
+def cheb_filter_host(H: Hamiltonian, X_host, Y_host, m: int, a: float, b: float, a0: float, panel_cols: int = 0, work=None,
+                     stream=None):
+    """The filter with X, Y in HOST memory (CPU float64 tensors, pinned for speed); copies are inside the call."""
+    torch = _torch()
+    for t in (X_host, Y_host):
+        if t.dtype != torch.float64 or t.is_cuda or t.dim() != 2 or (t.shape[1] > 1 and t.stride(1) != 1):
+            raise TypeError("X_host/Y_host must be row-major 2-D float64 CPU tensors")
+    if X_host.shape != Y_host.shape or X_host.shape[0] != H.M:
+        raise ValueError("shape mismatch")
+    ncols = X_host.shape[1]
+    ldx = X_host.stride(0) if X_host.shape[0] > 1 else ncols
+    ldy = Y_host.stride(0) if Y_host.shape[0] > 1 else ncols
+    if work is None:
+        work = torch.empty(cheb_filter_host_work_bytes(H, ncols, panel_cols) + 1024, dtype=torch.uint8, device="cuda")
+    wp = (work.data_ptr() + 1023) // 1024 * 1024
+    wbytes = work.numel() * work.element_size() - (wp - work.data_ptr())
+    _check(_load().ttdft_cheb_filter_host(H.handle, X_host.data_ptr(), ldx, Y_host.data_ptr(), ldy, ncols, m, a, b, a0,
+                                          panel_cols, wp, wbytes, _stream(stream)))
+    return Y_host
+
+
+def probe_fp64_peak(kind: int = 1, millis: int = 200, stream=None) -> float:
+    """Measured fp64 TFLOP/s of this GPU (0: DFMA loop, 1: DMMA m8n8k4 loop)."""
+    v = c_double()
+    _check(_load().ttdft_probe_fp64_peak(kind, millis, _stream(stream), byref(v)))
+    return v.value

@@ -1,0 +1,246 @@
+// bsr_dmma.cuh -- the hot kernel: block-sparse H (b x b fp64 tiles) times a dense column tile of
+// Y_k, with the recurrence's scale, shift and axpby fused into the epilogue
+// (PAPER.md:L218, L221:  Y_{k+1} = alpha (H Y_k - c Y_k) + beta Y_{k-1};  L236: the SpMM is the kernel).
+//
+// sm_100a design:
+//   * one CTA per (block row I, 128-column tile); 2*WR consumer warps (WR = b/32) + 1 producer warp
+//   * the producer streams H_IJ[:, k0:k0+16] (b x 16) and Y_k[J*b+k0 : +16, 128 cols] through a
+//     ring of NSTAGE shared-memory stages with TMA (cp.async.bulk.tensor.2d, SWIZZLE_128B) and
+//     mbarrier full/empty pairs -- no thread ever computes a global address for operands
+//   * consumers contract with fp64 tensor-core MMA (mma.sync.m8n8k4.f64 -> SASS DMMA.8x8x4; sm_100a
+//     has no f64 kind in tcgen05), 32 x 64 per warp, accumulators in registers
+//   * the k index and the row index inside an MMA are permuted so that every fragment load from the
+//     swizzled stages is bank-conflict free (A: LDS.128, B: LDS.64)
+//   * epilogue: out = alpha*acc + gamma*Y_k + beta*Y_{k-1} with 128-bit loads/stores
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ttdft {
+
+constexpr int K1_TN = 128;                 // columns per CTA tile
+constexpr int K1_KS = 16;                  // k-slab per stage (16 doubles = one 128-byte swizzle row)
+constexpr int K1_NGRP = K1_TN / 16;        // 16-column groups per tile (one TMA box each)
+constexpr int K1_BGRP_BYTES = K1_KS * 128; // 16 k-rows x 128 B
+constexpr int K1_NSTAGE = 6;
+
+struct K1Params {
+  const int32_t* brow_ptr;
+  const int32_t* bcol;
+  int32_t nb;          // block rows
+  int32_t nct;         // column tiles = ceil(ncols/128)
+  int32_t cg;          // column tiles per scheduling group (L2 reuse of Y_k across block rows)
+  int32_t vec;         // 1: S, Z, O are 16-byte aligned with even leading dimensions
+  int64_t ncols;
+  double alpha, gamma, beta;
+  const double* S;     // shift source (Y_k), read at the output position; unused if gamma == 0
+  int64_t lds;
+  const double* Z;     // Y_{k-1} (or Y for spmm), read at the output position; unused if beta == 0
+  int64_t ldz;
+  double* O;
+  int64_t ldo;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, int32_t x, int32_t y, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+          smem_u32(dst)),
+      "l"(map), "r"(x), "r"(y), "r"(smem_u32(bar))
+      : "memory");
+}
+__device__ __forceinline__ void dmma_8x8x4(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(c0), "+d"(c1)
+               : "d"(a), "d"(b));
+}
+
+template <int WR>
+struct K1Smem {
+  static constexpr int A_BYTES = WR * 32 * 128;
+  static constexpr int STAGE_BYTES = A_BYTES + K1_NGRP * K1_BGRP_BYTES;
+  static constexpr int BAR_OFFSET = K1_NSTAGE * STAGE_BYTES;
+  static constexpr int TOTAL = BAR_OFFSET + 2 * K1_NSTAGE * 8 + 1024;  // + alignment slack
+};
+
+template <int WR>
+__global__ void __launch_bounds__(32 * (2 * WR + 1), 1)
+bsr_dmma_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmX, const K1Params prm) {
+  constexpr int B = WR * 32;
+  constexpr int NCW = 2 * WR;  // consumer warps
+  using SM = K1Smem<WR>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + SM::BAR_OFFSET);
+  uint64_t* empty = full + K1_NSTAGE;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  // ---- tile decode: column-tile groups outermost, then block rows, column tile fastest ----
+  int32_t I, ct;
+  {
+    const int64_t per_group = (int64_t)prm.nb * prm.cg;
+    const int32_t ngroups = (prm.nct + prm.cg - 1) / prm.cg;
+    int32_t g = (int32_t)((int64_t)blockIdx.x / per_group);
+    if (g > ngroups - 1) g = ngroups - 1;
+    const int64_t rem = (int64_t)blockIdx.x - (int64_t)g * per_group;
+    const int32_t width = min(prm.cg, prm.nct - g * prm.cg);
+    I = (int32_t)(rem / width);
+    ct = g * prm.cg + (int32_t)(rem % width);
+  }
+  const int32_t p_begin = prm.brow_ptr[I], p_end = prm.brow_ptr[I + 1];
+  const int32_t col0 = ct * K1_TN;
+  const int32_t ngrp_valid = min(K1_NGRP, (int32_t)((prm.ncols - col0 + 15) / 16));
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < K1_NSTAGE; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], NCW);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp == NCW) {
+    // =========================== TMA producer (one elected lane) ===========================
+    if (lane == 0) {
+      asm volatile("prefetch.tensormap [%0];" ::"l"(&tmH) : "memory");
+      asm volatile("prefetch.tensormap [%0];" ::"l"(&tmX) : "memory");
+      const uint32_t tx_bytes = SM::A_BYTES + ngrp_valid * K1_BGRP_BYTES;
+      int stage = 0;
+      uint32_t phase = 0;
+      for (int32_t p = p_begin; p < p_end; ++p) {
+        const int32_t J = prm.bcol[p];
+#pragma unroll 1
+        for (int k0 = 0; k0 < B; k0 += K1_KS) {
+          mbar_wait(&empty[stage], phase ^ 1);
+          uint8_t* As = smem + stage * SM::STAGE_BYTES;
+          uint8_t* Bs = As + SM::A_BYTES;
+          mbar_expect_tx(&full[stage], tx_bytes);
+          tma_load_2d(As, &tmH, k0, p * B, &full[stage]);
+          for (int g = 0; g < ngrp_valid; ++g)
+            tma_load_2d(Bs + g * K1_BGRP_BYTES, &tmX, col0 + g * 16, J * B + k0, &full[stage]);
+          if (++stage == K1_NSTAGE) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+    return;
+  }
+
+  // ================================ consumers: 32 x 64 per warp ================================
+  const int wr = warp >> 1, wc = warp & 1;
+  const int g = lane >> 2, t = lane & 3;
+  const int rho = 4 * (g & 1) + (g >> 1);  // MMA row g  <->  tile row rho (bank-conflict-free LDS.128)
+
+  double acc[4][8][2];
+#pragma unroll
+  for (int p = 0; p < 4; ++p)
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { acc[p][q][0] = 0.0; acc[p][q][1] = 0.0; }
+
+  // per-lane byte offsets inside a stage
+  const uint32_t a_row = (uint32_t)(32 * wr + rho) * 128u;
+  const uint32_t a_off0 = a_row + (uint32_t)((t ^ rho) << 4);        // k = 2t, 2t+1
+  const uint32_t a_off1 = a_row + (uint32_t)(((4 + t) ^ rho) << 4);  // k = 8+2t, 8+2t+1
+  const uint32_t Lx = (uint32_t)((g >> 1) ^ (2 * t));                // lane part of the B chunk index
+  const uint32_t b_base = (uint32_t)SM::A_BYTES + (uint32_t)(4 * wc) * K1_BGRP_BYTES + (uint32_t)(2 * t) * 128u +
+                          (uint32_t)(g & 1) * 8u;
+
+  const int nstages_total = (p_end - p_begin) * (B / K1_KS);
+  int stage = 0;
+  uint32_t phase = 0;
+  const uint32_t smem_base = smem_u32(smem);
+#pragma unroll 1
+  for (int it = 0; it < nstages_total; ++it) {
+    mbar_wait(&full[stage], phase);
+    const uint32_t sb = smem_base + stage * SM::STAGE_BYTES;
+    // A fragments: a[p][s], MMA step s uses k = 2t + (s&1) + 8(s>>1)
+    double a[4][4];
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(a[p][0]), "=d"(a[p][1]) : "r"(sb + a_off0 + p * 1024u));
+      asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(a[p][2]), "=d"(a[p][3]) : "r"(sb + a_off1 + p * 1024u));
+    }
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+      double bf[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const uint32_t cqs = (uint32_t)((4 * (q & 1)) ^ (s & 1));
+        const uint32_t off = b_base + (uint32_t)(q >> 1) * K1_BGRP_BYTES + (uint32_t)((s & 1) + 8 * (s >> 1)) * 128u +
+                             ((Lx ^ cqs) << 4);
+        asm volatile("ld.shared.f64 %0, [%1];" : "=d"(bf[q]) : "r"(sb + off));
+      }
+#pragma unroll
+      for (int p = 0; p < 4; ++p)
+#pragma unroll
+        for (int q = 0; q < 8; ++q) dmma_8x8x4(acc[p][q][0], acc[p][q][1], a[p][s], bf[q]);
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[stage]);
+    if (++stage == K1_NSTAGE) { stage = 0; phase ^= 1; }
+  }
+
+  // ---- fused epilogue: out = alpha*acc + gamma*S + beta*Z at the output position ----
+  const double alpha = prm.alpha, gamma = prm.gamma, beta = prm.beta;
+  const bool use_s = (gamma != 0.0), use_z = (beta != 0.0);
+#pragma unroll
+  for (int p = 0; p < 4; ++p) {
+    const int64_t row = (int64_t)I * B + 32 * wr + 8 * p + rho;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      const int64_t col = (int64_t)col0 + 64 * wc + 8 * q + 2 * t;
+      if (col >= prm.ncols) continue;
+      double v0 = alpha * acc[p][q][0], v1 = alpha * acc[p][q][1];
+      if (prm.vec && col + 1 < prm.ncols) {
+        if (use_s) {
+          const double2 s2 = *reinterpret_cast<const double2*>(prm.S + row * prm.lds + col);
+          v0 = fma(gamma, s2.x, v0);
+          v1 = fma(gamma, s2.y, v1);
+        }
+        if (use_z) {
+          const double2 z2 = *reinterpret_cast<const double2*>(prm.Z + row * prm.ldz + col);
+          v0 = fma(beta, z2.x, v0);
+          v1 = fma(beta, z2.y, v1);
+        }
+        *reinterpret_cast<double2*>(prm.O + row * prm.ldo + col) = make_double2(v0, v1);
+      } else {
+        if (use_s) v0 = fma(gamma, prm.S[row * prm.lds + col], v0);
+        if (use_z) v0 = fma(beta, prm.Z[row * prm.ldz + col], v0);
+        prm.O[row * prm.ldo + col] = v0;
+        if (col + 1 < prm.ncols) {
+          if (use_s) v1 = fma(gamma, prm.S[row * prm.lds + col + 1], v1);
+          if (use_z) v1 = fma(beta, prm.Z[row * prm.ldz + col + 1], v1);
+          prm.O[row * prm.ldo + col + 1] = v1;
+        }
+      }
+    }
+  }
+}
+
+}  // namespace ttdft

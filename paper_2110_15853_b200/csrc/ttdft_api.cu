@@ -1,0 +1,866 @@
+// ttdft_api.cu -- C ABI of include/ttdft.h: storage builder (A0), host scalars (A1), step dispatch
+// (A2/A3), buffer rotation (A4), column-panel loop (A5), output placement (A6).
+// Algorithm 1 step 1 of arXiv 2110.15853.  No CPU fallback exists: every entry
+// point that computes launches the CUDA kernels below or fails with TTDFT_ERR_CUDA.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/ttdft.h"
+#include "bsr_dmma.cuh"
+#include "generic_spmm.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+std::atomic<int64_t> g_launches{0};
+
+ttdft_status fail(ttdft_status st, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return st;
+}
+
+#define CUDA_TRY(expr)                                                                                  \
+  do {                                                                                                  \
+    cudaError_t e__ = (expr);                                                                           \
+    if (e__ != cudaSuccess) return fail(TTDFT_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e__));     \
+  } while (0)
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ------------------------------------------------------------------------------------------------
+// driver entry point for tensor-map encoding (no link-time dependency on libcuda)
+// ------------------------------------------------------------------------------------------------
+typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+encode_tiled_fn get_encode() {
+  static encode_tiled_fn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return (encode_tiled_fn)p;
+  }();
+  return fn;
+}
+
+// 2-D fp64 row-major tensor [rows][cols] with row pitch ld (elements), box = box_rows x 16, 128B swizzle
+ttdft_status make_map_2d(CUtensorMap* map, const void* base, uint64_t cols, uint64_t rows, uint64_t ld,
+                         uint32_t box_rows) {
+  encode_tiled_fn enc = get_encode();
+  if (!enc) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {ld * 8};
+  cuuint32_t box[2] = {16, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<void*>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+  return TTDFT_OK;
+}
+
+bool k1_block_ok(int32_t b) { return b == 32 || b == 64 || b == 96 || b == 128; }
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// handle
+// ------------------------------------------------------------------------------------------------
+struct ttdft_h_s {
+  int64_t M = 0;
+  int32_t kernel = 0;       // 1 = K1 (BSR, TMA + DMMA), 0 = K2 generic
+  int32_t bsr = 0;          // storage is BSR
+  int32_t b = 0;
+  int64_t nb = 0;
+  int64_t nblocks = 0;      // BSR tiles, or CSR nnz
+  const int32_t* row_ptr = nullptr;   // device, inside dev_storage
+  const int32_t* col = nullptr;
+  const double* val = nullptr;
+  size_t storage_bytes = 0;
+  CUtensorMap tmH;          // K1 only
+  int32_t cg = 4;           // column tiles per scheduling group
+};
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// builder kernels (integer work + one pass over H)
+// ------------------------------------------------------------------------------------------------
+// flags[0] |= 1 : unsorted / duplicate / out-of-range index ; flags[0] |= 2 : not symmetric
+__global__ void check_sorted_kernel(int64_t nrows, const int32_t* row_ptr, const int32_t* col, int64_t ncolmax,
+                                    int32_t* flags) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= nrows) return;
+  int32_t e0 = row_ptr[i], e1 = row_ptr[i + 1];
+  bool bad = e1 < e0;
+  for (int32_t e = e0; e < e1 && !bad; ++e) {
+    int32_t c = col[e];
+    if (c < 0 || c >= ncolmax) bad = true;
+    if (e > e0 && col[e - 1] >= c) bad = true;
+  }
+  if (bad) atomicOr(flags, 1);
+}
+
+__device__ int32_t find_col(const int32_t* col, int32_t lo, int32_t hi, int32_t key) {
+  while (lo < hi) {
+    int32_t mid = (lo + hi) >> 1;
+    int32_t c = col[mid];
+    if (c == key) return mid;
+    if (c < key) lo = mid + 1; else hi = mid;
+  }
+  return -1;
+}
+
+__global__ void check_sym_csr_kernel(int64_t M, const int32_t* row_ptr, const int32_t* col, const double* val,
+                                     int32_t* flags) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= M) return;
+  for (int32_t e = row_ptr[i]; e < row_ptr[i + 1]; ++e) {
+    int32_t j = col[e];
+    double v = val[e];
+    int32_t f = find_col(col, row_ptr[j], row_ptr[j + 1], (int32_t)i);
+    double w = f >= 0 ? val[f] : 0.0;
+    if (!(v == w)) { atomicOr(flags, 2); return; }
+  }
+}
+
+// one CTA per stored tile (I,J): compare with the transpose of tile (J,I)
+__global__ void check_sym_bsr_kernel(int32_t b, const int32_t* brow_ptr, const int32_t* bcol, const double* val,
+                                     const int32_t* tile_row, int32_t* flags) {
+  int64_t p = blockIdx.x;
+  int32_t I = tile_row[p], J = bcol[p];
+  int32_t q = find_col(bcol, brow_ptr[J], brow_ptr[J + 1], I);
+  const double* T = val + (size_t)p * b * b;
+  bool bad = false;
+  for (int idx = threadIdx.x; idx < b * b && !bad; idx += blockDim.x) {
+    int r = idx / b, s = idx % b;
+    double v = T[idx];
+    double w = q >= 0 ? val[(size_t)q * b * b + (size_t)s * b + r] : 0.0;
+    if (!(v == w)) bad = true;
+  }
+  if (bad) atomicOr(flags, 2);
+}
+
+__global__ void tile_rows_kernel(int64_t nb, const int32_t* brow_ptr, int32_t* tile_row) {
+  int64_t I = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (I >= nb) return;
+  for (int32_t p = brow_ptr[I]; p < brow_ptr[I + 1]; ++p) tile_row[p] = (int32_t)I;
+}
+
+// hint analysis: labels must be non-decreasing with equal group sizes; out[0] = ok flag, out[1] = b
+__global__ void hint_check_kernel(int64_t M, const int32_t* lab, int32_t b, int32_t* bad) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= M) return;
+  // row i must carry the label of its group's first row, and groups must be strictly increasing
+  int64_t g0 = (i / b) * b;
+  if (lab[i] != lab[g0]) atomicOr(bad, 1);
+  if (i == g0 && i > 0 && !(lab[i] > lab[i - 1])) atomicOr(bad, 1);
+}
+
+// CSR -> BSR pass 1: one CTA per block row, bitmap of touched block columns -> count
+__global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_ptr, const int32_t* col, int32_t* counts,
+                                     int32_t nwords) {
+  extern __shared__ uint32_t bits[];
+  for (int w = threadIdx.x; w < nwords; w += blockDim.x) bits[w] = 0;
+  __syncthreads();
+  int64_t I = blockIdx.x;
+  int32_t e0 = row_ptr[I * b], e1 = row_ptr[(I + 1) * b];
+  for (int32_t e = e0 + threadIdx.x; e < e1; e += blockDim.x) {
+    int32_t J = col[e] / b;
+    atomicOr(&bits[J >> 5], 1u << (J & 31));
+  }
+  __syncthreads();
+  int32_t c = 0;
+  for (int w = threadIdx.x; w < nwords; w += blockDim.x) c += __popc(bits[w]);
+  for (int o = 16; o > 0; o >>= 1) c += __shfl_down_sync(0xffffffffu, c, o);
+  __shared__ int32_t tot;
+  if (threadIdx.x == 0) tot = 0;
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) atomicAdd(&tot, c);
+  __syncthreads();
+  if (threadIdx.x == 0) counts[I] = tot;
+}
+
+// pass 2: fill bcol (ascending) and scatter the entries into zero-initialised tiles
+__global__ void csr2bsr_fill_kernel(int64_t nb, int32_t b, const int32_t* row_ptr, const int32_t* col, const double* val,
+                                    const int32_t* brow_ptr, int32_t* bcol, double* tiles, int32_t nwords) {
+  extern __shared__ uint32_t sm[];
+  uint32_t* bits = sm;                    // nwords
+  uint32_t* pref = sm + nwords;           // nwords: tiles before word w
+  for (int w = threadIdx.x; w < nwords; w += blockDim.x) bits[w] = 0;
+  __syncthreads();
+  int64_t I = blockIdx.x;
+  int32_t e0 = row_ptr[I * b], e1 = row_ptr[(I + 1) * b];
+  for (int32_t e = e0 + threadIdx.x; e < e1; e += blockDim.x) {
+    int32_t J = col[e] / b;
+    atomicOr(&bits[J >> 5], 1u << (J & 31));
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t run = 0;
+    for (int w = 0; w < nwords; ++w) { pref[w] = run; run += __popc(bits[w]); }
+  }
+  __syncthreads();
+  const int32_t p0 = brow_ptr[I];
+  for (int w = threadIdx.x; w < nwords; w += blockDim.x) {
+    uint32_t m = bits[w];
+    uint32_t k = pref[w];
+    while (m) {
+      int bit = __ffs(m) - 1;
+      bcol[p0 + k++] = w * 32 + bit;
+      m &= m - 1;
+    }
+  }
+  // rows of this block row: scatter entries
+  for (int32_t r = 0; r < b; ++r) {
+    int64_t row = I * b + r;
+    for (int32_t e = row_ptr[row] + threadIdx.x; e < row_ptr[row + 1]; e += blockDim.x) {
+      int32_t j = col[e];
+      int32_t J = j / b;
+      uint32_t w = bits[J >> 5] & ((1u << (J & 31)) - 1u);
+      int32_t p = p0 + (int32_t)(pref[J >> 5] + __popc(w));
+      tiles[((size_t)p * b + r) * b + (j - J * b)] = val[e];
+    }
+  }
+}
+
+__global__ void exclusive_scan_small(int64_t n, const int32_t* counts, int32_t* out) {
+  // single thread: n is the number of block rows (<= a few thousand .. 1e5); builder-only cost
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    int32_t run = 0;
+    for (int64_t i = 0; i < n; ++i) { out[i] = run; run += counts[i]; }
+    out[n] = run;
+  }
+}
+
+// gather / copy helpers
+__global__ void copy2d_kernel(const double* __restrict__ src, int64_t lds, double* __restrict__ dst, int64_t ldd,
+                              int64_t rows, int64_t cols) {
+  int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  int64_t r = blockIdx.y;
+  for (; r < rows; r += gridDim.y)
+    if (c < cols) dst[r * ldd + c] = src[r * lds + c];
+}
+
+// ------------------------------------------------------------------------------------------------
+// fp64 peak probes
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) probe_dfma_kernel(double* out, int iters, double x, double y) {
+  double a[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) a[i] = threadIdx.x * 1e-9 + i;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) a[i] = fma(a[i], x, y);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += a[i];
+  if (s == 12345.678) out[0] = s;
+}
+__global__ void __launch_bounds__(256) probe_dmma_kernel(double* out, int iters, double x, double y) {
+  double c0[8], c1[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { c0[i] = threadIdx.x * 1e-9 + i; c1[i] = i; }
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) ttdft::dmma_8x8x4(c0[i], c1[i], x, y);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += c0[i] + c1[i];
+  if (s == 12345.678) out[0] = s;
+}
+
+// ------------------------------------------------------------------------------------------------
+// step dispatch:  O = alpha*H*X + gamma*X + beta*Z   (gamma = -alpha*c for a recurrence step)
+// ------------------------------------------------------------------------------------------------
+template <int WR>
+ttdft_status launch_k1(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
+                       const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, cudaStream_t st) {
+  using SM = ttdft::K1Smem<WR>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    CUDA_TRY(cudaFuncSetAttribute(ttdft::bsr_dmma_kernel<WR>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::TOTAL));
+    attr_set = true;
+  }
+  CUtensorMap tmX;
+  ttdft_status s = make_map_2d(&tmX, X, (uint64_t)ncols, (uint64_t)h->M, (uint64_t)ldx, ttdft::K1_KS);
+  if (s != TTDFT_OK) return s;
+  ttdft::K1Params p;
+  p.brow_ptr = h->row_ptr;
+  p.bcol = h->col;
+  p.nb = (int32_t)h->nb;
+  p.nct = (int32_t)((ncols + ttdft::K1_TN - 1) / ttdft::K1_TN);
+  p.cg = h->cg;
+  p.ncols = ncols;
+  p.alpha = alpha; p.gamma = gamma; p.beta = beta;
+  p.S = X; p.lds = ldx;
+  p.Z = Z; p.ldz = ldz;
+  p.O = O; p.ldo = ldo;
+  auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
+  p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
+  const int64_t tiles = (int64_t)p.nb * p.nct;
+  if (tiles > 0x7fffffffLL) return fail(TTDFT_ERR_UNSUPPORTED, "too many tiles (%lld)", (long long)tiles);
+  ttdft::bsr_dmma_kernel<WR><<<(unsigned)tiles, 32 * (2 * WR + 1), SM::TOTAL, st>>>(h->tmH, tmX, p);
+  CUDA_TRY(cudaGetLastError());
+  g_launches.fetch_add(1);
+  return TTDFT_OK;
+}
+
+ttdft_status launch_step(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
+                         const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, cudaStream_t st) {
+  if (h->M == 0) return TTDFT_OK;
+  const bool tma_ok = (reinterpret_cast<uintptr_t>(X) & 15) == 0 && (ldx % 2 == 0) && alpha != 0.0;
+  if (h->kernel == 1 && tma_ok) {
+    switch (h->b) {
+      case 32: return launch_k1<1>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+      case 64: return launch_k1<2>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+      case 96: return launch_k1<3>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+      case 128: return launch_k1<4>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+      default: break;
+    }
+  }
+  ttdft::K2Params p;
+  p.row_ptr = h->row_ptr; p.col = h->col; p.val = h->val;
+  p.M = h->M; p.b = h->b; p.ncols = ncols;
+  p.alpha = alpha; p.gamma = gamma; p.beta = beta;
+  p.X = X; p.ldx = ldx; p.Z = Z; p.ldz = ldz; p.O = O; p.ldo = ldo;
+  dim3 grid((unsigned)((h->M + ttdft::K2_ROWS - 1) / ttdft::K2_ROWS), (unsigned)((ncols + ttdft::K2_TN - 1) / ttdft::K2_TN));
+  if (grid.y > 65535) return fail(TTDFT_ERR_UNSUPPORTED, "ncols too large for the generic kernel");
+  if (h->bsr)
+    ttdft::generic_step_kernel<true><<<grid, 32 * ttdft::K2_ROWS, 0, st>>>(p);
+  else
+    ttdft::generic_step_kernel<false><<<grid, 32 * ttdft::K2_ROWS, 0, st>>>(p);
+  CUDA_TRY(cudaGetLastError());
+  g_launches.fetch_add(1);
+  return TTDFT_OK;
+}
+
+ttdft_status launch_copy2d(const double* src, int64_t lds, double* dst, int64_t ldd, int64_t rows, int64_t cols,
+                           cudaStream_t st) {
+  if (rows == 0 || cols == 0) return TTDFT_OK;
+  CUDA_TRY(cudaMemcpy2DAsync(dst, (size_t)ldd * 8, src, (size_t)lds * 8, (size_t)cols * 8, (size_t)rows,
+                             cudaMemcpyDeviceToDevice, st));
+  return TTDFT_OK;
+}
+
+// do [p, p + (rows-1)*ld + cols) and [q, ...) overlap?
+bool overlaps(const double* p, int64_t ldp, const double* q, int64_t ldq, int64_t rows, int64_t cols) {
+  if (rows == 0 || cols == 0) return false;
+  const double* pe = p + (rows - 1) * ldp + cols;
+  const double* qe = q + (rows - 1) * ldq + cols;
+  return p < qe && q < pe;
+}
+
+ttdft_status check_scalars(int32_t m, double a, double b, double a0) {
+  if (m < 0) return fail(TTDFT_ERR_INVALID_ARG, "degree m = %d must be >= 0", m);
+  if (!(a0 < a) || !(a < b) || !(a0 == a0) || !(b - b == 0.0) || !(a0 - a0 == 0.0))
+    return fail(TTDFT_ERR_INVALID_ARG, "bounds must be finite with a0 < a < b (got a0=%g a=%g b=%g)", a0, a, b);
+  return TTDFT_OK;
+}
+
+int64_t default_panel(int64_t ncols) { return ncols < 4096 ? ncols : 4096; }
+
+// Run the m recurrence steps of one column panel (A2-A4, A6).  Xp: input panel (ldx), Yp: output
+// panel (ldy), W: scratch (ldw).  inplace: Xp == Yp.
+ttdft_status filter_panel(const ttdft_h_s* h, const double* Xp, int64_t ldx, double* Yp, int64_t ldy, double* W,
+                          int64_t ldw, int64_t wc, int32_t m, double c, const double* alpha, const double* beta,
+                          bool inplace, cudaStream_t st) {
+  if (m == 0) {
+    if (!inplace) return launch_copy2d(Xp, ldx, Yp, ldy, h->M, wc, st);
+    return TTDFT_OK;
+  }
+  // destination of step k (1-based).  Out of place: Y_m lands in Yp, the iterates alternate Yp / W and
+  // Y_{k+1} overwrites Y_{k-1} (read only at the output position).  In place: even steps land in Yp.
+  auto dest = [&](int k, int64_t* ld) -> double* {
+    bool toY = inplace ? (k % 2 == 0) : ((m - k) % 2 == 0);
+    *ld = toY ? ldy : ldw;
+    return toY ? Yp : W;
+  };
+  for (int k = 1; k <= m; ++k) {
+    int64_t ldo, lds, ldz = 0;
+    double* O = dest(k, &ldo);
+    const double* S;
+    if (k == 1) { S = Xp; lds = ldx; } else { S = dest(k - 1, &lds); }
+    const double* Z = nullptr;
+    if (k == 2) { Z = Xp; ldz = ldx; }
+    else if (k > 2) { Z = dest(k - 2, &ldz); }
+    const double al = alpha[k - 1], be = (k == 1) ? 0.0 : beta[k - 1];
+    ttdft_status s = launch_step(h, al, -al * c, be, S, lds, Z, ldz, O, ldo, wc, st);
+    if (s != TTDFT_OK) return s;
+  }
+  if (inplace && (m % 2 == 1)) return launch_copy2d(W, ldw, Yp, ldy, h->M, wc, st);
+  return TTDFT_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+// C ABI
+// ================================================================================================
+extern "C" {
+
+const char* ttdft_last_error(void) { return g_err.c_str(); }
+int64_t ttdft_launch_count(void) { return g_launches.load(); }
+
+static ttdft_status desc_counts(const ttdft_h_desc* d, int64_t* nrows_idx, int64_t* nstored) {
+  if (!d) return fail(TTDFT_ERR_INVALID_ARG, "desc is NULL");
+  if (d->M < 0) return fail(TTDFT_ERR_INVALID_ARG, "M < 0");
+  if (d->fmt != TTDFT_FMT_CSR && d->fmt != TTDFT_FMT_BSR) return fail(TTDFT_ERR_INVALID_ARG, "unknown format");
+  if (d->M > 0 && (!d->row_ptr)) return fail(TTDFT_ERR_INVALID_ARG, "row_ptr is NULL");
+  if (d->fmt == TTDFT_FMT_BSR) {
+    if (d->block < 1) return fail(TTDFT_ERR_INVALID_ARG, "BSR block size must be >= 1");
+    if (d->M % d->block) return fail(TTDFT_ERR_INVALID_ARG, "M is not a multiple of the block size");
+    *nrows_idx = d->M / d->block;
+  } else {
+    *nrows_idx = d->M;
+  }
+  if (d->M >= 0x7fffffffLL) return fail(TTDFT_ERR_UNSUPPORTED, "M must fit int32");
+  int32_t last = 0;
+  if (d->M > 0) CUDA_TRY(cudaMemcpy(&last, d->row_ptr + *nrows_idx, 4, cudaMemcpyDeviceToHost));
+  if (last < 0) return fail(TTDFT_ERR_INVALID_ARG, "row_ptr[last] < 0");
+  *nstored = last;
+  if (last > 0 && (!d->col_idx || !d->values)) return fail(TTDFT_ERR_INVALID_ARG, "col_idx/values is NULL");
+  return TTDFT_OK;
+}
+
+// decide the device format; for CSR + usable hint returns the tile size in *hint_b (else 0)
+static ttdft_status plan_format(const ttdft_h_desc* d, int32_t* hint_b) {
+  *hint_b = 0;
+  if (d->fmt != TTDFT_FMT_CSR || !d->subdomain_of_row || (d->flags & TTDFT_FORCE_GENERIC) || d->M == 0) return TTDFT_OK;
+  // group size = index of the first label change (read the labels' prefix from the device)
+  std::vector<int32_t> lab((size_t)std::min<int64_t>(d->M, 129));
+  CUDA_TRY(cudaMemcpy(lab.data(), d->subdomain_of_row, lab.size() * 4, cudaMemcpyDeviceToHost));
+  size_t b = 1;
+  while (b < lab.size() && lab[b] == lab[0]) ++b;
+  if (!k1_block_ok((int32_t)b) || d->M % (int64_t)b) return TTDFT_OK;
+  if (d->M / (int64_t)b > (1 << 17)) return TTDFT_OK;   // bitmap of block columns must fit shared memory
+  int32_t* bad = nullptr;
+  CUDA_TRY(cudaMalloc(&bad, 4));                         // 4-byte transient flag
+  cudaMemset(bad, 0, 4);
+  hint_check_kernel<<<(unsigned)((d->M + 255) / 256), 256>>>(d->M, d->subdomain_of_row, (int32_t)b, bad);
+  g_launches.fetch_add(1);
+  int32_t hb = 1;
+  cudaError_t e = cudaMemcpy(&hb, bad, 4, cudaMemcpyDeviceToHost);
+  cudaFree(bad);
+  if (e != cudaSuccess) return fail(TTDFT_ERR_CUDA, "hint check: %s", cudaGetErrorString(e));
+  if (hb == 0) *hint_b = (int32_t)b;
+  return TTDFT_OK;
+}
+
+static ttdft_status csr2bsr_counts(const ttdft_h_desc* d, int32_t b, int32_t* dev_counts, cudaStream_t st) {
+  const int64_t nb = d->M / b;
+  const int32_t nwords = (int32_t)((nb + 31) / 32);
+  csr2bsr_count_kernel<<<(unsigned)nb, 256, (size_t)nwords * 4, st>>>(nb, b, d->row_ptr, d->col_idx, dev_counts, nwords);
+  CUDA_TRY(cudaGetLastError());
+  g_launches.fetch_add(1);
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_h_storage_bytes(const ttdft_h_desc* d, size_t* bytes) {
+  if (!bytes) return fail(TTDFT_ERR_INVALID_ARG, "bytes is NULL");
+  int64_t nidx, nstored;
+  ttdft_status s = desc_counts(d, &nidx, &nstored);
+  if (s != TTDFT_OK) return s;
+  int32_t hint_b;
+  s = plan_format(d, &hint_b);
+  if (s != TTDFT_OK) return s;
+  if (hint_b) {
+    // count the tiles the conversion will create (transient nb-int scratch)
+    const int64_t nb = d->M / hint_b;
+    int32_t* cnt = nullptr;
+    CUDA_TRY(cudaMalloc(&cnt, (size_t)nb * 4));
+    s = csr2bsr_counts(d, hint_b, cnt, 0);
+    std::vector<int32_t> hc((size_t)nb);
+    cudaError_t e = cudaMemcpy(hc.data(), cnt, (size_t)nb * 4, cudaMemcpyDeviceToHost);
+    cudaFree(cnt);
+    if (s != TTDFT_OK) return s;
+    if (e != cudaSuccess) return fail(TTDFT_ERR_CUDA, "tile count: %s", cudaGetErrorString(e));
+    int64_t nblocks = 0;
+    for (int32_t c : hc) nblocks += c;
+    *bytes = align_up((size_t)(nb + 1) * 4, 1024) + align_up((size_t)nb * 4, 1024) + align_up((size_t)nblocks * 4, 1024) +
+             align_up((size_t)nblocks * hint_b * hint_b * 8, 1024);
+    return TTDFT_OK;
+  }
+  const size_t per = (d->fmt == TTDFT_FMT_BSR) ? (size_t)d->block * d->block : 1;
+  // row_ptr | col | values | (BSR check scratch: tile_row)
+  const size_t nidxarr = (d->fmt == TTDFT_FMT_BSR) ? 2 : 1;
+  *bytes = align_up((size_t)(nidx + 1) * 4, 1024) + nidxarr * align_up((size_t)nstored * 4, 1024) +
+           align_up((size_t)nstored * per * 8, 1024) + 1024;
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t bytes, void* stream, ttdft_h_t* out) {
+  if (!out) return fail(TTDFT_ERR_INVALID_ARG, "out is NULL");
+  cudaStream_t st = (cudaStream_t)stream;
+  int64_t nidx, nstored;
+  ttdft_status s = desc_counts(d, &nidx, &nstored);
+  if (s != TTDFT_OK) return s;
+  size_t need;
+  s = ttdft_h_storage_bytes(d, &need);
+  if (s != TTDFT_OK) return s;
+  if (bytes < need) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "dev_storage has %zu bytes, %zu needed", bytes, need);
+  if (need > 0 && (!dev_storage || (reinterpret_cast<uintptr_t>(dev_storage) & 1023)))
+    return fail(TTDFT_ERR_INVALID_ARG, "dev_storage must be a 1024-byte aligned device pointer");
+  int32_t hint_b;
+  s = plan_format(d, &hint_b);
+  if (s != TTDFT_OK) return s;
+
+  // ---- validation on request (on the input arrays) ----
+  if (d->M > 0 && (d->flags & (TTDFT_CHECK_SORTED | TTDFT_CHECK_SYMMETRY))) {
+    int32_t* flags = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(dev_storage) + need - 1024);
+    int32_t* tile_row = nullptr;
+    if (hint_b == 0 && d->fmt == TTDFT_FMT_BSR)   // scratch region reserved in storage_bytes
+      tile_row = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(dev_storage) + align_up((size_t)(nidx + 1) * 4, 1024) +
+                                            align_up((size_t)nstored * 4, 1024));
+    CUDA_TRY(cudaMemsetAsync(flags, 0, 4, st));
+    const int64_t ncolmax = (d->fmt == TTDFT_FMT_BSR) ? d->M / d->block : d->M;
+    check_sorted_kernel<<<(unsigned)((nidx + 255) / 256), 256, 0, st>>>(nidx, d->row_ptr, d->col_idx, ncolmax, flags);
+    g_launches.fetch_add(1);
+    int32_t hf = 0;
+    CUDA_TRY(cudaMemcpyAsync(&hf, flags, 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (hf & 1) return fail(TTDFT_ERR_INVALID_ARG, "indices are out of range, unsorted or duplicated");
+    if (d->flags & TTDFT_CHECK_SYMMETRY) {
+      if (d->fmt == TTDFT_FMT_CSR) {
+        check_sym_csr_kernel<<<(unsigned)((d->M + 127) / 128), 128, 0, st>>>(d->M, d->row_ptr, d->col_idx, d->values, flags);
+        g_launches.fetch_add(1);
+      } else if (nstored > 0) {
+        tile_rows_kernel<<<(unsigned)((nidx + 255) / 256), 256, 0, st>>>(nidx, d->row_ptr, tile_row);
+        check_sym_bsr_kernel<<<(unsigned)nstored, 256, 0, st>>>(d->block, d->row_ptr, d->col_idx, d->values, tile_row, flags);
+        g_launches.fetch_add(2);
+      }
+      CUDA_TRY(cudaMemcpyAsync(&hf, flags, 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(cudaStreamSynchronize(st));
+      if (hf & 2) return fail(TTDFT_ERR_NOT_SYMMETRIC, "H is not symmetric");
+    }
+  }
+
+  ttdft_h_s* h = new (std::nothrow) ttdft_h_s;
+  if (!h) return fail(TTDFT_ERR_CUDA, "out of host memory");
+  h->M = d->M;
+  h->storage_bytes = need;
+  uint8_t* base = reinterpret_cast<uint8_t*>(dev_storage);
+
+  if (hint_b) {
+    // ---- CSR with subdomain labels -> block-sparse tiles (rows of a subdomain contiguous) ----
+    const int32_t b = hint_b;
+    const int64_t nb = d->M / b;
+    const int32_t nwords = (int32_t)((nb + 31) / 32);
+    int32_t* brow = reinterpret_cast<int32_t*>(base);
+    int32_t* counts = reinterpret_cast<int32_t*>(base + align_up((size_t)(nb + 1) * 4, 1024));
+    s = csr2bsr_counts(d, b, counts, st);
+    if (s != TTDFT_OK) { delete h; return s; }
+    exclusive_scan_small<<<1, 1, 0, st>>>(nb, counts, brow);
+    g_launches.fetch_add(1);
+    int32_t nblocks = 0;
+    cudaError_t e = cudaMemcpyAsync(&nblocks, brow + nb, 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "csr->bsr scan: %s", cudaGetErrorString(e)); }
+    int32_t* bcol = reinterpret_cast<int32_t*>(base + align_up((size_t)(nb + 1) * 4, 1024) + align_up((size_t)nb * 4, 1024));
+    double* tiles = reinterpret_cast<double*>(reinterpret_cast<uint8_t*>(bcol) + align_up((size_t)nblocks * 4, 1024));
+    e = cudaMemsetAsync(tiles, 0, (size_t)nblocks * b * b * 8, st);
+    if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "memset: %s", cudaGetErrorString(e)); }
+    csr2bsr_fill_kernel<<<(unsigned)nb, 256, (size_t)nwords * 8, st>>>(nb, b, d->row_ptr, d->col_idx, d->values, brow, bcol,
+                                                                       tiles, nwords);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "csr->bsr fill: %s", cudaGetErrorString(e)); }
+    g_launches.fetch_add(1);
+    h->bsr = 1; h->b = b; h->nb = nb; h->nblocks = nblocks;
+    h->row_ptr = brow; h->col = bcol; h->val = tiles;
+    h->kernel = 1;
+  } else {
+    // ---- keep the input format: copy the three arrays into dev_storage ----
+    const size_t per = (d->fmt == TTDFT_FMT_BSR) ? (size_t)d->block * d->block : 1;
+    int32_t* rp = reinterpret_cast<int32_t*>(base);
+    int32_t* col = reinterpret_cast<int32_t*>(base + align_up((size_t)(nidx + 1) * 4, 1024));
+    const size_t nidxarr = (d->fmt == TTDFT_FMT_BSR) ? 2 : 1;
+    double* val = reinterpret_cast<double*>(base + align_up((size_t)(nidx + 1) * 4, 1024) + nidxarr * align_up((size_t)nstored * 4, 1024));
+    cudaError_t e = cudaSuccess;
+    if (d->M > 0) e = cudaMemcpyAsync(rp, d->row_ptr, (size_t)(nidx + 1) * 4, cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess && nstored > 0) e = cudaMemcpyAsync(col, d->col_idx, (size_t)nstored * 4, cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess && nstored > 0) e = cudaMemcpyAsync(val, d->values, (size_t)nstored * per * 8, cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "copy of H: %s", cudaGetErrorString(e)); }
+    h->bsr = (d->fmt == TTDFT_FMT_BSR);
+    h->b = h->bsr ? d->block : 0;
+    h->nb = nidx;
+    h->nblocks = nstored;
+    h->row_ptr = rp; h->col = col; h->val = val;
+    h->kernel = (h->bsr && k1_block_ok(d->block) && !(d->flags & TTDFT_FORCE_GENERIC) && nstored > 0) ? 1 : 0;
+  }
+  if (h->kernel == 1) {
+    s = make_map_2d(&h->tmH, h->val, (uint64_t)h->b, (uint64_t)h->nblocks * h->b, (uint64_t)h->b, (uint32_t)h->b);
+    if (s != TTDFT_OK) { delete h; return s; }
+  }
+  *out = h;
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_h_info(ttdft_h_t h, ttdft_h_info_t* info) {
+  if (!h || !info) return fail(TTDFT_ERR_INVALID_ARG, "NULL argument");
+  info->M = h->M;
+  info->block = h->bsr ? h->b : 0;
+  info->kernel = h->kernel;
+  info->nblocks = h->bsr ? h->nblocks : 0;
+  info->nnz_stored = h->bsr ? h->nblocks * (int64_t)h->b * h->b : h->nblocks;
+  info->storage_bytes = h->storage_bytes;
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_h_destroy(ttdft_h_t h) {
+  delete h;
+  return TTDFT_OK;
+}
+
+static ttdft_status check_mat(const char* name, const double* p, int64_t ld, int64_t ncols) {
+  if (!p) return fail(TTDFT_ERR_INVALID_ARG, "%s is NULL", name);
+  if (ld < ncols) return fail(TTDFT_ERR_INVALID_ARG, "leading dimension of %s (%lld) < ncols (%lld)", name, (long long)ld,
+                              (long long)ncols);
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_spmm(ttdft_h_t h, double alpha, const double* X, int64_t ldx, double beta, double* Y, int64_t ldy,
+                        int64_t ncols, void* stream) {
+  if (!h) return fail(TTDFT_ERR_INVALID_ARG, "handle is NULL");
+  if (ncols < 1) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1");
+  ttdft_status s;
+  if ((s = check_mat("X", X, ldx, ncols)) != TTDFT_OK) return s;
+  if ((s = check_mat("Y", Y, ldy, ncols)) != TTDFT_OK) return s;
+  if (overlaps(X, ldx, Y, ldy, h->M, ncols)) return fail(TTDFT_ERR_INVALID_ARG, "X overlaps Y");
+  return launch_step(h, alpha, 0.0, beta, X, ldx, Y, ldy, Y, ldy, ncols, (cudaStream_t)stream);
+}
+
+ttdft_status ttdft_cheb_step(ttdft_h_t h, double alpha, double c, double beta, const double* Yk, int64_t ldk,
+                             const double* Ykm1, int64_t ldm, double* Yout, int64_t ldo, int64_t ncols, void* stream) {
+  if (!h) return fail(TTDFT_ERR_INVALID_ARG, "handle is NULL");
+  if (ncols < 1) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1");
+  ttdft_status s;
+  if ((s = check_mat("Yk", Yk, ldk, ncols)) != TTDFT_OK) return s;
+  if ((s = check_mat("Yout", Yout, ldo, ncols)) != TTDFT_OK) return s;
+  if (Ykm1 && (s = check_mat("Ykm1", Ykm1, ldm, ncols)) != TTDFT_OK) return s;
+  if (overlaps(Yk, ldk, Yout, ldo, h->M, ncols)) return fail(TTDFT_ERR_INVALID_ARG, "Yk overlaps Yout");
+  if (Ykm1 && !(Ykm1 == Yout && ldm == ldo) && overlaps(Ykm1, ldm, Yout, ldo, h->M, ncols))
+    return fail(TTDFT_ERR_INVALID_ARG, "Ykm1 partially overlaps Yout");
+  const double be = Ykm1 ? beta : 0.0;
+  return launch_step(h, alpha, -alpha * c, be, Yk, ldk, Ykm1, ldm, Yout, ldo, ncols, (cudaStream_t)stream);
+}
+
+ttdft_status ttdft_cheb_scalars(int32_t m, double a, double b, double a0, double* c_out, double* alpha, double* beta) {
+  ttdft_status s = check_scalars(m, a, b, a0);
+  if (s != TTDFT_OK) return s;
+  const double e = 0.5 * (b - a), c = 0.5 * (b + a);
+  if (c_out) *c_out = c;
+  if (m == 0) return TTDFT_OK;
+  if (!alpha || !beta) return fail(TTDFT_ERR_INVALID_ARG, "alpha/beta is NULL");
+  double sigma = e / (a0 - c);
+  const double sigma1 = sigma, gamma = 2.0 / sigma1;
+  alpha[0] = sigma1 / e;
+  beta[0] = 0.0;
+  for (int k = 1; k < m; ++k) {
+    const double sigma2 = 1.0 / (gamma - sigma);
+    alpha[k] = 2.0 * sigma2 / e;
+    beta[k] = -(sigma * sigma2);
+    sigma = sigma2;
+  }
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_cheb_filter_work_bytes(ttdft_h_t h, int64_t ncols, int64_t panel_cols, size_t* bytes) {
+  if (!h || !bytes) return fail(TTDFT_ERR_INVALID_ARG, "NULL argument");
+  if (ncols < 1 || panel_cols < 0) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1 and panel_cols >= 0");
+  int64_t w = panel_cols ? std::min(panel_cols, ncols) : default_panel(ncols);
+  w += (w & 1);   // even leading dimension keeps the scratch panel TMA / 128-bit friendly
+  *bytes = (size_t)h->M * (size_t)w * 8;
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_cheb_filter(ttdft_h_t h, const double* X, int64_t ldx, double* Y, int64_t ldy, int64_t ncols, int32_t m,
+                               double a, double b, double a0, int64_t panel_cols, void* work, size_t work_bytes,
+                               void* stream) {
+  if (!h) return fail(TTDFT_ERR_INVALID_ARG, "handle is NULL");
+  if (ncols < 1 || panel_cols < 0) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1 and panel_cols >= 0");
+  ttdft_status s;
+  if ((s = check_scalars(m, a, b, a0)) != TTDFT_OK) return s;
+  if ((s = check_mat("X", X, ldx, ncols)) != TTDFT_OK) return s;
+  if ((s = check_mat("Y", Y, ldy, ncols)) != TTDFT_OK) return s;
+  const bool inplace = (X == Y);
+  if (inplace && ldx != ldy) return fail(TTDFT_ERR_INVALID_ARG, "in-place call needs ldx == ldy");
+  if (!inplace && overlaps(X, ldx, Y, ldy, h->M, ncols)) return fail(TTDFT_ERR_INVALID_ARG, "X partially overlaps Y");
+  size_t need;
+  if ((s = ttdft_cheb_filter_work_bytes(h, ncols, panel_cols, &need)) != TTDFT_OK) return s;
+  const bool need_work = (m >= 2) || (m == 1 && inplace);
+  if (need_work) {
+    if (work_bytes < need) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, need);
+    if (!work || (reinterpret_cast<uintptr_t>(work) & 15)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 16-byte aligned device pointer");
+  }
+  std::vector<double> alpha((size_t)std::max(m, 1)), beta((size_t)std::max(m, 1));
+  double c;
+  if ((s = ttdft_cheb_scalars(m, a, b, a0, &c, alpha.data(), beta.data())) != TTDFT_OK) return s;
+  const int64_t w = panel_cols ? std::min(panel_cols, ncols) : default_panel(ncols);
+  const int64_t ldw = w + (w & 1);
+  for (int64_t c0 = 0; c0 < ncols; c0 += w) {
+    const int64_t wc = std::min(w, ncols - c0);
+    s = filter_panel(h, X + c0, ldx, Y + c0, ldy, reinterpret_cast<double*>(work), ldw, wc, m, c, alpha.data(), beta.data(),
+                     inplace, (cudaStream_t)stream);
+    if (s != TTDFT_OK) return s;
+  }
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_cheb_filter_host_work_bytes(ttdft_h_t h, int64_t ncols, int64_t panel_cols, size_t* bytes) {
+  if (!h || !bytes) return fail(TTDFT_ERR_INVALID_ARG, "NULL argument");
+  if (ncols < 1 || panel_cols < 0) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1 and panel_cols >= 0");
+  int64_t w = panel_cols ? std::min(panel_cols, ncols) : std::min<int64_t>(ncols, 1024);
+  w += (w & 1);
+  *bytes = 5 * align_up((size_t)h->M * (size_t)w * 8, 1024);   // 2 x (X panel, Y panel) + scratch
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* Xh, int64_t ldx, double* Yh, int64_t ldy, int64_t ncols,
+                                    int32_t m, double a, double b, double a0, int64_t panel_cols, void* work,
+                                    size_t work_bytes, void* stream) {
+  if (!h) return fail(TTDFT_ERR_INVALID_ARG, "handle is NULL");
+  if (ncols < 1 || panel_cols < 0) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1 and panel_cols >= 0");
+  ttdft_status s;
+  if ((s = check_scalars(m, a, b, a0)) != TTDFT_OK) return s;
+  if ((s = check_mat("X_host", Xh, ldx, ncols)) != TTDFT_OK) return s;
+  if ((s = check_mat("Y_host", Yh, ldy, ncols)) != TTDFT_OK) return s;
+  size_t need;
+  if ((s = ttdft_cheb_filter_host_work_bytes(h, ncols, panel_cols, &need)) != TTDFT_OK) return s;
+  if (work_bytes < need) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, need);
+  if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
+  std::vector<double> alpha((size_t)std::max(m, 1)), beta((size_t)std::max(m, 1));
+  double c;
+  if ((s = ttdft_cheb_scalars(m, a, b, a0, &c, alpha.data(), beta.data())) != TTDFT_OK) return s;
+  const int64_t w = panel_cols ? std::min(panel_cols, ncols) : std::min<int64_t>(ncols, 1024);
+  const int64_t ldw = w + (w & 1);
+  const size_t pbytes = align_up((size_t)h->M * (size_t)ldw * 8, 1024);
+  uint8_t* base = reinterpret_cast<uint8_t*>(work);
+  double* dX[2] = {reinterpret_cast<double*>(base), reinterpret_cast<double*>(base + pbytes)};
+  double* dY[2] = {reinterpret_cast<double*>(base + 2 * pbytes), reinterpret_cast<double*>(base + 3 * pbytes)};
+  double* dW = reinterpret_cast<double*>(base + 4 * pbytes);
+
+  cudaStream_t sc = (cudaStream_t)stream, sin = nullptr, sout = nullptr;
+  cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr}, ev_start = nullptr;
+  ttdft_status rc = TTDFT_OK;
+  auto cleanup = [&]() {
+    for (int i = 0; i < 2; ++i) {
+      if (ev_in[i]) cudaEventDestroy(ev_in[i]);
+      if (ev_comp[i]) cudaEventDestroy(ev_comp[i]);
+      if (ev_out[i]) cudaEventDestroy(ev_out[i]);
+    }
+    if (ev_start) cudaEventDestroy(ev_start);
+    if (sin) cudaStreamDestroy(sin);
+    if (sout) cudaStreamDestroy(sout);
+  };
+#define HOST_TRY(expr)                                                                     \
+  do {                                                                                     \
+    cudaError_t e__ = (expr);                                                              \
+    if (e__ != cudaSuccess) {                                                              \
+      rc = fail(TTDFT_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e__));                 \
+      cudaDeviceSynchronize();                                                             \
+      cleanup();                                                                           \
+      return rc;                                                                           \
+    }                                                                                      \
+  } while (0)
+  HOST_TRY(cudaStreamCreateWithFlags(&sin, cudaStreamNonBlocking));
+  HOST_TRY(cudaStreamCreateWithFlags(&sout, cudaStreamNonBlocking));
+  for (int i = 0; i < 2; ++i) {
+    HOST_TRY(cudaEventCreateWithFlags(&ev_in[i], cudaEventDisableTiming));
+    HOST_TRY(cudaEventCreateWithFlags(&ev_comp[i], cudaEventDisableTiming));
+    HOST_TRY(cudaEventCreateWithFlags(&ev_out[i], cudaEventDisableTiming));
+  }
+  HOST_TRY(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+  // copies must not start before work already queued on the caller's stream has finished
+  HOST_TRY(cudaEventRecord(ev_start, sc));
+  HOST_TRY(cudaStreamWaitEvent(sin, ev_start, 0));
+  HOST_TRY(cudaStreamWaitEvent(sout, ev_start, 0));
+  int64_t ip = 0;
+  for (int64_t c0 = 0; c0 < ncols; c0 += w, ++ip) {
+    const int buf = (int)(ip & 1);
+    const int64_t wc = std::min(w, ncols - c0);
+    // host -> device on the input stream once the compute that last read dX[buf] is done
+    if (ip >= 2) HOST_TRY(cudaStreamWaitEvent(sin, ev_comp[buf], 0));
+    HOST_TRY(cudaMemcpy2DAsync(dX[buf], (size_t)ldw * 8, Xh + c0, (size_t)ldx * 8, (size_t)wc * 8, (size_t)h->M,
+                               cudaMemcpyHostToDevice, sin));
+    HOST_TRY(cudaEventRecord(ev_in[buf], sin));
+    // compute once the panel has arrived and dY[buf]'s previous contents have left
+    HOST_TRY(cudaStreamWaitEvent(sc, ev_in[buf], 0));
+    if (ip >= 2) HOST_TRY(cudaStreamWaitEvent(sc, ev_out[buf], 0));
+    s = filter_panel(h, dX[buf], ldw, dY[buf], ldw, dW, ldw, wc, m, c, alpha.data(), beta.data(), false, sc);
+    if (s != TTDFT_OK) { cudaDeviceSynchronize(); cleanup(); return s; }
+    HOST_TRY(cudaEventRecord(ev_comp[buf], sc));
+    // device -> host on the output stream
+    HOST_TRY(cudaStreamWaitEvent(sout, ev_comp[buf], 0));
+    HOST_TRY(cudaMemcpy2DAsync(Yh + c0, (size_t)ldy * 8, dY[buf], (size_t)ldw * 8, (size_t)wc * 8, (size_t)h->M,
+                               cudaMemcpyDeviceToHost, sout));
+    HOST_TRY(cudaEventRecord(ev_out[buf], sout));
+  }
+  HOST_TRY(cudaStreamSynchronize(sin));
+  HOST_TRY(cudaStreamSynchronize(sc));
+  HOST_TRY(cudaStreamSynchronize(sout));
+#undef HOST_TRY
+  cleanup();
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, double* tflops) {
+  if (!tflops || (kind != 0 && kind != 1) || millis < 1) return fail(TTDFT_ERR_INVALID_ARG, "bad probe arguments");
+  cudaStream_t st = (cudaStream_t)stream;
+  int dev = 0, nsm = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+  double* out = nullptr;
+  CUDA_TRY(cudaMalloc(&out, 64));   // 64-byte transient sink for the probe kernels
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  const int iters = 20000;
+  const dim3 grid(nsm * 4), blk(256);
+  const double per_launch = kind == 0 ? (double)nsm * 4 * 256 * iters * 16.0 * 2.0 : (double)nsm * 4 * 8 * iters * 8.0 * 512.0;
+  auto launch = [&]() {
+    if (kind == 0) probe_dfma_kernel<<<grid, blk, 0, st>>>(out, iters, 1.0000001, 1e-9);
+    else probe_dmma_kernel<<<grid, blk, 0, st>>>(out, iters, 1.0000001, 1e-9);
+    g_launches.fetch_add(1);
+  };
+  launch();
+  cudaStreamSynchronize(st);
+  float ms = 0;
+  cudaEventRecord(e0, st);
+  launch();
+  cudaEventRecord(e1, st);
+  cudaEventSynchronize(e1);
+  cudaEventElapsedTime(&ms, e0, e1);
+  int n = (int)(millis / (ms > 0 ? ms : 1.0f));
+  if (n < 1) n = 1;
+  cudaEventRecord(e0, st);
+  for (int i = 0; i < n; ++i) launch();
+  cudaEventRecord(e1, st);
+  cudaError_t e = cudaEventSynchronize(e1);
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(out);
+  if (e != cudaSuccess) return fail(TTDFT_ERR_CUDA, "probe: %s", cudaGetErrorString(e));
+  *tflops = per_launch * n / (ms * 1e-3) / 1e12;
+  return TTDFT_OK;
+}
+
+}  // extern "C"
