@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the B200-native ChFSI Chebyshev filter (Algorithm 1 step 1).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload si|al|tiny] [--impl reference]
+
+One "step" = one whole pass of the hot path: one `ttdft_cheb_filter` call (all m fused recurrence
+steps, all column panels) over one batch X of synthetic wavefunctions.  The default workload is
+BASELINE.json's headline config 3 ("si": M=221,184, N=4,096, m=20).  Metric: useful fp64 GFLOP/s of
+the filter = 2*nnz*N*m / t (nnz = non-zero entries of H; explicit zeros inside tiles earn nothing).
+
+N > 1 (torchrun): column-band sharding (PAPER.md:L258 band parallelism with H replicated per
+group): every rank filters its own N-column band with a full replica of H, no data-path
+collective; "scaling": "weak".
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores on a bounded
+column sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import synth  # noqa: E402
+
+# fp64 ALU/DMMA peak derived from unit counts and clocks: 148 SMs x 64 fp64
+# FMA/clk/SM x 2 flop x 1.965 GHz (clocks.max.sm).  Measured on this pool: DMMA loop 37.15 TFLOP/s.
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# DRAM bytes per launch of the dominant kernel from the ncu --set full capture under profiles/
+# (dram__bytes_read.sum + dram__bytes_write.sum), keyed by workload; None = not captured.
+NCU_TRAFFIC_BYTES = {}
+
+
+def load_bounds(name: str):
+    with open(os.path.join(ROOT, "tests", "golden", "bounds.json")) as f:
+        d = json.load(f)[name]
+    return d["a"], d["b"], d["a0"]
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period: float = 0.1):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.sm, self.power, self.reasons = [], [], set()
+        self.sm_max = None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4),
+            "hw_power_brake": getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop_evt.wait(self.period)
+
+    def stop(self) -> dict:
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join()
+        if not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": self.sm_max, "power_w_max": max(self.power),
+                "samples": len(self.sm), "reasons": sorted(self.reasons)}
+
+
+def gen_hamiltonian(cfg):
+    H = synth.hamiltonian_bsr(cfg.G, cfg.b, cfg.z, cfg.seed)
+    nnz = int(np.count_nonzero(H.values))
+    return H, nnz
+
+
+def oracle_sample_run(cfg, H, ncols_sample: int, m: int, bounds):
+    """Time the oracle filter on `ncols_sample` seeded columns of the workload (exact: columns are independent)."""
+    import oracle
+    C = synth.bsr_to_csr_nonzeros(H)
+    cols = synth.column_sample(cfg.N, cfg.panel, ncols_sample, cfg.seed)
+    Xs = np.empty((cfg.M, len(cols)))
+    for k, c in enumerate(cols):
+        synth.dense_normal(cfg.M, 1, cfg.seed, synth.STREAM_X, col0=int(c), out=Xs[:, k:k + 1])
+    a, b, a0 = bounds
+    t0 = time.perf_counter()
+    Y = oracle.cheb_filter(C.row_ptr, C.col_idx, C.values, Xs, m, a, b, a0)
+    dt = time.perf_counter() - t0
+    return dt, C.nnz, cols, Xs, Y, oracle.num_threads()
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, bounded sample, same metric and config."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = synth.CONFIGS[args.workload]
+    H, nnz = gen_hamiltonian(cfg)
+    bounds = load_bounds(args.workload)
+    ns = args.ref_cols
+    import oracle
+    oracle.lib()
+    times = []
+    for it in range(args.warmup + args.steps):
+        dt, nnz_c, cols, _, _, threads = oracle_sample_run(cfg, H, ns, cfg.m, bounds)
+        if it >= args.warmup:
+            times.append(dt)
+    t = float(np.mean(times))
+    gflops = 2.0 * nnz * len(cols) * cfg.m / t / 1e9
+    sample = f"{len(cols)} seeded columns of {cfg.N} (all {cfg.M} rows, all m={cfg.m} steps) per step"
+    line = {
+        "impl": "reference", "metric": "ChFSI filter useful fp64 GFLOP/s", "value": gflops, "unit": "GFLOP/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg, nnz, H.nblocks, args),
+        "cpu_baseline": {"value": gflops, "unit": "GFLOP/s", "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": gflops, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, nnz, nblocks, args):
+    return {
+        "workload": f"BASELINE.json config '{cfg.name}': G={cfg.G} b={cfg.b} M={cfg.M} N={cfg.N} m={cfg.m} "
+                    f"z={cfg.z} (27-neighbour block-sparse symmetric H, seeded synthetic)",
+        "M": cfg.M, "N": cfg.N, "m": cfg.m, "block": cfg.b, "nblocks": nblocks, "nnz": nnz,
+        "panel_cols": args.panel if args.panel else cfg.panel,
+        "l2": "inputs larger than L2 (H %.2f GB, X %.2f GB per rank)" % (nblocks * cfg.b * cfg.b * 8 / 1e9, cfg.M * cfg.N * 8 / 1e9),
+        "parallelism": f"band x{args.gpus} (H replicated, columns sharded, no collective)",
+    }
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="si", choices=list(synth.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--panel", type=int, default=0, help="column-panel width (0 = config default)")
+    ap.add_argument("--ref-cols", type=int, default=16, help="columns in the oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2110_15853_b200 as tt
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = synth.CONFIGS[args.workload]
+    a, b, a0 = load_bounds(args.workload)
+    H, nnz = gen_hamiltonian(cfg)
+    dev = torch.device("cuda", local)
+    t_build0 = time.perf_counter()
+    Hd = tt.h_build_bsr(H.M, H.b, torch.from_numpy(H.row_ptr).to(dev), torch.from_numpy(H.col_idx).to(dev),
+                        torch.from_numpy(H.values).to(dev))
+    torch.cuda.synchronize()
+    t_build = time.perf_counter() - t_build0
+    info = Hd.info()
+    assert info["kernel"] == 1, "the block-sparse TMA/DMMA kernel must be the one that runs"
+
+    # this rank's band of wavefunctions: columns [rank*N, (rank+1)*N) of the global block (host, pinned)
+    Xh = torch.empty((cfg.M, cfg.N), dtype=torch.float64).pin_memory()
+    synth.dense_normal(cfg.M, cfg.N, cfg.seed, synth.STREAM_X, col0=rank * cfg.N, out=Xh.numpy())
+    Yh = torch.empty((cfg.M, cfg.N), dtype=torch.float64).pin_memory()
+    Xd = Xh.to(dev, non_blocking=True)
+    Yd = torch.empty_like(Xd)
+    panel = args.panel if args.panel else cfg.panel
+    work = torch.empty(tt.cheb_filter_work_bytes(Hd, cfg.N, panel) + 16, dtype=torch.uint8, device=dev)
+    torch.cuda.synchronize()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        tt.cheb_filter(Hd, Xd, Yd, cfg.m, a, b, a0, panel_cols=panel, work=work)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    n0 = tt.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    launches = tt.launch_count() - n0
+    clocks = sampler.stop()
+    t_region = e0.elapsed_time(e1) * 1e-3
+    if dist is not None:
+        tmax = torch.tensor([t_region], dtype=torch.float64, device=dev)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        t_region = float(tmax.item())
+    t_step = t_region / args.steps
+
+    # ---- end to end through the C-ABI host-buffer call: H2D of X and D2H of Y inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        del work
+        hwork = torch.empty(tt.cheb_filter_host_work_bytes(Hd, cfg.N, 1024) + 1024, dtype=torch.uint8, device=dev)
+        tt.cheb_filter_host(Hd, Xh, Yh, cfg.m, a, b, a0, panel_cols=1024, work=hwork)   # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        nrep = max(1, min(args.steps, 2))
+        for _ in range(nrep):
+            tt.cheb_filter_host(Hd, Xh, Yh, cfg.m, a, b, a0, panel_cols=1024, work=hwork)
+        barrier()
+        t_e2e = (time.perf_counter() - t0) / nrep
+        if dist is not None:
+            tm = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+            t_e2e = float(tm.item())
+        e2e = {"value": 2.0 * nnz * cfg.N * cfg.m * world / t_e2e / 1e9, "unit": "GFLOP/s",
+               "h2d_bytes_per_step": cfg.M * cfg.N * 8, "d2h_bytes_per_step": cfg.M * cfg.N * 8,
+               "ms_per_step": t_e2e * 1e3, "api": "ttdft_cheb_filter_host (pinned host X, Y; 1024-column panels)"}
+        # sanity: the host path and the device path agree bit for bit on this rank's band
+        same = bool(torch.equal(Yh.to(dev), Yd))
+        e2e["matches_device_path"] = same
+        del hwork
+
+    useful = 2.0 * nnz * cfg.N * cfg.m
+    executed = 2.0 * H.nblocks * cfg.b * cfg.b * cfg.N * cfg.m
+    npanels = -(-cfg.N // (panel if panel else min(cfg.N, 4096)))
+    alg_bytes = cfg.m * (npanels * 8.0 * nnz + 24.0 * cfg.M * cfg.N) - 8.0 * cfg.M * cfg.N
+    # dominant kernel: the fused step kernel; one launch = one recurrence step over one panel
+    step_launches = args.steps * cfg.m * npanels
+    t_launch = t_region / step_launches
+    flops_per_launch = useful / (cfg.m * npanels)
+    achieved_tf = flops_per_launch / t_launch / 1e12
+    roof = {"bound": "alu", "achieved": achieved_tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+            "frac": achieved_tf / FP64_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+            "kernel": "ttdft::bsr_dmma_kernel", "launch_ms": t_launch * 1e3,
+            "peak_source": "derived: 148 SM x 64 fp64 FMA/clk x 2 x 1.965 GHz (fp64 has no entry in MEASURED_PEAKS.json)",
+            "executed_tflops": executed / (cfg.m * npanels) / t_launch / 1e12,
+            "executed_frac": executed / (cfg.m * npanels) / t_launch / 1e12 / FP64_PEAK_TFLOPS,
+            "dense_tile_ceiling": useful / executed,
+            "hbm_alg_gbs": alg_bytes / t_step / 1e9}
+    try:
+        roof["peak_measured_dmma"] = tt.probe_fp64_peak(1, 300)
+    except Exception:
+        pass
+
+    line = {
+        "metric": "ChFSI filter useful fp64 GFLOP/s", "value": useful * world / t_step / 1e9, "unit": "GFLOP/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg, nnz, H.nblocks, args),
+        "clocks": clocks, "gpu_launches": int(launches), "roofline": roof,
+        "h_build_ms": t_build * 1e3,
+    }
+    if e2e is not None:
+        line["e2e"] = e2e
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        dt, _, cols, Xs, Yo, threads = oracle_sample_run(cfg, H, args.ref_cols, cfg.m, (a, b, a0))
+        got = Yd[:, torch.from_numpy(cols).to(dev)].cpu().numpy()
+        err = float(np.linalg.norm(got - Yo) / np.linalg.norm(Yo))
+        line["cpu_baseline"] = {"value": 2.0 * nnz * len(cols) * cfg.m / dt / 1e9, "unit": "GFLOP/s", "cores": threads,
+                                "kind": "oracle", "seconds": dt,
+                                "sample": f"{len(cols)} seeded columns of {cfg.N} (all rows, all m={cfg.m} steps)",
+                                "gpu_vs_oracle_relerr_on_sample": err}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
