@@ -1,0 +1,121 @@
+"""BASELINE.json config 5: a single H*X (ttdft_spmm) and a single fused recurrence step
+(ttdft_cheb_step) on config 3's H at N in {16, 64, 256, 1024, 4096}, in two layouts --
+subdomain-ordered BSR and CSR with rows/columns symmetrically permuted by seed (irregular-access
+stress) -- each reported against the binding roofline:
+    T_roof = max(alg_bytes / BW_hbm, useful_flops / P_fp64).
+
+    python -m paper_2110_15853_b200.sweep [--workload si] [--layouts bsr,csr] [--out gpurun_out/sweep.json]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import synth  # noqa: E402
+
+FP64_PEAK = 148 * 64 * 2 * 1.965e9        # flop/s, derived
+
+
+def hbm_peak() -> float:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f)["hbm_gbs"] * 1e9
+    return 6.65e12                            # B200_PROFILING.md fallback
+
+
+def time_launches(fn, reps, flush):
+    import torch
+    for _ in range(3):
+        fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(reps):
+        if flush is not None:
+            flush.zero_()                     # > L2 write between timed launches
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn()
+        e1.record()
+        e1.synchronize()
+        ts.append(e0.elapsed_time(e1) * 1e-3)
+    return float(np.median(ts)), float(np.min(ts))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--workload", default="si")
+    ap.add_argument("--layouts", default="bsr,csr")
+    ap.add_argument("--ns", default="16,64,256,1024,4096")
+    ap.add_argument("--reps", type=int, default=10)
+    ap.add_argument("--csr-max-n", type=int, default=4096)
+    ap.add_argument("--out", default="")
+    args = ap.parse_args()
+    import torch
+    import paper_2110_15853_b200 as tt
+
+    cfg = synth.CONFIGS[args.workload]
+    H = synth.hamiltonian_bsr(cfg.G, cfg.b, cfg.z, cfg.seed)
+    nnz = int(np.count_nonzero(H.values))
+    bw = hbm_peak()
+    dev = torch.device("cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    rows = []
+    handles = {}
+    if "bsr" in args.layouts:
+        handles["bsr"] = tt.h_build_bsr(H.M, H.b, torch.from_numpy(H.row_ptr).to(dev), torch.from_numpy(H.col_idx).to(dev),
+                                        torch.from_numpy(H.values).to(dev))
+    if "csr" in args.layouts:
+        C = synth.bsr_to_csr_nonzeros(H)
+        perm = synth.permutation(H.M, cfg.seed + 50)
+        Cp = synth.permute_csr(C, perm)
+        del C
+        handles["csr"] = tt.h_build_csr(Cp.M, torch.from_numpy(Cp.row_ptr).to(dev), torch.from_numpy(Cp.col_idx).to(dev),
+                                        torch.from_numpy(Cp.values).to(dev))
+        del Cp
+    stored = {k: h.info()["nnz_stored"] for k, h in handles.items()}
+    del H
+    for N in [int(x) for x in args.ns.split(",")]:
+        X = torch.randn(cfg.M, N, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(N))
+        Z = torch.randn(cfg.M, N, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(N + 1))
+        O = torch.empty_like(X)
+        for layout, Hd in handles.items():
+            if layout == "csr" and N > args.csr_max_n:
+                continue
+            for op in ("spmm", "step"):
+                if op == "spmm":
+                    fn = lambda: tt.spmm(Hd, 1.0, X, 0.0, O)
+                    alg_bytes = 8.0 * nnz + 16.0 * cfg.M * N
+                else:
+                    fn = lambda: tt.cheb_step(Hd, 0.1, 10.0, -0.2, X, Z, O)
+                    alg_bytes = 8.0 * nnz + 24.0 * cfg.M * N
+                reps = args.reps if (layout == "bsr" or N <= 256) else 3
+                t_med, t_min = time_launches(fn, reps, flush)
+                flops = 2.0 * nnz * N
+                t_roof = max(alg_bytes / bw, flops / FP64_PEAK)
+                row = {"layout": layout, "op": op, "N": N, "ms": t_med * 1e3, "ms_min": t_min * 1e3,
+                       "useful_tflops": flops / t_med / 1e12, "alg_gbs": alg_bytes / t_med / 1e9,
+                       "executed_tflops": 2.0 * stored[layout] * N / t_med / 1e12,
+                       "binds": "hbm" if alg_bytes / bw > flops / FP64_PEAK else "fp64",
+                       "roofline_frac": t_roof / t_med, "kernel": Hd.info()["kernel"]}
+                rows.append(row)
+                print(json.dumps(row), flush=True)
+        del X, Z, O
+    out = {"workload": args.workload, "M": cfg.M, "nnz": nnz, "hbm_peak_gbs": bw / 1e9, "fp64_peak_tflops": FP64_PEAK / 1e12,
+           "rows": rows}
+    if args.out:
+        os.makedirs(os.path.dirname(args.out) or ".", exist_ok=True)
+        with open(args.out, "w") as f:
+            json.dump(out, f, indent=1)
+
+
+if __name__ == "__main__":
+    main()
