@@ -8,6 +8,7 @@
 #include <atomic>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -93,7 +94,9 @@ struct ttdft_h_s {
   const int32_t* col = nullptr;
   const double* val = nullptr;
   size_t storage_bytes = 0;
-  CUtensorMap tmH;          // K1 only
+  CUtensorMap tmH;          // K1 only: box b x 16
+  CUtensorMap tmH_half;     // K1, b = 128: box 64 x 16 (two CTAs per block row, two CTAs per SM)
+  int32_t split = 0;
   int32_t cg = 4;           // column tiles per scheduling group
 };
 
@@ -291,13 +294,18 @@ __global__ void __launch_bounds__(256) probe_dmma_kernel(double* out, int iters,
 // ------------------------------------------------------------------------------------------------
 // step dispatch:  O = alpha*H*X + gamma*X + beta*Z   (gamma = -alpha*c for a recurrence step)
 // ------------------------------------------------------------------------------------------------
-template <int WR>
-ttdft_status launch_k1(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
-                       const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, cudaStream_t st) {
-  using SM = ttdft::K1Smem<WR>;
+int env_int(const char* name, int dflt) {
+  const char* v = getenv(name);
+  return v && *v ? atoi(v) : dflt;
+}
+
+template <int WR, int Q, int CPS, int RS>
+ttdft_status launch_k1(const ttdft_h_s* h, const CUtensorMap& tmH, double alpha, double gamma, double beta, const double* X,
+                       int64_t ldx, const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, cudaStream_t st) {
+  using SM = ttdft::K1Cfg<WR, Q, CPS, RS>;
   static bool attr_set = false;
   if (!attr_set) {
-    CUDA_TRY(cudaFuncSetAttribute(ttdft::bsr_dmma_kernel<WR>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::TOTAL));
+    CUDA_TRY(cudaFuncSetAttribute(ttdft::bsr_dmma_kernel<WR, Q, CPS, RS>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::TOTAL));
     attr_set = true;
   }
   CUtensorMap tmX;
@@ -307,7 +315,9 @@ ttdft_status launch_k1(const ttdft_h_s* h, double alpha, double gamma, double be
   p.brow_ptr = h->row_ptr;
   p.bcol = h->col;
   p.nb = (int32_t)h->nb;
-  p.nct = (int32_t)((ncols + ttdft::K1_TN - 1) / ttdft::K1_TN);
+  p.b = h->b;
+  p.rs = RS;
+  p.nct = (int32_t)((ncols + SM::TN - 1) / SM::TN);
   p.cg = h->cg;
   p.ncols = ncols;
   p.alpha = alpha; p.gamma = gamma; p.beta = beta;
@@ -316,12 +326,37 @@ ttdft_status launch_k1(const ttdft_h_s* h, double alpha, double gamma, double be
   p.O = O; p.ldo = ldo;
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
-  const int64_t tiles = (int64_t)p.nb * p.nct;
+  const int64_t tiles = (int64_t)p.nb * p.rs * p.nct;
   if (tiles > 0x7fffffffLL) return fail(TTDFT_ERR_UNSUPPORTED, "too many tiles (%lld)", (long long)tiles);
-  ttdft::bsr_dmma_kernel<WR><<<(unsigned)tiles, 32 * (2 * WR + 1), SM::TOTAL, st>>>(h->tmH, tmX, p);
+  ttdft::bsr_dmma_kernel<WR, Q, CPS, RS><<<(unsigned)tiles, SM::THREADS, SM::TOTAL, st>>>(tmH, tmX, p);
   CUDA_TRY(cudaGetLastError());
   g_launches.fetch_add(1);
   return TTDFT_OK;
+}
+
+// column-tile width by the number of columns: narrow tiles keep the HBM-bound small-N regime from
+// multiplying padding columns (BASELINE.json config 5, N = 16 / 64)
+template <int WR, int CPS, int RS>
+ttdft_status launch_k1_q(const ttdft_h_s* h, const CUtensorMap& tmH, double alpha, double gamma, double beta, const double* X,
+                         int64_t ldx, const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, cudaStream_t st) {
+  if (ncols <= 16) return launch_k1<WR, 1, CPS, RS>(h, tmH, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+  if (ncols <= 32) return launch_k1<WR, 2, CPS, RS>(h, tmH, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+  if (ncols <= 64) return launch_k1<WR, 4, CPS, RS>(h, tmH, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+  return launch_k1<WR, 8, CPS, RS>(h, tmH, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+}
+
+ttdft_status launch_k1_any(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
+                           const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, cudaStream_t st) {
+  switch (h->b) {
+    case 32: return launch_k1_q<1, 1, 1>(h, h->tmH, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+    case 64: return launch_k1_q<2, 1, 1>(h, h->tmH, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+    case 96: return launch_k1_q<3, 1, 1>(h, h->tmH, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+    case 128:
+      if (h->split) return launch_k1_q<2, 2, 2>(h, h->tmH_half, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+      return launch_k1_q<4, 1, 1>(h, h->tmH, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+    default: break;
+  }
+  return fail(TTDFT_ERR_UNSUPPORTED, "tile size %d has no block-sparse kernel", h->b);
 }
 
 ttdft_status launch_step(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
@@ -329,13 +364,15 @@ ttdft_status launch_step(const ttdft_h_s* h, double alpha, double gamma, double 
   if (h->M == 0) return TTDFT_OK;
   const bool tma_ok = (reinterpret_cast<uintptr_t>(X) & 15) == 0 && (ldx % 2 == 0) && alpha != 0.0;
   if (h->kernel == 1 && tma_ok) {
-    switch (h->b) {
-      case 32: return launch_k1<1>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
-      case 64: return launch_k1<2>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
-      case 96: return launch_k1<3>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
-      case 128: return launch_k1<4>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
-      default: break;
+    // full 128-column tiles first, then one narrower launch for a remainder of <= 64 columns
+    const int64_t rem = ncols % 128;
+    if (ncols > 128 && rem != 0 && rem <= 64) {
+      const int64_t main_cols = ncols - rem;
+      ttdft_status s = launch_k1_any(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, main_cols, st);
+      if (s != TTDFT_OK) return s;
+      return launch_k1_any(h, alpha, gamma, beta, X + main_cols, ldx, Z ? Z + main_cols : Z, ldz, O + main_cols, ldo, rem, st);
     }
+    return launch_k1_any(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
   }
   ttdft::K2Params p;
   p.row_ptr = h->row_ptr; p.col = h->col; p.val = h->val;
@@ -608,6 +645,13 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
   if (h->kernel == 1) {
     s = make_map_2d(&h->tmH, h->val, (uint64_t)h->b, (uint64_t)h->nblocks * h->b, (uint64_t)h->b, (uint32_t)h->b);
     if (s != TTDFT_OK) { delete h; return s; }
+    if (h->b == 128) {
+      s = make_map_2d(&h->tmH_half, h->val, (uint64_t)h->b, (uint64_t)h->nblocks * h->b, (uint64_t)h->b, 64u);
+      if (s != TTDFT_OK) { delete h; return s; }
+      h->split = env_int("TTDFT_K1_SPLIT", 0);
+    }
+    h->cg = env_int("TTDFT_K1_CG", 4);
+    if (h->cg < 1) h->cg = 1;
   }
   *out = h;
   return TTDFT_OK;
