@@ -47,6 +47,22 @@ typedef enum { TTDFT_FMT_CSR = 0, TTDFT_FMT_BSR = 1 } ttdft_format;
 #define TTDFT_CHECK_SORTED 1u   /* verify indices in range, ascending and unique per row (synchronises) */
 #define TTDFT_CHECK_SYMMETRY 2u /* verify H == H^T bit for bit (synchronises; needs sorted columns)      */
 #define TTDFT_FORCE_GENERIC 4u  /* keep the input format and use the generic row-per-warp kernel          */
+#define TTDFT_NO_I8 8u          /* do not build the int8 digit planes (saves 0.75x of the tile bytes)     */
+
+/*
+ * Arithmetic of the block-sparse product (every mode returns fp64 results inside north_star's
+ * tolerance; DESIGN.md "Kernel K3" has the error bound):
+ *   TTDFT_MATH_FP64  fp64 tensor-core MMA (DMMA), fp64 accumulation.
+ *   TTDFT_MATH_I8    each fp64 operand is split exactly into 6 balanced base-256 digit planes (47 bits
+ *                    below the maximum of its H row / Y column; the diagonal of H stays fp64), the
+ *                    plane products run on the int8 tensor cores with exact int32 accumulation, and
+ *                    the epilogue recombines them in fp64.  Needs scratch for the digit planes of one
+ *                    iterate, so it is used by the calls that take `work`.
+ *   TTDFT_MATH_AUTO  I8 where it is faster (tile size >= 64 and digit planes built), else FP64.
+ */
+#define TTDFT_MATH_AUTO 0
+#define TTDFT_MATH_FP64 1
+#define TTDFT_MATH_I8 2
 
 /*
  * Description of the input Hamiltonian (PAPER.md:L199-205 H^L; L250-252 block structure: "the
@@ -80,6 +96,8 @@ typedef struct {
   int32_t kernel;         /* 1 = block-sparse TMA + fp64 tensor-core kernel, 0 = generic    */
   int64_t nblocks;
   size_t storage_bytes;
+  int32_t i8_planes;      /* digit planes per operand stored for TTDFT_MATH_I8 (0: not built) */
+  int32_t math;           /* TTDFT_MATH_FP64 or TTDFT_MATH_I8: what calls that take `work` use */
 } ttdft_h_info_t;
 
 /* A0 -- storage builder (north_star "BSR/CSR storage builder"). */
@@ -97,6 +115,12 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* desc, void* dev_storage, size_t b
                            ttdft_h_t* out);
 ttdft_status ttdft_h_info(ttdft_h_t h, ttdft_h_info_t* info);
 ttdft_status ttdft_h_destroy(ttdft_h_t h);
+
+/* Select the arithmetic for the calls that take `work` (ttdft_cheb_filter*, ttdft_*_ws); the default
+ * is TTDFT_MATH_AUTO (or the value of the environment variable TTDFT_MATH at build time).  Changes the
+ * handle: do not call it while another thread is using the handle; query the work sizes again
+ * afterwards.  TTDFT_ERR_UNSUPPORTED if I8 is asked of a handle without digit planes. */
+ttdft_status ttdft_h_set_math_mode(ttdft_h_t h, int32_t mode);
 
 /*
  * Y = alpha * H * X + beta * Y         (the kernel of every filter step)
@@ -118,6 +142,18 @@ ttdft_status ttdft_cheb_step(ttdft_h_t h, double alpha, double c, double beta, c
                              void* stream);
 
 /*
+ * The same two operations with caller-provided scratch, which lets them run in the handle's math mode
+ * (TTDFT_MATH_I8 needs room for the digit planes of X / Yk): `work` is a 16-byte aligned DEVICE
+ * buffer of at least ttdft_step_work_bytes(h, ncols) bytes (0 in TTDFT_MATH_FP64: work may be NULL).
+ */
+ttdft_status ttdft_step_work_bytes(ttdft_h_t h, int64_t ncols, size_t* bytes);
+ttdft_status ttdft_spmm_ws(ttdft_h_t h, double alpha, const double* X, int64_t ldx, double beta, double* Y,
+                           int64_t ldy, int64_t ncols, void* work, size_t work_bytes, void* stream);
+ttdft_status ttdft_cheb_step_ws(ttdft_h_t h, double alpha, double c, double beta, const double* Yk, int64_t ldk,
+                                const double* Ykm1, int64_t ldm, double* Yout, int64_t ldo, int64_t ncols,
+                                void* work, size_t work_bytes, void* stream);
+
+/*
  * A1 -- the scalars of Algorithm 1, HOST arrays of length m:
  *   e = (b-a)/2, c = (b+a)/2, sigma_1 = e/(a0-c), gamma = 2/sigma_1, sigma_{k+1} = 1/(gamma-sigma_k)
  *   alpha[0] = sigma_1/e, beta[0] = 0;   alpha[k] = 2*sigma_{k+1}/e, beta[k] = -sigma_k*sigma_{k+1}
@@ -128,7 +164,8 @@ ttdft_status ttdft_cheb_scalars(int32_t m, double a, double b, double a0, double
                                 double* beta);
 
 /* Bytes of scratch ttdft_cheb_filter needs: one compact M x panel panel (panel_cols == 0: the
- * library's default panel width for this ncols). */
+ * library's default panel width for this ncols), plus, in TTDFT_MATH_I8, the int8 digit planes of
+ * one iterate (6 bytes per element) and two arrays of column maxima. */
 ttdft_status ttdft_cheb_filter_work_bytes(ttdft_h_t h, int64_t ncols, int64_t panel_cols, size_t* bytes);
 
 /*

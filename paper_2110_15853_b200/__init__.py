@@ -26,4 +26,9 @@ from .api import (  # noqa: F401
     CHECK_SORTED,
     CHECK_SYMMETRY,
     FORCE_GENERIC,
+    NO_I8,
+    MATH_AUTO,
+    MATH_FP64,
+    MATH_I8,
+    step_work_bytes,
 )

@@ -8,7 +8,8 @@ from ctypes import POINTER, byref, c_char_p, c_double, c_int32, c_int64, c_size_
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_PKG, "libttdft.so")
 
-CHECK_SORTED, CHECK_SYMMETRY, FORCE_GENERIC = 1, 2, 4
+CHECK_SORTED, CHECK_SYMMETRY, FORCE_GENERIC, NO_I8 = 1, 2, 4, 8
+MATH_AUTO, MATH_FP64, MATH_I8 = 0, 1, 2
 FMT_CSR, FMT_BSR = 0, 1
 _STATUS = {0: "OK", 1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "NOT_SYMMETRIC", 5: "CUDA"}
 
@@ -17,6 +18,7 @@ exported_symbols = [
     "ttdft_h_storage_bytes", "ttdft_h_build", "ttdft_h_info", "ttdft_h_destroy", "ttdft_spmm", "ttdft_cheb_step",
     "ttdft_cheb_scalars", "ttdft_cheb_filter_work_bytes", "ttdft_cheb_filter", "ttdft_cheb_filter_host_work_bytes",
     "ttdft_cheb_filter_host", "ttdft_probe_fp64_peak", "ttdft_launch_count", "ttdft_last_error",
+    "ttdft_h_set_math_mode", "ttdft_step_work_bytes", "ttdft_spmm_ws", "ttdft_cheb_step_ws",
 ]
 
 
@@ -34,7 +36,7 @@ class _Desc(ctypes.Structure):
 
 class _Info(ctypes.Structure):
     _fields_ = [("M", c_int64), ("nnz_stored", c_int64), ("block", c_int32), ("kernel", c_int32), ("nblocks", c_int64),
-                ("storage_bytes", c_size_t)]
+                ("storage_bytes", c_size_t), ("i8_planes", c_int32), ("math", c_int32)]
 
 
 _lib = None
@@ -66,6 +68,16 @@ def _load() -> ctypes.CDLL:
     L.ttdft_cheb_step.restype = st
     L.ttdft_cheb_step.argtypes = [c_void_p, c_double, c_double, c_double, c_void_p, c_int64, c_void_p, c_int64, c_void_p,
                                   c_int64, c_int64, c_void_p]
+    L.ttdft_h_set_math_mode.restype = st
+    L.ttdft_h_set_math_mode.argtypes = [c_void_p, c_int32]
+    L.ttdft_step_work_bytes.restype = st
+    L.ttdft_step_work_bytes.argtypes = [c_void_p, c_int64, POINTER(c_size_t)]
+    L.ttdft_spmm_ws.restype = st
+    L.ttdft_spmm_ws.argtypes = [c_void_p, c_double, c_void_p, c_int64, c_double, c_void_p, c_int64, c_int64, c_void_p, c_size_t,
+                                c_void_p]
+    L.ttdft_cheb_step_ws.restype = st
+    L.ttdft_cheb_step_ws.argtypes = [c_void_p, c_double, c_double, c_double, c_void_p, c_int64, c_void_p, c_int64, c_void_p,
+                                     c_int64, c_int64, c_void_p, c_size_t, c_void_p]
     L.ttdft_cheb_scalars.restype = st
     L.ttdft_cheb_scalars.argtypes = [c_int32, c_double, c_double, c_double, POINTER(c_double), POINTER(c_double),
                                      POINTER(c_double)]
@@ -144,6 +156,11 @@ class Hamiltonian:
         _check(_load().ttdft_h_info(self.handle, byref(inf)))
         return {k: getattr(inf, k) for k, _ in _Info._fields_}
 
+    def set_math_mode(self, mode: int):
+        """ttdft_h_set_math_mode: MATH_AUTO / MATH_FP64 / MATH_I8 for the calls that take `work`."""
+        _check(_load().ttdft_h_set_math_mode(self.handle, mode))
+        return self
+
     def destroy(self):
         if self._h is not None:
             _load().ttdft_h_destroy(self._h)
@@ -201,23 +218,47 @@ def h_build_csr(M, row_ptr, col_idx, values, subdomain_of_row=None, flags=0, str
     return h_build(FMT_CSR, M, 0, row_ptr, col_idx, values, subdomain_of_row, flags, stream)
 
 
-def spmm(H: Hamiltonian, alpha: float, X, beta: float, Y, stream=None):
-    """Y = alpha*H*X + beta*Y (ttdft_spmm)."""
+def step_work_bytes(H: Hamiltonian, ncols: int) -> int:
+    n = c_size_t()
+    _check(_load().ttdft_step_work_bytes(H.handle, ncols, byref(n)))
+    return int(n.value)
+
+
+def _work(H: Hamiltonian, ncols: int, work, device):
+    """(aligned pointer, usable bytes, keep-alive tensor) of the scratch of the *_ws calls."""
+    torch = _torch()
+    if work is None:
+        work = torch.empty(step_work_bytes(H, ncols) + 16, dtype=torch.uint8, device=device)
+    wp = (work.data_ptr() + 15) // 16 * 16
+    return wp, work.numel() * work.element_size() - (wp - work.data_ptr()), work
+
+
+def spmm(H: Hamiltonian, alpha: float, X, beta: float, Y, stream=None, work=None, use_work=False):
+    """Y = alpha*H*X + beta*Y (ttdft_spmm; with work / use_work: ttdft_spmm_ws in the handle's math mode)."""
     xp, ldx = _mat(X, "X")
     yp, ldy = _mat(Y, "Y")
     if X.shape != Y.shape or X.shape[0] != H.M:
         raise ValueError("shape mismatch")
+    if work is not None or use_work:
+        wp, wb, keep = _work(H, X.shape[1], work, X.device)
+        _check(_load().ttdft_spmm_ws(H.handle, alpha, xp, ldx, beta, yp, ldy, X.shape[1], wp, wb, _stream(stream)))
+        return Y
     _check(_load().ttdft_spmm(H.handle, alpha, xp, ldx, beta, yp, ldy, X.shape[1], _stream(stream)))
     return Y
 
 
-def cheb_step(H: Hamiltonian, alpha: float, c: float, beta: float, Yk, Ykm1, Yout, stream=None):
-    """Yout = alpha*(H*Yk - c*Yk) + beta*Ykm1 (ttdft_cheb_step); Ykm1 None = beta term absent."""
+def cheb_step(H: Hamiltonian, alpha: float, c: float, beta: float, Yk, Ykm1, Yout, stream=None, work=None, use_work=False):
+    """Yout = alpha*(H*Yk - c*Yk) + beta*Ykm1 (ttdft_cheb_step[_ws]); Ykm1 None = beta term absent."""
     kp, ldk = _mat(Yk, "Yk")
     op, ldo = _mat(Yout, "Yout")
     mp, ldm = (None, 0) if Ykm1 is None else _mat(Ykm1, "Ykm1")
     if Yk.shape != Yout.shape or Yk.shape[0] != H.M or (Ykm1 is not None and Ykm1.shape != Yk.shape):
         raise ValueError("shape mismatch")
+    if work is not None or use_work:
+        wp, wb, keep = _work(H, Yk.shape[1], work, Yk.device)
+        _check(_load().ttdft_cheb_step_ws(H.handle, alpha, c, beta, kp, ldk, mp, ldm, op, ldo, Yk.shape[1], wp, wb,
+                                          _stream(stream)))
+        return Yout
     _check(_load().ttdft_cheb_step(H.handle, alpha, c, beta, kp, ldk, mp, ldm, op, ldo, Yk.shape[1], _stream(stream)))
     return Yout
 

@@ -1,0 +1,336 @@
+// bsr_i8.cuh -- kernel K3: the filter step  O = alpha*(H*Y_k) + gamma*Y_k + beta*Y_{k-1}
+// (the product is "the main kernel", L236) with the block-dense contraction
+// carried by the 5th-generation tensor cores as exact int8 digit-plane products (i8_digits.cuh).
+//
+// sm_100a design:
+//   * persistent CTAs (one per SM), static round-robin over (block row I, 64-column tile) work items in
+//     the same L2-friendly order as K1
+//   * warp 0 (one lane): TMA producer.  Per tile (I,J) of the block row it brings the S digit planes of
+//     Y_k rows J*b.., 64 columns, with ONE 3-D bulk-tensor load (S x 64 x 128 B, SWIZZLE_128B) into one
+//     of two Y buffers, and the S digit planes of H_IJ (b x 128 B each) through a ring of 16 KB slots
+//   * warp 1 (one lane): tcgen05.mma.kind::i8 issuer.  For H plane p it multiplies against the
+//     CONCATENATION of Y planes 0..S-1-p (N = 64*(S-p), issued as <=256-column instructions), which lands
+//     in the contiguous TMEM column groups p..S-1 because digit-pair level g = p+q lives at columns
+//     [64g, 64g+64).  S(S+1)/2 plane pairs cost 4+... wide MMAs instead of S(S+1)/2 narrow ones, so the
+//     A operand is read from shared memory once per plane and the tensor pipe, not shared memory, binds
+//   * accumulators: S levels x 64 columns of int32 in TMEM (384 of 512 columns for S = 6), exact
+//   * warps 2-5: epilogue.  Each thread owns one row: Horner over the levels (least significant first)
+//     into 64 fp64 registers, releases TMEM, then  out = alpha*2^(eH_i+eY_j-14)*v + (alpha*hdiag_i+gamma)*y
+//     + beta*z  with 128-bit accesses, and accumulates the column maxima of `out` for the next step's
+//     digit scaling (warp REDUX + shared/global atomicMax on the upper word)
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "bsr_dmma.cuh"   // smem_u32, mbarrier and TMA wrappers
+#include "i8_digits.cuh"
+
+namespace ttdft {
+
+constexpr int K3_NT = 64;        // columns per work item
+constexpr int K3_THREADS = 192;  // producer warp, MMA warp, 4 epilogue warps
+
+struct K3Params {
+  const int32_t* brow_ptr;
+  const int32_t* bcol;
+  int32_t nb, b, nct, cg, vec;
+  int64_t ncols;
+  double alpha, gamma, beta;
+  const double* S;  int64_t lds;   // Y_k at the output position (diagonal + shift term)
+  const double* Z;  int64_t ldz;   // Y_{k-1}; unused if beta == 0
+  double* O;        int64_t ldo;
+  const int32_t* eH;               // row exponents of H          [M]
+  const double* hdiag;             // diagonal of H (fp64)         [M]
+  const uint32_t* cmaxS;           // column maxima of Y_k (upper words)   [ncols]
+  uint32_t* cmaxO;                 // out: column maxima of O, or NULL
+};
+
+template <int S>
+struct K3Cfg {
+  static constexpr int YBUF = S * K3_NT * 128;            // one Y buffer: S planes x 64 columns x 128 k-bytes
+  static constexpr int HSLOT = 128 * 128;                 // one H plane of one tile
+  static constexpr int NH = (232448 - 2048 - 2 * YBUF) / HSLOT;   // ring slots that fit beside two Y buffers
+  static constexpr int BAR_OFFSET = 2 * YBUF + NH * HSLOT;
+  static constexpr int NBAR = 4 + 2 * NH + 2;
+  static constexpr int CS_OFFSET = BAR_OFFSET + 8 * ((NBAR + 1) & ~1);   // 64 doubles: column scales
+  static constexpr int CM_OFFSET = CS_OFFSET + 64 * 8;                   // 64 words: column maxima
+  static constexpr int TOTAL = CM_OFFSET + 64 * 4 + 16 + 1024;           // + tmem slot + alignment slack
+  static_assert(S * K3_NT <= 512, "digit levels must fit TMEM");
+  static_assert(NH >= 3, "H ring too short");
+};
+
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, int32_t x, int32_t y, int32_t z, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+          smem_u32(dst)),
+      "l"(map), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar))
+      : "memory");
+}
+// shared-memory matrix descriptor: K-major rows of 128 bytes, SWIZZLE_128B, 8-row groups 1024 B apart
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
+  return (uint64_t)((saddr & 0x3ffffu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) |
+         ((uint64_t)2 << 61);
+}
+// instruction descriptor, kind::i8: D = s32, A = B = signed int8, both K-major, M = 128
+__device__ __forceinline__ uint32_t umma_idesc_i8(uint32_t n) {
+  return (2u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((128u >> 4) << 24);
+}
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n}\n" ::"r"(tmem_d),
+      "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+        "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr));
+}
+
+// work item t -> (block row I, column tile ct): column-tile groups outermost, block rows, tile fastest
+__device__ __forceinline__ void k3_decode(const K3Params& prm, int64_t t, int32_t& I, int32_t& ct) {
+  const int64_t per_group = (int64_t)prm.nb * prm.cg;
+  const int32_t ngroups = (prm.nct + prm.cg - 1) / prm.cg;
+  int32_t g = (int32_t)(t / per_group);
+  if (g > ngroups - 1) g = ngroups - 1;
+  const int64_t rem = t - (int64_t)g * per_group;
+  const int32_t width = min(prm.cg, prm.nct - g * prm.cg);
+  I = (int32_t)(rem / width);
+  ct = g * prm.cg + (int32_t)(rem % width);
+}
+
+template <int S>
+__global__ void __launch_bounds__(K3_THREADS, 1)
+bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ CUtensorMap tmYd, const K3Params prm) {
+  using C = K3Cfg<S>;
+  constexpr int NH = C::NH;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* ybuf = smem;                          // 2 x YBUF
+  uint8_t* hring = smem + 2 * C::YBUF;           // NH x HSLOT
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::BAR_OFFSET);
+  uint64_t* yfull = bars;                        // [2]
+  uint64_t* yempty = bars + 2;                   // [2]
+  uint64_t* hfull = bars + 4;                    // [NH]
+  uint64_t* hempty = bars + 4 + NH;              // [NH]
+  uint64_t* accfull = bars + 4 + 2 * NH;
+  uint64_t* accempty = accfull + 1;
+  double* cs_s = reinterpret_cast<double*>(smem + C::CS_OFFSET);        // 2^eY_j of the current tile
+  uint32_t* cm_s = reinterpret_cast<uint32_t*>(smem + C::CM_OFFSET);    // column maxima of the current tile
+  uint32_t* tmem_slot = cm_s + 64;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t ntiles = (int64_t)prm.nb * prm.nct;
+  const int32_t b = prm.b;
+  const int32_t ksteps = b >> 5;                 // 32-deep int8 MMAs per tile of H
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < 2; ++i) { mbar_init(&yfull[i], 1); mbar_init(&yempty[i], 1); }
+    for (int i = 0; i < NH; ++i) { mbar_init(&hfull[i], 1); mbar_init(&hempty[i], 1); }
+    mbar_init(accfull, 1);
+    mbar_init(accempty, 128);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(512));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;");
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ===================================== TMA producer =====================================
+    if (lane == 0) {
+      asm volatile("prefetch.tensormap [%0];" ::"l"(&tmHd) : "memory");
+      asm volatile("prefetch.tensormap [%0];" ::"l"(&tmYd) : "memory");
+      int yb = 0, hs = 0;
+      uint32_t yph = 0, hph = 0;
+      for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        int32_t I, ct;
+        k3_decode(prm, t, I, ct);
+        const int32_t p0 = prm.brow_ptr[I], p1 = prm.brow_ptr[I + 1];
+        for (int32_t p = p0; p < p1; ++p) {
+          const int32_t J = prm.bcol[p];
+          mbar_wait(&yempty[yb], yph ^ 1);
+          mbar_expect_tx(&yfull[yb], (uint32_t)C::YBUF);
+          tma_load_3d(ybuf + yb * C::YBUF, &tmYd, J * 128, ct * K3_NT, 0, &yfull[yb]);
+#pragma unroll 1
+          for (int q = 0; q < S; ++q) {
+            mbar_wait(&hempty[hs], hph ^ 1);
+            mbar_expect_tx(&hfull[hs], (uint32_t)b * 128u);
+            tma_load_2d(hring + hs * C::HSLOT, &tmHd, 0, (p * S + q) * b, &hfull[hs]);
+            if (++hs == NH) { hs = 0; hph ^= 1; }
+          }
+          yb ^= 1;
+          if (yb == 0) yph ^= 1;
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ====================================== MMA issuer ======================================
+    if (lane == 0) {
+      int yb = 0, hs = 0;
+      uint32_t yph = 0, hph = 0, aph = 0;
+      const uint32_t ybase = smem_u32(ybuf), hbase = smem_u32(hring);
+      for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        int32_t I, ct;
+        k3_decode(prm, t, I, ct);
+        const int32_t nJ = prm.brow_ptr[I + 1] - prm.brow_ptr[I];
+        if (nJ == 0) continue;
+        mbar_wait(accempty, aph ^ 1);            // the epilogue has drained the previous item's accumulators
+        asm volatile("tcgen05.fence::after_thread_sync;");
+        for (int32_t j = 0; j < nJ; ++j) {
+          mbar_wait(&yfull[yb], yph);
+          const uint32_t ya = ybase + yb * C::YBUF;
+#pragma unroll 1
+          for (int p = 0; p < S; ++p) {
+            mbar_wait(&hfull[hs], hph);
+            asm volatile("tcgen05.fence::after_thread_sync;");
+            const uint32_t ha = hbase + hs * C::HSLOT;
+            const int ntot = (S - p) * K3_NT;    // Y planes 0..S-1-p side by side -> levels p..S-1
+            for (int kk = 0; kk < ksteps; ++kk) {
+              const uint64_t da = umma_desc_sw128(ha + kk * 32);
+              const uint32_t acc = (j | kk | p) ? 1u : 0u;
+              for (int n0 = 0; n0 < ntot; n0 += 256) {
+                const int n = min(256, ntot - n0);
+                umma_i8(tmem_base + (uint32_t)(p * K3_NT + n0), da, umma_desc_sw128(ya + n0 * 128 + kk * 32), umma_idesc_i8(n), acc);
+              }
+            }
+            umma_commit(&hempty[hs]);            // slot free once these MMAs have read it
+            if (++hs == NH) { hs = 0; hph ^= 1; }
+          }
+          umma_commit(&yempty[yb]);
+          yb ^= 1;
+          if (yb == 0) yph ^= 1;
+        }
+        umma_commit(accfull);
+        aph ^= 1;
+      }
+    }
+  } else {
+    // ======================================= epilogue =======================================
+    const int quarter = warp & 3;                // TMEM lane quarter this warp may read
+    const int et = (warp - 2) * 32 + lane;       // 0..127 among the epilogue threads
+    const int r = quarter * 32 + lane;           // row inside the block row
+    const bool row_ok = r < b;
+    const double alpha = prm.alpha, beta = prm.beta;
+    const bool use_z = (beta != 0.0);
+    uint32_t aph = 0;
+    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+      int32_t I, ct;
+      k3_decode(prm, t, I, ct);
+      const int32_t nJ = prm.brow_ptr[I + 1] - prm.brow_ptr[I];
+      const int64_t col0 = (int64_t)ct * K3_NT;
+      const int64_t row = (int64_t)I * b + r;
+      if (et < 64) {
+        const int64_t cj = col0 + et;
+        cs_s[et] = pow2i(exp_from_hi(cj < prm.ncols ? prm.cmaxS[cj] : 0u));
+        cm_s[et] = 0;
+      }
+      double rsp = 0.0, gi = prm.gamma;
+      if (row_ok) {
+        rsp = pow2i(prm.eH[row] - 14);
+        gi = fma(alpha, prm.hdiag[row], prm.gamma);
+      }
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+
+      double v[K3_NT];
+      if (nJ > 0) {
+        mbar_wait(accfull, aph);
+        aph ^= 1;
+        asm volatile("tcgen05.fence::after_thread_sync;");
+        const uint32_t trow = tmem_base + ((uint32_t)(quarter * 32) << 16);
+#pragma unroll
+        for (int g = S - 1; g >= 0; --g) {       // Horner, least significant level first
+          uint32_t a[4][16];
+#pragma unroll
+          for (int c = 0; c < 4; ++c) tmem_ld16(trow + (uint32_t)(g * K3_NT + c * 16), a[c]);
+          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+          for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+              asm volatile("" : "+r"(a[c][i]));   // consumers must stay behind the wait
+              const double x = (double)(int32_t)a[c][i];
+              v[c * 16 + i] = (g == S - 1) ? x : fma(v[c * 16 + i], 0.00390625, x);
+            }
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;");
+        mbar_arrive(accempty);                   // TMEM is free for the next work item
+      } else {
+#pragma unroll
+        for (int i = 0; i < K3_NT; ++i) v[i] = 0.0;
+      }
+
+      // ---- out = alpha * 2^(eH+eY-14) * v + (alpha*hdiag + gamma) * y + beta * z ----
+      const bool full = (col0 + K3_NT <= prm.ncols);
+      const double* sp = prm.S + row * prm.lds + col0;
+      const double* zp = prm.Z + row * prm.ldz + col0;
+      double* op = prm.O + row * prm.ldo + col0;
+      if (prm.vec && full) {
+#pragma unroll
+        for (int c0 = 0; c0 < K3_NT; c0 += 8) {
+          double2 y2[4], z2[4];
+          if (row_ok) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) y2[i] = __ldg(reinterpret_cast<const double2*>(sp + c0 + 2 * i));
+            if (use_z) {
+#pragma unroll
+              for (int i = 0; i < 4; ++i) z2[i] = *reinterpret_cast<const double2*>(zp + c0 + 2 * i);
+            }
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int j = c0 + 2 * i;
+            double o0 = 0.0, o1 = 0.0;
+            if (row_ok) {
+              o0 = fma(gi, y2[i].x, alpha * (v[j] * cs_s[j] * rsp));
+              o1 = fma(gi, y2[i].y, alpha * (v[j + 1] * cs_s[j + 1] * rsp));
+              if (use_z) { o0 = fma(beta, z2[i].x, o0); o1 = fma(beta, z2[i].y, o1); }
+              *reinterpret_cast<double2*>(op + j) = make_double2(o0, o1);
+            }
+            v[j] = o0; v[j + 1] = o1;
+          }
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < K3_NT; ++j) {
+          double o = 0.0;
+          if (row_ok && col0 + j < prm.ncols) {
+            o = fma(gi, sp[j], alpha * (v[j] * cs_s[j] * rsp));
+            if (use_z) o = fma(beta, zp[j], o);
+            op[j] = o;
+          }
+          v[j] = o;
+        }
+      }
+      // ---- column maxima of the new iterate (upper words), for the next step's digit scaling ----
+      if (prm.cmaxO) {
+#pragma unroll
+        for (int j = 0; j < K3_NT; ++j) {
+          const uint32_t m = __reduce_max_sync(0xffffffffu, abs_hi(v[j]));
+          if (lane == (j & 31) && m) atomicMax(&cm_s[j], m);
+        }
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (et < 64 && col0 + et < prm.ncols && cm_s[et]) atomicMax(&prm.cmaxO[col0 + et], cm_s[et]);
+      }
+      asm volatile("bar.sync 1, 128;" ::: "memory");   // cs_s / cm_s are rewritten by the next item
+    }
+  }
+
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  __syncthreads();
+  if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(512));
+}
+
+}  // namespace ttdft

@@ -1,0 +1,200 @@
+// i8_digits.cuh -- exact splitting of fp64 operands into balanced base-256 digits (int8 planes) for the
+// integer tensor-core kernel K3 (bsr_i8.cuh).
+//
+// The product inside every filter step (H x Y_k) is a block-dense fp64
+// contraction that is bound by the fp64 pipe.  B200's 5th-generation tensor
+// cores have no f64 kind, but they multiply int8 at ~4.5 Pop/s with exact int32 accumulation.  K3
+// therefore evaluates the same product as a sum of exact integer products of digit planes:
+//
+//   row i of H (diagonal entry kept apart in fp64):  h_ik ~= 2^(eH_i-(8S-1)) * sum_p dH_p[i,k] 256^(S-1-p)
+//   column j of Y_k:                                 y_kj ~= 2^(eY_j-(8S-1)) * sum_q dY_q[k,j] 256^(S-1-q)
+//
+// with balanced digits d in [-128,127], 2^e > max|.| of the row/column, S = 6 or 7 planes.  The only
+// error is the rounding of each operand to 8S-1 bits below its row/column maximum (2^-47 for S = 6),
+// and the omission of digit-pair levels p+q >= S (below that rounding); all accumulation is exact.
+// DESIGN.md "Kernel K3" has the error bound.  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ttdft {
+
+constexpr int I8_EMIN = -960;   // exponent clamp: keeps every scale factor a normal double
+
+// Upper 32 bits of |x| (monotone in |x| for finite x): the currency of the column/row maxima.
+__device__ __forceinline__ uint32_t abs_hi(double x) { return (uint32_t)__double2hiint(x) & 0x7fffffffu; }
+
+// Exponent e with max|x| * 2^-e <= 0.9942 (inside the balanced-digit range 127/255*2 = 0.99608), from
+// the upper word of the maximum.  The lower word is unknown, hence the margin on the mantissa.
+__host__ __device__ __forceinline__ int32_t exp_from_hi(uint32_t hi) {
+  int32_t e = (int32_t)(hi >> 20) - 1022;          // 1.f * 2^(E-1023) < 2^(E-1022)
+  if ((hi & 0xfffffu) >= 0xfd000u) e += 1;
+  if (e < I8_EMIN) e = I8_EMIN;
+  return e;
+}
+// 2^k as a double, k in [-1022, 1023]
+__device__ __forceinline__ double pow2i(int32_t k) { return __longlong_as_double((long long)(k + 1023) << 52); }
+
+// Balanced base-256 digits of q = rn(x * scale), most significant first; |q| <= 0.9961 * 2^(8S-1).
+template <int S>
+__device__ __forceinline__ void balanced_digits(double x, double scale, int32_t (&d)[S]) {
+  long long q = __double2ll_rn(x * scale);
+#pragma unroll
+  for (int p = S - 1; p >= 0; --p) {
+    const int32_t lo = (int32_t)(q & 0xff);
+    const int32_t dd = (lo ^ 0x80) - 0x80;   // sign-extend the low byte
+    d[p] = dd;
+    q = (q - dd) >> 8;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// column maxima of a panel (first step only; later steps get them from K3's epilogue)
+// cmax[j] = max_i hi(|Y[i,j]|); cmax must be zero on entry.  grid (ceil(ncols/64), ceil(M/2048)), 256 thr
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) colmax_kernel(const double* __restrict__ Y, int64_t ld, int64_t M, int64_t ncols,
+                                                     uint32_t* __restrict__ cmax) {
+  const int64_t col = (int64_t)blockIdx.x * 64 + (threadIdx.x & 63);
+  const int sub = threadIdx.x >> 6;
+  const int64_t r0 = (int64_t)blockIdx.y * 2048;
+  const int64_t r1 = min(M, r0 + 2048);
+  uint32_t m = 0;
+  if (col < ncols)
+    for (int64_t r = r0 + sub; r < r1; r += 4) m = max(m, abs_hi(Y[r * ld + col]));
+  __shared__ uint32_t sm[4][64];
+  sm[sub][threadIdx.x & 63] = m;
+  __syncthreads();
+  if (sub == 0 && col < ncols) {
+    m = max(max(sm[0][threadIdx.x], sm[1][threadIdx.x]), max(sm[2][threadIdx.x], sm[3][threadIdx.x]));
+    if (m) atomicMax(&cmax[col], m);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// digit planes of a panel, transposed:  D[q][n][I*128 + k] = digit q of Y[I*b + k, n]   (k < b)
+// One CTA per (block row I, 64-column tile): coalesced fp64 reads along the columns, a shared-memory
+// transpose, 128-byte coalesced int8 rows out -- the K-major rows K3's B operand wants.
+// Also clears next_cmax (the maxima K3's epilogue will accumulate for the following step).
+// grid (nb, ceil(ncols/64)), 256 threads, dynamic smem S*64*33*4 bytes
+// ------------------------------------------------------------------------------------------------
+template <int S>
+__global__ void __launch_bounds__(256) y_digits_kernel(const double* __restrict__ Y, int64_t ld, int32_t b, int64_t ncols,
+                                                       const uint32_t* __restrict__ cmax, int8_t* __restrict__ D, int64_t Mk,
+                                                       uint32_t* __restrict__ next_cmax) {
+  extern __shared__ uint32_t sd[];   // [S][64][33] words: row (q,n) holds 128 k-bytes + 1 pad word
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t I = blockIdx.x;
+  const int64_t n0 = (int64_t)blockIdx.y * 64;
+  if (next_cmax && I == 0 && threadIdx.x < 64 && n0 + threadIdx.x < ncols) next_cmax[n0 + threadIdx.x] = 0;
+
+  double scale[2];
+  bool cv[2];
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const int64_t n = n0 + 32 * h + lane;
+    cv[h] = n < ncols;
+    scale[h] = pow2i(8 * S - 1 - exp_from_hi(cv[h] ? cmax[n] : 0u));
+  }
+  const int nquads = b >> 2;
+  for (int quad = warp; quad < 32; quad += 8) {
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      uint32_t w[S];
+#pragma unroll
+      for (int p = 0; p < S; ++p) w[p] = 0;
+      if (quad < nquads && cv[h]) {
+        const double* src = Y + ((int64_t)I * b + 4 * quad) * ld + n0 + 32 * h + lane;
+        double x[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) x[i] = src[(int64_t)i * ld];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          int32_t d[S];
+          balanced_digits<S>(x[i], scale[h], d);
+#pragma unroll
+          for (int p = 0; p < S; ++p) w[p] |= (uint32_t)(d[p] & 0xff) << (8 * i);
+        }
+      }
+#pragma unroll
+      for (int p = 0; p < S; ++p) sd[(p * 64 + 32 * h + lane) * 33 + quad] = w[p];
+    }
+  }
+  __syncthreads();
+  for (int row = warp; row < S * 64; row += 8) {
+    const int p = row >> 6, n = row & 63;
+    if (n0 + n < ncols) {
+      uint32_t* dst = reinterpret_cast<uint32_t*>(D + ((int64_t)p * ncols + n0 + n) * Mk + I * 128);
+      dst[lane] = sd[row * 33 + lane];
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// H side (builder, A0): row exponents + diagonal, then digit planes of every tile
+// ------------------------------------------------------------------------------------------------
+// grid nb, 256 threads.  eH[row] from the row maximum over all tiles of the block row, the diagonal
+// entry excluded (it is applied in fp64 by K3's epilogue: Kohn-Sham H is diagonally heavy, and keeping
+// the diagonal out of the row scale keeps the digits of the couplings at full resolution).
+__global__ void __launch_bounds__(256) h_rowscale_kernel(int32_t b, const int32_t* __restrict__ brow_ptr,
+                                                         const int32_t* __restrict__ bcol, const double* __restrict__ tiles,
+                                                         int32_t* __restrict__ eH, double* __restrict__ hdiag) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int32_t I = blockIdx.x;
+  const int32_t p0 = brow_ptr[I], p1 = brow_ptr[I + 1];
+  for (int r = warp; r < b; r += 8) {
+    uint32_t m = 0;
+    double dg = 0.0;
+    for (int32_t p = p0; p < p1; ++p) {
+      const bool diag_tile = (bcol[p] == I);
+      const double* row = tiles + ((size_t)p * b + r) * b;
+      for (int k = lane; k < b; k += 32) {
+        const double v = row[k];
+        if (diag_tile && k == r) dg = v;
+        else m = max(m, abs_hi(v));
+      }
+    }
+    m = __reduce_max_sync(0xffffffffu, m);
+    // exactly one lane saw the diagonal entry (or none): pass it on by a sum
+    for (int o = 16; o > 0; o >>= 1) dg += __shfl_xor_sync(0xffffffffu, dg, o);
+    if (lane == 0) {
+      eH[(int64_t)I * b + r] = exp_from_hi(m);
+      hdiag[(int64_t)I * b + r] = dg;
+    }
+  }
+}
+
+// grid nb, 256 threads: planes Hd[(p*S + q)*b + r][128 bytes] of every tile p of block row I
+template <int S>
+__global__ void __launch_bounds__(256) h_digits_kernel(int32_t b, const int32_t* __restrict__ brow_ptr,
+                                                       const int32_t* __restrict__ bcol, const double* __restrict__ tiles,
+                                                       const int32_t* __restrict__ eH, int8_t* __restrict__ Hd) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int32_t I = blockIdx.x;
+  const int32_t p0 = brow_ptr[I], p1 = brow_ptr[I + 1];
+  for (int32_t p = p0; p < p1; ++p) {
+    const bool diag_tile = (bcol[p] == I);
+    for (int r = warp; r < b; r += 8) {
+      const double scale = pow2i(8 * S - 1 - eH[(int64_t)I * b + r]);
+      uint32_t w[S];
+#pragma unroll
+      for (int q = 0; q < S; ++q) w[q] = 0;
+      if (4 * lane < b) {
+        const double* src = tiles + ((size_t)p * b + r) * b + 4 * lane;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          double x = src[i];
+          if (diag_tile && 4 * lane + i == r) x = 0.0;
+          int32_t d[S];
+          balanced_digits<S>(x, scale, d);
+#pragma unroll
+          for (int q = 0; q < S; ++q) w[q] |= (uint32_t)(d[q] & 0xff) << (8 * i);
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < S; ++q)
+        reinterpret_cast<uint32_t*>(Hd + (((size_t)p * S + q) * b + r) * 128)[lane] = w[q];
+    }
+  }
+}
+
+}  // namespace ttdft

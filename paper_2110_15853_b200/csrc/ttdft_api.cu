@@ -16,6 +16,7 @@
 
 #include "../../include/ttdft.h"
 #include "bsr_dmma.cuh"
+#include "bsr_i8.cuh"
 #include "generic_spmm.cuh"
 
 namespace {
@@ -78,6 +79,42 @@ ttdft_status make_map_2d(CUtensorMap* map, const void* base, uint64_t cols, uint
 
 bool k1_block_ok(int32_t b) { return b == 32 || b == 64 || b == 96 || b == 128; }
 
+constexpr int I8_S = 6;   // digit planes per operand: 47 bits below each row / column maximum
+
+// H digit planes: uint8 [rows][128 bytes], box = box_rows x 128 B, 128B swizzle
+ttdft_status make_map_hd(CUtensorMap* map, const void* base, uint64_t rows, uint32_t box_rows) {
+  encode_tiled_fn enc = get_encode();
+  if (!enc) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  cuuint64_t dims[2] = {128, rows};
+  cuuint64_t strides[1] = {128};
+  cuuint32_t box[2] = {128, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled(H digits) failed with CUresult %d", (int)r);
+  return TTDFT_OK;
+}
+// Y digit planes: uint8 [S][ncols][Mk bytes], box = S x 64 x 128 B, 128B swizzle (columns beyond ncols read as 0)
+ttdft_status make_map_yd(CUtensorMap* map, const void* base, uint64_t Mk, uint64_t ncols, uint32_t S) {
+  encode_tiled_fn enc = get_encode();
+  if (!enc) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  cuuint64_t dims[3] = {Mk, ncols, S};
+  cuuint64_t strides[2] = {Mk, Mk * ncols};
+  cuuint32_t box[3] = {128, (cuuint32_t)ttdft::K3_NT, S};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled(Y digits) failed with CUresult %d", (int)r);
+  return TTDFT_OK;
+}
+
+// extra device storage of the int8 path: digit planes of every tile, row exponents, diagonal
+size_t i8_storage_bytes(int64_t nblocks, int32_t b, int64_t M) {
+  return align_up((size_t)nblocks * I8_S * b * 128, 1024) + align_up((size_t)M * 4, 1024) + align_up((size_t)M * 8, 1024);
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------
@@ -98,6 +135,14 @@ struct ttdft_h_s {
   CUtensorMap tmH_half;     // K1, b = 128: box 64 x 16 (two CTAs per block row, two CTAs per SM)
   int32_t split = 0;
   int32_t cg = 4;           // column tiles per scheduling group
+  // K3 (int8 digit planes on the tcgen05 tensor cores); i8_S == 0: not built
+  int32_t i8_S = 0;
+  int32_t math = TTDFT_MATH_AUTO;
+  const int8_t* Hd = nullptr;     // [nblocks][S][b][128]
+  const int32_t* eH = nullptr;    // [M]
+  const double* hdiag = nullptr;  // [M]
+  CUtensorMap tmHd;
+  int32_t nsm = 148;
 };
 
 namespace {
@@ -390,6 +435,85 @@ ttdft_status launch_step(const ttdft_h_s* h, double alpha, double gamma, double 
   return TTDFT_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// K3 path: the same step through int8 digit planes on the tcgen05 tensor cores
+// ------------------------------------------------------------------------------------------------
+struct I8Work {            // views into the caller's scratch (ttdft_step_work_bytes)
+  int8_t* D = nullptr;     // digit planes of the source iterate: [S][w][nb*128]
+  uint32_t* cmax[2] = {nullptr, nullptr};   // column maxima (upper words): source / next iterate
+};
+size_t i8_work_bytes(const ttdft_h_s* h, int64_t w) {
+  return align_up((size_t)I8_S * (size_t)w * (size_t)h->nb * 128, 1024) + 2 * align_up((size_t)w * 4, 1024);
+}
+I8Work carve_i8_work(const ttdft_h_s* h, void* base, int64_t w) {
+  I8Work k;
+  uint8_t* p = reinterpret_cast<uint8_t*>(base);
+  k.D = reinterpret_cast<int8_t*>(p);
+  p += align_up((size_t)I8_S * (size_t)w * (size_t)h->nb * 128, 1024);
+  k.cmax[0] = reinterpret_cast<uint32_t*>(p);
+  k.cmax[1] = reinterpret_cast<uint32_t*>(p + align_up((size_t)w * 4, 1024));
+  return k;
+}
+bool want_i8(const ttdft_h_s* h) {
+  return h->i8_S > 0 && (h->math == TTDFT_MATH_I8 || (h->math == TTDFT_MATH_AUTO && h->b >= 64));
+}
+
+// src: index of the cmax array that holds (have_src_max) or will hold the maxima of X; the other one
+// receives the maxima of O if want_out_max.
+ttdft_status launch_step_i8(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
+                            const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, const I8Work& w, int src,
+                            bool have_src_max, bool want_out_max, cudaStream_t st) {
+  constexpr int S = I8_S;
+  if (h->M == 0) return TTDFT_OK;
+  const int64_t Mk = h->nb * 128;
+  const unsigned nct = (unsigned)((ncols + ttdft::K3_NT - 1) / ttdft::K3_NT);
+  uint32_t* cmS = w.cmax[src];
+  uint32_t* cmO = want_out_max ? w.cmax[src ^ 1] : nullptr;
+  if (!have_src_max) {
+    CUDA_TRY(cudaMemsetAsync(cmS, 0, (size_t)ncols * 4, st));
+    dim3 g(nct, (unsigned)((h->M + 2047) / 2048));
+    ttdft::colmax_kernel<<<g, 256, 0, st>>>(X, ldx, h->M, ncols, cmS);
+    CUDA_TRY(cudaGetLastError());
+    g_launches.fetch_add(1);
+  }
+  {
+    static bool attr_set = false;
+    const int smem = S * 64 * 33 * 4;
+    if (!attr_set) {
+      CUDA_TRY(cudaFuncSetAttribute(ttdft::y_digits_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+      attr_set = true;
+    }
+    dim3 g((unsigned)h->nb, nct);
+    ttdft::y_digits_kernel<S><<<g, 256, smem, st>>>(X, ldx, h->b, ncols, cmS, w.D, Mk, cmO);
+    CUDA_TRY(cudaGetLastError());
+    g_launches.fetch_add(1);
+  }
+  CUtensorMap tmYd;
+  ttdft_status s = make_map_yd(&tmYd, w.D, (uint64_t)Mk, (uint64_t)ncols, (uint32_t)S);
+  if (s != TTDFT_OK) return s;
+  ttdft::K3Params p;
+  p.brow_ptr = h->row_ptr; p.bcol = h->col;
+  p.nb = (int32_t)h->nb; p.b = h->b; p.nct = (int32_t)nct; p.cg = h->cg;
+  p.ncols = ncols;
+  p.alpha = alpha; p.gamma = gamma; p.beta = beta;
+  p.S = X; p.lds = ldx; p.Z = Z ? Z : X; p.ldz = Z ? ldz : ldx; p.O = O; p.ldo = ldo;
+  p.eH = h->eH; p.hdiag = h->hdiag; p.cmaxS = cmS; p.cmaxO = cmO;
+  auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
+  p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
+  using C3 = ttdft::K3Cfg<S>;
+  static bool attr3_set = false;
+  if (!attr3_set) {
+    CUDA_TRY(cudaFuncSetAttribute(ttdft::bsr_i8_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, C3::TOTAL));
+    attr3_set = true;
+  }
+  const int64_t tiles = (int64_t)h->nb * nct;
+  const unsigned grid = (unsigned)std::min<int64_t>(tiles, h->nsm);
+  ttdft::bsr_i8_kernel<S><<<grid, ttdft::K3_THREADS, C3::TOTAL, st>>>(h->tmHd, tmYd, p);
+  CUDA_TRY(cudaGetLastError());
+  g_launches.fetch_add(1);
+  return TTDFT_OK;
+}
+
 ttdft_status launch_copy2d(const double* src, int64_t lds, double* dst, int64_t ldd, int64_t rows, int64_t cols,
                            cudaStream_t st) {
   if (rows == 0 || cols == 0) return TTDFT_OK;
@@ -419,7 +543,7 @@ int64_t default_panel(int64_t ncols) { return ncols < 4096 ? ncols : 4096; }
 // panel (ldy), W: scratch (ldw).  inplace: Xp == Yp.
 ttdft_status filter_panel(const ttdft_h_s* h, const double* Xp, int64_t ldx, double* Yp, int64_t ldy, double* W,
                           int64_t ldw, int64_t wc, int32_t m, double c, const double* alpha, const double* beta,
-                          bool inplace, cudaStream_t st) {
+                          bool inplace, cudaStream_t st, const I8Work* i8 = nullptr) {
   if (m == 0) {
     if (!inplace) return launch_copy2d(Xp, ldx, Yp, ldy, h->M, wc, st);
     return TTDFT_OK;
@@ -440,7 +564,11 @@ ttdft_status filter_panel(const ttdft_h_s* h, const double* Xp, int64_t ldx, dou
     if (k == 2) { Z = Xp; ldz = ldx; }
     else if (k > 2) { Z = dest(k - 2, &ldz); }
     const double al = alpha[k - 1], be = (k == 1) ? 0.0 : beta[k - 1];
-    ttdft_status s = launch_step(h, al, -al * c, be, S, lds, Z, ldz, O, ldo, wc, st);
+    ttdft_status s;
+    if (i8)   // column maxima of iterate k-1 live in cmax[(k-1)&1]; the epilogue leaves those of iterate k in the other
+      s = launch_step_i8(h, al, -al * c, be, S, lds, Z, ldz, O, ldo, wc, *i8, (k - 1) & 1, k > 1, k < m, st);
+    else
+      s = launch_step(h, al, -al * c, be, S, lds, Z, ldz, O, ldo, wc, st);
     if (s != TTDFT_OK) return s;
   }
   if (inplace && (m % 2 == 1)) return launch_copy2d(W, ldw, Yp, ldy, h->M, wc, st);
@@ -511,8 +639,9 @@ static ttdft_status csr2bsr_counts(const ttdft_h_desc* d, int32_t b, int32_t* de
   return TTDFT_OK;
 }
 
-ttdft_status ttdft_h_storage_bytes(const ttdft_h_desc* d, size_t* bytes) {
-  if (!bytes) return fail(TTDFT_ERR_INVALID_ARG, "bytes is NULL");
+// base: the fp64 format (K1 / K2); i8: the digit planes of K3 that follow it (0 if not built)
+static ttdft_status storage_bytes_impl(const ttdft_h_desc* d, size_t* bytes, size_t* i8) {
+  *i8 = 0;
   int64_t nidx, nstored;
   ttdft_status s = desc_counts(d, &nidx, &nstored);
   if (s != TTDFT_OK) return s;
@@ -534,6 +663,7 @@ ttdft_status ttdft_h_storage_bytes(const ttdft_h_desc* d, size_t* bytes) {
     for (int32_t c : hc) nblocks += c;
     *bytes = align_up((size_t)(nb + 1) * 4, 1024) + align_up((size_t)nb * 4, 1024) + align_up((size_t)nblocks * 4, 1024) +
              align_up((size_t)nblocks * hint_b * hint_b * 8, 1024);
+    if (!(d->flags & TTDFT_NO_I8) && nblocks > 0) *i8 = i8_storage_bytes(nblocks, hint_b, d->M);
     return TTDFT_OK;
   }
   const size_t per = (d->fmt == TTDFT_FMT_BSR) ? (size_t)d->block * d->block : 1;
@@ -541,6 +671,17 @@ ttdft_status ttdft_h_storage_bytes(const ttdft_h_desc* d, size_t* bytes) {
   const size_t nidxarr = (d->fmt == TTDFT_FMT_BSR) ? 2 : 1;
   *bytes = align_up((size_t)(nidx + 1) * 4, 1024) + nidxarr * align_up((size_t)nstored * 4, 1024) +
            align_up((size_t)nstored * per * 8, 1024) + 1024;
+  if (d->fmt == TTDFT_FMT_BSR && k1_block_ok(d->block) && !(d->flags & (TTDFT_FORCE_GENERIC | TTDFT_NO_I8)) && nstored > 0)
+    *i8 = i8_storage_bytes(nstored, d->block, d->M);
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_h_storage_bytes(const ttdft_h_desc* d, size_t* bytes) {
+  if (!bytes) return fail(TTDFT_ERR_INVALID_ARG, "bytes is NULL");
+  size_t base = 0, i8 = 0;
+  ttdft_status s = storage_bytes_impl(d, &base, &i8);
+  if (s != TTDFT_OK) return s;
+  *bytes = base + i8;
   return TTDFT_OK;
 }
 
@@ -550,10 +691,11 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
   int64_t nidx, nstored;
   ttdft_status s = desc_counts(d, &nidx, &nstored);
   if (s != TTDFT_OK) return s;
-  size_t need;
-  s = ttdft_h_storage_bytes(d, &need);
+  size_t need, need_i8;
+  s = storage_bytes_impl(d, &need, &need_i8);   // need: the fp64 format; the digit planes follow it
   if (s != TTDFT_OK) return s;
-  if (bytes < need) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "dev_storage has %zu bytes, %zu needed", bytes, need);
+  if (bytes < need + need_i8)
+    return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "dev_storage has %zu bytes, %zu needed", bytes, need + need_i8);
   if (need > 0 && (!dev_storage || (reinterpret_cast<uintptr_t>(dev_storage) & 1023)))
     return fail(TTDFT_ERR_INVALID_ARG, "dev_storage must be a 1024-byte aligned device pointer");
   int32_t hint_b;
@@ -593,7 +735,7 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
   ttdft_h_s* h = new (std::nothrow) ttdft_h_s;
   if (!h) return fail(TTDFT_ERR_CUDA, "out of host memory");
   h->M = d->M;
-  h->storage_bytes = need;
+  h->storage_bytes = need + need_i8;
   uint8_t* base = reinterpret_cast<uint8_t*>(dev_storage);
 
   if (hint_b) {
@@ -653,6 +795,27 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     h->cg = env_int("TTDFT_K1_CG", 4);
     if (h->cg < 1) h->cg = 1;
   }
+  if (h->kernel == 1 && need_i8 > 0) {
+    // ---- int8 digit planes of every tile (K3): row exponents + diagonal, then the planes ----
+    uint8_t* q = base + need;
+    int8_t* Hd = reinterpret_cast<int8_t*>(q);
+    q += align_up((size_t)h->nblocks * I8_S * h->b * 128, 1024);
+    int32_t* eH = reinterpret_cast<int32_t*>(q);
+    q += align_up((size_t)h->M * 4, 1024);
+    double* hdiag = reinterpret_cast<double*>(q);
+    ttdft::h_rowscale_kernel<<<(unsigned)h->nb, 256, 0, st>>>(h->b, h->row_ptr, h->col, h->val, eH, hdiag);
+    ttdft::h_digits_kernel<I8_S><<<(unsigned)h->nb, 256, 0, st>>>(h->b, h->row_ptr, h->col, h->val, eH, Hd);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "H digit planes: %s", cudaGetErrorString(e)); }
+    g_launches.fetch_add(2);
+    s = make_map_hd(&h->tmHd, Hd, (uint64_t)h->nblocks * I8_S * h->b, (uint32_t)h->b);
+    if (s != TTDFT_OK) { delete h; return s; }
+    h->i8_S = I8_S; h->Hd = Hd; h->eH = eH; h->hdiag = hdiag;
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0)
+      h->nsm = nsm;
+    h->math = env_int("TTDFT_MATH", TTDFT_MATH_AUTO);
+  }
   *out = h;
   return TTDFT_OK;
 }
@@ -665,6 +828,18 @@ ttdft_status ttdft_h_info(ttdft_h_t h, ttdft_h_info_t* info) {
   info->nblocks = h->bsr ? h->nblocks : 0;
   info->nnz_stored = h->bsr ? h->nblocks * (int64_t)h->b * h->b : h->nblocks;
   info->storage_bytes = h->storage_bytes;
+  info->i8_planes = h->i8_S;
+  info->math = want_i8(h) ? TTDFT_MATH_I8 : TTDFT_MATH_FP64;
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_h_set_math_mode(ttdft_h_t h, int32_t mode) {
+  if (!h) return fail(TTDFT_ERR_INVALID_ARG, "handle is NULL");
+  if (mode != TTDFT_MATH_AUTO && mode != TTDFT_MATH_FP64 && mode != TTDFT_MATH_I8)
+    return fail(TTDFT_ERR_INVALID_ARG, "unknown math mode %d", mode);
+  if (mode == TTDFT_MATH_I8 && h->i8_S == 0)
+    return fail(TTDFT_ERR_UNSUPPORTED, "this handle was built without int8 digit planes");
+  h->math = mode;
   return TTDFT_OK;
 }
 
@@ -706,6 +881,51 @@ ttdft_status ttdft_cheb_step(ttdft_h_t h, double alpha, double c, double beta, c
   return launch_step(h, alpha, -alpha * c, be, Yk, ldk, Ykm1, ldm, Yout, ldo, ncols, (cudaStream_t)stream);
 }
 
+ttdft_status ttdft_step_work_bytes(ttdft_h_t h, int64_t ncols, size_t* bytes) {
+  if (!h || !bytes) return fail(TTDFT_ERR_INVALID_ARG, "NULL argument");
+  if (ncols < 1) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1");
+  *bytes = want_i8(h) ? i8_work_bytes(h, ncols) : 0;
+  return TTDFT_OK;
+}
+
+// one step with scratch: the int8 tensor-core kernel if the handle's math mode selects it
+static ttdft_status step_ws(ttdft_h_t h, double alpha, double gamma, double beta, const double* X, int64_t ldx, const double* Z,
+                            int64_t ldz, double* O, int64_t ldo, int64_t ncols, void* work, size_t work_bytes, cudaStream_t st) {
+  if (!want_i8(h) || alpha == 0.0 || h->M == 0) return launch_step(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+  const size_t need = i8_work_bytes(h, ncols);
+  if (work_bytes < need) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, need);
+  if (!work || (reinterpret_cast<uintptr_t>(work) & 15)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 16-byte aligned device pointer");
+  const I8Work k3 = carve_i8_work(h, work, ncols);
+  return launch_step_i8(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, k3, 0, false, false, st);
+}
+
+ttdft_status ttdft_spmm_ws(ttdft_h_t h, double alpha, const double* X, int64_t ldx, double beta, double* Y, int64_t ldy,
+                           int64_t ncols, void* work, size_t work_bytes, void* stream) {
+  if (!h) return fail(TTDFT_ERR_INVALID_ARG, "handle is NULL");
+  if (ncols < 1) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1");
+  ttdft_status s;
+  if ((s = check_mat("X", X, ldx, ncols)) != TTDFT_OK) return s;
+  if ((s = check_mat("Y", Y, ldy, ncols)) != TTDFT_OK) return s;
+  if (overlaps(X, ldx, Y, ldy, h->M, ncols)) return fail(TTDFT_ERR_INVALID_ARG, "X overlaps Y");
+  return step_ws(h, alpha, 0.0, beta, X, ldx, Y, ldy, Y, ldy, ncols, work, work_bytes, (cudaStream_t)stream);
+}
+
+ttdft_status ttdft_cheb_step_ws(ttdft_h_t h, double alpha, double c, double beta, const double* Yk, int64_t ldk,
+                                const double* Ykm1, int64_t ldm, double* Yout, int64_t ldo, int64_t ncols, void* work,
+                                size_t work_bytes, void* stream) {
+  if (!h) return fail(TTDFT_ERR_INVALID_ARG, "handle is NULL");
+  if (ncols < 1) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1");
+  ttdft_status s;
+  if ((s = check_mat("Yk", Yk, ldk, ncols)) != TTDFT_OK) return s;
+  if ((s = check_mat("Yout", Yout, ldo, ncols)) != TTDFT_OK) return s;
+  if (Ykm1 && (s = check_mat("Ykm1", Ykm1, ldm, ncols)) != TTDFT_OK) return s;
+  if (overlaps(Yk, ldk, Yout, ldo, h->M, ncols)) return fail(TTDFT_ERR_INVALID_ARG, "Yk overlaps Yout");
+  if (Ykm1 && !(Ykm1 == Yout && ldm == ldo) && overlaps(Ykm1, ldm, Yout, ldo, h->M, ncols))
+    return fail(TTDFT_ERR_INVALID_ARG, "Ykm1 partially overlaps Yout");
+  const double be = Ykm1 ? beta : 0.0;
+  return step_ws(h, alpha, -alpha * c, be, Yk, ldk, Ykm1, ldm, Yout, ldo, ncols, work, work_bytes, (cudaStream_t)stream);
+}
+
 ttdft_status ttdft_cheb_scalars(int32_t m, double a, double b, double a0, double* c_out, double* alpha, double* beta) {
   ttdft_status s = check_scalars(m, a, b, a0);
   if (s != TTDFT_OK) return s;
@@ -732,6 +952,7 @@ ttdft_status ttdft_cheb_filter_work_bytes(ttdft_h_t h, int64_t ncols, int64_t pa
   int64_t w = panel_cols ? std::min(panel_cols, ncols) : default_panel(ncols);
   w += (w & 1);   // even leading dimension keeps the scratch panel TMA / 128-bit friendly
   *bytes = (size_t)h->M * (size_t)w * 8;
+  if (want_i8(h)) *bytes = align_up(*bytes, 1024) + i8_work_bytes(h, w);   // + digit planes of one iterate
   return TTDFT_OK;
 }
 
@@ -749,7 +970,8 @@ ttdft_status ttdft_cheb_filter(ttdft_h_t h, const double* X, int64_t ldx, double
   if (!inplace && overlaps(X, ldx, Y, ldy, h->M, ncols)) return fail(TTDFT_ERR_INVALID_ARG, "X partially overlaps Y");
   size_t need;
   if ((s = ttdft_cheb_filter_work_bytes(h, ncols, panel_cols, &need)) != TTDFT_OK) return s;
-  const bool need_work = (m >= 2) || (m == 1 && inplace);
+  const bool i8 = want_i8(h) && m >= 1 && h->M > 0;
+  const bool need_work = (m >= 2) || (m == 1 && inplace) || i8;
   if (need_work) {
     if (work_bytes < need) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, need);
     if (!work || (reinterpret_cast<uintptr_t>(work) & 15)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 16-byte aligned device pointer");
@@ -759,10 +981,12 @@ ttdft_status ttdft_cheb_filter(ttdft_h_t h, const double* X, int64_t ldx, double
   if ((s = ttdft_cheb_scalars(m, a, b, a0, &c, alpha.data(), beta.data())) != TTDFT_OK) return s;
   const int64_t w = panel_cols ? std::min(panel_cols, ncols) : default_panel(ncols);
   const int64_t ldw = w + (w & 1);
+  I8Work k3;
+  if (i8) k3 = carve_i8_work(h, reinterpret_cast<uint8_t*>(work) + align_up((size_t)h->M * (size_t)ldw * 8, 1024), ldw);
   for (int64_t c0 = 0; c0 < ncols; c0 += w) {
     const int64_t wc = std::min(w, ncols - c0);
     s = filter_panel(h, X + c0, ldx, Y + c0, ldy, reinterpret_cast<double*>(work), ldw, wc, m, c, alpha.data(), beta.data(),
-                     inplace, (cudaStream_t)stream);
+                     inplace, (cudaStream_t)stream, i8 ? &k3 : nullptr);
     if (s != TTDFT_OK) return s;
   }
   return TTDFT_OK;
@@ -774,6 +998,7 @@ ttdft_status ttdft_cheb_filter_host_work_bytes(ttdft_h_t h, int64_t ncols, int64
   int64_t w = panel_cols ? std::min(panel_cols, ncols) : std::min<int64_t>(ncols, 1024);
   w += (w & 1);
   *bytes = 5 * align_up((size_t)h->M * (size_t)w * 8, 1024);   // 2 x (X panel, Y panel) + scratch
+  if (want_i8(h)) *bytes += i8_work_bytes(h, w);
   return TTDFT_OK;
 }
 
@@ -800,6 +1025,9 @@ ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* Xh, int64_t ldx, 
   double* dX[2] = {reinterpret_cast<double*>(base), reinterpret_cast<double*>(base + pbytes)};
   double* dY[2] = {reinterpret_cast<double*>(base + 2 * pbytes), reinterpret_cast<double*>(base + 3 * pbytes)};
   double* dW = reinterpret_cast<double*>(base + 4 * pbytes);
+  const bool i8 = want_i8(h) && m >= 1 && h->M > 0;
+  I8Work k3;
+  if (i8) k3 = carve_i8_work(h, base + 5 * pbytes, ldw);
 
   cudaStream_t sc = (cudaStream_t)stream, sin = nullptr, sout = nullptr;
   cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr}, ev_start = nullptr;
@@ -848,7 +1076,7 @@ ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* Xh, int64_t ldx, 
     // compute once the panel has arrived and dY[buf]'s previous contents have left
     HOST_TRY(cudaStreamWaitEvent(sc, ev_in[buf], 0));
     if (ip >= 2) HOST_TRY(cudaStreamWaitEvent(sc, ev_out[buf], 0));
-    s = filter_panel(h, dX[buf], ldw, dY[buf], ldw, dW, ldw, wc, m, c, alpha.data(), beta.data(), false, sc);
+    s = filter_panel(h, dX[buf], ldw, dY[buf], ldw, dW, ldw, wc, m, c, alpha.data(), beta.data(), false, sc, i8 ? &k3 : nullptr);
     if (s != TTDFT_OK) { cudaDeviceSynchronize(); cleanup(); return s; }
     HOST_TRY(cudaEventRecord(ev_comp[buf], sc));
     // device -> host on the output stream

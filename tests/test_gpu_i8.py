@@ -1,0 +1,176 @@
+"""GPU parity of the int8 digit-plane path (kernel K3, TTDFT_MATH_I8) against the CPU oracle.
+
+Same tolerances as the fp64 path (north_star): <= 1e-12 relative Frobenius per SpMM / fused step,
+<= 1e-10 after a filter.  K3 splits every operand exactly into 6 balanced base-256 digits below its
+row / column maximum and accumulates in exact integers, so the measured error
+is expected around 1e-14; ACC_SPMM pins that, so that a lost digit plane or level (>= 2^-40) fails."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from util import bounds_for, relerr, small_problem, worst_col_relerr
+
+pytestmark = pytest.mark.gpu
+
+TOL_SPMM = 1e-12
+TOL_FILTER = 1e-10
+ACC_SPMM = 2e-13      # what 47-bit operands must deliver on these inputs
+
+
+@pytest.fixture(scope="module")
+def tt():
+    import torch
+    import paper_2110_15853_b200 as t
+    assert torch.cuda.is_available()
+    return t
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def build_i8(t, H, flags=0):
+    Hd = t.h_build_bsr(H.M, H.b, dev(H.row_ptr), dev(H.col_idx), dev(H.values), flags=flags)
+    assert Hd.info()["i8_planes"] == 6
+    Hd.set_math_mode(t.MATH_I8)
+    assert Hd.info()["math"] == t.MATH_I8
+    return Hd
+
+
+@pytest.mark.parametrize("N,ld", [(32, 32), (33, 40), (1, 2), (64, 64), (130, 130), (257, 300)])
+def test_spmm_ws_tiny(tt, N, ld):
+    import torch
+    H, C, (rp, col, val), _ = small_problem(4, 32, 0.0, 1001)
+    Hd = build_i8(tt, H, flags=tt.CHECK_SORTED | tt.CHECK_SYMMETRY)
+    assert tt.step_work_bytes(Hd, N) > 0
+    X = synth.dense_normal(H.M, N, 11)
+    Y0 = synth.dense_normal(H.M, N, 12)
+    Xd = torch.zeros(H.M, ld, dtype=torch.float64, device="cuda")
+    Xd[:, :N] = dev(X)
+    Yd = torch.full((H.M, ld), float("nan"), dtype=torch.float64, device="cuda")
+    tt.spmm(Hd, 1.0, Xd[:, :N], 0.0, Yd[:, :N], use_work=True)      # beta = 0 must not read Y
+    ref = oracle.spmm(rp, col, val, 1.0, X)
+    got = Yd[:, :N].cpu().numpy()
+    assert relerr(got, ref) <= ACC_SPMM
+    assert worst_col_relerr(got, ref) <= 10 * ACC_SPMM
+    if ld > N:
+        assert torch.isnan(Yd[:, N:]).all()                           # nothing written outside the view
+    Yd[:, :N] = dev(Y0)
+    tt.spmm(Hd, -0.75, Xd[:, :N], 2.5, Yd[:, :N], use_work=True)
+    ref = oracle.spmm(rp, col, val, -0.75, X, 2.5, Y0.copy())
+    assert relerr(Yd[:, :N].cpu().numpy(), ref) <= TOL_SPMM
+
+
+@pytest.mark.parametrize("N", [32, 50])
+def test_cheb_step_ws_tiny(tt, N):
+    import torch
+    H, C, (rp, col, val), _ = small_problem(4, 32, 0.0, 1001)
+    Hd = build_i8(tt, H)
+    Yk = synth.dense_normal(H.M, N, 21)
+    Ykm1 = synth.dense_normal(H.M, N, 22)
+    alpha, c, beta = 0.173, 9.5, -0.31
+    ref = oracle.cheb_step(rp, col, val, alpha, c, beta, Yk, Ykm1)
+    out = torch.empty(H.M, N, dtype=torch.float64, device="cuda")
+    tt.cheb_step(Hd, alpha, c, beta, dev(Yk), dev(Ykm1), out, use_work=True)
+    assert relerr(out.cpu().numpy(), ref) <= TOL_SPMM
+    # in place over Y_{k-1}
+    z = dev(Ykm1)
+    tt.cheb_step(Hd, alpha, c, beta, dev(Yk), z, z, use_work=True)
+    assert relerr(z.cpu().numpy(), ref) <= TOL_SPMM
+    # first step: no beta term
+    ref1 = oracle.cheb_step(rp, col, val, alpha, c, 0.0, Yk, None)
+    tt.cheb_step(Hd, alpha, c, 123.0, dev(Yk), None, out, use_work=True)
+    assert relerr(out.cpu().numpy(), ref1) <= TOL_SPMM
+
+
+@pytest.mark.parametrize("m", [1, 2, 3, 10, 11])
+@pytest.mark.parametrize("inplace", [False, True])
+def test_filter_tiny_full_i8(tt, m, inplace):
+    import torch
+    cfg = synth.CONFIGS["tiny"]
+    H, C, (rp, col, val), (a0, b) = small_problem(cfg.G, cfg.b, cfg.z, cfg.seed)
+    a, b, a0 = bounds_for(a0, b, cfg.N, H.M)
+    Hd = build_i8(tt, H)
+    X = synth.dense_normal(H.M, cfg.N, cfg.seed)
+    ref = oracle.cheb_filter(rp, col, val, X, m, a, b, a0)
+    Xd = dev(X)
+    Yd = Xd if inplace else torch.empty_like(Xd)
+    tt.cheb_filter(Hd, Xd, Yd, m, a, b, a0)
+    got = Yd.cpu().numpy()
+    assert relerr(got, ref) <= TOL_FILTER
+    assert worst_col_relerr(got, ref) <= 10 * TOL_FILTER
+    if not inplace:
+        assert np.array_equal(Xd.cpu().numpy(), X)
+
+
+@pytest.mark.parametrize("N,panel", [(100, 48), (100, 100), (70, 32), (33, 16), (37, 7)])
+def test_filter_panels_and_ragged_i8(tt, N, panel):
+    """Panel width not dividing N, ragged N, odd panel width (unaligned views -> scalar epilogue)."""
+    import torch
+    H, C, (rp, col, val), (a0, b) = small_problem(4, 32, 0.0, 1001)
+    a, b, a0 = bounds_for(a0, b, 32, H.M, wide=True)
+    Hd = build_i8(tt, H)
+    X = synth.dense_normal(H.M, N, 31)
+    ref = oracle.cheb_filter(rp, col, val, X, 7, a, b, a0)
+    Y = torch.empty(H.M, N, dtype=torch.float64, device="cuda")
+    tt.cheb_filter(Hd, dev(X), Y, 7, a, b, a0, panel_cols=panel)
+    assert relerr(Y.cpu().numpy(), ref) <= TOL_FILTER
+    assert worst_col_relerr(Y.cpu().numpy(), ref) <= 10 * TOL_FILTER
+
+
+@pytest.mark.parametrize("G,b,z,N", [(3, 64, 0.3, 200), (2, 96, 0.4, 130), (3, 128, 0.4, 300)])
+def test_other_block_sizes_i8(tt, G, b, z, N):
+    import torch
+    H, C, (rp, col, val), (a0, bb) = small_problem(G, b, z, 2000 + b)
+    a, bb, a0 = bounds_for(a0, bb, N, H.M)
+    Hd = build_i8(tt, H)
+    X = synth.dense_normal(H.M, N, 51)
+    Y = torch.empty(H.M, N, dtype=torch.float64, device="cuda")
+    tt.spmm(Hd, 1.0, dev(X), 0.0, Y, use_work=True)
+    assert relerr(Y.cpu().numpy(), oracle.spmm(rp, col, val, 1.0, X)) <= ACC_SPMM
+    m = 20
+    ref = oracle.cheb_filter(C.row_ptr, C.col_idx, C.values, X, m, a, bb, a0)
+    tt.cheb_filter(Hd, dev(X), Y, m, a, bb, a0, panel_cols=128)
+    assert relerr(Y.cpu().numpy(), ref) <= TOL_FILTER
+    assert worst_col_relerr(Y.cpu().numpy(), ref) <= 10 * TOL_FILTER
+    # the fp64 tensor-core path on the same handle agrees with the same oracle
+    Hd.set_math_mode(tt.MATH_FP64)
+    Y2 = torch.empty_like(Y)
+    tt.cheb_filter(Hd, dev(X), Y2, m, a, bb, a0, panel_cols=128)
+    assert relerr(Y2.cpu().numpy(), ref) <= TOL_FILTER
+
+
+def test_column_dynamic_range_and_zero_columns(tt):
+    """Per-column scaling: columns 60 orders of magnitude apart, an all-zero column, a column with one
+    huge entry -- every column keeps its own relative accuracy."""
+    import torch
+    H, C, (rp, col, val), _ = small_problem(3, 64, 0.3, 2064)
+    Hd = build_i8(tt, H)
+    N = 70
+    X = synth.dense_normal(H.M, N, 61)
+    scale = 10.0 ** np.linspace(-30, 30, N)
+    X = X * scale[None, :]
+    X[:, 5] = 0.0
+    X[7, 9] = 1e6 * np.abs(X[:, 9]).max()          # one dominant entry: the rest of the column loses bits
+    ref = oracle.spmm(rp, col, val, 1.0, X)
+    Y = torch.empty(H.M, N, dtype=torch.float64, device="cuda")
+    tt.spmm(Hd, 1.0, dev(X), 0.0, Y, use_work=True)
+    got = Y.cpu().numpy()
+    assert np.all(got[:, 5] == 0.0)
+    cols = [j for j in range(N) if j not in (5, 9)]
+    assert worst_col_relerr(got[:, cols], ref[:, cols]) <= 10 * ACC_SPMM
+    assert worst_col_relerr(got[:, [9]], ref[:, [9]]) <= TOL_SPMM    # still norm-wise accurate
+
+
+def test_no_i8_flag_and_mode_errors(tt):
+    H, C, _, _ = small_problem(4, 32, 0.0, 1001)
+    Hd = tt.h_build_bsr(H.M, H.b, dev(H.row_ptr), dev(H.col_idx), dev(H.values), flags=tt.NO_I8)
+    assert Hd.info()["i8_planes"] == 0 and Hd.info()["math"] == tt.MATH_FP64
+    with pytest.raises(tt.TTDFTError) as e:
+        Hd.set_math_mode(tt.MATH_I8)
+    assert e.value.status_name == "UNSUPPORTED"
+    with pytest.raises(tt.TTDFTError):
+        Hd.set_math_mode(7)
+    assert tt.step_work_bytes(Hd, 64) == 0
