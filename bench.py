@@ -35,8 +35,21 @@ import synth  # noqa: E402
 # FMA/clk/SM x 2 flop x 1.965 GHz (clocks.max.sm).  Measured on this pool: DMMA loop 37.15 TFLOP/s.
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # DRAM bytes per launch of the dominant kernel from the ncu --set full capture under profiles/
-# (dram__bytes_read.sum + dram__bytes_write.sum), keyed by workload; None = not captured.
+# (dram__bytes_read.sum + dram__bytes_write.sum), keyed by (workload, kernel); None = not captured.
 NCU_TRAFFIC_BYTES = {}
+# nominal dense tensor-core ratio int8 : bf16 on B200 (4.5 : 2.25 Pop/s, B200_PROFILING.md table)
+INT8_OVER_BF16 = 2.0
+
+
+def int8_peak_tops():
+    """Dense int8 tensor peak = measured bf16 peak (sustained: the kernel is timed inside a long step)
+    x the nominal int8:bf16 ratio; falls back to the profiling guide's 1.4 PFLOP/s sustained figure."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            d = json.load(f)
+        return INT8_OVER_BF16 * float(d["bf16_tflops_sustained"]), "of measured: MEASURED_PEAKS.json bf16_tflops_sustained x 2 (nominal int8:bf16)"
+    except Exception:
+        return INT8_OVER_BF16 * 1400.0, "of fallback: B200_PROFILING.md sustained bf16 1.4 PFLOP/s x 2 (nominal int8:bf16)"
 
 
 def load_bounds(name: str):
@@ -173,6 +186,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--panel", type=int, default=0, help="column-panel width (0 = config default)")
     ap.add_argument("--ref-cols", type=int, default=16, help="columns in the oracle sample")
+    ap.add_argument("--math", default="auto", choices=["auto", "fp64", "i8"],
+                    help="arithmetic of the block product: fp64 DMMA, int8 digit planes (fp64-accurate), auto")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -202,8 +217,10 @@ def main():
                         torch.from_numpy(H.values).to(dev))
     torch.cuda.synchronize()
     t_build = time.perf_counter() - t_build0
+    Hd.set_math_mode({"auto": tt.MATH_AUTO, "fp64": tt.MATH_FP64, "i8": tt.MATH_I8}[args.math])
     info = Hd.info()
-    assert info["kernel"] == 1, "the block-sparse TMA/DMMA kernel must be the one that runs"
+    assert info["kernel"] == 1, "a block-sparse tensor-core kernel must be the one that runs"
+    use_i8 = info["math"] == tt.MATH_I8
 
     # this rank's band of wavefunctions: columns [rank*N, (rank+1)*N) of the global block (host, pinned)
     Xh = torch.empty((cfg.M, cfg.N), dtype=torch.float64).pin_memory()
@@ -228,6 +245,9 @@ def main():
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
+    for k in tt.KERNEL_IDS:
+        tt.timing_read(k)
+    tt.timing_enable(True)       # CUDA event pairs around every library kernel, on the launching stream
     n0 = tt.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
@@ -236,6 +256,8 @@ def main():
     e1.record()
     barrier()
     launches = tt.launch_count() - n0
+    tt.timing_enable(False)
+    ktimes = {k: tt.timing_read(k) for k in tt.KERNEL_IDS}
     clocks = sampler.stop()
     t_region = e0.elapsed_time(e1) * 1e-3
     if dist is not None:
@@ -273,19 +295,41 @@ def main():
     executed = 2.0 * H.nblocks * cfg.b * cfg.b * cfg.N * cfg.m
     npanels = -(-cfg.N // (panel if panel else min(cfg.N, 4096)))
     alg_bytes = cfg.m * (npanels * 8.0 * nnz + 24.0 * cfg.M * cfg.N) - 8.0 * cfg.M * cfg.N
-    # dominant kernel: the fused step kernel; one launch = one recurrence step over one panel
-    step_launches = args.steps * cfg.m * npanels
-    t_launch = t_region / step_launches
+    # dominant kernel: the fused step kernel; one launch = one recurrence step over one panel.
+    # Its launch time comes from the library's CUDA event pairs recorded inside the timed region.
+    kname = "bsr_i8" if use_i8 else "bsr_dmma"
+    k_ms, k_n = ktimes[kname]
+    assert k_n == args.steps * cfg.m * npanels, (k_n, args.steps, cfg.m, npanels)
+    t_launch = k_ms * 1e-3 / k_n
     flops_per_launch = useful / (cfg.m * npanels)
-    achieved_tf = flops_per_launch / t_launch / 1e12
-    roof = {"bound": "alu", "achieved": achieved_tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-            "frac": achieved_tf / FP64_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
-            "kernel": "ttdft::bsr_dmma_kernel", "launch_ms": t_launch * 1e3,
-            "peak_source": "derived: 148 SM x 64 fp64 FMA/clk x 2 x 1.965 GHz (fp64 has no entry in MEASURED_PEAKS.json)",
-            "executed_tflops": executed / (cfg.m * npanels) / t_launch / 1e12,
-            "executed_frac": executed / (cfg.m * npanels) / t_launch / 1e12 / FP64_PEAK_TFLOPS,
-            "dense_tile_ceiling": useful / executed,
-            "hbm_alg_gbs": alg_bytes / t_step / 1e9}
+    fp64_equiv = {"achieved": flops_per_launch / t_launch / 1e12, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                  "frac": flops_per_launch / t_launch / 1e12 / FP64_PEAK_TFLOPS,
+                  "peak_source": "derived: 148 SM x 64 fp64 FMA/clk x 2 x 1.965 GHz (native fp64 ALU/DMMA pipe; "
+                                 "fp64 has no entry in MEASURED_PEAKS.json)",
+                  "executed_tflops": executed / (cfg.m * npanels) / t_launch / 1e12,
+                  "dense_tile_ceiling": useful / executed}
+    shares = {k: v[0] / (t_region * 1e3) for k, v in ktimes.items() if v[1]}
+    if use_i8:
+        # K3: the product runs as S(S+1)/2 exact int8 digit-plane products on the tensor pipe, so the
+        # tensor pipe bounds it.  Algorithmic ops per launch = 2 * pairs * nnz * N (non-zeros only).
+        S = info["i8_planes"]
+        pairs = S * (S + 1) // 2
+        peak, peak_src = int8_peak_tops()
+        ops_launch = 2.0 * pairs * nnz * cfg.N / npanels
+        ops_exec = 2.0 * pairs * H.nblocks * 128 * cfg.b * (-(-cfg.N // 64) * 64) / npanels
+        roof = {"bound": "tensor", "achieved": ops_launch / t_launch / 1e12, "peak": peak, "unit": "TFLOP/s",
+                "frac": ops_launch / t_launch / 1e12 / peak, "traffic": NCU_TRAFFIC_BYTES.get((args.workload, kname)),
+                "kernel": "ttdft::bsr_i8_kernel", "launch_ms": t_launch * 1e3, "peak_source": peak_src,
+                "ops": f"int8 multiply-add = 2 ops; {pairs} digit-plane products per fp64 product ({S} planes per operand)",
+                "executed_tops": ops_exec / t_launch / 1e12, "executed_frac": ops_exec / t_launch / 1e12 / peak,
+                "fp64_equivalent": fp64_equiv, "step_share": shares, "hbm_alg_gbs": alg_bytes / t_step / 1e9}
+    else:
+        roof = {"bound": "alu", "achieved": fp64_equiv["achieved"], "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": fp64_equiv["frac"], "traffic": NCU_TRAFFIC_BYTES.get((args.workload, kname)),
+                "kernel": "ttdft::bsr_dmma_kernel", "launch_ms": t_launch * 1e3, "peak_source": fp64_equiv["peak_source"],
+                "executed_tflops": fp64_equiv["executed_tflops"],
+                "executed_frac": fp64_equiv["executed_tflops"] / FP64_PEAK_TFLOPS,
+                "dense_tile_ceiling": useful / executed, "step_share": shares, "hbm_alg_gbs": alg_bytes / t_step / 1e9}
     try:
         roof["peak_measured_dmma"] = tt.probe_fp64_peak(1, 300)
     except Exception:
@@ -295,7 +339,9 @@ def main():
         "metric": "ChFSI filter useful fp64 GFLOP/s", "value": useful * world / t_step / 1e9, "unit": "GFLOP/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(cfg, nnz, H.nblocks, args),
+        "config": dict(workload_config(cfg, nnz, H.nblocks, args),
+                       math="int8 digit planes (6 x 8 bit per operand, exact int32 accumulation, fp64 in/out)" if use_i8
+                       else "fp64 tensor-core MMA"),
         "clocks": clocks, "gpu_launches": int(launches), "roofline": roof,
         "h_build_ms": t_build * 1e3,
     }

@@ -194,6 +194,16 @@ ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* X_host, int64_t l
  * runs for about `millis` ms on `stream`, synchronises, returns TFLOP/s in *tflops. */
 ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, double* tflops);
 
+/*
+ * Device timing of the library's own kernels.  While enabled, every launch of the kernels below is
+ * bracketed by a CUDA event pair on the launching stream; ttdft_timing_read waits for the events of
+ * one kernel, returns the sum of their durations and their count, and clears them.
+ *   kernel_id: 1 = block-sparse fp64 DMMA step, 2 = generic CSR/BSR step, 3 = block-sparse int8
+ *   tensor-core step, 4 = digit planes of an iterate, 5 = column maxima of a panel.
+ */
+ttdft_status ttdft_timing_enable(int32_t on);
+ttdft_status ttdft_timing_read(int32_t kernel_id, double* total_ms, int64_t* launches);
+
 /* Number of kernels this library has launched since load (all threads). */
 int64_t ttdft_launch_count(void);
 

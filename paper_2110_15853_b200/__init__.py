@@ -31,4 +31,7 @@ from .api import (  # noqa: F401
     MATH_FP64,
     MATH_I8,
     step_work_bytes,
+    timing_enable,
+    timing_read,
+    KERNEL_IDS,
 )

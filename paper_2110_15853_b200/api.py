@@ -19,6 +19,7 @@ exported_symbols = [
     "ttdft_cheb_scalars", "ttdft_cheb_filter_work_bytes", "ttdft_cheb_filter", "ttdft_cheb_filter_host_work_bytes",
     "ttdft_cheb_filter_host", "ttdft_probe_fp64_peak", "ttdft_launch_count", "ttdft_last_error",
     "ttdft_h_set_math_mode", "ttdft_step_work_bytes", "ttdft_spmm_ws", "ttdft_cheb_step_ws",
+    "ttdft_timing_enable", "ttdft_timing_read",
 ]
 
 
@@ -92,6 +93,10 @@ def _load() -> ctypes.CDLL:
                        c_int64, c_void_p, c_size_t, c_void_p]
     L.ttdft_probe_fp64_peak.restype = st
     L.ttdft_probe_fp64_peak.argtypes = [c_int32, c_int32, c_void_p, POINTER(c_double)]
+    L.ttdft_timing_enable.restype = st
+    L.ttdft_timing_enable.argtypes = [c_int32]
+    L.ttdft_timing_read.restype = st
+    L.ttdft_timing_read.argtypes = [c_int32, POINTER(c_double), POINTER(c_int64)]
     L.ttdft_launch_count.restype = c_int64
     L.ttdft_launch_count.argtypes = []
     L.ttdft_last_error.restype = c_char_p
@@ -102,6 +107,21 @@ def _load() -> ctypes.CDLL:
 
 def last_error() -> str:
     return _load().ttdft_last_error().decode()
+
+
+KERNEL_IDS = {"bsr_dmma": 1, "generic": 2, "bsr_i8": 3, "y_digits": 4, "colmax": 5}
+
+
+def timing_enable(on: bool = True):
+    """ttdft_timing_enable: bracket the library's kernel launches with CUDA events on their stream."""
+    _check(_load().ttdft_timing_enable(1 if on else 0))
+
+
+def timing_read(kernel: str):
+    """(total milliseconds, launches) of one kernel since the last read (ttdft_timing_read)."""
+    ms, n = c_double(), c_int64()
+    _check(_load().ttdft_timing_read(KERNEL_IDS[kernel], byref(ms), byref(n)))
+    return ms.value, int(n.value)
 
 
 def launch_count() -> int:

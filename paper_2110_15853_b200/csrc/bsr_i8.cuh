@@ -94,6 +94,14 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
       : "r"(taddr));
 }
 
+// one lane of the (converged) calling warp; lets ptxas feed the uniform-register operands of
+// UTMALDG / UTCIMMA from that lane directly instead of through a broadcast loop
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}\n" : "=r"(pred));
+  return pred != 0;
+}
+
 // work item t -> (block row I, column tile ct): column-tile groups outermost, block rows, tile fastest
 __device__ __forceinline__ void k3_decode(const K3Params& prm, int64_t t, int32_t& I, int32_t& ct) {
   const int64_t per_group = (int64_t)prm.nb * prm.cg;
@@ -150,7 +158,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
 
   if (warp == 0) {
     // ===================================== TMA producer =====================================
-    if (lane == 0) {
+    if (elect_one()) {
       asm volatile("prefetch.tensormap [%0];" ::"l"(&tmHd) : "memory");
       asm volatile("prefetch.tensormap [%0];" ::"l"(&tmYd) : "memory");
       int yb = 0, hs = 0;
@@ -178,10 +186,12 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
     }
   } else if (warp == 1) {
     // ====================================== MMA issuer ======================================
-    if (lane == 0) {
+    if (elect_one()) {
       int yb = 0, hs = 0;
       uint32_t yph = 0, hph = 0, aph = 0;
-      const uint32_t ybase = smem_u32(ybuf), hbase = smem_u32(hring);
+      // descriptors differ only in the 14-bit start-address field of the low word
+      const uint64_t dbase = umma_desc_sw128(0);
+      const uint32_t ylo0 = (smem_u32(ybuf) & 0x3ffffu) >> 4, hlo0 = (smem_u32(hring) & 0x3ffffu) >> 4;
       for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
         int32_t I, ct;
         k3_decode(prm, t, I, ct);
@@ -191,19 +201,23 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         asm volatile("tcgen05.fence::after_thread_sync;");
         for (int32_t j = 0; j < nJ; ++j) {
           mbar_wait(&yfull[yb], yph);
-          const uint32_t ya = ybase + yb * C::YBUF;
-#pragma unroll 1
+          const uint32_t ylo = ylo0 + (uint32_t)yb * (C::YBUF >> 4);
+#pragma unroll
           for (int p = 0; p < S; ++p) {
             mbar_wait(&hfull[hs], hph);
             asm volatile("tcgen05.fence::after_thread_sync;");
-            const uint32_t ha = hbase + hs * C::HSLOT;
-            const int ntot = (S - p) * K3_NT;    // Y planes 0..S-1-p side by side -> levels p..S-1
-            for (int kk = 0; kk < ksteps; ++kk) {
-              const uint64_t da = umma_desc_sw128(ha + kk * 32);
-              const uint32_t acc = (j | kk | p) ? 1u : 0u;
-              for (int n0 = 0; n0 < ntot; n0 += 256) {
-                const int n = min(256, ntot - n0);
-                umma_i8(tmem_base + (uint32_t)(p * K3_NT + n0), da, umma_desc_sw128(ya + n0 * 128 + kk * 32), umma_idesc_i8(n), acc);
+            const uint32_t hlo = hlo0 + (uint32_t)hs * (C::HSLOT >> 4);
+            const int ntot = (S - p) * K3_NT;       // Y planes 0..S-1-p side by side -> levels p..S-1
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {
+              if (kk < ksteps) {
+                const uint64_t da = dbase | (uint64_t)(hlo + kk * 2);
+                const uint32_t acc = (p > 0 || kk > 0) ? 1u : (j > 0 ? 1u : 0u);
+#pragma unroll
+                for (int n0 = 0; n0 < ntot; n0 += 256) {
+                  const int n = (ntot - n0) < 256 ? (ntot - n0) : 256;
+                  umma_i8(tmem_base + (uint32_t)(p * K3_NT + n0), da, dbase | (uint64_t)(ylo + n0 * 8 + kk * 2), umma_idesc_i8(n), acc);
+                }
               }
             }
             umma_commit(&hempty[hs]);            // slot free once these MMAs have read it

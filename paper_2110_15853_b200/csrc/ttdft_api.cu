@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -23,6 +24,37 @@ namespace {
 
 thread_local std::string g_err;
 std::atomic<int64_t> g_launches{0};
+
+// ---- optional per-kernel device timing (ttdft_timing_*): CUDA events on the launching stream ----
+constexpr int NKID = 6;   // 1 = K1 bsr_dmma, 2 = K2 generic, 3 = K3 bsr_i8, 4 = y_digits, 5 = colmax
+struct KernelTimer {
+  std::atomic<int> on{0};
+  std::mutex mu;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[NKID];
+  std::vector<cudaEvent_t> pool;
+  cudaEvent_t get() {
+    if (!pool.empty()) { cudaEvent_t e = pool.back(); pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+  }
+};
+KernelTimer g_timer;
+struct TimedLaunch {       // records an event pair around one launch while timing is enabled
+  int kid; cudaStream_t st; cudaEvent_t e0 = nullptr, e1 = nullptr;
+  TimedLaunch(int kid_, cudaStream_t st_) : kid(kid_), st(st_) {
+    if (!g_timer.on.load(std::memory_order_relaxed)) return;
+    std::lock_guard<std::mutex> lk(g_timer.mu);
+    e0 = g_timer.get(); e1 = g_timer.get();
+    if (e0) cudaEventRecord(e0, st);
+  }
+  ~TimedLaunch() {
+    if (!e0 || !e1) return;
+    cudaEventRecord(e1, st);
+    std::lock_guard<std::mutex> lk(g_timer.mu);
+    g_timer.ev[kid].push_back({e0, e1});
+  }
+};
 
 ttdft_status fail(ttdft_status st, const char* fmt, ...) {
   char buf[512];
@@ -373,6 +405,7 @@ ttdft_status launch_k1(const ttdft_h_s* h, const CUtensorMap& tmH, double alpha,
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
   const int64_t tiles = (int64_t)p.nb * p.rs * p.nct;
   if (tiles > 0x7fffffffLL) return fail(TTDFT_ERR_UNSUPPORTED, "too many tiles (%lld)", (long long)tiles);
+  TimedLaunch tl(1, st);
   ttdft::bsr_dmma_kernel<WR, Q, CPS, RS><<<(unsigned)tiles, SM::THREADS, SM::TOTAL, st>>>(tmH, tmX, p);
   CUDA_TRY(cudaGetLastError());
   g_launches.fetch_add(1);
@@ -426,6 +459,7 @@ ttdft_status launch_step(const ttdft_h_s* h, double alpha, double gamma, double 
   p.X = X; p.ldx = ldx; p.Z = Z; p.ldz = ldz; p.O = O; p.ldo = ldo;
   dim3 grid((unsigned)((h->M + ttdft::K2_ROWS - 1) / ttdft::K2_ROWS), (unsigned)((ncols + ttdft::K2_TN - 1) / ttdft::K2_TN));
   if (grid.y > 65535) return fail(TTDFT_ERR_UNSUPPORTED, "ncols too large for the generic kernel");
+  TimedLaunch tl(2, st);
   if (h->bsr)
     ttdft::generic_step_kernel<true><<<grid, 32 * ttdft::K2_ROWS, 0, st>>>(p);
   else
@@ -472,6 +506,7 @@ ttdft_status launch_step_i8(const ttdft_h_s* h, double alpha, double gamma, doub
   if (!have_src_max) {
     CUDA_TRY(cudaMemsetAsync(cmS, 0, (size_t)ncols * 4, st));
     dim3 g(nct, (unsigned)((h->M + 2047) / 2048));
+    TimedLaunch tl(5, st);
     ttdft::colmax_kernel<<<g, 256, 0, st>>>(X, ldx, h->M, ncols, cmS);
     CUDA_TRY(cudaGetLastError());
     g_launches.fetch_add(1);
@@ -484,6 +519,7 @@ ttdft_status launch_step_i8(const ttdft_h_s* h, double alpha, double gamma, doub
       attr_set = true;
     }
     dim3 g((unsigned)h->nb, nct);
+    TimedLaunch tl(4, st);
     ttdft::y_digits_kernel<S><<<g, 256, smem, st>>>(X, ldx, h->b, ncols, cmS, w.D, Mk, cmO);
     CUDA_TRY(cudaGetLastError());
     g_launches.fetch_add(1);
@@ -508,6 +544,7 @@ ttdft_status launch_step_i8(const ttdft_h_s* h, double alpha, double gamma, doub
   }
   const int64_t tiles = (int64_t)h->nb * nct;
   const unsigned grid = (unsigned)std::min<int64_t>(tiles, h->nsm);
+  TimedLaunch tl(3, st);
   ttdft::bsr_i8_kernel<S><<<grid, ttdft::K3_THREADS, C3::TOTAL, st>>>(h->tmHd, tmYd, p);
   CUDA_TRY(cudaGetLastError());
   g_launches.fetch_add(1);
@@ -583,6 +620,31 @@ ttdft_status filter_panel(const ttdft_h_s* h, const double* Xp, int64_t ldx, dou
 extern "C" {
 
 const char* ttdft_last_error(void) { return g_err.c_str(); }
+
+ttdft_status ttdft_timing_enable(int32_t on) {
+  g_timer.on.store(on ? 1 : 0);
+  return TTDFT_OK;
+}
+ttdft_status ttdft_timing_read(int32_t kernel_id, double* total_ms, int64_t* launches) {
+  if (kernel_id < 1 || kernel_id >= NKID || !total_ms || !launches) return fail(TTDFT_ERR_INVALID_ARG, "bad timing arguments");
+  std::lock_guard<std::mutex> lk(g_timer.mu);
+  double tot = 0.0;
+  int64_t n = 0;
+  for (auto& pr : g_timer.ev[kernel_id]) {
+    float ms = 0.f;
+    cudaError_t e = cudaEventSynchronize(pr.second);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, pr.first, pr.second);
+    if (e != cudaSuccess) return fail(TTDFT_ERR_CUDA, "timing read: %s", cudaGetErrorString(e));
+    tot += ms;
+    ++n;
+    g_timer.pool.push_back(pr.first);
+    g_timer.pool.push_back(pr.second);
+  }
+  g_timer.ev[kernel_id].clear();
+  *total_ms = tot;
+  *launches = n;
+  return TTDFT_OK;
+}
 int64_t ttdft_launch_count(void) { return g_launches.load(); }
 
 static ttdft_status desc_counts(const ttdft_h_desc* d, int64_t* nrows_idx, int64_t* nstored) {

@@ -3,6 +3,9 @@
 subdomain-ordered BSR and CSR with rows/columns symmetrically permuted by seed (irregular-access
 stress) -- each reported against the binding roofline:
     T_roof = max(alg_bytes / BW_hbm, useful_flops / P_fp64).
+The BSR layout runs twice: fp64 tensor-core MMA (kernel 1) and int8 digit planes (kernel 3, through
+the *_ws entry points; its time includes the digit extraction of X); roofline_frac > 1 there means
+the fp64-accurate product ran faster than the native fp64 pipe could.
 
     python -m paper_2110_15853_b200.sweep [--workload si] [--layouts bsr,csr] [--out gpurun_out/sweep.json]
 """
@@ -57,6 +60,7 @@ def main():
     ap.add_argument("--ns", default="16,64,256,1024,4096")
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--csr-max-n", type=int, default=4096)
+    ap.add_argument("--math", default="fp64,i8", help="arithmetic of the bsr layout: fp64 (DMMA), i8 (digit planes)")
     ap.add_argument("--out", default="")
     args = ap.parse_args()
     import torch
@@ -81,6 +85,11 @@ def main():
         handles["csr"] = tt.h_build_csr(Cp.M, torch.from_numpy(Cp.row_ptr).to(dev), torch.from_numpy(Cp.col_idx).to(dev),
                                         torch.from_numpy(Cp.values).to(dev))
         del Cp
+    if "bsr" in handles and handles["bsr"].info()["i8_planes"] and "i8" in args.math:
+        # the same handle through the int8 digit-plane kernel (ttdft_*_ws entry points)
+        handles["bsr-i8"] = handles["bsr"]
+    if "fp64" not in args.math:
+        handles.pop("bsr", None)
     stored = {k: h.info()["nnz_stored"] for k, h in handles.items()}
     del H
     for N in [int(x) for x in args.ns.split(",")]:
@@ -90,12 +99,18 @@ def main():
         for layout, Hd in handles.items():
             if layout == "csr" and N > args.csr_max_n:
                 continue
+            i8 = layout == "bsr-i8"
+            work = None
+            if layout.startswith("bsr"):
+                Hd.set_math_mode(tt.MATH_I8 if i8 else tt.MATH_FP64)
+            if i8:
+                work = torch.empty(tt.step_work_bytes(Hd, N) + 16, dtype=torch.uint8, device=dev)
             for op in ("spmm", "step"):
                 if op == "spmm":
-                    fn = lambda: tt.spmm(Hd, 1.0, X, 0.0, O)
+                    fn = lambda: tt.spmm(Hd, 1.0, X, 0.0, O, work=work)
                     alg_bytes = 8.0 * nnz + 16.0 * cfg.M * N
                 else:
-                    fn = lambda: tt.cheb_step(Hd, 0.1, 10.0, -0.2, X, Z, O)
+                    fn = lambda: tt.cheb_step(Hd, 0.1, 10.0, -0.2, X, Z, O, work=work)
                     alg_bytes = 8.0 * nnz + 24.0 * cfg.M * N
                 reps = args.reps if (layout == "bsr" or N <= 256) else 3
                 t_med, t_min = time_launches(fn, reps, flush)
@@ -105,7 +120,7 @@ def main():
                        "useful_tflops": flops / t_med / 1e12, "alg_gbs": alg_bytes / t_med / 1e9,
                        "executed_tflops": 2.0 * stored[layout] * N / t_med / 1e12,
                        "binds": "hbm" if alg_bytes / bw > flops / FP64_PEAK else "fp64",
-                       "roofline_frac": t_roof / t_med, "kernel": Hd.info()["kernel"]}
+                       "roofline_frac": t_roof / t_med, "kernel": 3 if i8 else Hd.info()["kernel"]}
                 rows.append(row)
                 print(json.dumps(row), flush=True)
         del X, Z, O

@@ -270,6 +270,14 @@ def test_launch_counter_and_probe(tt):
     X = dev(synth.dense_normal(H.M, 8, 1))
     import torch
     Y = torch.empty_like(X)
+    n1 = tt.launch_count()
+    assert n1 == n0 + 2                      # the builder's two digit-plane kernels (row scales, planes)
     tt.spmm(Hd, 1.0, X, 0.0, Y)
-    assert tt.launch_count() == n0 + 1
+    assert tt.launch_count() == n1 + 1       # one fused kernel per product
+    tt.timing_enable(True)
+    tt.spmm(Hd, 1.0, X, 0.0, Y)
+    tt.timing_enable(False)
+    ms, n = tt.timing_read("bsr_dmma")
+    assert n == 1 and ms > 0.0
+    assert tt.timing_read("bsr_dmma") == (0.0, 0)
     assert tt.probe_fp64_peak(1, 50) > 5.0
