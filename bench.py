@@ -186,8 +186,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--panel", type=int, default=0, help="column-panel width (0 = config default)")
     ap.add_argument("--ref-cols", type=int, default=16, help="columns in the oracle sample")
-    ap.add_argument("--math", default="auto", choices=["auto", "fp64", "i8"],
-                    help="arithmetic of the block product: fp64 DMMA, int8 digit planes (fp64-accurate), auto")
+    ap.add_argument("--math", default="auto", choices=["auto", "fp64", "i8", "i8x7"],
+                    help="arithmetic of the block product: fp64 DMMA; exact int8 digit planes on the tcgen05 tensor "
+                         "cores with 7 planes (55 bits, i8x7) or 6 planes (47 bits, i8); auto = i8x7 for tiles >= 64")
+    ap.add_argument("--no-other-modes", action="store_true", help="skip the short runs of the other math modes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -217,10 +219,13 @@ def main():
                         torch.from_numpy(H.values).to(dev))
     torch.cuda.synchronize()
     t_build = time.perf_counter() - t_build0
-    Hd.set_math_mode({"auto": tt.MATH_AUTO, "fp64": tt.MATH_FP64, "i8": tt.MATH_I8}[args.math])
+    MODES = {"auto": tt.MATH_AUTO, "fp64": tt.MATH_FP64, "i8": tt.MATH_I8, "i8x7": tt.MATH_I8X7}
+    Hd.set_math_mode(MODES[args.math])
     info = Hd.info()
     assert info["kernel"] == 1, "a block-sparse tensor-core kernel must be the one that runs"
-    use_i8 = info["math"] == tt.MATH_I8
+    use_i8 = info["math"] in (tt.MATH_I8, tt.MATH_I8X7)
+    planes = {tt.MATH_I8: 6, tt.MATH_I8X7: 7}.get(info["math"], 0)
+    mode_name = {tt.MATH_FP64: "fp64", tt.MATH_I8: "i8", tt.MATH_I8X7: "i8x7"}[info["math"]]
 
     # this rank's band of wavefunctions: columns [rank*N, (rank+1)*N) of the global block (host, pinned)
     Xh = torch.empty((cfg.M, cfg.N), dtype=torch.float64).pin_memory()
@@ -312,7 +317,7 @@ def main():
     if use_i8:
         # K3: the product runs as S(S+1)/2 exact int8 digit-plane products on the tensor pipe, so the
         # tensor pipe bounds it.  Algorithmic ops per launch = 2 * pairs * nnz * N (non-zeros only).
-        S = info["i8_planes"]
+        S = planes
         pairs = S * (S + 1) // 2
         peak, peak_src = int8_peak_tops()
         ops_launch = 2.0 * pairs * nnz * cfg.N / npanels
@@ -340,18 +345,47 @@ def main():
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": dict(workload_config(cfg, nnz, H.nblocks, args),
-                       math="int8 digit planes (6 x 8 bit per operand, exact int32 accumulation, fp64 in/out)" if use_i8
-                       else "fp64 tensor-core MMA"),
+                       math=(f"{mode_name}: exact int8 digit planes on tcgen05 ({planes} x 8 bit per fp64 operand = "
+                             f"{8 * planes - 1} bits below the row/column maximum, exact int32 accumulation, fp64 "
+                             "recombination, fp64 in/out)") if use_i8 else "fp64: fp64 tensor-core MMA (DMMA)"),
         "clocks": clocks, "gpu_launches": int(launches), "roofline": roof,
         "h_build_ms": t_build * 1e3,
     }
     if e2e is not None:
         line["e2e"] = e2e
 
+    # ---- the other arithmetic modes on the same handle and inputs: 1 warm-up + 1 timed filter each ----
+    cols_d = torch.from_numpy(synth.column_sample(cfg.N, cfg.panel, args.ref_cols, cfg.seed)).to(dev)
+    samples = {mode_name: Yd[:, cols_d].clone()}
+    others = {}
+    if rank == 0 and world == 1 and not args.no_other_modes:
+        for name in ("fp64", "i8x7", "i8"):
+            if name == mode_name or (name != "fp64" and not info["i8_planes"]):
+                continue
+            Hd.set_math_mode(MODES[name])
+            w2 = torch.empty(tt.cheb_filter_work_bytes(Hd, cfg.N, panel) + 16, dtype=torch.uint8, device=dev)
+            tt.cheb_filter(Hd, Xd, Yd, cfg.m, a, b, a0, panel_cols=panel, work=w2)
+            torch.cuda.synchronize()
+            f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            f0.record()
+            tt.cheb_filter(Hd, Xd, Yd, cfg.m, a, b, a0, panel_cols=panel, work=w2)
+            f1.record()
+            torch.cuda.synchronize()
+            t_o = f0.elapsed_time(f1) * 1e-3
+            others[name] = {"value": useful / t_o / 1e9, "unit": "GFLOP/s", "ms_per_step": t_o * 1e3, "steps": 1, "warmup": 1,
+                            "frac_of_fp64_peak": useful / t_o / 1e12 / FP64_PEAK_TFLOPS}
+            samples[name] = Yd[:, cols_d].clone()
+            del w2
+        Hd.set_math_mode(MODES[args.math])
+        line["other_math_modes"] = others
+
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         dt, _, cols, Xs, Yo, threads = oracle_sample_run(cfg, H, args.ref_cols, cfg.m, (a, b, a0))
-        got = Yd[:, torch.from_numpy(cols).to(dev)].cpu().numpy()
+        got = samples[mode_name].cpu().numpy()
         err = float(np.linalg.norm(got - Yo) / np.linalg.norm(Yo))
+        for name in others:
+            g2 = samples[name].cpu().numpy()
+            others[name]["gpu_vs_oracle_relerr_on_sample"] = float(np.linalg.norm(g2 - Yo) / np.linalg.norm(Yo))
         line["cpu_baseline"] = {"value": 2.0 * nnz * len(cols) * cfg.m / dt / 1e9, "unit": "GFLOP/s", "cores": threads,
                                 "kind": "oracle", "seconds": dt,
                                 "sample": f"{len(cols)} seeded columns of {cfg.N} (all rows, all m={cfg.m} steps)",

@@ -47,22 +47,26 @@ typedef enum { TTDFT_FMT_CSR = 0, TTDFT_FMT_BSR = 1 } ttdft_format;
 #define TTDFT_CHECK_SORTED 1u   /* verify indices in range, ascending and unique per row (synchronises) */
 #define TTDFT_CHECK_SYMMETRY 2u /* verify H == H^T bit for bit (synchronises; needs sorted columns)      */
 #define TTDFT_FORCE_GENERIC 4u  /* keep the input format and use the generic row-per-warp kernel          */
-#define TTDFT_NO_I8 8u          /* do not build the int8 digit planes (saves 0.75x of the tile bytes)     */
+#define TTDFT_NO_I8 8u          /* do not build the int8 digit planes (saves 0.875x of the tile bytes)    */
 
 /*
  * Arithmetic of the block-sparse product (every mode returns fp64 results inside north_star's
  * tolerance; DESIGN.md "Kernel K3" has the error bound):
  *   TTDFT_MATH_FP64  fp64 tensor-core MMA (DMMA), fp64 accumulation.
- *   TTDFT_MATH_I8    each fp64 operand is split exactly into 6 balanced base-256 digit planes (47 bits
+ *   TTDFT_MATH_I8X7  each fp64 operand is split exactly into 7 balanced base-256 digit planes (55 bits
  *                    below the maximum of its H row / Y column; the diagonal of H stays fp64), the
- *                    plane products run on the int8 tensor cores with exact int32 accumulation, and
- *                    the epilogue recombines them in fp64.  Needs scratch for the digit planes of one
- *                    iterate, so it is used by the calls that take `work`.
- *   TTDFT_MATH_AUTO  I8 where it is faster (tile size >= 64 and digit planes built), else FP64.
+ *                    plane products of significance >= 2^-55 (28 of 49) run on the int8 tensor cores
+ *                    with exact int32 accumulation, and the epilogue recombines them in fp64: the
+ *                    product's error bound is below that of an fp64 dot product.  Needs scratch for the
+ *                    digit planes of one iterate, so it is used by the calls that take `work`.
+ *   TTDFT_MATH_I8    the same with the leading 6 planes (47 bits, 21 plane products): ~1.3x faster,
+ *                    error ~1e-14 per product, still 100x inside north_star's 1e-12.
+ *   TTDFT_MATH_AUTO  I8X7 where it is faster than FP64 (tile size >= 64 and digit planes built), else FP64.
  */
 #define TTDFT_MATH_AUTO 0
 #define TTDFT_MATH_FP64 1
 #define TTDFT_MATH_I8 2
+#define TTDFT_MATH_I8X7 3
 
 /*
  * Description of the input Hamiltonian (PAPER.md:L199-205 H^L; L250-252 block structure: "the
@@ -96,8 +100,8 @@ typedef struct {
   int32_t kernel;         /* 1 = block-sparse TMA + fp64 tensor-core kernel, 0 = generic    */
   int64_t nblocks;
   size_t storage_bytes;
-  int32_t i8_planes;      /* digit planes per operand stored for TTDFT_MATH_I8 (0: not built) */
-  int32_t math;           /* TTDFT_MATH_FP64 or TTDFT_MATH_I8: what calls that take `work` use */
+  int32_t i8_planes;      /* digit planes per operand of H stored for the I8 modes (0: not built) */
+  int32_t math;           /* TTDFT_MATH_FP64, _I8 or _I8X7: what calls that take `work` use */
 } ttdft_h_info_t;
 
 /* A0 -- storage builder (north_star "BSR/CSR storage builder"). */
@@ -119,7 +123,7 @@ ttdft_status ttdft_h_destroy(ttdft_h_t h);
 /* Select the arithmetic for the calls that take `work` (ttdft_cheb_filter*, ttdft_*_ws); the default
  * is TTDFT_MATH_AUTO (or the value of the environment variable TTDFT_MATH at build time).  Changes the
  * handle: do not call it while another thread is using the handle; query the work sizes again
- * afterwards.  TTDFT_ERR_UNSUPPORTED if I8 is asked of a handle without digit planes. */
+ * afterwards.  TTDFT_ERR_UNSUPPORTED if an I8 mode is asked of a handle without digit planes. */
 ttdft_status ttdft_h_set_math_mode(ttdft_h_t h, int32_t mode);
 
 /*
@@ -165,7 +169,7 @@ ttdft_status ttdft_cheb_scalars(int32_t m, double a, double b, double a0, double
 
 /* Bytes of scratch ttdft_cheb_filter needs: one compact M x panel panel (panel_cols == 0: the
  * library's default panel width for this ncols), plus, in TTDFT_MATH_I8, the int8 digit planes of
- * one iterate (6 bytes per element) and two arrays of column maxima. */
+ * one iterate (6 or 7 bytes per element) and two arrays of column maxima. */
 ttdft_status ttdft_cheb_filter_work_bytes(ttdft_h_t h, int64_t ncols, int64_t panel_cols, size_t* bytes);
 
 /*

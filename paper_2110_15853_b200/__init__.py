@@ -30,6 +30,7 @@ from .api import (  # noqa: F401
     MATH_AUTO,
     MATH_FP64,
     MATH_I8,
+    MATH_I8X7,
     step_work_bytes,
     timing_enable,
     timing_read,

@@ -9,7 +9,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_PKG, "libttdft.so")
 
 CHECK_SORTED, CHECK_SYMMETRY, FORCE_GENERIC, NO_I8 = 1, 2, 4, 8
-MATH_AUTO, MATH_FP64, MATH_I8 = 0, 1, 2
+MATH_AUTO, MATH_FP64, MATH_I8, MATH_I8X7 = 0, 1, 2, 3
 FMT_CSR, FMT_BSR = 0, 1
 _STATUS = {0: "OK", 1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "NOT_SYMMETRIC", 5: "CUDA"}
 
@@ -177,7 +177,7 @@ class Hamiltonian:
         return {k: getattr(inf, k) for k, _ in _Info._fields_}
 
     def set_math_mode(self, mode: int):
-        """ttdft_h_set_math_mode: MATH_AUTO / MATH_FP64 / MATH_I8 for the calls that take `work`."""
+        """ttdft_h_set_math_mode: MATH_AUTO / MATH_FP64 / MATH_I8 / MATH_I8X7 for the calls that take `work`."""
         _check(_load().ttdft_h_set_math_mode(self.handle, mode))
         return self
 

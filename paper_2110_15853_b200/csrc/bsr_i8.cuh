@@ -35,6 +35,7 @@ struct K3Params {
   const int32_t* brow_ptr;
   const int32_t* bcol;
   int32_t nb, b, nct, cg, vec;
+  int32_t hplanes;                 // digit planes STORED per tile of H (>= S; the kernel uses the leading S)
   int64_t ncols;
   double alpha, gamma, beta;
   const double* S;  int64_t lds;   // Y_k at the output position (diagonal + shift term)
@@ -176,7 +177,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
           for (int q = 0; q < S; ++q) {
             mbar_wait(&hempty[hs], hph ^ 1);
             mbar_expect_tx(&hfull[hs], (uint32_t)b * 128u);
-            tma_load_2d(hring + hs * C::HSLOT, &tmHd, 0, (p * S + q) * b, &hfull[hs]);
+            tma_load_2d(hring + hs * C::HSLOT, &tmHd, 0, (p * prm.hplanes + q) * b, &hfull[hs]);
             if (++hs == NH) { hs = 0; hph ^= 1; }
           }
           yb ^= 1;

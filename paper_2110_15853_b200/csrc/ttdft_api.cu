@@ -111,7 +111,9 @@ ttdft_status make_map_2d(CUtensorMap* map, const void* base, uint64_t cols, uint
 
 bool k1_block_ok(int32_t b) { return b == 32 || b == 64 || b == 96 || b == 128; }
 
-constexpr int I8_S = 6;   // digit planes per operand: 47 bits below each row / column maximum
+constexpr int I8_S = 7;   // digit planes STORED per operand of H: 55 bits below each row maximum.  TTDFT_MATH_I8X7 uses
+                          // all of them; TTDFT_MATH_I8 uses the leading 6 (a balanced expansion cut after 6 digits is
+                          // the 47-bit rounding of the operand up to 0.502 ulp)
 
 // H digit planes: uint8 [rows][128 bytes], box = box_rows x 128 B, 128B swizzle
 ttdft_status make_map_hd(CUtensorMap* map, const void* base, uint64_t rows, uint32_t box_rows) {
@@ -168,7 +170,8 @@ struct ttdft_h_s {
   int32_t split = 0;
   int32_t cg = 4;           // column tiles per scheduling group
   // K3 (int8 digit planes on the tcgen05 tensor cores); i8_S == 0: not built
-  int32_t i8_S = 0;
+  int32_t i8_S = 0;         // planes stored per tile
+  int32_t auto_planes = 7;  // planes TTDFT_MATH_AUTO uses (env TTDFT_I8_AUTO_PLANES: 6 or 7)
   int32_t math = TTDFT_MATH_AUTO;
   const int8_t* Hd = nullptr;     // [nblocks][S][b][128]
   const int32_t* eH = nullptr;    // [M]
@@ -476,28 +479,34 @@ struct I8Work {            // views into the caller's scratch (ttdft_step_work_b
   int8_t* D = nullptr;     // digit planes of the source iterate: [S][w][nb*128]
   uint32_t* cmax[2] = {nullptr, nullptr};   // column maxima (upper words): source / next iterate
 };
+// digit planes per operand the handle's math mode uses: 0 (fp64 DMMA), 6 or 7
+int i8_planes_in_use(const ttdft_h_s* h) {
+  if (h->i8_S == 0) return 0;
+  if (h->math == TTDFT_MATH_I8) return 6;
+  if (h->math == TTDFT_MATH_I8X7) return 7;
+  if (h->math == TTDFT_MATH_AUTO && h->b >= 64) return h->auto_planes;
+  return 0;
+}
+bool want_i8(const ttdft_h_s* h) { return i8_planes_in_use(h) > 0; }
 size_t i8_work_bytes(const ttdft_h_s* h, int64_t w) {
-  return align_up((size_t)I8_S * (size_t)w * (size_t)h->nb * 128, 1024) + 2 * align_up((size_t)w * 4, 1024);
+  return align_up((size_t)i8_planes_in_use(h) * (size_t)w * (size_t)h->nb * 128, 1024) + 2 * align_up((size_t)w * 4, 1024);
 }
 I8Work carve_i8_work(const ttdft_h_s* h, void* base, int64_t w) {
   I8Work k;
   uint8_t* p = reinterpret_cast<uint8_t*>(base);
   k.D = reinterpret_cast<int8_t*>(p);
-  p += align_up((size_t)I8_S * (size_t)w * (size_t)h->nb * 128, 1024);
+  p += align_up((size_t)i8_planes_in_use(h) * (size_t)w * (size_t)h->nb * 128, 1024);
   k.cmax[0] = reinterpret_cast<uint32_t*>(p);
   k.cmax[1] = reinterpret_cast<uint32_t*>(p + align_up((size_t)w * 4, 1024));
   return k;
 }
-bool want_i8(const ttdft_h_s* h) {
-  return h->i8_S > 0 && (h->math == TTDFT_MATH_I8 || (h->math == TTDFT_MATH_AUTO && h->b >= 64));
-}
 
 // src: index of the cmax array that holds (have_src_max) or will hold the maxima of X; the other one
 // receives the maxima of O if want_out_max.
-ttdft_status launch_step_i8(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
-                            const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, const I8Work& w, int src,
-                            bool have_src_max, bool want_out_max, cudaStream_t st) {
-  constexpr int S = I8_S;
+template <int S>
+ttdft_status launch_step_i8_t(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
+                              const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, const I8Work& w, int src,
+                              bool have_src_max, bool want_out_max, cudaStream_t st) {
   if (h->M == 0) return TTDFT_OK;
   const int64_t Mk = h->nb * 128;
   const unsigned nct = (unsigned)((ncols + ttdft::K3_NT - 1) / ttdft::K3_NT);
@@ -530,6 +539,7 @@ ttdft_status launch_step_i8(const ttdft_h_s* h, double alpha, double gamma, doub
   ttdft::K3Params p;
   p.brow_ptr = h->row_ptr; p.bcol = h->col;
   p.nb = (int32_t)h->nb; p.b = h->b; p.nct = (int32_t)nct; p.cg = h->cg;
+  p.hplanes = h->i8_S;
   p.ncols = ncols;
   p.alpha = alpha; p.gamma = gamma; p.beta = beta;
   p.S = X; p.lds = ldx; p.Z = Z ? Z : X; p.ldz = Z ? ldz : ldx; p.O = O; p.ldo = ldo;
@@ -549,6 +559,13 @@ ttdft_status launch_step_i8(const ttdft_h_s* h, double alpha, double gamma, doub
   CUDA_TRY(cudaGetLastError());
   g_launches.fetch_add(1);
   return TTDFT_OK;
+}
+ttdft_status launch_step_i8(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
+                            const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, const I8Work& w, int src,
+                            bool have_src_max, bool want_out_max, cudaStream_t st) {
+  if (i8_planes_in_use(h) == 7)
+    return launch_step_i8_t<7>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, w, src, have_src_max, want_out_max, st);
+  return launch_step_i8_t<6>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, w, src, have_src_max, want_out_max, st);
 }
 
 ttdft_status launch_copy2d(const double* src, int64_t lds, double* dst, int64_t ldd, int64_t rows, int64_t cols,
@@ -857,7 +874,18 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     h->cg = env_int("TTDFT_K1_CG", 4);
     if (h->cg < 1) h->cg = 1;
   }
-  if (h->kernel == 1 && need_i8 > 0) {
+  bool i8_ok = (h->kernel == 1 && need_i8 > 0);
+  if (i8_ok) {
+    // exact int32 accumulation needs  planes x tiles-per-block-row x b x 128^2 < 2^31  (146 tiles at b = 128)
+    std::vector<int32_t> hb((size_t)h->nb + 1);
+    cudaError_t e = cudaMemcpyAsync(hb.data(), h->row_ptr, hb.size() * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "block row pointers: %s", cudaGetErrorString(e)); }
+    int64_t maxj = 0;
+    for (int64_t I = 0; I < h->nb; ++I) maxj = std::max<int64_t>(maxj, hb[(size_t)I + 1] - hb[(size_t)I]);
+    if ((int64_t)I8_S * maxj * h->b * 16384 >= (int64_t)1 << 31) i8_ok = false;
+  }
+  if (i8_ok) {
     // ---- int8 digit planes of every tile (K3): row exponents + diagonal, then the planes ----
     uint8_t* q = base + need;
     int8_t* Hd = reinterpret_cast<int8_t*>(q);
@@ -877,6 +905,8 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0)
       h->nsm = nsm;
     h->math = env_int("TTDFT_MATH", TTDFT_MATH_AUTO);
+    if (h->math < TTDFT_MATH_AUTO || h->math > TTDFT_MATH_I8X7) h->math = TTDFT_MATH_AUTO;
+    h->auto_planes = env_int("TTDFT_I8_AUTO_PLANES", 7) == 6 ? 6 : 7;
   }
   *out = h;
   return TTDFT_OK;
@@ -891,15 +921,16 @@ ttdft_status ttdft_h_info(ttdft_h_t h, ttdft_h_info_t* info) {
   info->nnz_stored = h->bsr ? h->nblocks * (int64_t)h->b * h->b : h->nblocks;
   info->storage_bytes = h->storage_bytes;
   info->i8_planes = h->i8_S;
-  info->math = want_i8(h) ? TTDFT_MATH_I8 : TTDFT_MATH_FP64;
+  const int used = i8_planes_in_use(h);
+  info->math = used == 7 ? TTDFT_MATH_I8X7 : used == 6 ? TTDFT_MATH_I8 : TTDFT_MATH_FP64;
   return TTDFT_OK;
 }
 
 ttdft_status ttdft_h_set_math_mode(ttdft_h_t h, int32_t mode) {
   if (!h) return fail(TTDFT_ERR_INVALID_ARG, "handle is NULL");
-  if (mode != TTDFT_MATH_AUTO && mode != TTDFT_MATH_FP64 && mode != TTDFT_MATH_I8)
+  if (mode != TTDFT_MATH_AUTO && mode != TTDFT_MATH_FP64 && mode != TTDFT_MATH_I8 && mode != TTDFT_MATH_I8X7)
     return fail(TTDFT_ERR_INVALID_ARG, "unknown math mode %d", mode);
-  if (mode == TTDFT_MATH_I8 && h->i8_S == 0)
+  if ((mode == TTDFT_MATH_I8 || mode == TTDFT_MATH_I8X7) && h->i8_S == 0)
     return fail(TTDFT_ERR_UNSUPPORTED, "this handle was built without int8 digit planes");
   h->math = mode;
   return TTDFT_OK;

@@ -3,7 +3,7 @@
 subdomain-ordered BSR and CSR with rows/columns symmetrically permuted by seed (irregular-access
 stress) -- each reported against the binding roofline:
     T_roof = max(alg_bytes / BW_hbm, useful_flops / P_fp64).
-The BSR layout runs twice: fp64 tensor-core MMA (kernel 1) and int8 digit planes (kernel 3, through
+The BSR layout runs three times: fp64 tensor-core MMA (kernel 1) and int8 digit planes (kernel 3 with 7 and 6 planes, through
 the *_ws entry points; its time includes the digit extraction of X); roofline_frac > 1 there means
 the fp64-accurate product ran faster than the native fp64 pipe could.
 
@@ -60,7 +60,7 @@ def main():
     ap.add_argument("--ns", default="16,64,256,1024,4096")
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--csr-max-n", type=int, default=4096)
-    ap.add_argument("--math", default="fp64,i8", help="arithmetic of the bsr layout: fp64 (DMMA), i8 (digit planes)")
+    ap.add_argument("--math", default="fp64,i8x7,i8", help="arithmetic of the bsr layout: fp64 (DMMA), i8x7 / i8 (7 / 6 digit planes)")
     ap.add_argument("--out", default="")
     args = ap.parse_args()
     import torch
@@ -85,10 +85,14 @@ def main():
         handles["csr"] = tt.h_build_csr(Cp.M, torch.from_numpy(Cp.row_ptr).to(dev), torch.from_numpy(Cp.col_idx).to(dev),
                                         torch.from_numpy(Cp.values).to(dev))
         del Cp
-    if "bsr" in handles and handles["bsr"].info()["i8_planes"] and "i8" in args.math:
-        # the same handle through the int8 digit-plane kernel (ttdft_*_ws entry points)
-        handles["bsr-i8"] = handles["bsr"]
-    if "fp64" not in args.math:
+    maths = args.math.split(",")
+    if "bsr" in handles and handles["bsr"].info()["i8_planes"]:
+        # the same handle through the int8 digit-plane kernel (ttdft_*_ws entry points), 7 and 6 planes
+        if "i8x7" in maths:
+            handles["bsr-i8x7"] = handles["bsr"]
+        if "i8" in maths:
+            handles["bsr-i8"] = handles["bsr"]
+    if "fp64" not in maths:
         handles.pop("bsr", None)
     stored = {k: h.info()["nnz_stored"] for k, h in handles.items()}
     del H
@@ -99,10 +103,10 @@ def main():
         for layout, Hd in handles.items():
             if layout == "csr" and N > args.csr_max_n:
                 continue
-            i8 = layout == "bsr-i8"
+            i8 = layout.startswith("bsr-i8")
             work = None
             if layout.startswith("bsr"):
-                Hd.set_math_mode(tt.MATH_I8 if i8 else tt.MATH_FP64)
+                Hd.set_math_mode({"bsr": tt.MATH_FP64, "bsr-i8": tt.MATH_I8, "bsr-i8x7": tt.MATH_I8X7}[layout])
             if i8:
                 work = torch.empty(tt.step_work_bytes(Hd, N) + 16, dtype=torch.uint8, device=dev)
             for op in ("spmm", "step"):

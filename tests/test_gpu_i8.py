@@ -1,9 +1,11 @@
-"""GPU parity of the int8 digit-plane path (kernel K3, TTDFT_MATH_I8) against the CPU oracle.
+"""GPU parity of the int8 digit-plane path (kernel K3, TTDFT_MATH_I8 / TTDFT_MATH_I8X7) against the
+CPU oracle.
 
 Same tolerances as the fp64 path (north_star): <= 1e-12 relative Frobenius per SpMM / fused step,
-<= 1e-10 after a filter.  K3 splits every operand exactly into 6 balanced base-256 digits below its
-row / column maximum and accumulates in exact integers, so the measured error
-is expected around 1e-14; ACC_SPMM pins that, so that a lost digit plane or level (>= 2^-40) fails."""
+<= 1e-10 after a filter.  K3 splits every operand exactly into 6 (I8) or 7 (I8X7) balanced base-256
+digits below its row / column maximum and accumulates in exact integers, so
+the measured error is expected around 1e-14 (47 bits) and 1e-16..1e-15 (55 bits: the fp64 rounding
+of the epilogue dominates); ACC_SPMM pins that, so that a lost digit plane or level fails."""
 import numpy as np
 import pytest
 
@@ -15,7 +17,9 @@ pytestmark = pytest.mark.gpu
 
 TOL_SPMM = 1e-12
 TOL_FILTER = 1e-10
-ACC_SPMM = 2e-13      # what 47-bit operands must deliver on these inputs
+ACC = {"i8": 2e-13,    # what 47-bit operands must deliver on these inputs
+       "i8x7": 4e-15}  # 55-bit operands: as accurate as an fp64 dot product
+ACC_SPMM = ACC["i8"]
 
 
 @pytest.fixture(scope="module")
@@ -31,19 +35,22 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-def build_i8(t, H, flags=0):
+def build_i8(t, H, flags=0, mode="i8"):
     Hd = t.h_build_bsr(H.M, H.b, dev(H.row_ptr), dev(H.col_idx), dev(H.values), flags=flags)
-    assert Hd.info()["i8_planes"] == 6
-    Hd.set_math_mode(t.MATH_I8)
-    assert Hd.info()["math"] == t.MATH_I8
+    assert Hd.info()["i8_planes"] == 7
+    want = {"i8": t.MATH_I8, "i8x7": t.MATH_I8X7}[mode]
+    Hd.set_math_mode(want)
+    assert Hd.info()["math"] == want
     return Hd
 
 
+@pytest.mark.parametrize("mode", ["i8", "i8x7"])
 @pytest.mark.parametrize("N,ld", [(32, 32), (33, 40), (1, 2), (64, 64), (130, 130), (257, 300)])
-def test_spmm_ws_tiny(tt, N, ld):
+def test_spmm_ws_tiny(tt, N, ld, mode):
     import torch
+    ACC_SPMM = ACC[mode]
     H, C, (rp, col, val), _ = small_problem(4, 32, 0.0, 1001)
-    Hd = build_i8(tt, H, flags=tt.CHECK_SORTED | tt.CHECK_SYMMETRY)
+    Hd = build_i8(tt, H, flags=tt.CHECK_SORTED | tt.CHECK_SYMMETRY, mode=mode)
     assert tt.step_work_bytes(Hd, N) > 0
     X = synth.dense_normal(H.M, N, 11)
     Y0 = synth.dense_normal(H.M, N, 12)
@@ -85,14 +92,15 @@ def test_cheb_step_ws_tiny(tt, N):
     assert relerr(out.cpu().numpy(), ref1) <= TOL_SPMM
 
 
+@pytest.mark.parametrize("mode", ["i8", "i8x7"])
 @pytest.mark.parametrize("m", [1, 2, 3, 10, 11])
 @pytest.mark.parametrize("inplace", [False, True])
-def test_filter_tiny_full_i8(tt, m, inplace):
+def test_filter_tiny_full_i8(tt, m, inplace, mode):
     import torch
     cfg = synth.CONFIGS["tiny"]
     H, C, (rp, col, val), (a0, b) = small_problem(cfg.G, cfg.b, cfg.z, cfg.seed)
     a, b, a0 = bounds_for(a0, b, cfg.N, H.M)
-    Hd = build_i8(tt, H)
+    Hd = build_i8(tt, H, mode=mode)
     X = synth.dense_normal(H.M, cfg.N, cfg.seed)
     ref = oracle.cheb_filter(rp, col, val, X, m, a, b, a0)
     Xd = dev(X)
@@ -120,12 +128,14 @@ def test_filter_panels_and_ragged_i8(tt, N, panel):
     assert worst_col_relerr(Y.cpu().numpy(), ref) <= 10 * TOL_FILTER
 
 
+@pytest.mark.parametrize("mode", ["i8", "i8x7"])
 @pytest.mark.parametrize("G,b,z,N", [(3, 64, 0.3, 200), (2, 96, 0.4, 130), (3, 128, 0.4, 300)])
-def test_other_block_sizes_i8(tt, G, b, z, N):
+def test_other_block_sizes_i8(tt, G, b, z, N, mode):
     import torch
+    ACC_SPMM = ACC[mode]
     H, C, (rp, col, val), (a0, bb) = small_problem(G, b, z, 2000 + b)
     a, bb, a0 = bounds_for(a0, bb, N, H.M)
-    Hd = build_i8(tt, H)
+    Hd = build_i8(tt, H, mode=mode)
     X = synth.dense_normal(H.M, N, 51)
     Y = torch.empty(H.M, N, dtype=torch.float64, device="cuda")
     tt.spmm(Hd, 1.0, dev(X), 0.0, Y, use_work=True)
@@ -172,5 +182,21 @@ def test_no_i8_flag_and_mode_errors(tt):
         Hd.set_math_mode(tt.MATH_I8)
     assert e.value.status_name == "UNSUPPORTED"
     with pytest.raises(tt.TTDFTError):
+        Hd.set_math_mode(tt.MATH_I8X7)
+    with pytest.raises(tt.TTDFTError):
         Hd.set_math_mode(7)
     assert tt.step_work_bytes(Hd, 64) == 0
+
+
+def test_auto_mode_is_i8x7_for_wide_tiles(tt):
+    """TTDFT_MATH_AUTO: 7 planes for tile size >= 64, fp64 DMMA below; work sizes follow the mode."""
+    H, C, _, _ = small_problem(3, 64, 0.3, 2064)
+    Hd = tt.h_build_bsr(H.M, H.b, dev(H.row_ptr), dev(H.col_idx), dev(H.values))
+    assert Hd.info()["math"] == tt.MATH_I8X7
+    w7 = tt.step_work_bytes(Hd, 64)
+    Hd.set_math_mode(tt.MATH_I8)
+    w6 = tt.step_work_bytes(Hd, 64)
+    assert w7 > w6 > 0
+    H, C, _, _ = small_problem(4, 32, 0.0, 1001)
+    Hd = tt.h_build_bsr(H.M, H.b, dev(H.row_ptr), dev(H.col_idx), dev(H.values))
+    assert Hd.info()["math"] == tt.MATH_FP64

@@ -6,6 +6,8 @@ The oracle cannot filter 4,096-14,336 columns of a 2-4e5-row H in reasonable tim
   * EVERY column is covered by the self-adjointness (Freivalds-style) identity
         <u, F(X)[:, j]> = <F(u), X[:, j]>    (F = p_m(H) is symmetric, PAPER.md:L238)
     with F(u) computed by the oracle for r seeded Gaussian probes u.
+Every arithmetic mode of the library (fp64 DMMA, int8 digit planes x7 / x6) runs against the same
+oracle values and the same tolerance.
 """
 import json
 import os
@@ -58,20 +60,33 @@ def run_full(name, nsample, nprobe, inplace):
     ref_s, FU = ref[:, :len(cols)], ref[:, len(cols):]
     FtX = (torch.from_numpy(FU).cuda().T @ Xd).cpu().numpy()        # <F(u), X_j>, before X may be overwritten
 
-    Yd = Xd if inplace else torch.empty_like(Xd)
-    tt.cheb_filter(Hd, Xd, Yd, cfg.m, a, b, a0, panel_cols=cfg.panel)
-    torch.cuda.synchronize()
-    got = Yd[:, torch.from_numpy(cols).cuda()].cpu().numpy()
-    e_f, e_c = relerr(got, ref_s), worst_col_relerr(got, ref_s)
     Ud = torch.from_numpy(U).cuda()
-    UtY = (Ud.T @ Yd).cpu().numpy()
-    ynorm = torch.linalg.vector_norm(Yd, dim=0).cpu().numpy()
     unorm = np.linalg.norm(U, axis=0)
-    adj = np.abs(UtY - FtX) / (unorm[:, None] * ynorm[None, :])
-    print(f"{name}: sample relerr {e_f:.2e} worst col {e_c:.2e}; adjoint check max {adj.max():.2e} over {cfg.N} columns")
-    assert np.isfinite(ynorm).all()
-    assert e_f <= TOL_FILTER and e_c <= 10 * TOL_FILTER
-    assert adj.max() <= TOL_FILTER
+    cols_d = torch.from_numpy(cols).cuda()
+    modes = [("fp64", tt.MATH_FP64)]
+    if Hd.info()["i8_planes"]:
+        modes += [("i8x7", tt.MATH_I8X7), ("i8", tt.MATH_I8)]
+    X0 = Xd.clone() if (inplace and len(modes) > 1) else None     # in place overwrites X: restore it per mode
+    Yd = Xd if inplace else torch.empty_like(Xd)
+    for k, (mname, mode) in enumerate(modes):
+        if inplace and k > 0:
+            Xd.copy_(X0)
+        elif not inplace:
+            Yd.fill_(float("nan"))
+        Hd.set_math_mode(mode)
+        assert Hd.info()["math"] == mode
+        tt.cheb_filter(Hd, Xd, Yd, cfg.m, a, b, a0, panel_cols=cfg.panel)
+        torch.cuda.synchronize()
+        got = Yd[:, cols_d].cpu().numpy()
+        e_f, e_c = relerr(got, ref_s), worst_col_relerr(got, ref_s)
+        UtY = (Ud.T @ Yd).cpu().numpy()
+        ynorm = torch.linalg.vector_norm(Yd, dim=0).cpu().numpy()
+        adj = np.abs(UtY - FtX) / (unorm[:, None] * ynorm[None, :])
+        print(f"{name}/{mname}: sample relerr {e_f:.2e} worst col {e_c:.2e}; adjoint check max {adj.max():.2e} "
+              f"over {cfg.N} columns")
+        assert np.isfinite(ynorm).all()
+        assert e_f <= TOL_FILTER and e_c <= 10 * TOL_FILTER
+        assert adj.max() <= TOL_FILTER
 
 
 def test_full_config2_al():
