@@ -3,11 +3,14 @@
 // carried by the 5th-generation tensor cores as exact int8 digit-plane products (i8_digits.cuh).
 //
 // sm_100a design:
-//   * persistent CTAs (one per SM), static round-robin over (block row I, 64-column tile) work items in
-//     the same L2-friendly order as K1
+//   * persistent CTAs (one per SM) in clusters of C along the columns: the C CTAs of a cluster work on the
+//     same block row I and C adjacent 64-column tiles, static round-robin over (I, tile group) work items
 //   * warp 0 (one lane): TMA producer.  Per tile (I,J) of the block row it brings the S digit planes of
-//     Y_k rows J*b.., 64 columns, with ONE 3-D bulk-tensor load (S x 64 x 128 B, SWIZZLE_128B) into one
-//     of two Y buffers, and the S digit planes of H_IJ (b x 128 B each) through a ring of 16 KB slots
+//     Y_k rows J*b.., 64 columns, with ONE 3-D bulk-tensor load (S x 64 x 128 B, SWIZZLE_128B; the planes of
+//     a tile are contiguous in HBM) into one of two Y buffers, and the S digit planes of H_IJ (b x 128 B
+//     each) through a ring of 16 KB slots.  Every CTA of the cluster fetches b/C rows of each H plane and
+//     MULTICASTS them into the same slot of all C CTAs, so a plane leaves L2 once per cluster: the kernel
+//     was bound by L2->SM throughput before (profiles/r01a_*), H being 2/3 of those bytes
 //   * warp 1 (one lane): tcgen05.mma.kind::i8 issuer.  For H plane p it multiplies against the
 //     CONCATENATION of Y planes 0..S-1-p (N = 64*(S-p), issued as <=256-column instructions), which lands
 //     in the contiguous TMEM column groups p..S-1 because digit-pair level g = p+q lives at columns
@@ -34,7 +37,9 @@ constexpr int K3_THREADS = 192;  // producer warp, MMA warp, 4 epilogue warps
 struct K3Params {
   const int32_t* brow_ptr;
   const int32_t* bcol;
-  int32_t nb, b, nct, cg, vec;
+  int32_t nb, b, vec;
+  int32_t nct;                     // 64-column tiles of the whole panel (index space of the Y digit tiles)
+  int32_t ct_begin, nctg, cgc;     // this launch: first column tile, tile groups (of C tiles), groups per scheduling group
   int32_t hplanes;                 // digit planes STORED per tile of H (>= S; the kernel uses the leading S)
   int64_t ncols;
   double alpha, gamma, beta;
@@ -103,46 +108,75 @@ __device__ __forceinline__ bool elect_one() {
   return pred != 0;
 }
 
-// work item t -> (block row I, column tile ct): column-tile groups outermost, block rows, tile fastest
-__device__ __forceinline__ void k3_decode(const K3Params& prm, int64_t t, int32_t& I, int32_t& ct) {
-  const int64_t per_group = (int64_t)prm.nb * prm.cg;
-  const int32_t ngroups = (prm.nct + prm.cg - 1) / prm.cg;
-  int32_t g = (int32_t)(t / per_group);
-  if (g > ngroups - 1) g = ngroups - 1;
-  const int64_t rem = t - (int64_t)g * per_group;
-  const int32_t width = min(prm.cg, prm.nct - g * prm.cg);
-  I = (int32_t)(rem / width);
-  ct = g * prm.cg + (int32_t)(rem % width);
+__device__ __forceinline__ void tma_load_2d_mc(void* dst, const CUtensorMap* map, int32_t x, int32_t y, uint64_t* bar, uint16_t mask) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1, {%2, %3}], [%4], %5;" ::"r"(
+          smem_u32(dst)),
+      "l"(map), "r"(x), "r"(y), "r"(smem_u32(bar)), "h"(mask)
+      : "memory");
+}
+// arrive on the barrier at this offset in every CTA of the mask once the MMAs issued so far have completed
+__device__ __forceinline__ void umma_commit_mc(uint64_t* bar, uint16_t mask) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(smem_u32(bar)),
+               "h"(mask)
+               : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
-template <int S>
+// cluster work item u -> (block row I, tile group ctg): scheduling groups of cgc tile groups outermost, then
+// block rows, tile group fastest (clusters that run at the same time share H planes and Y rows in L2)
+__device__ __forceinline__ void k3_decode(const K3Params& prm, int64_t u, int32_t& I, int32_t& ctg) {
+  const int64_t per_group = (int64_t)prm.nb * prm.cgc;
+  const int32_t ngroups = (prm.nctg + prm.cgc - 1) / prm.cgc;
+  int32_t g = (int32_t)(u / per_group);
+  if (g > ngroups - 1) g = ngroups - 1;
+  const int64_t rem = u - (int64_t)g * per_group;
+  const int32_t width = min(prm.cgc, prm.nctg - g * prm.cgc);
+  I = (int32_t)(rem / width);
+  ctg = g * prm.cgc + (int32_t)(rem % width);
+}
+
+// tmHd: box (b/C rows) x 128 B of the H digit planes; tmYd: box S x 64 x 128 B of the Y digit tiles.
+// Launched with cluster dimension C (C == 1: a plain launch).  gridDim.x is a multiple of C.
+template <int S, int C>
 __global__ void __launch_bounds__(K3_THREADS, 1)
 bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ CUtensorMap tmYd, const K3Params prm) {
-  using C = K3Cfg<S>;
-  constexpr int NH = C::NH;
+  using Cf = K3Cfg<S>;
+  constexpr int NH = Cf::NH;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* ybuf = smem;                          // 2 x YBUF
-  uint8_t* hring = smem + 2 * C::YBUF;           // NH x HSLOT
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::BAR_OFFSET);
+  uint8_t* hring = smem + 2 * Cf::YBUF;           // NH x HSLOT
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Cf::BAR_OFFSET);
   uint64_t* yfull = bars;                        // [2]
   uint64_t* yempty = bars + 2;                   // [2]
   uint64_t* hfull = bars + 4;                    // [NH]
   uint64_t* hempty = bars + 4 + NH;              // [NH]
   uint64_t* accfull = bars + 4 + 2 * NH;
   uint64_t* accempty = accfull + 1;
-  double* cs_s = reinterpret_cast<double*>(smem + C::CS_OFFSET);        // 2^eY_j of the current tile
-  uint32_t* cm_s = reinterpret_cast<uint32_t*>(smem + C::CM_OFFSET);    // column maxima of the current tile
+  double* cs_s = reinterpret_cast<double*>(smem + Cf::CS_OFFSET);        // 2^eY_j of the current tile
+  uint32_t* cm_s = reinterpret_cast<uint32_t*>(smem + Cf::CM_OFFSET);    // column maxima of the current tile
   uint32_t* tmem_slot = cm_s + 64;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t ntiles = (int64_t)prm.nb * prm.nct;
+  const int64_t nitems = (int64_t)prm.nb * prm.nctg;          // cluster work items
+  const int32_t crank = (C > 1) ? (int32_t)cluster_ctarank() : 0;
+  const int64_t cluster0 = blockIdx.x / C, nclusters = gridDim.x / C;
+  constexpr uint16_t cmask = (uint16_t)((1u << C) - 1u);
   const int32_t b = prm.b;
   const int32_t ksteps = b >> 5;                 // 32-deep int8 MMAs per tile of H
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < 2; ++i) { mbar_init(&yfull[i], 1); mbar_init(&yempty[i], 1); }
-    for (int i = 0; i < NH; ++i) { mbar_init(&hfull[i], 1); mbar_init(&hempty[i], 1); }
+    for (int i = 0; i < NH; ++i) { mbar_init(&hfull[i], 1); mbar_init(&hempty[i], C); }   // a slot is free once all C CTAs have read it
     mbar_init(accfull, 1);
     mbar_init(accempty, 128);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -154,6 +188,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();
+  if (C > 1) cluster_sync_all();                 // peers' barriers are initialised before anything is sent to them
   asm volatile("tcgen05.fence::after_thread_sync;");
   const uint32_t tmem_base = *tmem_slot;
 
@@ -164,20 +199,26 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       asm volatile("prefetch.tensormap [%0];" ::"l"(&tmYd) : "memory");
       int yb = 0, hs = 0;
       uint32_t yph = 0, hph = 0;
-      for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
-        int32_t I, ct;
-        k3_decode(prm, t, I, ct);
+      const int32_t hrows = b / C;               // rows of every H plane this CTA fetches for the cluster
+      for (int64_t u = cluster0; u < nitems; u += nclusters) {
+        int32_t I, ctg;
+        k3_decode(prm, u, I, ctg);
+        const int32_t ct = prm.ct_begin + ctg * C + crank;
         const int32_t p0 = prm.brow_ptr[I], p1 = prm.brow_ptr[I + 1];
         for (int32_t p = p0; p < p1; ++p) {
           const int32_t J = prm.bcol[p];
           mbar_wait(&yempty[yb], yph ^ 1);
-          mbar_expect_tx(&yfull[yb], (uint32_t)C::YBUF);
-          tma_load_3d(ybuf + yb * C::YBUF, &tmYd, J * 128, ct * K3_NT, 0, &yfull[yb]);
+          mbar_expect_tx(&yfull[yb], (uint32_t)Cf::YBUF);
+          tma_load_3d(ybuf + yb * Cf::YBUF, &tmYd, 0, 0, (J * prm.nct + ct) * S, &yfull[yb]);
 #pragma unroll 1
           for (int q = 0; q < S; ++q) {
-            mbar_wait(&hempty[hs], hph ^ 1);
+            mbar_wait(&hempty[hs], hph ^ 1);       // all C CTAs have finished with this slot
             mbar_expect_tx(&hfull[hs], (uint32_t)b * 128u);
-            tma_load_2d(hring + hs * C::HSLOT, &tmHd, 0, (p * prm.hplanes + q) * b, &hfull[hs]);
+            if (C > 1)
+              tma_load_2d_mc(hring + hs * Cf::HSLOT + crank * hrows * 128, &tmHd, 0, (p * prm.hplanes + q) * b + crank * hrows,
+                             &hfull[hs], cmask);
+            else
+              tma_load_2d(hring + hs * Cf::HSLOT, &tmHd, 0, (p * prm.hplanes + q) * b, &hfull[hs]);
             if (++hs == NH) { hs = 0; hph ^= 1; }
           }
           yb ^= 1;
@@ -193,21 +234,21 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       // descriptors differ only in the 14-bit start-address field of the low word
       const uint64_t dbase = umma_desc_sw128(0);
       const uint32_t ylo0 = (smem_u32(ybuf) & 0x3ffffu) >> 4, hlo0 = (smem_u32(hring) & 0x3ffffu) >> 4;
-      for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
-        int32_t I, ct;
-        k3_decode(prm, t, I, ct);
+      for (int64_t u = cluster0; u < nitems; u += nclusters) {
+        int32_t I, ctg;
+        k3_decode(prm, u, I, ctg);
         const int32_t nJ = prm.brow_ptr[I + 1] - prm.brow_ptr[I];
         if (nJ == 0) continue;
         mbar_wait(accempty, aph ^ 1);            // the epilogue has drained the previous item's accumulators
         asm volatile("tcgen05.fence::after_thread_sync;");
         for (int32_t j = 0; j < nJ; ++j) {
           mbar_wait(&yfull[yb], yph);
-          const uint32_t ylo = ylo0 + (uint32_t)yb * (C::YBUF >> 4);
+          const uint32_t ylo = ylo0 + (uint32_t)yb * (Cf::YBUF >> 4);
 #pragma unroll
           for (int p = 0; p < S; ++p) {
             mbar_wait(&hfull[hs], hph);
             asm volatile("tcgen05.fence::after_thread_sync;");
-            const uint32_t hlo = hlo0 + (uint32_t)hs * (C::HSLOT >> 4);
+            const uint32_t hlo = hlo0 + (uint32_t)hs * (Cf::HSLOT >> 4);
             const int ntot = (S - p) * K3_NT;       // Y planes 0..S-1-p side by side -> levels p..S-1
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk) {
@@ -221,7 +262,8 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
                 }
               }
             }
-            umma_commit(&hempty[hs]);            // slot free once these MMAs have read it
+            if (C > 1) umma_commit_mc(&hempty[hs], cmask);   // slot free (in every CTA) once these MMAs have read it
+            else umma_commit(&hempty[hs]);
             if (++hs == NH) { hs = 0; hph ^= 1; }
           }
           umma_commit(&yempty[yb]);
@@ -241,9 +283,10 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
     const double alpha = prm.alpha, beta = prm.beta;
     const bool use_z = (beta != 0.0);
     uint32_t aph = 0;
-    for (int64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
-      int32_t I, ct;
-      k3_decode(prm, t, I, ct);
+    for (int64_t u = cluster0; u < nitems; u += nclusters) {
+      int32_t I, ctg;
+      k3_decode(prm, u, I, ctg);
+      const int32_t ct = prm.ct_begin + ctg * C + crank;
       const int32_t nJ = prm.brow_ptr[I + 1] - prm.brow_ptr[I];
       const int64_t col0 = (int64_t)ct * K3_NT;
       const int64_t row = (int64_t)I * b + r;
@@ -345,6 +388,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
 
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();
+  if (C > 1) cluster_sync_all();                 // no CTA leaves while a peer may still signal its barriers
   if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(512));
 }
 

@@ -71,7 +71,9 @@ __global__ void __launch_bounds__(256) colmax_kernel(const double* __restrict__ 
 }
 
 // ------------------------------------------------------------------------------------------------
-// digit planes of a panel, transposed:  D[q][n][I*128 + k] = digit q of Y[I*b + k, n]   (k < b)
+// digit planes of a panel, transposed and tiled:  D[I][ct][q][n][k] = digit q of Y[I*b + k, 64*ct + n]
+// (k < 128, n < 64; zero for k >= b and for columns beyond ncols), i.e. the S planes of one (block row,
+// 64-column tile) are ONE contiguous S*8 KB piece of HBM -- what one TMA load of K3 fetches.
 // One CTA per (block row I, 64-column tile): coalesced fp64 reads along the columns, a shared-memory
 // transpose, 128-byte coalesced int8 rows out -- the K-major rows K3's B operand wants.
 // Also clears next_cmax (the maxima K3's epilogue will accumulate for the following step).
@@ -79,7 +81,7 @@ __global__ void __launch_bounds__(256) colmax_kernel(const double* __restrict__ 
 // ------------------------------------------------------------------------------------------------
 template <int S>
 __global__ void __launch_bounds__(256) y_digits_kernel(const double* __restrict__ Y, int64_t ld, int32_t b, int64_t ncols,
-                                                       const uint32_t* __restrict__ cmax, int8_t* __restrict__ D, int64_t Mk,
+                                                       const uint32_t* __restrict__ cmax, int8_t* __restrict__ D,
                                                        uint32_t* __restrict__ next_cmax) {
   extern __shared__ uint32_t sd[];   // [S][64][33] words: row (q,n) holds 128 k-bytes + 1 pad word
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -97,36 +99,34 @@ __global__ void __launch_bounds__(256) y_digits_kernel(const double* __restrict_
   }
   const int nquads = b >> 2;
   for (int quad = warp; quad < 32; quad += 8) {
+    // all eight loads of this quad of rows (two 32-column halves) are in flight before any digit work
+    double x[2][4];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const double* src = Y + ((int64_t)I * b + 4 * quad) * ld + n0 + 32 * h + lane;
+#pragma unroll
+      for (int i = 0; i < 4; ++i) x[h][i] = (quad < nquads && cv[h]) ? __ldcs(src + (int64_t)i * ld) : 0.0;
+    }
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       uint32_t w[S];
 #pragma unroll
       for (int p = 0; p < S; ++p) w[p] = 0;
-      if (quad < nquads && cv[h]) {
-        const double* src = Y + ((int64_t)I * b + 4 * quad) * ld + n0 + 32 * h + lane;
-        double x[4];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) x[i] = src[(int64_t)i * ld];
+      for (int i = 0; i < 4; ++i) {
+        int32_t d[S];
+        balanced_digits<S>(x[h][i], scale[h], d);
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          int32_t d[S];
-          balanced_digits<S>(x[i], scale[h], d);
-#pragma unroll
-          for (int p = 0; p < S; ++p) w[p] |= (uint32_t)(d[p] & 0xff) << (8 * i);
-        }
+        for (int p = 0; p < S; ++p) w[p] |= (uint32_t)(d[p] & 0xff) << (8 * i);
       }
 #pragma unroll
       for (int p = 0; p < S; ++p) sd[(p * 64 + 32 * h + lane) * 33 + quad] = w[p];
     }
   }
   __syncthreads();
-  for (int row = warp; row < S * 64; row += 8) {
-    const int p = row >> 6, n = row & 63;
-    if (n0 + n < ncols) {
-      uint32_t* dst = reinterpret_cast<uint32_t*>(D + ((int64_t)p * ncols + n0 + n) * Mk + I * 128);
-      dst[lane] = sd[row * 33 + lane];
-    }
-  }
+  // rows (q, n) of this tile are consecutive 128-byte lines of D
+  uint32_t* dst = reinterpret_cast<uint32_t*>(D + (I * gridDim.y + blockIdx.y) * (int64_t)(S * 64 * 128));
+  for (int row = warp; row < S * 64; row += 8) dst[row * 32 + lane] = sd[row * 33 + lane];
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -129,12 +129,12 @@ ttdft_status make_map_hd(CUtensorMap* map, const void* base, uint64_t rows, uint
   if (r != CUDA_SUCCESS) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled(H digits) failed with CUresult %d", (int)r);
   return TTDFT_OK;
 }
-// Y digit planes: uint8 [S][ncols][Mk bytes], box = S x 64 x 128 B, 128B swizzle (columns beyond ncols read as 0)
-ttdft_status make_map_yd(CUtensorMap* map, const void* base, uint64_t Mk, uint64_t ncols, uint32_t S) {
+// Y digit tiles: uint8 [nb*nct*S][64 columns][128 k-bytes], box = S x 64 x 128 B, 128B swizzle
+ttdft_status make_map_yd(CUtensorMap* map, const void* base, uint64_t ntile_planes, uint32_t S) {
   encode_tiled_fn enc = get_encode();
   if (!enc) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
-  cuuint64_t dims[3] = {Mk, ncols, S};
-  cuuint64_t strides[2] = {Mk, Mk * ncols};
+  cuuint64_t dims[3] = {128, (cuuint64_t)ttdft::K3_NT, ntile_planes};
+  cuuint64_t strides[2] = {128, 128 * (cuuint64_t)ttdft::K3_NT};
   cuuint32_t box[3] = {128, (cuuint32_t)ttdft::K3_NT, S};
   cuuint32_t estr[3] = {1, 1, 1};
   CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(base), dims, strides, box, estr,
@@ -176,8 +176,11 @@ struct ttdft_h_s {
   const int8_t* Hd = nullptr;     // [nblocks][S][b][128]
   const int32_t* eH = nullptr;    // [M]
   const double* hdiag = nullptr;  // [M]
-  CUtensorMap tmHd;
+  CUtensorMap tmHd[4];      // box rows b, b/2, b/4, b/8: K3 in clusters of 1, 2, 4, 8 CTAs (every CTA fetches b/C rows of a plane)
   int32_t nsm = 148;
+  int32_t k3_cluster = 0;   // 0: choose per launch; 1, 2, 4, 8: forced (env TTDFT_K3_CLUSTER)
+  int32_t k3_cg = 0;        // column tiles per scheduling group of K3 (env TTDFT_K3_CG; 0: one cluster's tiles)
+  int32_t k3_max_clusters[4] = {0, 0, 0, 0};   // co-resident clusters of 1, 2, 4, 8 CTAs (filled at the first launch)
 };
 
 namespace {
@@ -332,15 +335,6 @@ __global__ void exclusive_scan_small(int64_t n, const int32_t* counts, int32_t* 
   }
 }
 
-// gather / copy helpers
-__global__ void copy2d_kernel(const double* __restrict__ src, int64_t lds, double* __restrict__ dst, int64_t ldd,
-                              int64_t rows, int64_t cols) {
-  int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-  int64_t r = blockIdx.y;
-  for (; r < rows; r += gridDim.y)
-    if (c < cols) dst[r * ldd + c] = src[r * lds + c];
-}
-
 // ------------------------------------------------------------------------------------------------
 // fp64 peak probes
 // ------------------------------------------------------------------------------------------------
@@ -488,27 +482,103 @@ int i8_planes_in_use(const ttdft_h_s* h) {
   return 0;
 }
 bool want_i8(const ttdft_h_s* h) { return i8_planes_in_use(h) > 0; }
-size_t i8_work_bytes(const ttdft_h_s* h, int64_t w) {
-  return align_up((size_t)i8_planes_in_use(h) * (size_t)w * (size_t)h->nb * 128, 1024) + 2 * align_up((size_t)w * 4, 1024);
+// digit tiles of one iterate: [nb][ceil(w/64)][planes][64][128] bytes
+size_t i8_digit_bytes(const ttdft_h_s* h, int64_t w) {
+  const size_t nct = (size_t)((w + ttdft::K3_NT - 1) / ttdft::K3_NT);
+  return align_up((size_t)i8_planes_in_use(h) * nct * ttdft::K3_NT * (size_t)h->nb * 128, 1024);
 }
+size_t i8_work_bytes(const ttdft_h_s* h, int64_t w) { return i8_digit_bytes(h, w) + 2 * align_up((size_t)w * 4, 1024); }
 I8Work carve_i8_work(const ttdft_h_s* h, void* base, int64_t w) {
   I8Work k;
   uint8_t* p = reinterpret_cast<uint8_t*>(base);
   k.D = reinterpret_cast<int8_t*>(p);
-  p += align_up((size_t)i8_planes_in_use(h) * (size_t)w * (size_t)h->nb * 128, 1024);
+  p += i8_digit_bytes(h, w);
   k.cmax[0] = reinterpret_cast<uint32_t*>(p);
   k.cmax[1] = reinterpret_cast<uint32_t*>(p + align_up((size_t)w * 4, 1024));
   return k;
 }
 
+// launch configuration of bsr_i8_kernel<S, C>: one CTA per SM (shared memory), clusters of C along the grid
+template <int S, int C>
+void k3_launch_config(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* at, unsigned grid, cudaStream_t st) {
+  *cfg = cudaLaunchConfig_t{};
+  cfg->gridDim = dim3(grid);
+  cfg->blockDim = dim3(ttdft::K3_THREADS);
+  cfg->dynamicSmemBytes = ttdft::K3Cfg<S>::TOTAL;
+  cfg->stream = st;
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg->attrs = at;
+  cfg->numAttrs = C > 1 ? 1 : 0;
+}
+
+// co-resident clusters of C CTAs of bsr_i8_kernel<S, C>, cached in the handle (same value whoever writes it)
+template <int S, int C>
+int k3_max_clusters(ttdft_h_s* h) {
+  constexpr int ci = C == 1 ? 0 : C == 2 ? 1 : C == 4 ? 2 : 3;
+  if (h->k3_max_clusters[ci] > 0) return h->k3_max_clusters[ci];
+  int n = h->nsm / C;
+  if (C > 1) {
+    auto kern = ttdft::bsr_i8_kernel<S, C>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ttdft::K3Cfg<S>::TOTAL) != cudaSuccess)
+      (void)cudaGetLastError();
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute at[1];
+    k3_launch_config<S, C>(&cfg, at, (unsigned)(h->nsm / C * C), nullptr);
+    int q = 0;
+    if (cudaOccupancyMaxActiveClusters(&q, kern, &cfg) == cudaSuccess && q > 0) n = std::min(n, q);
+    else (void)cudaGetLastError();
+  }
+  h->k3_max_clusters[ci] = std::max(n, 1);
+  if (env_int("TTDFT_DEBUG", 0))
+    fprintf(stderr, "[ttdft] K3<%d,%d>: %d co-resident clusters on %d SMs\n", S, C, h->k3_max_clusters[ci], h->nsm);
+  return h->k3_max_clusters[ci];
+}
+
+// one K3 launch over column tiles [ct_begin, ct_begin + nct_launch) in clusters of C CTAs (nct_launch % C == 0)
+template <int S, int C>
+ttdft_status launch_k3(ttdft_h_s* h, const CUtensorMap& tmYd, ttdft::K3Params p, int32_t ct_begin, int32_t nct_launch,
+                       cudaStream_t st) {
+  constexpr int ci = C == 1 ? 0 : C == 2 ? 1 : C == 4 ? 2 : 3;
+  auto kern = ttdft::bsr_i8_kernel<S, C>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ttdft::K3Cfg<S>::TOTAL));
+    attr_set = true;
+  }
+  const int maxc = k3_max_clusters<S, C>(h);
+  p.ct_begin = ct_begin;
+  p.nctg = nct_launch / C;
+  p.cgc = std::max(1, (h->k3_cg > 0 ? h->k3_cg : 8) / C);   // default: 8 column tiles per scheduling group
+  const int64_t items = (int64_t)h->nb * p.nctg;
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute at[1];
+  k3_launch_config<S, C>(&cfg, at, (unsigned)(std::min<int64_t>(items, maxc) * C), st);
+  TimedLaunch tl(3, st);
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, h->tmHd[ci], tmYd, p));
+  g_launches.fetch_add(1);
+  return TTDFT_OK;
+}
+
+// cluster size of K3: the widest of {4, 2, 1} that fits the tile height (b/C rows per CTA must be whole
+// 8-row swizzle atoms) and whose co-resident clusters still cover (nearly) every SM -- GPCs with an SM
+// count that is not a multiple of 4 leave SMs idle under 4-CTA clusters
+template <int S>
+int k3_pick_cluster(ttdft_h_s* h) {
+  if (h->k3_cluster == 1 || h->k3_cluster == 2 || h->k3_cluster == 4 || h->k3_cluster == 8) return h->k3_cluster;
+  const int floor_sms = h->nsm - h->nsm / 50;      // tolerate up to 2 % idle SMs
+  if (h->b % 32 == 0 && k3_max_clusters<S, 4>(h) * 4 >= floor_sms) return 4;
+  if (h->b % 16 == 0 && k3_max_clusters<S, 2>(h) * 2 >= floor_sms) return 2;
+  return 1;
+}
+
 // src: index of the cmax array that holds (have_src_max) or will hold the maxima of X; the other one
 // receives the maxima of O if want_out_max.
 template <int S>
-ttdft_status launch_step_i8_t(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
+ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
                               const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, const I8Work& w, int src,
                               bool have_src_max, bool want_out_max, cudaStream_t st) {
   if (h->M == 0) return TTDFT_OK;
-  const int64_t Mk = h->nb * 128;
   const unsigned nct = (unsigned)((ncols + ttdft::K3_NT - 1) / ttdft::K3_NT);
   uint32_t* cmS = w.cmax[src];
   uint32_t* cmO = want_out_max ? w.cmax[src ^ 1] : nullptr;
@@ -529,16 +599,16 @@ ttdft_status launch_step_i8_t(const ttdft_h_s* h, double alpha, double gamma, do
     }
     dim3 g((unsigned)h->nb, nct);
     TimedLaunch tl(4, st);
-    ttdft::y_digits_kernel<S><<<g, 256, smem, st>>>(X, ldx, h->b, ncols, cmS, w.D, Mk, cmO);
+    ttdft::y_digits_kernel<S><<<g, 256, smem, st>>>(X, ldx, h->b, ncols, cmS, w.D, cmO);
     CUDA_TRY(cudaGetLastError());
     g_launches.fetch_add(1);
   }
   CUtensorMap tmYd;
-  ttdft_status s = make_map_yd(&tmYd, w.D, (uint64_t)Mk, (uint64_t)ncols, (uint32_t)S);
+  ttdft_status s = make_map_yd(&tmYd, w.D, (uint64_t)h->nb * nct * S, (uint32_t)S);
   if (s != TTDFT_OK) return s;
   ttdft::K3Params p;
   p.brow_ptr = h->row_ptr; p.bcol = h->col;
-  p.nb = (int32_t)h->nb; p.b = h->b; p.nct = (int32_t)nct; p.cg = h->cg;
+  p.nb = (int32_t)h->nb; p.b = h->b; p.nct = (int32_t)nct;
   p.hplanes = h->i8_S;
   p.ncols = ncols;
   p.alpha = alpha; p.gamma = gamma; p.beta = beta;
@@ -546,21 +616,19 @@ ttdft_status launch_step_i8_t(const ttdft_h_s* h, double alpha, double gamma, do
   p.eH = h->eH; p.hdiag = h->hdiag; p.cmaxS = cmS; p.cmaxO = cmO;
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
-  using C3 = ttdft::K3Cfg<S>;
-  static bool attr3_set = false;
-  if (!attr3_set) {
-    CUDA_TRY(cudaFuncSetAttribute(ttdft::bsr_i8_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, C3::TOTAL));
-    attr3_set = true;
-  }
-  const int64_t tiles = (int64_t)h->nb * nct;
-  const unsigned grid = (unsigned)std::min<int64_t>(tiles, h->nsm);
-  TimedLaunch tl(3, st);
-  ttdft::bsr_i8_kernel<S><<<grid, ttdft::K3_THREADS, C3::TOTAL, st>>>(h->tmHd, tmYd, p);
-  CUDA_TRY(cudaGetLastError());
-  g_launches.fetch_add(1);
+  // column tiles in clusters of C; a remainder of < C tiles runs as single CTAs
+  int C = k3_pick_cluster<S>(h);
+  while (C > 1 && (h->b % (8 * C) != 0 || (int)nct < C)) C >>= 1;
+  const int32_t main_tiles = (int32_t)(nct / C * C);
+  if (C == 8) s = launch_k3<S, 8>(h, tmYd, p, 0, main_tiles, st);
+  else if (C == 4) s = launch_k3<S, 4>(h, tmYd, p, 0, main_tiles, st);
+  else if (C == 2) s = launch_k3<S, 2>(h, tmYd, p, 0, main_tiles, st);
+  else s = launch_k3<S, 1>(h, tmYd, p, 0, main_tiles, st);
+  if (s != TTDFT_OK) return s;
+  if (main_tiles < (int32_t)nct) return launch_k3<S, 1>(h, tmYd, p, main_tiles, (int32_t)nct - main_tiles, st);
   return TTDFT_OK;
 }
-ttdft_status launch_step_i8(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
+ttdft_status launch_step_i8(ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
                             const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, const I8Work& w, int src,
                             bool have_src_max, bool want_out_max, cudaStream_t st) {
   if (i8_planes_in_use(h) == 7)
@@ -595,7 +663,7 @@ int64_t default_panel(int64_t ncols) { return ncols < 4096 ? ncols : 4096; }
 
 // Run the m recurrence steps of one column panel (A2-A4, A6).  Xp: input panel (ldx), Yp: output
 // panel (ldy), W: scratch (ldw).  inplace: Xp == Yp.
-ttdft_status filter_panel(const ttdft_h_s* h, const double* Xp, int64_t ldx, double* Yp, int64_t ldy, double* W,
+ttdft_status filter_panel(ttdft_h_s* h, const double* Xp, int64_t ldx, double* Yp, int64_t ldy, double* W,
                           int64_t ldw, int64_t wc, int32_t m, double c, const double* alpha, const double* beta,
                           bool inplace, cudaStream_t st, const I8Work* i8 = nullptr) {
   if (m == 0) {
@@ -898,8 +966,13 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "H digit planes: %s", cudaGetErrorString(e)); }
     g_launches.fetch_add(2);
-    s = make_map_hd(&h->tmHd, Hd, (uint64_t)h->nblocks * I8_S * h->b, (uint32_t)h->b);
-    if (s != TTDFT_OK) { delete h; return s; }
+    for (int ci = 0; ci < 4; ++ci) {
+      if (h->b % (8 << ci)) continue;              // b/C rows must be whole 8-row swizzle atoms
+      s = make_map_hd(&h->tmHd[ci], Hd, (uint64_t)h->nblocks * I8_S * h->b, (uint32_t)(h->b >> ci));
+      if (s != TTDFT_OK) { delete h; return s; }
+    }
+    h->k3_cluster = env_int("TTDFT_K3_CLUSTER", 0);
+    h->k3_cg = env_int("TTDFT_K3_CG", 0);
     h->i8_S = I8_S; h->Hd = Hd; h->eH = eH; h->hdiag = hdiag;
     int dev = 0, nsm = 0;
     if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0)
