@@ -75,10 +75,18 @@ typedef enum { TTDFT_FMT_CSR = 0, TTDFT_FMT_BSR = 1 } ttdft_format;
  *        allowed and treated as values.  nnz < 2^31.
  *   BSR: row_ptr[M/block+1], col_idx[nblocks] block columns ascending per block row,
  *        values[nblocks*block*block], each block a row-major block x block tile.  M % block == 0.
- *   subdomain_of_row (CSR only, optional, may be NULL): subdomain label of every row.  If the labels
- *        are non-decreasing and every subdomain owns the same number b of rows, with b in
- *        {32, 64, 96, 128}, the builder groups each localized subdomain's basis functions into b x b
- *        tiles (block-sparse storage); otherwise the CSR is kept as is.
+ *   subdomain_of_row (CSR only, optional, may be NULL): subdomain label of every row.  If every subdomain
+ *        owns the same number b of rows, b in {32, 64, 96, 128}, the builder groups each localized
+ *        subdomain's basis functions into b x b tiles (block-sparse storage).  Two label layouts qualify:
+ *        (1) rows already grouped: labels strictly increasing from group to group (any integers);
+ *        (2) rows in ANY order: labels are the subdomain indices 0 .. M/b-1.  The builder then REORDERS:
+ *            reordered row L*b + r is the r-th row (in input order) labelled L, H is stored as the tiles of
+ *            P H P^T, and the handle keeps the row map.  The caller never sees the reordering: X and Y stay
+ *            in the caller's row order; ttdft_cheb_filter gathers each X panel into tile order once, runs
+ *            all m steps there, and scatters the result (two extra passes per panel, no extra scratch).
+ *            Single steps on such a handle: ttdft_*_ws gather/scatter through scratch; the calls without
+ *            scratch run the generic kernel through the row map.
+ *        Otherwise the CSR is kept as is.
  * All four arrays are DEVICE pointers; the struct itself is a HOST object.
  */
 typedef struct {
@@ -102,6 +110,8 @@ typedef struct {
   size_t storage_bytes;
   int32_t i8_planes;      /* digit planes per operand of H stored for the I8 modes (0: not built) */
   int32_t math;           /* TTDFT_MATH_FP64, _I8 or _I8X7: what calls that take `work` use */
+  int32_t reordered;      /* 1: rows were regrouped by subdomain label (the handle keeps the row map) */
+  int32_t reserved;
 } ttdft_h_info_t;
 
 /* A0 -- storage builder (north_star "BSR/CSR storage builder"). */
@@ -148,7 +158,8 @@ ttdft_status ttdft_cheb_step(ttdft_h_t h, double alpha, double c, double beta, c
 /*
  * The same two operations with caller-provided scratch, which lets them run in the handle's math mode
  * (TTDFT_MATH_I8 needs room for the digit planes of X / Yk): `work` is a 16-byte aligned DEVICE
- * buffer of at least ttdft_step_work_bytes(h, ncols) bytes (0 in TTDFT_MATH_FP64: work may be NULL).
+ * buffer of at least ttdft_step_work_bytes(h, ncols) bytes (0 in TTDFT_MATH_FP64 on a handle that was not
+ * reordered: work may be NULL; a reordered handle adds two M x ncols panels in tile order).
  */
 ttdft_status ttdft_step_work_bytes(ttdft_h_t h, int64_t ncols, size_t* bytes);
 ttdft_status ttdft_spmm_ws(ttdft_h_t h, double alpha, const double* X, int64_t ldx, double beta, double* Y,

@@ -37,7 +37,7 @@ class _Desc(ctypes.Structure):
 
 class _Info(ctypes.Structure):
     _fields_ = [("M", c_int64), ("nnz_stored", c_int64), ("block", c_int32), ("kernel", c_int32), ("nblocks", c_int64),
-                ("storage_bytes", c_size_t), ("i8_planes", c_int32), ("math", c_int32)]
+                ("storage_bytes", c_size_t), ("i8_planes", c_int32), ("math", c_int32), ("reordered", c_int32), ("reserved", c_int32)]
 
 
 _lib = None

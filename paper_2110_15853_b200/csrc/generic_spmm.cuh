@@ -23,6 +23,7 @@ struct K2Params {
   const double* X; int64_t ldx;     // the multiplied block (Y_k)
   const double* Z; int64_t ldz;     // Y_{k-1} / Y, read at the output position if beta != 0
   double* O; int64_t ldo;
+  const int32_t* perm;      // BSR handles built from permuted subdomain labels: row r of H is row perm[r] of X/Z/O (else NULL)
 };
 
 template <bool BSR>
@@ -30,6 +31,7 @@ __global__ void __launch_bounds__(32 * K2_ROWS) generic_step_kernel(const K2Para
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t row = (int64_t)blockIdx.x * K2_ROWS + warp;
   if (row >= p.M) return;
+  const int64_t urow = (BSR && p.perm) ? p.perm[row] : row;   // the caller's row
   const int64_t c0 = (int64_t)blockIdx.y * K2_TN + lane;
   double acc[K2_CPL];
   bool ok[K2_CPL];
@@ -42,13 +44,13 @@ __global__ void __launch_bounds__(32 * K2_ROWS) generic_step_kernel(const K2Para
       const int32_t rr = (int32_t)(row - I * p.b);
       for (int32_t q = p.row_ptr[I]; q < p.row_ptr[I + 1]; ++q) {
         const double* tile = p.val + ((size_t)q * p.b + rr) * p.b;
-        const double* xr = p.X + (int64_t)p.col[q] * p.b * p.ldx + c0;
+        const int64_t xrow0 = (int64_t)p.col[q] * p.b;
         for (int32_t s = 0; s < p.b; ++s) {
           const double h = __ldg(tile + s);
+          const double* xr = p.X + (p.perm ? (int64_t)p.perm[xrow0 + s] : xrow0 + s) * p.ldx + c0;
 #pragma unroll
           for (int c = 0; c < K2_CPL; ++c)
             if (ok[c]) acc[c] = fma(h, __ldg(xr + 32 * c), acc[c]);
-          xr += p.ldx;
         }
       }
     } else {
@@ -77,9 +79,9 @@ __global__ void __launch_bounds__(32 * K2_ROWS) generic_step_kernel(const K2Para
     if (!ok[c]) continue;
     const int64_t col = c0 + 32 * c;
     double v = p.alpha * acc[c];
-    if (use_s) v = fma(p.gamma, p.X[row * p.ldx + col], v);
-    if (use_z) v = fma(p.beta, p.Z[row * p.ldz + col], v);
-    p.O[row * p.ldo + col] = v;
+    if (use_s) v = fma(p.gamma, p.X[urow * p.ldx + col], v);
+    if (use_z) v = fma(p.beta, p.Z[urow * p.ldz + col], v);
+    p.O[urow * p.ldo + col] = v;
   }
 }
 

@@ -178,6 +178,7 @@ struct ttdft_h_s {
   const double* hdiag = nullptr;  // [M]
   CUtensorMap tmHd[4];      // box rows b, b/2, b/4, b/8: K3 in clusters of 1, 2, 4, 8 CTAs (every CTA fetches b/C rows of a plane)
   int32_t nsm = 148;
+  const int32_t* perm = nullptr;   // rows reordered by subdomain label: row r of the tiles is the caller's row perm[r]
   int32_t k3_cluster = 0;   // 0: choose per launch; 1, 2, 4, 8: forced (env TTDFT_K3_CLUSTER)
   int32_t k3_cg = 0;        // column tiles per scheduling group of K3 (env TTDFT_K3_CG; 0: one cluster's tiles)
   int32_t k3_max_clusters[4] = {0, 0, 0, 0};   // co-resident clusters of 1, 2, 4, 8 CTAs (filled at the first launch)
@@ -259,17 +260,70 @@ __global__ void hint_check_kernel(int64_t M, const int32_t* lab, int32_t b, int3
   if (i == g0 && i > 0 && !(lab[i] > lab[i - 1])) atomicOr(bad, 1);
 }
 
-// CSR -> BSR pass 1: one CTA per block row, bitmap of touched block columns -> count
-__global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_ptr, const int32_t* col, int32_t* counts,
-                                     int32_t nwords) {
+// ---- subdomain labels in arbitrary row order (A0 reorder): labels must be the subdomain indices 0..nb-1 ----
+// hist[L] = rows labelled L; flags |= 1 on a label outside [0, M)
+__global__ void label_hist_kernel(int64_t M, const int32_t* lab, int32_t* hist, int32_t* flags) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= M) return;
+  const int32_t L = lab[i];
+  if (L < 0 || L >= M) atomicOr(flags, 1);
+  else atomicAdd(&hist[L], 1);
+}
+// every subdomain 0..nb-1 must own exactly b rows
+__global__ void label_hist_check_kernel(int64_t nb, int32_t b, const int32_t* hist, int32_t* flags) {
+  int64_t L = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (L < nb && hist[L] != b) atomicOr(flags, 1);
+}
+// One CTA per subdomain L: ordered (stable, deterministic) compaction of the rows labelled L.
+// perm[L*b + rank] = row, inv[row] = L*b + rank.  blockDim = 256.
+__global__ void __launch_bounds__(256) label_perm_kernel(int64_t M, int32_t b, const int32_t* lab, int32_t* perm, int32_t* inv) {
+  __shared__ int32_t wsum[8];
+  __shared__ int32_t base_s;
+  const int32_t L = blockIdx.x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) base_s = 0;
+  __syncthreads();
+  for (int64_t i0 = 0; i0 < M; i0 += 256) {
+    const int64_t i = i0 + threadIdx.x;
+    const bool hit = (i < M) && (lab[i] == L);
+    const uint32_t bal = __ballot_sync(0xffffffffu, hit);
+    if (lane == 0) wsum[warp] = __popc(bal);
+    __syncthreads();
+    int32_t before = base_s;
+    for (int w = 0; w < warp; ++w) before += wsum[w];
+    if (hit) {
+      const int32_t rank = before + __popc(bal & ((1u << lane) - 1u));
+      if (rank < b) {
+        perm[(int64_t)L * b + rank] = (int32_t)i;
+        inv[i] = L * b + rank;
+      }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int32_t t = 0;
+      for (int w = 0; w < 8; ++w) t += wsum[w];
+      base_s += t;
+    }
+    __syncthreads();
+  }
+}
+
+// CSR -> BSR pass 1: one CTA per block row (of the reordered matrix), bitmap of touched block columns -> count.
+// perm/inv: reordered row r is input row perm[r], input column j is reordered column inv[j] (NULL: identity).
+__global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_ptr, const int32_t* col, const int32_t* perm,
+                                     const int32_t* inv, int32_t* counts, int32_t nwords) {
   extern __shared__ uint32_t bits[];
   for (int w = threadIdx.x; w < nwords; w += blockDim.x) bits[w] = 0;
   __syncthreads();
-  int64_t I = blockIdx.x;
-  int32_t e0 = row_ptr[I * b], e1 = row_ptr[(I + 1) * b];
-  for (int32_t e = e0 + threadIdx.x; e < e1; e += blockDim.x) {
-    int32_t J = col[e] / b;
-    atomicOr(&bits[J >> 5], 1u << (J & 31));
+  const int64_t I = blockIdx.x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+  for (int32_t r = warp; r < b; r += nwarps) {
+    const int64_t row = perm ? perm[I * b + r] : I * b + r;
+    for (int32_t e = row_ptr[row] + lane; e < row_ptr[row + 1]; e += 32) {
+      const int32_t j = inv ? inv[col[e]] : col[e];
+      const int32_t J = j / b;
+      atomicOr(&bits[J >> 5], 1u << (J & 31));
+    }
   }
   __syncthreads();
   int32_t c = 0;
@@ -285,17 +339,22 @@ __global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_p
 
 // pass 2: fill bcol (ascending) and scatter the entries into zero-initialised tiles
 __global__ void csr2bsr_fill_kernel(int64_t nb, int32_t b, const int32_t* row_ptr, const int32_t* col, const double* val,
-                                    const int32_t* brow_ptr, int32_t* bcol, double* tiles, int32_t nwords) {
+                                    const int32_t* perm, const int32_t* inv, const int32_t* brow_ptr, int32_t* bcol,
+                                    double* tiles, int32_t nwords) {
   extern __shared__ uint32_t sm[];
   uint32_t* bits = sm;                    // nwords
   uint32_t* pref = sm + nwords;           // nwords: tiles before word w
   for (int w = threadIdx.x; w < nwords; w += blockDim.x) bits[w] = 0;
   __syncthreads();
-  int64_t I = blockIdx.x;
-  int32_t e0 = row_ptr[I * b], e1 = row_ptr[(I + 1) * b];
-  for (int32_t e = e0 + threadIdx.x; e < e1; e += blockDim.x) {
-    int32_t J = col[e] / b;
-    atomicOr(&bits[J >> 5], 1u << (J & 31));
+  const int64_t I = blockIdx.x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+  for (int32_t r = warp; r < b; r += nwarps) {
+    const int64_t row = perm ? perm[I * b + r] : I * b + r;
+    for (int32_t e = row_ptr[row] + lane; e < row_ptr[row + 1]; e += 32) {
+      const int32_t j = inv ? inv[col[e]] : col[e];
+      const int32_t J = j / b;
+      atomicOr(&bits[J >> 5], 1u << (J & 31));
+    }
   }
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -314,16 +373,27 @@ __global__ void csr2bsr_fill_kernel(int64_t nb, int32_t b, const int32_t* row_pt
     }
   }
   // rows of this block row: scatter entries
-  for (int32_t r = 0; r < b; ++r) {
-    int64_t row = I * b + r;
-    for (int32_t e = row_ptr[row] + threadIdx.x; e < row_ptr[row + 1]; e += blockDim.x) {
-      int32_t j = col[e];
-      int32_t J = j / b;
-      uint32_t w = bits[J >> 5] & ((1u << (J & 31)) - 1u);
-      int32_t p = p0 + (int32_t)(pref[J >> 5] + __popc(w));
+  for (int32_t r = warp; r < b; r += nwarps) {
+    const int64_t row = perm ? perm[I * b + r] : I * b + r;
+    for (int32_t e = row_ptr[row] + lane; e < row_ptr[row + 1]; e += 32) {
+      const int32_t j = inv ? inv[col[e]] : col[e];
+      const int32_t J = j / b;
+      const uint32_t w = bits[J >> 5] & ((1u << (J & 31)) - 1u);
+      const int32_t p = p0 + (int32_t)(pref[J >> 5] + __popc(w));
       tiles[((size_t)p * b + r) * b + (j - J * b)] = val[e];
     }
   }
+}
+
+// rows of a panel through a row map:  scatter == 0: dst[r, :] = src[map[r], :];  else dst[map[r], :] = src[r, :]
+__global__ void __launch_bounds__(256) permute_rows_kernel(const double* __restrict__ src, int64_t lds, double* __restrict__ dst,
+                                                           int64_t ldd, int64_t rows, int64_t cols,
+                                                           const int32_t* __restrict__ map, int scatter) {
+  const int64_t r = blockIdx.x;
+  const int64_t m = map[r];
+  const double* s = src + (scatter ? r : m) * lds;
+  double* d = dst + (scatter ? m : r) * ldd;
+  for (int64_t c = (int64_t)blockIdx.y * 1024 + threadIdx.x; c < min(cols, ((int64_t)blockIdx.y + 1) * 1024); c += 256) d[c] = s[c];
 }
 
 __global__ void exclusive_scan_small(int64_t n, const int32_t* counts, int32_t* out) {
@@ -434,11 +504,15 @@ ttdft_status launch_k1_any(const ttdft_h_s* h, double alpha, double gamma, doubl
   return fail(TTDFT_ERR_UNSUPPORTED, "tile size %d has no block-sparse kernel", h->b);
 }
 
+// user_rows: X, Z, O are in the caller's row order (matters for handles whose rows were reordered by label:
+// those run the generic kernel through the row map; the tile kernels work on buffers in tile order)
 ttdft_status launch_step(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
-                         const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, cudaStream_t st) {
+                         const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, cudaStream_t st,
+                         bool user_rows = false) {
   if (h->M == 0) return TTDFT_OK;
+  const int32_t* perm = user_rows ? h->perm : nullptr;
   const bool tma_ok = (reinterpret_cast<uintptr_t>(X) & 15) == 0 && (ldx % 2 == 0) && alpha != 0.0;
-  if (h->kernel == 1 && tma_ok) {
+  if (h->kernel == 1 && tma_ok && !perm) {
     // full 128-column tiles first, then one narrower launch for a remainder of <= 64 columns
     const int64_t rem = ncols % 128;
     if (ncols > 128 && rem != 0 && rem <= 64) {
@@ -454,6 +528,7 @@ ttdft_status launch_step(const ttdft_h_s* h, double alpha, double gamma, double 
   p.M = h->M; p.b = h->b; p.ncols = ncols;
   p.alpha = alpha; p.gamma = gamma; p.beta = beta;
   p.X = X; p.ldx = ldx; p.Z = Z; p.ldz = ldz; p.O = O; p.ldo = ldo;
+  p.perm = perm;
   dim3 grid((unsigned)((h->M + ttdft::K2_ROWS - 1) / ttdft::K2_ROWS), (unsigned)((ncols + ttdft::K2_TN - 1) / ttdft::K2_TN));
   if (grid.y > 65535) return fail(TTDFT_ERR_UNSUPPORTED, "ncols too large for the generic kernel");
   TimedLaunch tl(2, st);
@@ -560,13 +635,15 @@ ttdft_status launch_k3(ttdft_h_s* h, const CUtensorMap& tmYd, ttdft::K3Params p,
   return TTDFT_OK;
 }
 
-// cluster size of K3: the widest of {4, 2, 1} that fits the tile height (b/C rows per CTA must be whole
-// 8-row swizzle atoms) and whose co-resident clusters still cover (nearly) every SM -- GPCs with an SM
-// count that is not a multiple of 4 leave SMs idle under 4-CTA clusters
+// Cluster size of K3: the widest of {4, 2, 1} whose co-resident clusters still cover at least 98 % of the SMs
+// (b/C rows per CTA must be whole 8-row swizzle atoms).  On B200 only 33 four-CTA clusters are co-resident
+// (132 of 148 SMs: GPCs whose SM count is not a multiple of 4 leave SMs idle), so this picks 2.  Measured on
+// config 3 (profiles/r01b_*): at the board's power limit, where the filter runs, C = 2 / 4 / 8 take the same
+// time within 3 % (fewer SMs clock higher); with free clocks (one launch under ncu) C = 2 is 10 % faster.
 template <int S>
 int k3_pick_cluster(ttdft_h_s* h) {
   if (h->k3_cluster == 1 || h->k3_cluster == 2 || h->k3_cluster == 4 || h->k3_cluster == 8) return h->k3_cluster;
-  const int floor_sms = h->nsm - h->nsm / 50;      // tolerate up to 2 % idle SMs
+  const int floor_sms = h->nsm - h->nsm / 50;
   if (h->b % 32 == 0 && k3_max_clusters<S, 4>(h) * 4 >= floor_sms) return 4;
   if (h->b % 16 == 0 && k3_max_clusters<S, 2>(h) * 2 >= floor_sms) return 2;
   return 1;
@@ -661,6 +738,24 @@ ttdft_status check_scalars(int32_t m, double a, double b, double a0) {
 
 int64_t default_panel(int64_t ncols) { return ncols < 4096 ? ncols : 4096; }
 
+ttdft_status launch_permute(const double* src, int64_t lds, double* dst, int64_t ldd, int64_t rows, int64_t cols,
+                            const int32_t* map, int scatter, cudaStream_t st) {
+  if (rows == 0 || cols == 0) return TTDFT_OK;
+  dim3 grid((unsigned)rows, (unsigned)((cols + 1023) / 1024));
+  permute_rows_kernel<<<grid, 256, 0, st>>>(src, lds, dst, ldd, rows, cols, map, scatter);
+  CUDA_TRY(cudaGetLastError());
+  g_launches.fetch_add(1);
+  return TTDFT_OK;
+}
+
+// one step on buffers in tile order, by the handle's math mode
+ttdft_status panel_step(ttdft_h_s* h, double al, double ga, double be, const double* S, int64_t lds, const double* Z, int64_t ldz,
+                        double* O, int64_t ldo, int64_t wc, const I8Work* i8, int k, int m, cudaStream_t st) {
+  if (i8)   // column maxima of iterate k-1 live in cmax[(k-1)&1]; the epilogue leaves those of iterate k in the other
+    return launch_step_i8(h, al, ga, be, S, lds, Z, ldz, O, ldo, wc, *i8, (k - 1) & 1, k > 1, k < m, st);
+  return launch_step(h, al, ga, be, S, lds, Z, ldz, O, ldo, wc, st);
+}
+
 // Run the m recurrence steps of one column panel (A2-A4, A6).  Xp: input panel (ldx), Yp: output
 // panel (ldy), W: scratch (ldw).  inplace: Xp == Yp.
 ttdft_status filter_panel(ttdft_h_s* h, const double* Xp, int64_t ldx, double* Yp, int64_t ldy, double* W,
@@ -669,6 +764,26 @@ ttdft_status filter_panel(ttdft_h_s* h, const double* Xp, int64_t ldx, double* Y
   if (m == 0) {
     if (!inplace) return launch_copy2d(Xp, ldx, Yp, ldy, h->M, wc, st);
     return TTDFT_OK;
+  }
+  ttdft_status s;
+  if (h->perm) {
+    // Rows reordered by subdomain label (A0): gather X into tile order, run all m steps there between W and
+    // the Y panel (Y_{k+1} overwrites Y_{k-1}), and scatter the last iterate back.  Iterate k sits in buf[k&1];
+    // the last one must end in W so that the scatter into Yp is out of place.
+    const bool w_first = inplace || (m % 2 == 0);
+    double* buf[2] = {w_first ? W : Yp, w_first ? Yp : W};
+    const int64_t ldb[2] = {w_first ? ldw : ldy, w_first ? ldy : ldw};
+    if ((s = launch_permute(Xp, ldx, buf[0], ldb[0], h->M, wc, h->perm, 0, st)) != TTDFT_OK) return s;
+    for (int k = 1; k <= m; ++k) {
+      const int o = k & 1;
+      const double al = alpha[k - 1], be = (k == 1) ? 0.0 : beta[k - 1];
+      s = panel_step(h, al, -al * c, be, buf[o ^ 1], ldb[o ^ 1], k >= 2 ? buf[o] : nullptr, ldb[o], buf[o], ldb[o], wc, i8, k, m, st);
+      if (s != TTDFT_OK) return s;
+    }
+    if (buf[m & 1] != W) {   // in place with odd m: the result sits in Yp in tile order
+      if ((s = launch_copy2d(Yp, ldy, W, ldw, h->M, wc, st)) != TTDFT_OK) return s;
+    }
+    return launch_permute(W, ldw, Yp, ldy, h->M, wc, h->perm, 1, st);
   }
   // destination of step k (1-based).  Out of place: Y_m lands in Yp, the iterates alternate Yp / W and
   // Y_{k+1} overwrites Y_{k-1} (read only at the output position).  In place: even steps land in Yp.
@@ -686,11 +801,7 @@ ttdft_status filter_panel(ttdft_h_s* h, const double* Xp, int64_t ldx, double* Y
     if (k == 2) { Z = Xp; ldz = ldx; }
     else if (k > 2) { Z = dest(k - 2, &ldz); }
     const double al = alpha[k - 1], be = (k == 1) ? 0.0 : beta[k - 1];
-    ttdft_status s;
-    if (i8)   // column maxima of iterate k-1 live in cmax[(k-1)&1]; the epilogue leaves those of iterate k in the other
-      s = launch_step_i8(h, al, -al * c, be, S, lds, Z, ldz, O, ldo, wc, *i8, (k - 1) & 1, k > 1, k < m, st);
-    else
-      s = launch_step(h, al, -al * c, be, S, lds, Z, ldz, O, ldo, wc, st);
+    s = panel_step(h, al, -al * c, be, S, lds, Z, ldz, O, ldo, wc, i8, k, m, st);
     if (s != TTDFT_OK) return s;
   }
   if (inplace && (m % 2 == 1)) return launch_copy2d(W, ldw, Yp, ldy, h->M, wc, st);
@@ -754,33 +865,55 @@ static ttdft_status desc_counts(const ttdft_h_desc* d, int64_t* nrows_idx, int64
 }
 
 // decide the device format; for CSR + usable hint returns the tile size in *hint_b (else 0)
-static ttdft_status plan_format(const ttdft_h_desc* d, int32_t* hint_b) {
+// Decide the device format.  For CSR + usable subdomain labels: *hint_b = tile size (else 0) and *permuted tells
+// whether the rows have to be reordered (labels not already grouped).
+static ttdft_status plan_format(const ttdft_h_desc* d, int32_t* hint_b, bool* permuted) {
   *hint_b = 0;
+  *permuted = false;
   if (d->fmt != TTDFT_FMT_CSR || !d->subdomain_of_row || (d->flags & TTDFT_FORCE_GENERIC) || d->M == 0) return TTDFT_OK;
-  // group size = index of the first label change (read the labels' prefix from the device)
+  int32_t* bad = nullptr;
+  CUDA_TRY(cudaMalloc(&bad, 4));                         // 4-byte transient flag
+  struct Free { void* p; ~Free() { cudaFree(p); } } free_bad{bad};
+  // (1) labels already grouped: group size = index of the first label change
   std::vector<int32_t> lab((size_t)std::min<int64_t>(d->M, 129));
   CUDA_TRY(cudaMemcpy(lab.data(), d->subdomain_of_row, lab.size() * 4, cudaMemcpyDeviceToHost));
   size_t b = 1;
   while (b < lab.size() && lab[b] == lab[0]) ++b;
-  if (!k1_block_ok((int32_t)b) || d->M % (int64_t)b) return TTDFT_OK;
-  if (d->M / (int64_t)b > (1 << 17)) return TTDFT_OK;   // bitmap of block columns must fit shared memory
-  int32_t* bad = nullptr;
-  CUDA_TRY(cudaMalloc(&bad, 4));                         // 4-byte transient flag
-  cudaMemset(bad, 0, 4);
-  hint_check_kernel<<<(unsigned)((d->M + 255) / 256), 256>>>(d->M, d->subdomain_of_row, (int32_t)b, bad);
-  g_launches.fetch_add(1);
   int32_t hb = 1;
-  cudaError_t e = cudaMemcpy(&hb, bad, 4, cudaMemcpyDeviceToHost);
-  cudaFree(bad);
-  if (e != cudaSuccess) return fail(TTDFT_ERR_CUDA, "hint check: %s", cudaGetErrorString(e));
-  if (hb == 0) *hint_b = (int32_t)b;
+  if (k1_block_ok((int32_t)b) && d->M % (int64_t)b == 0 && d->M / (int64_t)b <= (1 << 17)) {   // bitmap of block columns must fit shared memory
+    CUDA_TRY(cudaMemset(bad, 0, 4));
+    hint_check_kernel<<<(unsigned)((d->M + 255) / 256), 256>>>(d->M, d->subdomain_of_row, (int32_t)b, bad);
+    g_launches.fetch_add(1);
+    CUDA_TRY(cudaMemcpy(&hb, bad, 4, cudaMemcpyDeviceToHost));
+    if (hb == 0) { *hint_b = (int32_t)b; return TTDFT_OK; }
+  }
+  // (2) labels in any row order: they must be the subdomain indices 0..nb-1, each owning the same number b of rows
+  int32_t* hist = nullptr;
+  CUDA_TRY(cudaMalloc(&hist, (size_t)d->M * 4));         // transient M-int histogram
+  Free free_hist{hist};
+  CUDA_TRY(cudaMemset(hist, 0, (size_t)d->M * 4));
+  CUDA_TRY(cudaMemset(bad, 0, 4));
+  label_hist_kernel<<<(unsigned)((d->M + 255) / 256), 256>>>(d->M, d->subdomain_of_row, hist, bad);
+  g_launches.fetch_add(1);
+  int32_t b0 = 0;
+  CUDA_TRY(cudaMemcpy(&b0, hist, 4, cudaMemcpyDeviceToHost));
+  CUDA_TRY(cudaMemcpy(&hb, bad, 4, cudaMemcpyDeviceToHost));
+  if (hb != 0 || !k1_block_ok(b0) || d->M % b0 || d->M / b0 > (1 << 17)) return TTDFT_OK;
+  const int64_t nb = d->M / b0;
+  label_hist_check_kernel<<<(unsigned)((nb + 255) / 256), 256>>>(nb, b0, hist, bad);
+  g_launches.fetch_add(1);
+  CUDA_TRY(cudaMemcpy(&hb, bad, 4, cudaMemcpyDeviceToHost));
+  if (hb != 0) return TTDFT_OK;
+  *hint_b = b0;
+  *permuted = true;
   return TTDFT_OK;
 }
 
-static ttdft_status csr2bsr_counts(const ttdft_h_desc* d, int32_t b, int32_t* dev_counts, cudaStream_t st) {
+static ttdft_status csr2bsr_counts(const ttdft_h_desc* d, int32_t b, const int32_t* perm, const int32_t* inv, int32_t* dev_counts,
+                                   cudaStream_t st) {
   const int64_t nb = d->M / b;
   const int32_t nwords = (int32_t)((nb + 31) / 32);
-  csr2bsr_count_kernel<<<(unsigned)nb, 256, (size_t)nwords * 4, st>>>(nb, b, d->row_ptr, d->col_idx, dev_counts, nwords);
+  csr2bsr_count_kernel<<<(unsigned)nb, 256, (size_t)nwords * 4, st>>>(nb, b, d->row_ptr, d->col_idx, perm, inv, dev_counts, nwords);
   CUDA_TRY(cudaGetLastError());
   g_launches.fetch_add(1);
   return TTDFT_OK;
@@ -793,14 +926,22 @@ static ttdft_status storage_bytes_impl(const ttdft_h_desc* d, size_t* bytes, siz
   ttdft_status s = desc_counts(d, &nidx, &nstored);
   if (s != TTDFT_OK) return s;
   int32_t hint_b;
-  s = plan_format(d, &hint_b);
+  bool permuted;
+  s = plan_format(d, &hint_b, &permuted);
   if (s != TTDFT_OK) return s;
   if (hint_b) {
-    // count the tiles the conversion will create (transient nb-int scratch)
+    // count the tiles the conversion will create (transient scratch: nb counts, and the row maps if reordering)
     const int64_t nb = d->M / hint_b;
     int32_t* cnt = nullptr;
-    CUDA_TRY(cudaMalloc(&cnt, (size_t)nb * 4));
-    s = csr2bsr_counts(d, hint_b, cnt, 0);
+    CUDA_TRY(cudaMalloc(&cnt, ((size_t)nb + (permuted ? 2 * (size_t)d->M : 0)) * 4));
+    int32_t *perm = nullptr, *inv = nullptr;
+    if (permuted) {
+      perm = cnt + nb;
+      inv = perm + d->M;
+      label_perm_kernel<<<(unsigned)nb, 256>>>(d->M, hint_b, d->subdomain_of_row, perm, inv);
+      g_launches.fetch_add(1);
+    }
+    s = csr2bsr_counts(d, hint_b, perm, inv, cnt, 0);
     std::vector<int32_t> hc((size_t)nb);
     cudaError_t e = cudaMemcpy(hc.data(), cnt, (size_t)nb * 4, cudaMemcpyDeviceToHost);
     cudaFree(cnt);
@@ -808,8 +949,9 @@ static ttdft_status storage_bytes_impl(const ttdft_h_desc* d, size_t* bytes, siz
     if (e != cudaSuccess) return fail(TTDFT_ERR_CUDA, "tile count: %s", cudaGetErrorString(e));
     int64_t nblocks = 0;
     for (int32_t c : hc) nblocks += c;
+    // brow_ptr | counts | bcol | tiles | (perm | inv)
     *bytes = align_up((size_t)(nb + 1) * 4, 1024) + align_up((size_t)nb * 4, 1024) + align_up((size_t)nblocks * 4, 1024) +
-             align_up((size_t)nblocks * hint_b * hint_b * 8, 1024);
+             align_up((size_t)nblocks * hint_b * hint_b * 8, 1024) + (permuted ? 2 * align_up((size_t)d->M * 4, 1024) : 0);
     if (!(d->flags & TTDFT_NO_I8) && nblocks > 0) *i8 = i8_storage_bytes(nblocks, hint_b, d->M);
     return TTDFT_OK;
   }
@@ -846,7 +988,8 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
   if (need > 0 && (!dev_storage || (reinterpret_cast<uintptr_t>(dev_storage) & 1023)))
     return fail(TTDFT_ERR_INVALID_ARG, "dev_storage must be a 1024-byte aligned device pointer");
   int32_t hint_b;
-  s = plan_format(d, &hint_b);
+  bool permuted;
+  s = plan_format(d, &hint_b, &permuted);
   if (s != TTDFT_OK) return s;
 
   // ---- validation on request (on the input arrays) ----
@@ -892,7 +1035,15 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     const int32_t nwords = (int32_t)((nb + 31) / 32);
     int32_t* brow = reinterpret_cast<int32_t*>(base);
     int32_t* counts = reinterpret_cast<int32_t*>(base + align_up((size_t)(nb + 1) * 4, 1024));
-    s = csr2bsr_counts(d, b, counts, st);
+    int32_t *perm = nullptr, *inv = nullptr;
+    if (permuted) {
+      // the row maps live at the end of the fp64 format: reordered row r is the caller's row perm[r]
+      inv = reinterpret_cast<int32_t*>(base + need - align_up((size_t)d->M * 4, 1024));
+      perm = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(inv) - align_up((size_t)d->M * 4, 1024));
+      label_perm_kernel<<<(unsigned)nb, 256, 0, st>>>(d->M, b, d->subdomain_of_row, perm, inv);
+      g_launches.fetch_add(1);
+    }
+    s = csr2bsr_counts(d, b, perm, inv, counts, st);
     if (s != TTDFT_OK) { delete h; return s; }
     exclusive_scan_small<<<1, 1, 0, st>>>(nb, counts, brow);
     g_launches.fetch_add(1);
@@ -904,11 +1055,12 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     double* tiles = reinterpret_cast<double*>(reinterpret_cast<uint8_t*>(bcol) + align_up((size_t)nblocks * 4, 1024));
     e = cudaMemsetAsync(tiles, 0, (size_t)nblocks * b * b * 8, st);
     if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "memset: %s", cudaGetErrorString(e)); }
-    csr2bsr_fill_kernel<<<(unsigned)nb, 256, (size_t)nwords * 8, st>>>(nb, b, d->row_ptr, d->col_idx, d->values, brow, bcol,
-                                                                       tiles, nwords);
+    csr2bsr_fill_kernel<<<(unsigned)nb, 256, (size_t)nwords * 8, st>>>(nb, b, d->row_ptr, d->col_idx, d->values, perm, inv, brow,
+                                                                       bcol, tiles, nwords);
     e = cudaGetLastError();
     if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "csr->bsr fill: %s", cudaGetErrorString(e)); }
     g_launches.fetch_add(1);
+    h->perm = perm;
     h->bsr = 1; h->b = b; h->nb = nb; h->nblocks = nblocks;
     h->row_ptr = brow; h->col = bcol; h->val = tiles;
     h->kernel = 1;
@@ -994,6 +1146,8 @@ ttdft_status ttdft_h_info(ttdft_h_t h, ttdft_h_info_t* info) {
   info->nnz_stored = h->bsr ? h->nblocks * (int64_t)h->b * h->b : h->nblocks;
   info->storage_bytes = h->storage_bytes;
   info->i8_planes = h->i8_S;
+  info->reordered = h->perm ? 1 : 0;
+  info->reserved = 0;
   const int used = i8_planes_in_use(h);
   info->math = used == 7 ? TTDFT_MATH_I8X7 : used == 6 ? TTDFT_MATH_I8 : TTDFT_MATH_FP64;
   return TTDFT_OK;
@@ -1029,7 +1183,7 @@ ttdft_status ttdft_spmm(ttdft_h_t h, double alpha, const double* X, int64_t ldx,
   if ((s = check_mat("X", X, ldx, ncols)) != TTDFT_OK) return s;
   if ((s = check_mat("Y", Y, ldy, ncols)) != TTDFT_OK) return s;
   if (overlaps(X, ldx, Y, ldy, h->M, ncols)) return fail(TTDFT_ERR_INVALID_ARG, "X overlaps Y");
-  return launch_step(h, alpha, 0.0, beta, X, ldx, Y, ldy, Y, ldy, ncols, (cudaStream_t)stream);
+  return launch_step(h, alpha, 0.0, beta, X, ldx, Y, ldy, Y, ldy, ncols, (cudaStream_t)stream, true);
 }
 
 ttdft_status ttdft_cheb_step(ttdft_h_t h, double alpha, double c, double beta, const double* Yk, int64_t ldk,
@@ -1044,25 +1198,52 @@ ttdft_status ttdft_cheb_step(ttdft_h_t h, double alpha, double c, double beta, c
   if (Ykm1 && !(Ykm1 == Yout && ldm == ldo) && overlaps(Ykm1, ldm, Yout, ldo, h->M, ncols))
     return fail(TTDFT_ERR_INVALID_ARG, "Ykm1 partially overlaps Yout");
   const double be = Ykm1 ? beta : 0.0;
-  return launch_step(h, alpha, -alpha * c, be, Yk, ldk, Ykm1, ldm, Yout, ldo, ncols, (cudaStream_t)stream);
+  return launch_step(h, alpha, -alpha * c, be, Yk, ldk, Ykm1, ldm, Yout, ldo, ncols, (cudaStream_t)stream, true);
+}
+
+// scratch of a single step: the digit planes of the multiplied block (int8 modes), and for handles whose rows
+// were reordered by label two panels in tile order (the multiplied block; the output, which also carries Z in)
+static size_t step_work_need(const ttdft_h_s* h, int64_t ncols, size_t* panel_bytes) {
+  const int64_t ldp = ncols + (ncols & 1);
+  *panel_bytes = h->perm ? align_up((size_t)h->M * (size_t)ldp * 8, 1024) : 0;
+  return 2 * *panel_bytes + (want_i8(h) ? i8_work_bytes(h, ncols) : 0);
 }
 
 ttdft_status ttdft_step_work_bytes(ttdft_h_t h, int64_t ncols, size_t* bytes) {
   if (!h || !bytes) return fail(TTDFT_ERR_INVALID_ARG, "NULL argument");
   if (ncols < 1) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1");
-  *bytes = want_i8(h) ? i8_work_bytes(h, ncols) : 0;
+  size_t pb;
+  *bytes = step_work_need(h, ncols, &pb);
   return TTDFT_OK;
 }
 
 // one step with scratch: the int8 tensor-core kernel if the handle's math mode selects it
 static ttdft_status step_ws(ttdft_h_t h, double alpha, double gamma, double beta, const double* X, int64_t ldx, const double* Z,
                             int64_t ldz, double* O, int64_t ldo, int64_t ncols, void* work, size_t work_bytes, cudaStream_t st) {
-  if (!want_i8(h) || alpha == 0.0 || h->M == 0) return launch_step(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
-  const size_t need = i8_work_bytes(h, ncols);
+  if (alpha == 0.0 || h->M == 0 || (!want_i8(h) && !h->perm))
+    return launch_step(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st, true);
+  size_t pb;
+  const size_t need = step_work_need(h, ncols, &pb);
   if (work_bytes < need) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, need);
   if (!work || (reinterpret_cast<uintptr_t>(work) & 15)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 16-byte aligned device pointer");
-  const I8Work k3 = carve_i8_work(h, work, ncols);
-  return launch_step_i8(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, k3, 0, false, false, st);
+  uint8_t* wb = reinterpret_cast<uint8_t*>(work);
+  I8Work k3;
+  if (want_i8(h)) k3 = carve_i8_work(h, wb + 2 * pb, ncols);
+  if (!h->perm) return launch_step_i8(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, k3, 0, false, false, st);
+  // reordered rows: gather the operands into tile order, step there, scatter the result back
+  const int64_t ldp = ncols + (ncols & 1);
+  double* Xt = reinterpret_cast<double*>(wb);
+  double* Ot = reinterpret_cast<double*>(wb + pb);
+  ttdft_status s = launch_permute(X, ldx, Xt, ldp, h->M, ncols, h->perm, 0, st);
+  if (s != TTDFT_OK) return s;
+  const bool use_z = (beta != 0.0) && Z;
+  if (use_z && (s = launch_permute(Z, ldz, Ot, ldp, h->M, ncols, h->perm, 0, st)) != TTDFT_OK) return s;
+  if (want_i8(h))
+    s = launch_step_i8(h, alpha, gamma, use_z ? beta : 0.0, Xt, ldp, use_z ? Ot : nullptr, ldp, Ot, ldp, ncols, k3, 0, false, false, st);
+  else
+    s = launch_step(h, alpha, gamma, use_z ? beta : 0.0, Xt, ldp, use_z ? Ot : nullptr, ldp, Ot, ldp, ncols, st);
+  if (s != TTDFT_OK) return s;
+  return launch_permute(Ot, ldp, O, ldo, h->M, ncols, h->perm, 1, st);
 }
 
 ttdft_status ttdft_spmm_ws(ttdft_h_t h, double alpha, const double* X, int64_t ldx, double beta, double* Y, int64_t ldy,

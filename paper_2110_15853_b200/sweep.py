@@ -1,7 +1,8 @@
 """BASELINE.json config 5: a single H*X (ttdft_spmm) and a single fused recurrence step
 (ttdft_cheb_step) on config 3's H at N in {16, 64, 256, 1024, 4096}, in two layouts --
 subdomain-ordered BSR and CSR with rows/columns symmetrically permuted by seed (irregular-access
-stress) -- each reported against the binding roofline:
+stress; once as given -> generic kernel, once with the subdomain index of every row -> h_build regroups the rows
+into tiles and the *_ws calls gather / scatter around the tile kernel) -- each reported against the binding roofline:
     T_roof = max(alg_bytes / BW_hbm, useful_flops / P_fp64).
 The BSR layout runs three times: fp64 tensor-core MMA (kernel 1) and int8 digit planes (kernel 3 with 7 and 6 planes, through
 the *_ws entry points; its time includes the digit extraction of X); roofline_frac > 1 there means
@@ -56,7 +57,7 @@ def time_launches(fn, reps, flush):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--workload", default="si")
-    ap.add_argument("--layouts", default="bsr,csr")
+    ap.add_argument("--layouts", default="bsr,csr,csr+labels")
     ap.add_argument("--ns", default="16,64,256,1024,4096")
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--csr-max-n", type=int, default=4096)
@@ -82,9 +83,16 @@ def main():
         perm = synth.permutation(H.M, cfg.seed + 50)
         Cp = synth.permute_csr(C, perm)
         del C
-        handles["csr"] = tt.h_build_csr(Cp.M, torch.from_numpy(Cp.row_ptr).to(dev), torch.from_numpy(Cp.col_idx).to(dev),
-                                        torch.from_numpy(Cp.values).to(dev))
-        del Cp
+        rp_d, ci_d, va_d = (torch.from_numpy(Cp.row_ptr).to(dev), torch.from_numpy(Cp.col_idx).to(dev),
+                            torch.from_numpy(Cp.values).to(dev))
+        handles["csr"] = tt.h_build_csr(Cp.M, rp_d, ci_d, va_d)
+        if "csr+labels" in args.layouts:
+            # the same permuted CSR plus the subdomain index of every row: h_build regroups the rows into tiles (A0)
+            labels = np.empty(Cp.M, np.int32)
+            labels[perm] = (np.arange(Cp.M) // cfg.b).astype(np.int32)
+            handles["csr+labels-i8x7"] = tt.h_build_csr(Cp.M, rp_d, ci_d, va_d, subdomain_of_row=torch.from_numpy(labels).to(dev))
+            assert handles["csr+labels-i8x7"].info()["reordered"] == 1
+        del Cp, rp_d, ci_d, va_d
     maths = args.math.split(",")
     if "bsr" in handles and handles["bsr"].info()["i8_planes"]:
         # the same handle through the int8 digit-plane kernel (ttdft_*_ws entry points), 7 and 6 planes
@@ -103,10 +111,11 @@ def main():
         for layout, Hd in handles.items():
             if layout == "csr" and N > args.csr_max_n:
                 continue
-            i8 = layout.startswith("bsr-i8")
+            i8 = layout.endswith("-i8") or layout.endswith("-i8x7")
             work = None
-            if layout.startswith("bsr"):
-                Hd.set_math_mode({"bsr": tt.MATH_FP64, "bsr-i8": tt.MATH_I8, "bsr-i8x7": tt.MATH_I8X7}[layout])
+            if layout != "csr":
+                Hd.set_math_mode({"bsr": tt.MATH_FP64, "bsr-i8": tt.MATH_I8, "bsr-i8x7": tt.MATH_I8X7,
+                                  "csr+labels-i8x7": tt.MATH_I8X7}[layout])
             if i8:
                 work = torch.empty(tt.step_work_bytes(Hd, N) + 16, dtype=torch.uint8, device=dev)
             for op in ("spmm", "step"):
