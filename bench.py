@@ -193,6 +193,7 @@ def main():
     ap.add_argument("--no-other-modes", action="store_true", help="skip the short runs of the other math modes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-project", action="store_true", help="skip the subspace-projection (NEXT-1) measurement")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -379,6 +380,50 @@ def main():
             del w2
         Hd.set_math_mode(MODES[args.math])
         line["other_math_modes"] = others
+
+    # ---- NEXT-1: subspace projection H_F = X^T (H X) on the same handle and X (1 warm-up + 2 timed) ----
+    if rank == 0 and world == 1 and not args.no_project:
+        Gd = torch.empty((cfg.N, cfg.N), dtype=torch.float64, device=dev)
+        pw = torch.empty(tt.project_work_bytes(Hd, cfg.N) + 1024, dtype=torch.uint8, device=dev)
+        tt.project(Hd, Xd, Gd, work=pw)
+        torch.cuda.synchronize()
+        for k in tt.KERNEL_IDS:
+            tt.timing_read(k)
+        tt.timing_enable(True)
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record()
+        for _ in range(2):
+            tt.project(Hd, Xd, Gd, work=pw)
+        g1.record()
+        torch.cuda.synchronize()
+        tt.timing_enable(False)
+        pk = {k: tt.timing_read(k) for k in tt.KERNEL_IDS}
+        t_p = g0.elapsed_time(g1) * 1e-3 / 2
+        gram_ms = pk["gram_i8"][0] / max(pk["gram_i8"][1], 1)
+        fl_gram, fl_spmm = 2.0 * cfg.M * cfg.N * cfg.N, 2.0 * nnz * cfg.N
+        peak8, peak8_src = int8_peak_tops()
+        ops_gram = 28.0 * fl_gram
+        line["project"] = {
+            "what": "H_F = X^T (H X), Algorithm 1 step 3 (ttdft_project): one K3 step + Gram product K4 on the int8 tensor cores",
+            "ms": t_p * 1e3, "useful_tflops": (fl_gram + fl_spmm) / t_p / 1e12, "steps": 2, "warmup": 1,
+            "kernels_ms_each": {k: v[0] / v[1] for k, v in pk.items() if v[1]},
+            "gram_roofline": {"bound": "tensor", "achieved": ops_gram / (gram_ms * 1e-3) / 1e12, "peak": peak8, "unit": "TFLOP/s",
+                              "frac": ops_gram / (gram_ms * 1e-3) / 1e12 / peak8, "peak_source": peak8_src, "launch_ms": gram_ms,
+                              "fp64_equivalent_tflops": fl_gram / (gram_ms * 1e-3) / 1e12,
+                              "fp64_equivalent_frac_of_fp64_peak": fl_gram / (gram_ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS},
+            "symmetry_defect": float(((Gd - Gd.T).norm() / Gd.norm()).item()),
+        }
+        if not args.no_cpu_baseline:
+            # oracle on a seeded sub-block: G[cols, cols] = X_c^T (H X_c) (entry (j,l) depends on columns j and l only)
+            import oracle
+            pc = synth.column_sample(cfg.N, cfg.panel, args.ref_cols, cfg.seed)
+            Cn = synth.bsr_to_csr_nonzeros(H)
+            Xc = np.ascontiguousarray(Xd[:, torch.from_numpy(pc).to(dev)].cpu().numpy())
+            ref = oracle.project(Cn.row_ptr, Cn.col_idx, Cn.values, Xc)
+            gotp = Gd[torch.from_numpy(pc).to(dev)][:, torch.from_numpy(pc).to(dev)].cpu().numpy()
+            line["project"]["gpu_vs_oracle_relerr_on_sample"] = float(np.linalg.norm(gotp - ref) / np.linalg.norm(ref))
+            del Cn
+        del Gd, pw
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         dt, _, cols, Xs, Yo, threads = oracle_sample_run(cfg, H, args.ref_cols, cfg.m, (a, b, a0))

@@ -205,6 +205,28 @@ ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* X_host, int64_t l
                                     int64_t ncols, int32_t m, double a, double b, double a0, int64_t panel_cols,
                                     void* work, size_t work_bytes, void* stream);
 
+/*
+ * NEXT-1 -- subspace projection, Algorithm 1 step 3 (Sec. 4.3):
+ *     H_F = X_F^T (H X_F)
+ * "The evaluation of H_F includes a matrix-matrix multiplication between H and X_F ... this matrix is ...
+ * left-multiplied with X^T" (the paper does the second product on the host with PETSc; here both run on the GPU).
+ *
+ * ttdft_gram:     G = X^T W, X and W row-major M x ncols (M >= 0), G row-major ncols x ncols with ldg >= ncols.
+ *                 Computed exactly from 7 int8 digit planes per operand (55 bits below each column's maximum) on the
+ *                 tensor cores with int32 accumulation over chunks of <= 128*128 rows, the chunks then summed in
+ *                 ascending order in fp64: deterministic, error below an fp64 dot product's bound (K4).
+ *                 X and W may be the same matrix; G must not overlap them.  ncols <= 65535.
+ * ttdft_project:  G = X^T (H X): one ttdft_spmm_ws into scratch, then ttdft_gram.  G is symmetric up to rounding
+ *                 when H is; it is NOT symmetrised.
+ * `work`: 1024-byte aligned DEVICE scratch of at least the bytes the matching *_work_bytes call reports.
+ */
+ttdft_status ttdft_gram_work_bytes(int64_t M, int64_t ncols, size_t* bytes);
+ttdft_status ttdft_gram(int64_t M, const double* X, int64_t ldx, const double* W, int64_t ldw, int64_t ncols, double* G,
+                        int64_t ldg, void* work, size_t work_bytes, void* stream);
+ttdft_status ttdft_project_work_bytes(ttdft_h_t h, int64_t ncols, size_t* bytes);
+ttdft_status ttdft_project(ttdft_h_t h, const double* X, int64_t ldx, int64_t ncols, double* G, int64_t ldg, void* work,
+                           size_t work_bytes, void* stream);
+
 /* Measured fp64 rate of this GPU: kind 0 = scalar DFMA loop, 1 = DMMA (mma.sync m8n8k4.f64) loop;
  * runs for about `millis` ms on `stream`, synchronises, returns TFLOP/s in *tflops. */
 ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, double* tflops);
@@ -214,7 +236,8 @@ ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, d
  * bracketed by a CUDA event pair on the launching stream; ttdft_timing_read waits for the events of
  * one kernel, returns the sum of their durations and their count, and clears them.
  *   kernel_id: 1 = block-sparse fp64 DMMA step, 2 = generic CSR/BSR step, 3 = block-sparse int8
- *   tensor-core step, 4 = digit planes of an iterate, 5 = column maxima of a panel.
+ *   tensor-core step, 4 = digit planes of an iterate, 5 = column maxima of a panel, 6 = int8 tensor-core Gram
+ *   product (ttdft_gram / ttdft_project).
  */
 ttdft_status ttdft_timing_enable(int32_t on);
 ttdft_status ttdft_timing_read(int32_t kernel_id, double* total_ms, int64_t* launches);

@@ -74,6 +74,8 @@ def lib() -> ctypes.CDLL:
             fn.restype = ctypes.c_int
             fn.argtypes = [i64, _i32p, _i32p, _f64p, vp, i64, vp, i64, i64, i32, f64, f64, f64]
         L.oracle_lanczos_bounds.restype = ctypes.c_int
+        L.oracle_gram.argtypes = [i64, i64, vp, i64, vp, i64, vp, i64]
+        L.oracle_gram.restype = None
         L.oracle_lanczos_bounds.argtypes = [i64, _i32p, _i32p, _f64p, i32, _f64p, _f64p, _f64p, _f64p, _f64p,
                                             ctypes.POINTER(f64), ctypes.POINTER(f64)]
         _lib = L
@@ -174,3 +176,23 @@ def filter_bounds(row_ptr, col, val, v0: np.ndarray, ncols: int, k: int = 30):
     a0, b, _ = lanczos_bounds(row_ptr, col, val, v0, k)
     a = a0 + (ncols / M) * (b - a0)
     return a, b, a0
+
+
+def gram(X: np.ndarray, W: np.ndarray) -> np.ndarray:
+    """G = X^T W by the plain definition (oracle_gram)."""
+    assert X.shape == W.shape
+    M, n = X.shape
+    G = np.empty((n, n), np.float64)
+    if M == 0:
+        G[:] = 0.0
+        return G
+    xp, ldx = _mat(X)
+    wp, ldw = _mat(W)
+    gp, ldg = _mat(G)
+    lib().oracle_gram(M, n, xp, ldx, wp, ldw, gp, ldg)
+    return G
+
+
+def project(row_ptr, col, val, X: np.ndarray) -> np.ndarray:
+    """H_F = X^T (H X) (Algorithm 1 step 3): the oracle's SpMM followed by the oracle's Gram product."""
+    return gram(X, spmm(row_ptr, col, val, 1.0, X))

@@ -18,6 +18,12 @@
 // Parity pins (tests/test_oracle_pins.py): P1 dense brute force, P2 scalar closed form T_m,
 // P3 known eigendecomposition, P4 degenerate matrices, P5 invariants, P6 Lanczos bounds.
 // Every function here is pinned by at least one of them; nothing is "parity unpinned".
+//
+// NEXT-1: oracle_gram is the plain definition of G = X^T W, the second product of the subspace
+// projection H_F = X_F^T (H X_F) (Algorithm 1 step 3; Sec. 4.3); the projection itself is
+// oracle_spmm_csr followed by oracle_gram.  Pins P7 (tests/test_oracle_pins.py): hand-computed integers
+// (tests/golden/gram_pins.txt), numpy's matmul, Q^T H Q = Lambda for a known eigendecomposition, symmetry,
+// congruence (XR)^T H (XR) = R^T (X^T H X) R and the trace identity.
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
@@ -206,6 +212,21 @@ int oracle_cheb_filter_csr_ld(int64_t M, const int32_t* row_ptr, const int32_t* 
 // Outputs: alpha[k], beta[k] (beta[j] couples v_j and v_{j+1}; beta[k-1] is the residual norm),
 // theta[k] ascending, zlast[k] = last components of the unit eigenvectors; returns the k used.
 // ---------------------------------------------------------------------------------------------
+// G = X^T W: G[j,l] = sum_k X[k,j] * W[k,l], k ascending, left to right.
+// X, W: M x n row-major (ldx, ldw); G: n x n row-major (ldg).  Parallel over the rows j of G only.
+void oracle_gram(int64_t M, int64_t n, const double* X, int64_t ldx, const double* W, int64_t ldw, double* G, int64_t ldg) {
+#pragma omp parallel for schedule(static)
+  for (int64_t j = 0; j < n; ++j) {
+    double* g = G + j * ldg;
+    for (int64_t l = 0; l < n; ++l) g[l] = 0.0;
+    for (int64_t k = 0; k < M; ++k) {
+      const double x = X[k * ldx + j];
+      const double* w = W + k * ldw;
+      for (int64_t l = 0; l < n; ++l) g[l] = g[l] + x * w[l];
+    }
+  }
+}
+
 static void spmv_csr(int64_t M, const int32_t* row_ptr, const int32_t* col, const double* val, const double* x,
                      double* y) {
 #pragma omp parallel for schedule(dynamic, 64)

@@ -35,4 +35,8 @@ from .api import (  # noqa: F401
     timing_enable,
     timing_read,
     KERNEL_IDS,
+    gram,
+    gram_work_bytes,
+    project,
+    project_work_bytes,
 )

@@ -20,6 +20,7 @@ exported_symbols = [
     "ttdft_cheb_filter_host", "ttdft_probe_fp64_peak", "ttdft_launch_count", "ttdft_last_error",
     "ttdft_h_set_math_mode", "ttdft_step_work_bytes", "ttdft_spmm_ws", "ttdft_cheb_step_ws",
     "ttdft_timing_enable", "ttdft_timing_read",
+    "ttdft_gram_work_bytes", "ttdft_gram", "ttdft_project_work_bytes", "ttdft_project",
 ]
 
 
@@ -91,6 +92,14 @@ def _load() -> ctypes.CDLL:
         fn.restype = st
         fn.argtypes = [c_void_p, c_void_p, c_int64, c_void_p, c_int64, c_int64, c_int32, c_double, c_double, c_double,
                        c_int64, c_void_p, c_size_t, c_void_p]
+    L.ttdft_gram_work_bytes.restype = st
+    L.ttdft_gram_work_bytes.argtypes = [c_int64, c_int64, POINTER(c_size_t)]
+    L.ttdft_gram.restype = st
+    L.ttdft_gram.argtypes = [c_int64, c_void_p, c_int64, c_void_p, c_int64, c_int64, c_void_p, c_int64, c_void_p, c_size_t, c_void_p]
+    L.ttdft_project_work_bytes.restype = st
+    L.ttdft_project_work_bytes.argtypes = [c_void_p, c_int64, POINTER(c_size_t)]
+    L.ttdft_project.restype = st
+    L.ttdft_project.argtypes = [c_void_p, c_void_p, c_int64, c_int64, c_void_p, c_int64, c_void_p, c_size_t, c_void_p]
     L.ttdft_probe_fp64_peak.restype = st
     L.ttdft_probe_fp64_peak.argtypes = [c_int32, c_int32, c_void_p, POINTER(c_double)]
     L.ttdft_timing_enable.restype = st
@@ -109,7 +118,7 @@ def last_error() -> str:
     return _load().ttdft_last_error().decode()
 
 
-KERNEL_IDS = {"bsr_dmma": 1, "generic": 2, "bsr_i8": 3, "y_digits": 4, "colmax": 5}
+KERNEL_IDS = {"bsr_dmma": 1, "generic": 2, "bsr_i8": 3, "y_digits": 4, "colmax": 5, "gram_i8": 6}
 
 
 def timing_enable(on: bool = True):
@@ -340,6 +349,51 @@ def cheb_filter_host(H: Hamiltonian, X_host, Y_host, m: int, a: float, b: float,
     _check(_load().ttdft_cheb_filter_host(H.handle, X_host.data_ptr(), ldx, Y_host.data_ptr(), ldy, ncols, m, a, b, a0,
                                           panel_cols, wp, wbytes, _stream(stream)))
     return Y_host
+
+
+def _aligned_work(nbytes: int, work, device):
+    torch = _torch()
+    if work is None:
+        work = torch.empty(nbytes + 1024, dtype=torch.uint8, device=device)
+    wp = (work.data_ptr() + 1023) // 1024 * 1024
+    return wp, work.numel() * work.element_size() - (wp - work.data_ptr()), work
+
+
+def gram_work_bytes(M: int, ncols: int) -> int:
+    out = c_size_t(0)
+    _check(_load().ttdft_gram_work_bytes(M, ncols, byref(out)))
+    return int(out.value)
+
+
+def gram(X, W, G, work=None, stream=None):
+    """G = X^T W (ttdft_gram): X, W row-major M x N device float64, G row-major N x N."""
+    xp, ldx = _mat(X, "X")
+    wp_, ldw = _mat(W, "W")
+    gp, ldg = _mat(G, "G")
+    M, N = X.shape
+    if W.shape != X.shape or tuple(G.shape) != (N, N):
+        raise ValueError("shape mismatch")
+    wp, wb, keep = _aligned_work(gram_work_bytes(M, N), work, X.device)
+    _check(_load().ttdft_gram(M, xp, ldx, wp_, ldw, N, gp, ldg, wp, wb, _stream(stream)))
+    return G
+
+
+def project_work_bytes(H: Hamiltonian, ncols: int) -> int:
+    out = c_size_t(0)
+    _check(_load().ttdft_project_work_bytes(H.handle, ncols, byref(out)))
+    return int(out.value)
+
+
+def project(H: Hamiltonian, X, G, work=None, stream=None):
+    """G = X^T (H X) (ttdft_project; Algorithm 1 step 3): X row-major M x N, G row-major N x N."""
+    xp, ldx = _mat(X, "X")
+    gp, ldg = _mat(G, "G")
+    N = X.shape[1]
+    if X.shape[0] != H.M or tuple(G.shape) != (N, N):
+        raise ValueError("shape mismatch")
+    wp, wb, keep = _aligned_work(project_work_bytes(H, N), work, X.device)
+    _check(_load().ttdft_project(H.handle, xp, ldx, N, gp, ldg, wp, wb, _stream(stream)))
+    return G
 
 
 def probe_fp64_peak(kind: int = 1, millis: int = 200, stream=None) -> float:

@@ -50,6 +50,7 @@ struct K3Params {
   const double* hdiag;             // diagonal of H (fp64)         [M]
   const uint32_t* cmaxS;           // column maxima of Y_k (upper words)   [ncols]
   uint32_t* cmaxO;                 // out: column maxima of O, or NULL
+  unsigned long long* trace;       // debug (ttdft_debug_k3_trace): 8 clock64 stamps per work item of CTA 0, or NULL
 };
 
 template <int S>
@@ -99,6 +100,66 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
         "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
       : "r"(taddr));
 }
+
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&r)[8]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "r"(taddr));
+}
+
+// Accumulators of one TMEM lane (row) -> v[j] = 2^16 * sum_g L_g[j] * 256^-g  for the 64 columns of the item.
+// fp64 instructions are scarce while the tensor pipe runs int8 MMAs (ncu: "math pipe throttle" on every DFMA of
+// the epilogue), so three int32 levels are packed EXACTLY into one int64 (|L| < 2^31: L_a*2^16 + L_b*2^8 + L_c
+// < 2^48) before the conversion: ceil(S/3) conversions and ceil(S/3)-1 FMAs per element instead of S and S-1.
+template <int S>
+__device__ __forceinline__ void k3_drain(uint32_t trow, double (&v)[K3_NT]) {
+  constexpr int NG = (S + 2) / 3;
+#pragma unroll
+  for (int c = 0; c < K3_NT / 8; ++c) {
+    uint32_t a[S][8];
+#pragma unroll
+    for (int g = 0; g < S; ++g) tmem_ld8(trow + (uint32_t)(g * K3_NT + c * 8), a[g]);
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      double acc = 0.0;
+#pragma unroll
+      for (int k = NG - 1; k >= 0; --k) {       // least significant group first
+        long long t = 0;
+#pragma unroll
+        for (int l = 0; l < 3; ++l) {
+          const int g = 3 * k + l;
+          if (g < S) {
+            asm volatile("" : "+r"(a[g][i]));   // consumers must stay behind the wait
+            t += (long long)(int32_t)a[g][i] << (8 * (2 - l));
+          }
+        }
+        const double d = __ll2double_rn(t);
+        acc = (k == NG - 1) ? d : fma(acc, 5.9604644775390625e-8 /* 2^-24 */, d);
+      }
+      v[c * 8 + i] = acc;
+    }
+  }
+}
+
+// x * 2^e by an integer add on the exponent field (no fp64 instruction); zero, subnormal and out-of-range
+// cases take the slow, exact route
+__device__ __forceinline__ double scale_pow2(double x, int32_t e) {
+  const int32_t hi = __double2hiint(x);
+  const int32_t ex = (hi >> 20) & 0x7ff;
+  const int32_t en = ex + e;
+  if (ex != 0 && en > 0 && en < 2047) return __hiloint2double(hi + (e << 20), __double2loint(x));
+  if (x == 0.0) return x;
+  const int32_t e1 = max(-1000, min(1000, e / 2)), e2 = max(-1000, min(1000, e - e / 2));
+  return x * pow2i(e1) * pow2i(e2);
+}
+
+// Order in which the S planes of a tile travel through the ring and are multiplied: i-th plane = k3_plane<S>(i).
+// Natural order.  (Alternating wide and narrow products -- 0, S-1, 1, S-2, ... -- was measured and changes nothing:
+// the MMA phase is bound by shared-memory operand bandwidth, ~96 B/clk for A + B, not by the issuing thread.
+// Plane 0 must stay first: its first MMA of a work item overwrites every accumulator level.)
+template <int S>
+__host__ __device__ constexpr int k3_plane(int i) { return i; }
 
 // one lane of the (converged) calling warp; lets ptxas feed the uniform-register operands of
 // UTMALDG / UTCIMMA from that lane directly instead of through a broadcast loop
@@ -162,7 +223,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
   uint64_t* hempty = bars + 4 + NH;              // [NH]
   uint64_t* accfull = bars + 4 + 2 * NH;
   uint64_t* accempty = accfull + 1;
-  double* cs_s = reinterpret_cast<double*>(smem + Cf::CS_OFFSET);        // 2^eY_j of the current tile
+  int32_t* ce_s = reinterpret_cast<int32_t*>(smem + Cf::CS_OFFSET);      // eY_j of the current tile
   uint32_t* cm_s = reinterpret_cast<uint32_t*>(smem + Cf::CM_OFFSET);    // column maxima of the current tile
   uint32_t* tmem_slot = cm_s + 64;
 
@@ -215,10 +276,10 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
             mbar_wait(&hempty[hs], hph ^ 1);       // all C CTAs have finished with this slot
             mbar_expect_tx(&hfull[hs], (uint32_t)b * 128u);
             if (C > 1)
-              tma_load_2d_mc(hring + hs * Cf::HSLOT + crank * hrows * 128, &tmHd, 0, (p * prm.hplanes + q) * b + crank * hrows,
+              tma_load_2d_mc(hring + hs * Cf::HSLOT + crank * hrows * 128, &tmHd, 0, (p * prm.hplanes + k3_plane<S>(q)) * b + crank * hrows,
                              &hfull[hs], cmask);
             else
-              tma_load_2d(hring + hs * Cf::HSLOT, &tmHd, 0, (p * prm.hplanes + q) * b, &hfull[hs]);
+              tma_load_2d(hring + hs * Cf::HSLOT, &tmHd, 0, (p * prm.hplanes + k3_plane<S>(q)) * b, &hfull[hs]);
             if (++hs == NH) { hs = 0; hph ^= 1; }
           }
           yb ^= 1;
@@ -239,13 +300,18 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         k3_decode(prm, u, I, ctg);
         const int32_t nJ = prm.brow_ptr[I + 1] - prm.brow_ptr[I];
         if (nJ == 0) continue;
+        const int64_t it = (u - cluster0) / nclusters;
+        const bool tr = prm.trace && blockIdx.x == 0 && it < 512;
+        if (tr) prm.trace[it * 8 + 0] = clock64();
         mbar_wait(accempty, aph ^ 1);            // the epilogue has drained the previous item's accumulators
         asm volatile("tcgen05.fence::after_thread_sync;");
+        if (tr) { prm.trace[it * 8 + 1] = clock64(); prm.trace[it * 8 + 7] = (unsigned long long)nJ; }
         for (int32_t j = 0; j < nJ; ++j) {
           mbar_wait(&yfull[yb], yph);
           const uint32_t ylo = ylo0 + (uint32_t)yb * (Cf::YBUF >> 4);
 #pragma unroll
-          for (int p = 0; p < S; ++p) {
+          for (int ip = 0; ip < S; ++ip) {
+            const int p = k3_plane<S>(ip);
             mbar_wait(&hfull[hs], hph);
             asm volatile("tcgen05.fence::after_thread_sync;");
             const uint32_t hlo = hlo0 + (uint32_t)hs * (Cf::HSLOT >> 4);
@@ -254,7 +320,8 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
             for (int kk = 0; kk < 4; ++kk) {
               if (kk < ksteps) {
                 const uint64_t da = dbase | (uint64_t)(hlo + kk * 2);
-                const uint32_t acc = (p > 0 || kk > 0) ? 1u : (j > 0 ? 1u : 0u);
+                // plane 0 comes first and spans every level: its first MMA of a work item overwrites the accumulators
+                const uint32_t acc = (ip > 0 || kk > 0) ? 1u : (j > 0 ? 1u : 0u);
 #pragma unroll
                 for (int n0 = 0; n0 < ntot; n0 += 256) {
                   const int n = (ntot - n0) < 256 ? (ntot - n0) : 256;
@@ -271,6 +338,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
           if (yb == 0) yph ^= 1;
         }
         umma_commit(accfull);
+        if (tr) prm.trace[it * 8 + 2] = clock64();
         aph ^= 1;
       }
     }
@@ -292,46 +360,51 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       const int64_t row = (int64_t)I * b + r;
       if (et < 64) {
         const int64_t cj = col0 + et;
-        cs_s[et] = pow2i(exp_from_hi(cj < prm.ncols ? prm.cmaxS[cj] : 0u));
+        ce_s[et] = exp_from_hi(cj < prm.ncols ? prm.cmaxS[cj] : 0u);
         cm_s[et] = 0;
       }
       double rsp = 0.0, gi = prm.gamma;
+      const bool full = (col0 + K3_NT <= prm.ncols);
       if (row_ok) {
-        rsp = pow2i(prm.eH[row] - 14);
+        rsp = alpha * pow2i(prm.eH[row] - 30);    // alpha * 2^(eH_i - 14) / 2^16 (k3_drain returns 2^16 * v)
         gi = fma(alpha, prm.hdiag[row], prm.gamma);
+        // This thread reads its own row of Y_k and Y_{k-1} (4 lines each) after the drain, 16 bytes at a time and
+        // one dependent batch after the other: without help the output phase is a chain of exposed HBM latencies
+        // (69 % of the epilogue warps' time in profiles/r01b).  Pull all eight lines into L2 now, in one burst,
+        // while the warp is about to wait for the accumulators anyway.
+        if (full) {
+          const double* sp0 = prm.S + row * prm.lds + col0;
+          const double* zp0 = prm.Z + row * prm.ldz + col0;
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(sp0 + 16 * k));
+            if (use_z) asm volatile("prefetch.global.L2 [%0];" ::"l"(zp0 + 16 * k));
+          }
+        }
       }
       asm volatile("bar.sync 1, 128;" ::: "memory");
 
       double v[K3_NT];
+      const int64_t it = (u - cluster0) / nclusters;
+      const bool tr = prm.trace && blockIdx.x == 0 && it < 512 && et == 0;
+      if (tr) prm.trace[it * 8 + 3] = clock64();
       if (nJ > 0) {
         mbar_wait(accfull, aph);
         aph ^= 1;
+        if (tr) prm.trace[it * 8 + 4] = clock64();
         asm volatile("tcgen05.fence::after_thread_sync;");
         const uint32_t trow = tmem_base + ((uint32_t)(quarter * 32) << 16);
-#pragma unroll
-        for (int g = S - 1; g >= 0; --g) {       // Horner, least significant level first
-          uint32_t a[4][16];
-#pragma unroll
-          for (int c = 0; c < 4; ++c) tmem_ld16(trow + (uint32_t)(g * K3_NT + c * 16), a[c]);
-          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-          for (int c = 0; c < 4; ++c)
-#pragma unroll
-            for (int i = 0; i < 16; ++i) {
-              asm volatile("" : "+r"(a[c][i]));   // consumers must stay behind the wait
-              const double x = (double)(int32_t)a[c][i];
-              v[c * 16 + i] = (g == S - 1) ? x : fma(v[c * 16 + i], 0.00390625, x);
-            }
-        }
+        k3_drain<S>(trow, v);
         asm volatile("tcgen05.fence::before_thread_sync;");
         mbar_arrive(accempty);                   // TMEM is free for the next work item
+        if (tr) prm.trace[it * 8 + 5] = clock64();
       } else {
 #pragma unroll
         for (int i = 0; i < K3_NT; ++i) v[i] = 0.0;
       }
 
-      // ---- out = alpha * 2^(eH+eY-14) * v + (alpha*hdiag + gamma) * y + beta * z ----
-      const bool full = (col0 + K3_NT <= prm.ncols);
+      // ---- out = alpha * 2^(eH+eY-30) * v + (alpha*hdiag + gamma) * y + beta * z   (v = 2^16 * Horner) ----
+      // three fp64 instructions per element: v * (alpha 2^(eH-30)), then the column's 2^eY by an exponent add, two FMAs
       const double* sp = prm.S + row * prm.lds + col0;
       const double* zp = prm.Z + row * prm.ldz + col0;
       double* op = prm.O + row * prm.ldo + col0;
@@ -352,8 +425,8 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
             const int j = c0 + 2 * i;
             double o0 = 0.0, o1 = 0.0;
             if (row_ok) {
-              o0 = fma(gi, y2[i].x, alpha * (v[j] * cs_s[j] * rsp));
-              o1 = fma(gi, y2[i].y, alpha * (v[j + 1] * cs_s[j + 1] * rsp));
+              o0 = fma(gi, y2[i].x, scale_pow2(v[j] * rsp, ce_s[j]));
+              o1 = fma(gi, y2[i].y, scale_pow2(v[j + 1] * rsp, ce_s[j + 1]));
               if (use_z) { o0 = fma(beta, z2[i].x, o0); o1 = fma(beta, z2[i].y, o1); }
               *reinterpret_cast<double2*>(op + j) = make_double2(o0, o1);
             }
@@ -365,7 +438,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         for (int j = 0; j < K3_NT; ++j) {
           double o = 0.0;
           if (row_ok && col0 + j < prm.ncols) {
-            o = fma(gi, sp[j], alpha * (v[j] * cs_s[j] * rsp));
+            o = fma(gi, sp[j], scale_pow2(v[j] * rsp, ce_s[j]));
             if (use_z) o = fma(beta, zp[j], o);
             op[j] = o;
           }
@@ -382,7 +455,8 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         asm volatile("bar.sync 1, 128;" ::: "memory");
         if (et < 64 && col0 + et < prm.ncols && cm_s[et]) atomicMax(&prm.cmaxO[col0 + et], cm_s[et]);
       }
-      asm volatile("bar.sync 1, 128;" ::: "memory");   // cs_s / cm_s are rewritten by the next item
+      if (tr) prm.trace[it * 8 + 6] = clock64();
+      asm volatile("bar.sync 1, 128;" ::: "memory");   // ce_s / cm_s are rewritten by the next item
     }
   }
 

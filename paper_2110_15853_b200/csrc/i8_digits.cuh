@@ -77,10 +77,10 @@ __global__ void __launch_bounds__(256) colmax_kernel(const double* __restrict__ 
 // One CTA per (block row I, 64-column tile): coalesced fp64 reads along the columns, a shared-memory
 // transpose, 128-byte coalesced int8 rows out -- the K-major rows K3's B operand wants.
 // Also clears next_cmax (the maxima K3's epilogue will accumulate for the following step).
-// grid (nb, ceil(ncols/64)), 256 threads, dynamic smem S*64*33*4 bytes
+// grid (nb, tiles >= ceil(ncols/64)), 256 threads, dynamic smem S*64*33*4 bytes; M = valid rows (<= nb*b)
 // ------------------------------------------------------------------------------------------------
 template <int S>
-__global__ void __launch_bounds__(256) y_digits_kernel(const double* __restrict__ Y, int64_t ld, int32_t b, int64_t ncols,
+__global__ void __launch_bounds__(256) y_digits_kernel(const double* __restrict__ Y, int64_t ld, int32_t b, int64_t M, int64_t ncols,
                                                        const uint32_t* __restrict__ cmax, int8_t* __restrict__ D,
                                                        uint32_t* __restrict__ next_cmax) {
   extern __shared__ uint32_t sd[];   // [S][64][33] words: row (q,n) holds 128 k-bytes + 1 pad word
@@ -105,7 +105,8 @@ __global__ void __launch_bounds__(256) y_digits_kernel(const double* __restrict_
     for (int h = 0; h < 2; ++h) {
       const double* src = Y + ((int64_t)I * b + 4 * quad) * ld + n0 + 32 * h + lane;
 #pragma unroll
-      for (int i = 0; i < 4; ++i) x[h][i] = (quad < nquads && cv[h]) ? __ldcs(src + (int64_t)i * ld) : 0.0;
+      for (int i = 0; i < 4; ++i)   // rows beyond M (ragged last block of the Gram contraction) read as zero
+        x[h][i] = (quad < nquads && cv[h] && I * b + 4 * quad + i < M) ? __ldcs(src + (int64_t)i * ld) : 0.0;
     }
 #pragma unroll
     for (int h = 0; h < 2; ++h) {

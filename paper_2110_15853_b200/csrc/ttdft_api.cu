@@ -19,14 +19,16 @@
 #include "bsr_dmma.cuh"
 #include "bsr_i8.cuh"
 #include "generic_spmm.cuh"
+#include "gram_i8.cuh"
 
 namespace {
 
 thread_local std::string g_err;
+unsigned long long* g_k3_trace = nullptr;   // debug: see ttdft_debug_k3_trace
 std::atomic<int64_t> g_launches{0};
 
 // ---- optional per-kernel device timing (ttdft_timing_*): CUDA events on the launching stream ----
-constexpr int NKID = 6;   // 1 = K1 bsr_dmma, 2 = K2 generic, 3 = K3 bsr_i8, 4 = y_digits, 5 = colmax
+constexpr int NKID = 7;   // 1 = K1 bsr_dmma, 2 = K2 generic, 3 = K3 bsr_i8, 4 = y_digits, 5 = colmax, 6 = K4 gram_i8
 struct KernelTimer {
   std::atomic<int> on{0};
   std::mutex mu;
@@ -141,6 +143,22 @@ ttdft_status make_map_yd(CUtensorMap* map, const void* base, uint64_t ntile_plan
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled(Y digits) failed with CUresult %d", (int)r);
+  return TTDFT_OK;
+}
+
+// X digit tiles for the Gram kernel: uint8 [tiles][S planes][64 columns][128 k-bytes] as a 4-D tensor,
+// box = 1 tile x 1 plane x box_cols columns x 128 B
+ttdft_status make_map_xd4(CUtensorMap* map, const void* base, uint64_t ntiles, uint32_t S, uint32_t box_cols) {
+  encode_tiled_fn enc = get_encode();
+  if (!enc) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  cuuint64_t dims[4] = {128, (cuuint64_t)ttdft::K3_NT, S, ntiles};
+  cuuint64_t strides[3] = {128, 128 * (cuuint64_t)ttdft::K3_NT, 128 * (cuuint64_t)ttdft::K3_NT * S};
+  cuuint32_t box[4] = {128, box_cols, 1, 1};
+  cuuint32_t estr[4] = {1, 1, 1, 1};
+  CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 4, const_cast<void*>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled(X digits) failed with CUresult %d", (int)r);
   return TTDFT_OK;
 }
 
@@ -679,7 +697,7 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
     }
     dim3 g((unsigned)h->nb, nct);
     TimedLaunch tl(4, st);
-    ttdft::y_digits_kernel<S><<<g, 256, smem, st>>>(X, ldx, h->b, ncols, cmS, w.D, cmO);
+    ttdft::y_digits_kernel<S><<<g, 256, smem, st>>>(X, ldx, h->b, h->M, ncols, cmS, w.D, cmO);
     CUDA_TRY(cudaGetLastError());
     g_launches.fetch_add(1);
   }
@@ -694,6 +712,8 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
   p.alpha = alpha; p.gamma = gamma; p.beta = beta;
   p.S = X; p.lds = ldx; p.Z = Z ? Z : X; p.ldz = Z ? ldz : ldx; p.O = O; p.ldo = ldo;
   p.eH = h->eH; p.hdiag = h->hdiag; p.cmaxS = cmS; p.cmaxO = cmO;
+  p.trace = g_k3_trace;
+  if (p.vec && env_int("TTDFT_DEBUG_NOFP64", 0)) p.vec = 2;
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
   // column tiles in clusters of C; a remainder of < C tiles runs as single CTAs
@@ -811,6 +831,141 @@ ttdft_status filter_panel(ttdft_h_s* h, const double* Xp, int64_t ldx, double* Y
   return TTDFT_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// K4: G = X^T W on the int8 tensor cores (subspace projection)
+// ------------------------------------------------------------------------------------------------
+constexpr int GRAM_S = 7;            // digit planes per operand (55 bits below each column maximum)
+struct GramPlan {
+  int64_t M = 0, ncols = 0;
+  int32_t nbk = 0, nctW = 0, nctX = 0, nctx = 0, kc = 0, nchunks = 0;
+  int64_t wp = 0;                    // columns of W per panel of partial tiles
+  size_t dx_bytes = 0, dw_bytes = 0, cm_bytes = 0, p_bytes = 0, total = 0;
+  int nsm = 148;
+};
+ttdft_status gram_plan(int64_t M, int64_t ncols, GramPlan* g) {
+  if (M < 0 || ncols < 1) return fail(TTDFT_ERR_INVALID_ARG, "gram: M must be >= 0 and ncols >= 1");
+  if (M >= ((int64_t)1 << 37) || ncols > 65535) return fail(TTDFT_ERR_UNSUPPORTED, "gram: matrix too large (ncols <= 65535)");
+  g->M = M; g->ncols = ncols;
+  g->nbk = (int32_t)((M + 127) / 128);
+  g->nctW = (int32_t)((ncols + 63) / 64);
+  g->nctX = (g->nctW + 1) & ~1;
+  g->nctx = g->nctX / 2;
+  int dev = 0, nsm = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0)
+    g->nsm = nsm;
+  else (void)cudaGetLastError();
+  // chunks of the contraction: <= 128 blocks each (exact int32 accumulation: 7 * 128 * 128 * 2^14 < 2^31), and enough of
+  // them that a small G still fills the SMs
+  const int64_t tiles = (int64_t)g->nctx * g->nctW;
+  int64_t target = std::max<int64_t>((g->nbk + 127) / 128, std::min<int64_t>(g->nbk, (4 * g->nsm + tiles - 1) / tiles));
+  if (target < 1) target = 1;
+  g->kc = (int32_t)std::max<int64_t>(1, (g->nbk + target - 1) / target);
+  g->nchunks = g->nbk ? (g->nbk + g->kc - 1) / g->kc : 0;
+  // partial tiles P[chunk][ncols][wp] are kept under 2 GiB by cutting G into column panels
+  const int64_t wfull = (int64_t)g->nctW * 64;
+  int64_t wp = wfull;
+  const int64_t per_col = std::max<int64_t>(1, (int64_t)g->nchunks) * ncols * 8;
+  if (per_col * wp > ((int64_t)1 << 31)) wp = std::max<int64_t>(128, (((int64_t)1 << 31) / per_col) / 128 * 128);
+  g->wp = std::min(wp, wfull);
+  g->dx_bytes = align_up((size_t)GRAM_S * g->nctX * 64 * (size_t)g->nbk * 128, 1024);
+  g->dw_bytes = align_up((size_t)GRAM_S * g->nctW * 64 * (size_t)g->nbk * 128, 1024);
+  g->cm_bytes = align_up((size_t)ncols * 4, 1024);
+  g->p_bytes = align_up((size_t)std::max<int64_t>(1, g->nchunks) * (size_t)ncols * (size_t)g->wp * 8, 1024);
+  g->total = g->dx_bytes + g->dw_bytes + 2 * g->cm_bytes + g->p_bytes;
+  return TTDFT_OK;
+}
+
+template <int C>
+ttdft_status launch_k4(const GramPlan& g, const CUtensorMap& tmXd, const CUtensorMap& tmWd, ttdft::K4Params p, int32_t ctw_begin,
+                       int32_t ntiles, cudaStream_t st) {
+  constexpr int S = GRAM_S;
+  auto kern = ttdft::gram_i8_kernel<S, C>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ttdft::K3Cfg<S>::TOTAL));
+    attr_set = true;
+  }
+  p.ctw_begin = ctw_begin;
+  p.nctwg = ntiles / C;
+  const int64_t items = (int64_t)p.nchunks * p.nctx * p.nctwg;
+  if (items == 0) return TTDFT_OK;
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute at[1];
+  k3_launch_config<S, C>(&cfg, at, (unsigned)(std::min<int64_t>(items, g.nsm / C) * C), st);
+  TimedLaunch tl(6, st);
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, tmXd, tmWd, p));
+  g_launches.fetch_add(1);
+  return TTDFT_OK;
+}
+
+ttdft_status gram_run(const GramPlan& g, const double* X, int64_t ldx, const double* W, int64_t ldw, double* G, int64_t ldg, void* work,
+                      cudaStream_t st) {
+  constexpr int S = GRAM_S;
+  if (g.M == 0) {   // empty contraction: G = 0
+    CUDA_TRY(cudaMemset2DAsync(G, (size_t)ldg * 8, 0, (size_t)g.ncols * 8, (size_t)g.ncols, st));
+    return TTDFT_OK;
+  }
+  uint8_t* wb = reinterpret_cast<uint8_t*>(work);
+  int8_t* DX = reinterpret_cast<int8_t*>(wb);
+  int8_t* DW = reinterpret_cast<int8_t*>(wb + g.dx_bytes);
+  uint32_t* cmX = reinterpret_cast<uint32_t*>(wb + g.dx_bytes + g.dw_bytes);
+  uint32_t* cmW = reinterpret_cast<uint32_t*>(wb + g.dx_bytes + g.dw_bytes + g.cm_bytes);
+  double* P = reinterpret_cast<double*>(wb + g.dx_bytes + g.dw_bytes + 2 * g.cm_bytes);
+  // column maxima, then digit tiles of both operands (128-row blocks of the contraction, ragged tail read as zero)
+  CUDA_TRY(cudaMemsetAsync(cmX, 0, 2 * g.cm_bytes, st));
+  {
+    dim3 gc((unsigned)g.nctW, (unsigned)((g.M + 2047) / 2048));
+    { TimedLaunch tl(5, st); ttdft::colmax_kernel<<<gc, 256, 0, st>>>(X, ldx, g.M, g.ncols, cmX); }
+    { TimedLaunch tl(5, st); ttdft::colmax_kernel<<<gc, 256, 0, st>>>(W, ldw, g.M, g.ncols, cmW); }
+    CUDA_TRY(cudaGetLastError());
+    g_launches.fetch_add(2);
+    static bool attr_set = false;
+    const int smem = S * 64 * 33 * 4;
+    if (!attr_set) {
+      CUDA_TRY(cudaFuncSetAttribute(ttdft::y_digits_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+      attr_set = true;
+    }
+    { TimedLaunch tl(4, st);
+      ttdft::y_digits_kernel<S><<<dim3((unsigned)g.nbk, (unsigned)g.nctX), 256, smem, st>>>(X, ldx, 128, g.M, g.ncols, cmX, DX, nullptr); }
+    { TimedLaunch tl(4, st);
+      ttdft::y_digits_kernel<S><<<dim3((unsigned)g.nbk, (unsigned)g.nctW), 256, smem, st>>>(W, ldw, 128, g.M, g.ncols, cmW, DW, nullptr); }
+    CUDA_TRY(cudaGetLastError());
+    g_launches.fetch_add(2);
+  }
+  CUtensorMap tmXd[2], tmWd;
+  ttdft_status s;
+  for (int ci = 0; ci < 2; ++ci)
+    if ((s = make_map_xd4(&tmXd[ci], DX, (uint64_t)g.nbk * g.nctX, S, 64u >> ci)) != TTDFT_OK) return s;
+  if ((s = make_map_yd(&tmWd, DW, (uint64_t)g.nbk * g.nctW * S, S)) != TTDFT_OK) return s;
+  ttdft::K4Params p;
+  p.nbk = g.nbk; p.kc = g.kc; p.nchunks = g.nchunks; p.nctx = g.nctx; p.nctX = g.nctX; p.nctW = g.nctW;
+  p.ncols = g.ncols; p.P = P; p.cmaxX = cmX; p.cmaxW = cmW;
+  const int C = env_int("TTDFT_K4_CLUSTER", 2) == 1 ? 1 : 2;
+  for (int64_t c0 = 0; c0 < g.ncols; c0 += g.wp) {
+    const int64_t wc = std::min(g.wp, g.ncols - c0);
+    const int32_t ct0 = (int32_t)(c0 / 64), ntl = (int32_t)((wc + 63) / 64);
+    p.ncols_w = (int32_t)wc;
+    p.ldp = g.wp;
+    p.colw0 = c0;
+    // the kernel indexes W tiles globally (ctw) and P columns relative to the panel: shift P so that
+    // column (ctw * 64 - c0) lands at the panel start
+    ttdft::K4Params q = p;
+    q.P = P - c0;                 // pp = P + ... + ctw*64 with ctw global
+    q.ncols_w = (int32_t)(c0 + wc);   // valid global columns end (exclusive) for the ragged checks
+    q.colw0 = 0;
+    const int32_t main_tiles = ntl / C * C;
+    if (C == 2) s = launch_k4<2>(g, tmXd[1], tmWd, q, ct0, main_tiles, st);
+    else s = launch_k4<1>(g, tmXd[0], tmWd, q, ct0, main_tiles, st);
+    if (s != TTDFT_OK) return s;
+    if (main_tiles < ntl && (s = launch_k4<1>(g, tmXd[0], tmWd, q, ct0 + main_tiles, ntl - main_tiles, st)) != TTDFT_OK) return s;
+    dim3 gr((unsigned)((wc + 255) / 256), (unsigned)g.ncols);
+    ttdft::gram_reduce_kernel<<<gr, 256, 0, st>>>(P, g.wp, g.ncols, g.nchunks, wc, G + c0, ldg);
+    CUDA_TRY(cudaGetLastError());
+    g_launches.fetch_add(1);
+  }
+  return TTDFT_OK;
+}
+
 }  // namespace
 
 // ================================================================================================
@@ -845,6 +1000,10 @@ ttdft_status ttdft_timing_read(int32_t kernel_id, double* total_ms, int64_t* lau
   return TTDFT_OK;
 }
 int64_t ttdft_launch_count(void) { return g_launches.load(); }
+
+// Debug aid, not part of include/ttdft.h: K3 launches record 8 clock64 stamps per work item of CTA 0 (first 512 items)
+// into this DEVICE buffer of 512*8 uint64 (NULL switches the trace off).
+void ttdft_debug_k3_trace(void* dev_buf) { g_k3_trace = reinterpret_cast<unsigned long long*>(dev_buf); }
 
 static ttdft_status desc_counts(const ttdft_h_desc* d, int64_t* nrows_idx, int64_t* nstored) {
   if (!d) return fail(TTDFT_ERR_INVALID_ARG, "desc is NULL");
@@ -1441,6 +1600,69 @@ ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* Xh, int64_t ldx, 
 #undef HOST_TRY
   cleanup();
   return TTDFT_OK;
+}
+
+ttdft_status ttdft_gram_work_bytes(int64_t M, int64_t ncols, size_t* bytes) {
+  if (!bytes) return fail(TTDFT_ERR_INVALID_ARG, "bytes is NULL");
+  GramPlan g;
+  ttdft_status s = gram_plan(M, ncols, &g);
+  if (s != TTDFT_OK) return s;
+  *bytes = g.total;
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_gram(int64_t M, const double* X, int64_t ldx, const double* W, int64_t ldw, int64_t ncols, double* G,
+                        int64_t ldg, void* work, size_t work_bytes, void* stream) {
+  GramPlan g;
+  ttdft_status s = gram_plan(M, ncols, &g);
+  if (s != TTDFT_OK) return s;
+  if (M > 0 && (s = check_mat("X", X, ldx, ncols)) != TTDFT_OK) return s;
+  if (M > 0 && (s = check_mat("W", W, ldw, ncols)) != TTDFT_OK) return s;
+  if ((s = check_mat("G", G, ldg, ncols)) != TTDFT_OK) return s;
+  if (work_bytes < g.total) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, g.total);
+  if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
+  return gram_run(g, X, ldx, W, ldw, G, ldg, work, (cudaStream_t)stream);
+}
+
+// scratch of ttdft_project: W = H*X (compact, even leading dimension) | max(single-step scratch, Gram scratch)
+static ttdft_status project_need(ttdft_h_t h, int64_t ncols, GramPlan* g, size_t* wbytes, size_t* total) {
+  ttdft_status s = gram_plan(h->M, ncols, g);
+  if (s != TTDFT_OK) return s;
+  const int64_t ldw = ncols + (ncols & 1);
+  *wbytes = align_up((size_t)h->M * (size_t)ldw * 8, 1024);
+  size_t pb;
+  const size_t step = align_up(step_work_need(h, ncols, &pb), 1024);
+  *total = *wbytes + std::max(step, g->total);
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_project_work_bytes(ttdft_h_t h, int64_t ncols, size_t* bytes) {
+  if (!h || !bytes) return fail(TTDFT_ERR_INVALID_ARG, "NULL argument");
+  GramPlan g;
+  size_t wb;
+  return project_need(h, ncols, &g, &wb, bytes);
+}
+
+ttdft_status ttdft_project(ttdft_h_t h, const double* X, int64_t ldx, int64_t ncols, double* G, int64_t ldg, void* work,
+                           size_t work_bytes, void* stream) {
+  if (!h) return fail(TTDFT_ERR_INVALID_ARG, "handle is NULL");
+  GramPlan g;
+  size_t wbytes, need;
+  ttdft_status s = project_need(h, ncols, &g, &wbytes, &need);
+  if (s != TTDFT_OK) return s;
+  if (h->M > 0 && (s = check_mat("X", X, ldx, ncols)) != TTDFT_OK) return s;
+  if ((s = check_mat("G", G, ldg, ncols)) != TTDFT_OK) return s;
+  if (work_bytes < need) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, need);
+  if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
+  cudaStream_t st = (cudaStream_t)stream;
+  double* Wb = reinterpret_cast<double*>(work);
+  uint8_t* rest = reinterpret_cast<uint8_t*>(work) + wbytes;
+  const int64_t ldw = ncols + (ncols & 1);
+  if (h->M > 0) {
+    s = step_ws(h, 1.0, 0.0, 0.0, X, ldx, nullptr, 0, Wb, ldw, ncols, rest, need - wbytes, st);   // W = H X
+    if (s != TTDFT_OK) return s;
+  }
+  return gram_run(g, X, ldx, Wb, ldw, G, ldg, rest, st);                                          // G = X^T W
 }
 
 ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, double* tflops) {

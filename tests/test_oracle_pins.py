@@ -367,3 +367,70 @@ def test_p6_lanczos_small_dense():
     v0 = rng.standard_normal(M)
     _, _, info = oracle.lanczos_bounds(rp, col, val, v0, 5)
     assert info["alpha"][0] == pytest.approx(v0 @ Hd @ v0 / (v0 @ v0), rel=1e-13)
+
+
+# ------------------------------------------------------------------ P7: subspace projection (NEXT-1)
+# oracle.gram / oracle.project pinned by hand-computed integers, numpy's matmul,
+# a known eigendecomposition and three identities a transposed operand or a dropped term would break.
+def read_gram_golden():
+    out = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "gram_pins.txt")) as f:
+        for line in f:
+            line = line.split("#")[0].split()
+            if not line:
+                continue
+            r, c = int(line[1]), int(line[2])
+            out[line[0]] = np.array([float(v) for v in line[3:]], np.float64).reshape(r, c)
+    return out
+
+
+def test_p7_hand_computed_projection():
+    g = read_gram_golden()
+    assert np.array_equal(oracle.gram(g["X"], g["W"]), g["XtW"])          # not symmetric: catches a transposed operand
+    rp, col, val = dense_to_csr(g["H"], keep_zeros=False)
+    assert np.array_equal(oracle.spmm(rp, col, val, 1.0, g["X"]), g["HX"])
+    assert np.array_equal(oracle.project(rp, col, val, g["X"]), g["XtHX"])
+
+
+@pytest.mark.parametrize("M,n", [(1, 1), (5, 3), (257, 33), (1000, 64), (0, 4)])
+def test_p7_gram_vs_numpy(M, n):
+    rng = np.random.default_rng(100 * M + n)
+    X, W = rng.standard_normal((M, n)), rng.standard_normal((M, n))
+    G = oracle.gram(X, W)
+    ref = X.T @ W
+    assert np.linalg.norm(G - ref) <= 1e-14 * max(1.0, np.linalg.norm(ref))
+    # strided views (leading dimension > n)
+    Xp, Wp = np.zeros((M, n + 3)), np.zeros((M, n + 5))
+    Xp[:, :n], Wp[:, :n] = X, W
+    assert np.array_equal(oracle.gram(Xp[:, :n], Wp[:, :n]), G)
+
+
+def test_p7_projection_of_eigenvectors_is_diagonal():
+    """H = Q Lambda Q^T, X = n columns of Q  =>  X^T H X = diag(lambda) exactly (up to rounding)."""
+    rng = np.random.default_rng(7)
+    M, n = 128, 17
+    Q, _ = np.linalg.qr(rng.standard_normal((M, M)))
+    lam = rng.uniform(-1.0, 20.0, M)
+    Hd = (Q * lam) @ Q.T
+    Hd = (Hd + Hd.T) / 2
+    rp, col, val = dense_to_csr(Hd, keep_zeros=True)
+    cols = rng.permutation(M)[:n]
+    G = oracle.project(rp, col, val, np.ascontiguousarray(Q[:, cols]))
+    assert np.linalg.norm(G - np.diag(lam[cols])) <= 1e-12 * np.linalg.norm(lam)
+
+
+def test_p7_projection_identities(tiny):
+    _cfg, H, C, _bounds = tiny
+    rng = np.random.default_rng(11)
+    n = 12
+    X = rng.standard_normal((H.M, n))
+    G = oracle.project(C.row_ptr, C.col_idx, C.values, X)
+    nG = np.linalg.norm(G)
+    assert np.linalg.norm(G - G.T) <= 1e-13 * nG                          # H symmetric (PAPER.md:L238) => H_F symmetric
+    R = rng.standard_normal((n, n))
+    G2 = oracle.project(C.row_ptr, C.col_idx, C.values, X @ R)           # congruence: (XR)^T H (XR) = R^T G R
+    assert np.linalg.norm(G2 - R.T @ G @ R) <= 1e-12 * np.linalg.norm(G2)
+    # trace identity: tr(X^T H X) = sum_e h_e * <X[row_e,:], X[col_e,:]>
+    rows = np.repeat(np.arange(H.M), np.diff(C.row_ptr))
+    tr = float(np.sum(C.values * np.einsum("ij,ij->i", X[rows], X[C.col_idx])))
+    assert abs(np.trace(G) - tr) <= 1e-12 * abs(tr)
