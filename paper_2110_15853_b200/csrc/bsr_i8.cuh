@@ -32,7 +32,8 @@
 namespace ttdft {
 
 constexpr int K3_NT = 64;        // columns per work item
-constexpr int K3_THREADS = 192;  // producer warp, MMA warp, 4 epilogue warps
+constexpr int K3_THREADS = 320;  // producer warp, MMA warp, 8 epilogue warps (two per TMEM lane quarter, 32 columns each)
+constexpr int K4_THREADS = 192;  // gram_i8.cuh: producer warp, MMA warp, 4 epilogue warps
 
 struct K3Params {
   const int32_t* brow_ptr;
@@ -107,15 +108,15 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&r)[8]) {
                : "r"(taddr));
 }
 
-// Accumulators of one TMEM lane (row) -> v[j] = 2^16 * sum_g L_g[j] * 256^-g  for the 64 columns of the item.
+// Accumulators of one TMEM lane (row) -> v[j] = 2^16 * sum_g L_g[j] * 256^-g  for NC consecutive columns of the item.
 // fp64 instructions are scarce while the tensor pipe runs int8 MMAs (ncu: "math pipe throttle" on every DFMA of
 // the epilogue), so three int32 levels are packed EXACTLY into one int64 (|L| < 2^31: L_a*2^16 + L_b*2^8 + L_c
 // < 2^48) before the conversion: ceil(S/3) conversions and ceil(S/3)-1 FMAs per element instead of S and S-1.
-template <int S>
-__device__ __forceinline__ void k3_drain(uint32_t trow, double (&v)[K3_NT]) {
+template <int S, int NC>
+__device__ __forceinline__ void k3_drain(uint32_t trow, double (&v)[NC]) {   // trow: TMEM address of the first column
   constexpr int NG = (S + 2) / 3;
 #pragma unroll
-  for (int c = 0; c < K3_NT / 8; ++c) {
+  for (int c = 0; c < NC / 8; ++c) {
     uint32_t a[S][8];
 #pragma unroll
     for (int g = 0; g < S; ++g) tmem_ld8(trow + (uint32_t)(g * K3_NT + c * 8), a[g]);
@@ -239,7 +240,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
     for (int i = 0; i < 2; ++i) { mbar_init(&yfull[i], 1); mbar_init(&yempty[i], 1); }
     for (int i = 0; i < NH; ++i) { mbar_init(&hfull[i], 1); mbar_init(&hempty[i], C); }   // a slot is free once all C CTAs have read it
     mbar_init(accfull, 1);
-    mbar_init(accempty, 128);
+    mbar_init(accempty, 256);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
@@ -344,10 +345,18 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
     }
   } else {
     // ======================================= epilogue =======================================
-    const int quarter = warp & 3;                // TMEM lane quarter this warp may read
-    const int et = (warp - 2) * 32 + lane;       // 0..127 among the epilogue threads
+    // 8 warps: warp w reads TMEM lane quarter w & 3 (rows 32q..32q+31 of the block row) and column half
+    // (w - 2) >> 2 (32 of the item's 64 columns): twice the warps of a one-warp-per-quarter epilogue and half the
+    // registers per thread, i.e. four times the loads in flight -- the output phase is a chain of dependent
+    // load -> fma -> store batches whose latency is ~8 K cycles behind the TMA traffic of the same SM, and with
+    // 4 warps it took 70 K cycles per item, longer than the MMAs of every block row with <= 18 tiles.
+    constexpr int NCW = K3_NT / 2;               // columns per warp
+    const int quarter = warp & 3;
+    const int half = (warp - 2) >> 2;
+    const int et = (warp - 2) * 32 + lane;       // 0..255 among the epilogue threads
     const int r = quarter * 32 + lane;           // row inside the block row
     const bool row_ok = r < b;
+    const bool warp_ok = (quarter * 32) < b;     // b is a multiple of 32: a warp's rows are all valid or all padding
     const double alpha = prm.alpha, beta = prm.beta;
     const bool use_z = (beta != 0.0);
     uint32_t aph = 0;
@@ -356,7 +365,8 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       k3_decode(prm, u, I, ctg);
       const int32_t ct = prm.ct_begin + ctg * C + crank;
       const int32_t nJ = prm.brow_ptr[I + 1] - prm.brow_ptr[I];
-      const int64_t col0 = (int64_t)ct * K3_NT;
+      const int64_t col0 = (int64_t)ct * K3_NT;          // first column of the item
+      const int64_t colw = col0 + half * NCW;            // first column of this warp
       const int64_t row = (int64_t)I * b + r;
       if (et < 64) {
         const int64_t cj = col0 + et;
@@ -368,23 +378,19 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       if (row_ok) {
         rsp = alpha * pow2i(prm.eH[row] - 30);    // alpha * 2^(eH_i - 14) / 2^16 (k3_drain returns 2^16 * v)
         gi = fma(alpha, prm.hdiag[row], prm.gamma);
-        // This thread reads its own row of Y_k and Y_{k-1} (4 lines each) after the drain, 16 bytes at a time and
-        // one dependent batch after the other: without help the output phase is a chain of exposed HBM latencies
-        // (69 % of the epilogue warps' time in profiles/r01b).  Pull all eight lines into L2 now, in one burst,
-        // while the warp is about to wait for the accumulators anyway.
-        if (full) {
-          const double* sp0 = prm.S + row * prm.lds + col0;
-          const double* zp0 = prm.Z + row * prm.ldz + col0;
+        if (full) {   // pull this thread's two lines of Y_k and Y_{k-1} towards L2 while the warp waits for the accumulators
+          const double* sp0 = prm.S + row * prm.lds + colw;
+          const double* zp0 = prm.Z + row * prm.ldz + colw;
 #pragma unroll
-          for (int k = 0; k < 4; ++k) {
+          for (int k = 0; k < 2; ++k) {
             asm volatile("prefetch.global.L2 [%0];" ::"l"(sp0 + 16 * k));
             if (use_z) asm volatile("prefetch.global.L2 [%0];" ::"l"(zp0 + 16 * k));
           }
         }
       }
-      asm volatile("bar.sync 1, 128;" ::: "memory");
+      asm volatile("bar.sync 1, 256;" ::: "memory");
 
-      double v[K3_NT];
+      double v[NCW];
       const int64_t it = (u - cluster0) / nclusters;
       const bool tr = prm.trace && blockIdx.x == 0 && it < 512 && et == 0;
       if (tr) prm.trace[it * 8 + 3] = clock64();
@@ -393,52 +399,74 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         aph ^= 1;
         if (tr) prm.trace[it * 8 + 4] = clock64();
         asm volatile("tcgen05.fence::after_thread_sync;");
-        const uint32_t trow = tmem_base + ((uint32_t)(quarter * 32) << 16);
-        k3_drain<S>(trow, v);
+        k3_drain<S, NCW>(tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(half * NCW), v);
         asm volatile("tcgen05.fence::before_thread_sync;");
         mbar_arrive(accempty);                   // TMEM is free for the next work item
         if (tr) prm.trace[it * 8 + 5] = clock64();
       } else {
 #pragma unroll
-        for (int i = 0; i < K3_NT; ++i) v[i] = 0.0;
+        for (int i = 0; i < NCW; ++i) v[i] = 0.0;
       }
 
       // ---- out = alpha * 2^(eH+eY-30) * v + (alpha*hdiag + gamma) * y + beta * z   (v = 2^16 * Horner) ----
       // three fp64 instructions per element: v * (alpha 2^(eH-30)), then the column's 2^eY by an exponent add, two FMAs
-      const double* sp = prm.S + row * prm.lds + col0;
-      const double* zp = prm.Z + row * prm.ldz + col0;
-      double* op = prm.O + row * prm.ldo + col0;
-      if (prm.vec && full) {
+      uint32_t cmx = 0;                           // column maximum (upper word) this lane has seen
+      bool cmax_done = false;
+      if (full) {
+        // Coalesced output: after the drain a thread owns one ROW (32 columns); written that way every access of
+        // a warp would touch 32 different lines.  The 32 x 32 block of the warp is transposed in registers (5 shuffle
+        // stages): afterwards lane l owns column l of all 32 rows and every access is one contiguous 256-byte segment.
 #pragma unroll
-        for (int c0 = 0; c0 < K3_NT; c0 += 8) {
-          double2 y2[4], z2[4];
-          if (row_ok) {
+        for (int c = 0; c < NCW; ++c) v[c] *= rsp;               // x alpha 2^(eH_i-30), own row
 #pragma unroll
-            for (int i = 0; i < 4; ++i) y2[i] = __ldg(reinterpret_cast<const double2*>(sp + c0 + 2 * i));
-            if (use_z) {
+        for (int k = 16; k >= 1; k >>= 1) {
+          const bool up = (lane & k) != 0;
 #pragma unroll
-              for (int i = 0; i < 4; ++i) z2[i] = *reinterpret_cast<const double2*>(zp + c0 + 2 * i);
-            }
-          }
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int j = c0 + 2 * i;
-            double o0 = 0.0, o1 = 0.0;
-            if (row_ok) {
-              o0 = fma(gi, y2[i].x, scale_pow2(v[j] * rsp, ce_s[j]));
-              o1 = fma(gi, y2[i].y, scale_pow2(v[j + 1] * rsp, ce_s[j + 1]));
-              if (use_z) { o0 = fma(beta, z2[i].x, o0); o1 = fma(beta, z2[i].y, o1); }
-              *reinterpret_cast<double2*>(op + j) = make_double2(o0, o1);
-            }
-            v[j] = o0; v[j + 1] = o1;
+          for (int j = 0; j < 32; ++j) {
+            if (j & k) continue;
+            const double snd = up ? v[j] : v[j | k];
+            const double rcv = __shfl_xor_sync(0xffffffffu, snd, k);
+            if (up) v[j] = rcv; else v[j | k] = rcv;
           }
         }
-      } else {
+        // v[r] = (row r of this warp, column colw + lane)
+        const int32_t ce = ce_s[half * NCW + lane];
+        if (warp_ok) {
+          const int64_t wrow0 = (int64_t)I * b + quarter * 32;
+          const double* sw = prm.S + wrow0 * prm.lds + colw + lane;
+          const double* zw = prm.Z + wrow0 * prm.ldz + colw + lane;
+          double* ow = prm.O + wrow0 * prm.ldo + colw + lane;
 #pragma unroll
-        for (int j = 0; j < K3_NT; ++j) {
+          for (int r0 = 0; r0 < 32; r0 += 8) {
+            double y[8], z[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) y[i] = __ldg(sw + (int64_t)(r0 + i) * prm.lds);
+            if (use_z) {
+#pragma unroll
+              for (int i = 0; i < 8; ++i) z[i] = zw[(int64_t)(r0 + i) * prm.ldz];
+            }
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              const double gr = __shfl_sync(0xffffffffu, gi, r0 + i);     // alpha * hdiag + gamma of row r0+i
+              double o = fma(gr, y[i], scale_pow2(v[r0 + i], ce));
+              if (use_z) o = fma(beta, z[i], o);
+              ow[(int64_t)(r0 + i) * prm.ldo] = o;
+              cmx = max(cmx, abs_hi(o));
+            }
+          }
+        }
+        if (prm.cmaxO && cmx) atomicMax(&cm_s[half * NCW + lane], cmx);   // this lane has seen all 32 rows of its column
+        cmax_done = true;
+      } else {
+        // ragged last column tile: every thread writes its own row
+        const double* sp = prm.S + row * prm.lds + colw;
+        const double* zp = prm.Z + row * prm.ldz + colw;
+        double* op = prm.O + row * prm.ldo + colw;
+#pragma unroll
+        for (int j = 0; j < NCW; ++j) {
           double o = 0.0;
-          if (row_ok && col0 + j < prm.ncols) {
-            o = fma(gi, sp[j], scale_pow2(v[j] * rsp, ce_s[j]));
+          if (row_ok && colw + j < prm.ncols) {
+            o = fma(gi, sp[j], scale_pow2(v[j] * rsp, ce_s[half * NCW + j]));
             if (use_z) o = fma(beta, zp[j], o);
             op[j] = o;
           }
@@ -447,16 +475,18 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       }
       // ---- column maxima of the new iterate (upper words), for the next step's digit scaling ----
       if (prm.cmaxO) {
+        if (!cmax_done) {
 #pragma unroll
-        for (int j = 0; j < K3_NT; ++j) {
-          const uint32_t m = __reduce_max_sync(0xffffffffu, abs_hi(v[j]));
-          if (lane == (j & 31) && m) atomicMax(&cm_s[j], m);
+          for (int j = 0; j < NCW; ++j) {
+            const uint32_t m = __reduce_max_sync(0xffffffffu, abs_hi(v[j]));
+            if (lane == j && m) atomicMax(&cm_s[half * NCW + j], m);
+          }
         }
-        asm volatile("bar.sync 1, 128;" ::: "memory");
+        asm volatile("bar.sync 1, 256;" ::: "memory");
         if (et < 64 && col0 + et < prm.ncols && cm_s[et]) atomicMax(&prm.cmaxO[col0 + et], cm_s[et]);
       }
       if (tr) prm.trace[it * 8 + 6] = clock64();
-      asm volatile("bar.sync 1, 128;" ::: "memory");   // ce_s / cm_s are rewritten by the next item
+      asm volatile("bar.sync 1, 256;" ::: "memory");   // ce_s / cm_s are rewritten by the next item
     }
   }
 

@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(256) gram_reduce_kernel(const double* __restri
 //       of a cluster fetches 64/C columns of both tiles of a plane (two boxes) and multicasts them;
 // tmWd: 3-D map of the W digit tiles, box S x 64 x 128 B (as K3's Y map).
 template <int S, int C>
-__global__ void __launch_bounds__(K3_THREADS, 1)
+__global__ void __launch_bounds__(K4_THREADS, 1)
 gram_i8_kernel(const __grid_constant__ CUtensorMap tmXd, const __grid_constant__ CUtensorMap tmWd, const K4Params prm) {
   using Cf = K3Cfg<S>;
   constexpr int NH = Cf::NH;
@@ -225,7 +225,7 @@ gram_i8_kernel(const __grid_constant__ CUtensorMap tmXd, const __grid_constant__
       aph ^= 1;
       asm volatile("tcgen05.fence::after_thread_sync;");
       const uint32_t trow = tmem_base + ((uint32_t)(quarter * 32) << 16);
-      k3_drain<S>(trow, v);
+      k3_drain<S, K3_NT>(trow, v);
       asm volatile("tcgen05.fence::before_thread_sync;");
       mbar_arrive(accempty);
 

@@ -593,10 +593,10 @@ I8Work carve_i8_work(const ttdft_h_s* h, void* base, int64_t w) {
 
 // launch configuration of bsr_i8_kernel<S, C>: one CTA per SM (shared memory), clusters of C along the grid
 template <int S, int C>
-void k3_launch_config(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* at, unsigned grid, cudaStream_t st) {
+void k3_launch_config(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* at, unsigned grid, cudaStream_t st, int threads = ttdft::K3_THREADS) {
   *cfg = cudaLaunchConfig_t{};
   cfg->gridDim = dim3(grid);
-  cfg->blockDim = dim3(ttdft::K3_THREADS);
+  cfg->blockDim = dim3(threads);
   cfg->dynamicSmemBytes = ttdft::K3Cfg<S>::TOTAL;
   cfg->stream = st;
   at[0].id = cudaLaunchAttributeClusterDimension;
@@ -891,7 +891,7 @@ ttdft_status launch_k4(const GramPlan& g, const CUtensorMap& tmXd, const CUtenso
   if (items == 0) return TTDFT_OK;
   cudaLaunchConfig_t cfg;
   cudaLaunchAttribute at[1];
-  k3_launch_config<S, C>(&cfg, at, (unsigned)(std::min<int64_t>(items, g.nsm / C) * C), st);
+  k3_launch_config<S, C>(&cfg, at, (unsigned)(std::min<int64_t>(items, g.nsm / C) * C), st, ttdft::K4_THREADS);
   TimedLaunch tl(6, st);
   CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, tmXd, tmWd, p));
   g_launches.fetch_add(1);
