@@ -51,6 +51,7 @@ struct K3Params {
   const double* hdiag;             // diagonal of H (fp64)         [M]
   const uint32_t* cmaxS;           // column maxima of Y_k (upper words)   [ncols]
   uint32_t* cmaxO;                 // out: column maxima of O, or NULL
+  int32_t l2hints;                 // 1: evict-first H planes, evict-last Y digit tiles; 2: only the latter; 0: none
   unsigned long long* trace;       // debug (ttdft_debug_k3_trace): 8 clock64 stamps per work item of CTA 0, or NULL
 };
 
@@ -75,6 +76,33 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, i
       "l"(map), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar))
       : "memory");
 }
+// L2 eviction-priority hints for TMA loads (the fixed policy encodings CUTLASS passes as cache hints)
+constexpr uint64_t L2_EVICT_FIRST = 0x12F0000000000000ull;   // streamed once: the H digit planes
+constexpr uint64_t L2_EVICT_LAST = 0x14F0000000000000ull;    // reused by up to 27 block rows: the Y digit tiles
+__device__ __forceinline__ void tma_load_3d_hint(void* dst, const CUtensorMap* map, int32_t x, int32_t y, int32_t z, uint64_t* bar,
+                                                 uint64_t hint) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;" ::"r"(
+          smem_u32(dst)),
+      "l"(map), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar)), "l"(hint)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_2d_hint(void* dst, const CUtensorMap* map, int32_t x, int32_t y, uint64_t* bar, uint64_t hint) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;" ::"r"(
+          smem_u32(dst)),
+      "l"(map), "r"(x), "r"(y), "r"(smem_u32(bar)), "l"(hint)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_2d_mc_hint(void* dst, const CUtensorMap* map, int32_t x, int32_t y, uint64_t* bar, uint16_t mask,
+                                                    uint64_t hint) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5, %6;" ::"r"(
+          smem_u32(dst)),
+      "l"(map), "r"(x), "r"(y), "r"(smem_u32(bar)), "h"(mask), "l"(hint)
+      : "memory");
+}
+
 // shared-memory matrix descriptor: K-major rows of 128 bytes, SWIZZLE_128B, 8-row groups 1024 B apart
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
   return (uint64_t)((saddr & 0x3ffffu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) |
@@ -271,16 +299,21 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
           const int32_t J = prm.bcol[p];
           mbar_wait(&yempty[yb], yph ^ 1);
           mbar_expect_tx(&yfull[yb], (uint32_t)Cf::YBUF);
-          tma_load_3d(ybuf + yb * Cf::YBUF, &tmYd, 0, 0, (J * prm.nct + ct) * S, &yfull[yb]);
+          if (prm.l2hints) tma_load_3d_hint(ybuf + yb * Cf::YBUF, &tmYd, 0, 0, (J * prm.nct + ct) * S, &yfull[yb], L2_EVICT_LAST);
+          else tma_load_3d(ybuf + yb * Cf::YBUF, &tmYd, 0, 0, (J * prm.nct + ct) * S, &yfull[yb]);
 #pragma unroll 1
           for (int q = 0; q < S; ++q) {
             mbar_wait(&hempty[hs], hph ^ 1);       // all C CTAs have finished with this slot
             mbar_expect_tx(&hfull[hs], (uint32_t)b * 128u);
-            if (C > 1)
-              tma_load_2d_mc(hring + hs * Cf::HSLOT + crank * hrows * 128, &tmHd, 0, (p * prm.hplanes + k3_plane<S>(q)) * b + crank * hrows,
-                             &hfull[hs], cmask);
-            else
-              tma_load_2d(hring + hs * Cf::HSLOT, &tmHd, 0, (p * prm.hplanes + k3_plane<S>(q)) * b, &hfull[hs]);
+            uint8_t* hdst = hring + hs * Cf::HSLOT + (C > 1 ? crank * hrows * 128 : 0);
+            const int32_t hrow = (p * prm.hplanes + k3_plane<S>(q)) * b + (C > 1 ? crank * hrows : 0);
+            if (C > 1) {
+              if (prm.l2hints == 1) tma_load_2d_mc_hint(hdst, &tmHd, 0, hrow, &hfull[hs], cmask, L2_EVICT_FIRST);
+              else tma_load_2d_mc(hdst, &tmHd, 0, hrow, &hfull[hs], cmask);
+            } else {
+              if (prm.l2hints == 1) tma_load_2d_hint(hdst, &tmHd, 0, hrow, &hfull[hs], L2_EVICT_FIRST);
+              else tma_load_2d(hdst, &tmHd, 0, hrow, &hfull[hs]);
+            }
             if (++hs == NH) { hs = 0; hph ^= 1; }
           }
           yb ^= 1;
@@ -440,17 +473,17 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
           for (int r0 = 0; r0 < 32; r0 += 8) {
             double y[8], z[8];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) y[i] = __ldg(sw + (int64_t)(r0 + i) * prm.lds);
+            for (int i = 0; i < 8; ++i) y[i] = __ldcs(sw + (int64_t)(r0 + i) * prm.lds);      // read once: evict first
             if (use_z) {
 #pragma unroll
-              for (int i = 0; i < 8; ++i) z[i] = zw[(int64_t)(r0 + i) * prm.ldz];
+              for (int i = 0; i < 8; ++i) z[i] = __ldcs(zw + (int64_t)(r0 + i) * prm.ldz);
             }
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
               const double gr = __shfl_sync(0xffffffffu, gi, r0 + i);     // alpha * hdiag + gamma of row r0+i
               double o = fma(gr, y[i], scale_pow2(v[r0 + i], ce));
               if (use_z) o = fma(beta, z[i], o);
-              ow[(int64_t)(r0 + i) * prm.ldo] = o;
+              __stcs(ow + (int64_t)(r0 + i) * prm.ldo, o);
               cmx = max(cmx, abs_hi(o));
             }
           }
