@@ -50,14 +50,23 @@ __device__ __forceinline__ void tma_load_4d_mc(void* dst, const CUtensorMap* map
       : "memory");
 }
 
-// cluster work item u -> (chunk, row tile ctx, tile group ctwg): chunks outermost, then row tiles, tile groups
-// fastest -- clusters that run at the same time walk the same blocks of the contraction and share both operands in L2
+// cluster work item u -> (chunk, row tile ctx, tile group ctwg).  Chunks outermost; inside a chunk the tiles of G are
+// walked in super-tiles of 8 row tiles x 9 tile groups (72 ~ the 74 co-resident 2-CTA clusters), so that the clusters
+// running at the same time walk the same blocks of the contraction on few distinct operand tiles: 8 X tile pairs +
+// 18 W tiles per block instead of 2-3 X pairs + 64 W tiles, i.e. each W tile is fetched from HBM once per 8 row tiles
+// instead of once per row tile.
 __device__ __forceinline__ void k4_decode(const K4Params& prm, int64_t u, int32_t& chunk, int32_t& ctx, int32_t& ctwg) {
+  constexpr int SX = 8, SW = 9;
   const int64_t per_chunk = (int64_t)prm.nctx * prm.nctwg;
   chunk = (int32_t)(u / per_chunk);
-  const int64_t rem = u - (int64_t)chunk * per_chunk;
-  ctx = (int32_t)(rem / prm.nctwg);
-  ctwg = (int32_t)(rem - (int64_t)ctx * prm.nctwg);
+  const int32_t rem = (int32_t)(u - (int64_t)chunk * per_chunk);
+  const int32_t sx = rem / (SX * prm.nctwg);
+  const int32_t hx = min(SX, prm.nctx - sx * SX);            // row tiles in this super row
+  const int32_t rem2 = rem - sx * SX * prm.nctwg;
+  const int32_t sw = rem2 / (hx * SW);
+  const int32_t rem3 = rem2 - sw * hx * SW;
+  ctx = sx * SX + rem3 % hx;
+  ctwg = sw * SW + rem3 / hx;
 }
 
 // P[chunk] summed in ascending chunk order:  G[j, colw0 + l] = sum_c P[c][j][l]
