@@ -714,7 +714,6 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
   p.eH = h->eH; p.hdiag = h->hdiag; p.cmaxS = cmS; p.cmaxO = cmO;
   p.trace = g_k3_trace;
   p.l2hints = env_int("TTDFT_K3_L2HINTS", 1);
-  if (p.vec && env_int("TTDFT_DEBUG_NOFP64", 0)) p.vec = 2;
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
   // column tiles in clusters of C; a remainder of < C tiles runs as single CTAs
