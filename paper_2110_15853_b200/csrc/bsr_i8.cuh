@@ -10,17 +10,18 @@
 //     a tile are contiguous in HBM) into one of two Y buffers, and the S digit planes of H_IJ (b x 128 B
 //     each) through a ring of 16 KB slots.  Every CTA of the cluster fetches b/C rows of each H plane and
 //     MULTICASTS them into the same slot of all C CTAs, so a plane leaves L2 once per cluster: the kernel
-//     was bound by L2->SM throughput before (profiles/r01a_*), H being 2/3 of those bytes
+//     was bound by L2->SM throughput before (profiles/r01a_*), H being 2/3 of those bytes.  H planes carry an
+//     L2 evict-first hint (streamed), Y tiles evict-last (re-used by up to 27 block rows)
 //   * warp 1 (one lane): tcgen05.mma.kind::i8 issuer.  For H plane p it multiplies against the
 //     CONCATENATION of Y planes 0..S-1-p (N = 64*(S-p), issued as <=256-column instructions), which lands
 //     in the contiguous TMEM column groups p..S-1 because digit-pair level g = p+q lives at columns
-//     [64g, 64g+64).  S(S+1)/2 plane pairs cost 4+... wide MMAs instead of S(S+1)/2 narrow ones, so the
-//     A operand is read from shared memory once per plane and the tensor pipe, not shared memory, binds
-//   * accumulators: S levels x 64 columns of int32 in TMEM (384 of 512 columns for S = 6), exact
-//   * warps 2-5: epilogue.  Each thread owns one row: Horner over the levels (least significant first)
-//     into 64 fp64 registers, releases TMEM, then  out = alpha*2^(eH_i+eY_j-14)*v + (alpha*hdiag_i+gamma)*y
-//     + beta*z  with 128-bit accesses, and accumulates the column maxima of `out` for the next step's
-//     digit scaling (warp REDUX + shared/global atomicMax on the upper word)
+//     [64g, 64g+64): 10 wide MMAs per k-step instead of S(S+1)/2 = 28 narrow ones
+//   * accumulators: S levels x 64 columns of int32 in TMEM (448 of 512 columns for S = 7), exact
+//   * warps 2-9: epilogue, two warps per TMEM lane quarter (32 columns each).  Drain: three int32 levels are packed
+//     exactly into one int64 before the conversion to fp64; TMEM released.  Output: the warp's 32 x 32 block is
+//     transposed in registers so that every access is one contiguous 256-byte row segment, then
+//     out = scale_pow2(alpha*2^(eH_i-30)*v, eY_j) + (alpha*hdiag_i+gamma)*y + beta*z, and the column maxima of `out`
+//     for the next step's digit scaling (per lane, then shared/global atomicMax on the upper word)
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
