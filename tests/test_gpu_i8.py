@@ -200,3 +200,32 @@ def test_auto_mode_is_i8x7_for_wide_tiles(tt):
     H, C, _, _ = small_problem(4, 32, 0.0, 1001)
     Hd = tt.h_build_bsr(H.M, H.b, dev(H.row_ptr), dev(H.col_idx), dev(H.values))
     assert Hd.info()["math"] == tt.MATH_FP64
+
+
+@pytest.mark.parametrize("cluster,hints", [("1", "1"), ("2", "0"), ("2", "2"), ("4", "1"), ("8", "1")])
+def test_cluster_sizes_and_l2_hints(tt, cluster, hints):
+    """Every cluster size of K3 (TMA multicast of the H planes across 1/2/4/8 CTAs, incl. the single-CTA remainder launch
+    when the tile count is not a multiple of the cluster size) and every L2-hint mode gives the same bits."""
+    import os
+    import torch
+    H, C, (rp, col, val), (a0, bb) = small_problem(3, 128, 0.4, 2128)
+    N, m = 5 * 64 + 7, 5                                     # 6 column tiles: 4 + remainder 2 under 4-CTA clusters
+    a, bb, a0 = bounds_for(a0, bb, N, H.M, wide=True)
+    X = synth.dense_normal(H.M, N, 71)
+    ref = oracle.cheb_filter(rp, col, val, X, m, a, bb, a0)
+    out = {}
+    for env in (None, (cluster, hints)):
+        for k in ("TTDFT_K3_CLUSTER", "TTDFT_K3_L2HINTS"):
+            os.environ.pop(k, None)
+        if env:
+            os.environ["TTDFT_K3_CLUSTER"], os.environ["TTDFT_K3_L2HINTS"] = env
+        try:
+            Hd = build_i8(tt, H, mode="i8x7")
+            Y = torch.empty(H.M, N, dtype=torch.float64, device="cuda")
+            tt.cheb_filter(Hd, dev(X), Y, m, a, bb, a0)
+            out[env] = Y.cpu().numpy()
+        finally:
+            for k in ("TTDFT_K3_CLUSTER", "TTDFT_K3_L2HINTS"):
+                os.environ.pop(k, None)
+    assert relerr(out[None], ref) <= TOL_FILTER
+    assert np.array_equal(out[None], out[(cluster, hints)])
