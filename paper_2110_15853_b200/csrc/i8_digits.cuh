@@ -35,16 +35,35 @@ __host__ __device__ __forceinline__ int32_t exp_from_hi(uint32_t hi) {
 // 2^k as a double, k in [-1022, 1023]
 __device__ __forceinline__ double pow2i(int32_t k) { return __longlong_as_double((long long)(k + 1023) << 52); }
 
-// Balanced base-256 digits of q = rn(x * scale), most significant first; |q| <= 0.9961 * 2^(8S-1).
+// Digit planes of FOUR values at once, packed for the k-major operand layout: w[p] = bytes (digit p of x0, x1, x2, x3).
+// q + B with B = 0x80...80 (S bytes) has the plain base-256 bytes d_i + 128 of the balanced digits d_i, so
+// t = (q + B) ^ B holds every digit as a two's-complement byte -- one 64-bit add and xor instead of a digit loop --
+// and a 4 x S byte transpose (PRMT) gathers byte i of the four values.  Byte i of t is the digit of weight 256^i,
+// i.e. plane S-1-i.  This is what makes y_digits memory-bound instead of issue-bound at the filter's power-limited clock.
 template <int S>
-__device__ __forceinline__ void balanced_digits(double x, double scale, int32_t (&d)[S]) {
-  long long q = __double2ll_rn(x * scale);
+__device__ __forceinline__ void digits4(const double (&x)[4], double scale, uint32_t (&w)[S]) {
+  static_assert(S >= 5 && S <= 8, "4 low bytes + up to 4 high bytes");
+  constexpr unsigned long long B = 0x8080808080808080ull >> (8 * (8 - S));
+  uint32_t lo[4], hi[4];
 #pragma unroll
-  for (int p = S - 1; p >= 0; --p) {
-    const int32_t lo = (int32_t)(q & 0xff);
-    const int32_t dd = (lo ^ 0x80) - 0x80;   // sign-extend the low byte
-    d[p] = dd;
-    q = (q - dd) >> 8;
+  for (int i = 0; i < 4; ++i) {
+    const unsigned long long t = ((unsigned long long)__double2ll_rn(x[i] * scale) + B) ^ B;
+    lo[i] = (uint32_t)t;
+    hi[i] = (uint32_t)(t >> 32);
+  }
+  uint32_t a = __byte_perm(lo[0], lo[1], 0x5140), b = __byte_perm(lo[2], lo[3], 0x5140);
+  uint32_t c = __byte_perm(lo[0], lo[1], 0x7362), d = __byte_perm(lo[2], lo[3], 0x7362);
+  w[S - 1] = __byte_perm(a, b, 0x5410);
+  w[S - 2] = __byte_perm(a, b, 0x7632);
+  w[S - 3] = __byte_perm(c, d, 0x5410);
+  w[S - 4] = __byte_perm(c, d, 0x7632);
+  a = __byte_perm(hi[0], hi[1], 0x5140); b = __byte_perm(hi[2], hi[3], 0x5140);
+  w[S - 5] = __byte_perm(a, b, 0x5410);
+  if (S >= 6) w[S - 6] = __byte_perm(a, b, 0x7632);
+  if (S >= 7) {
+    c = __byte_perm(hi[0], hi[1], 0x7362); d = __byte_perm(hi[2], hi[3], 0x7362);
+    w[S - 7] = __byte_perm(c, d, 0x5410);
+    if (S >= 8) w[0] = __byte_perm(c, d, 0x7632);
   }
 }
 
@@ -111,15 +130,7 @@ __global__ void __launch_bounds__(256) y_digits_kernel(const double* __restrict_
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       uint32_t w[S];
-#pragma unroll
-      for (int p = 0; p < S; ++p) w[p] = 0;
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        int32_t d[S];
-        balanced_digits<S>(x[h][i], scale[h], d);
-#pragma unroll
-        for (int p = 0; p < S; ++p) w[p] |= (uint32_t)(d[p] & 0xff) << (8 * i);
-      }
+      digits4<S>(x[h], scale[h], w);
 #pragma unroll
       for (int p = 0; p < S; ++p) sd[(p * 64 + 32 * h + lane) * 33 + quad] = w[p];
     }
@@ -177,20 +188,13 @@ __global__ void __launch_bounds__(256) h_digits_kernel(int32_t b, const int32_t*
     for (int r = warp; r < b; r += 8) {
       const double scale = pow2i(8 * S - 1 - eH[(int64_t)I * b + r]);
       uint32_t w[S];
-#pragma unroll
-      for (int q = 0; q < S; ++q) w[q] = 0;
+      double x[4] = {0.0, 0.0, 0.0, 0.0};      // columns >= b of the 128-byte row stay zero
       if (4 * lane < b) {
         const double* src = tiles + ((size_t)p * b + r) * b + 4 * lane;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          double x = src[i];
-          if (diag_tile && 4 * lane + i == r) x = 0.0;
-          int32_t d[S];
-          balanced_digits<S>(x, scale, d);
-#pragma unroll
-          for (int q = 0; q < S; ++q) w[q] |= (uint32_t)(d[q] & 0xff) << (8 * i);
-        }
+        for (int i = 0; i < 4; ++i) x[i] = (diag_tile && 4 * lane + i == r) ? 0.0 : src[i];
       }
+      digits4<S>(x, scale, w);
 #pragma unroll
       for (int q = 0; q < S; ++q)
         reinterpret_cast<uint32_t*>(Hd + (((size_t)p * S + q) * b + r) * 128)[lane] = w[q];
