@@ -424,6 +424,25 @@ def main():
             line["project"]["gpu_vs_oracle_relerr_on_sample"] = float(np.linalg.norm(gotp - ref) / np.linalg.norm(ref))
             del Cn
         del Gd, pw
+        # ---- Algorithm 1 step 5: rotation Psi = X Q (ttdft_rotate), Q a seeded N x N matrix (1 warm-up + 2 timed) ----
+        Qd = torch.randn(cfg.N, cfg.N, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(cfg.seed))
+        rw = torch.empty(tt.rotate_work_bytes(cfg.M, cfg.N, cfg.N) + 1024, dtype=torch.uint8, device=dev)
+        tt.rotate(Xd, Qd, Yd, work=rw)
+        torch.cuda.synchronize()
+        g0.record()
+        for _ in range(2):
+            tt.rotate(Xd, Qd, Yd, work=rw)
+        g1.record()
+        torch.cuda.synchronize()
+        t_r = g0.elapsed_time(g1) * 1e-3 / 2
+        line["rotate"] = {"what": "Psi = X Q, Algorithm 1 step 5 (ttdft_rotate): kernel K3 on row-scaled digit tiles of X",
+                          "ms": t_r * 1e3, "fp64_equivalent_tflops": fl_gram / t_r / 1e12, "steps": 2, "warmup": 1,
+                          "frac_of_fp64_peak": fl_gram / t_r / 1e12 / FP64_PEAK_TFLOPS}
+        if not args.no_cpu_baseline:
+            rr = torch.from_numpy(np.unique(np.random.default_rng(cfg.seed).integers(0, cfg.M, 16))).to(dev)
+            refr = oracle.rotate(np.ascontiguousarray(Xd[rr].cpu().numpy()), Qd.cpu().numpy())
+            line["rotate"]["gpu_vs_oracle_relerr_on_sample"] = float(np.linalg.norm(Yd[rr].cpu().numpy() - refr) / np.linalg.norm(refr))
+        del Qd, rw
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         dt, _, cols, Xs, Yo, threads = oracle_sample_run(cfg, H, args.ref_cols, cfg.m, (a, b, a0))

@@ -227,6 +227,19 @@ ttdft_status ttdft_project_work_bytes(ttdft_h_t h, int64_t ncols, size_t* bytes)
 ttdft_status ttdft_project(ttdft_h_t h, const double* X, int64_t ldx, int64_t ncols, double* G, int64_t ldg, void* work,
                            size_t work_bytes, void* stream);
 
+/*
+ * Algorithm 1 step 5 ("Rotate the basis Psi = X Q") and the product every
+ * orthonormalisation of step 2 ends with (X R^-1):
+ *     Y = X * Q          X: M x k row-major (ldx >= k), Q: k x n row-major (ldq >= n), Y: M x n row-major (ldy >= n)
+ * computed by the int8 tensor-core step kernel: X is cut into 128 x 128 tiles of 7 digit planes scaled per ROW of X,
+ * Q into digit tiles scaled per COLUMN of Q, all accumulation exact in int32 (k <= 18560), recombined in fp64:
+ * error below an fp64 dot product's bound.  Y must not overlap X or Q.  M >= 0, k >= 1, n >= 1.
+ * `work`: 1024-byte aligned DEVICE scratch of at least ttdft_rotate_work_bytes (about 7/8 of the bytes of X).
+ */
+ttdft_status ttdft_rotate_work_bytes(int64_t M, int64_t k, int64_t n, size_t* bytes);
+ttdft_status ttdft_rotate(int64_t M, const double* X, int64_t ldx, int64_t k, const double* Q, int64_t ldq, int64_t n, double* Y,
+                          int64_t ldy, void* work, size_t work_bytes, void* stream);
+
 /* Measured fp64 rate of this GPU: kind 0 = scalar DFMA loop, 1 = DMMA (mma.sync m8n8k4.f64) loop;
  * runs for about `millis` ms on `stream`, synchronises, returns TFLOP/s in *tflops. */
 ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, double* tflops);

@@ -75,6 +75,8 @@ def lib() -> ctypes.CDLL:
             fn.argtypes = [i64, _i32p, _i32p, _f64p, vp, i64, vp, i64, i64, i32, f64, f64, f64]
         L.oracle_lanczos_bounds.restype = ctypes.c_int
         L.oracle_gram.argtypes = [i64, i64, vp, i64, vp, i64, vp, i64]
+        L.oracle_rotate.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64]
+        L.oracle_rotate.restype = None
         L.oracle_gram.restype = None
         L.oracle_lanczos_bounds.argtypes = [i64, _i32p, _i32p, _f64p, i32, _f64p, _f64p, _f64p, _f64p, _f64p,
                                             ctypes.POINTER(f64), ctypes.POINTER(f64)]
@@ -196,3 +198,18 @@ def gram(X: np.ndarray, W: np.ndarray) -> np.ndarray:
 def project(row_ptr, col, val, X: np.ndarray) -> np.ndarray:
     """H_F = X^T (H X) (Algorithm 1 step 3): the oracle's SpMM followed by the oracle's Gram product."""
     return gram(X, spmm(row_ptr, col, val, 1.0, X))
+
+
+def rotate(X: np.ndarray, Q: np.ndarray) -> np.ndarray:
+    """Y = X Q by the plain definition (oracle_rotate; Algorithm 1 step 5)."""
+    M, K = X.shape
+    assert Q.shape[0] == K
+    n = Q.shape[1]
+    Y = np.zeros((M, n), np.float64)
+    if M == 0:
+        return Y
+    xp, ldx = _mat(X)
+    qp, ldq = _mat(Q)
+    yp, ldy = _mat(Y)
+    lib().oracle_rotate(M, K, n, xp, ldx, qp, ldq, yp, ldy)
+    return Y

@@ -23,7 +23,9 @@
 // projection H_F = X_F^T (H X_F) (Algorithm 1 step 3; Sec. 4.3); the projection itself is
 // oracle_spmm_csr followed by oracle_gram.  Pins P7 (tests/test_oracle_pins.py): hand-computed integers
 // (tests/golden/gram_pins.txt), numpy's matmul, Q^T H Q = Lambda for a known eigendecomposition, symmetry,
-// congruence (XR)^T H (XR) = R^T (X^T H X) R and the trace identity.
+// congruence (XR)^T H (XR) = R^T (X^T H X) R and the trace identity.  oracle_rotate is the plain definition of
+// Y = X Q (Algorithm 1 step 5); pins P8: hand-computed integers, numpy's matmul, Q = I and a column
+// permutation (exact), and the identity (XQ)^T (XQ) = Q^T (X^T X) Q through oracle_gram.
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
@@ -223,6 +225,21 @@ void oracle_gram(int64_t M, int64_t n, const double* X, int64_t ldx, const doubl
       const double x = X[k * ldx + j];
       const double* w = W + k * ldw;
       for (int64_t l = 0; l < n; ++l) g[l] = g[l] + x * w[l];
+    }
+  }
+}
+
+// Y = X Q (Algorithm 1 step 5 "Rotate the basis"): Y[i,l] = sum_k X[i,k] * Q[k,l], k ascending.
+// X: M x K (ldx), Q: K x n (ldq), Y: M x n (ldy), all row-major.  Parallel over the rows of Y only.
+void oracle_rotate(int64_t M, int64_t K, int64_t n, const double* X, int64_t ldx, const double* Q, int64_t ldq, double* Y, int64_t ldy) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < M; ++i) {
+    double* y = Y + i * ldy;
+    for (int64_t l = 0; l < n; ++l) y[l] = 0.0;
+    for (int64_t k = 0; k < K; ++k) {
+      const double x = X[i * ldx + k];
+      const double* q = Q + k * ldq;
+      for (int64_t l = 0; l < n; ++l) y[l] = y[l] + x * q[l];
     }
   }
 }

@@ -39,4 +39,6 @@ from .api import (  # noqa: F401
     gram_work_bytes,
     project,
     project_work_bytes,
+    rotate,
+    rotate_work_bytes,
 )

@@ -21,6 +21,7 @@ exported_symbols = [
     "ttdft_h_set_math_mode", "ttdft_step_work_bytes", "ttdft_spmm_ws", "ttdft_cheb_step_ws",
     "ttdft_timing_enable", "ttdft_timing_read",
     "ttdft_gram_work_bytes", "ttdft_gram", "ttdft_project_work_bytes", "ttdft_project",
+    "ttdft_rotate_work_bytes", "ttdft_rotate",
 ]
 
 
@@ -100,6 +101,10 @@ def _load() -> ctypes.CDLL:
     L.ttdft_project_work_bytes.argtypes = [c_void_p, c_int64, POINTER(c_size_t)]
     L.ttdft_project.restype = st
     L.ttdft_project.argtypes = [c_void_p, c_void_p, c_int64, c_int64, c_void_p, c_int64, c_void_p, c_size_t, c_void_p]
+    L.ttdft_rotate_work_bytes.restype = st
+    L.ttdft_rotate_work_bytes.argtypes = [c_int64, c_int64, c_int64, POINTER(c_size_t)]
+    L.ttdft_rotate.restype = st
+    L.ttdft_rotate.argtypes = [c_int64, c_void_p, c_int64, c_int64, c_void_p, c_int64, c_int64, c_void_p, c_int64, c_void_p, c_size_t, c_void_p]
     L.ttdft_probe_fp64_peak.restype = st
     L.ttdft_probe_fp64_peak.argtypes = [c_int32, c_int32, c_void_p, POINTER(c_double)]
     L.ttdft_timing_enable.restype = st
@@ -394,6 +399,26 @@ def project(H: Hamiltonian, X, G, work=None, stream=None):
     wp, wb, keep = _aligned_work(project_work_bytes(H, N), work, X.device)
     _check(_load().ttdft_project(H.handle, xp, ldx, N, gp, ldg, wp, wb, _stream(stream)))
     return G
+
+
+def rotate_work_bytes(M: int, k: int, n: int) -> int:
+    out = c_size_t(0)
+    _check(_load().ttdft_rotate_work_bytes(M, k, n, byref(out)))
+    return int(out.value)
+
+
+def rotate(X, Q, Y, work=None, stream=None):
+    """Y = X Q (ttdft_rotate; Algorithm 1 step 5): X row-major M x k, Q row-major k x n, Y row-major M x n."""
+    xp, ldx = _mat(X, "X")
+    qp, ldq = _mat(Q, "Q")
+    yp, ldy = _mat(Y, "Y")
+    M, k = X.shape
+    n = Q.shape[1]
+    if Q.shape[0] != k or tuple(Y.shape) != (M, n):
+        raise ValueError("shape mismatch")
+    wp, wb, keep = _aligned_work(rotate_work_bytes(M, k, n), work, X.device)
+    _check(_load().ttdft_rotate(M, xp, ldx, k, qp, ldq, n, yp, ldy, wp, wb, _stream(stream)))
+    return Y
 
 
 def probe_fp64_peak(kind: int = 1, millis: int = 200, stream=None) -> float:

@@ -45,13 +45,14 @@ struct K3Params {
   int32_t hplanes;                 // digit planes STORED per tile of H (>= S; the kernel uses the leading S)
   int64_t ncols;
   double alpha, gamma, beta;
-  const double* S;  int64_t lds;   // Y_k at the output position (diagonal + shift term)
+  const double* S;  int64_t lds;   // Y_k at the output position (diagonal + shift term); NULL: no such term
   const double* Z;  int64_t ldz;   // Y_{k-1}; unused if beta == 0
   double* O;        int64_t ldo;
   const int32_t* eH;               // row exponents of H          [M]
-  const double* hdiag;             // diagonal of H (fp64)         [M]
+  const double* hdiag;             // diagonal of H (fp64)         [M]; NULL: zero
   const uint32_t* cmaxS;           // column maxima of Y_k (upper words)   [ncols]
   uint32_t* cmaxO;                 // out: column maxima of O, or NULL
+  int64_t mrows;                   // valid rows (= nb*b for a Hamiltonian; < nb*b for the ragged last block of ttdft_rotate)
   int32_t l2hints;                 // 1: evict-first H planes, evict-last Y digit tiles; 2: only the latter; 0: none
   unsigned long long* trace;       // debug (ttdft_debug_k3_trace): 8 clock64 stamps per work item of CTA 0, or NULL
 };
@@ -393,6 +394,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
     const bool warp_ok = (quarter * 32) < b;     // b is a multiple of 32: a warp's rows are all valid or all padding
     const double alpha = prm.alpha, beta = prm.beta;
     const bool use_z = (beta != 0.0);
+    const bool use_s = (prm.S != nullptr);
     uint32_t aph = 0;
     for (int64_t u = cluster0; u < nitems; u += nclusters) {
       int32_t I, ctg;
@@ -402,6 +404,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       const int64_t col0 = (int64_t)ct * K3_NT;          // first column of the item
       const int64_t colw = col0 + half * NCW;            // first column of this warp
       const int64_t row = (int64_t)I * b + r;
+      const bool row_in = row_ok && row < prm.mrows;
       if (et < 64) {
         const int64_t cj = col0 + et;
         ce_s[et] = exp_from_hi(cj < prm.ncols ? prm.cmaxS[cj] : 0u);
@@ -409,15 +412,15 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       }
       double rsp = 0.0, gi = prm.gamma;
       const bool full = (col0 + K3_NT <= prm.ncols);
-      if (row_ok) {
+      if (row_in) {
         rsp = alpha * pow2i(prm.eH[row] - 30);    // alpha * 2^(eH_i - 14) / 2^16 (k3_drain returns 2^16 * v)
-        gi = fma(alpha, prm.hdiag[row], prm.gamma);
+        gi = prm.hdiag ? fma(alpha, prm.hdiag[row], prm.gamma) : prm.gamma;
         if (full) {   // pull this thread's two lines of Y_k and Y_{k-1} towards L2 while the warp waits for the accumulators
           const double* sp0 = prm.S + row * prm.lds + colw;
           const double* zp0 = prm.Z + row * prm.ldz + colw;
 #pragma unroll
           for (int k = 0; k < 2; ++k) {
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(sp0 + 16 * k));
+            if (use_s) asm volatile("prefetch.global.L2 [%0];" ::"l"(sp0 + 16 * k));
             if (use_z) asm volatile("prefetch.global.L2 [%0];" ::"l"(zp0 + 16 * k));
           }
         }
@@ -470,22 +473,30 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
           const double* sw = prm.S + wrow0 * prm.lds + colw + lane;
           const double* zw = prm.Z + wrow0 * prm.ldz + colw + lane;
           double* ow = prm.O + wrow0 * prm.ldo + colw + lane;
+          const int nrow = (int)min((int64_t)32, prm.mrows - wrow0);       // < 32 only in a ragged last block (warp-uniform)
 #pragma unroll
           for (int r0 = 0; r0 < 32; r0 += 8) {
-            double y[8], z[8];
+            if (r0 < nrow) {
+              double y[8], z[8];
+              if (use_s) {
 #pragma unroll
-            for (int i = 0; i < 8; ++i) y[i] = __ldcs(sw + (int64_t)(r0 + i) * prm.lds);      // read once: evict first
-            if (use_z) {
+                for (int i = 0; i < 8; ++i) y[i] = (r0 + i < nrow) ? __ldcs(sw + (int64_t)(r0 + i) * prm.lds) : 0.0;   // read once: evict first
+              }
+              if (use_z) {
 #pragma unroll
-              for (int i = 0; i < 8; ++i) z[i] = __ldcs(zw + (int64_t)(r0 + i) * prm.ldz);
-            }
+                for (int i = 0; i < 8; ++i) z[i] = (r0 + i < nrow) ? __ldcs(zw + (int64_t)(r0 + i) * prm.ldz) : 0.0;
+              }
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-              const double gr = __shfl_sync(0xffffffffu, gi, r0 + i);     // alpha * hdiag + gamma of row r0+i
-              double o = fma(gr, y[i], scale_pow2(v[r0 + i], ce));
-              if (use_z) o = fma(beta, z[i], o);
-              __stcs(ow + (int64_t)(r0 + i) * prm.ldo, o);
-              cmx = max(cmx, abs_hi(o));
+              for (int i = 0; i < 8; ++i) {
+                const double gr = __shfl_sync(0xffffffffu, gi, r0 + i);     // alpha * hdiag + gamma of row r0+i
+                double o = scale_pow2(v[r0 + i], ce);
+                if (use_s) o = fma(gr, y[i], o);
+                if (use_z) o = fma(beta, z[i], o);
+                if (r0 + i < nrow) {
+                  __stcs(ow + (int64_t)(r0 + i) * prm.ldo, o);
+                  cmx = max(cmx, abs_hi(o));
+                }
+              }
             }
           }
         }
@@ -499,8 +510,9 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
 #pragma unroll
         for (int j = 0; j < NCW; ++j) {
           double o = 0.0;
-          if (row_ok && colw + j < prm.ncols) {
-            o = fma(gi, sp[j], scale_pow2(v[j] * rsp, ce_s[half * NCW + j]));
+          if (row_in && colw + j < prm.ncols) {
+            o = scale_pow2(v[j] * rsp, ce_s[half * NCW + j]);
+            if (use_s) o = fma(gi, sp[j], o);
             if (use_z) o = fma(beta, zp[j], o);
             op[j] = o;
           }

@@ -202,4 +202,49 @@ __global__ void __launch_bounds__(256) h_digits_kernel(int32_t b, const int32_t*
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Row-scaled digit tiles of a dense row-major matrix X (M x K), the A operand of ttdft_rotate (Y = X Q):
+//   eX[i] from the maximum of row i;   Dx[(I*nkb + J)*S + q][r][k] = digit q of X[I*128 + r, J*128 + k]
+// -- the tile format of the H digit planes with tile (I, J) = rows I*128.., columns J*128.. of X.
+// ------------------------------------------------------------------------------------------------
+// one warp per row; grid ceil(Mpad/8), 256 threads.  Rows >= M get the smallest exponent.
+__global__ void __launch_bounds__(256) x_rowexp_kernel(const double* __restrict__ X, int64_t ld, int64_t M, int64_t Mpad, int64_t K,
+                                                       int32_t* __restrict__ eX) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t row = (int64_t)blockIdx.x * 8 + warp;
+  if (row >= Mpad) return;
+  uint32_t m = 0;
+  if (row < M)
+    for (int64_t k = lane; k < K; k += 32) m = max(m, abs_hi(X[row * ld + k]));
+  m = __reduce_max_sync(0xffffffffu, m);
+  if (lane == 0) eX[row] = exp_from_hi(m);
+}
+
+// grid (nbm, nkb), 256 threads: thread (r = tid/32 + 8*it, kq = tid%32) converts 4 consecutive k of one row
+template <int S>
+__global__ void __launch_bounds__(256) x_digits_rows_kernel(const double* __restrict__ X, int64_t ld, int64_t M, int64_t K,
+                                                            const int32_t* __restrict__ eX, int8_t* __restrict__ Dx) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t I = blockIdx.x, J = blockIdx.y, nkb = gridDim.y;
+  int8_t* tile = Dx + (I * nkb + J) * (int64_t)(S * 128 * 128);
+  for (int r = warp; r < 128; r += 8) {
+    const int64_t row = I * 128 + r;
+    const int64_t k0 = J * 128 + 4 * lane;
+    double x[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) x[i] = (row < M && k0 + i < K) ? __ldcs(X + row * ld + k0 + i) : 0.0;
+    uint32_t w[S];
+    digits4<S>(x, pow2i(8 * S - 1 - eX[row]), w);
+#pragma unroll
+    for (int q = 0; q < S; ++q) reinterpret_cast<uint32_t*>(tile + ((size_t)q * 128 + r) * 128)[lane] = w[q];
+  }
+}
+
+// block row pointers / block columns of a dense nbm x nkb grid of tiles
+__global__ void dense_tile_index_kernel(int32_t nbm, int32_t nkb, int32_t* __restrict__ brow_ptr, int32_t* __restrict__ bcol) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i <= nbm) brow_ptr[i] = (int32_t)(i * nkb);
+  if (i < (int64_t)nbm * nkb) bcol[i] = (int32_t)(i % nkb);
+}
+
 }  // namespace ttdft

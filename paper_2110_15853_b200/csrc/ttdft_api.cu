@@ -714,6 +714,7 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
   p.eH = h->eH; p.hdiag = h->hdiag; p.cmaxS = cmS; p.cmaxO = cmO;
   p.trace = g_k3_trace;
   p.l2hints = env_int("TTDFT_K3_L2HINTS", 1);
+  p.mrows = h->M;
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
   // column tiles in clusters of C; a remainder of < C tiles runs as single CTAs
@@ -963,6 +964,91 @@ ttdft_status gram_run(const GramPlan& g, const double* X, int64_t ldx, const dou
     CUDA_TRY(cudaGetLastError());
     g_launches.fetch_add(1);
   }
+  return TTDFT_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// ttdft_rotate: Y = X Q through kernel K3 (X as a dense grid of 128 x 128 digit tiles, Q as the "iterate")
+// ------------------------------------------------------------------------------------------------
+struct RotatePlan {
+  int64_t M = 0, K = 0, N = 0;
+  int32_t nbm = 0, nkb = 0, nct = 0;
+  size_t dx = 0, ex = 0, dq = 0, cm = 0, idx = 0, total = 0;
+};
+ttdft_status rotate_plan(int64_t M, int64_t K, int64_t N, RotatePlan* r) {
+  if (M < 0 || K < 1 || N < 1) return fail(TTDFT_ERR_INVALID_ARG, "rotate: M >= 0, k >= 1, n >= 1 required");
+  r->M = M; r->K = K; r->N = N;
+  r->nbm = (int32_t)((M + 127) / 128);
+  r->nkb = (int32_t)((K + 127) / 128);
+  r->nct = (int32_t)((N + 63) / 64);
+  // exact int32 accumulation over a whole row of tiles: 7 * nkb * 128 * 2^14 < 2^31
+  if ((int64_t)GRAM_S * r->nkb * 128 * 16384 >= ((int64_t)1 << 31)) return fail(TTDFT_ERR_UNSUPPORTED, "rotate: k must be <= 18560");
+  if ((int64_t)r->nbm * r->nkb >= ((int64_t)1 << 31) / GRAM_S / 128) return fail(TTDFT_ERR_UNSUPPORTED, "rotate: matrix too large");
+  r->dx = align_up((size_t)r->nbm * r->nkb * GRAM_S * 128 * 128, 1024);
+  r->ex = align_up((size_t)r->nbm * 128 * 4, 1024);
+  r->dq = align_up((size_t)r->nkb * r->nct * GRAM_S * 64 * 128, 1024);
+  r->cm = align_up((size_t)N * 4, 1024);
+  r->idx = align_up(((size_t)r->nbm + 1) * 4, 1024) + align_up((size_t)r->nbm * r->nkb * 4 + 4, 1024);
+  r->total = r->dx + r->ex + r->dq + r->cm + r->idx;
+  return TTDFT_OK;
+}
+
+ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const double* Q, int64_t ldq, double* Y, int64_t ldy, void* work,
+                        cudaStream_t st) {
+  constexpr int S = GRAM_S;
+  if (r.M == 0) return TTDFT_OK;
+  uint8_t* wb = reinterpret_cast<uint8_t*>(work);
+  int8_t* DX = reinterpret_cast<int8_t*>(wb);
+  int32_t* eX = reinterpret_cast<int32_t*>(wb + r.dx);
+  int8_t* DQ = reinterpret_cast<int8_t*>(wb + r.dx + r.ex);
+  uint32_t* cmQ = reinterpret_cast<uint32_t*>(wb + r.dx + r.ex + r.dq);
+  int32_t* brow = reinterpret_cast<int32_t*>(wb + r.dx + r.ex + r.dq + r.cm);
+  int32_t* bcol = reinterpret_cast<int32_t*>(wb + r.dx + r.ex + r.dq + r.cm + align_up(((size_t)r.nbm + 1) * 4, 1024));
+  const int64_t Mpad = (int64_t)r.nbm * 128;
+  // A operand: row exponents and digit tiles of X; tile index arrays of the dense grid
+  ttdft::x_rowexp_kernel<<<(unsigned)((Mpad + 7) / 8), 256, 0, st>>>(X, ldx, r.M, Mpad, r.K, eX);
+  ttdft::x_digits_rows_kernel<S><<<dim3((unsigned)r.nbm, (unsigned)r.nkb), 256, 0, st>>>(X, ldx, r.M, r.K, eX, DX);
+  const int64_t nidx = std::max<int64_t>((int64_t)r.nbm * r.nkb, (int64_t)r.nbm + 1);
+  ttdft::dense_tile_index_kernel<<<(unsigned)((nidx + 255) / 256), 256, 0, st>>>(r.nbm, r.nkb, brow, bcol);
+  // B operand: column maxima and digit tiles of Q (its k rows in blocks of 128, ragged tail read as zero)
+  CUDA_TRY(cudaMemsetAsync(cmQ, 0, r.cm, st));
+  ttdft::colmax_kernel<<<dim3((unsigned)r.nct, (unsigned)((r.K + 2047) / 2048)), 256, 0, st>>>(Q, ldq, r.K, r.N, cmQ);
+  {
+    static bool attr_set = false;
+    const int smem = S * 64 * 33 * 4;
+    if (!attr_set) {
+      CUDA_TRY(cudaFuncSetAttribute(ttdft::y_digits_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+      attr_set = true;
+    }
+    ttdft::y_digits_kernel<S><<<dim3((unsigned)r.nkb, (unsigned)r.nct), 256, smem, st>>>(Q, ldq, 128, r.K, r.N, cmQ, DQ, nullptr);
+  }
+  CUDA_TRY(cudaGetLastError());
+  g_launches.fetch_add(5);
+  // a transient handle describing X as a block-sparse matrix with nbm block rows of nkb dense 128 x 128 tiles
+  ttdft_h_s hx;
+  hx.M = r.M; hx.kernel = 1; hx.bsr = 1; hx.b = 128; hx.nb = r.nbm; hx.nblocks = (int64_t)r.nbm * r.nkb;
+  hx.row_ptr = brow; hx.col = bcol;
+  hx.i8_S = S; hx.math = TTDFT_MATH_I8X7; hx.eH = eX; hx.hdiag = nullptr;
+  int dev = 0, nsm = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0) hx.nsm = nsm;
+  ttdft_status s;
+  for (int ci = 0; ci < 2; ++ci)
+    if ((s = make_map_hd(&hx.tmHd[ci], DX, (uint64_t)hx.nblocks * S * 128, 128u >> ci)) != TTDFT_OK) return s;
+  CUtensorMap tmQd;
+  if ((s = make_map_yd(&tmQd, DQ, (uint64_t)r.nkb * r.nct * S, S)) != TTDFT_OK) return s;
+  ttdft::K3Params p;
+  p.brow_ptr = brow; p.bcol = bcol;
+  p.nb = r.nbm; p.b = 128; p.nct = r.nct; p.hplanes = S; p.ncols = r.N;
+  p.alpha = 1.0; p.gamma = 0.0; p.beta = 0.0;
+  p.S = nullptr; p.lds = 0; p.Z = Y; p.ldz = ldy; p.O = Y; p.ldo = ldy;
+  p.eH = eX; p.hdiag = nullptr; p.cmaxS = cmQ; p.cmaxO = nullptr;
+  p.vec = 0; p.trace = nullptr; p.l2hints = env_int("TTDFT_K3_L2HINTS", 1); p.mrows = r.M;
+  const int C = (r.nct >= 2) ? 2 : 1;
+  const int32_t main_tiles = r.nct / C * C;
+  if (C == 2) s = launch_k3<S, 2>(&hx, tmQd, p, 0, main_tiles, st);
+  else s = launch_k3<S, 1>(&hx, tmQd, p, 0, main_tiles, st);
+  if (s != TTDFT_OK) return s;
+  if (main_tiles < r.nct) return launch_k3<S, 1>(&hx, tmQd, p, main_tiles, r.nct - main_tiles, st);
   return TTDFT_OK;
 }
 
@@ -1663,6 +1749,29 @@ ttdft_status ttdft_project(ttdft_h_t h, const double* X, int64_t ldx, int64_t nc
     if (s != TTDFT_OK) return s;
   }
   return gram_run(g, X, ldx, Wb, ldw, G, ldg, rest, st);                                          // G = X^T W
+}
+
+ttdft_status ttdft_rotate_work_bytes(int64_t M, int64_t k, int64_t n, size_t* bytes) {
+  if (!bytes) return fail(TTDFT_ERR_INVALID_ARG, "bytes is NULL");
+  RotatePlan r;
+  ttdft_status s = rotate_plan(M, k, n, &r);
+  if (s != TTDFT_OK) return s;
+  *bytes = r.total;
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_rotate(int64_t M, const double* X, int64_t ldx, int64_t k, const double* Q, int64_t ldq, int64_t n, double* Y,
+                          int64_t ldy, void* work, size_t work_bytes, void* stream) {
+  RotatePlan r;
+  ttdft_status s = rotate_plan(M, k, n, &r);
+  if (s != TTDFT_OK) return s;
+  if (M > 0 && (s = check_mat("X", X, ldx, k)) != TTDFT_OK) return s;
+  if ((s = check_mat("Q", Q, ldq, n)) != TTDFT_OK) return s;
+  if (M > 0 && (s = check_mat("Y", Y, ldy, n)) != TTDFT_OK) return s;
+  if (M > 0 && overlaps(X, ldx, Y, ldy, M, std::min(k, n)) ) return fail(TTDFT_ERR_INVALID_ARG, "X overlaps Y");
+  if (work_bytes < r.total) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, r.total);
+  if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
+  return rotate_run(r, X, ldx, Q, ldq, Y, ldy, work, (cudaStream_t)stream);
 }
 
 ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, double* tflops) {

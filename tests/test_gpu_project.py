@@ -173,3 +173,69 @@ def test_project_full_config3_si():
     z = oracle.spmm(C.row_ptr, C.col_idx, C.values, 1.0, Xh @ u)
     rhs = Xh.T @ z
     assert relerr(got @ u, rhs) <= 1e-11
+
+
+# ---------------------------------------------------------------- rotation Y = X Q (Algorithm 1 step 5)
+@pytest.mark.parametrize("M,K,N,pad", [(2048, 32, 32, 0), (1000, 70, 33, 3), (300, 1, 1, 1), (4113, 130, 257, 5), (77, 300, 64, 0),
+                                       (128 * 40, 512, 200, 0)])
+def test_rotate_vs_oracle(tt, M, K, N, pad):
+    import torch
+    X = synth.dense_normal(M, K, 401) * 10.0 ** np.linspace(-6, 6, M)[:, None]      # rows of very different size
+    Q = synth.dense_normal(K, N, 402) * 10.0 ** np.linspace(5, -5, N)[None, :]      # columns of very different size
+    ref = oracle.rotate(X, Q)
+    Xd = torch.zeros(M, K + pad, dtype=torch.float64, device="cuda")
+    Qd = torch.zeros(K, N + pad, dtype=torch.float64, device="cuda")
+    Xd[:, :K], Qd[:, :N] = dev(X), dev(Q)
+    Yd = torch.full((M, N + pad), float("nan"), dtype=torch.float64, device="cuda")
+    tt.rotate(Xd[:, :K], Qd[:, :N], Yd[:, :N])
+    got = Yd[:, :N].cpu().numpy()
+    # entry-wise against the scale of each entry, |x_i| |q_l| (row- and column-scaled fixed point)
+    scale = np.outer(np.linalg.norm(X, axis=1), np.linalg.norm(Q, axis=0))
+    scale[scale == 0] = 1.0
+    assert np.max(np.abs(got - ref) / scale) <= 1e-15 * np.sqrt(K) + 1e-16
+    if pad:
+        assert torch.isnan(Yd[:, N:]).all()                  # nothing written outside the view
+    Y2 = torch.empty(M, N, dtype=torch.float64, device="cuda")
+    tt.rotate(Xd[:, :K], Qd[:, :N], Y2)
+    assert np.array_equal(Y2.cpu().numpy(), got)             # deterministic
+
+
+def test_rotate_identity_and_gram_congruence(tt):
+    import torch
+    M, K = 3000, 96
+    X = synth.dense_normal(M, K, 411)
+    Xd = dev(X)
+    Y = torch.empty(M, K, dtype=torch.float64, device="cuda")
+    tt.rotate(Xd, torch.eye(K, dtype=torch.float64, device="cuda"), Y)
+    assert relerr(Y.cpu().numpy(), X) <= 1e-15               # Q = I (exact up to the 55-bit rounding of the rows)
+    Q = synth.dense_normal(K, K, 412)
+    tt.rotate(Xd, dev(Q), Y)
+    G, GY = torch.empty(K, K, dtype=torch.float64, device="cuda"), torch.empty(K, K, dtype=torch.float64, device="cuda")
+    tt.gram(Xd, Xd, G)
+    tt.gram(Y, Y, GY)                                        # (XQ)^T (XQ) = Q^T (X^T X) Q
+    assert relerr(GY.cpu().numpy(), Q.T @ G.cpu().numpy() @ Q) <= 1e-12
+
+
+def test_rotate_full_config3_shape():
+    """Config 3's shape (M = 221,184, k = n = 4,096): seeded rows compared entry by entry with the oracle (row i of Y depends on
+    row i of X only) and every entry covered by the Freivalds identity Y u = X (Q u)."""
+    import torch
+    import paper_2110_15853_b200 as tt
+    cfg = synth.CONFIGS["si"]
+    M, K = cfg.M, cfg.N
+    Xh = np.empty((M, K))
+    synth.dense_normal(M, K, cfg.seed, synth.STREAM_X, out=Xh)
+    Qh = synth.dense_normal(K, K, 421) / np.sqrt(K)
+    Xd, Qd = dev(Xh), dev(Qh)
+    Yd = torch.empty(M, K, dtype=torch.float64, device="cuda")
+    tt.rotate(Xd, Qd, Yd)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(6)
+    rows = np.unique(np.concatenate([[0, 127, 128, M - 1], rng.integers(0, M, 28)]))
+    ref = oracle.rotate(np.ascontiguousarray(Xh[rows]), Qh)
+    got_rows = Yd[torch.from_numpy(rows).cuda()].cpu().numpy()
+    assert relerr(got_rows, ref) <= TOL
+    u = torch.from_numpy(rng.standard_normal((K, 2))).cuda()
+    lhs = (Yd @ u).cpu().numpy()
+    rhs = Xh @ (Qh @ u.cpu().numpy())
+    assert relerr(lhs, rhs) <= 1e-12

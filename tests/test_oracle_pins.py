@@ -434,3 +434,24 @@ def test_p7_projection_identities(tiny):
     rows = np.repeat(np.arange(H.M), np.diff(C.row_ptr))
     tr = float(np.sum(C.values * np.einsum("ij,ij->i", X[rows], X[C.col_idx])))
     assert abs(np.trace(G) - tr) <= 1e-12 * abs(tr)
+
+
+# ------------------------------------------------------------------ P8: rotation Y = X Q (Algorithm 1 step 5)
+def test_p8_rotate_pins():
+    g = read_gram_golden()
+    assert np.array_equal(oracle.rotate(g["X"], g["Qrot"]), g["XQ"])       # hand-computed, non-square Q
+    rng = np.random.default_rng(8)
+    for M, K, n in [(1, 1, 1), (7, 5, 3), (300, 130, 70), (64, 257, 33)]:
+        X, Q = rng.standard_normal((M, K)), rng.standard_normal((K, n))
+        Y = oracle.rotate(X, Q)
+        ref = X @ Q
+        assert np.linalg.norm(Y - ref) <= 1e-14 * max(1.0, np.linalg.norm(ref))
+    X = rng.standard_normal((50, 9))
+    assert np.array_equal(oracle.rotate(X, np.eye(9)), X)                 # Q = I
+    perm = rng.permutation(9)
+    assert np.array_equal(oracle.rotate(X, np.ascontiguousarray(np.eye(9)[:, perm])), X[:, perm])   # a column permutation is exact
+    Q = rng.standard_normal((9, 9))
+    G = oracle.gram(X, X)
+    Y = oracle.rotate(X, Q)
+    lhs = oracle.gram(Y, Y)                                               # (XQ)^T (XQ) = Q^T (X^T X) Q
+    assert np.linalg.norm(lhs - Q.T @ G @ Q) <= 1e-12 * np.linalg.norm(lhs)
