@@ -443,6 +443,23 @@ def main():
             refr = oracle.rotate(np.ascontiguousarray(Xd[rr].cpu().numpy()), Qd.cpu().numpy())
             line["rotate"]["gpu_vs_oracle_relerr_on_sample"] = float(np.linalg.norm(Yd[rr].cpu().numpy() - refr) / np.linalg.norm(refr))
         del Qd, rw
+        # ---- Algorithm 1 step 2: X_F = Orth(X) (ttdft_orthonormalize, Cholesky-QR2; 1 warm-up + 1 timed) ----
+        ow = torch.empty(tt.orthonormalize_work_bytes(cfg.M, cfg.N, 2) + 1024, dtype=torch.uint8, device=dev)
+        tt.orthonormalize(Xd, Yd, passes=2, work=ow)
+        torch.cuda.synchronize()
+        g0.record()
+        tt.orthonormalize(Xd, Yd, passes=2, work=ow)
+        g1.record()
+        torch.cuda.synchronize()
+        t_o = g0.elapsed_time(g1) * 1e-3
+        line["orthonormalize"] = {"what": "X_F = Orth(X), Algorithm 1 step 2 (ttdft_orthonormalize): Cholesky-QR2 = 2 x (Gram product K4, "
+                                          "n x n Cholesky + inverse, rotation on K3)",
+                                  "ms": t_o * 1e3, "fp64_equivalent_tflops": 4.0 * fl_gram / t_o / 1e12, "steps": 1, "warmup": 1}
+        if not args.no_cpu_baseline:
+            lead = 16      # column j of Q depends on columns 0..j of X only: the leading block against the oracle's Gram-Schmidt
+            refq = oracle.orthonormalize(np.ascontiguousarray(Xd[:, :lead].cpu().numpy()))
+            line["orthonormalize"]["gpu_vs_oracle_relerr_on_sample"] = float(np.linalg.norm(Yd[:, :lead].cpu().numpy() - refq) / np.linalg.norm(refq))
+        del ow
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         dt, _, cols, Xs, Yo, threads = oracle_sample_run(cfg, H, args.ref_cols, cfg.m, (a, b, a0))

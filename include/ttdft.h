@@ -38,7 +38,8 @@ typedef enum {
   TTDFT_ERR_UNSUPPORTED = 2,
   TTDFT_ERR_WORKSPACE_TOO_SMALL = 3,
   TTDFT_ERR_NOT_SYMMETRIC = 4,
-  TTDFT_ERR_CUDA = 5
+  TTDFT_ERR_CUDA = 5,
+  TTDFT_ERR_BREAKDOWN = 6 /* ttdft_orthonormalize: X^T X not positive definite (dependent columns) */
 } ttdft_status;
 
 typedef enum { TTDFT_FMT_CSR = 0, TTDFT_FMT_BSR = 1 } ttdft_format;
@@ -239,6 +240,23 @@ ttdft_status ttdft_project(ttdft_h_t h, const double* X, int64_t ldx, int64_t nc
 ttdft_status ttdft_rotate_work_bytes(int64_t M, int64_t k, int64_t n, size_t* bytes);
 ttdft_status ttdft_rotate(int64_t M, const double* X, int64_t ldx, int64_t k, const double* Q, int64_t ldq, int64_t n, double* Y,
                           int64_t ldy, void* work, size_t work_bytes, void* stream);
+
+/*
+ * NEXT-2 -- Algorithm 1 step 2 ("Orthonormalize the Chebyshev filtered basis functions,
+ * X_F = Orth(X)", L230 "Gram-Schmidt orthogonalization procedure"; the paper leaves it on the CPU and names it the
+ * bottleneck after GPU offload, L378):
+ *     Y = X R^-1,  X^T X = R^T R,  R upper triangular with positive diagonal      (Cholesky-QR)
+ * which for full-rank X is exactly the Q of Gram-Schmidt.  One pass = ttdft_gram(X, X), an n x n Cholesky factorisation
+ * and triangular inverse (plain fp64 kernels), ttdft_rotate(X, R^-1).  passes = 2 (Cholesky-QR2, recommended) repeats it
+ * on the result and restores orthogonality to rounding level for cond(X) up to ~1e7; passes = 1 loses orthogonality as
+ * cond(X)^2 * 1e-16.  X: M x n row-major, M >= n; Y: M x n row-major, must not overlap X.
+ * Returns TTDFT_ERR_BREAKDOWN (Y undefined) if X^T X is not positive definite to working precision.
+ * The call SYNCHRONISES `stream` once per pass (it reads the factorisation's breakdown flag).
+ * `work`: 1024-byte aligned DEVICE scratch of at least ttdft_orthonormalize_work_bytes.
+ */
+ttdft_status ttdft_orthonormalize_work_bytes(int64_t M, int64_t n, int32_t passes, size_t* bytes);
+ttdft_status ttdft_orthonormalize(int64_t M, const double* X, int64_t ldx, int64_t n, double* Y, int64_t ldy, int32_t passes, void* work,
+                                  size_t work_bytes, void* stream);
 
 /* Measured fp64 rate of this GPU: kind 0 = scalar DFMA loop, 1 = DMMA (mma.sync m8n8k4.f64) loop;
  * runs for about `millis` ms on `stream`, synchronises, returns TFLOP/s in *tflops. */

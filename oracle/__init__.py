@@ -77,6 +77,8 @@ def lib() -> ctypes.CDLL:
         L.oracle_gram.argtypes = [i64, i64, vp, i64, vp, i64, vp, i64]
         L.oracle_rotate.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64]
         L.oracle_rotate.restype = None
+        L.oracle_orth_gs.argtypes = [i64, i64, vp, i64, vp, i64, i32]
+        L.oracle_orth_gs.restype = ctypes.c_int
         L.oracle_gram.restype = None
         L.oracle_lanczos_bounds.argtypes = [i64, _i32p, _i32p, _f64p, i32, _f64p, _f64p, _f64p, _f64p, _f64p,
                                             ctypes.POINTER(f64), ctypes.POINTER(f64)]
@@ -213,3 +215,15 @@ def rotate(X: np.ndarray, Q: np.ndarray) -> np.ndarray:
     yp, ldy = _mat(Y)
     lib().oracle_rotate(M, K, n, xp, ldx, qp, ldq, yp, ldy)
     return Y
+
+
+def orthonormalize(X: np.ndarray, sweeps: int = 2) -> np.ndarray:
+    """X_F = Orth(X) by Gram-Schmidt (oracle_orth_gs; Algorithm 1 step 2)."""
+    M, n = X.shape
+    Q = np.zeros((M, n), np.float64)
+    xp, ldx = _mat(X)
+    qp, ldq = _mat(Q)
+    rc = lib().oracle_orth_gs(M, n, xp, ldx, qp, ldq, sweeps)
+    if rc:
+        raise np.linalg.LinAlgError(f"column {rc - 1} is linearly dependent on the previous ones")
+    return Q

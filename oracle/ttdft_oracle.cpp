@@ -25,7 +25,9 @@
 // (tests/golden/gram_pins.txt), numpy's matmul, Q^T H Q = Lambda for a known eigendecomposition, symmetry,
 // congruence (XR)^T H (XR) = R^T (X^T H X) R and the trace identity.  oracle_rotate is the plain definition of
 // Y = X Q (Algorithm 1 step 5); pins P8: hand-computed integers, numpy's matmul, Q = I and a column
-// permutation (exact), and the identity (XQ)^T (XQ) = Q^T (X^T X) Q through oracle_gram.
+// permutation (exact), and the identity (XQ)^T (XQ) = Q^T (X^T X) Q through oracle_gram.  oracle_orth_gs is Gram-Schmidt
+// (Algorithm 1 step 2); pins P9: a hand-computed 2 x 2 case, numpy's QR with the signs of R's diagonal made
+// positive, Q^T Q = I, Q^T X upper triangular with positive diagonal, X = Q (Q^T X).
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
@@ -242,6 +244,30 @@ void oracle_rotate(int64_t M, int64_t K, int64_t n, const double* X, int64_t ldx
       for (int64_t l = 0; l < n; ++l) y[l] = y[l] + x * q[l];
     }
   }
+}
+
+// X_F = Orth(X) (Algorithm 1 step 2; L230 "Gram-Schmidt orthogonalization procedure"): Gram-Schmidt column by
+// column, the projections removed one at a time (modified Gram-Schmidt) and the whole sweep repeated `sweeps` times
+// ("twice is enough": with 2 sweeps the result is orthonormal to rounding level for any X that is numerically full rank):
+//   v = x_j;  repeat sweeps times: for i < j: v = v - (q_i . v) q_i;   q_j = v / ||v||_2
+// X, Q: M x n row-major.  Returns 1 + j if column j has no component outside the span of the previous ones, else 0.
+int oracle_orth_gs(int64_t M, int64_t n, const double* X, int64_t ldx, double* Q, int64_t ldq, int32_t sweeps) {
+  std::vector<double> v((size_t)M);
+  for (int64_t j = 0; j < n; ++j) {
+    for (int64_t k = 0; k < M; ++k) v[(size_t)k] = X[k * ldx + j];
+    for (int32_t s = 0; s < sweeps; ++s)
+      for (int64_t i = 0; i < j; ++i) {
+        double r = 0.0;
+        for (int64_t k = 0; k < M; ++k) r = r + Q[k * ldq + i] * v[(size_t)k];
+        for (int64_t k = 0; k < M; ++k) v[(size_t)k] = v[(size_t)k] - r * Q[k * ldq + i];
+      }
+    double nrm2 = 0.0;
+    for (int64_t k = 0; k < M; ++k) nrm2 = nrm2 + v[(size_t)k] * v[(size_t)k];
+    if (!(nrm2 > 0.0)) return (int)(1 + j);
+    const double nrm = std::sqrt(nrm2);
+    for (int64_t k = 0; k < M; ++k) Q[k * ldq + j] = v[(size_t)k] / nrm;
+  }
+  return 0;
 }
 
 static void spmv_csr(int64_t M, const int32_t* row_ptr, const int32_t* col, const double* val, const double* x,

@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_PKG, "libttdft.so")
 CHECK_SORTED, CHECK_SYMMETRY, FORCE_GENERIC, NO_I8 = 1, 2, 4, 8
 MATH_AUTO, MATH_FP64, MATH_I8, MATH_I8X7 = 0, 1, 2, 3
 FMT_CSR, FMT_BSR = 0, 1
-_STATUS = {0: "OK", 1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "NOT_SYMMETRIC", 5: "CUDA"}
+_STATUS = {0: "OK", 1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "NOT_SYMMETRIC", 5: "CUDA", 6: "BREAKDOWN"}
 
 # every symbol include/ttdft.h declares
 exported_symbols = [
@@ -21,7 +21,7 @@ exported_symbols = [
     "ttdft_h_set_math_mode", "ttdft_step_work_bytes", "ttdft_spmm_ws", "ttdft_cheb_step_ws",
     "ttdft_timing_enable", "ttdft_timing_read",
     "ttdft_gram_work_bytes", "ttdft_gram", "ttdft_project_work_bytes", "ttdft_project",
-    "ttdft_rotate_work_bytes", "ttdft_rotate",
+    "ttdft_rotate_work_bytes", "ttdft_rotate", "ttdft_orthonormalize_work_bytes", "ttdft_orthonormalize",
 ]
 
 
@@ -105,6 +105,10 @@ def _load() -> ctypes.CDLL:
     L.ttdft_rotate_work_bytes.argtypes = [c_int64, c_int64, c_int64, POINTER(c_size_t)]
     L.ttdft_rotate.restype = st
     L.ttdft_rotate.argtypes = [c_int64, c_void_p, c_int64, c_int64, c_void_p, c_int64, c_int64, c_void_p, c_int64, c_void_p, c_size_t, c_void_p]
+    L.ttdft_orthonormalize_work_bytes.restype = st
+    L.ttdft_orthonormalize_work_bytes.argtypes = [c_int64, c_int64, c_int32, POINTER(c_size_t)]
+    L.ttdft_orthonormalize.restype = st
+    L.ttdft_orthonormalize.argtypes = [c_int64, c_void_p, c_int64, c_int64, c_void_p, c_int64, c_int32, c_void_p, c_size_t, c_void_p]
     L.ttdft_probe_fp64_peak.restype = st
     L.ttdft_probe_fp64_peak.argtypes = [c_int32, c_int32, c_void_p, POINTER(c_double)]
     L.ttdft_timing_enable.restype = st
@@ -418,6 +422,24 @@ def rotate(X, Q, Y, work=None, stream=None):
         raise ValueError("shape mismatch")
     wp, wb, keep = _aligned_work(rotate_work_bytes(M, k, n), work, X.device)
     _check(_load().ttdft_rotate(M, xp, ldx, k, qp, ldq, n, yp, ldy, wp, wb, _stream(stream)))
+    return Y
+
+
+def orthonormalize_work_bytes(M: int, n: int, passes: int = 2) -> int:
+    out = c_size_t(0)
+    _check(_load().ttdft_orthonormalize_work_bytes(M, n, passes, byref(out)))
+    return int(out.value)
+
+
+def orthonormalize(X, Y, passes: int = 2, work=None, stream=None):
+    """Y = X R^-1 with X^T X = R^T R (ttdft_orthonormalize; Algorithm 1 step 2): columns of Y are orthonormal."""
+    xp, ldx = _mat(X, "X")
+    yp, ldy = _mat(Y, "Y")
+    M, n = X.shape
+    if tuple(Y.shape) != (M, n):
+        raise ValueError("shape mismatch")
+    wp, wb, keep = _aligned_work(orthonormalize_work_bytes(M, n, passes), work, X.device)
+    _check(_load().ttdft_orthonormalize(M, xp, ldx, n, yp, ldy, passes, wp, wb, _stream(stream)))
     return Y
 
 

@@ -19,6 +19,7 @@
 #include "bsr_dmma.cuh"
 #include "bsr_i8.cuh"
 #include "generic_spmm.cuh"
+#include "cholesky.cuh"
 #include "gram_i8.cuh"
 
 namespace {
@@ -1052,6 +1053,92 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
   return TTDFT_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// ttdft_orthonormalize: Cholesky-QR (repeated `passes` times) = Gram product + n x n Cholesky + inverse + rotation
+// ------------------------------------------------------------------------------------------------
+struct OrthPlan {
+  int64_t M = 0, n = 0;
+  int32_t passes = 2;
+  GramPlan g;
+  RotatePlan r;
+  size_t nn = 0, tmp = 0, inner = 0, total = 0;     // one n x n matrix | M x n temporary (2 passes) | max(gram, rotate) scratch
+};
+ttdft_status orth_plan(int64_t M, int64_t n, int32_t passes, OrthPlan* o) {
+  if (passes < 1 || passes > 3) return fail(TTDFT_ERR_INVALID_ARG, "orthonormalize: passes must be 1, 2 or 3");
+  if (M < n) return fail(TTDFT_ERR_INVALID_ARG, "orthonormalize: M >= n required (got M=%lld, n=%lld)", (long long)M, (long long)n);
+  ttdft_status s;
+  if ((s = gram_plan(M, n, &o->g)) != TTDFT_OK) return s;
+  if ((s = rotate_plan(M, n, n, &o->r)) != TTDFT_OK) return s;
+  o->M = M; o->n = n; o->passes = passes;
+  const int64_t ldn = n + (n & 1);
+  o->nn = align_up((size_t)n * (size_t)ldn * 8, 1024);
+  o->tmp = passes > 1 ? align_up((size_t)M * (size_t)ldn * 8, 1024) : 0;
+  o->inner = std::max(o->g.total, o->r.total);
+  o->total = 2 * o->nn + 1024 + o->tmp + o->inner;
+  return TTDFT_OK;
+}
+
+// G (lower triangle) -> L in place; Rinv = L^-T.  Returns the breakdown flag through *hflag (synchronises st).
+ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Rinv, int64_t ldr, int32_t* dflag, int32_t* hflag, cudaStream_t st) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
+    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_trinv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * ttdft::CH_TILE_BYTES));
+    attr_set = true;
+  }
+  CUDA_TRY(cudaMemsetAsync(dflag, 0, 4, st));
+  for (int32_t k0 = 0; k0 < n; k0 += ttdft::CH_NB) {
+    const int32_t nbk = std::min(ttdft::CH_NB, n - k0);
+    ttdft::ch_potf2_kernel<<<1, 256, 0, st>>>(G, ldg, k0, nbk, dflag);
+    const int32_t rem = n - k0 - nbk;
+    if (rem > 0) {
+      const unsigned tiles = (unsigned)((rem + 63) / 64);
+      ttdft::ch_trsm_kernel<<<tiles, 64, 0, st>>>(G, ldg, n, k0, nbk);
+      ttdft::ch_syrk_kernel<<<dim3(tiles, tiles), 256, 2 * ttdft::CH_TILE_BYTES, st>>>(G, ldg, n, k0, nbk);
+      g_launches.fetch_add(2);
+    }
+    g_launches.fetch_add(1);
+  }
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaMemcpyAsync(hflag, dflag, 4, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (*hflag) return TTDFT_OK;                      // caller reports the breakdown
+  CUDA_TRY(cudaMemset2DAsync(Rinv, (size_t)ldr * 8, 0, (size_t)n * 8, (size_t)n, st));
+  ttdft::ch_trinv_kernel<<<(unsigned)((n + ttdft::CH_NB - 1) / ttdft::CH_NB), 256, 3 * ttdft::CH_TILE_BYTES, st>>>(G, ldg, n, Rinv, ldr);
+  CUDA_TRY(cudaGetLastError());
+  g_launches.fetch_add(1);
+  return TTDFT_OK;
+}
+
+ttdft_status orth_run(const OrthPlan& o, const double* X, int64_t ldx, double* Y, int64_t ldy, void* work, cudaStream_t st) {
+  uint8_t* wb = reinterpret_cast<uint8_t*>(work);
+  const int64_t ldn = o.n + (o.n & 1);
+  double* G = reinterpret_cast<double*>(wb);
+  double* Rinv = reinterpret_cast<double*>(wb + o.nn);
+  int32_t* dflag = reinterpret_cast<int32_t*>(wb + 2 * o.nn);
+  double* T = reinterpret_cast<double*>(wb + 2 * o.nn + 1024);
+  void* inner = wb + 2 * o.nn + 1024 + o.tmp;
+  // pass p reads `src` and writes `dst`; the last pass must land in Y, intermediate results alternate Y / T
+  const double* src = X;
+  int64_t lds = ldx;
+  for (int32_t p = 0; p < o.passes; ++p) {
+    const bool to_y = ((o.passes - 1 - p) % 2 == 0);
+    double* dst = to_y ? Y : T;
+    const int64_t ldd = to_y ? ldy : ldn;
+    ttdft_status s = gram_run(o.g, src, lds, src, lds, G, ldn, inner, st);          // G = src^T src
+    if (s != TTDFT_OK) return s;
+    int32_t hflag = 0;
+    if ((s = chol_inverse(G, ldn, (int32_t)o.n, Rinv, ldn, dflag, &hflag, st)) != TTDFT_OK) return s;
+    if (hflag)
+      return fail(TTDFT_ERR_BREAKDOWN, "orthonormalize: X^T X is not positive definite in pass %d (pivot %d): columns are linearly "
+                                       "dependent to working precision", p + 1, hflag - 1);
+    if ((s = rotate_run(o.r, src, lds, Rinv, ldn, dst, ldd, inner, st)) != TTDFT_OK) return s;   // dst = src R^-1
+    src = dst;
+    lds = ldd;
+  }
+  return TTDFT_OK;
+}
+
 }  // namespace
 
 // ================================================================================================
@@ -1772,6 +1859,28 @@ ttdft_status ttdft_rotate(int64_t M, const double* X, int64_t ldx, int64_t k, co
   if (work_bytes < r.total) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, r.total);
   if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
   return rotate_run(r, X, ldx, Q, ldq, Y, ldy, work, (cudaStream_t)stream);
+}
+
+ttdft_status ttdft_orthonormalize_work_bytes(int64_t M, int64_t n, int32_t passes, size_t* bytes) {
+  if (!bytes) return fail(TTDFT_ERR_INVALID_ARG, "bytes is NULL");
+  OrthPlan o;
+  ttdft_status s = orth_plan(M, n, passes, &o);
+  if (s != TTDFT_OK) return s;
+  *bytes = o.total;
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_orthonormalize(int64_t M, const double* X, int64_t ldx, int64_t n, double* Y, int64_t ldy, int32_t passes, void* work,
+                                  size_t work_bytes, void* stream) {
+  OrthPlan o;
+  ttdft_status s = orth_plan(M, n, passes, &o);
+  if (s != TTDFT_OK) return s;
+  if ((s = check_mat("X", X, ldx, n)) != TTDFT_OK) return s;
+  if ((s = check_mat("Y", Y, ldy, n)) != TTDFT_OK) return s;
+  if (overlaps(X, ldx, Y, ldy, M, n)) return fail(TTDFT_ERR_INVALID_ARG, "X overlaps Y");
+  if (work_bytes < o.total) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, o.total);
+  if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
+  return orth_run(o, X, ldx, Y, ldy, work, (cudaStream_t)stream);
 }
 
 ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, double* tflops) {

@@ -455,3 +455,25 @@ def test_p8_rotate_pins():
     Y = oracle.rotate(X, Q)
     lhs = oracle.gram(Y, Y)                                               # (XQ)^T (XQ) = Q^T (X^T X) Q
     assert np.linalg.norm(lhs - Q.T @ G @ Q) <= 1e-12 * np.linalg.norm(lhs)
+
+
+# ------------------------------------------------------------------ P9: orthonormalisation X_F = Orth(X) (Algorithm 1 step 2)
+def test_p9_gram_schmidt_pins():
+    g = read_gram_golden()
+    assert np.linalg.norm(oracle.orthonormalize(g["Xgs"]) - g["Qgs"]) <= 1e-15          # hand-computed
+    rng = np.random.default_rng(9)
+    for M, n, cond in [(5, 3, 1.0), (200, 17, 1.0), (300, 40, 1e6)]:
+        X = rng.standard_normal((M, n))
+        if cond > 1.0:                                            # ill-conditioned: graded singular values
+            U, _, Vt = np.linalg.svd(X, full_matrices=False)
+            X = (U * np.logspace(0, -np.log10(cond), n)) @ Vt
+        Q = oracle.orthonormalize(X)
+        Qn, Rn = np.linalg.qr(X)                                  # library QR, signs fixed so that diag(R) > 0
+        sgn = np.sign(np.diag(Rn))
+        assert np.linalg.norm(Q - Qn * sgn) <= 1e-13 * cond * np.sqrt(n)
+        assert np.linalg.norm(Q.T @ Q - np.eye(n)) <= 1e-14 * n   # orthonormal to rounding level, whatever cond(X)
+        R = Q.T @ X
+        assert np.linalg.norm(np.tril(R, -1)) <= 1e-13 * np.linalg.norm(R) and np.all(np.diag(R) > 0)
+        assert np.linalg.norm(Q @ R - X) <= 1e-13 * np.linalg.norm(X)
+    with pytest.raises(np.linalg.LinAlgError):
+        oracle.orthonormalize(np.zeros((4, 2)))
