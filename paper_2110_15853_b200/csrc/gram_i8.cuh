@@ -32,6 +32,7 @@ struct K4Params {
   const uint32_t* cmaxX;       // column maxima (upper words) of X  [ncols]
   const uint32_t* cmaxW;       // column maxima of W                [ncols]
   int64_t colw0;               // first column of W of this panel (global), for cmaxW
+  int32_t sym;                 // 1: W is X (G = X^T X): tile groups entirely below the diagonal are skipped, the reduction mirrors
 };
 
 __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, int32_t x, int32_t y, int32_t z, int32_t w, uint64_t* bar) {
@@ -69,14 +70,21 @@ __device__ __forceinline__ void k4_decode(const K4Params& prm, int64_t u, int32_
   ctwg = sw * SW + rem3 / hx;
 }
 
-// P[chunk] summed in ascending chunk order:  G[j, colw0 + l] = sum_c P[c][j][l]
+// a work item is skipped in symmetric mode if even its last 64-column tile lies entirely below the diagonal of G
+__device__ __forceinline__ bool k4_skip(const K4Params& prm, int32_t ctx, int32_t ctw_last) {
+  return prm.sym && ((int64_t)ctw_last * K3_NT + K3_NT - 1 < (int64_t)ctx * 128);
+}
+
+// P[chunk] summed in ascending chunk order:  G[j, colw0 + l] = sum_c P[c][j][l]; in symmetric mode (single panel) the
+// entries below the diagonal are the mirror images of the computed ones, so G comes out exactly symmetric
 __global__ void __launch_bounds__(256) gram_reduce_kernel(const double* __restrict__ P, int64_t ldp, int64_t rows, int32_t nchunks,
-                                                          int64_t ncols_w, double* __restrict__ G, int64_t ldg) {
+                                                          int64_t ncols_w, double* __restrict__ G, int64_t ldg, int32_t sym) {
   const int64_t j = blockIdx.y;
   const int64_t l = (int64_t)blockIdx.x * 256 + threadIdx.x;
   if (l >= ncols_w) return;
+  const int64_t pj = (sym && l < j) ? l : j, pl = (sym && l < j) ? j : l;
   double acc = 0.0;
-  for (int32_t c = 0; c < nchunks; ++c) acc += P[((int64_t)c * rows + j) * ldp + l];
+  for (int32_t c = 0; c < nchunks; ++c) acc += P[((int64_t)c * rows + pj) * ldp + pl];
   G[j * ldg + l] = acc;
 }
 
@@ -138,6 +146,7 @@ gram_i8_kernel(const __grid_constant__ CUtensorMap tmXd, const __grid_constant__
         int32_t chunk, ctx, ctwg;
         k4_decode(prm, u, chunk, ctx, ctwg);
         const int32_t ctw = prm.ctw_begin + ctwg * C + crank;
+        if (k4_skip(prm, ctx, prm.ctw_begin + ctwg * C + C - 1)) continue;
         const int32_t I0 = chunk * prm.kc, I1 = min(prm.nbk, I0 + prm.kc);
         for (int32_t I = I0; I < I1; ++I) {
           mbar_wait(&yempty[yb], yph ^ 1);
@@ -174,6 +183,7 @@ gram_i8_kernel(const __grid_constant__ CUtensorMap tmXd, const __grid_constant__
       for (int64_t u = cluster0; u < nitems; u += nclusters) {
         int32_t chunk, ctx, ctwg;
         k4_decode(prm, u, chunk, ctx, ctwg);
+        if (k4_skip(prm, ctx, prm.ctw_begin + ctwg * C + C - 1)) continue;
         const int32_t nI = min(prm.nbk, chunk * prm.kc + prm.kc) - chunk * prm.kc;
         mbar_wait(accempty, aph ^ 1);
         asm volatile("tcgen05.fence::after_thread_sync;");
@@ -219,6 +229,7 @@ gram_i8_kernel(const __grid_constant__ CUtensorMap tmXd, const __grid_constant__
       int32_t chunk, ctx, ctwg;
       k4_decode(prm, u, chunk, ctx, ctwg);
       const int32_t ctw = prm.ctw_begin + ctwg * C + crank;
+      if (k4_skip(prm, ctx, prm.ctw_begin + ctwg * C + C - 1)) continue;
       const int64_t lcol0 = (int64_t)ctw * K3_NT;            // column inside the panel
       const int64_t grow = (int64_t)ctx * 128 + r;           // row of G
       const bool row_ok = grow < prm.ncols;

@@ -942,6 +942,9 @@ ttdft_status gram_run(const GramPlan& g, const double* X, int64_t ldx, const dou
   ttdft::K4Params p;
   p.nbk = g.nbk; p.kc = g.kc; p.nchunks = g.nchunks; p.nctx = g.nctx; p.nctX = g.nctX; p.nctW = g.nctW;
   p.ncols = g.ncols; p.P = P; p.cmaxX = cmX; p.cmaxW = cmW;
+  // G = X^T X: only the tiles that touch the upper triangle are computed (single panel only: the mirror image of an
+  // entry must be in the same panel of partial tiles)
+  p.sym = (X == W && ldx == ldw && g.wp >= g.ncols && env_int("TTDFT_K4_SYM", 1)) ? 1 : 0;
   const int C = env_int("TTDFT_K4_CLUSTER", 2) == 1 ? 1 : 2;
   for (int64_t c0 = 0; c0 < g.ncols; c0 += g.wp) {
     const int64_t wc = std::min(g.wp, g.ncols - c0);
@@ -961,7 +964,7 @@ ttdft_status gram_run(const GramPlan& g, const double* X, int64_t ldx, const dou
     if (s != TTDFT_OK) return s;
     if (main_tiles < ntl && (s = launch_k4<1>(g, tmXd[0], tmWd, q, ct0 + main_tiles, ntl - main_tiles, st)) != TTDFT_OK) return s;
     dim3 gr((unsigned)((wc + 255) / 256), (unsigned)g.ncols);
-    ttdft::gram_reduce_kernel<<<gr, 256, 0, st>>>(P, g.wp, g.ncols, g.nchunks, wc, G + c0, ldg);
+    ttdft::gram_reduce_kernel<<<gr, 256, 0, st>>>(P, g.wp, g.ncols, g.nchunks, wc, G + c0, ldg, p.sym);
     CUDA_TRY(cudaGetLastError());
     g_launches.fetch_add(1);
   }
