@@ -1,6 +1,6 @@
 // cholesky.cuh -- the small dense fp64 pieces of the Cholesky-QR orthonormalisation (Algorithm 1 step 2,
 // PAPER.md:L226 "X_F = Orth(X)", L230 "Gram-Schmidt orthogonalization procedure"):
-//   G = X^T X  (ttdft_gram)  ->  G = L L^T  (potrf below)  ->  R^-1 = L^-T  (trinv below)  ->  X_F = X R^-1  (ttdft_rotate)
+//   G = X^T X  (ttdft_gram)  ->  G = L L^T  (potf2/trsm/syrk below)  ->  R^-1 = L^-T  (diaginv/level/transpose below)  ->  X_F = X R^-1  (ttdft_rotate)
 // For full-rank X the Q of Cholesky-QR is the Q of Gram-Schmidt (R is the unique upper-triangular factor with a
 // positive diagonal); the O(M n^2) work runs on the tensor cores, what is left here is O(n^3) on an n x n matrix
 // (23 GFLOP at n = 4,096) and is written for clarity, not speed: right-looking blocked Cholesky with 64-wide panels.
@@ -106,68 +106,97 @@ __global__ void __launch_bounds__(256) ch_syrk_kernel(double* __restrict__ A, in
     }
 }
 
-// R^-1 = L^-T, upper triangular, row-major n x n (ldr); the strict lower triangle of Rinv must be zero on entry.
-// W = L^-1 is computed by block columns: one CTA (256 threads) per block column k walks down the block rows
-//   W_ik = L_ii^-1 (delta_ik I - sum_{j=k}^{i-1} L_ij W_jk)
-// and stores W_ik transposed: Rinv[k0 + c, i0 + r] = W_ik[r, c].  Earlier blocks W_jk are re-read from Rinv (L2).
-__global__ void __launch_bounds__(256) ch_trinv_kernel(const double* __restrict__ A, int64_t ld, int32_t n, double* __restrict__ Rinv, int64_t ldr) {
-  extern __shared__ double ch_smem[];                        // 3 tiles (dynamic: 3 * CH_TILE_BYTES)
-  ch_tile_t& T = *reinterpret_cast<ch_tile_t*>(ch_smem);
-  ch_tile_t& Lb = *reinterpret_cast<ch_tile_t*>(ch_smem + CH_NB * (CH_NB + 1));
-  ch_tile_t& Wb = *reinterpret_cast<ch_tile_t*>(ch_smem + 2 * CH_NB * (CH_NB + 1));
-  const int32_t nb = (n + CH_NB - 1) / CH_NB;
-  const int32_t k = blockIdx.x, k0 = k * CH_NB, nk = min(CH_NB, n - k0);
-  const int tid = threadIdx.x;
-  const int tr = (tid >> 4) * 4, tc = (tid & 15) * 4;
-  for (int32_t i = k; i < nb; ++i) {
-    const int32_t i0 = i * CH_NB, ni = min(CH_NB, n - i0);
-    double acc[4][4] = {};
-    for (int32_t j = k; j < i; ++j) {
-      const int32_t j0 = j * CH_NB;                          // full block (j < i <= nb-1)
-      __syncthreads();
-      for (int e = tid; e < CH_NB * CH_NB; e += 256) {
-        const int r = e / CH_NB, c = e % CH_NB;
-        Lb[r][c] = (r < ni) ? A[(int64_t)(i0 + r) * ld + j0 + c] : 0.0;            // L_ij[r][c]
-        Wb[r][c] = (c < nk) ? Rinv[(int64_t)(k0 + c) * ldr + j0 + r] : 0.0;        // W_jk[r][c]
-      }
-      __syncthreads();
-      for (int t = 0; t < CH_NB; ++t) {
-        double a[4], b[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) { a[u] = Lb[tr + u][t]; b[u] = Wb[t][tc + u]; }
-#pragma unroll
-        for (int u = 0; u < 4; ++u)
-#pragma unroll
-          for (int w = 0; w < 4; ++w) acc[u][w] = fma(a[u], b[w], acc[u][w]);
-      }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int u = 0; u < 4; ++u)
-#pragma unroll
-      for (int w = 0; w < 4; ++w) T[tr + u][tc + w] = ((i == k && tr + u == tc + w) ? 1.0 : 0.0) - acc[u][w];
-    for (int e = tid; e < CH_NB * CH_NB; e += 256) {
-      const int r = e / CH_NB, c = e % CH_NB;
-      Lb[r][c] = (r < ni && c <= r) ? A[(int64_t)(i0 + r) * ld + i0 + c] : ((r == c) ? 1.0 : 0.0);   // L_ii, identity-padded
-    }
-    __syncthreads();
-    if (tid < CH_NB) {                                       // forward substitution, one thread per column of T
-      const int c = tid;
-      for (int r = 0; r < CH_NB; ++r) {
-        double v = T[r][c];
-        for (int t = 0; t < r; ++t) v -= Lb[r][t] * T[t][c];
-        T[r][c] = v / Lb[r][r];
-      }
-    }
-    __syncthreads();
-    for (int e = tid; e < CH_NB * CH_NB; e += 256) {
-      const int c = e / CH_NB, r = e % CH_NB;                // consecutive threads -> consecutive columns of Rinv
-      if (r < ni && c < nk) Rinv[(int64_t)(k0 + c) * ldr + i0 + r] = T[r][c];
-    }
-    __threadfence_block();
+// ------------------------------------------------------------------------------------------------
+// W = L^-1 by recursive doubling over 64-blocks, then R^-1 = W^T:
+//   W_kk = L_kk^-1 for every diagonal block (ch_diaginv), and for half sizes sb = 1, 2, 4, ... blocks, every pair of
+//   adjacent groups   [ L11  0  ]^-1   [      W11          0  ]
+//                     [ L21 L22 ]    = [ -W22 (L21 W11)   W22 ]      (ch_level: two block GEMMs, all pairs and tiles in one grid)
+// The dependency chain is 2 (1 + 2 + ... + nb/2) block products instead of nb^2 / 2 for a column-by-column substitution,
+// and every level keeps all SMs busy.  Triangular operands are not multiplied through their zero blocks.
+// ------------------------------------------------------------------------------------------------
+// grid nb, 64 threads: W_kk = L_kk^-1 (forward substitution on the identity, one thread per column)
+__global__ void __launch_bounds__(64) ch_diaginv_kernel(const double* __restrict__ A, int64_t ld, int32_t n, double* __restrict__ W, int64_t ldw) {
+  __shared__ double Lb[CH_NB][CH_NB + 1];
+  const int32_t k0 = blockIdx.x * CH_NB, nk = min(CH_NB, n - k0);
+  for (int e = threadIdx.x; e < nk * nk; e += 64) {
+    const int r = e / nk, c = e % nk;
+    Lb[r][c] = (c <= r) ? A[(int64_t)(k0 + r) * ld + k0 + c] : 0.0;
   }
+  __syncthreads();
+  const int c = threadIdx.x;
+  if (c >= nk) return;
+  double x[CH_NB];
+#pragma unroll 1
+  for (int r = 0; r < nk; ++r) {
+    double v = (r == c) ? 1.0 : 0.0;
+    for (int t = c; t < r; ++t) v -= Lb[r][t] * x[t];       // x[t] = 0 for t < c
+    x[r] = v / Lb[r][r];
+  }
+  for (int r = c; r < nk; ++r) W[(int64_t)(k0 + r) * ldw + k0 + c] = x[r];
 }
 
-// R^-1 of two passes combined is not needed: the second pass rotates the already rotated block.
+// One level of the recursion, one 64 x 64 output tile per CTA (256 threads, 4 x 4 register tiles), dynamic smem 2 tiles.
+//   mode 1:  T[bi, bj] =   sum_{t in first half, t >= bj} L[bi, t] W[t, bj]       (W11 is lower triangular)
+//   mode 2:  W[bi, bj] = - sum_{t in second half, t <= bi} W[bi, t] T[t, bj]      (W22 is lower triangular)
+// for bi in the second half of the pair, bj in the first half.  grid (sb, sb, pairs).
+__global__ void __launch_bounds__(256) ch_level_kernel(const double* __restrict__ A, int64_t lda, const double* __restrict__ B, int64_t ldb,
+                                                       double* __restrict__ C, int64_t ldc, int32_t n, int32_t sb, int32_t mode) {
+  extern __shared__ double ch_smem[];
+  ch_tile_t& As = *reinterpret_cast<ch_tile_t*>(ch_smem);
+  ch_tile_t& Bs = *reinterpret_cast<ch_tile_t*>(ch_smem + CH_NB * (CH_NB + 1));
+  const int32_t nb = (n + CH_NB - 1) / CH_NB;
+  const int32_t f0 = blockIdx.z * 2 * sb, s0 = f0 + sb, s1 = min(s0 + sb, nb);       // first half [f0, s0), second [s0, s1)
+  const int32_t bi = s0 + blockIdx.y, bj = f0 + blockIdx.x;
+  if (bi >= s1) return;
+  const int32_t tlo = (mode == 1) ? bj : s0, thi = (mode == 1) ? s0 : bi + 1;
+  const int tid = threadIdx.x, tr = (tid >> 4) * 4, tc = (tid & 15) * 4;
+  double acc[4][4] = {};
+  for (int32_t t = tlo; t < thi; ++t) {
+    __syncthreads();
+    for (int e = tid; e < CH_NB * CH_NB; e += 256) {
+      const int r = e / CH_NB, c = e % CH_NB;
+      const int64_t ar = (int64_t)bi * CH_NB + r, ac = (int64_t)t * CH_NB + c, br = (int64_t)t * CH_NB + r, bc = (int64_t)bj * CH_NB + c;
+      // triangular operands: only the lower part of a diagonal block is defined
+      const bool a_ok = ar < n && ac < n && !(mode == 2 && t == bi && c > r);
+      const bool b_ok = br < n && bc < n && !(mode == 1 && t == bj && c > r);
+      As[r][c] = a_ok ? A[ar * lda + ac] : 0.0;
+      Bs[r][c] = b_ok ? B[br * ldb + bc] : 0.0;
+    }
+    __syncthreads();
+    for (int k = 0; k < CH_NB; ++k) {
+      double a[4], b[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { a[u] = As[tr + u][k]; b[u] = Bs[k][tc + u]; }
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int w = 0; w < 4; ++w) acc[u][w] = fma(a[u], b[w], acc[u][w]);
+    }
+  }
+  const double sgn = (mode == 2) ? -1.0 : 1.0;
+#pragma unroll
+  for (int u = 0; u < 4; ++u)
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const int64_t i = (int64_t)bi * CH_NB + tr + u, j = (int64_t)bj * CH_NB + tc + w;
+      if (i < n && j < n) C[i * ldc + j] = sgn * acc[u][w];
+    }
+}
+
+// Rinv = W^T (upper triangular, zero below the diagonal); 32 x 32 tiles through shared memory
+__global__ void __launch_bounds__(256) ch_transpose_upper_kernel(const double* __restrict__ W, int64_t ldw, int32_t n, double* __restrict__ Rinv, int64_t ldr) {
+  __shared__ double t[32][33];
+  const int64_t a0 = (int64_t)blockIdx.y * 32, b0 = (int64_t)blockIdx.x * 32;       // Rinv tile rows a0.., columns b0..
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  for (int r = ty; r < 32; r += 8) {
+    const int64_t wb = b0 + r, wa = a0 + tx;                                         // W[b][a]
+    t[r][tx] = (wb < n && wa < n && wb >= wa) ? W[wb * ldw + wa] : 0.0;
+  }
+  __syncthreads();
+  for (int r = ty; r < 32; r += 8) {
+    const int64_t a = a0 + r, bcol = b0 + tx;
+    if (a < n && bcol < n) Rinv[a * ldr + bcol] = t[tx][r];
+  }
+}
 
 }  // namespace ttdft

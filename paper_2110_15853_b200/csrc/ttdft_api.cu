@@ -1077,16 +1077,18 @@ ttdft_status orth_plan(int64_t M, int64_t n, int32_t passes, OrthPlan* o) {
   o->nn = align_up((size_t)n * (size_t)ldn * 8, 1024);
   o->tmp = passes > 1 ? align_up((size_t)M * (size_t)ldn * 8, 1024) : 0;
   o->inner = std::max(o->g.total, o->r.total);
-  o->total = 2 * o->nn + 1024 + o->tmp + o->inner;
+  o->total = 3 * o->nn + 1024 + o->tmp + o->inner;
   return TTDFT_OK;
 }
 
-// G (lower triangle) -> L in place; Rinv = L^-T.  Returns the breakdown flag through *hflag (synchronises st).
-ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Rinv, int64_t ldr, int32_t* dflag, int32_t* hflag, cudaStream_t st) {
+// G (lower triangle) -> L in place; W = L^-1 (scratch); Rinv = L^-T (also the scratch T of the recursion).
+// Returns the breakdown flag through *hflag (synchronises st).
+ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Wm, double* Rinv, int64_t ldr, int32_t* dflag, int32_t* hflag,
+                          cudaStream_t st) {
   static bool attr_set = false;
   if (!attr_set) {
     CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
-    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_trinv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * ttdft::CH_TILE_BYTES));
+    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_level_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
     attr_set = true;
   }
   CUDA_TRY(cudaMemsetAsync(dflag, 0, 4, st));
@@ -1106,8 +1108,18 @@ ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Rinv, int64
   CUDA_TRY(cudaMemcpyAsync(hflag, dflag, 4, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   if (*hflag) return TTDFT_OK;                      // caller reports the breakdown
-  CUDA_TRY(cudaMemset2DAsync(Rinv, (size_t)ldr * 8, 0, (size_t)n * 8, (size_t)n, st));
-  ttdft::ch_trinv_kernel<<<(unsigned)((n + ttdft::CH_NB - 1) / ttdft::CH_NB), 256, 3 * ttdft::CH_TILE_BYTES, st>>>(G, ldg, n, Rinv, ldr);
+  // W = L^-1 by recursive doubling (Rinv's buffer serves as the intermediate T), then Rinv = W^T
+  const int32_t nb = (n + ttdft::CH_NB - 1) / ttdft::CH_NB;
+  ttdft::ch_diaginv_kernel<<<(unsigned)nb, 64, 0, st>>>(G, ldg, n, Wm, ldr);
+  g_launches.fetch_add(1);
+  for (int32_t sb = 1; sb < nb; sb *= 2) {
+    const unsigned pairs = (unsigned)((nb + 2 * sb - 1) / (2 * sb));
+    const dim3 grid((unsigned)sb, (unsigned)sb, pairs);
+    ttdft::ch_level_kernel<<<grid, 256, 2 * ttdft::CH_TILE_BYTES, st>>>(G, ldg, Wm, ldr, Rinv, ldr, n, sb, 1);    // T = L21 W11
+    ttdft::ch_level_kernel<<<grid, 256, 2 * ttdft::CH_TILE_BYTES, st>>>(Wm, ldr, Rinv, ldr, Wm, ldr, n, sb, 2);   // W21 = -W22 T
+    g_launches.fetch_add(2);
+  }
+  ttdft::ch_transpose_upper_kernel<<<dim3((unsigned)((n + 31) / 32), (unsigned)((n + 31) / 32)), 256, 0, st>>>(Wm, ldr, n, Rinv, ldr);
   CUDA_TRY(cudaGetLastError());
   g_launches.fetch_add(1);
   return TTDFT_OK;
@@ -1118,9 +1130,10 @@ ttdft_status orth_run(const OrthPlan& o, const double* X, int64_t ldx, double* Y
   const int64_t ldn = o.n + (o.n & 1);
   double* G = reinterpret_cast<double*>(wb);
   double* Rinv = reinterpret_cast<double*>(wb + o.nn);
-  int32_t* dflag = reinterpret_cast<int32_t*>(wb + 2 * o.nn);
-  double* T = reinterpret_cast<double*>(wb + 2 * o.nn + 1024);
-  void* inner = wb + 2 * o.nn + 1024 + o.tmp;
+  double* Wm = reinterpret_cast<double*>(wb + 2 * o.nn);
+  int32_t* dflag = reinterpret_cast<int32_t*>(wb + 3 * o.nn);
+  double* T = reinterpret_cast<double*>(wb + 3 * o.nn + 1024);
+  void* inner = wb + 3 * o.nn + 1024 + o.tmp;
   // pass p reads `src` and writes `dst`; the last pass must land in Y, intermediate results alternate Y / T
   const double* src = X;
   int64_t lds = ldx;
@@ -1131,7 +1144,7 @@ ttdft_status orth_run(const OrthPlan& o, const double* X, int64_t ldx, double* Y
     ttdft_status s = gram_run(o.g, src, lds, src, lds, G, ldn, inner, st);          // G = src^T src
     if (s != TTDFT_OK) return s;
     int32_t hflag = 0;
-    if ((s = chol_inverse(G, ldn, (int32_t)o.n, Rinv, ldn, dflag, &hflag, st)) != TTDFT_OK) return s;
+    if ((s = chol_inverse(G, ldn, (int32_t)o.n, Wm, Rinv, ldn, dflag, &hflag, st)) != TTDFT_OK) return s;
     if (hflag)
       return fail(TTDFT_ERR_BREAKDOWN, "orthonormalize: X^T X is not positive definite in pass %d (pivot %d): columns are linearly "
                                        "dependent to working precision", p + 1, hflag - 1);
