@@ -218,7 +218,7 @@ def main():
     dev = torch.device("cuda", local)
     t_build0 = time.perf_counter()
     Hd = tt.h_build_bsr(H.M, H.b, torch.from_numpy(H.row_ptr).to(dev), torch.from_numpy(H.col_idx).to(dev),
-                        torch.from_numpy(H.values).to(dev))
+                        torch.from_numpy(H.values).to(dev), flags=tt.CHECK_SORTED | tt.CHECK_SYMMETRY)
     torch.cuda.synchronize()
     t_build = time.perf_counter() - t_build0
     MODES = {"auto": tt.MATH_AUTO, "fp64": tt.MATH_FP64, "i8": tt.MATH_I8, "i8x7": tt.MATH_I8X7}

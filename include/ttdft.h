@@ -218,7 +218,9 @@ ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* X_host, int64_t l
  *                 ascending order in fp64: deterministic, error below an fp64 dot product's bound (K4).
  *                 X and W may be the same matrix; G must not overlap them.  ncols <= 65535.
  * ttdft_project:  G = X^T (H X): one ttdft_spmm_ws into scratch, then ttdft_gram.  G is symmetric up to rounding
- *                 when H is; it is NOT symmetrised.
+ *                 when H is.  If the handle was built with TTDFT_CHECK_SYMMETRY (H == H^T verified), only the upper
+ *                 triangle is computed and mirrored (G exactly symmetric, ~1/4 less time); otherwise every entry is
+ *                 computed as it stands and G is NOT symmetrised.
  * `work`: 1024-byte aligned DEVICE scratch of at least the bytes the matching *_work_bytes call reports.
  */
 ttdft_status ttdft_gram_work_bytes(int64_t M, int64_t ncols, size_t* bytes);

@@ -197,6 +197,7 @@ struct ttdft_h_s {
   const double* hdiag = nullptr;  // [M]
   CUtensorMap tmHd[4];      // box rows b, b/2, b/4, b/8: K3 in clusters of 1, 2, 4, 8 CTAs (every CTA fetches b/C rows of a plane)
   int32_t nsm = 148;
+  int32_t sym_checked = 0;         // TTDFT_CHECK_SYMMETRY passed at build: H == H^T bit for bit
   const int32_t* perm = nullptr;   // rows reordered by subdomain label: row r of the tiles is the caller's row perm[r]
   int32_t k3_cluster = 0;   // 0: choose per launch; 1, 2, 4, 8: forced (env TTDFT_K3_CLUSTER)
   int32_t k3_cg = 0;        // column tiles per scheduling group of K3 (env TTDFT_K3_CG; 0: one cluster's tiles)
@@ -900,8 +901,10 @@ ttdft_status launch_k4(const GramPlan& g, const CUtensorMap& tmXd, const CUtenso
   return TTDFT_OK;
 }
 
+// sym_hint: the caller knows G is symmetric (W = H X with a symmetry-checked H): as for W == X only the tile groups that
+// touch the upper triangle are computed and the reduction mirrors them
 ttdft_status gram_run(const GramPlan& g, const double* X, int64_t ldx, const double* W, int64_t ldw, double* G, int64_t ldg, void* work,
-                      cudaStream_t st) {
+                      cudaStream_t st, bool sym_hint = false) {
   constexpr int S = GRAM_S;
   if (g.M == 0) {   // empty contraction: G = 0
     CUDA_TRY(cudaMemset2DAsync(G, (size_t)ldg * 8, 0, (size_t)g.ncols * 8, (size_t)g.ncols, st));
@@ -944,7 +947,7 @@ ttdft_status gram_run(const GramPlan& g, const double* X, int64_t ldx, const dou
   p.ncols = g.ncols; p.P = P; p.cmaxX = cmX; p.cmaxW = cmW;
   // G = X^T X: only the tiles that touch the upper triangle are computed (single panel only: the mirror image of an
   // entry must be in the same panel of partial tiles)
-  p.sym = (X == W && ldx == ldw && g.wp >= g.ncols && env_int("TTDFT_K4_SYM", 1)) ? 1 : 0;
+  p.sym = (((X == W && ldx == ldw) || sym_hint) && g.wp >= g.ncols && env_int("TTDFT_K4_SYM", 1)) ? 1 : 0;
   const int C = env_int("TTDFT_K4_CLUSTER", 2) == 1 ? 1 : 2;
   for (int64_t c0 = 0; c0 < g.ncols; c0 += g.wp) {
     const int64_t wc = std::min(g.wp, g.ncols - c0);
@@ -1376,6 +1379,7 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
   ttdft_h_s* h = new (std::nothrow) ttdft_h_s;
   if (!h) return fail(TTDFT_ERR_CUDA, "out of host memory");
   h->M = d->M;
+  h->sym_checked = (d->M > 0 && (d->flags & TTDFT_CHECK_SYMMETRY)) ? 1 : 0;   // reached only if the check passed
   h->storage_bytes = need + need_i8;
   uint8_t* base = reinterpret_cast<uint8_t*>(dev_storage);
 
@@ -1851,7 +1855,7 @@ ttdft_status ttdft_project(ttdft_h_t h, const double* X, int64_t ldx, int64_t nc
     s = step_ws(h, 1.0, 0.0, 0.0, X, ldx, nullptr, 0, Wb, ldw, ncols, rest, need - wbytes, st);   // W = H X
     if (s != TTDFT_OK) return s;
   }
-  return gram_run(g, X, ldx, Wb, ldw, G, ldg, rest, st);                                          // G = X^T W
+  return gram_run(g, X, ldx, Wb, ldw, G, ldg, rest, st, h->sym_checked != 0);                     // G = X^T W
 }
 
 ttdft_status ttdft_rotate_work_bytes(int64_t M, int64_t k, int64_t n, size_t* bytes) {

@@ -112,6 +112,21 @@ def test_project_vs_oracle(tt, G_, b, z, N):
     assert relerr(Gd.cpu().numpy(), ref) <= TOL
 
 
+def test_project_symmetric_shortcut(tt):
+    """A handle whose symmetry was verified at build computes only the upper triangle of H_F and mirrors it."""
+    import torch
+    H, C, _, _ = small_problem(3, 128, 0.4, 2128)
+    N = 300
+    X = synth.dense_normal(H.M, N, 361)
+    ref = oracle.project(C.row_ptr, C.col_idx, C.values, X)
+    Hd = tt.h_build_bsr(H.M, H.b, dev(H.row_ptr), dev(H.col_idx), dev(H.values), flags=tt.CHECK_SORTED | tt.CHECK_SYMMETRY)
+    Gd = torch.full((N, N), float("nan"), dtype=torch.float64, device="cuda")
+    tt.project(Hd, dev(X), Gd)
+    got = Gd.cpu().numpy()
+    assert relerr(got, ref) <= TOL
+    assert np.array_equal(got, got.T)                        # mirrored: exactly symmetric
+
+
 def test_project_csr_and_reordered_handles(tt):
     import torch
     H, C, _, _ = small_problem(3, 64, 0.3, 2064)
