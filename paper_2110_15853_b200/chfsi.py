@@ -1,0 +1,51 @@
+"""One pass of Algorithm 1 (ChFSI) composed from the library's calls -- a usage example and an
+end-to-end check, not a new kernel:
+
+    step 1  ttdft_cheb_filter      X~  = p_m(H) X                      (the hot path)
+    step 2  ttdft_orthonormalize   X_F = Orth(X~)                      (8(f)-2)
+    step 3  ttdft_project          H_F = X_F^T H X_F                   (8(f)-1)
+    step 4  torch.linalg.eigh      H_F Q = Q Lambda                    (n x n dense symmetric eigenproblem: the ONE library call;
+                                                                        "library-shaped" in SURVEY.md 8(f)-4, not implemented here)
+    step 5  ttdft_rotate           Psi = X_F Q                         (8(f)-4)
+
+Everything of size M x n runs in the library's CUDA kernels; PyTorch allocates the buffers and solves the n x n problem.
+"""
+from __future__ import annotations
+
+from . import api
+
+
+def chfsi_iteration(H: "api.Hamiltonian", X, m: int, a: float, b: float, a0: float, panel_cols: int = 0):
+    """Returns (Psi, Lambda): Psi M x n with orthonormal columns spanning the filtered subspace, rotated to the Ritz vectors;
+    Lambda the n Ritz values in ascending order.  X: M x n float64 CUDA tensor (not modified)."""
+    import torch
+    M, n = X.shape
+    Xf = torch.empty_like(X)
+    api.cheb_filter(H, X, Xf, m, a, b, a0, panel_cols=panel_cols)          # step 1
+    Xo = torch.empty_like(X)
+    api.orthonormalize(Xf, Xo, passes=2)                                   # step 2
+    del Xf
+    HF = torch.empty((n, n), dtype=torch.float64, device=X.device)
+    api.project(H, Xo, HF)                                                 # step 3
+    HF = 0.5 * (HF + HF.T)
+    lam, Q = torch.linalg.eigh(HF)                                         # step 4 (library)
+    Psi = torch.empty_like(X)
+    api.rotate(Xo, Q.contiguous(), Psi)                                    # step 5
+    return Psi, lam
+
+
+def chfsi(H: "api.Hamiltonian", X, m: int, b: float, a0: float, iterations: int, a: float | None = None):
+    """`iterations` passes of Algorithm 1 with the usual bound update between passes (the paper takes the bounds as inputs and
+    refers to [30, 31]): the filter damps [a, b]; after every pass a = largest Ritz value (the upper edge of the wanted
+    spectrum), a0 = smallest Ritz value.  Returns (Psi, Lambda) of the last pass."""
+    lam = None
+    for _ in range(iterations):
+        if lam is not None:
+            a = float(lam[-1])
+            a0 = min(a0, float(lam[0]))
+        if a is None:
+            a = a0 + (b - a0) * X.shape[1] / X.shape[0]
+        if not (a0 < a < b):
+            a = a0 + 1e-3 * (b - a0)
+        X, lam = chfsi_iteration(H, X, m, a, b, a0)
+    return X, lam
