@@ -229,3 +229,40 @@ def test_cluster_sizes_and_l2_hints(tt, cluster, hints):
                 os.environ.pop(k, None)
     assert relerr(out[None], ref) <= TOL_FILTER
     assert np.array_equal(out[None], out[(cluster, hints)])
+
+
+def test_row_dynamic_range_and_zero_rows(tt):
+    """Per-row scaling of H: rows 40 orders of magnitude apart, an all-zero row, a row with only its diagonal entry -- every row
+    keeps its own relative accuracy (the product is defined for a non-symmetric H too)."""
+    import copy
+    import torch
+    H0, _, _, _ = small_problem(3, 64, 0.3, 2064)
+    H = copy.copy(H0)
+    vals = H0.values.copy().reshape(H0.nblocks, H0.b, H0.b)
+    scale = 10.0 ** np.linspace(-20, 20, H0.M)
+    tile_row = np.repeat(np.arange(H0.M // H0.b), np.diff(H0.row_ptr))
+    for p in range(H0.nblocks):
+        vals[p] *= scale[tile_row[p] * H0.b:(tile_row[p] + 1) * H0.b, None]
+    zr, dr = 5, 70                                            # global rows: all zero / diagonal only
+    for p in range(H0.nblocks):
+        I, J = tile_row[p], H0.col_idx[p]
+        if I == zr // H0.b:
+            vals[p][zr % H0.b, :] = 0.0
+        if I == dr // H0.b:
+            d = vals[p][dr % H0.b, dr % H0.b] if J == I else 0.0
+            vals[p][dr % H0.b, :] = 0.0
+            if J == I:
+                vals[p][dr % H0.b, dr % H0.b] = d
+    H.values = vals.reshape(H0.values.shape)
+    rp, col, val = oracle.bsr_to_csr(H.b, H.row_ptr, H.col_idx, H.values)
+    Hd = build_i8(tt, H, mode="i8x7")
+    N = 96
+    X = synth.dense_normal(H.M, N, 81)
+    ref = oracle.spmm(rp, col, val, 1.0, X)
+    Y = torch.empty(H.M, N, dtype=torch.float64, device="cuda")
+    tt.spmm(Hd, 1.0, dev(X), 0.0, Y, use_work=True)
+    got = Y.cpu().numpy()
+    assert np.all(got[zr] == 0.0)
+    rn = np.linalg.norm(ref, axis=1)
+    rn[rn == 0] = 1.0
+    assert np.max(np.linalg.norm(got - ref, axis=1) / rn) <= 10 * ACC["i8x7"]
