@@ -260,6 +260,19 @@ ttdft_status ttdft_orthonormalize_work_bytes(int64_t M, int64_t n, int32_t passe
 ttdft_status ttdft_orthonormalize(int64_t M, const double* X, int64_t ldx, int64_t n, double* Y, int64_t ldy, int32_t passes, void* work,
                                   size_t work_bytes, void* stream);
 
+/*
+ * Spectral bounds by a k-step Lanczos.  Algorithm 1 takes eps_0 and eps_ub^uw as inputs and refers to
+ * [30, 31] for them; reading #5: k steps of plain Lanczos (no reorthogonalisation) from the
+ * start vector v0, eigenpairs (theta, z) of the k x k tridiagonal, and the residual-corrected Ritz bounds
+ *     b = theta_max + |beta_k z_max[k]|  >= lambda_max(H),      a0 = theta_min - |beta_k z_min[k]|  <= lambda_min(H) (nearly always)
+ * v0: DEVICE vector of length M (stride 1), not modified.  1 <= k <= 64.  a0_out, b_out: HOST.  theta_out: HOST array of k
+ * Ritz values in ascending order, or NULL.  steps_out: HOST, the number of steps actually taken (< k if an invariant subspace
+ * was found), or NULL.  The call synchronises `stream`.  `work`: 1024-byte aligned DEVICE scratch of ttdft_lanczos_work_bytes.
+ */
+ttdft_status ttdft_lanczos_work_bytes(ttdft_h_t h, size_t* bytes);
+ttdft_status ttdft_lanczos_bounds(ttdft_h_t h, int32_t k, const double* v0, void* work, size_t work_bytes, void* stream, double* a0_out,
+                                  double* b_out, double* theta_out, int32_t* steps_out);
+
 /* Measured fp64 rate of this GPU: kind 0 = scalar DFMA loop, 1 = DMMA (mma.sync m8n8k4.f64) loop;
  * runs for about `millis` ms on `stream`, synchronises, returns TFLOP/s in *tflops. */
 ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, double* tflops);

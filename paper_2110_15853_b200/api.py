@@ -22,6 +22,7 @@ exported_symbols = [
     "ttdft_timing_enable", "ttdft_timing_read",
     "ttdft_gram_work_bytes", "ttdft_gram", "ttdft_project_work_bytes", "ttdft_project",
     "ttdft_rotate_work_bytes", "ttdft_rotate", "ttdft_orthonormalize_work_bytes", "ttdft_orthonormalize",
+    "ttdft_lanczos_work_bytes", "ttdft_lanczos_bounds",
 ]
 
 
@@ -109,6 +110,11 @@ def _load() -> ctypes.CDLL:
     L.ttdft_orthonormalize_work_bytes.argtypes = [c_int64, c_int64, c_int32, POINTER(c_size_t)]
     L.ttdft_orthonormalize.restype = st
     L.ttdft_orthonormalize.argtypes = [c_int64, c_void_p, c_int64, c_int64, c_void_p, c_int64, c_int32, c_void_p, c_size_t, c_void_p]
+    L.ttdft_lanczos_work_bytes.restype = st
+    L.ttdft_lanczos_work_bytes.argtypes = [c_void_p, POINTER(c_size_t)]
+    L.ttdft_lanczos_bounds.restype = st
+    L.ttdft_lanczos_bounds.argtypes = [c_void_p, c_int32, c_void_p, c_void_p, c_size_t, c_void_p, POINTER(c_double), POINTER(c_double),
+                                       POINTER(c_double), POINTER(c_int32)]
     L.ttdft_probe_fp64_peak.restype = st
     L.ttdft_probe_fp64_peak.argtypes = [c_int32, c_int32, c_void_p, POINTER(c_double)]
     L.ttdft_timing_enable.restype = st
@@ -441,6 +447,21 @@ def orthonormalize(X, Y, passes: int = 2, work=None, stream=None):
     wp, wb, keep = _aligned_work(orthonormalize_work_bytes(M, n, passes), work, X.device)
     _check(_load().ttdft_orthonormalize(M, xp, ldx, n, yp, ldy, passes, wp, wb, _stream(stream)))
     return Y
+
+
+def lanczos_bounds(H: Hamiltonian, v0, k: int = 30, stream=None):
+    """(a0, b, theta) from k Lanczos steps (ttdft_lanczos_bounds): a0 <= lambda_min (nearly always), b >= lambda_max, theta the Ritz values."""
+    torch = _torch()
+    if v0.dtype != torch.float64 or not v0.is_cuda or v0.dim() != 1 or v0.shape[0] != H.M or (H.M > 1 and v0.stride(0) != 1):
+        raise TypeError("v0 must be a contiguous 1-D float64 CUDA tensor of length M")
+    out = c_size_t(0)
+    _check(_load().ttdft_lanczos_work_bytes(H.handle, byref(out)))
+    wp, wb, keep = _aligned_work(int(out.value), None, v0.device)
+    a0, b = c_double(0.0), c_double(0.0)
+    theta = (c_double * 64)()
+    steps = c_int32(0)
+    _check(_load().ttdft_lanczos_bounds(H.handle, k, v0.data_ptr(), wp, wb, _stream(stream), byref(a0), byref(b), theta, byref(steps)))
+    return a0.value, b.value, [theta[i] for i in range(steps.value)]
 
 
 def probe_fp64_peak(kind: int = 1, millis: int = 200, stream=None) -> float:

@@ -34,6 +34,15 @@ def chfsi_iteration(H: "api.Hamiltonian", X, m: int, a: float, b: float, a0: flo
     return Psi, lam
 
 
+def bounds(H: "api.Hamiltonian", k: int = 30, seed: int = 0):
+    """(a0, b): lower and upper bound of the spectrum by k Lanczos steps on the GPU (ttdft_lanczos_bounds) from a seeded start vector."""
+    import torch
+    g = torch.Generator(device="cuda").manual_seed(seed)
+    v0 = torch.randn(H.M, dtype=torch.float64, device="cuda", generator=g)
+    a0, b, _ = api.lanczos_bounds(H, v0, k)
+    return a0, b
+
+
 def chfsi(H: "api.Hamiltonian", X, m: int, b: float, a0: float, iterations: int, a: float | None = None):
     """`iterations` passes of Algorithm 1 with the usual bound update between passes (the paper takes the bounds as inputs and
     refers to [30, 31]): the filter damps [a, b]; after every pass a = largest Ritz value (the upper edge of the wanted

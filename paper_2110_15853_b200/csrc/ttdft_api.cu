@@ -5,10 +5,12 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <atomic>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
+#include <cmath>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -21,6 +23,7 @@
 #include "generic_spmm.cuh"
 #include "cholesky.cuh"
 #include "gram_i8.cuh"
+#include "lanczos.cuh"
 
 namespace {
 
@@ -1158,6 +1161,44 @@ ttdft_status orth_run(const OrthPlan& o, const double* X, int64_t ldx, double* Y
   return TTDFT_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// ttdft_lanczos_bounds: host side -- eigenpairs of the k x k Lanczos tridiagonal by cyclic Jacobi (k <= 64, O(k^3) host work
+// like the scalars of A1), then the residual-corrected Ritz bounds of DESIGN.md reading #5
+// ------------------------------------------------------------------------------------------------
+void host_jacobi_eig(int n, std::vector<double>& A, std::vector<double>& V) {
+  V.assign((size_t)n * n, 0.0);
+  for (int i = 0; i < n; ++i) V[(size_t)i * n + i] = 1.0;
+  for (int sweep = 0; sweep < 100; ++sweep) {
+    double off = 0.0, diag = 0.0;
+    for (int i = 0; i < n; ++i)
+      for (int j = 0; j < n; ++j) (i == j ? diag : off) += A[(size_t)i * n + j] * A[(size_t)i * n + j];
+    if (off <= 1e-32 * diag || off == 0.0) break;
+    for (int p = 0; p < n - 1; ++p)
+      for (int q = p + 1; q < n; ++q) {
+        const double apq = A[(size_t)p * n + q];
+        if (apq == 0.0) continue;
+        const double tau = (A[(size_t)q * n + q] - A[(size_t)p * n + p]) / (2.0 * apq);
+        const double t = (tau >= 0.0 ? 1.0 : -1.0) / (std::fabs(tau) + std::sqrt(1.0 + tau * tau));
+        const double c = 1.0 / std::sqrt(1.0 + t * t), sn = t * c;
+        for (int k = 0; k < n; ++k) {       // columns p, q
+          const double akp = A[(size_t)k * n + p], akq = A[(size_t)k * n + q];
+          A[(size_t)k * n + p] = c * akp - sn * akq;
+          A[(size_t)k * n + q] = sn * akp + c * akq;
+        }
+        for (int k = 0; k < n; ++k) {       // rows p, q
+          const double apk = A[(size_t)p * n + k], aqk = A[(size_t)q * n + k];
+          A[(size_t)p * n + k] = c * apk - sn * aqk;
+          A[(size_t)q * n + k] = sn * apk + c * aqk;
+        }
+        for (int k = 0; k < n; ++k) {
+          const double vkp = V[(size_t)k * n + p], vkq = V[(size_t)k * n + q];
+          V[(size_t)k * n + p] = c * vkp - sn * vkq;
+          V[(size_t)k * n + q] = sn * vkp + c * vkq;
+        }
+      }
+  }
+}
+
 }  // namespace
 
 // ================================================================================================
@@ -1901,6 +1942,83 @@ ttdft_status ttdft_orthonormalize(int64_t M, const double* X, int64_t ldx, int64
   if (work_bytes < o.total) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, o.total);
   if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
   return orth_run(o, X, ldx, Y, ldy, work, (cudaStream_t)stream);
+}
+
+ttdft_status ttdft_lanczos_work_bytes(ttdft_h_t h, size_t* bytes) {
+  if (!h || !bytes) return fail(TTDFT_ERR_INVALID_ARG, "NULL argument");
+  *bytes = 3 * align_up((size_t)h->M * ttdft::LZ_LD * 8, 1024) + 4 * 8192;
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_lanczos_bounds(ttdft_h_t h, int32_t k, const double* v0, void* work, size_t work_bytes, void* stream, double* a0_out,
+                                  double* b_out, double* theta_out, int32_t* steps_out) {
+  if (!h || !v0 || !a0_out || !b_out) return fail(TTDFT_ERR_INVALID_ARG, "NULL argument");
+  if (k < 1 || k > 64) return fail(TTDFT_ERR_INVALID_ARG, "lanczos: 1 <= k <= 64 required");
+  if (h->M < 1) return fail(TTDFT_ERR_INVALID_ARG, "lanczos: empty matrix");
+  if (k > h->M) k = (int32_t)h->M;
+  size_t need;
+  ttdft_lanczos_work_bytes(h, &need);
+  if (work_bytes < need) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, need);
+  if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t M = h->M;
+  const size_t vb = align_up((size_t)M * ttdft::LZ_LD * 8, 1024);
+  uint8_t* wb = reinterpret_cast<uint8_t*>(work);
+  double* v = reinterpret_cast<double*>(wb);
+  double* vprev = reinterpret_cast<double*>(wb + vb);
+  double* w = reinterpret_cast<double*>(wb + 2 * vb);
+  double* part = reinterpret_cast<double*>(wb + 3 * vb);
+  double* part2 = reinterpret_cast<double*>(wb + 3 * vb + 8192);
+  double* dalpha = reinterpret_cast<double*>(wb + 3 * vb + 2 * 8192);
+  double* dbeta = dalpha + 64;
+  int32_t* dstatus = reinterpret_cast<int32_t*>(wb + 3 * vb + 3 * 8192);
+  CUDA_TRY(cudaMemsetAsync(wb, 0, 3 * vb, st));                      // column 1 of the panels stays zero
+  // v0 is a plain vector (stride 1): its squared norm through a strided view is not available, so copy it into w's column 0
+  CUDA_TRY(cudaMemcpy2DAsync(w, ttdft::LZ_LD * 8, v0, 8, 8, (size_t)M, cudaMemcpyDeviceToDevice, st));
+  ttdft::lz_dot_kernel<<<ttdft::LZ_GRID, 256, 0, st>>>(w, w, M, part);
+  ttdft::lz_start_kernel<<<ttdft::LZ_GRID, 256, 0, st>>>(v0, M, part, v, vprev, dstatus);
+  g_launches.fetch_add(2);
+  for (int32_t j = 0; j < k; ++j) {
+    ttdft_status s = launch_step(h, 1.0, 0.0, 0.0, v, ttdft::LZ_LD, nullptr, 0, w, ttdft::LZ_LD, 1, st, true);   // w = H v
+    if (s != TTDFT_OK) return s;
+    ttdft::lz_dot_kernel<<<ttdft::LZ_GRID, 256, 0, st>>>(w, v, M, part);
+    ttdft::lz_update_kernel<<<ttdft::LZ_GRID, 256, 0, st>>>(w, v, vprev, M, part, dalpha, dbeta, j, part2);
+    ttdft::lz_finish_kernel<<<ttdft::LZ_GRID, 256, 0, st>>>(w, v, vprev, M, part2, dbeta, j);
+    g_launches.fetch_add(3);
+  }
+  CUDA_TRY(cudaGetLastError());
+  double ha[64], hb[64];
+  int32_t hstat = 0;
+  CUDA_TRY(cudaMemcpyAsync(ha, dalpha, (size_t)k * 8, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemcpyAsync(hb, dbeta, (size_t)k * 8, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaMemcpyAsync(&hstat, dstatus, 4, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (hstat) return fail(TTDFT_ERR_INVALID_ARG, "lanczos: the start vector is zero (or not finite)");
+  int kk = k;
+  for (int j = 0; j < k; ++j)
+    if (hb[j] == 0.0) { kk = j + 1; break; }                         // invariant subspace: the bounds are exact
+  std::vector<double> T((size_t)kk * kk, 0.0), V;
+  for (int j = 0; j < kk; ++j) {
+    T[(size_t)j * kk + j] = ha[j];
+    if (j + 1 < kk) { T[(size_t)j * kk + j + 1] = hb[j]; T[(size_t)(j + 1) * kk + j] = hb[j]; }
+  }
+  host_jacobi_eig(kk, T, V);
+  int imin = 0, imax = 0;
+  for (int j = 1; j < kk; ++j) {
+    if (T[(size_t)j * kk + j] < T[(size_t)imin * kk + imin]) imin = j;
+    if (T[(size_t)j * kk + j] > T[(size_t)imax * kk + imax]) imax = j;
+  }
+  const double res = hb[kk - 1];
+  *b_out = T[(size_t)imax * kk + imax] + std::fabs(res * V[(size_t)(kk - 1) * kk + imax]);
+  *a0_out = T[(size_t)imin * kk + imin] - std::fabs(res * V[(size_t)(kk - 1) * kk + imin]);
+  if (theta_out) {
+    std::vector<double> th((size_t)kk);
+    for (int j = 0; j < kk; ++j) th[(size_t)j] = T[(size_t)j * kk + j];
+    std::sort(th.begin(), th.end());
+    for (int j = 0; j < kk; ++j) theta_out[j] = th[(size_t)j];
+  }
+  if (steps_out) *steps_out = kk;
+  return TTDFT_OK;
 }
 
 ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, double* tflops) {
