@@ -231,7 +231,9 @@ def main():
 
     # this rank's band of wavefunctions: columns [rank*N, (rank+1)*N) of the global block (host, pinned)
     Xh = torch.empty((cfg.M, cfg.N), dtype=torch.float64).pin_memory()
-    synth.dense_normal(cfg.M, cfg.N, cfg.seed, synth.STREAM_X, col0=rank * cfg.N, out=Xh.numpy())
+    from paper_2110_15853_b200 import bands
+    band0, _ = bands.weak_band(rank, cfg.N)
+    synth.dense_normal(cfg.M, cfg.N, cfg.seed, synth.STREAM_X, col0=band0, out=Xh.numpy())
     Yh = torch.empty((cfg.M, cfg.N), dtype=torch.float64).pin_memory()
     Xd = Xh.to(dev, non_blocking=True)
     Yd = torch.empty_like(Xd)
