@@ -106,7 +106,7 @@ typedef struct {
   int64_t M;
   int64_t nnz_stored;     /* stored scalar entries incl. explicit zeros (BSR: nblocks*b*b) */
   int32_t block;          /* tile size of the device format, 0 if CSR                       */
-  int32_t kernel;         /* 1 = block-sparse TMA + fp64 tensor-core kernel, 0 = generic    */
+  int32_t kernel;         /* 1 = block-sparse tile kernels (fp64 / int8 tensor cores), 0 = generic */
   int64_t nblocks;
   size_t storage_bytes;
   int32_t i8_planes;      /* digit planes per operand of H stored for the I8 modes (0: not built) */
