@@ -1,6 +1,6 @@
 // cholesky.cuh -- the small dense fp64 pieces of the Cholesky-QR orthonormalisation (Algorithm 1 step 2,
 // PAPER.md:L226 "X_F = Orth(X)", L230 "Gram-Schmidt orthogonalization procedure"):
-//   G = X^T X  (ttdft_gram)  ->  G = L L^T  (potf2/trsm/syrk below)  ->  R^-1 = L^-T  (diaginv/level/transpose below)  ->  X_F = X R^-1  (ttdft_rotate)
+//   G = X^T X  (ttdft_gram)  ->  G = L L^T  (potf2/panel/syrk below)  ->  R^-1 = L^-T  (level/transpose below)  ->  X_F = X R^-1  (ttdft_rotate)
 // For full-rank X the Q of Cholesky-QR is the Q of Gram-Schmidt (R is the unique upper-triangular factor with a
 // positive diagonal); the O(M n^2) work runs on the tensor cores, what is left here is O(n^3) on an n x n matrix
 // (23 GFLOP at n = 4,096) and is written for clarity, not speed: right-looking blocked Cholesky with 64-wide panels.
@@ -17,8 +17,12 @@ typedef double ch_tile_t[CH_NB][CH_NB + 1];
 
 // Diagonal block: A[k0:k0+nbk, k0:k0+nbk] = L_kk L_kk^T, unblocked, one CTA of 256 threads.
 // flag[0] = 1 + (index of the first non-positive pivot) if the matrix is not positive definite.
-__global__ void __launch_bounds__(256) ch_potf2_kernel(double* __restrict__ A, int64_t ld, int32_t k0, int32_t nbk, int32_t* __restrict__ flag) {
-  __shared__ double s[CH_NB][CH_NB + 1];
+// Also W[k0.., k0..] = L_kk^-1 (lower triangular), which turns the panel solve into a product and seeds the inverse.
+__global__ void __launch_bounds__(256) ch_potf2_kernel(double* __restrict__ A, int64_t ld, int32_t k0, int32_t nbk, int32_t* __restrict__ flag,
+                                                       double* __restrict__ W, int64_t ldw) {
+  extern __shared__ double ch_smem[];                        // 2 tiles (dynamic: 2 * CH_TILE_BYTES): L_kk and its inverse
+  ch_tile_t& s = *reinterpret_cast<ch_tile_t*>(ch_smem);
+  ch_tile_t& w = *reinterpret_cast<ch_tile_t*>(ch_smem + CH_NB * (CH_NB + 1));
   const int tid = threadIdx.x;
   for (int e = tid; e < nbk * nbk; e += 256) {
     const int r = e / nbk, c = e % nbk;
@@ -47,28 +51,52 @@ __global__ void __launch_bounds__(256) ch_potf2_kernel(double* __restrict__ A, i
     const int r = e / nbk, c = e % nbk;
     if (c <= r) A[(int64_t)(k0 + r) * ld + k0 + c] = s[r][c];
   }
-}
-
-// Panel below the diagonal block: A[i, k0:k0+nbk] <- A[i, k0:k0+nbk] L_kk^-T for rows i >= k0+nbk.
-// One CTA per 64 rows, one thread per row (forward substitution along the row), L_kk in shared memory.
-__global__ void __launch_bounds__(64) ch_trsm_kernel(double* __restrict__ A, int64_t ld, int32_t n, int32_t k0, int32_t nbk) {
-  __shared__ double L[CH_NB][CH_NB + 1];
-  for (int e = threadIdx.x; e < nbk * nbk; e += 64) {
-    const int r = e / nbk, c = e % nbk;
-    L[r][c] = (c <= r) ? A[(int64_t)(k0 + r) * ld + k0 + c] : 0.0;
+  // W_kk = L_kk^-1: forward substitution on the identity, one thread per column, then stored
+  if (tid < nbk) {
+    const int c = tid;
+    for (int r = c; r < nbk; ++r) {
+      double v = (r == c) ? 1.0 : 0.0;
+      for (int t = c; t < r; ++t) v -= s[r][t] * w[t][c];
+      w[r][c] = v / s[r][r];
+    }
   }
   __syncthreads();
-  const int64_t i = (int64_t)k0 + nbk + (int64_t)blockIdx.x * 64 + threadIdx.x;
-  if (i >= n) return;
-  double* a = A + i * ld + k0;
-  double x[CH_NB];
-#pragma unroll 1
-  for (int c = 0; c < nbk; ++c) {
-    double v = a[c];
-    for (int t = 0; t < c; ++t) v -= x[t] * L[c][t];
-    x[c] = v / L[c][c];
+  for (int e = tid; e < nbk * nbk; e += 256) {
+    const int r = e / nbk, c = e % nbk;
+    if (c <= r) W[(int64_t)(k0 + r) * ldw + k0 + c] = w[r][c];
   }
-  for (int c = 0; c < nbk; ++c) a[c] = x[c];
+}
+
+// Panel below the diagonal block: A[i, k0:k0+nbk] <- A[i, k0:k0+nbk] L_kk^-T = A[i, :] W_kk^T for rows i >= k0+nbk.
+// One CTA (256 threads, 4 x 4 register tiles) per 64 rows; dynamic smem 2 tiles.
+__global__ void __launch_bounds__(256) ch_panel_kernel(double* __restrict__ A, int64_t ld, int32_t n, int32_t k0, int32_t nbk,
+                                                       const double* __restrict__ W, int64_t ldw) {
+  extern __shared__ double ch_smem[];
+  ch_tile_t& As = *reinterpret_cast<ch_tile_t*>(ch_smem);
+  ch_tile_t& Ws = *reinterpret_cast<ch_tile_t*>(ch_smem + CH_NB * (CH_NB + 1));
+  const int64_t i0 = (int64_t)k0 + nbk + (int64_t)blockIdx.x * 64;
+  for (int e = threadIdx.x; e < CH_NB * CH_NB; e += 256) {
+    const int r = e / CH_NB, c = e % CH_NB;
+    As[r][c] = (i0 + r < n && c < nbk) ? A[(i0 + r) * ld + k0 + c] : 0.0;
+    Ws[r][c] = (r < nbk && c <= r) ? W[(int64_t)(k0 + r) * ldw + k0 + c] : 0.0;      // W_kk[r][c], lower triangular
+  }
+  __syncthreads();
+  const int tr = (threadIdx.x >> 4) * 4, tc = (threadIdx.x & 15) * 4;
+  double acc[4][4] = {};
+  for (int t = 0; t < nbk; ++t) {            // P[i][c] = sum_t A[i][t] W_kk[c][t]
+    double a[4], b[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { a[u] = As[tr + u][t]; b[u] = Ws[tc + u][t]; }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+      for (int w = 0; w < 4; ++w) acc[u][w] = fma(a[u], b[w], acc[u][w]);
+  }
+#pragma unroll
+  for (int u = 0; u < 4; ++u)
+#pragma unroll
+    for (int w = 0; w < 4; ++w)
+      if (i0 + tr + u < n && tc + w < nbk) A[(i0 + tr + u) * ld + k0 + tc + w] = acc[u][w];
 }
 
 // Trailing update: A[i, j] -= sum_t P[i, t] P[j, t] for k1 <= j <= i < n (lower triangle), P = A[:, k0:k0+nbk], k1 = k0+nbk.
@@ -108,33 +136,12 @@ __global__ void __launch_bounds__(256) ch_syrk_kernel(double* __restrict__ A, in
 
 // ------------------------------------------------------------------------------------------------
 // W = L^-1 by recursive doubling over 64-blocks, then R^-1 = W^T:
-//   W_kk = L_kk^-1 for every diagonal block (ch_diaginv), and for half sizes sb = 1, 2, 4, ... blocks, every pair of
+//   W_kk = L_kk^-1 for every diagonal block (written by ch_potf2), and for half sizes sb = 1, 2, 4, ... blocks, every pair of
 //   adjacent groups   [ L11  0  ]^-1   [      W11          0  ]
 //                     [ L21 L22 ]    = [ -W22 (L21 W11)   W22 ]      (ch_level: two block GEMMs, all pairs and tiles in one grid)
 // The dependency chain is 2 (1 + 2 + ... + nb/2) block products instead of nb^2 / 2 for a column-by-column substitution,
 // and every level keeps all SMs busy.  Triangular operands are not multiplied through their zero blocks.
 // ------------------------------------------------------------------------------------------------
-// grid nb, 64 threads: W_kk = L_kk^-1 (forward substitution on the identity, one thread per column)
-__global__ void __launch_bounds__(64) ch_diaginv_kernel(const double* __restrict__ A, int64_t ld, int32_t n, double* __restrict__ W, int64_t ldw) {
-  __shared__ double Lb[CH_NB][CH_NB + 1];
-  const int32_t k0 = blockIdx.x * CH_NB, nk = min(CH_NB, n - k0);
-  for (int e = threadIdx.x; e < nk * nk; e += 64) {
-    const int r = e / nk, c = e % nk;
-    Lb[r][c] = (c <= r) ? A[(int64_t)(k0 + r) * ld + k0 + c] : 0.0;
-  }
-  __syncthreads();
-  const int c = threadIdx.x;
-  if (c >= nk) return;
-  double x[CH_NB];
-#pragma unroll 1
-  for (int r = 0; r < nk; ++r) {
-    double v = (r == c) ? 1.0 : 0.0;
-    for (int t = c; t < r; ++t) v -= Lb[r][t] * x[t];       // x[t] = 0 for t < c
-    x[r] = v / Lb[r][r];
-  }
-  for (int r = c; r < nk; ++r) W[(int64_t)(k0 + r) * ldw + k0 + c] = x[r];
-}
-
 // One level of the recursion, one 64 x 64 output tile per CTA (256 threads, 4 x 4 register tiles), dynamic smem 2 tiles.
 //   mode 1:  T[bi, bj] =   sum_{t in first half, t >= bj} L[bi, t] W[t, bj]       (W11 is lower triangular)
 //   mode 2:  W[bi, bj] = - sum_{t in second half, t <= bi} W[bi, t] T[t, bj]      (W22 is lower triangular)

@@ -1095,16 +1095,18 @@ ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Wm, double*
   if (!attr_set) {
     CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
     CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_level_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
+    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
+    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_potf2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
     attr_set = true;
   }
   CUDA_TRY(cudaMemsetAsync(dflag, 0, 4, st));
   for (int32_t k0 = 0; k0 < n; k0 += ttdft::CH_NB) {
     const int32_t nbk = std::min(ttdft::CH_NB, n - k0);
-    ttdft::ch_potf2_kernel<<<1, 256, 0, st>>>(G, ldg, k0, nbk, dflag);
+    ttdft::ch_potf2_kernel<<<1, 256, 2 * ttdft::CH_TILE_BYTES, st>>>(G, ldg, k0, nbk, dflag, Wm, ldr);
     const int32_t rem = n - k0 - nbk;
     if (rem > 0) {
       const unsigned tiles = (unsigned)((rem + 63) / 64);
-      ttdft::ch_trsm_kernel<<<tiles, 64, 0, st>>>(G, ldg, n, k0, nbk);
+      ttdft::ch_panel_kernel<<<tiles, 256, 2 * ttdft::CH_TILE_BYTES, st>>>(G, ldg, n, k0, nbk, Wm, ldr);
       ttdft::ch_syrk_kernel<<<dim3(tiles, tiles), 256, 2 * ttdft::CH_TILE_BYTES, st>>>(G, ldg, n, k0, nbk);
       g_launches.fetch_add(2);
     }
@@ -1116,8 +1118,6 @@ ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Wm, double*
   if (*hflag) return TTDFT_OK;                      // caller reports the breakdown
   // W = L^-1 by recursive doubling (Rinv's buffer serves as the intermediate T), then Rinv = W^T
   const int32_t nb = (n + ttdft::CH_NB - 1) / ttdft::CH_NB;
-  ttdft::ch_diaginv_kernel<<<(unsigned)nb, 64, 0, st>>>(G, ldg, n, Wm, ldr);
-  g_launches.fetch_add(1);
   for (int32_t sb = 1; sb < nb; sb *= 2) {
     const unsigned pairs = (unsigned)((nb + 2 * sb - 1) / (2 * sb));
     const dim3 grid((unsigned)sb, (unsigned)sb, pairs);
