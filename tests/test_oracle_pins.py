@@ -477,3 +477,83 @@ def test_p9_gram_schmidt_pins():
         assert np.linalg.norm(Q @ R - X) <= 1e-13 * np.linalg.norm(X)
     with pytest.raises(np.linalg.LinAlgError):
         oracle.orthonormalize(np.zeros((4, 2)))
+
+
+# ------------------------------------------------------------------ P10: subdomain recovery for unlabelled, permuted CSR (A0; reading #18)
+def _canonical(labels):
+    """Partition written canonically: every row gets the smallest row index of its group."""
+    labels = np.asarray(labels)
+    first = {}
+    for i, l in enumerate(labels):
+        first.setdefault(int(l), i)
+    return np.array([first[int(l)] for l in labels])
+
+
+def _planted(G, b, z, seed):
+    from oracle.recover import recover_subdomains  # noqa: F401
+    H = synth.hamiltonian_bsr(G, b, z, seed)
+    C = synth.bsr_to_csr_nonzeros(H)
+    perm = synth.permutation(H.M, seed + 50)
+    Cp = synth.permute_csr(C, perm)
+    truth = np.empty(H.M, np.int32)
+    truth[perm] = (np.arange(H.M) // b).astype(np.int32)
+    return H, C, Cp, truth
+
+
+@pytest.mark.parametrize("G,b,z", [(3, 8, 0.0), (3, 32, 0.0), (3, 16, 0.4), (3, 32, 0.4), (4, 8, 0.3)])
+def test_p10_recover_planted_partition(G, b, z):
+    from oracle.recover import recover_subdomains
+    H, C, Cp, truth = _planted(G, b, z, 7100 + b)
+    labels, n = recover_subdomains(Cp.row_ptr, Cp.col_idx)
+    assert n == G ** 3
+    assert np.array_equal(_canonical(labels), _canonical(truth))          # the planted partition, exactly
+    assert np.array_equal(np.bincount(labels), np.full(n, b))
+    # labels are numbered by the smallest row index of the group
+    firsts = [int(np.flatnonzero(labels == k)[0]) for k in range(n)]
+    assert firsts == sorted(firsts)
+    # unpermuted input: the groups are the generator's blocks, numbered in order
+    labels0, n0 = recover_subdomains(C.row_ptr, C.col_idx)
+    assert n0 == G ** 3 and np.array_equal(labels0, np.arange(H.M) // b)
+
+
+def test_p10_recover_closed_forms_and_invariants():
+    from oracle.recover import recover_subdomains
+    # z = 0: rows of a subdomain have identical column sets, so the groups are the classes of equal rows (closed form)
+    H, C, Cp, truth = _planted(3, 8, 0.0, 7200)
+    rows = [tuple(Cp.col_idx[Cp.row_ptr[i]:Cp.row_ptr[i + 1]]) for i in range(Cp.M)]
+    classes = {}
+    for i, r in enumerate(rows):
+        classes.setdefault(r, i)
+    labels, n = recover_subdomains(Cp.row_ptr, Cp.col_idx)
+    assert np.array_equal(_canonical(labels), np.array([classes[r] for r in rows]))
+    # the library step (A A^T) and plain set intersections give the same labels
+    labels_sets, n_sets = recover_subdomains(Cp.row_ptr, Cp.col_idx, counts="sets")
+    assert n_sets == n and np.array_equal(labels_sets, labels)
+    # a diagonal matrix: M singletons, label(i) = i
+    M = 37
+    labels, n = recover_subdomains(np.arange(M + 1, dtype=np.int32), np.arange(M, dtype=np.int32))
+    assert n == M and np.array_equal(labels, np.arange(M))
+    # an empty row and a row without a diagonal entry are singletons / still grouped by pattern
+    rp = np.array([0, 0, 2, 4, 5], np.int32)
+    ci = np.array([2, 3, 1, 3, 3], np.int32)     # rows 1 and 2 point at each other and at 3; row 3 only at itself
+    labels, n = recover_subdomains(rp, ci)
+    assert labels is not None and labels[0] == 0 and n >= 2
+    # two complete cliques of different size joined by nothing: two groups
+    k1, k2 = 5, 9
+    rp = [0]
+    ci = []
+    for i in range(k1 + k2):
+        grp = range(0, k1) if i < k1 else range(k1, k1 + k2)
+        ci += list(grp)
+        rp.append(len(ci))
+    labels, n = recover_subdomains(np.array(rp, np.int32), np.array(ci, np.int32))
+    assert n == 2 and np.array_equal(labels, np.array([0] * k1 + [1] * k2))
+    # G = 2, z = 0: every subdomain neighbours every other, H is fully dense and all rows look alike: "no structure"
+    H, C, Cp, truth = _planted(2, 32, 0.0, 7300)
+    assert recover_subdomains(Cp.row_ptr, Cp.col_idx) == (None, 0)
+    # a candidate set above the cap (one dense 200-clique): reported as "no structure"
+    k = 200
+    rp = np.arange(0, k * k + 1, k, dtype=np.int32)
+    ci = np.tile(np.arange(k, dtype=np.int32), k)
+    labels, n = recover_subdomains(rp, ci)
+    assert labels is None and n == 0
