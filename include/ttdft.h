@@ -273,6 +273,24 @@ ttdft_status ttdft_lanczos_work_bytes(ttdft_h_t h, size_t* bytes);
 ttdft_status ttdft_lanczos_bounds(ttdft_h_t h, int32_t k, const double* v0, void* work, size_t work_bytes, void* stream, double* a0_out,
                                   double* b_out, double* theta_out, int32_t* steps_out);
 
+/*
+ * A0 without labels: recover the subdomain of every row of a CSR from its sparsity pattern (SURVEY.md 8(a) A0 "group rows so each
+ * subdomain's basis functions are contiguous", 8(f)-4 "locality recovery for unhinted CSR").  The paper states the structure that
+ * makes it possible -- functions of a subdomain overlap each other (dense diagonal blocks) and the neighbouring subdomains'
+ * -- but no algorithm; the rule is DESIGN.md reading #18: rows whose column sets have a Jaccard
+ * similarity within 80 % of the row's best match are candidates, a pair is kept if the two candidate sets agree on at least half
+ * of the larger one, groups are the sets reachable along kept pairs, numbered by their smallest row.  Exact integer arithmetic.
+ * desc: a CSR description (DEVICE arrays; values and subdomain_of_row are not read; columns ascending and unique per row).
+ * labels: DEVICE int32[M], written only when *n_groups > 0: the group 0..n_groups-1 of every row -- pass it as subdomain_of_row to
+ * ttdft_h_build, which regroups the rows into tiles if every group has the same size b in {32, 64, 96, 128} and otherwise keeps
+ * the generic format.  n_groups: HOST; 0 means "no recoverable structure" (some row has more than 192 candidates).
+ * Returns TTDFT_ERR_UNSUPPORTED if M bits plus two ints per entry of the longest row exceed 200 KB of shared memory.
+ * The call synchronises `stream`.  `work`: 1024-byte aligned DEVICE scratch of ttdft_recover_subdomains_work_bytes (804 B per row).
+ */
+ttdft_status ttdft_recover_subdomains_work_bytes(int64_t M, size_t* bytes);
+ttdft_status ttdft_recover_subdomains(const ttdft_h_desc* desc, int32_t* labels, void* work, size_t work_bytes, void* stream,
+                                      int32_t* n_groups);
+
 /* Measured fp64 rate of this GPU: kind 0 = scalar DFMA loop, 1 = DMMA (mma.sync m8n8k4.f64) loop;
  * runs for about `millis` ms on `stream`, synchronises, returns TFLOP/s in *tflops. */
 ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, double* tflops);

@@ -23,6 +23,7 @@ exported_symbols = [
     "ttdft_gram_work_bytes", "ttdft_gram", "ttdft_project_work_bytes", "ttdft_project",
     "ttdft_rotate_work_bytes", "ttdft_rotate", "ttdft_orthonormalize_work_bytes", "ttdft_orthonormalize",
     "ttdft_lanczos_work_bytes", "ttdft_lanczos_bounds",
+    "ttdft_recover_subdomains_work_bytes", "ttdft_recover_subdomains",
 ]
 
 
@@ -115,6 +116,10 @@ def _load() -> ctypes.CDLL:
     L.ttdft_lanczos_bounds.restype = st
     L.ttdft_lanczos_bounds.argtypes = [c_void_p, c_int32, c_void_p, c_void_p, c_size_t, c_void_p, POINTER(c_double), POINTER(c_double),
                                        POINTER(c_double), POINTER(c_int32)]
+    L.ttdft_recover_subdomains_work_bytes.restype = st
+    L.ttdft_recover_subdomains_work_bytes.argtypes = [c_int64, POINTER(c_size_t)]
+    L.ttdft_recover_subdomains.restype = st
+    L.ttdft_recover_subdomains.argtypes = [POINTER(_Desc), c_void_p, c_void_p, c_size_t, c_void_p, POINTER(c_int32)]
     L.ttdft_probe_fp64_peak.restype = st
     L.ttdft_probe_fp64_peak.argtypes = [c_int32, c_int32, c_void_p, POINTER(c_double)]
     L.ttdft_timing_enable.restype = st
@@ -258,7 +263,10 @@ def h_build_bsr(M, block, row_ptr, col_idx, values, flags=0, stream=None) -> Ham
     return h_build(FMT_BSR, M, block, row_ptr, col_idx, values.reshape(-1), None, flags, stream)
 
 
-def h_build_csr(M, row_ptr, col_idx, values, subdomain_of_row=None, flags=0, stream=None) -> Hamiltonian:
+def h_build_csr(M, row_ptr, col_idx, values, subdomain_of_row=None, flags=0, stream=None, recover=False) -> Hamiltonian:
+    """CSR build.  recover=True and no labels: ttdft_recover_subdomains first, its labels (if any) go to ttdft_h_build."""
+    if recover and subdomain_of_row is None and M > 0:
+        subdomain_of_row, _ = recover_subdomains(M, row_ptr, col_idx, stream)
     return h_build(FMT_CSR, M, 0, row_ptr, col_idx, values, subdomain_of_row, flags, stream)
 
 
@@ -462,6 +470,21 @@ def lanczos_bounds(H: Hamiltonian, v0, k: int = 30, stream=None):
     steps = c_int32(0)
     _check(_load().ttdft_lanczos_bounds(H.handle, k, v0.data_ptr(), wp, wb, _stream(stream), byref(a0), byref(b), theta, byref(steps)))
     return a0.value, b.value, [theta[i] for i in range(steps.value)]
+
+
+def recover_subdomains(M, row_ptr, col_idx, stream=None):
+    """ttdft_recover_subdomains: (labels int32[M] CUDA tensor, n_groups) from the sparsity pattern of an unlabelled CSR;
+    (None, 0) if the pattern has no recoverable structure.  Pass the labels as subdomain_of_row to h_build_csr."""
+    torch = _torch()
+    d = _desc(FMT_CSR, M, 0, row_ptr, col_idx, None, None, 0)
+    out = c_size_t(0)
+    _check(_load().ttdft_recover_subdomains_work_bytes(M, byref(out)))
+    wp, wb, keep = _aligned_work(int(out.value), None, row_ptr.device)
+    labels = torch.empty(max(M, 1), dtype=torch.int32, device=row_ptr.device)[:M]
+    n = c_int32(0)
+    _check(_load().ttdft_recover_subdomains(byref(d), labels.data_ptr(), wp, wb, _stream(stream), byref(n)))
+    del keep
+    return (labels, n.value) if n.value > 0 else (None, 0)
 
 
 def probe_fp64_peak(kind: int = 1, millis: int = 200, stream=None) -> float:

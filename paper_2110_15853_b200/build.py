@@ -8,7 +8,7 @@ import sys
 PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 SRC = [os.path.join(PKG, "csrc", "ttdft_api.cu")]
-DEPS = [os.path.join(PKG, "csrc", f) for f in ("bsr_dmma.cuh", "bsr_i8.cuh", "i8_digits.cuh", "generic_spmm.cuh")] + [os.path.join(ROOT, "include", "ttdft.h")]
+DEPS = sorted(os.path.join(PKG, "csrc", f) for f in os.listdir(os.path.join(PKG, "csrc")) if f.endswith(".cuh")) + [os.path.join(ROOT, "include", "ttdft.h")]
 OUT = os.path.join(PKG, "libttdft.so")
 
 NVCC_FLAGS = [

@@ -24,6 +24,7 @@
 #include "cholesky.cuh"
 #include "gram_i8.cuh"
 #include "lanczos.cuh"
+#include "recover.cuh"
 
 namespace {
 
@@ -2018,6 +2019,81 @@ ttdft_status ttdft_lanczos_bounds(ttdft_h_t h, int32_t k, const double* v0, void
     for (int j = 0; j < kk; ++j) theta_out[j] = th[(size_t)j];
   }
   if (steps_out) *steps_out = kk;
+  return TTDFT_OK;
+}
+
+// ---- A0 without labels: recover the subdomain of every row of a CSR from its sparsity pattern (recover.cuh) ----
+static size_t rc_region(size_t n_ints) { return align_up(n_ints * 4, 1024); }
+
+ttdft_status ttdft_recover_subdomains_work_bytes(int64_t M, size_t* bytes) {
+  if (!bytes) return fail(TTDFT_ERR_INVALID_ARG, "bytes is NULL");
+  if (M < 0) return fail(TTDFT_ERR_INVALID_ARG, "M < 0");
+  // S | nS | Vm | L | ids | flags
+  *bytes = rc_region((size_t)M * ttdft::RC_CAP) + rc_region((size_t)M) + rc_region((size_t)M * ttdft::RC_MASKW) + 2 * rc_region((size_t)M) + 1024;
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_recover_subdomains(const ttdft_h_desc* d, int32_t* labels, void* work, size_t work_bytes, void* stream, int32_t* n_groups) {
+  if (!d || !labels || !n_groups) return fail(TTDFT_ERR_INVALID_ARG, "NULL argument");
+  *n_groups = 0;
+  if (d->fmt != TTDFT_FMT_CSR) return fail(TTDFT_ERR_INVALID_ARG, "recover_subdomains takes a CSR description");
+  const int64_t M = d->M;
+  if (M < 0) return fail(TTDFT_ERR_INVALID_ARG, "M < 0");
+  if (M >= 0x7fffffffLL) return fail(TTDFT_ERR_UNSUPPORTED, "M must fit int32");
+  if (M == 0) return TTDFT_OK;
+  if (!d->row_ptr) return fail(TTDFT_ERR_INVALID_ARG, "row_ptr is NULL");
+  int32_t last = 0;
+  CUDA_TRY(cudaMemcpy(&last, d->row_ptr + M, 4, cudaMemcpyDeviceToHost));
+  if (last < 0 || (last > 0 && !d->col_idx)) return fail(TTDFT_ERR_INVALID_ARG, "row_ptr[M] < 0 or col_idx is NULL");
+  size_t need;
+  ttdft_recover_subdomains_work_bytes(M, &need);
+  if (work_bytes < need) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, need);
+  if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
+  cudaStream_t st = (cudaStream_t)stream;
+  uint8_t* q = reinterpret_cast<uint8_t*>(work);
+  int32_t* S = reinterpret_cast<int32_t*>(q);      q += rc_region((size_t)M * ttdft::RC_CAP);
+  int32_t* nS = reinterpret_cast<int32_t*>(q);     q += rc_region((size_t)M);
+  uint32_t* Vm = reinterpret_cast<uint32_t*>(q);   q += rc_region((size_t)M * ttdft::RC_MASKW);
+  int32_t* L = reinterpret_cast<int32_t*>(q);      q += rc_region((size_t)M);
+  int32_t* ids = reinterpret_cast<int32_t*>(q);    q += rc_region((size_t)M);
+  int32_t* flags = reinterpret_cast<int32_t*>(q);  // [0] longest row, [1] overflow, [2] changed, [3] number of roots
+  int32_t hf[4] = {0, 0, 0, 0};
+  CUDA_TRY(cudaMemsetAsync(flags, 0, 16, st));
+  ttdft::rc_maxlen_kernel<<<(unsigned)((M + 255) / 256), 256, 0, st>>>(M, d->row_ptr, flags);
+  g_launches.fetch_add(1);
+  CUDA_TRY(cudaMemcpyAsync(hf, flags, 16, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  const int32_t maxlen = std::max(hf[0], 1);
+  const int32_t W = (int32_t)((M + 31) / 32);
+  const size_t smem1 = ((size_t)W + 2 * (size_t)maxlen) * 4, smem2 = (size_t)W * 4;
+  if (smem1 > 200 * 1024) return fail(TTDFT_ERR_UNSUPPORTED, "recover_subdomains: M = %lld with rows of up to %d entries needs %zu bytes of shared memory",
+                                      (long long)M, maxlen, smem1);
+  CUDA_TRY(cudaFuncSetAttribute(ttdft::rc_candidates_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
+  CUDA_TRY(cudaFuncSetAttribute(ttdft::rc_verify_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+  ttdft::rc_candidates_kernel<<<(unsigned)M, ttdft::RC_T1, smem1, st>>>(M, d->row_ptr, d->col_idx, W, maxlen, S, nS, flags);
+  CUDA_TRY(cudaGetLastError());
+  g_launches.fetch_add(1);
+  CUDA_TRY(cudaMemcpyAsync(hf, flags, 16, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (hf[1]) return TTDFT_OK;                       // a candidate set above RC_CAP: no recoverable structure, *n_groups = 0
+  ttdft::rc_verify_kernel<<<(unsigned)M, ttdft::RC_T2, smem2, st>>>(M, W, S, nS, Vm, L);
+  CUDA_TRY(cudaGetLastError());
+  g_launches.fetch_add(1);
+  for (int it = 0; it < 64; ++it) {
+    CUDA_TRY(cudaMemsetAsync(flags + 2, 0, 4, st));
+    ttdft::rc_propagate_kernel<<<(unsigned)((M * 32 + 255) / 256), 256, 0, st>>>(M, S, nS, Vm, L, flags);
+    g_launches.fetch_add(1);
+    CUDA_TRY(cudaMemcpyAsync(hf, flags, 16, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (!hf[2]) break;
+    if (it == 63) return fail(TTDFT_ERR_CUDA, "recover_subdomains: label propagation did not converge");
+  }
+  ttdft::rc_number_roots_kernel<<<1, 1024, 0, st>>>(M, L, ids, flags);
+  ttdft::rc_label_kernel<<<(unsigned)((M + 255) / 256), 256, 0, st>>>(M, L, ids, labels);
+  g_launches.fetch_add(2);
+  CUDA_TRY(cudaMemcpyAsync(hf, flags, 16, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  *n_groups = hf[3];
   return TTDFT_OK;
 }
 

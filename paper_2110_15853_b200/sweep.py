@@ -2,7 +2,8 @@
 (ttdft_cheb_step) on config 3's H at N in {16, 64, 256, 1024, 4096}, in two layouts --
 subdomain-ordered BSR and CSR with rows/columns symmetrically permuted by seed (irregular-access
 stress; once as given -> generic kernel, once with the subdomain index of every row -> h_build regroups the rows
-into tiles and the *_ws calls gather / scatter around the tile kernel) -- each reported against the binding roofline:
+into tiles and the *_ws calls gather / scatter around the tile kernel; `csr+recovered`: no labels given, the library recovers
+them from the sparsity pattern first) -- each reported against the binding roofline:
     T_roof = max(alg_bytes / BW_hbm, useful_flops / P_fp64).
 The BSR layout runs three times: fp64 tensor-core MMA (kernel 1) and int8 digit planes (kernel 3 with 7 and 6 planes, through
 the *_ws entry points; its time includes the digit extraction of X); roofline_frac > 1 there means
@@ -57,7 +58,7 @@ def time_launches(fn, reps, flush):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--workload", default="si")
-    ap.add_argument("--layouts", default="bsr,csr,csr+labels")
+    ap.add_argument("--layouts", default="bsr,csr,csr+labels,csr+recovered")
     ap.add_argument("--ns", default="16,64,256,1024,4096")
     ap.add_argument("--reps", type=int, default=10)
     ap.add_argument("--csr-max-n", type=int, default=4096)
@@ -92,6 +93,30 @@ def main():
             labels[perm] = (np.arange(Cp.M) // cfg.b).astype(np.int32)
             handles["csr+labels-i8x7"] = tt.h_build_csr(Cp.M, rp_d, ci_d, va_d, subdomain_of_row=torch.from_numpy(labels).to(dev))
             assert handles["csr+labels-i8x7"].info()["reordered"] == 1
+        if "csr+recovered" in args.layouts:
+            # the same permuted CSR WITHOUT labels: ttdft_recover_subdomains finds the subdomains from the sparsity pattern
+            # (reading #18), then the labelled build as above
+            import time
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            rec, n_groups = tt.recover_subdomains(Cp.M, rp_d, ci_d)
+            torch.cuda.synchronize()
+            t1 = time.perf_counter()
+            assert n_groups == cfg.M // cfg.b, n_groups
+            handles["csr+recovered-i8x7"] = tt.h_build_csr(Cp.M, rp_d, ci_d, va_d, subdomain_of_row=rec)
+            torch.cuda.synchronize()
+            t2 = time.perf_counter()
+            inf = handles["csr+recovered-i8x7"].info()
+            assert inf["reordered"] == 1 and inf["block"] == cfg.b
+            truth = np.empty(Cp.M, np.int32)
+            truth[perm] = (np.arange(Cp.M) // cfg.b).astype(np.int32)
+            got = rec.cpu().numpy()
+            first = np.full(n_groups, Cp.M, np.int64)
+            np.minimum.at(first, truth, np.arange(Cp.M))
+            same = bool(np.array_equal(np.argsort(np.argsort(first))[truth], got))   # planted groups numbered by their smallest row
+            print(json.dumps({"recover_subdomains_s": t1 - t0, "labelled_build_s": t2 - t1, "n_groups": n_groups,
+                              "equals_planted_partition": same, "nblocks": inf["nblocks"]}), flush=True)
+            assert same
         del Cp, rp_d, ci_d, va_d
     maths = args.math.split(",")
     if "bsr" in handles and handles["bsr"].info()["i8_planes"]:
@@ -115,7 +140,8 @@ def main():
             work = None
             if layout != "csr":
                 Hd.set_math_mode({"bsr": tt.MATH_FP64, "bsr-i8": tt.MATH_I8, "bsr-i8x7": tt.MATH_I8X7,
-                                  "csr+labels-i8x7": tt.MATH_I8X7}[layout])
+                                  "csr+labels-i8x7": tt.MATH_I8X7,
+                                  "csr+recovered-i8x7": tt.MATH_I8X7}[layout])
             if i8:
                 work = torch.empty(tt.step_work_bytes(Hd, N) + 16, dtype=torch.uint8, device=dev)
             for op in ("spmm", "step"):
