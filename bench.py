@@ -186,7 +186,7 @@ def main():
     ap.add_argument("--workload", default="si", choices=list(synth.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--panel", type=int, default=0, help="column-panel width (0 = config default)")
-    ap.add_argument("--ref-cols", type=int, default=16, help="columns in the oracle sample")
+    ap.add_argument("--ref-cols", type=int, default=48, help="columns in the oracle sample (48 columns = about 18 s on 16 host cores)")
     ap.add_argument("--math", default="auto", choices=["auto", "fp64", "i8", "i8x7"],
                     help="arithmetic of the block product: fp64 DMMA; exact int8 digit planes on the tcgen05 tensor "
                          "cores with 7 planes (55 bits, i8x7) or 6 planes (47 bits, i8); auto = i8x7 for tiles >= 64")
