@@ -266,7 +266,11 @@ def h_build_bsr(M, block, row_ptr, col_idx, values, flags=0, stream=None) -> Ham
 def h_build_csr(M, row_ptr, col_idx, values, subdomain_of_row=None, flags=0, stream=None, recover=False) -> Hamiltonian:
     """CSR build.  recover=True and no labels: ttdft_recover_subdomains first, its labels (if any) go to ttdft_h_build."""
     if recover and subdomain_of_row is None and M > 0:
-        subdomain_of_row, _ = recover_subdomains(M, row_ptr, col_idx, stream)
+        try:
+            subdomain_of_row, _ = recover_subdomains(M, row_ptr, col_idx, stream)
+        except TTDFTError as e:
+            if e.status_name != "UNSUPPORTED":      # pattern too large for the shared-memory column map: build without labels
+                raise
     return h_build(FMT_CSR, M, 0, row_ptr, col_idx, values, subdomain_of_row, flags, stream)
 
 
