@@ -110,3 +110,37 @@ def test_unlabelled_permuted_csr_runs_tile_kernels_after_recovery(tt, G, b, z):
     tt.cheb_filter(Hd, dev(X), Y, m, a, bq, a0q)
     got = Y.cpu().numpy()
     assert relerr(got, ref) <= 1e-10 and worst_col_relerr(got, ref) <= 1e-9
+
+
+def test_full_config3_unlabelled_permuted_csr(tt):
+    """BASELINE.json config 5 layout (ii) at full size: config 3's H as a symmetrically permuted CSR without labels.  The recovered
+    groups are the generator's 1,728 subdomains exactly (integer work: bit-exact), the handle built from them has exactly the
+    generator's tiles, and a product in the caller's row order matches the oracle on the permuted CSR."""
+    import torch
+    cfg = synth.CONFIGS["si"]
+    H = synth.hamiltonian_bsr(cfg.G, cfg.b, cfg.z, cfg.seed)
+    nblocks = H.nblocks
+    C = synth.bsr_to_csr_nonzeros(H)
+    del H
+    perm = synth.permutation(cfg.M, cfg.seed + 50)
+    Cp = synth.permute_csr(C, perm)
+    del C
+    rp, ci, va = dev(Cp.row_ptr), dev(Cp.col_idx), dev(Cp.values)
+    labels, n = tt.recover_subdomains(cfg.M, rp, ci)
+    assert n == cfg.M // cfg.b
+    truth = np.empty(cfg.M, np.int32)
+    truth[perm] = (np.arange(cfg.M) // cfg.b).astype(np.int32)
+    first = np.full(n, cfg.M, np.int64)
+    np.minimum.at(first, truth, np.arange(cfg.M))
+    assert np.array_equal(np.argsort(np.argsort(first))[truth], labels.cpu().numpy())   # planted groups numbered by smallest row
+    Hd = tt.h_build_csr(cfg.M, rp, ci, va, subdomain_of_row=labels)
+    info = Hd.info()
+    assert info["kernel"] == 1 and info["block"] == cfg.b and info["reordered"] == 1 and info["nblocks"] == nblocks
+    del rp, ci, va
+    N = 24
+    X = synth.dense_normal(cfg.M, N, 8400)
+    ref = oracle.spmm(Cp.row_ptr, Cp.col_idx, Cp.values, 1.0, X)
+    Y = torch.empty((cfg.M, N), dtype=torch.float64, device="cuda")
+    tt.spmm(Hd, 1.0, dev(X), 0.0, Y, use_work=True)
+    got = Y.cpu().numpy()
+    assert relerr(got, ref) <= 1e-12 and worst_col_relerr(got, ref) <= 1e-11
