@@ -81,6 +81,12 @@ ttdft_status fail(ttdft_status st, const char* fmt, ...) {
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// Function attributes (the dynamic shared-memory limit) are per device: one bit per device ordinal says whether they have been set
+// there.  The bit is set AFTER the attributes, so a second thread either sets them again (idempotent) or finds them set.
+inline uint64_t attr_bit() { int dev = 0; cudaGetDevice(&dev); return 1ull << (dev & 63); }
+inline bool attr_done(const std::atomic<uint64_t>& seen) { return (seen.load(std::memory_order_acquire) & attr_bit()) != 0; }
+inline void attr_mark(std::atomic<uint64_t>& seen) { seen.fetch_or(attr_bit(), std::memory_order_release); }
+
 // ------------------------------------------------------------------------------------------------
 // driver entry point for tensor-map encoding (no link-time dependency on libcuda)
 // ------------------------------------------------------------------------------------------------
@@ -471,10 +477,10 @@ template <int WR, int Q, int CPS, int RS>
 ttdft_status launch_k1(const ttdft_h_s* h, const CUtensorMap& tmH, double alpha, double gamma, double beta, const double* X,
                        int64_t ldx, const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, cudaStream_t st) {
   using SM = ttdft::K1Cfg<WR, Q, CPS, RS>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static std::atomic<uint64_t> attr_seen{0};
+  if (!attr_done(attr_seen)) {
     CUDA_TRY(cudaFuncSetAttribute(ttdft::bsr_dmma_kernel<WR, Q, CPS, RS>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::TOTAL));
-    attr_set = true;
+    attr_mark(attr_seen);
   }
   CUtensorMap tmX;
   ttdft_status s = make_map_2d(&tmX, X, (uint64_t)ncols, (uint64_t)h->M, (uint64_t)ldx, ttdft::K1_KS);
@@ -640,10 +646,10 @@ ttdft_status launch_k3(ttdft_h_s* h, const CUtensorMap& tmYd, ttdft::K3Params p,
                        cudaStream_t st) {
   constexpr int ci = C == 1 ? 0 : C == 2 ? 1 : C == 4 ? 2 : 3;
   auto kern = ttdft::bsr_i8_kernel<S, C>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static std::atomic<uint64_t> attr_seen{0};
+  if (!attr_done(attr_seen)) {
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ttdft::K3Cfg<S>::TOTAL));
-    attr_set = true;
+    attr_mark(attr_seen);
   }
   const int maxc = k3_max_clusters<S, C>(h);
   p.ct_begin = ct_begin;
@@ -695,11 +701,11 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
     g_launches.fetch_add(1);
   }
   {
-    static bool attr_set = false;
+    static std::atomic<uint64_t> attr_seen{0};
     const int smem = S * 64 * 33 * 4;
-    if (!attr_set) {
+    if (!attr_done(attr_seen)) {
       CUDA_TRY(cudaFuncSetAttribute(ttdft::y_digits_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-      attr_set = true;
+      attr_mark(attr_seen);
     }
     dim3 g((unsigned)h->nb, nct);
     TimedLaunch tl(4, st);
@@ -887,10 +893,10 @@ ttdft_status launch_k4(const GramPlan& g, const CUtensorMap& tmXd, const CUtenso
                        int32_t ntiles, cudaStream_t st) {
   constexpr int S = GRAM_S;
   auto kern = ttdft::gram_i8_kernel<S, C>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static std::atomic<uint64_t> attr_seen{0};
+  if (!attr_done(attr_seen)) {
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, ttdft::K3Cfg<S>::TOTAL));
-    attr_set = true;
+    attr_mark(attr_seen);
   }
   p.ctw_begin = ctw_begin;
   p.nctwg = ntiles / C;
@@ -928,11 +934,11 @@ ttdft_status gram_run(const GramPlan& g, const double* X, int64_t ldx, const dou
     { TimedLaunch tl(5, st); ttdft::colmax_kernel<<<gc, 256, 0, st>>>(W, ldw, g.M, g.ncols, cmW); }
     CUDA_TRY(cudaGetLastError());
     g_launches.fetch_add(2);
-    static bool attr_set = false;
+    static std::atomic<uint64_t> attr_seen{0};
     const int smem = S * 64 * 33 * 4;
-    if (!attr_set) {
+    if (!attr_done(attr_seen)) {
       CUDA_TRY(cudaFuncSetAttribute(ttdft::y_digits_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-      attr_set = true;
+      attr_mark(attr_seen);
     }
     { TimedLaunch tl(4, st);
       ttdft::y_digits_kernel<S><<<dim3((unsigned)g.nbk, (unsigned)g.nctX), 256, smem, st>>>(X, ldx, 128, g.M, g.ncols, cmX, DX, nullptr); }
@@ -1025,11 +1031,11 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
   CUDA_TRY(cudaMemsetAsync(cmQ, 0, r.cm, st));
   ttdft::colmax_kernel<<<dim3((unsigned)r.nct, (unsigned)((r.K + 2047) / 2048)), 256, 0, st>>>(Q, ldq, r.K, r.N, cmQ);
   {
-    static bool attr_set = false;
+    static std::atomic<uint64_t> attr_seen{0};
     const int smem = S * 64 * 33 * 4;
-    if (!attr_set) {
+    if (!attr_done(attr_seen)) {
       CUDA_TRY(cudaFuncSetAttribute(ttdft::y_digits_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-      attr_set = true;
+      attr_mark(attr_seen);
     }
     ttdft::y_digits_kernel<S><<<dim3((unsigned)r.nkb, (unsigned)r.nct), 256, smem, st>>>(Q, ldq, 128, r.K, r.N, cmQ, DQ, nullptr);
   }
@@ -1092,13 +1098,13 @@ ttdft_status orth_plan(int64_t M, int64_t n, int32_t passes, OrthPlan* o) {
 // Returns the breakdown flag through *hflag (synchronises st).
 ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Wm, double* Rinv, int64_t ldr, int32_t* dflag, int32_t* hflag,
                           cudaStream_t st) {
-  static bool attr_set = false;
-  if (!attr_set) {
+  static std::atomic<uint64_t> attr_seen{0};
+  if (!attr_done(attr_seen)) {
     CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
     CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_level_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
     CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
     CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_potf2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
-    attr_set = true;
+    attr_mark(attr_seen);
   }
   CUDA_TRY(cudaMemsetAsync(dflag, 0, 4, st));
   for (int32_t k0 = 0; k0 < n; k0 += ttdft::CH_NB) {
