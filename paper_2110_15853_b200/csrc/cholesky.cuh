@@ -51,13 +51,19 @@ __global__ void __launch_bounds__(256) ch_potf2_kernel(double* __restrict__ A, i
     const int r = e / nbk, c = e % nbk;
     if (c <= r) A[(int64_t)(k0 + r) * ld + k0 + c] = s[r][c];
   }
-  // W_kk = L_kk^-1: forward substitution on the identity, one thread per column, then stored
-  if (tid < nbk) {
-    const int c = tid;
-    for (int r = c; r < nbk; ++r) {
-      double v = (r == c) ? 1.0 : 0.0;
-      for (int t = c; t < r; ++t) v -= s[r][t] * w[t][c];
-      w[r][c] = v / s[r][r];
+  // W_kk = L_kk^-1: forward substitution on the identity, four threads per column (partial sums over t = q mod 4, combined by
+  // two shuffles; the four threads of a column sit in one warp, so a warp barrier orders the row just written), then stored
+  {
+    const int c = tid >> 2, q = tid & 3;                     // 256 threads = 64 columns x 4
+    for (int r = 0; r < nbk; ++r) {
+      const bool on = (c < nbk && r >= c);
+      double v = 0.0;
+      if (on)
+        for (int t = c + q; t < r; t += 4) v -= s[r][t] * w[t][c];
+      v += __shfl_xor_sync(0xffffffffu, v, 1);               // all lanes take part, whatever their column
+      v += __shfl_xor_sync(0xffffffffu, v, 2);
+      if (on && q == 0) w[r][c] = (v + ((r == c) ? 1.0 : 0.0)) / s[r][r];
+      __syncwarp();
     }
   }
   __syncthreads();
