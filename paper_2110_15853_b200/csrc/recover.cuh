@@ -49,21 +49,21 @@ __global__ void __launch_bounds__(RC_T1) rc_candidates_kernel(int64_t M, const i
   __syncthreads();
   for (int t = tid; t < len; t += RC_T1) {
     const int32_t k = col[s + t];
-    atomicOr(&bm[k >> 5], 1u << (k & 31));
+    if ((uint32_t)k < (uint32_t)M) atomicOr(&bm[k >> 5], 1u << (k & 31));      // an out-of-range column (invalid input) is ignored, not a fault
   }
   __syncthreads();
   // one warp per neighbour j: c = number of columns of row j that are columns of row i
   for (int t = warp; t < len; t += RC_T1 / 32) {
     const int32_t j = col[s + t];
-    const int32_t sj = rp[j], lj = rp[j + 1] - sj;
+    const bool valid = (uint32_t)j < (uint32_t)M && j != i;
+    const int32_t sj = valid ? rp[j] : 0, lj = valid ? rp[j + 1] - sj : 0;
     int32_t c = 0;
-    if (j != i)
-      for (int q = lane; q < lj; q += 32) {
-        const int32_t k = __ldg(col + sj + q);
-        c += (bm[k >> 5] >> (k & 31)) & 1u;
-      }
+    for (int q = lane; q < lj; q += 32) {
+      const int32_t k = __ldg(col + sj + q);
+      if ((uint32_t)k < (uint32_t)M) c += (bm[k >> 5] >> (k & 31)) & 1u;
+    }
     for (int o = 16; o; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
-    if (lane == 0) { cc[t] = (j != i) ? c : -1; uu[t] = len + lj - c; }
+    if (lane == 0) { cc[t] = valid ? c : -1; uu[t] = len + lj - c; }
   }
   __syncthreads();
   // largest fraction of the row
