@@ -186,7 +186,9 @@ def main():
     ap.add_argument("--workload", default="si", choices=list(synth.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--panel", type=int, default=0, help="column-panel width (0 = config default)")
-    ap.add_argument("--ref-cols", type=int, default=48, help="columns in the oracle sample (48 columns = about 18 s on 16 host cores)")
+    ap.add_argument("--ref-cols", type=int, default=0,
+                    help="columns in the oracle sample; 0 = 48 for the cpu_baseline leg (about 18 s on 16 host cores) and 16 per step "
+                         "for --impl reference (about 6 s per step, so that any --steps/--warmup ends within a few minutes)")
     ap.add_argument("--math", default="auto", choices=["auto", "fp64", "i8", "i8x7"],
                     help="arithmetic of the block product: fp64 DMMA; exact int8 digit planes on the tcgen05 tensor "
                          "cores with 7 planes (55 bits, i8x7) or 6 planes (47 bits, i8); auto = i8x7 for tiles >= 64")
@@ -195,6 +197,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-project", action="store_true", help="skip the subspace-projection (NEXT-1) measurement")
     args = ap.parse_args()
+    if args.ref_cols <= 0:
+        args.ref_cols = 16 if args.impl == "reference" else 48
     if args.impl == "reference":
         return run_reference(args)
 
