@@ -54,6 +54,8 @@ struct K3Params {
   uint32_t* cmaxO;                 // out: column maxima of O, or NULL
   int64_t mrows;                   // valid rows (= nb*b for a Hamiltonian; < nb*b for the ragged last block of ttdft_rotate)
   int32_t l2hints;                 // 1: evict-first H planes, evict-last Y digit tiles; 2: only the latter; 0: none
+  int32_t jlimit = 0;              // > 0: only the first jlimit tiles of every block row are multiplied (ttdft_rotate with an
+                                   // upper-triangular right factor: the k-tiles below the launch's column range are zero)
   unsigned long long* trace;       // debug (ttdft_debug_k3_trace): 8 clock64 stamps per work item of CTA 0, or NULL
 };
 
@@ -296,7 +298,8 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         int32_t I, ctg;
         k3_decode(prm, u, I, ctg);
         const int32_t ct = prm.ct_begin + ctg * C + crank;
-        const int32_t p0 = prm.brow_ptr[I], p1 = prm.brow_ptr[I + 1];
+        const int32_t p0 = prm.brow_ptr[I];
+        const int32_t p1 = prm.jlimit > 0 ? min(prm.brow_ptr[I + 1], p0 + prm.jlimit) : prm.brow_ptr[I + 1];
         for (int32_t p = p0; p < p1; ++p) {
           const int32_t J = prm.bcol[p];
           mbar_wait(&yempty[yb], yph ^ 1);
@@ -334,7 +337,8 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       for (int64_t u = cluster0; u < nitems; u += nclusters) {
         int32_t I, ctg;
         k3_decode(prm, u, I, ctg);
-        const int32_t nJ = prm.brow_ptr[I + 1] - prm.brow_ptr[I];
+        int32_t nJ = prm.brow_ptr[I + 1] - prm.brow_ptr[I];
+        if (prm.jlimit > 0) nJ = min(nJ, prm.jlimit);
         if (nJ == 0) continue;
         const int64_t it = (u - cluster0) / nclusters;
         const bool tr = prm.trace && blockIdx.x == 0 && it < 512;

@@ -1010,8 +1010,10 @@ ttdft_status rotate_plan(int64_t M, int64_t K, int64_t N, RotatePlan* r) {
   return TTDFT_OK;
 }
 
+// upper_tri: Q is upper triangular (the R^-1 of a Cholesky-QR): column tile ct then needs only the k-tiles J <= ceil((ct + 1) / 2) - 1,
+// so the column tiles are launched in groups of 8, each with its own tile limit (K3Params::jlimit): 56 % of the full product's work.
 ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const double* Q, int64_t ldq, double* Y, int64_t ldy, void* work,
-                        cudaStream_t st) {
+                        cudaStream_t st, bool upper_tri = false) {
   constexpr int S = GRAM_S;
   if (r.M == 0) return TTDFT_OK;
   uint8_t* wb = reinterpret_cast<uint8_t*>(work);
@@ -1060,12 +1062,22 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
   p.S = nullptr; p.lds = 0; p.Z = Y; p.ldz = ldy; p.O = Y; p.ldo = ldy;
   p.eH = eX; p.hdiag = nullptr; p.cmaxS = cmQ; p.cmaxO = nullptr;
   p.vec = 0; p.trace = nullptr; p.l2hints = env_int("TTDFT_K3_L2HINTS", 1); p.mrows = r.M;
-  const int C = (r.nct >= 2) ? 2 : 1;
-  const int32_t main_tiles = r.nct / C * C;
-  if (C == 2) s = launch_k3<S, 2>(&hx, tmQd, p, 0, main_tiles, st);
-  else s = launch_k3<S, 1>(&hx, tmQd, p, 0, main_tiles, st);
-  if (s != TTDFT_OK) return s;
-  if (main_tiles < r.nct) return launch_k3<S, 1>(&hx, tmQd, p, main_tiles, r.nct - main_tiles, st);
+  auto launch_range = [&](int32_t c0, int32_t n, int32_t jlimit) -> ttdft_status {
+    p.jlimit = jlimit;
+    const int C = (n >= 2) ? 2 : 1;
+    const int32_t main_tiles = n / C * C;
+    ttdft_status q = (C == 2) ? launch_k3<S, 2>(&hx, tmQd, p, c0, main_tiles, st) : launch_k3<S, 1>(&hx, tmQd, p, c0, main_tiles, st);
+    if (q != TTDFT_OK) return q;
+    if (main_tiles < n) return launch_k3<S, 1>(&hx, tmQd, p, c0 + main_tiles, n - main_tiles, st);
+    return TTDFT_OK;
+  };
+  if (!upper_tri || r.nct < 16 || !env_int("TTDFT_ROTATE_TRI", 1)) return launch_range(0, r.nct, 0);
+  const int32_t gsz = 8;
+  for (int32_t c0 = 0; c0 < r.nct; c0 += gsz) {
+    const int32_t n = std::min(gsz, r.nct - c0);
+    const int32_t jl = std::min<int32_t>(r.nkb, (c0 + n + 1) / 2);       // k-tiles of 128 rows that reach column 64 (c0 + n) - 1
+    if ((s = launch_range(c0, n, jl)) != TTDFT_OK) return s;
+  }
   return TTDFT_OK;
 }
 
@@ -1161,7 +1173,7 @@ ttdft_status orth_run(const OrthPlan& o, const double* X, int64_t ldx, double* Y
     if (hflag)
       return fail(TTDFT_ERR_BREAKDOWN, "orthonormalize: X^T X is not positive definite in pass %d (pivot %d): columns are linearly "
                                        "dependent to working precision", p + 1, hflag - 1);
-    if ((s = rotate_run(o.r, src, lds, Rinv, ldn, dst, ldd, inner, st)) != TTDFT_OK) return s;   // dst = src R^-1
+    if ((s = rotate_run(o.r, src, lds, Rinv, ldn, dst, ldd, inner, st, true)) != TTDFT_OK) return s;   // dst = src R^-1, R^-1 upper triangular
     src = dst;
     lds = ldd;
   }
