@@ -54,8 +54,9 @@ struct K3Params {
   uint32_t* cmaxO;                 // out: column maxima of O, or NULL
   int64_t mrows;                   // valid rows (= nb*b for a Hamiltonian; < nb*b for the ragged last block of ttdft_rotate)
   int32_t l2hints;                 // 1: evict-first H planes, evict-last Y digit tiles; 2: only the latter; 0: none
-  int32_t jlimit = 0;              // > 0: only the first jlimit tiles of every block row are multiplied (ttdft_rotate with an
-                                   // upper-triangular right factor: the k-tiles below the launch's column range are zero)
+  int32_t jlimit = 0;              // > 0: only the first jlimit tiles of every block row are multiplied; < 0: the right factor is
+                                   // upper triangular (the R^-1 of ttdft_orthonormalize's rotation; tiles = 128 rows of it in order):
+                                   // a cluster whose last column tile is ct multiplies the first ceil((ct + 1) / 2) tiles only
   unsigned long long* trace;       // debug (ttdft_debug_k3_trace): 8 clock64 stamps per work item of CTA 0, or NULL
 };
 
@@ -238,6 +239,14 @@ __device__ __forceinline__ void k3_decode(const K3Params& prm, int64_t u, int32_
   ctg = g * prm.cgc + (int32_t)(rem % width);
 }
 
+// tiles of a block row that the cluster of tile group ctg multiplies (K3Params::jlimit)
+template <int C>
+__device__ __forceinline__ int32_t k3_jlimit(const K3Params& prm, int32_t ctg) {
+  if (prm.jlimit == 0) return 0x7fffffff;
+  if (prm.jlimit > 0) return prm.jlimit;
+  return (prm.ct_begin + ctg * C + C + 1) / 2;      // ceil((ct_last + 1) / 2), ct_last = ct_begin + ctg * C + C - 1
+}
+
 // tmHd: box (b/C rows) x 128 B of the H digit planes; tmYd: box S x 64 x 128 B of the Y digit tiles.
 // Launched with cluster dimension C (C == 1: a plain launch).  gridDim.x is a multiple of C.
 template <int S, int C>
@@ -299,7 +308,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         k3_decode(prm, u, I, ctg);
         const int32_t ct = prm.ct_begin + ctg * C + crank;
         const int32_t p0 = prm.brow_ptr[I];
-        const int32_t p1 = prm.jlimit > 0 ? min(prm.brow_ptr[I + 1], p0 + prm.jlimit) : prm.brow_ptr[I + 1];
+        const int32_t p1 = p0 + min(prm.brow_ptr[I + 1] - p0, k3_jlimit<C>(prm, ctg));
         for (int32_t p = p0; p < p1; ++p) {
           const int32_t J = prm.bcol[p];
           mbar_wait(&yempty[yb], yph ^ 1);
@@ -337,8 +346,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       for (int64_t u = cluster0; u < nitems; u += nclusters) {
         int32_t I, ctg;
         k3_decode(prm, u, I, ctg);
-        int32_t nJ = prm.brow_ptr[I + 1] - prm.brow_ptr[I];
-        if (prm.jlimit > 0) nJ = min(nJ, prm.jlimit);
+        const int32_t nJ = min(prm.brow_ptr[I + 1] - prm.brow_ptr[I], k3_jlimit<C>(prm, ctg));
         if (nJ == 0) continue;
         const int64_t it = (u - cluster0) / nclusters;
         const bool tr = prm.trace && blockIdx.x == 0 && it < 512;

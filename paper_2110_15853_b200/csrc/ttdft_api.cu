@@ -1010,8 +1010,8 @@ ttdft_status rotate_plan(int64_t M, int64_t K, int64_t N, RotatePlan* r) {
   return TTDFT_OK;
 }
 
-// upper_tri: Q is upper triangular (the R^-1 of a Cholesky-QR): column tile ct then needs only the k-tiles J <= ceil((ct + 1) / 2) - 1,
-// so the column tiles are launched in groups of 8, each with its own tile limit (K3Params::jlimit): 56 % of the full product's work.
+// upper_tri: Q is upper triangular (the R^-1 of a Cholesky-QR): column tile ct then needs only the k-tiles J <= ceil((ct + 1) / 2) - 1;
+// K3 stops every work item's tile loop there (K3Params::jlimit = -1): about half of the full product's work.
 ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const double* Q, int64_t ldq, double* Y, int64_t ldy, void* work,
                         cudaStream_t st, bool upper_tri = false) {
   constexpr int S = GRAM_S;
@@ -1071,14 +1071,7 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
     if (main_tiles < n) return launch_k3<S, 1>(&hx, tmQd, p, c0 + main_tiles, n - main_tiles, st);
     return TTDFT_OK;
   };
-  if (!upper_tri || r.nct < 16 || !env_int("TTDFT_ROTATE_TRI", 1)) return launch_range(0, r.nct, 0);
-  const int32_t gsz = 8;
-  for (int32_t c0 = 0; c0 < r.nct; c0 += gsz) {
-    const int32_t n = std::min(gsz, r.nct - c0);
-    const int32_t jl = std::min<int32_t>(r.nkb, (c0 + n + 1) / 2);       // k-tiles of 128 rows that reach column 64 (c0 + n) - 1
-    if ((s = launch_range(c0, n, jl)) != TTDFT_OK) return s;
-  }
-  return TTDFT_OK;
+  return launch_range(0, r.nct, (upper_tri && env_int("TTDFT_ROTATE_TRI", 1)) ? -1 : 0);
 }
 
 // ------------------------------------------------------------------------------------------------
