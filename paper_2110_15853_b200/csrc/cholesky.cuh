@@ -24,33 +24,33 @@ __global__ void __launch_bounds__(256) ch_potf2_kernel(double* __restrict__ A, i
   ch_tile_t& s = *reinterpret_cast<ch_tile_t*>(ch_smem);
   ch_tile_t& w = *reinterpret_cast<ch_tile_t*>(ch_smem + CH_NB * (CH_NB + 1));
   const int tid = threadIdx.x;
-  for (int e = tid; e < nbk * nbk; e += 256) {
-    const int r = e / nbk, c = e % nbk;
-    s[r][c] = (c <= r) ? A[(int64_t)(k0 + r) * ld + k0 + c] : 0.0;
-  }
+  const int tx = tid & 15, ty = tid >> 4;                    // 16 x 16 threads over the tile (no integer divisions in the loops)
+  __shared__ double dg[CH_NB];                               // the diagonal of L_kk
+  for (int r = ty; r < nbk; r += 16)
+    for (int c = tx; c < nbk; c += 16) s[r][c] = (c <= r) ? A[(int64_t)(k0 + r) * ld + k0 + c] : 0.0;
   __syncthreads();
   for (int j = 0; j < nbk; ++j) {
+    // column j: every thread takes the pivot from s[j][j] (not written in this phase), one of them records it
+    const double d = s[j][j];
+    const bool ok = d > 0.0;
+    const double ljj = ok ? sqrt(d) : 1.0;
     if (tid == 0) {
-      const double d = s[j][j];
-      if (!(d > 0.0)) { s[j][j] = 1.0; if (flag[0] == 0) flag[0] = 1 + k0 + j; }
-      else s[j][j] = sqrt(d);
+      dg[j] = ljj;
+      if (!ok && flag[0] == 0) flag[0] = 1 + k0 + j;
     }
-    __syncthreads();
-    const double ljj = s[j][j];
     for (int r = j + 1 + tid; r < nbk; r += 256) s[r][j] /= ljj;
     __syncthreads();
     // trailing update of the lower triangle: s[r][c] -= s[r][j] * s[c][j], j < c <= r
-    const int m = nbk - j - 1;
-    for (int e = tid; e < m * m; e += 256) {
-      const int r = j + 1 + e / m, c = j + 1 + e % m;
-      if (c <= r) s[r][c] -= s[r][j] * s[c][j];
+    for (int r = j + 1 + ty; r < nbk; r += 16) {
+      const double lrj = s[r][j];
+      for (int c = j + 1 + tx; c <= r; c += 16) s[r][c] -= lrj * s[c][j];
     }
     __syncthreads();
   }
-  for (int e = tid; e < nbk * nbk; e += 256) {
-    const int r = e / nbk, c = e % nbk;
-    if (c <= r) A[(int64_t)(k0 + r) * ld + k0 + c] = s[r][c];
-  }
+  if (tid < nbk) s[tid][tid] = dg[tid];
+  __syncthreads();
+  for (int r = ty; r < nbk; r += 16)
+    for (int c = tx; c <= r && c < nbk; c += 16) A[(int64_t)(k0 + r) * ld + k0 + c] = s[r][c];
   // W_kk = L_kk^-1: forward substitution on the identity, four threads per column (partial sums over t = q mod 4, combined by
   // two shuffles; the four threads of a column sit in one warp, so a warp barrier orders the row just written), then stored
   {
@@ -67,10 +67,8 @@ __global__ void __launch_bounds__(256) ch_potf2_kernel(double* __restrict__ A, i
     }
   }
   __syncthreads();
-  for (int e = tid; e < nbk * nbk; e += 256) {
-    const int r = e / nbk, c = e % nbk;
-    if (c <= r) W[(int64_t)(k0 + r) * ldw + k0 + c] = w[r][c];
-  }
+  for (int r = ty; r < nbk; r += 16)
+    for (int c = tx; c <= r && c < nbk; c += 16) W[(int64_t)(k0 + r) * ldw + k0 + c] = w[r][c];
 }
 
 // Panel below the diagonal block: A[i, k0:k0+nbk] <- A[i, k0:k0+nbk] L_kk^-T = A[i, :] W_kk^T for rows i >= k0+nbk.
