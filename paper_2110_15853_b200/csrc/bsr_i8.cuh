@@ -53,7 +53,7 @@ struct K3Params {
   const uint32_t* cmaxS;           // column maxima of Y_k (upper words)   [ncols]
   uint32_t* cmaxO;                 // out: column maxima of O, or NULL
   int64_t mrows;                   // valid rows (= nb*b for a Hamiltonian; < nb*b for the ragged last block of ttdft_rotate)
-  int32_t l2hints;                 // 1: evict-first H planes, evict-last Y digit tiles; 2: only the latter; 0: none
+  int32_t l2hints;                 // 1: evict-first H planes, evict-last Y digit tiles; 2: only the latter; 0: none (< 0 on the host: chosen per launch)
   int32_t jlimit = 0;              // > 0: only the first jlimit tiles of every block row are multiplied; < 0: the right factor is
                                    // upper triangular (the R^-1 of ttdft_orthonormalize's rotation; tiles = 128 rows of it in order):
                                    // a cluster whose last column tile is ct multiplies the first ceil((ct + 1) / 2) tiles only

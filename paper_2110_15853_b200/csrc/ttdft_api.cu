@@ -210,7 +210,7 @@ struct ttdft_h_s {
   int32_t sym_checked = 0;         // TTDFT_CHECK_SYMMETRY passed at build: H == H^T bit for bit
   const int32_t* perm = nullptr;   // rows reordered by subdomain label: row r of the tiles is the caller's row perm[r]
   int32_t k3_cluster = 0;   // 0: choose per launch; 1, 2, 4, 8: forced (env TTDFT_K3_CLUSTER)
-  int32_t k3_cg = 0;        // column tiles per scheduling group of K3 (env TTDFT_K3_CG; 0: one cluster's tiles)
+  int32_t k3_cg = 0;        // column tiles per scheduling group of K3 (env TTDFT_K3_CG; 0: all tiles of the launch, < 0: one cluster's tiles)
   int32_t k3_max_clusters[4] = {0, 0, 0, 0};   // co-resident clusters of 1, 2, 4, 8 CTAs (filled at the first launch)
 };
 
@@ -654,10 +654,17 @@ ttdft_status launch_k3(ttdft_h_s* h, const CUtensorMap& tmYd, ttdft::K3Params p,
   const int maxc = k3_max_clusters<S, C>(h);
   p.ct_begin = ct_begin;
   p.nctg = nct_launch / C;
-  // default: one cluster's tiles per scheduling group, i.e. co-resident clusters walk consecutive block rows on the
-  // same C column tiles, which share the most Y tiles in L2 (205 GB of DRAM reads per launch on config 3 vs 237 GB
-  // with 8 tiles per group; the time is the same, the kernel runs at the power limit)
-  p.cgc = std::max(1, (h->k3_cg > 0 ? h->k3_cg : C) / C);
+  // default (k3_cg = 0): ALL column tiles of the launch form one scheduling group, i.e. co-resident clusters work on the same two
+  // or three block rows at a time and share their H planes through L2 (each plane then comes from HBM once instead of once per
+  // cluster column), with the Y digit tiles of the ~27 neighbouring block rows held in L2 by the evict-last hint (l2hints = 2:
+  // no evict-first on H).  Same-box A/B on config 3: filter 1,236-1,241 ms -> 1,181-1,197 ms against the former default
+  // (TTDFT_K3_CG=-1 TTDFT_K3_L2HINTS=1: one cluster's tiles per group, clusters walk consecutive block rows).
+  // Tiles narrower than 128 keep the former order: a 56 KB Y digit tile feeds only b/32 k-steps of MMAs, so at b = 96 the Y
+  // traffic per MMA cycle is 4/3 of b = 128's and the Y-friendly order wins (config 4: 8.17 s vs 8.38 s per filter).
+  const bool share_h = (h->k3_cg == 0) ? (h->b >= 128) : (h->k3_cg > 0);
+  p.cgc = h->k3_cg > 0 ? std::max(1, h->k3_cg / C) : (share_h ? std::max(1, p.nctg) : 1);
+  // evict-first on H only where every H plane is used by ONE cluster (no sharing, or a single cluster column: N <= 128)
+  if (p.l2hints < 0) p.l2hints = (p.cgc <= 1 || p.nctg <= 1) ? 1 : 2;
   const int64_t items = (int64_t)h->nb * p.nctg;
   cudaLaunchConfig_t cfg;
   cudaLaunchAttribute at[1];
@@ -725,7 +732,7 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
   p.S = X; p.lds = ldx; p.Z = Z ? Z : X; p.ldz = Z ? ldz : ldx; p.O = O; p.ldo = ldo;
   p.eH = h->eH; p.hdiag = h->hdiag; p.cmaxS = cmS; p.cmaxO = cmO;
   p.trace = g_k3_trace;
-  p.l2hints = env_int("TTDFT_K3_L2HINTS", 1);
+  p.l2hints = env_int("TTDFT_K3_L2HINTS", -1);
   p.mrows = h->M;
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
@@ -1048,6 +1055,7 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
   hx.M = r.M; hx.kernel = 1; hx.bsr = 1; hx.b = 128; hx.nb = r.nbm; hx.nblocks = (int64_t)r.nbm * r.nkb;
   hx.row_ptr = brow; hx.col = bcol;
   hx.i8_S = S; hx.math = TTDFT_MATH_I8X7; hx.eH = eX; hx.hdiag = nullptr;
+  hx.k3_cg = env_int("TTDFT_K3_CG", 0);
   int dev = 0, nsm = 0;
   if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0) hx.nsm = nsm;
   ttdft_status s;
@@ -1061,7 +1069,7 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
   p.alpha = 1.0; p.gamma = 0.0; p.beta = 0.0;
   p.S = nullptr; p.lds = 0; p.Z = Y; p.ldz = ldy; p.O = Y; p.ldo = ldy;
   p.eH = eX; p.hdiag = nullptr; p.cmaxS = cmQ; p.cmaxO = nullptr;
-  p.vec = 0; p.trace = nullptr; p.l2hints = env_int("TTDFT_K3_L2HINTS", 1); p.mrows = r.M;
+  p.vec = 0; p.trace = nullptr; p.l2hints = env_int("TTDFT_K3_L2HINTS", -1); p.mrows = r.M;
   auto launch_range = [&](int32_t c0, int32_t n, int32_t jlimit) -> ttdft_status {
     p.jlimit = jlimit;
     const int C = (n >= 2) ? 2 : 1;
