@@ -36,7 +36,7 @@ import synth  # noqa: E402
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # DRAM bytes per launch of the dominant kernel from the ncu --set full capture under profiles/
 # (dram__bytes_read.sum + dram__bytes_write.sum), keyed by (workload, kernel); None = not captured.
-NCU_TRAFFIC_BYTES = {("si", "bsr_i8"): 192.489e9 + 7.238e9,     # profiles/r01d_k3_si_full.txt
+NCU_TRAFFIC_BYTES = {("si", "bsr_i8"): 160.202e9 + 7.253e9,     # profiles/r01g_k3_si_full.txt
                      ("si", "bsr_dmma"): 88.096e9 + 7.241e9}   # profiles/r01_k1_si_full.txt
 # nominal dense tensor-core ratio int8 : bf16 on B200 (4.5 : 2.25 Pop/s, B200_PROFILING.md table)
 INT8_OVER_BF16 = 2.0
