@@ -34,7 +34,8 @@ def conditioned(M, n, cond, seed):
 
 
 @pytest.mark.parametrize("M,n,cond,pad", [(2048, 32, 1.0, 0), (1000, 70, 1.0, 3), (4113, 130, 1e3, 0), (300, 1, 1.0, 1),
-                                          (5000, 257, 1e5, 5), (128, 128, 1.0, 0)])
+                                          (5000, 257, 1e5, 5), (128, 128, 1.0, 0),
+                                          (3000, 449, 1e2, 1), (2500, 320, 1.0, 0)])     # 8 and 5 column tiles: the triangular tile limit of the rotation
 def test_orthonormalize_vs_gram_schmidt(tt, M, n, cond, pad):
     import torch
     X = conditioned(M, n, cond, 501)
