@@ -58,3 +58,55 @@ def chfsi(H: "api.Hamiltonian", X, m: int, b: float, a0: float, iterations: int,
             a = a0 + 1e-3 * (b - a0)
         X, lam = chfsi_iteration(H, X, m, a, b, a0)
     return X, lam
+
+
+def main():
+    """python -m paper_2110_15853_b200.chfsi [workload]: two passes of Algorithm 1 at the workload's shape (default config 3 "si"),
+    every step timed with CUDA events (torch's current stream is the stream the library launches on here)."""
+    import json
+    import os
+    import sys
+    import torch
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    if root not in sys.path:
+        sys.path.insert(0, root)
+    import synth
+    name = sys.argv[1] if len(sys.argv) > 1 else "si"
+    cfg = synth.CONFIGS[name]
+    d = json.load(open(os.path.join(root, "tests", "golden", "bounds.json")))[name]
+    a, b, a0 = d["a"], d["b"], d["a0"]
+    dev = torch.device("cuda")
+    Hs = synth.hamiltonian_bsr(cfg.G, cfg.b, cfg.z, cfg.seed)
+    H = api.h_build_bsr(Hs.M, Hs.b, *(torch.from_numpy(x).to(dev) for x in (Hs.row_ptr, Hs.col_idx, Hs.values)))
+    del Hs
+    M, n = cfg.M, cfg.N
+    X = torch.randn(M, n, dtype=torch.float64, device=dev)
+    for rep in range(2):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
+        ev[0].record()
+        Xf = torch.empty_like(X)
+        api.cheb_filter(H, X, Xf, cfg.m, a, b, a0)
+        ev[1].record()
+        Xo = torch.empty_like(X)
+        api.orthonormalize(Xf, Xo, passes=2)
+        ev[2].record()
+        del Xf
+        HF = torch.empty((n, n), dtype=torch.float64, device=dev)
+        api.project(H, Xo, HF)
+        ev[3].record()
+        lam, Q = torch.linalg.eigh(0.5 * (HF + HF.T))
+        ev[4].record()
+        Psi = torch.empty_like(X)
+        api.rotate(Xo, Q.contiguous(), Psi)
+        ev[5].record()
+        torch.cuda.synchronize()
+        t = [ev[i].elapsed_time(ev[i + 1]) for i in range(5)]
+        print(json.dumps({"workload": name, "pass": rep + 1, "filter_ms": t[0], "orthonormalize_ms": t[1], "project_ms": t[2],
+                          "eigh_torch_ms": t[3], "rotate_ms": t[4], "pass_ms": sum(t), "ritz_min": float(lam[0]), "ritz_max": float(lam[-1])}),
+              flush=True)
+        X = Psi
+        del Xo, HF, Q
+
+
+if __name__ == "__main__":
+    main()
