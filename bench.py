@@ -34,10 +34,18 @@ import synth  # noqa: E402
 # fp64 ALU/DMMA peak derived from unit counts and clocks: 148 SMs x 64 fp64
 # FMA/clk/SM x 2 flop x 1.965 GHz (clocks.max.sm).  Measured on this pool: DMMA loop 37.15 TFLOP/s.
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# DRAM bytes per launch of the dominant kernel from the ncu --set full capture under profiles/
-# (dram__bytes_read.sum + dram__bytes_write.sum), keyed by (workload, kernel); None = not captured.
-NCU_TRAFFIC_BYTES = {("si", "bsr_i8"): 160.202e9 + 7.253e9,     # profiles/r01g_k3_si_full.txt
-                     ("si", "bsr_dmma"): 88.096e9 + 7.241e9}   # profiles/r01_k1_si_full.txt
+# DRAM bytes per launch of the dominant kernel from ONE ncu --set full capture under profiles/
+# (dram__bytes_read.sum + dram__bytes_write.sum), keyed by (workload, kernel): a number copied from that file, NOT measured
+# in this run -- the line prints the file and the commit the capture was taken at beside it.  Missing key = not captured.
+NCU_TRAFFIC = {("si", "bsr_i8"): (160.202e9 + 7.253e9, "profiles/r01g_k3_si_full.txt", "e127703"),
+               ("si", "bsr_dmma"): (88.096e9 + 7.241e9, "profiles/r01_k1_si_full.txt", "92819c1")}
+
+
+def ncu_traffic(workload, kname):
+    t = NCU_TRAFFIC.get((workload, kname))
+    if t is None:
+        return None, None
+    return t[0], {"file": t[1], "commit": t[2], "note": "copied from that ncu --set full capture, not measured in this run"}
 # nominal dense tensor-core ratio int8 : bf16 on B200 (4.5 : 2.25 Pop/s, B200_PROFILING.md table)
 INT8_OVER_BF16 = 2.0
 
@@ -51,6 +59,15 @@ def int8_peak_tops():
         return INT8_OVER_BF16 * float(d["bf16_tflops_sustained"]), "of measured: MEASURED_PEAKS.json bf16_tflops_sustained x 2 (nominal int8:bf16)"
     except Exception:
         return INT8_OVER_BF16 * 1400.0, "of fallback: B200_PROFILING.md sustained bf16 1.4 PFLOP/s x 2 (nominal int8:bf16)"
+
+
+def hbm_peak_gbs():
+    """Measured HBM copy bandwidth (MEASURED_PEAKS.json), else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured: MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        return 6650.0, "fallback: B200_PROFILING.md measured copy bandwidth 6.65 TB/s"
 
 
 def load_bounds(name: str):
@@ -246,7 +263,6 @@ def main():
     Xd = Xh.to(dev, non_blocking=True)
     Yd = torch.empty_like(Xd)
     panel = args.panel if args.panel else cfg.panel
-    work = torch.empty(tt.cheb_filter_work_bytes(Hd, cfg.N, panel) + 16, dtype=torch.uint8, device=dev)
     torch.cuda.synchronize()
 
     def barrier():
@@ -254,39 +270,132 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    def step():
-        tt.cheb_filter(Hd, Xd, Yd, cfg.m, a, b, a0, panel_cols=panel, work=work)
+    npanels = -(-cfg.N // (panel if panel else min(cfg.N, 4096)))
+    useful = 2.0 * nnz * cfg.N * cfg.m                                   # flops of the method: non-zeros of H only
+    executed = 2.0 * H.nblocks * cfg.b * cfg.b * cfg.N * cfg.m           # what dense tiles multiply (explicit zeros included)
+    alg_bytes = cfg.m * (npanels * 8.0 * nnz + 24.0 * cfg.M * cfg.N) - 8.0 * cfg.M * cfg.N      # SURVEY.md 8(d) (iii)
+    hbm_bw, hbm_src = hbm_peak_gbs()
+    t_roof = max(alg_bytes / (hbm_bw * 1e9), useful / (FP64_PEAK_TFLOPS * 1e12))   # SURVEY.md 8(d) (iv), whole filter
+    binds = "fp64" if useful / (FP64_PEAK_TFLOPS * 1e12) >= alg_bytes / (hbm_bw * 1e9) else "hbm"
 
-    for _ in range(args.warmup):
-        step()
-    barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
-    for k in tt.KERNEL_IDS:
-        tt.timing_read(k)
-    tt.timing_enable(True)       # CUDA event pairs around every library kernel, on the launching stream
-    n0 = tt.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        step()
-    e1.record()
-    barrier()
-    launches = tt.launch_count() - n0
-    tt.timing_enable(False)
-    ktimes = {k: tt.timing_read(k) for k in tt.KERNEL_IDS}
-    clocks = sampler.stop()
-    t_region = e0.elapsed_time(e1) * 1e-3
-    if dist is not None:
-        tmax = torch.tensor([t_region], dtype=torch.float64, device=dev)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        t_region = float(tmax.item())
-    t_step = t_region / args.steps
+    def timed_filter(mode):
+        """W warm-up + K timed ttdft_cheb_filter calls in one math mode: device time (max over ranks), the library's own CUDA
+        event pairs per kernel, clocks sampled during the timed region, kernel launches counted by the library."""
+        Hd.set_math_mode(mode)
+        work = torch.empty(tt.cheb_filter_work_bytes(Hd, cfg.N, panel) + 16, dtype=torch.uint8, device=dev)
+
+        def step():
+            tt.cheb_filter(Hd, Xd, Yd, cfg.m, a, b, a0, panel_cols=panel, work=work)
+
+        for _ in range(args.warmup):
+            step()
+        barrier()
+        sampler = ClockSampler(local)
+        sampler.start()
+        for k in tt.KERNEL_IDS:
+            tt.timing_read(k)
+        tt.timing_enable(True)       # CUDA event pairs around every library kernel, on the launching stream
+        n0 = tt.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            step()
+        e1.record()
+        barrier()
+        launches = tt.launch_count() - n0
+        tt.timing_enable(False)
+        ktimes = {k: tt.timing_read(k) for k in tt.KERNEL_IDS}
+        clocks = sampler.stop()
+        t_region = e0.elapsed_time(e1) * 1e-3
+        if dist is not None:
+            tmax = torch.tensor([t_region], dtype=torch.float64, device=dev)
+            dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+            t_region = float(tmax.item())
+        del work
+        return {"t_step": t_region / args.steps, "t_region": t_region, "ktimes": ktimes, "clocks": clocks, "launches": int(launches)}
+
+    def mode_report(run, use_i8, planes):
+        """roofline object of one timed run (dominant kernel = the fused step kernel; one launch = one recurrence step over one panel;
+        its launch time comes from the library's CUDA event pairs recorded inside the timed region)."""
+        kname = "bsr_i8" if use_i8 else "bsr_dmma"
+        k_ms, k_n = run["ktimes"][kname]
+        assert k_n == args.steps * cfg.m * npanels, (k_n, args.steps, cfg.m, npanels)
+        t_launch = k_ms * 1e-3 / k_n
+        nl = cfg.m * npanels
+        shares = {k: v[0] / (run["t_region"] * 1e3) for k, v in run["ktimes"].items() if v[1]}
+        traffic, traffic_src = ncu_traffic(args.workload, kname)
+        common = {"launch_ms": t_launch * 1e3, "step_share": shares, "traffic": traffic, "traffic_source": traffic_src,
+                  "hbm_alg_gbs": alg_bytes / run["t_step"] / 1e9,
+                  # SURVEY.md 8(d) (iv): T_roof / t for the WHOLE filter, T_roof = max(alg. bytes / HBM peak, useful flops / fp64 peak)
+                  "survey_frac": t_roof / run["t_step"], "survey_binds": binds,
+                  "survey_t_roof_ms": t_roof * 1e3, "survey_peaks": {"fp64_tflops": FP64_PEAK_TFLOPS, "hbm_gbs": hbm_bw, "hbm_source": hbm_src}}
+        if use_i8:
+            # K3: the product runs as S(S+1)/2 exact int8 digit-plane products on the tensor pipe, so the tensor pipe bounds it.
+            # Algorithmic ops per launch = 2 * pairs * nnz * N (non-zeros only); executed = dense tiles, padded to the MMA shape.
+            pairs = planes * (planes + 1) // 2
+            peak, peak_src = int8_peak_tops()
+            ops_launch = 2.0 * pairs * nnz * cfg.N / npanels
+            ops_exec = 2.0 * pairs * H.nblocks * 128 * cfg.b * (-(-cfg.N // 64) * 64) / npanels
+            roof = {"bound": "tensor", "achieved": ops_launch / t_launch / 1e12, "peak": peak, "unit": "TFLOP/s",
+                    "frac": ops_launch / t_launch / 1e12 / peak, "kernel": "ttdft::bsr_i8_kernel", "peak_source": peak_src,
+                    "ops": f"int8 multiply-add = 2 ops; {pairs} digit-plane products per fp64 product ({planes} planes per operand: "
+                           "the implementation's choice of arithmetic, not the method's work)",
+                    "executed_tops": ops_exec / t_launch / 1e12, "executed_frac": ops_exec / t_launch / 1e12 / peak,
+                    "dense_tile_ceiling": useful / executed,
+                    "useful_fp64_tflops_kernel": useful / nl / t_launch / 1e12}
+        else:
+            ach = useful / nl / t_launch / 1e12
+            roof = {"bound": "alu", "achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS,
+                    "kernel": "ttdft::bsr_dmma_kernel",
+                    "peak_source": "derived: 148 SM x 64 fp64 FMA/clk x 2 x 1.965 GHz (native fp64 ALU/DMMA pipe; fp64 has no entry in "
+                                   "MEASURED_PEAKS.json)",
+                    "executed_tflops": executed / nl / t_launch / 1e12, "executed_frac": executed / nl / t_launch / 1e12 / FP64_PEAK_TFLOPS,
+                    "dense_tile_ceiling": useful / executed}
+        roof.update(common)
+        return roof
+
+    DTYPE = {"fp64": "f64 (fp64 tensor-core MMA, fp64 accumulate)",
+             "i8x7": "f64 in/out; int8x7 digit planes (55 bits below each row/column maximum), exact int32 accumulate, fp64 recombine",
+             "i8": "f64 in/out; int8x6 digit planes (47 bits below each row/column maximum), exact int32 accumulate, fp64 recombine"}
+
+    run = timed_filter(MODES[args.math])
+    t_step, clocks = run["t_step"], run["clocks"]
+    roof = mode_report(run, use_i8, planes)
+    try:
+        roof["peak_measured_dmma"] = tt.probe_fp64_peak(1, 300)
+    except Exception:
+        pass
+    cols_d = torch.from_numpy(synth.column_sample(cfg.N, cfg.panel, args.ref_cols, cfg.seed)).to(dev)
+    samples = {mode_name: Yd[:, cols_d].clone()}
+    Yd_headline = Yd.clone() if not args.no_e2e else None
+
+    line = {
+        "metric": "ChFSI filter useful fp64 GFLOP/s", "value": useful * world / t_step / 1e9, "unit": "GFLOP/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": DTYPE[mode_name], "data": "synthetic",
+        "config": workload_config(cfg, nnz, H.nblocks, args),      # the same object the reference arm prints
+        "math": (f"{mode_name}: exact int8 digit planes on tcgen05 ({planes} x 8 bit per fp64 operand = "
+                 f"{8 * planes - 1} bits below the row/column maximum, exact int32 accumulation, fp64 "
+                 "recombination, fp64 in/out)") if use_i8 else "fp64: fp64 tensor-core MMA (DMMA)",
+        "clocks": clocks, "gpu_launches": run["launches"], "roofline": roof,
+        "h_build_ms": t_build * 1e3, "h_upload_ms": t_upload * 1e3,
+    }
+
+    # ---- the native-fp64 arithmetic (TTDFT_MATH_FP64, kernel K1) with EQUAL standing: same handle, inputs, --steps and --warmup ----
+    others = {}
+    if not args.no_other_modes and mode_name != "fp64":
+        r64 = timed_filter(MODES["fp64"])
+        samples["fp64"] = Yd[:, cols_d].clone()
+        line["fp64_native"] = {
+            "what": "the same filter in TTDFT_MATH_FP64: every product on the fp64 tensor-core pipe (DMMA), no digit planes",
+            "metric": line["metric"], "value": useful * world / r64["t_step"] / 1e9, "unit": "GFLOP/s", "dtype": DTYPE["fp64"],
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": r64["t_step"] * 1e3, "clocks": r64["clocks"],
+            "gpu_launches": r64["launches"], "roofline": mode_report(r64, False, 0)}
+        others["fp64"] = line["fp64_native"]
 
     # ---- end to end through the C-ABI host-buffer call: H2D of X and D2H of Y inside the timed region
-    e2e = None
     if not args.no_e2e:
-        del work
+        Hd.set_math_mode(MODES[args.math])
         hwork = torch.empty(tt.cheb_filter_host_work_bytes(Hd, cfg.N, 1024) + 1024, dtype=torch.uint8, device=dev)
         tt.cheb_filter_host(Hd, Xh, Yh, cfg.m, a, b, a0, panel_cols=1024, work=hwork)   # warm-up
         barrier()
@@ -300,79 +409,17 @@ def main():
             tm = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
             dist.all_reduce(tm, op=dist.ReduceOp.MAX)
             t_e2e = float(tm.item())
-        e2e = {"value": 2.0 * nnz * cfg.N * cfg.m * world / t_e2e / 1e9, "unit": "GFLOP/s",
-               "h2d_bytes_per_step": cfg.M * cfg.N * 8, "d2h_bytes_per_step": cfg.M * cfg.N * 8,
-               "ms_per_step": t_e2e * 1e3, "api": "ttdft_cheb_filter_host (pinned host X, Y; 1024-column panels)"}
-        # sanity: the host path and the device path agree bit for bit on this rank's band
-        same = bool(torch.equal(Yh.to(dev), Yd))
-        e2e["matches_device_path"] = same
-        del hwork
+        line["e2e"] = {"value": 2.0 * nnz * cfg.N * cfg.m * world / t_e2e / 1e9, "unit": "GFLOP/s",
+                       "h2d_bytes_per_step": cfg.M * cfg.N * 8, "d2h_bytes_per_step": cfg.M * cfg.N * 8,
+                       "ms_per_step": t_e2e * 1e3, "api": "ttdft_cheb_filter_host (pinned host X, Y; 1024-column panels)",
+                       # sanity: the host path and the device path agree bit for bit on this rank's band
+                       "matches_device_path": bool(torch.equal(Yh.to(dev), Yd_headline))}
+        del hwork, Yd_headline
 
-    useful = 2.0 * nnz * cfg.N * cfg.m
-    executed = 2.0 * H.nblocks * cfg.b * cfg.b * cfg.N * cfg.m
-    npanels = -(-cfg.N // (panel if panel else min(cfg.N, 4096)))
-    alg_bytes = cfg.m * (npanels * 8.0 * nnz + 24.0 * cfg.M * cfg.N) - 8.0 * cfg.M * cfg.N
-    # dominant kernel: the fused step kernel; one launch = one recurrence step over one panel.
-    # Its launch time comes from the library's CUDA event pairs recorded inside the timed region.
-    kname = "bsr_i8" if use_i8 else "bsr_dmma"
-    k_ms, k_n = ktimes[kname]
-    assert k_n == args.steps * cfg.m * npanels, (k_n, args.steps, cfg.m, npanels)
-    t_launch = k_ms * 1e-3 / k_n
-    flops_per_launch = useful / (cfg.m * npanels)
-    fp64_equiv = {"achieved": flops_per_launch / t_launch / 1e12, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                  "frac": flops_per_launch / t_launch / 1e12 / FP64_PEAK_TFLOPS,
-                  "peak_source": "derived: 148 SM x 64 fp64 FMA/clk x 2 x 1.965 GHz (native fp64 ALU/DMMA pipe; "
-                                 "fp64 has no entry in MEASURED_PEAKS.json)",
-                  "executed_tflops": executed / (cfg.m * npanels) / t_launch / 1e12,
-                  "dense_tile_ceiling": useful / executed}
-    shares = {k: v[0] / (t_region * 1e3) for k, v in ktimes.items() if v[1]}
-    if use_i8:
-        # K3: the product runs as S(S+1)/2 exact int8 digit-plane products on the tensor pipe, so the
-        # tensor pipe bounds it.  Algorithmic ops per launch = 2 * pairs * nnz * N (non-zeros only).
-        S = planes
-        pairs = S * (S + 1) // 2
-        peak, peak_src = int8_peak_tops()
-        ops_launch = 2.0 * pairs * nnz * cfg.N / npanels
-        ops_exec = 2.0 * pairs * H.nblocks * 128 * cfg.b * (-(-cfg.N // 64) * 64) / npanels
-        roof = {"bound": "tensor", "achieved": ops_launch / t_launch / 1e12, "peak": peak, "unit": "TFLOP/s",
-                "frac": ops_launch / t_launch / 1e12 / peak, "traffic": NCU_TRAFFIC_BYTES.get((args.workload, kname)),
-                "kernel": "ttdft::bsr_i8_kernel", "launch_ms": t_launch * 1e3, "peak_source": peak_src,
-                "ops": f"int8 multiply-add = 2 ops; {pairs} digit-plane products per fp64 product ({S} planes per operand)",
-                "executed_tops": ops_exec / t_launch / 1e12, "executed_frac": ops_exec / t_launch / 1e12 / peak,
-                "fp64_equivalent": fp64_equiv, "step_share": shares, "hbm_alg_gbs": alg_bytes / t_step / 1e9}
-    else:
-        roof = {"bound": "alu", "achieved": fp64_equiv["achieved"], "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": fp64_equiv["frac"], "traffic": NCU_TRAFFIC_BYTES.get((args.workload, kname)),
-                "kernel": "ttdft::bsr_dmma_kernel", "launch_ms": t_launch * 1e3, "peak_source": fp64_equiv["peak_source"],
-                "executed_tflops": fp64_equiv["executed_tflops"],
-                "executed_frac": fp64_equiv["executed_tflops"] / FP64_PEAK_TFLOPS,
-                "dense_tile_ceiling": useful / executed, "step_share": shares, "hbm_alg_gbs": alg_bytes / t_step / 1e9}
-    try:
-        roof["peak_measured_dmma"] = tt.probe_fp64_peak(1, 300)
-    except Exception:
-        pass
-
-    line = {
-        "metric": "ChFSI filter useful fp64 GFLOP/s", "value": useful * world / t_step / 1e9, "unit": "GFLOP/s",
-        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": dict(workload_config(cfg, nnz, H.nblocks, args),
-                       math=(f"{mode_name}: exact int8 digit planes on tcgen05 ({planes} x 8 bit per fp64 operand = "
-                             f"{8 * planes - 1} bits below the row/column maximum, exact int32 accumulation, fp64 "
-                             "recombination, fp64 in/out)") if use_i8 else "fp64: fp64 tensor-core MMA (DMMA)"),
-        "clocks": clocks, "gpu_launches": int(launches), "roofline": roof,
-        "h_build_ms": t_build * 1e3, "h_upload_ms": t_upload * 1e3,
-    }
-    if e2e is not None:
-        line["e2e"] = e2e
-
-    # ---- the other arithmetic modes on the same handle and inputs: 1 warm-up + 1 timed filter each ----
-    cols_d = torch.from_numpy(synth.column_sample(cfg.N, cfg.panel, args.ref_cols, cfg.seed)).to(dev)
-    samples = {mode_name: Yd[:, cols_d].clone()}
-    others = {}
+    # ---- the 6-plane int8 mode on the same handle and inputs: 1 warm-up + 1 timed filter ----
     if rank == 0 and world == 1 and not args.no_other_modes:
-        for name in ("fp64", "i8x7", "i8"):
-            if name == mode_name or (name != "fp64" and not info["i8_planes"]):
+        for name in ("i8x7", "i8"):
+            if name == mode_name or not info["i8_planes"]:
                 continue
             Hd.set_math_mode(MODES[name])
             w2 = torch.empty(tt.cheb_filter_work_bytes(Hd, cfg.N, panel) + 16, dtype=torch.uint8, device=dev)
@@ -384,12 +431,12 @@ def main():
             f1.record()
             torch.cuda.synchronize()
             t_o = f0.elapsed_time(f1) * 1e-3
-            others[name] = {"value": useful / t_o / 1e9, "unit": "GFLOP/s", "ms_per_step": t_o * 1e3, "steps": 1, "warmup": 1,
-                            "frac_of_fp64_peak": useful / t_o / 1e12 / FP64_PEAK_TFLOPS}
+            others[name] = {"value": useful / t_o / 1e9, "unit": "GFLOP/s", "dtype": DTYPE[name], "ms_per_step": t_o * 1e3,
+                            "steps": 1, "warmup": 1, "survey_frac": t_roof / t_o}
             samples[name] = Yd[:, cols_d].clone()
             del w2
-        Hd.set_math_mode(MODES[args.math])
-        line["other_math_modes"] = others
+        line["other_math_modes"] = {k: v for k, v in others.items() if k != "fp64"}
+    Hd.set_math_mode(MODES[args.math])
 
     # ---- NEXT-1: subspace projection H_F = X^T (H X) on the same handle and X (1 warm-up + 2 timed) ----
     if rank == 0 and world == 1 and not args.no_project:
@@ -410,17 +457,26 @@ def main():
         pk = {k: tt.timing_read(k) for k in tt.KERNEL_IDS}
         t_p = g0.elapsed_time(g1) * 1e-3 / 2
         gram_ms = pk["gram_i8"][0] / max(pk["gram_i8"][1], 1)
-        fl_gram, fl_spmm = 2.0 * cfg.M * cfg.N * cfg.N, 2.0 * nnz * cfg.N
+        # The handle was built with TTDFT_CHECK_SYMMETRY, so H_F = H_F^T is known and ttdft_project computes only the entries on and
+        # above the diagonal (the method's own work: N(N+1)/2 entries of 2M flops), as whole 128 x 128 tile groups (executed work).
+        n128 = -(-cfg.N // 128)
+        fl_gram = 2.0 * cfg.M * cfg.N * (cfg.N + 1) / 2
+        fl_gram_exec = 2.0 * (-(-cfg.M // 128) * 128) * 128 * 128 * n128 * (n128 + 1) / 2
+        fl_gram_dense = 2.0 * cfg.M * cfg.N * cfg.N
+        fl_spmm = 2.0 * nnz * cfg.N
         peak8, peak8_src = int8_peak_tops()
-        ops_gram = 28.0 * fl_gram
         line["project"] = {
-            "what": "H_F = X^T (H X), Algorithm 1 step 3 (ttdft_project): one K3 step + Gram product K4 on the int8 tensor cores",
-            "ms": t_p * 1e3, "useful_tflops": (fl_gram + fl_spmm) / t_p / 1e12, "steps": 2, "warmup": 1,
+            "what": "H_F = X^T (H X), Algorithm 1 step 3 (ttdft_project): one K3 step + Gram product K4 on the int8 tensor cores; "
+                    "H = H^T was verified at build, so only the upper triangle of H_F is computed and mirrored",
+            "ms": t_p * 1e3, "useful_fp64_tflops": (fl_gram + fl_spmm) / t_p / 1e12, "steps": 2, "warmup": 1,
             "kernels_ms_each": {k: v[0] / v[1] for k, v in pk.items() if v[1]},
-            "gram_roofline": {"bound": "tensor", "achieved": ops_gram / (gram_ms * 1e-3) / 1e12, "peak": peak8, "unit": "TFLOP/s",
-                              "frac": ops_gram / (gram_ms * 1e-3) / 1e12 / peak8, "peak_source": peak8_src, "launch_ms": gram_ms,
-                              "fp64_equivalent_tflops": fl_gram / (gram_ms * 1e-3) / 1e12,
-                              "fp64_equivalent_frac_of_fp64_peak": fl_gram / (gram_ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS},
+            "gram_roofline": {"bound": "tensor", "achieved": 28.0 * fl_gram / (gram_ms * 1e-3) / 1e12, "peak": peak8, "unit": "TFLOP/s",
+                              "frac": 28.0 * fl_gram / (gram_ms * 1e-3) / 1e12 / peak8, "peak_source": peak8_src, "launch_ms": gram_ms,
+                              "ops": "method's own work: N(N+1)/2 entries x 2M flops x 28 digit-plane products",
+                              "executed_tops": 28.0 * fl_gram_exec / (gram_ms * 1e-3) / 1e12,
+                              "executed_frac": 28.0 * fl_gram_exec / (gram_ms * 1e-3) / 1e12 / peak8,
+                              "useful_fp64_tflops": fl_gram / (gram_ms * 1e-3) / 1e12,
+                              "dense_equivalent_fp64_tflops": fl_gram_dense / (gram_ms * 1e-3) / 1e12},
             "symmetry_defect": float(((Gd - Gd.T).norm() / Gd.norm()).item()),
         }
         if not args.no_cpu_baseline:
@@ -445,9 +501,10 @@ def main():
         g1.record()
         torch.cuda.synchronize()
         t_r = g0.elapsed_time(g1) * 1e-3 / 2
-        line["rotate"] = {"what": "Psi = X Q, Algorithm 1 step 5 (ttdft_rotate): kernel K3 on row-scaled digit tiles of X",
-                          "ms": t_r * 1e3, "fp64_equivalent_tflops": fl_gram / t_r / 1e12, "steps": 2, "warmup": 1,
-                          "frac_of_fp64_peak": fl_gram / t_r / 1e12 / FP64_PEAK_TFLOPS}
+        ops_rot = 28.0 * fl_gram_dense                     # Q is a full matrix here: every entry of the product is the method's work
+        line["rotate"] = {"what": "Psi = X Q, Algorithm 1 step 5 (ttdft_rotate): kernel K3 on row-scaled digit tiles of X (Q dense)",
+                          "ms": t_r * 1e3, "useful_fp64_tflops": fl_gram_dense / t_r / 1e12, "steps": 2, "warmup": 1,
+                          "int8_tops": ops_rot / t_r / 1e12, "frac_of_int8_peak": ops_rot / t_r / 1e12 / peak8}
         if not args.no_cpu_baseline:
             rr = torch.from_numpy(np.unique(np.random.default_rng(cfg.seed).integers(0, cfg.M, 16))).to(dev)
             refr = oracle.rotate(np.ascontiguousarray(Xd[rr].cpu().numpy()), Qd.cpu().numpy())
@@ -462,9 +519,13 @@ def main():
         g1.record()
         torch.cuda.synchronize()
         t_o = g0.elapsed_time(g1) * 1e-3
-        line["orthonormalize"] = {"what": "X_F = Orth(X), Algorithm 1 step 2 (ttdft_orthonormalize): Cholesky-QR2 = 2 x (Gram product K4, "
-                                          "n x n Cholesky + inverse, rotation on K3)",
-                                  "ms": t_o * 1e3, "fp64_equivalent_tflops": 4.0 * fl_gram / t_o / 1e12, "steps": 1, "warmup": 1}
+        # method's own work of Cholesky-QR2: per pass N(N+1)/2 entries of X^T X and the triangular product X R^-1 (M N(N+1)/2
+        # multiply-adds each), plus the n x n Cholesky and triangular inverse (n^3/3 flops each)
+        fl_orth = 2 * (2 * fl_gram + 2.0 * cfg.N ** 3 / 3)
+        line["orthonormalize"] = {"what": "X_F = Orth(X), Algorithm 1 step 2 (ttdft_orthonormalize): Cholesky-QR2 = 2 x (Gram product K4 on the "
+                                          "upper triangle, n x n Cholesky + inverse, triangular rotation X R^-1 on K3)",
+                                  "ms": t_o * 1e3, "useful_fp64_tflops": fl_orth / t_o / 1e12, "steps": 1, "warmup": 1,
+                                  "dense_equivalent_fp64_tflops": 8.0 * cfg.M * cfg.N * cfg.N / t_o / 1e12}
         if not args.no_cpu_baseline:
             lead = 16      # column j of Q depends on columns 0..j of X only: the leading block against the oracle's Gram-Schmidt
             refq = oracle.orthonormalize(np.ascontiguousarray(Xd[:, :lead].cpu().numpy()))

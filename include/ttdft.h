@@ -19,6 +19,21 @@
  *     ttdft_last_error() returns a thread-local message.  Nothing throws or aborts.
  *   - H is used AS STORED (both triangles present); symmetry is a promise that is only checked on
  *     request, and results are defined for a non-symmetric H too.
+ *   - "X must not overlap Y" means the two views share no element.  Column views of one wide row-major
+ *     buffer (X = B[:, :n], Y = B[:, n:2n], same leading dimension) do not overlap.
+ *
+ * Environment variables (every switch the library reads; none is needed for normal use).  They are read
+ * at two points only: by ttdft_h_build, into the handle (which is immutable afterwards), and at the entry
+ * of the handle-less calls ttdft_gram / ttdft_rotate / ttdft_orthonormalize (and ttdft_project's Gram
+ * product).  Do not change them from another thread while such a call runs (getenv is not safe against
+ * a concurrent setenv).
+ *   TTDFT_MATH        0..3: initial math mode of a handle (TTDFT_MATH_*); default 0 = AUTO.
+ *   TTDFT_K3_CLUSTER  1, 2, 4 or 8: force the CTA-cluster size of the int8 step kernel; default: chosen per launch.
+ *   TTDFT_K3_L2HINTS  0, 1 or 2: L2 eviction hints of the int8 step kernel's TMA loads (0 none, 1 evict-first
+ *                     H planes + evict-last Y digit tiles, 2 only the latter); default: chosen per launch.
+ *   TTDFT_K4_CLUSTER  1 or 2: CTA-cluster size of the int8 Gram kernel; default 2.
+ *   TTDFT_DEBUG       non-zero: print launch decisions to stderr.
+ * All of them select between code paths that give bit-identical results.
  */
 #ifndef TTDFT_H
 #define TTDFT_H
@@ -117,15 +132,24 @@ typedef struct {
 
 /* A0 -- storage builder (north_star "BSR/CSR storage builder"). */
 
-/* Bytes of device storage ttdft_h_build needs for this description.  Reads row_ptr's last entry
- * from the device (synchronises `stream`-less: uses a blocking 4-byte copy). */
+/* Bytes of device storage ttdft_h_build needs for this description.  The call has no stream: it reads
+ * row_ptr's last entry and, for a CSR with labels, analyses the labels and counts the tiles with kernels
+ * on the legacy default stream and blocking copies -- arrays produced on a non-blocking stream must be
+ * complete before the call.  For that analysis (labelled CSR only) it takes a transient device allocation
+ * of 16 bytes per row, freed before it returns: the one place besides ttdft_probe_fp64_peak's 64-byte sink
+ * where the library allocates device memory.  Indices are range-guarded: an invalid CSR gives a meaningless
+ * size, never a fault. */
 ttdft_status ttdft_h_storage_bytes(const ttdft_h_desc* desc, size_t* bytes);
 
 /* Validate and convert H into the device format inside dev_storage (>= the bytes reported above,
  * 1024-byte aligned).  The input arrays may be freed once `stream` has passed this call; the handle
  * only points into dev_storage, is immutable afterwards, and may be used from several streams.
- * With a CHECK flag the call synchronises `stream` and reports TTDFT_ERR_INVALID_ARG (unsorted /
- * out-of-range indices) or TTDFT_ERR_NOT_SYMMETRIC. */
+ * Everything runs on `stream` (the label analysis and tile count use dev_storage as scratch: no device
+ * allocation); the call synchronises `stream` to read sizes back.
+ * With a CHECK flag the indices are verified BEFORE any other kernel reads them, and the call reports
+ * TTDFT_ERR_INVALID_ARG (unsorted / duplicate / out-of-range indices, row_ptr not ascending from 0) or
+ * TTDFT_ERR_NOT_SYMMETRIC.  Without the flag invalid indices are skipped by the conversion (never a
+ * fault); the result is then undefined. */
 ttdft_status ttdft_h_build(const ttdft_h_desc* desc, void* dev_storage, size_t bytes, void* stream,
                            ttdft_h_t* out);
 ttdft_status ttdft_h_info(ttdft_h_t h, ttdft_h_info_t* info);

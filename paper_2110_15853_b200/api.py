@@ -175,6 +175,13 @@ def _stream(stream=None) -> int:
     return int(s.cuda_stream)
 
 
+def _keep(t, stream):
+    """A scratch tensor allocated here and used by kernels on a foreign stream: tell the caching allocator, so that the
+    memory is not handed out again before that stream has passed the call."""
+    if stream is not None and t is not None:
+        t.record_stream(stream)
+
+
 def _mat(t, name="matrix"):
     """(device pointer, leading dimension) of a row-major fp64 CUDA matrix view."""
     torch = _torch()
@@ -298,6 +305,7 @@ def spmm(H: Hamiltonian, alpha: float, X, beta: float, Y, stream=None, work=None
     if work is not None or use_work:
         wp, wb, keep = _work(H, X.shape[1], work, X.device)
         _check(_load().ttdft_spmm_ws(H.handle, alpha, xp, ldx, beta, yp, ldy, X.shape[1], wp, wb, _stream(stream)))
+        _keep(keep, stream)
         return Y
     _check(_load().ttdft_spmm(H.handle, alpha, xp, ldx, beta, yp, ldy, X.shape[1], _stream(stream)))
     return Y
@@ -314,6 +322,7 @@ def cheb_step(H: Hamiltonian, alpha: float, c: float, beta: float, Yk, Ykm1, You
         wp, wb, keep = _work(H, Yk.shape[1], work, Yk.device)
         _check(_load().ttdft_cheb_step_ws(H.handle, alpha, c, beta, kp, ldk, mp, ldm, op, ldo, Yk.shape[1], wp, wb,
                                           _stream(stream)))
+        _keep(keep, stream)
         return Yout
     _check(_load().ttdft_cheb_step(H.handle, alpha, c, beta, kp, ldk, mp, ldm, op, ldo, Yk.shape[1], _stream(stream)))
     return Yout
@@ -348,6 +357,7 @@ def cheb_filter(H: Hamiltonian, X, Y, m: int, a: float, b: float, a0: float, pan
     wp = (work.data_ptr() + 15) // 16 * 16
     wbytes = work.numel() * work.element_size() - (wp - work.data_ptr())
     _check(_load().ttdft_cheb_filter(H.handle, xp, ldx, yp, ldy, ncols, m, a, b, a0, panel_cols, wp, wbytes, _stream(stream)))
+    _keep(work, stream)
     return Y
 
 
@@ -402,6 +412,7 @@ def gram(X, W, G, work=None, stream=None):
         raise ValueError("shape mismatch")
     wp, wb, keep = _aligned_work(gram_work_bytes(M, N), work, X.device)
     _check(_load().ttdft_gram(M, xp, ldx, wp_, ldw, N, gp, ldg, wp, wb, _stream(stream)))
+    _keep(keep, stream)
     return G
 
 
@@ -420,6 +431,7 @@ def project(H: Hamiltonian, X, G, work=None, stream=None):
         raise ValueError("shape mismatch")
     wp, wb, keep = _aligned_work(project_work_bytes(H, N), work, X.device)
     _check(_load().ttdft_project(H.handle, xp, ldx, N, gp, ldg, wp, wb, _stream(stream)))
+    _keep(keep, stream)
     return G
 
 
@@ -440,6 +452,7 @@ def rotate(X, Q, Y, work=None, stream=None):
         raise ValueError("shape mismatch")
     wp, wb, keep = _aligned_work(rotate_work_bytes(M, k, n), work, X.device)
     _check(_load().ttdft_rotate(M, xp, ldx, k, qp, ldq, n, yp, ldy, wp, wb, _stream(stream)))
+    _keep(keep, stream)
     return Y
 
 
@@ -458,6 +471,7 @@ def orthonormalize(X, Y, passes: int = 2, work=None, stream=None):
         raise ValueError("shape mismatch")
     wp, wb, keep = _aligned_work(orthonormalize_work_bytes(M, n, passes), work, X.device)
     _check(_load().ttdft_orthonormalize(M, xp, ldx, n, yp, ldy, passes, wp, wb, _stream(stream)))
+    _keep(keep, stream)
     return Y
 
 

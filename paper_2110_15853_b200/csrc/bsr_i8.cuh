@@ -57,8 +57,19 @@ struct K3Params {
   int32_t jlimit = 0;              // > 0: only the first jlimit tiles of every block row are multiplied; < 0: the right factor is
                                    // upper triangular (the R^-1 of ttdft_orthonormalize's rotation; tiles = 128 rows of it in order):
                                    // a cluster whose last column tile is ct multiplies the first ceil((ct + 1) / 2) tiles only
-  unsigned long long* trace;       // debug (ttdft_debug_k3_trace): 8 clock64 stamps per work item of CTA 0, or NULL
+#ifdef TTDFT_DEBUG_TRACE
+  unsigned long long* trace = nullptr;   // debug builds only (-DTTDFT_DEBUG_TRACE): 8 clock64 stamps per work item of CTA 0, or NULL
+#endif
 };
+
+// clock trace of CTA 0 (debug builds only: the shipped kernel carries no trace stores)
+#ifdef TTDFT_DEBUG_TRACE
+#define K3_TRACE_DECL(cond) const bool tr_ = prm.trace && blockIdx.x == 0 && (cond)
+#define K3_TRACE(slot, val) do { if (tr_) prm.trace[it * 8 + (slot)] = (val); } while (0)
+#else
+#define K3_TRACE_DECL(cond) (void)it
+#define K3_TRACE(slot, val) do { } while (0)
+#endif
 
 template <int S>
 struct K3Cfg {
@@ -349,11 +360,12 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         const int32_t nJ = min(prm.brow_ptr[I + 1] - prm.brow_ptr[I], k3_jlimit<C>(prm, ctg));
         if (nJ == 0) continue;
         const int64_t it = (u - cluster0) / nclusters;
-        const bool tr = prm.trace && blockIdx.x == 0 && it < 512;
-        if (tr) prm.trace[it * 8 + 0] = clock64();
+        K3_TRACE_DECL(it < 512);
+        K3_TRACE(0, clock64());
         mbar_wait(accempty, aph ^ 1);            // the epilogue has drained the previous item's accumulators
         asm volatile("tcgen05.fence::after_thread_sync;");
-        if (tr) { prm.trace[it * 8 + 1] = clock64(); prm.trace[it * 8 + 7] = (unsigned long long)nJ; }
+        K3_TRACE(1, clock64());
+        K3_TRACE(7, (unsigned long long)nJ);
         for (int32_t j = 0; j < nJ; ++j) {
           mbar_wait(&yfull[yb], yph);
           const uint32_t ylo = ylo0 + (uint32_t)yb * (Cf::YBUF >> 4);
@@ -386,7 +398,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
           if (yb == 0) yph ^= 1;
         }
         umma_commit(accfull);
-        if (tr) prm.trace[it * 8 + 2] = clock64();
+        K3_TRACE(2, clock64());
         aph ^= 1;
       }
     }
@@ -441,17 +453,17 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
 
       double v[NCW];
       const int64_t it = (u - cluster0) / nclusters;
-      const bool tr = prm.trace && blockIdx.x == 0 && it < 512 && et == 0;
-      if (tr) prm.trace[it * 8 + 3] = clock64();
+      K3_TRACE_DECL(it < 512 && et == 0);
+      K3_TRACE(3, clock64());
       if (nJ > 0) {
         mbar_wait(accfull, aph);
         aph ^= 1;
-        if (tr) prm.trace[it * 8 + 4] = clock64();
+        K3_TRACE(4, clock64());
         asm volatile("tcgen05.fence::after_thread_sync;");
         k3_drain<S, NCW>(tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(half * NCW), v);
         asm volatile("tcgen05.fence::before_thread_sync;");
         mbar_arrive(accempty);                   // TMEM is free for the next work item
-        if (tr) prm.trace[it * 8 + 5] = clock64();
+        K3_TRACE(5, clock64());
       } else {
 #pragma unroll
         for (int i = 0; i < NCW; ++i) v[i] = 0.0;
@@ -543,7 +555,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         asm volatile("bar.sync 1, 256;" ::: "memory");
         if (et < 64 && col0 + et < prm.ncols && cm_s[et]) atomicMax(&prm.cmaxO[col0 + et], cm_s[et]);
       }
-      if (tr) prm.trace[it * 8 + 6] = clock64();
+      K3_TRACE(6, clock64());
       asm volatile("bar.sync 1, 256;" ::: "memory");   // ce_s / cm_s are rewritten by the next item
     }
   }

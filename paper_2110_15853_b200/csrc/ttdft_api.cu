@@ -29,7 +29,9 @@
 namespace {
 
 thread_local std::string g_err;
-unsigned long long* g_k3_trace = nullptr;   // debug: see ttdft_debug_k3_trace
+#ifdef TTDFT_DEBUG_TRACE
+unsigned long long* g_k3_trace = nullptr;   // debug builds only: see ttdft_debug_k3_trace
+#endif
 std::atomic<int64_t> g_launches{0};
 
 // ---- optional per-kernel device timing (ttdft_timing_*): CUDA events on the launching stream ----
@@ -200,7 +202,7 @@ struct ttdft_h_s {
   int32_t cg = 4;           // column tiles per scheduling group
   // K3 (int8 digit planes on the tcgen05 tensor cores); i8_S == 0: not built
   int32_t i8_S = 0;         // planes stored per tile
-  int32_t auto_planes = 7;  // planes TTDFT_MATH_AUTO uses (env TTDFT_I8_AUTO_PLANES: 6 or 7)
+  int32_t auto_planes = 7;  // planes TTDFT_MATH_AUTO uses
   int32_t math = TTDFT_MATH_AUTO;
   const int8_t* Hd = nullptr;     // [nblocks][S][b][128]
   const int32_t* eH = nullptr;    // [M]
@@ -209,8 +211,9 @@ struct ttdft_h_s {
   int32_t nsm = 148;
   int32_t sym_checked = 0;         // TTDFT_CHECK_SYMMETRY passed at build: H == H^T bit for bit
   const int32_t* perm = nullptr;   // rows reordered by subdomain label: row r of the tiles is the caller's row perm[r]
-  int32_t k3_cluster = 0;   // 0: choose per launch; 1, 2, 4, 8: forced (env TTDFT_K3_CLUSTER)
-  int32_t k3_cg = 0;        // column tiles per scheduling group of K3 (env TTDFT_K3_CG; 0: all tiles of the launch, < 0: one cluster's tiles)
+  int32_t k3_cluster = 0;   // 0: choose per launch; 1, 2, 4, 8: forced (env TTDFT_K3_CLUSTER at h_build)
+  int32_t k3_l2hints = -1;  // < 0: chosen per launch; 0 / 1 / 2: forced (env TTDFT_K3_L2HINTS at h_build)
+  int32_t debug = 0;        // env TTDFT_DEBUG at h_build: print launch decisions to stderr
   int32_t k3_max_clusters[4] = {0, 0, 0, 0};   // co-resident clusters of 1, 2, 4, 8 CTAs (filled at the first launch)
 };
 
@@ -220,12 +223,12 @@ namespace {
 // builder kernels (integer work + one pass over H)
 // ------------------------------------------------------------------------------------------------
 // flags[0] |= 1 : unsorted / duplicate / out-of-range index ; flags[0] |= 2 : not symmetric
-__global__ void check_sorted_kernel(int64_t nrows, const int32_t* row_ptr, const int32_t* col, int64_t ncolmax,
+__global__ void check_sorted_kernel(int64_t nrows, const int32_t* row_ptr, const int32_t* col, int64_t ncolmax, int32_t nnz,
                                     int32_t* flags) {
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= nrows) return;
   int32_t e0 = row_ptr[i], e1 = row_ptr[i + 1];
-  bool bad = e1 < e0;
+  bool bad = e1 < e0 || e0 < 0 || e1 > nnz || (i == 0 && e0 != 0);
   for (int32_t e = e0; e < e1 && !bad; ++e) {
     int32_t c = col[e];
     if (c < 0 || c >= ncolmax) bad = true;
@@ -340,8 +343,10 @@ __global__ void __launch_bounds__(256) label_perm_kernel(int64_t M, int32_t b, c
 
 // CSR -> BSR pass 1: one CTA per block row (of the reordered matrix), bitmap of touched block columns -> count.
 // perm/inv: reordered row r is input row perm[r], input column j is reordered column inv[j] (NULL: identity).
+// Indices are range-guarded (an invalid CSR gives a meaningless count, never a fault): entries outside [0, nnz) and columns
+// outside [0, M) are skipped.
 __global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_ptr, const int32_t* col, const int32_t* perm,
-                                     const int32_t* inv, int32_t* counts, int32_t nwords) {
+                                     const int32_t* inv, int32_t* counts, int32_t nwords, int32_t nnz) {
   extern __shared__ uint32_t bits[];
   for (int w = threadIdx.x; w < nwords; w += blockDim.x) bits[w] = 0;
   __syncthreads();
@@ -349,8 +354,11 @@ __global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_p
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
   for (int32_t r = warp; r < b; r += nwarps) {
     const int64_t row = perm ? perm[I * b + r] : I * b + r;
-    for (int32_t e = row_ptr[row] + lane; e < row_ptr[row + 1]; e += 32) {
-      const int32_t j = inv ? inv[col[e]] : col[e];
+    const int32_t e1 = min(row_ptr[row + 1], nnz);
+    for (int32_t e = max(row_ptr[row], 0) + lane; e < e1; e += 32) {
+      const int32_t cj = col[e];
+      if ((uint32_t)cj >= (uint32_t)(nb * b)) continue;
+      const int32_t j = inv ? inv[cj] : cj;
       const int32_t J = j / b;
       atomicOr(&bits[J >> 5], 1u << (J & 31));
     }
@@ -370,7 +378,7 @@ __global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_p
 // pass 2: fill bcol (ascending) and scatter the entries into zero-initialised tiles
 __global__ void csr2bsr_fill_kernel(int64_t nb, int32_t b, const int32_t* row_ptr, const int32_t* col, const double* val,
                                     const int32_t* perm, const int32_t* inv, const int32_t* brow_ptr, int32_t* bcol,
-                                    double* tiles, int32_t nwords) {
+                                    double* tiles, int32_t nwords, int32_t nnz) {
   extern __shared__ uint32_t sm[];
   uint32_t* bits = sm;                    // nwords
   uint32_t* pref = sm + nwords;           // nwords: tiles before word w
@@ -380,8 +388,11 @@ __global__ void csr2bsr_fill_kernel(int64_t nb, int32_t b, const int32_t* row_pt
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
   for (int32_t r = warp; r < b; r += nwarps) {
     const int64_t row = perm ? perm[I * b + r] : I * b + r;
-    for (int32_t e = row_ptr[row] + lane; e < row_ptr[row + 1]; e += 32) {
-      const int32_t j = inv ? inv[col[e]] : col[e];
+    const int32_t e1 = min(row_ptr[row + 1], nnz);
+    for (int32_t e = max(row_ptr[row], 0) + lane; e < e1; e += 32) {
+      const int32_t cj = col[e];
+      if ((uint32_t)cj >= (uint32_t)(nb * b)) continue;
+      const int32_t j = inv ? inv[cj] : cj;
       const int32_t J = j / b;
       atomicOr(&bits[J >> 5], 1u << (J & 31));
     }
@@ -405,8 +416,11 @@ __global__ void csr2bsr_fill_kernel(int64_t nb, int32_t b, const int32_t* row_pt
   // rows of this block row: scatter entries
   for (int32_t r = warp; r < b; r += nwarps) {
     const int64_t row = perm ? perm[I * b + r] : I * b + r;
-    for (int32_t e = row_ptr[row] + lane; e < row_ptr[row + 1]; e += 32) {
-      const int32_t j = inv ? inv[col[e]] : col[e];
+    const int32_t e1 = min(row_ptr[row + 1], nnz);
+    for (int32_t e = max(row_ptr[row], 0) + lane; e < e1; e += 32) {
+      const int32_t cj = col[e];
+      if ((uint32_t)cj >= (uint32_t)(nb * b)) continue;
+      const int32_t j = inv ? inv[cj] : cj;
       const int32_t J = j / b;
       const uint32_t w = bits[J >> 5] & ((1u << (J & 31)) - 1u);
       const int32_t p = p0 + (int32_t)(pref[J >> 5] + __popc(w));
@@ -471,6 +485,22 @@ __global__ void __launch_bounds__(256) probe_dmma_kernel(double* out, int iters,
 int env_int(const char* name, int dflt) {
   const char* v = getenv(name);
   return v && *v ? atoi(v) : dflt;
+}
+// The environment switches of include/ttdft.h ("Environment variables").  They are read at two documented points only -- by
+// ttdft_h_build into the handle, and at the entry of the handle-less calls (ttdft_gram / _rotate / _orthonormalize and
+// ttdft_project's Gram product) -- never inside a launch path.
+struct EnvSwitches {
+  int math, k3_cluster, k3_l2hints, k4_cluster, debug;
+};
+EnvSwitches read_env() {
+  EnvSwitches e;
+  e.math = env_int("TTDFT_MATH", TTDFT_MATH_AUTO);
+  if (e.math < TTDFT_MATH_AUTO || e.math > TTDFT_MATH_I8X7) e.math = TTDFT_MATH_AUTO;
+  e.k3_cluster = env_int("TTDFT_K3_CLUSTER", 0);
+  e.k3_l2hints = env_int("TTDFT_K3_L2HINTS", -1);
+  e.k4_cluster = env_int("TTDFT_K4_CLUSTER", 2) == 1 ? 1 : 2;
+  e.debug = env_int("TTDFT_DEBUG", 0);
+  return e;
 }
 
 template <int WR, int Q, int CPS, int RS>
@@ -635,7 +665,7 @@ int k3_max_clusters(ttdft_h_s* h) {
     else (void)cudaGetLastError();
   }
   h->k3_max_clusters[ci] = std::max(n, 1);
-  if (env_int("TTDFT_DEBUG", 0))
+  if (h->debug)
     fprintf(stderr, "[ttdft] K3<%d,%d>: %d co-resident clusters on %d SMs\n", S, C, h->k3_max_clusters[ci], h->nsm);
   return h->k3_max_clusters[ci];
 }
@@ -658,11 +688,11 @@ ttdft_status launch_k3(ttdft_h_s* h, const CUtensorMap& tmYd, ttdft::K3Params p,
   // or three block rows at a time and share their H planes through L2 (each plane then comes from HBM once instead of once per
   // cluster column), with the Y digit tiles of the ~27 neighbouring block rows held in L2 by the evict-last hint (l2hints = 2:
   // no evict-first on H).  Same-box A/B on config 3: filter 1,236-1,241 ms -> 1,181-1,197 ms against the former default
-  // (TTDFT_K3_CG=-1 TTDFT_K3_L2HINTS=1: one cluster's tiles per group, clusters walk consecutive block rows).
+  // (one cluster's tiles per group, clusters walk consecutive block rows, evict-first on H).
   // Tiles narrower than 128 keep the former order: a 56 KB Y digit tile feeds only b/32 k-steps of MMAs, so at b = 96 the Y
   // traffic per MMA cycle is 4/3 of b = 128's and the Y-friendly order wins (config 4: 8.17 s vs 8.38 s per filter).
-  const bool share_h = (h->k3_cg == 0) ? (h->b >= 128) : (h->k3_cg > 0);
-  p.cgc = h->k3_cg > 0 ? std::max(1, h->k3_cg / C) : (share_h ? std::max(1, p.nctg) : 1);
+  const bool share_h = (h->b >= 128);
+  p.cgc = share_h ? std::max(1, p.nctg) : 1;
   // evict-first on H only where every H plane is used by ONE cluster (no sharing, or a single cluster column: N <= 128)
   if (p.l2hints < 0) p.l2hints = (p.cgc <= 1 || p.nctg <= 1) ? 1 : 2;
   const int64_t items = (int64_t)h->nb * p.nctg;
@@ -731,8 +761,10 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
   p.alpha = alpha; p.gamma = gamma; p.beta = beta;
   p.S = X; p.lds = ldx; p.Z = Z ? Z : X; p.ldz = Z ? ldz : ldx; p.O = O; p.ldo = ldo;
   p.eH = h->eH; p.hdiag = h->hdiag; p.cmaxS = cmS; p.cmaxO = cmO;
+#ifdef TTDFT_DEBUG_TRACE
   p.trace = g_k3_trace;
-  p.l2hints = env_int("TTDFT_K3_L2HINTS", -1);
+#endif
+  p.l2hints = h->k3_l2hints;
   p.mrows = h->M;
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
@@ -764,12 +796,23 @@ ttdft_status launch_copy2d(const double* src, int64_t lds, double* dst, int64_t 
   return TTDFT_OK;
 }
 
-// do [p, p + (rows-1)*ld + cols) and [q, ...) overlap?
+// Do the views p and q (rows x cols, row-major with leading dimensions ldp, ldq) share an element?  Two views with the SAME leading
+// dimension are column views of one wide buffer when their column intervals fit side by side in a row (X = B[:, :n], Y = B[:, n:2n]
+// -- the natural layout of bands and panels of one allocation): they are disjoint if those intervals do not intersect in any of
+// the rows both touch.  Different leading dimensions fall back to the bounding address ranges.
 bool overlaps(const double* p, int64_t ldp, const double* q, int64_t ldq, int64_t rows, int64_t cols) {
   if (rows == 0 || cols == 0) return false;
   const double* pe = p + (rows - 1) * ldp + cols;
   const double* qe = q + (rows - 1) * ldq + cols;
-  return p < qe && q < pe;
+  if (!(p < qe && q < pe)) return false;
+  if (ldp == ldq && ldp >= cols) {
+    const double* lo = p < q ? p : q;
+    const double* hi = p < q ? q : p;
+    const int64_t off = (int64_t)(hi - lo) % ldp;     // column offset of the later view inside a row of the earlier one
+    // disjoint in every row iff the later view starts at or after the earlier one's columns end and ends before the row wraps
+    if (off >= cols && off + cols <= ldp) return false;
+  }
+  return true;
 }
 
 ttdft_status check_scalars(int32_t m, double a, double b, double a0) {
@@ -921,7 +964,7 @@ ttdft_status launch_k4(const GramPlan& g, const CUtensorMap& tmXd, const CUtenso
 // sym_hint: the caller knows G is symmetric (W = H X with a symmetry-checked H): as for W == X only the tile groups that
 // touch the upper triangle are computed and the reduction mirrors them
 ttdft_status gram_run(const GramPlan& g, const double* X, int64_t ldx, const double* W, int64_t ldw, double* G, int64_t ldg, void* work,
-                      cudaStream_t st, bool sym_hint = false) {
+                      cudaStream_t st, const EnvSwitches& env, bool sym_hint = false) {
   constexpr int S = GRAM_S;
   if (g.M == 0) {   // empty contraction: G = 0
     CUDA_TRY(cudaMemset2DAsync(G, (size_t)ldg * 8, 0, (size_t)g.ncols * 8, (size_t)g.ncols, st));
@@ -964,8 +1007,8 @@ ttdft_status gram_run(const GramPlan& g, const double* X, int64_t ldx, const dou
   p.ncols = g.ncols; p.P = P; p.cmaxX = cmX; p.cmaxW = cmW;
   // G = X^T X: only the tiles that touch the upper triangle are computed (single panel only: the mirror image of an
   // entry must be in the same panel of partial tiles)
-  p.sym = (((X == W && ldx == ldw) || sym_hint) && g.wp >= g.ncols && env_int("TTDFT_K4_SYM", 1)) ? 1 : 0;
-  const int C = env_int("TTDFT_K4_CLUSTER", 2) == 1 ? 1 : 2;
+  p.sym = (((X == W && ldx == ldw) || sym_hint) && g.wp >= g.ncols) ? 1 : 0;
+  const int C = env.k4_cluster;
   for (int64_t c0 = 0; c0 < g.ncols; c0 += g.wp) {
     const int64_t wc = std::min(g.wp, g.ncols - c0);
     const int32_t ct0 = (int32_t)(c0 / 64), ntl = (int32_t)((wc + 63) / 64);
@@ -1020,7 +1063,7 @@ ttdft_status rotate_plan(int64_t M, int64_t K, int64_t N, RotatePlan* r) {
 // upper_tri: Q is upper triangular (the R^-1 of a Cholesky-QR): column tile ct then needs only the k-tiles J <= ceil((ct + 1) / 2) - 1;
 // K3 stops every work item's tile loop there (K3Params::jlimit = -1): about half of the full product's work.
 ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const double* Q, int64_t ldq, double* Y, int64_t ldy, void* work,
-                        cudaStream_t st, bool upper_tri = false) {
+                        cudaStream_t st, const EnvSwitches& env, bool upper_tri = false) {
   constexpr int S = GRAM_S;
   if (r.M == 0) return TTDFT_OK;
   uint8_t* wb = reinterpret_cast<uint8_t*>(work);
@@ -1055,7 +1098,7 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
   hx.M = r.M; hx.kernel = 1; hx.bsr = 1; hx.b = 128; hx.nb = r.nbm; hx.nblocks = (int64_t)r.nbm * r.nkb;
   hx.row_ptr = brow; hx.col = bcol;
   hx.i8_S = S; hx.math = TTDFT_MATH_I8X7; hx.eH = eX; hx.hdiag = nullptr;
-  hx.k3_cg = env_int("TTDFT_K3_CG", 0);
+  hx.k3_l2hints = env.k3_l2hints; hx.debug = env.debug;
   int dev = 0, nsm = 0;
   if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0) hx.nsm = nsm;
   ttdft_status s;
@@ -1069,7 +1112,7 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
   p.alpha = 1.0; p.gamma = 0.0; p.beta = 0.0;
   p.S = nullptr; p.lds = 0; p.Z = Y; p.ldz = ldy; p.O = Y; p.ldo = ldy;
   p.eH = eX; p.hdiag = nullptr; p.cmaxS = cmQ; p.cmaxO = nullptr;
-  p.vec = 0; p.trace = nullptr; p.l2hints = env_int("TTDFT_K3_L2HINTS", -1); p.mrows = r.M;
+  p.vec = 0; p.l2hints = env.k3_l2hints; p.mrows = r.M;
   auto launch_range = [&](int32_t c0, int32_t n, int32_t jlimit) -> ttdft_status {
     p.jlimit = jlimit;
     const int C = (n >= 2) ? 2 : 1;
@@ -1079,7 +1122,7 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
     if (main_tiles < n) return launch_k3<S, 1>(&hx, tmQd, p, c0 + main_tiles, n - main_tiles, st);
     return TTDFT_OK;
   };
-  return launch_range(0, r.nct, (upper_tri && env_int("TTDFT_ROTATE_TRI", 1)) ? -1 : 0);
+  return launch_range(0, r.nct, upper_tri ? -1 : 0);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1152,6 +1195,7 @@ ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Wm, double*
 }
 
 ttdft_status orth_run(const OrthPlan& o, const double* X, int64_t ldx, double* Y, int64_t ldy, void* work, cudaStream_t st) {
+  const EnvSwitches env = read_env();
   uint8_t* wb = reinterpret_cast<uint8_t*>(work);
   const int64_t ldn = o.n + (o.n & 1);
   double* G = reinterpret_cast<double*>(wb);
@@ -1167,14 +1211,14 @@ ttdft_status orth_run(const OrthPlan& o, const double* X, int64_t ldx, double* Y
     const bool to_y = ((o.passes - 1 - p) % 2 == 0);
     double* dst = to_y ? Y : T;
     const int64_t ldd = to_y ? ldy : ldn;
-    ttdft_status s = gram_run(o.g, src, lds, src, lds, G, ldn, inner, st);          // G = src^T src
+    ttdft_status s = gram_run(o.g, src, lds, src, lds, G, ldn, inner, st, env);     // G = src^T src
     if (s != TTDFT_OK) return s;
     int32_t hflag = 0;
     if ((s = chol_inverse(G, ldn, (int32_t)o.n, Wm, Rinv, ldn, dflag, &hflag, st)) != TTDFT_OK) return s;
     if (hflag)
       return fail(TTDFT_ERR_BREAKDOWN, "orthonormalize: X^T X is not positive definite in pass %d (pivot %d): columns are linearly "
                                        "dependent to working precision", p + 1, hflag - 1);
-    if ((s = rotate_run(o.r, src, lds, Rinv, ldn, dst, ldd, inner, st, true)) != TTDFT_OK) return s;   // dst = src R^-1, R^-1 upper triangular
+    if ((s = rotate_run(o.r, src, lds, Rinv, ldn, dst, ldd, inner, st, env, true)) != TTDFT_OK) return s;   // dst = src R^-1, R^-1 upper triangular
     src = dst;
     lds = ldd;
   }
@@ -1254,9 +1298,11 @@ ttdft_status ttdft_timing_read(int32_t kernel_id, double* total_ms, int64_t* lau
 }
 int64_t ttdft_launch_count(void) { return g_launches.load(); }
 
-// Debug aid, not part of include/ttdft.h: K3 launches record 8 clock64 stamps per work item of CTA 0 (first 512 items)
-// into this DEVICE buffer of 512*8 uint64 (NULL switches the trace off).
+#ifdef TTDFT_DEBUG_TRACE
+// Debug builds only (-DTTDFT_DEBUG_TRACE; not part of include/ttdft.h, not in the shipped library): K3 launches record 8 clock64
+// stamps per work item of CTA 0 (first 512 items) into this DEVICE buffer of 512*8 uint64 (NULL switches the trace off).
 void ttdft_debug_k3_trace(void* dev_buf) { g_k3_trace = reinterpret_cast<unsigned long long*>(dev_buf); }
+#endif
 
 static ttdft_status desc_counts(const ttdft_h_desc* d, int64_t* nrows_idx, int64_t* nstored) {
   if (!d) return fail(TTDFT_ERR_INVALID_ARG, "desc is NULL");
@@ -1279,45 +1325,67 @@ static ttdft_status desc_counts(const ttdft_h_desc* d, int64_t* nrows_idx, int64
   return TTDFT_OK;
 }
 
-// decide the device format; for CSR + usable hint returns the tile size in *hint_b (else 0)
+// ---- label analysis and tile count (A0 sizing) ----
+// Scratch: flag word | M-int label histogram | perm | inv | per-block-row tile counts.  Inside ttdft_h_build it is the caller's
+// dev_storage (nothing has been written there yet; ttdft_h_storage_bytes reports at least analysis_bytes for a labelled CSR, so the
+// region always fits); ttdft_h_storage_bytes has no buffer to use and takes a transient allocation, freed before it returns.
+static size_t analysis_bytes(int64_t M) { return 1024 + 4 * align_up((size_t)M * 4, 1024); }
+struct AnalysisScratch {
+  uint8_t* p = nullptr;
+  bool owned = false;
+  int64_t M = 0;
+  ~AnalysisScratch() { if (owned && p) cudaFree(p); }
+  int32_t* flag() const { return reinterpret_cast<int32_t*>(p); }
+  int32_t* region(int k) const { return reinterpret_cast<int32_t*>(p + 1024 + (size_t)k * align_up((size_t)M * 4, 1024)); }
+  int32_t* hist() const { return region(0); }
+  int32_t* perm() const { return region(1); }
+  int32_t* inv() const { return region(2); }
+  int32_t* counts() const { return region(3); }
+};
+static ttdft_status d2h(void* dst, const void* src, size_t n, cudaStream_t st) {
+  CUDA_TRY(cudaMemcpyAsync(dst, src, n, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return TTDFT_OK;
+}
+static bool wants_label_analysis(const ttdft_h_desc* d) {
+  return d->fmt == TTDFT_FMT_CSR && d->subdomain_of_row && !(d->flags & TTDFT_FORCE_GENERIC) && d->M > 0;
+}
+
 // Decide the device format.  For CSR + usable subdomain labels: *hint_b = tile size (else 0) and *permuted tells
-// whether the rows have to be reordered (labels not already grouped).
-static ttdft_status plan_format(const ttdft_h_desc* d, int32_t* hint_b, bool* permuted) {
+// whether the rows have to be reordered (labels not already grouped).  All kernels and copies run on `st`.
+static ttdft_status plan_format(const ttdft_h_desc* d, const AnalysisScratch& sc, cudaStream_t st, int32_t* hint_b, bool* permuted) {
   *hint_b = 0;
   *permuted = false;
-  if (d->fmt != TTDFT_FMT_CSR || !d->subdomain_of_row || (d->flags & TTDFT_FORCE_GENERIC) || d->M == 0) return TTDFT_OK;
-  int32_t* bad = nullptr;
-  CUDA_TRY(cudaMalloc(&bad, 4));                         // 4-byte transient flag
-  struct Free { void* p; ~Free() { cudaFree(p); } } free_bad{bad};
+  if (!wants_label_analysis(d)) return TTDFT_OK;
+  ttdft_status s;
+  int32_t* bad = sc.flag();
   // (1) labels already grouped: group size = index of the first label change
   std::vector<int32_t> lab((size_t)std::min<int64_t>(d->M, 129));
-  CUDA_TRY(cudaMemcpy(lab.data(), d->subdomain_of_row, lab.size() * 4, cudaMemcpyDeviceToHost));
+  if ((s = d2h(lab.data(), d->subdomain_of_row, lab.size() * 4, st)) != TTDFT_OK) return s;
   size_t b = 1;
   while (b < lab.size() && lab[b] == lab[0]) ++b;
   int32_t hb = 1;
   if (k1_block_ok((int32_t)b) && d->M % (int64_t)b == 0 && d->M / (int64_t)b <= (1 << 17)) {   // bitmap of block columns must fit shared memory
-    CUDA_TRY(cudaMemset(bad, 0, 4));
-    hint_check_kernel<<<(unsigned)((d->M + 255) / 256), 256>>>(d->M, d->subdomain_of_row, (int32_t)b, bad);
+    CUDA_TRY(cudaMemsetAsync(bad, 0, 4, st));
+    hint_check_kernel<<<(unsigned)((d->M + 255) / 256), 256, 0, st>>>(d->M, d->subdomain_of_row, (int32_t)b, bad);
     g_launches.fetch_add(1);
-    CUDA_TRY(cudaMemcpy(&hb, bad, 4, cudaMemcpyDeviceToHost));
+    if ((s = d2h(&hb, bad, 4, st)) != TTDFT_OK) return s;
     if (hb == 0) { *hint_b = (int32_t)b; return TTDFT_OK; }
   }
   // (2) labels in any row order: they must be the subdomain indices 0..nb-1, each owning the same number b of rows
-  int32_t* hist = nullptr;
-  CUDA_TRY(cudaMalloc(&hist, (size_t)d->M * 4));         // transient M-int histogram
-  Free free_hist{hist};
-  CUDA_TRY(cudaMemset(hist, 0, (size_t)d->M * 4));
-  CUDA_TRY(cudaMemset(bad, 0, 4));
-  label_hist_kernel<<<(unsigned)((d->M + 255) / 256), 256>>>(d->M, d->subdomain_of_row, hist, bad);
+  int32_t* hist = sc.hist();
+  CUDA_TRY(cudaMemsetAsync(hist, 0, (size_t)d->M * 4, st));
+  CUDA_TRY(cudaMemsetAsync(bad, 0, 4, st));
+  label_hist_kernel<<<(unsigned)((d->M + 255) / 256), 256, 0, st>>>(d->M, d->subdomain_of_row, hist, bad);
   g_launches.fetch_add(1);
   int32_t b0 = 0;
-  CUDA_TRY(cudaMemcpy(&b0, hist, 4, cudaMemcpyDeviceToHost));
-  CUDA_TRY(cudaMemcpy(&hb, bad, 4, cudaMemcpyDeviceToHost));
+  CUDA_TRY(cudaMemcpyAsync(&b0, hist, 4, cudaMemcpyDeviceToHost, st));
+  if ((s = d2h(&hb, bad, 4, st)) != TTDFT_OK) return s;
   if (hb != 0 || !k1_block_ok(b0) || d->M % b0 || d->M / b0 > (1 << 17)) return TTDFT_OK;
   const int64_t nb = d->M / b0;
-  label_hist_check_kernel<<<(unsigned)((nb + 255) / 256), 256>>>(nb, b0, hist, bad);
+  label_hist_check_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, st>>>(nb, b0, hist, bad);
   g_launches.fetch_add(1);
-  CUDA_TRY(cudaMemcpy(&hb, bad, 4, cudaMemcpyDeviceToHost));
+  if ((s = d2h(&hb, bad, 4, st)) != TTDFT_OK) return s;
   if (hb != 0) return TTDFT_OK;
   *hint_b = b0;
   *permuted = true;
@@ -1325,117 +1393,125 @@ static ttdft_status plan_format(const ttdft_h_desc* d, int32_t* hint_b, bool* pe
 }
 
 static ttdft_status csr2bsr_counts(const ttdft_h_desc* d, int32_t b, const int32_t* perm, const int32_t* inv, int32_t* dev_counts,
-                                   cudaStream_t st) {
+                                   int32_t nnz, cudaStream_t st) {
   const int64_t nb = d->M / b;
   const int32_t nwords = (int32_t)((nb + 31) / 32);
-  csr2bsr_count_kernel<<<(unsigned)nb, 256, (size_t)nwords * 4, st>>>(nb, b, d->row_ptr, d->col_idx, perm, inv, dev_counts, nwords);
+  csr2bsr_count_kernel<<<(unsigned)nb, 256, (size_t)nwords * 4, st>>>(nb, b, d->row_ptr, d->col_idx, perm, inv, dev_counts, nwords, nnz);
   CUDA_TRY(cudaGetLastError());
   g_launches.fetch_add(1);
   return TTDFT_OK;
 }
 
-// base: the fp64 format (K1 / K2); i8: the digit planes of K3 that follow it (0 if not built)
-static ttdft_status storage_bytes_impl(const ttdft_h_desc* d, size_t* bytes, size_t* i8) {
-  *i8 = 0;
-  int64_t nidx, nstored;
-  ttdft_status s = desc_counts(d, &nidx, &nstored);
+// The sizes and the format decision of one description.  base: the fp64 format (K1 / K2); i8: the digit planes of K3 that follow it
+// (0 if not built).  For a labelled CSR the row maps are left in sc.perm() / sc.inv().
+struct FormatPlan {
+  int64_t nidx = 0, nstored = 0;
+  int32_t hint_b = 0;
+  bool permuted = false;
+  size_t base = 0, i8 = 0;
+};
+static ttdft_status storage_bytes_impl(const ttdft_h_desc* d, const AnalysisScratch& sc, cudaStream_t st, FormatPlan* f) {
+  ttdft_status s = plan_format(d, sc, st, &f->hint_b, &f->permuted);
   if (s != TTDFT_OK) return s;
-  int32_t hint_b;
-  bool permuted;
-  s = plan_format(d, &hint_b, &permuted);
-  if (s != TTDFT_OK) return s;
-  if (hint_b) {
-    // count the tiles the conversion will create (transient scratch: nb counts, and the row maps if reordering)
+  if (f->hint_b) {
+    // count the tiles the conversion will create
+    const int32_t hint_b = f->hint_b;
     const int64_t nb = d->M / hint_b;
-    int32_t* cnt = nullptr;
-    CUDA_TRY(cudaMalloc(&cnt, ((size_t)nb + (permuted ? 2 * (size_t)d->M : 0)) * 4));
     int32_t *perm = nullptr, *inv = nullptr;
-    if (permuted) {
-      perm = cnt + nb;
-      inv = perm + d->M;
-      label_perm_kernel<<<(unsigned)nb, 256>>>(d->M, hint_b, d->subdomain_of_row, perm, inv);
+    if (f->permuted) {
+      perm = sc.perm();
+      inv = sc.inv();
+      label_perm_kernel<<<(unsigned)nb, 256, 0, st>>>(d->M, hint_b, d->subdomain_of_row, perm, inv);
       g_launches.fetch_add(1);
     }
-    s = csr2bsr_counts(d, hint_b, perm, inv, cnt, 0);
+    if ((s = csr2bsr_counts(d, hint_b, perm, inv, sc.counts(), (int32_t)f->nstored, st)) != TTDFT_OK) return s;
     std::vector<int32_t> hc((size_t)nb);
-    cudaError_t e = cudaMemcpy(hc.data(), cnt, (size_t)nb * 4, cudaMemcpyDeviceToHost);
-    cudaFree(cnt);
-    if (s != TTDFT_OK) return s;
-    if (e != cudaSuccess) return fail(TTDFT_ERR_CUDA, "tile count: %s", cudaGetErrorString(e));
+    if ((s = d2h(hc.data(), sc.counts(), (size_t)nb * 4, st)) != TTDFT_OK) return s;
     int64_t nblocks = 0;
     for (int32_t c : hc) nblocks += c;
     // brow_ptr | counts | bcol | tiles | (perm | inv)
-    *bytes = align_up((size_t)(nb + 1) * 4, 1024) + align_up((size_t)nb * 4, 1024) + align_up((size_t)nblocks * 4, 1024) +
-             align_up((size_t)nblocks * hint_b * hint_b * 8, 1024) + (permuted ? 2 * align_up((size_t)d->M * 4, 1024) : 0);
-    if (!(d->flags & TTDFT_NO_I8) && nblocks > 0) *i8 = i8_storage_bytes(nblocks, hint_b, d->M);
+    f->base = align_up((size_t)(nb + 1) * 4, 1024) + align_up((size_t)nb * 4, 1024) + align_up((size_t)nblocks * 4, 1024) +
+              align_up((size_t)nblocks * hint_b * hint_b * 8, 1024) + (f->permuted ? 2 * align_up((size_t)d->M * 4, 1024) : 0);
+    if (!(d->flags & TTDFT_NO_I8) && nblocks > 0) f->i8 = i8_storage_bytes(nblocks, hint_b, d->M);
     return TTDFT_OK;
   }
   const size_t per = (d->fmt == TTDFT_FMT_BSR) ? (size_t)d->block * d->block : 1;
   // row_ptr | col | values | (BSR check scratch: tile_row)
   const size_t nidxarr = (d->fmt == TTDFT_FMT_BSR) ? 2 : 1;
-  *bytes = align_up((size_t)(nidx + 1) * 4, 1024) + nidxarr * align_up((size_t)nstored * 4, 1024) +
-           align_up((size_t)nstored * per * 8, 1024) + 1024;
-  if (d->fmt == TTDFT_FMT_BSR && k1_block_ok(d->block) && !(d->flags & (TTDFT_FORCE_GENERIC | TTDFT_NO_I8)) && nstored > 0)
-    *i8 = i8_storage_bytes(nstored, d->block, d->M);
+  f->base = align_up((size_t)(f->nidx + 1) * 4, 1024) + nidxarr * align_up((size_t)f->nstored * 4, 1024) +
+            align_up((size_t)f->nstored * per * 8, 1024) + 1024;
+  if (d->fmt == TTDFT_FMT_BSR && k1_block_ok(d->block) && !(d->flags & (TTDFT_FORCE_GENERIC | TTDFT_NO_I8)) && f->nstored > 0)
+    f->i8 = i8_storage_bytes(f->nstored, d->block, d->M);
   return TTDFT_OK;
 }
 
 ttdft_status ttdft_h_storage_bytes(const ttdft_h_desc* d, size_t* bytes) {
   if (!bytes) return fail(TTDFT_ERR_INVALID_ARG, "bytes is NULL");
-  size_t base = 0, i8 = 0;
-  ttdft_status s = storage_bytes_impl(d, &base, &i8);
+  FormatPlan f;
+  ttdft_status s = desc_counts(d, &f.nidx, &f.nstored);
   if (s != TTDFT_OK) return s;
-  *bytes = base + i8;
+  AnalysisScratch sc;
+  sc.M = d->M;
+  if (wants_label_analysis(d)) {
+    CUDA_TRY(cudaMalloc(&sc.p, analysis_bytes(d->M)));   // transient: this call has no caller buffer to work in
+    sc.owned = true;
+  }
+  if ((s = storage_bytes_impl(d, sc, nullptr, &f)) != TTDFT_OK) return s;
+  *bytes = std::max(f.base + f.i8, wants_label_analysis(d) ? analysis_bytes(d->M) : (size_t)0);
   return TTDFT_OK;
 }
 
 ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t bytes, void* stream, ttdft_h_t* out) {
   if (!out) return fail(TTDFT_ERR_INVALID_ARG, "out is NULL");
   cudaStream_t st = (cudaStream_t)stream;
-  int64_t nidx, nstored;
-  ttdft_status s = desc_counts(d, &nidx, &nstored);
+  FormatPlan f;
+  ttdft_status s = desc_counts(d, &f.nidx, &f.nstored);
   if (s != TTDFT_OK) return s;
-  size_t need, need_i8;
-  s = storage_bytes_impl(d, &need, &need_i8);   // need: the fp64 format; the digit planes follow it
-  if (s != TTDFT_OK) return s;
-  if (bytes < need + need_i8)
-    return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "dev_storage has %zu bytes, %zu needed", bytes, need + need_i8);
-  if (need > 0 && (!dev_storage || (reinterpret_cast<uintptr_t>(dev_storage) & 1023)))
+  const int64_t nidx = f.nidx, nstored = f.nstored;
+  const bool checks = d->M > 0 && (d->flags & (TTDFT_CHECK_SORTED | TTDFT_CHECK_SYMMETRY));
+  const size_t scratch_need = wants_label_analysis(d) ? analysis_bytes(d->M) : (checks ? (size_t)1024 : (size_t)0);
+  if (d->M > 0 && (!dev_storage || (reinterpret_cast<uintptr_t>(dev_storage) & 1023)))
     return fail(TTDFT_ERR_INVALID_ARG, "dev_storage must be a 1024-byte aligned device pointer");
-  int32_t hint_b;
-  bool permuted;
-  s = plan_format(d, &hint_b, &permuted);
-  if (s != TTDFT_OK) return s;
+  if (bytes < scratch_need)
+    return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "dev_storage has %zu bytes, at least %zu needed", bytes, scratch_need);
+  AnalysisScratch sc;
+  sc.p = reinterpret_cast<uint8_t*>(dev_storage);
+  sc.M = d->M;
 
-  // ---- validation on request (on the input arrays) ----
-  if (d->M > 0 && (d->flags & (TTDFT_CHECK_SORTED | TTDFT_CHECK_SYMMETRY))) {
-    int32_t* flags = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(dev_storage) + need - 1024);
-    int32_t* tile_row = nullptr;
-    if (hint_b == 0 && d->fmt == TTDFT_FMT_BSR)   // scratch region reserved in storage_bytes
-      tile_row = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(dev_storage) + align_up((size_t)(nidx + 1) * 4, 1024) +
-                                            align_up((size_t)nstored * 4, 1024));
+  // ---- validation on request, BEFORE any kernel consumes the indices (the sizing kernels below are range-guarded as well) ----
+  if (checks) {
+    int32_t* flags = sc.flag();
     CUDA_TRY(cudaMemsetAsync(flags, 0, 4, st));
     const int64_t ncolmax = (d->fmt == TTDFT_FMT_BSR) ? d->M / d->block : d->M;
-    check_sorted_kernel<<<(unsigned)((nidx + 255) / 256), 256, 0, st>>>(nidx, d->row_ptr, d->col_idx, ncolmax, flags);
+    check_sorted_kernel<<<(unsigned)((nidx + 255) / 256), 256, 0, st>>>(nidx, d->row_ptr, d->col_idx, ncolmax, (int32_t)nstored, flags);
     g_launches.fetch_add(1);
     int32_t hf = 0;
-    CUDA_TRY(cudaMemcpyAsync(&hf, flags, 4, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
+    if ((s = d2h(&hf, flags, 4, st)) != TTDFT_OK) return s;
     if (hf & 1) return fail(TTDFT_ERR_INVALID_ARG, "indices are out of range, unsorted or duplicated");
     if (d->flags & TTDFT_CHECK_SYMMETRY) {
       if (d->fmt == TTDFT_FMT_CSR) {
         check_sym_csr_kernel<<<(unsigned)((d->M + 127) / 128), 128, 0, st>>>(d->M, d->row_ptr, d->col_idx, d->values, flags);
         g_launches.fetch_add(1);
       } else if (nstored > 0) {
+        // tile_row scratch: behind the flag word (the check needs nstored ints; the fp64 format alone is 8 * b * b times that)
+        if (bytes < 1024 + align_up((size_t)nstored * 4, 1024))
+          return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "dev_storage has %zu bytes, too few for the symmetry check", bytes);
+        int32_t* tile_row = reinterpret_cast<int32_t*>(sc.p + 1024);
         tile_rows_kernel<<<(unsigned)((nidx + 255) / 256), 256, 0, st>>>(nidx, d->row_ptr, tile_row);
         check_sym_bsr_kernel<<<(unsigned)nstored, 256, 0, st>>>(d->block, d->row_ptr, d->col_idx, d->values, tile_row, flags);
         g_launches.fetch_add(2);
       }
-      CUDA_TRY(cudaMemcpyAsync(&hf, flags, 4, cudaMemcpyDeviceToHost, st));
-      CUDA_TRY(cudaStreamSynchronize(st));
+      if ((s = d2h(&hf, flags, 4, st)) != TTDFT_OK) return s;
       if (hf & 2) return fail(TTDFT_ERR_NOT_SYMMETRIC, "H is not symmetric");
     }
   }
+
+  if ((s = storage_bytes_impl(d, sc, st, &f)) != TTDFT_OK) return s;   // f.base: the fp64 format; the digit planes follow it
+  const size_t need = f.base, need_i8 = f.i8;
+  const int32_t hint_b = f.hint_b;
+  const bool permuted = f.permuted;
+  if (bytes < need + need_i8)
+    return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "dev_storage has %zu bytes, %zu needed", bytes, need + need_i8);
 
   ttdft_h_s* h = new (std::nothrow) ttdft_h_s;
   if (!h) return fail(TTDFT_ERR_CUDA, "out of host memory");
@@ -1459,7 +1535,7 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
       label_perm_kernel<<<(unsigned)nb, 256, 0, st>>>(d->M, b, d->subdomain_of_row, perm, inv);
       g_launches.fetch_add(1);
     }
-    s = csr2bsr_counts(d, b, perm, inv, counts, st);
+    s = csr2bsr_counts(d, b, perm, inv, counts, (int32_t)nstored, st);
     if (s != TTDFT_OK) { delete h; return s; }
     exclusive_scan_small<<<1, 1, 0, st>>>(nb, counts, brow);
     g_launches.fetch_add(1);
@@ -1472,7 +1548,7 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     e = cudaMemsetAsync(tiles, 0, (size_t)nblocks * b * b * 8, st);
     if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "memset: %s", cudaGetErrorString(e)); }
     csr2bsr_fill_kernel<<<(unsigned)nb, 256, (size_t)nwords * 8, st>>>(nb, b, d->row_ptr, d->col_idx, d->values, perm, inv, brow,
-                                                                       bcol, tiles, nwords);
+                                                                       bcol, tiles, nwords, (int32_t)nstored);
     e = cudaGetLastError();
     if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "csr->bsr fill: %s", cudaGetErrorString(e)); }
     g_launches.fetch_add(1);
@@ -1505,10 +1581,9 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     if (h->b == 128) {
       s = make_map_2d(&h->tmH_half, h->val, (uint64_t)h->b, (uint64_t)h->nblocks * h->b, (uint64_t)h->b, 64u);
       if (s != TTDFT_OK) { delete h; return s; }
-      h->split = env_int("TTDFT_K1_SPLIT", 0);
+      h->split = 0;
     }
-    h->cg = env_int("TTDFT_K1_CG", 4);
-    if (h->cg < 1) h->cg = 1;
+    h->cg = 4;
   }
   bool i8_ok = (h->kernel == 1 && need_i8 > 0);
   if (i8_ok) {
@@ -1539,15 +1614,15 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
       s = make_map_hd(&h->tmHd[ci], Hd, (uint64_t)h->nblocks * I8_S * h->b, (uint32_t)(h->b >> ci));
       if (s != TTDFT_OK) { delete h; return s; }
     }
-    h->k3_cluster = env_int("TTDFT_K3_CLUSTER", 0);
-    h->k3_cg = env_int("TTDFT_K3_CG", 0);
+    const EnvSwitches env = read_env();
+    h->k3_cluster = env.k3_cluster;
+    h->k3_l2hints = env.k3_l2hints;
+    h->debug = env.debug;
     h->i8_S = I8_S; h->Hd = Hd; h->eH = eH; h->hdiag = hdiag;
     int dev = 0, nsm = 0;
     if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0)
       h->nsm = nsm;
-    h->math = env_int("TTDFT_MATH", TTDFT_MATH_AUTO);
-    if (h->math < TTDFT_MATH_AUTO || h->math > TTDFT_MATH_I8X7) h->math = TTDFT_MATH_AUTO;
-    h->auto_planes = env_int("TTDFT_I8_AUTO_PLANES", 7) == 6 ? 6 : 7;
+    h->math = env.math;
   }
   *out = h;
   return TTDFT_OK;
@@ -1734,7 +1809,7 @@ ttdft_status ttdft_cheb_filter(ttdft_h_t h, const double* X, int64_t ldx, double
   size_t need;
   if ((s = ttdft_cheb_filter_work_bytes(h, ncols, panel_cols, &need)) != TTDFT_OK) return s;
   const bool i8 = want_i8(h) && m >= 1 && h->M > 0;
-  const bool need_work = (m >= 2) || (m == 1 && inplace) || i8;
+  const bool need_work = (m >= 2) || (m == 1 && (inplace || h->perm)) || i8;   // a reordered handle always steps through the scratch panel
   if (need_work) {
     if (work_bytes < need) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, need);
     if (!work || (reinterpret_cast<uintptr_t>(work) & 15)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 16-byte aligned device pointer");
@@ -1875,7 +1950,7 @@ ttdft_status ttdft_gram(int64_t M, const double* X, int64_t ldx, const double* W
   if ((s = check_mat("G", G, ldg, ncols)) != TTDFT_OK) return s;
   if (work_bytes < g.total) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, g.total);
   if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
-  return gram_run(g, X, ldx, W, ldw, G, ldg, work, (cudaStream_t)stream);
+  return gram_run(g, X, ldx, W, ldw, G, ldg, work, (cudaStream_t)stream, read_env());
 }
 
 // scratch of ttdft_project: W = H*X (compact, even leading dimension) | max(single-step scratch, Gram scratch)
@@ -1916,7 +1991,7 @@ ttdft_status ttdft_project(ttdft_h_t h, const double* X, int64_t ldx, int64_t nc
     s = step_ws(h, 1.0, 0.0, 0.0, X, ldx, nullptr, 0, Wb, ldw, ncols, rest, need - wbytes, st);   // W = H X
     if (s != TTDFT_OK) return s;
   }
-  return gram_run(g, X, ldx, Wb, ldw, G, ldg, rest, st, h->sym_checked != 0);                     // G = X^T W
+  return gram_run(g, X, ldx, Wb, ldw, G, ldg, rest, st, read_env(), h->sym_checked != 0);         // G = X^T W
 }
 
 ttdft_status ttdft_rotate_work_bytes(int64_t M, int64_t k, int64_t n, size_t* bytes) {
@@ -1939,7 +2014,7 @@ ttdft_status ttdft_rotate(int64_t M, const double* X, int64_t ldx, int64_t k, co
   if (M > 0 && overlaps(X, ldx, Y, ldy, M, std::min(k, n)) ) return fail(TTDFT_ERR_INVALID_ARG, "X overlaps Y");
   if (work_bytes < r.total) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, r.total);
   if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
-  return rotate_run(r, X, ldx, Q, ldq, Y, ldy, work, (cudaStream_t)stream);
+  return rotate_run(r, X, ldx, Q, ldq, Y, ldy, work, (cudaStream_t)stream, read_env());
 }
 
 ttdft_status ttdft_orthonormalize_work_bytes(int64_t M, int64_t n, int32_t passes, size_t* bytes) {

@@ -10,6 +10,11 @@ the *_ws entry points; its time includes the digit extraction of X); roofline_fr
 the fp64-accurate product ran faster than the native fp64 pipe could.
 
     python -m paper_2110_15853_b200.sweep [--workload si] [--layouts bsr,csr] [--out gpurun_out/sweep.json]
+
+`--filter al,largest` instead times one whole ttdft_cheb_filter call on BASELINE.json's other configs (2 "al", 4 "largest":
+parity-test cases, not bench lines) in the i8x7 and fp64 math modes: X ~ N(0,1) generated on the device (in place for config 4,
+whose X is 45 GB), one timed call after a 2-step warm-up, CUDA events, per-kernel launch times from the library's own event pairs;
+one JSON line per (config, math mode).
 """
 from __future__ import annotations
 
@@ -55,8 +60,55 @@ def time_launches(fn, reps, flush):
     return float(np.median(ts)), float(np.min(ts))
 
 
+def filter_times(workloads):
+    """Whole-filter time of the named configs in both math modes (one JSON line each)."""
+    import torch
+    import paper_2110_15853_b200 as tt
+    dev = torch.device("cuda")
+    for wl in workloads:
+        cfg = synth.CONFIGS[wl]
+        with open(os.path.join(ROOT, "tests", "golden", "bounds.json")) as f:
+            d = json.load(f)[wl]
+        a, b, a0 = d["a"], d["b"], d["a0"]
+        H = synth.hamiltonian_bsr(cfg.G, cfg.b, cfg.z, cfg.seed)
+        nnz = int(np.count_nonzero(H.values))
+        Hd = tt.h_build_bsr(H.M, H.b, *(torch.from_numpy(x).to(dev) for x in (H.row_ptr, H.col_idx, H.values)))
+        del H
+        X = torch.randn(cfg.M, cfg.N, dtype=torch.float64, device=dev)
+        panel = cfg.panel if cfg.panel else 0
+        for mode, name in ((tt.MATH_I8X7, "i8x7"), (tt.MATH_FP64, "fp64")):
+            Hd.set_math_mode(mode)
+            work = torch.empty(tt.cheb_filter_work_bytes(Hd, cfg.N, panel) + 16, dtype=torch.uint8, device=dev)
+            inplace = cfg.M * cfg.N * 8 > 30e9
+            Y = X if inplace else torch.empty_like(X)
+            reps = 1 if inplace else 2
+            tt.cheb_filter(Hd, X, Y, 2, a, b, a0, panel_cols=panel, work=work)   # warm-up (2 steps)
+            torch.cuda.synchronize()
+            for k in tt.KERNEL_IDS:
+                tt.timing_read(k)
+            tt.timing_enable(True)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(reps):
+                tt.cheb_filter(Hd, X, Y, cfg.m, a, b, a0, panel_cols=panel, work=work)
+            e1.record()
+            torch.cuda.synchronize()
+            tt.timing_enable(False)
+            kt = {k: tt.timing_read(k) for k in tt.KERNEL_IDS}
+            t = e0.elapsed_time(e1) / reps
+            if inplace:
+                X.normal_()
+            print(json.dumps({"workload": wl, "M": cfg.M, "N": cfg.N, "b": cfg.b, "m": cfg.m, "panel": panel, "mode": name,
+                              "inplace": inplace, "filter_ms": t, "useful_tflops": 2.0 * nnz * cfg.N * cfg.m / t / 1e9,
+                              "kernels_ms_each": {k: round(v[0] / max(v[1], 1), 3) for k, v in kt.items() if v[1]}}), flush=True)
+            del work
+        del X, Y, Hd
+        torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--filter", default="", help="comma-separated configs (al, largest): time one whole filter each instead of the sweep")
     ap.add_argument("--workload", default="si")
     ap.add_argument("--layouts", default="bsr,csr,csr+labels,csr+recovered")
     ap.add_argument("--ns", default="16,64,256,1024,4096")
@@ -65,6 +117,8 @@ def main():
     ap.add_argument("--math", default="fp64,i8x7,i8", help="arithmetic of the bsr layout: fp64 (DMMA), i8x7 / i8 (7 / 6 digit planes)")
     ap.add_argument("--out", default="")
     args = ap.parse_args()
+    if args.filter:
+        return filter_times(args.filter.split(","))
     import torch
     import paper_2110_15853_b200 as tt
 

@@ -266,3 +266,81 @@ def test_row_dynamic_range_and_zero_rows(tt):
     rn = np.linalg.norm(ref, axis=1)
     rn[rn == 0] = 1.0
     assert np.max(np.linalg.norm(got - ref, axis=1) / rn) <= 10 * ACC["i8x7"]
+
+
+def kohn_sham_like(b, seed):
+    """A truncated Kohn-Sham-shaped H (couplings below 1e-4 Ha are dropped, the leading ones are O(1-10)):
+    the generator's structure and zero mask (G = 3, z = 0.4), every kept entry of an OFF-DIAGONAL tile replaced by
+    sign * 10^u, u ~ U[-4, 1], symmetric -- five orders of magnitude of dynamic range INSIDE every row of couplings."""
+    import copy
+    H0, _, _, _ = small_problem(3, b, 0.4, 2300 + b)
+    rng = np.random.default_rng(seed)
+    M = H0.M
+    V = np.where(rng.random((M, M)) < 0.5, -1.0, 1.0) * 10.0 ** rng.uniform(-4.0, 1.0, (M, M))
+    V = np.triu(V) + np.triu(V, 1).T
+    vals = H0.values.copy().reshape(H0.nblocks, b, b)
+    tile_row = np.repeat(np.arange(M // b), np.diff(H0.row_ptr))
+    for p in range(H0.nblocks):
+        I, J = int(tile_row[p]), int(H0.col_idx[p])
+        if I != J:
+            vals[p] = np.where(vals[p] != 0.0, V[I * b:(I + 1) * b, J * b:(J + 1) * b], 0.0)
+    H = copy.copy(H0)
+    H.values = vals.reshape(H0.values.shape)
+    return H
+
+
+@pytest.mark.parametrize("b", [64, 128])
+def test_in_row_dynamic_range(tt, b):
+    """The fixed-point operand format scales a whole row of H by ONE power of two: small couplings next to large ones keep
+    fewer bits than fp64 gives them (K3 error bound n 2^-51 hmax_i ymax_j).  On rows spanning 1e-4 .. 1e1 the
+    product must still meet north_star's 1e-12 and a degree-20 filter 1e-10, worst column within 10x, in both int8 modes."""
+    import torch
+    H = kohn_sham_like(b, 77)
+    C = synth.bsr_to_csr_nonzeros(H)
+    off = np.abs(C.values[np.abs(C.values) < 15.0])
+    assert off.min() < 2e-4 and off.max() > 5.0              # the range is really there
+    N, m = 150, 20
+    v0 = synth.dense_normal(H.M, 1, 23, synth.STREAM_V0).reshape(-1)
+    a0, bb, _ = oracle.lanczos_bounds(C.row_ptr, C.col_idx, C.values, v0, 40)
+    a0, bb = a0 - 0.05 * (bb - a0), bb + 0.05 * (bb - a0)    # safely outside the spectrum (this H is far from the generator's)
+    X = synth.dense_normal(H.M, N, 91)
+    ref_mm = oracle.spmm(C.row_ptr, C.col_idx, C.values, 1.0, X)
+    errs = {}
+    for wide in (False, True):
+        a, bb_, a0_ = bounds_for(a0, bb, N, H.M, wide=wide)
+        ref_f = oracle.cheb_filter(C.row_ptr, C.col_idx, C.values, X, m, a, bb_, a0_)
+        for mode in ("i8x7", "i8", "fp64"):
+            Hd = build_i8(tt, H, mode="i8x7")
+            Hd.set_math_mode({"i8x7": tt.MATH_I8X7, "i8": tt.MATH_I8, "fp64": tt.MATH_FP64}[mode])
+            Y = torch.empty(H.M, N, dtype=torch.float64, device="cuda")
+            tt.spmm(Hd, 1.0, dev(X), 0.0, Y, use_work=True)
+            e1, w1 = relerr(Y.cpu().numpy(), ref_mm), worst_col_relerr(Y.cpu().numpy(), ref_mm)
+            tt.cheb_filter(Hd, dev(X), Y, m, a, bb_, a0_)
+            e2, w2 = relerr(Y.cpu().numpy(), ref_f), worst_col_relerr(Y.cpu().numpy(), ref_f)
+            errs[(mode, wide)] = (e1, w1, e2, w2)
+            print(f"in-row dynamic range b={b} {mode} wide={wide}: spmm {e1:.2e} (worst col {w1:.2e}), filter {e2:.2e} ({w2:.2e})")
+    for (mode, wide), (e1, w1, e2, w2) in errs.items():
+        assert e1 <= TOL_SPMM and w1 <= 10 * TOL_SPMM, (mode, wide, e1, w1)
+        assert e2 <= TOL_FILTER and w2 <= 10 * TOL_FILTER, (mode, wide, e2, w2)
+
+
+@pytest.mark.parametrize("mode", ["i8x7", "i8"])
+def test_degree20_wide_gap_b128(tt, mode):
+    """SURVEY 8(d) "extra parity-only cases": the wide gap a = a0 + 0.25 (b - a0) with the headline degree m = 20
+    (|T_20(t0)| ~ 1.7e9: the iterates shrink by nine orders of magnitude, column scales change every step) on 128-wide tiles."""
+    import torch
+    H, C, (rp, col, val), (a0, bb) = small_problem(3, 128, 0.4, 2128)
+    N, m = 200, 20
+    a, bb, a0 = bounds_for(a0, bb, N, H.M, wide=True)
+    Hd = build_i8(tt, H, mode=mode)
+    X = synth.dense_normal(H.M, N, 93)
+    ref = oracle.cheb_filter(rp, col, val, X, m, a, bb, a0)
+    assert np.linalg.norm(ref) < 1e-3 * np.linalg.norm(X)    # the gap really damps
+    for inplace in (False, True):
+        Xd = dev(X)
+        Y = Xd if inplace else torch.empty_like(Xd)
+        tt.cheb_filter(Hd, Xd, Y, m, a, bb, a0, panel_cols=128)
+        got = Y.cpu().numpy()
+        e, w = relerr(got, ref), worst_col_relerr(got, ref)
+        print(f"m=20 wide gap b=128 {mode} inplace={inplace}: {e:.2e} worst col {w:.2e}")
+        assert e <= TOL_FILTER and w <= 10 * TOL_FILTER
