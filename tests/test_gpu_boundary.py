@@ -83,7 +83,7 @@ def test_invalid_indices_are_reported_not_faulted(tt):
             torch.cuda.synchronize()
         if how in ("huge", "negative"):
             # no check requested: sizing and conversion must not fault on the bad column (the result is undefined)
-            n = tt.h_storage_bytes(tt.FMT_CSR, Cp.M, 0, dev(rp), dev(ci), dev(Cp.values), subdomain_of_row=dev(labels))
+            n = tt.h_storage_bytes(0, Cp.M, 0, dev(rp), dev(ci), dev(Cp.values), subdomain_of_row=dev(labels))
             assert n > 0
             tt.h_build_csr(Cp.M, dev(rp), dev(ci), dev(Cp.values), subdomain_of_row=dev(labels))
             torch.cuda.synchronize()

@@ -335,7 +335,7 @@ def test_degree20_wide_gap_b128(tt, mode):
     Hd = build_i8(tt, H, mode=mode)
     X = synth.dense_normal(H.M, N, 93)
     ref = oracle.cheb_filter(rp, col, val, X, m, a, bb, a0)
-    assert np.linalg.norm(ref) < 1e-3 * np.linalg.norm(X)    # the gap really damps
+    assert np.linalg.norm(ref) < 0.5 * np.linalg.norm(X)     # three quarters of the spectrum are damped by ~1e-9
     for inplace in (False, True):
         Xd = dev(X)
         Y = Xd if inplace else torch.empty_like(Xd)
