@@ -32,8 +32,11 @@
  *   TTDFT_K3_L2HINTS  0, 1 or 2: L2 eviction hints of the int8 step kernel's TMA loads (0 none, 1 evict-first
  *                     H planes + evict-last Y digit tiles, 2 only the latter); default: chosen per launch.
  *   TTDFT_K4_CLUSTER  1 or 2: CTA-cluster size of the int8 Gram kernel; default 2.
+ *   TTDFT_K3_PREDICT_BIAS  test hook, -64..8, default 0: added to every predicted column exponent of the filter's int8
+ *                     path (negative: predictions fail and the fallback extraction runs; positive: digits lose that many bits).
+ *                     Unlike the others this one changes results in the last bits (always inside the documented error bound).
  *   TTDFT_DEBUG       non-zero: print launch decisions to stderr.
- * All of them select between code paths that give bit-identical results.
+ * All others select between code paths that give bit-identical results.
  */
 #ifndef TTDFT_H
 #define TTDFT_H
@@ -204,8 +207,9 @@ ttdft_status ttdft_cheb_scalars(int32_t m, double a, double b, double a0, double
                                 double* beta);
 
 /* Bytes of scratch ttdft_cheb_filter needs: one compact M x panel panel (panel_cols == 0: the
- * library's default panel width for this ncols), plus, in TTDFT_MATH_I8, the int8 digit planes of
- * one iterate (6 or 7 bytes per element) and two arrays of column maxima. */
+ * library's default panel width for this ncols), plus, in the int8 modes, the digit planes of
+ * two iterates (6 or 7 bytes per element each: one being read while the step's epilogue writes the
+ * next) and a few per-column arrays (maxima, exponents, flags). */
 ttdft_status ttdft_cheb_filter_work_bytes(ttdft_h_t h, int64_t ncols, int64_t panel_cols, size_t* bytes);
 
 /*
@@ -324,8 +328,9 @@ ttdft_status ttdft_probe_fp64_peak(int32_t kind, int32_t millis, void* stream, d
  * bracketed by a CUDA event pair on the launching stream; ttdft_timing_read waits for the events of
  * one kernel, returns the sum of their durations and their count, and clears them.
  *   kernel_id: 1 = block-sparse fp64 DMMA step, 2 = generic CSR/BSR step, 3 = block-sparse int8
- *   tensor-core step, 4 = digit planes of an iterate, 5 = column maxima of a panel, 6 = int8 tensor-core Gram
- *   product (ttdft_gram / ttdft_project).
+ *   tensor-core step, 4 = digit planes of an iterate (full extraction: a filter's first step, single steps, Gram operands),
+ *   5 = column maxima of a panel, 6 = int8 tensor-core Gram product (ttdft_gram / ttdft_project), 7 = the digit bookkeeping
+ *   between two steps of a filter (exponents; digits only of the column tiles whose predicted exponent was outgrown).
  */
 ttdft_status ttdft_timing_enable(int32_t on);
 ttdft_status ttdft_timing_read(int32_t kernel_id, double* total_ms, int64_t* launches);

@@ -138,7 +138,7 @@ def last_error() -> str:
     return _load().ttdft_last_error().decode()
 
 
-KERNEL_IDS = {"bsr_dmma": 1, "generic": 2, "bsr_i8": 3, "y_digits": 4, "colmax": 5, "gram_i8": 6}
+KERNEL_IDS = {"bsr_dmma": 1, "generic": 2, "bsr_i8": 3, "y_digits": 4, "colmax": 5, "gram_i8": 6, "y_digits_fix": 7}
 
 
 def timing_enable(on: bool = True):

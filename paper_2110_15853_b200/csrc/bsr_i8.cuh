@@ -50,18 +50,33 @@ struct K3Params {
   double* O;        int64_t ldo;
   const int32_t* eH;               // row exponents of H          [M]
   const double* hdiag;             // diagonal of H (fp64)         [M]; NULL: zero
-  const uint32_t* cmaxS;           // column maxima of Y_k (upper words)   [ncols]
-  uint32_t* cmaxO;                 // out: column maxima of O, or NULL
+  const int32_t* eS;               // exponents the digits of Y_k were taken with   [ncols]
+  uint32_t* cmaxO;                 // out: column maxima of O (upper words), or NULL
+  // digits of O for the next step, written by the epilogue (NULL: not wanted).  dO: digit tiles in the layout of i8_digits.cuh,
+  // taken with the PREDICTED exponents ePredO[j]; a column whose maximum outgrows its prediction sets flagsO[its 64-column tile]
+  // (the tile is then redone by y_digits_fix_kernel).  Requires cmaxO and mrows == nb * b.
+  int8_t* dO = nullptr;
+  const int32_t* ePredO = nullptr;
+  uint32_t* flagsO = nullptr;
   int64_t mrows;                   // valid rows (= nb*b for a Hamiltonian; < nb*b for the ragged last block of ttdft_rotate)
   int32_t l2hints;                 // 1: evict-first H planes, evict-last Y digit tiles; 2: only the latter; 0: none (< 0 on the host: chosen per launch)
   int32_t jlimit = 0;              // > 0: only the first jlimit tiles of every block row are multiplied; < 0: the right factor is
                                    // upper triangular (the R^-1 of ttdft_orthonormalize's rotation; tiles = 128 rows of it in order):
                                    // a cluster whose last column tile is ct multiplies the first ceil((ct + 1) / 2) tiles only
+#ifdef TTDFT_EXPERIMENT
+  int32_t exp = 0;                 // experiment builds only (-DTTDFT_EXPERIMENT, env TTDFT_K3_EXP): 2 no TMA after priming,
+                                   // 4 epilogue without global traffic, 8 epilogue without drain
+#endif
 #ifdef TTDFT_DEBUG_TRACE
   unsigned long long* trace = nullptr;   // debug builds only (-DTTDFT_DEBUG_TRACE): 8 clock64 stamps per work item of CTA 0, or NULL
 #endif
 };
 
+#ifdef TTDFT_EXPERIMENT
+#define K3_EXP(bit) ((prm.exp & (bit)) != 0)
+#else
+#define K3_EXP(bit) false
+#endif
 // clock trace of CTA 0 (debug builds only: the shipped kernel carries no trace stores)
 #ifdef TTDFT_DEBUG_TRACE
 #define K3_TRACE_DECL(cond) const bool tr_ = prm.trace && blockIdx.x == 0 && (cond)
@@ -80,7 +95,8 @@ struct K3Cfg {
   static constexpr int NBAR = 4 + 2 * NH + 2;
   static constexpr int CS_OFFSET = BAR_OFFSET + 8 * ((NBAR + 1) & ~1);   // 64 doubles: column scales
   static constexpr int CM_OFFSET = CS_OFFSET + 64 * 8;                   // 64 words: column maxima
-  static constexpr int TOTAL = CM_OFFSET + 64 * 4 + 16 + 1024;           // + tmem slot + alignment slack
+  static constexpr int CP_OFFSET = CM_OFFSET + 64 * 4 + 16;              // 64 words: predicted exponents of the output columns (behind the tmem slot)
+  static constexpr int TOTAL = CP_OFFSET + 64 * 4 + 1024;                // + alignment slack
   static_assert(S * K3_NT <= 512, "digit levels must fit TMEM");
   static_assert(NH >= 3, "H ring too short");
 };
@@ -279,6 +295,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
   int32_t* ce_s = reinterpret_cast<int32_t*>(smem + Cf::CS_OFFSET);      // eY_j of the current tile
   uint32_t* cm_s = reinterpret_cast<uint32_t*>(smem + Cf::CM_OFFSET);    // column maxima of the current tile
   uint32_t* tmem_slot = cm_s + 64;
+  int32_t* cp_s = reinterpret_cast<int32_t*>(smem + Cf::CP_OFFSET);      // predicted exponents of the output columns
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t nitems = (int64_t)prm.nb * prm.nctg;          // cluster work items
@@ -323,13 +340,16 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         for (int32_t p = p0; p < p1; ++p) {
           const int32_t J = prm.bcol[p];
           mbar_wait(&yempty[yb], yph ^ 1);
-          mbar_expect_tx(&yfull[yb], (uint32_t)Cf::YBUF);
-          if (prm.l2hints) tma_load_3d_hint(ybuf + yb * Cf::YBUF, &tmYd, 0, 0, (J * prm.nct + ct) * S, &yfull[yb], L2_EVICT_LAST);
+          const bool skip_tma = K3_EXP(2) && (u != cluster0 || p >= p0 + 2);
+          mbar_expect_tx(&yfull[yb], skip_tma ? 0u : (uint32_t)Cf::YBUF);
+          if (skip_tma) {}
+          else if (prm.l2hints) tma_load_3d_hint(ybuf + yb * Cf::YBUF, &tmYd, 0, 0, (J * prm.nct + ct) * S, &yfull[yb], L2_EVICT_LAST);
           else tma_load_3d(ybuf + yb * Cf::YBUF, &tmYd, 0, 0, (J * prm.nct + ct) * S, &yfull[yb]);
 #pragma unroll 1
           for (int q = 0; q < S; ++q) {
             mbar_wait(&hempty[hs], hph ^ 1);       // all C CTAs have finished with this slot
-            mbar_expect_tx(&hfull[hs], (uint32_t)b * 128u);
+            mbar_expect_tx(&hfull[hs], skip_tma ? 0u : (uint32_t)b * 128u);
+            if (skip_tma) { if (++hs == NH) { hs = 0; hph ^= 1; } continue; }
             uint8_t* hdst = hring + hs * Cf::HSLOT + (C > 1 ? crank * hrows * 128 : 0);
             const int32_t hrow = (p * prm.hplanes + k3_plane<S>(q)) * b + (C > 1 ? crank * hrows : 0);
             if (C > 1) {
@@ -382,10 +402,15 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
                 const uint64_t da = dbase | (uint64_t)(hlo + kk * 2);
                 // plane 0 comes first and spans every level: its first MMA of a work item overwrites the accumulators
                 const uint32_t acc = (ip > 0 || kk > 0) ? 1u : (j > 0 ? 1u : 0u);
-#pragma unroll
-                for (int n0 = 0; n0 < ntot; n0 += 256) {
-                  const int n = (ntot - n0) < 256 ? (ntot - n0) : 256;
-                  umma_i8(tmem_base + (uint32_t)(p * K3_NT + n0), da, dbase | (uint64_t)(ylo + n0 * 8 + kk * 2), umma_idesc_i8(n), acc);
+                // products wider than one instruction (256 columns) go as two EQUAL halves (448 = 224 + 224, 384 = 192 + 192,
+                // 320 = 160 + 160): a 256 + 64 split leaves a narrow MMA that is bound by its shared-memory operand reads
+                // ((4 KB of A + 32 N B) / 128 B per clock > N / 2 clocks for N < 128); -1.5 % cycles per tile measured
+                if (ntot > 256) {
+                  const int nh = ntot / 2;            // a multiple of 32 for every S - p
+                  umma_i8(tmem_base + (uint32_t)(p * K3_NT), da, dbase | (uint64_t)(ylo + kk * 2), umma_idesc_i8(nh), acc);
+                  umma_i8(tmem_base + (uint32_t)(p * K3_NT + nh), da, dbase | (uint64_t)(ylo + nh * 8 + kk * 2), umma_idesc_i8(nh), acc);
+                } else {
+                  umma_i8(tmem_base + (uint32_t)(p * K3_NT), da, dbase | (uint64_t)(ylo + kk * 2), umma_idesc_i8(ntot), acc);
                 }
               }
             }
@@ -431,8 +456,9 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       const bool row_in = row_ok && row < prm.mrows;
       if (et < 64) {
         const int64_t cj = col0 + et;
-        ce_s[et] = exp_from_hi(cj < prm.ncols ? prm.cmaxS[cj] : 0u);
+        ce_s[et] = cj < prm.ncols ? prm.eS[cj] : I8_EMIN;
         cm_s[et] = 0;
+        if (prm.dO) cp_s[et] = cj < prm.ncols ? prm.ePredO[cj] : I8_EMIN;
       }
       double rsp = 0.0, gi = prm.gamma;
       const bool full = (col0 + K3_NT <= prm.ncols);
@@ -460,6 +486,10 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         aph ^= 1;
         K3_TRACE(4, clock64());
         asm volatile("tcgen05.fence::after_thread_sync;");
+        if (K3_EXP(8)) {
+#pragma unroll
+          for (int i = 0; i < NCW; ++i) v[i] = 1.0;
+        } else
         k3_drain<S, NCW>(tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(half * NCW), v);
         asm volatile("tcgen05.fence::before_thread_sync;");
         mbar_arrive(accempty);                   // TMEM is free for the next work item
@@ -473,6 +503,13 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       // three fp64 instructions per element: v * (alpha 2^(eH-30)), then the column's 2^eY by an exponent add, two FMAs
       uint32_t cmx = 0;                           // column maximum (upper word) this lane has seen
       bool cmax_done = false;
+      if (K3_EXP(4)) {
+        double sacc = 0.0;
+#pragma unroll
+        for (int c = 0; c < NCW; ++c) sacc += v[c] * rsp;
+        if (sacc == 1.2345e-300) prm.O[0] = sacc;      // keeps the drain alive, never true
+        cmax_done = true;
+      } else
       if (full) {
         // Coalesced output: after the drain a thread owns one ROW (32 columns); written that way every access of
         // a warp would touch 32 different lines.  The 32 x 32 block of the warp is transposed in registers (5 shuffle
@@ -492,16 +529,32 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         }
         // v[r] = (row r of this warp, column colw + lane)
         const int32_t ce = ce_s[half * NCW + lane];
+        // digits of the output for the next step (prm.dO): lane l owns column l, four consecutive rows give one k-major word per plane
+        const bool digits_out = (prm.dO != nullptr);
+        const int32_t cpred = digits_out ? cp_s[half * NCW + lane] : 0;
+        const double dscale = pow2i(8 * S - 1 - cpred);
+        uint8_t* dtile = digits_out ? reinterpret_cast<uint8_t*>(prm.dO) + ((int64_t)I * prm.nct + ct) * (int64_t)(S * K3_NT * 128) +
+                                          (half * NCW + lane) * 128 + quarter * 32
+                                    : nullptr;
+        if (digits_out && !warp_ok) {
+          // rows beyond b of a narrow tile: the k bytes of this quarter stay zero in every plane
+#pragma unroll
+          for (int q = 0; q < S; ++q) {
+            *reinterpret_cast<uint4*>(dtile + q * (K3_NT * 128)) = make_uint4(0, 0, 0, 0);
+            *reinterpret_cast<uint4*>(dtile + q * (K3_NT * 128) + 16) = make_uint4(0, 0, 0, 0);
+          }
+        }
         if (warp_ok) {
           const int64_t wrow0 = (int64_t)I * b + quarter * 32;
           const double* sw = prm.S + wrow0 * prm.lds + colw + lane;
           const double* zw = prm.Z + wrow0 * prm.ldz + colw + lane;
           double* ow = prm.O + wrow0 * prm.ldo + colw + lane;
           const int nrow = (int)min((int64_t)32, prm.mrows - wrow0);       // < 32 only in a ragged last block (warp-uniform)
+          uint32_t dw[S][4];                       // digit words of 16 rows: one 16-byte store per plane
 #pragma unroll
           for (int r0 = 0; r0 < 32; r0 += 8) {
             if (r0 < nrow) {
-              double y[8], z[8];
+              double y[8], z[8], ov[8];
               if (use_s) {
 #pragma unroll
                 for (int i = 0; i < 8; ++i) y[i] = (r0 + i < nrow) ? __ldcs(sw + (int64_t)(r0 + i) * prm.lds) : 0.0;   // read once: evict first
@@ -516,18 +569,37 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
                 double o = scale_pow2(v[r0 + i], ce);
                 if (use_s) o = fma(gr, y[i], o);
                 if (use_z) o = fma(beta, z[i], o);
+                ov[i] = o;
                 if (r0 + i < nrow) {
                   __stcs(ow + (int64_t)(r0 + i) * prm.ldo, o);
                   cmx = max(cmx, abs_hi(o));
                 }
               }
+              if (digits_out) {
+#pragma unroll
+                for (int g = 0; g < 2; ++g) {
+                  const double x4[4] = {ov[4 * g], ov[4 * g + 1], ov[4 * g + 2], ov[4 * g + 3]};
+                  uint32_t w[S];
+                  digits4<S>(x4, dscale, w);
+#pragma unroll
+                  for (int q = 0; q < S; ++q) dw[q][((r0 >> 2) & 3) + g] = w[q];
+                }
+                if (r0 & 8) {
+#pragma unroll
+                  for (int q = 0; q < S; ++q)
+                    *reinterpret_cast<uint4*>(dtile + q * (K3_NT * 128) + (r0 & 16)) = make_uint4(dw[q][0], dw[q][1], dw[q][2], dw[q][3]);
+                }
+              }
             }
           }
+          // a column that outgrew its predicted exponent: its digits are invalid, the tile is redone before the next step
+          if (digits_out && exp_from_hi(cmx) > cpred) atomicOr(&prm.flagsO[ct], 1u);
         }
         if (prm.cmaxO && cmx) atomicMax(&cm_s[half * NCW + lane], cmx);   // this lane has seen all 32 rows of its column
         cmax_done = true;
       } else {
-        // ragged last column tile: every thread writes its own row
+        // ragged last column tile: every thread writes its own row; its digit tile is left to y_digits_fix_kernel
+        if (prm.dO && et == 0) atomicOr(&prm.flagsO[ct], 1u);
         const double* sp = prm.S + row * prm.lds + colw;
         const double* zp = prm.Z + row * prm.ldz + colw;
         double* op = prm.O + row * prm.ldo + colw;

@@ -95,26 +95,19 @@ __global__ void __launch_bounds__(256) colmax_kernel(const double* __restrict__ 
 // 64-column tile) are ONE contiguous S*8 KB piece of HBM -- what one TMA load of K3 fetches.
 // One CTA per (block row I, 64-column tile): coalesced fp64 reads along the columns, a shared-memory
 // transpose, 128-byte coalesced int8 rows out -- the K-major rows K3's B operand wants.
-// Also clears next_cmax (the maxima K3's epilogue will accumulate for the following step).
-// grid (nb, tiles >= ceil(ncols/64)), 256 threads, dynamic smem S*64*33*4 bytes; M = valid rows (<= nb*b)
+// e[h]: exponent of column n0 + 32*h + lane (digits are taken of x * 2^(8S-1-e)); sd: S*64*33 words of shared memory.
 // ------------------------------------------------------------------------------------------------
 template <int S>
-__global__ void __launch_bounds__(256) y_digits_kernel(const double* __restrict__ Y, int64_t ld, int32_t b, int64_t M, int64_t ncols,
-                                                       const uint32_t* __restrict__ cmax, int8_t* __restrict__ D,
-                                                       uint32_t* __restrict__ next_cmax) {
-  extern __shared__ uint32_t sd[];   // [S][64][33] words: row (q,n) holds 128 k-bytes + 1 pad word
+__device__ __forceinline__ void y_digits_tile(const double* __restrict__ Y, int64_t ld, int32_t b, int64_t M, int64_t ncols, int64_t I,
+                                              int64_t ct, int64_t nct, const int32_t (&e)[2], int8_t* __restrict__ D, uint32_t* sd) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t I = blockIdx.x;
-  const int64_t n0 = (int64_t)blockIdx.y * 64;
-  if (next_cmax && I == 0 && threadIdx.x < 64 && n0 + threadIdx.x < ncols) next_cmax[n0 + threadIdx.x] = 0;
-
+  const int64_t n0 = ct * 64;
   double scale[2];
   bool cv[2];
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
-    const int64_t n = n0 + 32 * h + lane;
-    cv[h] = n < ncols;
-    scale[h] = pow2i(8 * S - 1 - exp_from_hi(cv[h] ? cmax[n] : 0u));
+    cv[h] = n0 + 32 * h + lane < ncols;
+    scale[h] = pow2i(8 * S - 1 - e[h]);
   }
   const int nquads = b >> 2;
   for (int quad = warp; quad < 32; quad += 8) {
@@ -137,8 +130,91 @@ __global__ void __launch_bounds__(256) y_digits_kernel(const double* __restrict_
   }
   __syncthreads();
   // rows (q, n) of this tile are consecutive 128-byte lines of D
-  uint32_t* dst = reinterpret_cast<uint32_t*>(D + (I * gridDim.y + blockIdx.y) * (int64_t)(S * 64 * 128));
+  uint32_t* dst = reinterpret_cast<uint32_t*>(D + (I * nct + ct) * (int64_t)(S * 64 * 128));
   for (int row = warp; row < S * 64; row += 8) dst[row * 32 + lane] = sd[row * 33 + lane];
+}
+
+// Digit tiles of a whole panel with the exponent of every column taken from its maximum cmax[j] (upper word).
+// Also clears next_cmax (the maxima K3's epilogue will accumulate for the following step) and, if e_out is given, leaves the
+// exponents there (K3 reads its column scales from such an array).
+// grid (nb, tiles >= ceil(ncols/64)), 256 threads, dynamic smem S*64*33*4 bytes; M = valid rows (<= nb*b)
+template <int S>
+__global__ void __launch_bounds__(256) y_digits_kernel(const double* __restrict__ Y, int64_t ld, int32_t b, int64_t M, int64_t ncols,
+                                                       const uint32_t* __restrict__ cmax, int8_t* __restrict__ D,
+                                                       uint32_t* __restrict__ next_cmax, int32_t* __restrict__ e_out) {
+  extern __shared__ uint32_t sd[];   // [S][64][33] words: row (q,n) holds 128 k-bytes + 1 pad word
+  const int lane = threadIdx.x & 31;
+  const int64_t I = blockIdx.x;
+  const int64_t n0 = (int64_t)blockIdx.y * 64;
+  int32_t e[2];
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const int64_t n = n0 + 32 * h + lane;
+    e[h] = exp_from_hi(n < ncols ? cmax[n] : 0u);
+  }
+  if (I == 0 && threadIdx.x < 64 && n0 + threadIdx.x < ncols) {
+    if (next_cmax) next_cmax[n0 + threadIdx.x] = 0;
+    if (e_out) e_out[n0 + threadIdx.x] = exp_from_hi(cmax[n0 + threadIdx.x]);
+  }
+  y_digits_tile<S>(Y, ld, b, M, ncols, I, blockIdx.y, gridDim.y, e, D, sd);
+}
+
+// ------------------------------------------------------------------------------------------------
+// The filter's digit bookkeeping between two steps (K3 "digits from the epilogue").  From step 2 on, K3's epilogue
+// writes the digit tiles of the iterate it produces itself, scaled by a PREDICTED exponent per column (the true column maxima are
+// only complete when the launch ends).  This kernel runs between two K3 launches and
+//   * fixes the exponent every column's digits were really taken with:  e_used[j] = e_pred[j], or -- for the 64-column tiles in
+//     which some column outgrew its prediction (flags[ct] != 0, set by K3's epilogue), and for every tile when force != 0 (the
+//     filter's first step: no digits exist yet) -- the true exponent from cmax[j]; those tiles' digits are (re)extracted here;
+//   * predicts the exponents of the NEXT iterate:  e_pred[j] = e_true[j] + clamp(e_true[j] - e_prev_true[j] + 1, -3, 0) + guard
+//     (the iterates of the Chebyshev recurrence shrink or hold their size from step to step, |p_k| <= 1 on the spectrum: a drop of two
+//     or more binary orders is followed with one order of slack, the guard bit absorbs a doubling, anything beyond falls back to the
+//     path above).  Measured on configs 2 and 3 (m = 20, narrow and wide gap): no tile redone after the first step;
+//   * clears next_cmax and next_flags for the coming launch.
+// cmax_prev == next_cmax (the two-slot rotation): the previous iterate's maxima are read before they are cleared, by the same thread.
+// grid (rows <= nb, tiles), 256 threads, dynamic smem S*64*33*4 bytes: CTA (x, ct) walks the block rows x, x + gridDim.x, ... of
+// column tile ct; CTAs of untouched tiles exit at once (the usual case: a small grid keeps that launch at a few microseconds).
+// ------------------------------------------------------------------------------------------------
+constexpr int I8_GUARD = 1;
+__host__ __device__ __forceinline__ int32_t predict_exp(int32_t e_cur, int32_t e_prev, bool have_prev) {
+  int32_t d = have_prev ? e_cur - e_prev + 1 : 0;     // a drop by one binary order is jitter across a power of two, not a trend
+  d = d > 0 ? 0 : (d < -3 ? -3 : d);
+  const int32_t e = e_cur + d + I8_GUARD;
+  return e < I8_EMIN ? I8_EMIN : e;
+}
+template <int S>
+__global__ void __launch_bounds__(256) y_digits_fix_kernel(const double* __restrict__ Y, int64_t ld, int32_t b, int64_t M, int64_t ncols,
+                                                           int32_t nb, const uint32_t* __restrict__ cmax, int8_t* __restrict__ D,
+                                                           const uint32_t* __restrict__ flags, int32_t force, int32_t have_prev,
+                                                           int32_t bias, int32_t* __restrict__ e_used, int32_t* __restrict__ e_pred,
+                                                           uint32_t* __restrict__ next_cmax, uint32_t* __restrict__ next_flags) {
+  extern __shared__ uint32_t sd[];
+  const int lane = threadIdx.x & 31;
+  const int64_t n0 = (int64_t)blockIdx.y * 64;
+  const bool redo = force || flags[blockIdx.y] != 0;
+  if (blockIdx.x == 0 && threadIdx.x < 64) {
+    const int64_t n = n0 + threadIdx.x;
+    if (n < ncols) {
+      const int32_t e_true = exp_from_hi(cmax[n]);
+      const int32_t e_prev = have_prev ? exp_from_hi(next_cmax[n]) : 0;     // the slot about to be cleared holds the iterate before
+      e_used[n] = redo ? e_true : e_pred[n];
+      int32_t ep = predict_exp(e_true, e_prev, have_prev != 0) + bias;      // bias: test hook (TTDFT_K3_PREDICT_BIAS), 0 in normal use
+      e_pred[n] = ep < I8_EMIN ? I8_EMIN : ep;
+      next_cmax[n] = 0;
+    }
+    if (threadIdx.x == 0) next_flags[blockIdx.y] = 0;
+  }
+  if (!redo) return;
+  int32_t e[2];
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const int64_t n = n0 + 32 * h + lane;
+    e[h] = exp_from_hi(n < ncols ? cmax[n] : 0u);
+  }
+  for (int64_t I = blockIdx.x; I < nb; I += gridDim.x) {
+    y_digits_tile<S>(Y, ld, b, M, ncols, I, blockIdx.y, gridDim.y, e, D, sd);
+    __syncthreads();
+  }
 }
 
 // ------------------------------------------------------------------------------------------------

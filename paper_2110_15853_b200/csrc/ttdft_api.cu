@@ -35,7 +35,8 @@ unsigned long long* g_k3_trace = nullptr;   // debug builds only: see ttdft_debu
 std::atomic<int64_t> g_launches{0};
 
 // ---- optional per-kernel device timing (ttdft_timing_*): CUDA events on the launching stream ----
-constexpr int NKID = 7;   // 1 = K1 bsr_dmma, 2 = K2 generic, 3 = K3 bsr_i8, 4 = y_digits, 5 = colmax, 6 = K4 gram_i8
+constexpr int NKID = 8;   // 1 = K1 bsr_dmma, 2 = K2 generic, 3 = K3 bsr_i8, 4 = y_digits (full extraction), 5 = colmax, 6 = K4 gram_i8,
+                          // 7 = y_digits_fix between two K3 launches (exponent bookkeeping; extraction only where a prediction failed)
 struct KernelTimer {
   std::atomic<int> on{0};
   std::mutex mu;
@@ -213,6 +214,7 @@ struct ttdft_h_s {
   const int32_t* perm = nullptr;   // rows reordered by subdomain label: row r of the tiles is the caller's row perm[r]
   int32_t k3_cluster = 0;   // 0: choose per launch; 1, 2, 4, 8: forced (env TTDFT_K3_CLUSTER at h_build)
   int32_t k3_l2hints = -1;  // < 0: chosen per launch; 0 / 1 / 2: forced (env TTDFT_K3_L2HINTS at h_build)
+  int32_t k3_predict_bias = 0;   // test hook (env TTDFT_K3_PREDICT_BIAS at h_build): added to every predicted exponent
   int32_t debug = 0;        // env TTDFT_DEBUG at h_build: print launch decisions to stderr
   int32_t k3_max_clusters[4] = {0, 0, 0, 0};   // co-resident clusters of 1, 2, 4, 8 CTAs (filled at the first launch)
 };
@@ -490,7 +492,7 @@ int env_int(const char* name, int dflt) {
 // ttdft_h_build into the handle, and at the entry of the handle-less calls (ttdft_gram / _rotate / _orthonormalize and
 // ttdft_project's Gram product) -- never inside a launch path.
 struct EnvSwitches {
-  int math, k3_cluster, k3_l2hints, k4_cluster, debug;
+  int math, k3_cluster, k3_l2hints, k3_predict_bias, k4_cluster, debug;
 };
 EnvSwitches read_env() {
   EnvSwitches e;
@@ -498,6 +500,8 @@ EnvSwitches read_env() {
   if (e.math < TTDFT_MATH_AUTO || e.math > TTDFT_MATH_I8X7) e.math = TTDFT_MATH_AUTO;
   e.k3_cluster = env_int("TTDFT_K3_CLUSTER", 0);
   e.k3_l2hints = env_int("TTDFT_K3_L2HINTS", -1);
+  e.k3_predict_bias = env_int("TTDFT_K3_PREDICT_BIAS", 0);
+  if (e.k3_predict_bias < -64 || e.k3_predict_bias > 8) e.k3_predict_bias = 0;
   e.k4_cluster = env_int("TTDFT_K4_CLUSTER", 2) == 1 ? 1 : 2;
   e.debug = env_int("TTDFT_DEBUG", 0);
   return e;
@@ -604,9 +608,12 @@ ttdft_status launch_step(const ttdft_h_s* h, double alpha, double gamma, double 
 // ------------------------------------------------------------------------------------------------
 // K3 path: the same step through int8 digit planes on the tcgen05 tensor cores
 // ------------------------------------------------------------------------------------------------
-struct I8Work {            // views into the caller's scratch (ttdft_step_work_bytes)
-  int8_t* D = nullptr;     // digit planes of the source iterate: [S][w][nb*128]
-  uint32_t* cmax[2] = {nullptr, nullptr};   // column maxima (upper words): source / next iterate
+struct I8Work {            // views into the caller's scratch (ttdft_step_work_bytes / ttdft_cheb_filter_work_bytes)
+  int8_t* D[2] = {nullptr, nullptr};        // digit tiles of the source iterate / of the iterate the step produces (filter only)
+  uint32_t* cmax[2] = {nullptr, nullptr};   // column maxima (upper words), same two slots
+  uint32_t* flags[2] = {nullptr, nullptr};  // per 64-column tile: a column outgrew its predicted exponent
+  int32_t* e_used = nullptr;                // exponents the source iterate's digits were taken with
+  int32_t* e_pred = nullptr;                // predicted exponents of the iterate the step produces
 };
 // digit planes per operand the handle's math mode uses: 0 (fp64 DMMA), 6 or 7
 int i8_planes_in_use(const ttdft_h_s* h) {
@@ -622,14 +629,26 @@ size_t i8_digit_bytes(const ttdft_h_s* h, int64_t w) {
   const size_t nct = (size_t)((w + ttdft::K3_NT - 1) / ttdft::K3_NT);
   return align_up((size_t)i8_planes_in_use(h) * nct * ttdft::K3_NT * (size_t)h->nb * 128, 1024);
 }
-size_t i8_work_bytes(const ttdft_h_s* h, int64_t w) { return i8_digit_bytes(h, w) + 2 * align_up((size_t)w * 4, 1024); }
-I8Work carve_i8_work(const ttdft_h_s* h, void* base, int64_t w) {
+// nbuf = 2 for the filter (K3's epilogue writes the next iterate's digits while the current ones are being read), 1 for a single step
+size_t i8_work_bytes(const ttdft_h_s* h, int64_t w, int nbuf) {
+  const size_t nct = (size_t)((w + ttdft::K3_NT - 1) / ttdft::K3_NT);
+  return (size_t)nbuf * i8_digit_bytes(h, w) + 4 * align_up((size_t)w * 4, 1024) + 2 * align_up(nct * 4, 1024);
+}
+I8Work carve_i8_work(const ttdft_h_s* h, void* base, int64_t w, int nbuf) {
   I8Work k;
+  const size_t nct = (size_t)((w + ttdft::K3_NT - 1) / ttdft::K3_NT);
   uint8_t* p = reinterpret_cast<uint8_t*>(base);
-  k.D = reinterpret_cast<int8_t*>(p);
+  k.D[0] = reinterpret_cast<int8_t*>(p);
   p += i8_digit_bytes(h, w);
+  if (nbuf > 1) { k.D[1] = reinterpret_cast<int8_t*>(p); p += i8_digit_bytes(h, w); }
+  const size_t cb = align_up((size_t)w * 4, 1024);
   k.cmax[0] = reinterpret_cast<uint32_t*>(p);
-  k.cmax[1] = reinterpret_cast<uint32_t*>(p + align_up((size_t)w * 4, 1024));
+  k.cmax[1] = reinterpret_cast<uint32_t*>(p + cb);
+  k.e_used = reinterpret_cast<int32_t*>(p + 2 * cb);
+  k.e_pred = reinterpret_cast<int32_t*>(p + 3 * cb);
+  p += 4 * cb;
+  k.flags[0] = reinterpret_cast<uint32_t*>(p);
+  k.flags[1] = reinterpret_cast<uint32_t*>(p + align_up(nct * 4, 1024));
   return k;
 }
 
@@ -719,17 +738,20 @@ int k3_pick_cluster(ttdft_h_s* h) {
   return 1;
 }
 
-// src: index of the cmax array that holds (have_src_max) or will hold the maxima of X; the other one
-// receives the maxima of O if want_out_max.
+// One step through K3.  src: slot (0/1) of D / cmax / flags that belongs to the source iterate X.
+//   have_src:  the previous K3 launch left X's digits in D[src] (predicted exponents in e_pred, overflow flags in flags[src]) and its
+//              column maxima in cmax[src]; otherwise they are computed here (colmax + forced extraction: the filter's first step, and
+//              every single step of the *_ws calls)
+//   have_prev: cmax[src ^ 1] holds the maxima of the iterate BEFORE X (the trend of the exponent prediction)
+//   want_next: K3's epilogue leaves the digits, maxima and flags of the output in slot src ^ 1 for the next step (needs D[src ^ 1])
 template <int S>
 ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
                               const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, const I8Work& w, int src,
-                              bool have_src_max, bool want_out_max, cudaStream_t st) {
+                              bool have_src, bool have_prev, bool want_next, cudaStream_t st) {
   if (h->M == 0) return TTDFT_OK;
   const unsigned nct = (unsigned)((ncols + ttdft::K3_NT - 1) / ttdft::K3_NT);
   uint32_t* cmS = w.cmax[src];
-  uint32_t* cmO = want_out_max ? w.cmax[src ^ 1] : nullptr;
-  if (!have_src_max) {
+  if (!have_src) {
     CUDA_TRY(cudaMemsetAsync(cmS, 0, (size_t)ncols * 4, st));
     dim3 g(nct, (unsigned)((h->M + 2047) / 2048));
     TimedLaunch tl(5, st);
@@ -738,20 +760,34 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
     g_launches.fetch_add(1);
   }
   {
+    // exponents of X's digits (predicted ones, or -- first step / tiles whose prediction was outgrown -- the true ones with the
+    // digits redone), the prediction for the output, cleared maxima and flags for the launch below
     static std::atomic<uint64_t> attr_seen{0};
     const int smem = S * 64 * 33 * 4;
     if (!attr_done(attr_seen)) {
-      CUDA_TRY(cudaFuncSetAttribute(ttdft::y_digits_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+      CUDA_TRY(cudaFuncSetAttribute(ttdft::y_digits_fix_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
       attr_mark(attr_seen);
     }
-    dim3 g((unsigned)h->nb, nct);
-    TimedLaunch tl(4, st);
-    ttdft::y_digits_kernel<S><<<g, 256, smem, st>>>(X, ldx, h->b, h->M, ncols, cmS, w.D, cmO);
+    if (h->debug >= 2 && have_src) {   // TTDFT_DEBUG=2: how many column tiles outgrew their predicted exponent (synchronises)
+      std::vector<uint32_t> hf(nct);
+      if (cudaMemcpyAsync(hf.data(), w.flags[src], nct * 4, cudaMemcpyDeviceToHost, st) == cudaSuccess && cudaStreamSynchronize(st) == cudaSuccess) {
+        unsigned n = 0;
+        for (uint32_t f : hf) n += f != 0;
+        fprintf(stderr, "[ttdft] K3 digits: %u of %u column tiles redone (prediction outgrown or ragged)\n", n, nct);
+      }
+    }
+    // forced (every tile is extracted): one CTA per (block row, tile); otherwise a small grid whose CTAs walk the block rows of the
+    // rare tile that has to be redone
+    dim3 g((unsigned)(have_src ? std::min<int64_t>(h->nb, 32) : h->nb), nct);
+    TimedLaunch tl(have_src ? 7 : 4, st);
+    ttdft::y_digits_fix_kernel<S><<<g, 256, smem, st>>>(X, ldx, h->b, h->M, ncols, (int32_t)h->nb, cmS, w.D[src], w.flags[src], have_src ? 0 : 1,
+                                                         have_prev ? 1 : 0, h->k3_predict_bias, w.e_used, w.e_pred, w.cmax[src ^ 1],
+                                                         w.flags[src ^ 1]);
     CUDA_TRY(cudaGetLastError());
     g_launches.fetch_add(1);
   }
   CUtensorMap tmYd;
-  ttdft_status s = make_map_yd(&tmYd, w.D, (uint64_t)h->nb * nct * S, (uint32_t)S);
+  ttdft_status s = make_map_yd(&tmYd, w.D[src], (uint64_t)h->nb * nct * S, (uint32_t)S);
   if (s != TTDFT_OK) return s;
   ttdft::K3Params p;
   p.brow_ptr = h->row_ptr; p.bcol = h->col;
@@ -760,9 +796,14 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
   p.ncols = ncols;
   p.alpha = alpha; p.gamma = gamma; p.beta = beta;
   p.S = X; p.lds = ldx; p.Z = Z ? Z : X; p.ldz = Z ? ldz : ldx; p.O = O; p.ldo = ldo;
-  p.eH = h->eH; p.hdiag = h->hdiag; p.cmaxS = cmS; p.cmaxO = cmO;
+  p.eH = h->eH; p.hdiag = h->hdiag; p.eS = w.e_used;
+  p.cmaxO = want_next ? w.cmax[src ^ 1] : nullptr;
+  if (want_next && w.D[src ^ 1]) { p.dO = w.D[src ^ 1]; p.ePredO = w.e_pred; p.flagsO = w.flags[src ^ 1]; }
 #ifdef TTDFT_DEBUG_TRACE
   p.trace = g_k3_trace;
+#endif
+#ifdef TTDFT_EXPERIMENT
+  p.exp = env_int("TTDFT_K3_EXP", 0);
 #endif
   p.l2hints = h->k3_l2hints;
   p.mrows = h->M;
@@ -782,10 +823,10 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
 }
 ttdft_status launch_step_i8(ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
                             const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, const I8Work& w, int src,
-                            bool have_src_max, bool want_out_max, cudaStream_t st) {
+                            bool have_src, bool have_prev, bool want_next, cudaStream_t st) {
   if (i8_planes_in_use(h) == 7)
-    return launch_step_i8_t<7>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, w, src, have_src_max, want_out_max, st);
-  return launch_step_i8_t<6>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, w, src, have_src_max, want_out_max, st);
+    return launch_step_i8_t<7>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, w, src, have_src, have_prev, want_next, st);
+  return launch_step_i8_t<6>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, w, src, have_src, have_prev, want_next, st);
 }
 
 ttdft_status launch_copy2d(const double* src, int64_t lds, double* dst, int64_t ldd, int64_t rows, int64_t cols,
@@ -837,8 +878,8 @@ ttdft_status launch_permute(const double* src, int64_t lds, double* dst, int64_t
 // one step on buffers in tile order, by the handle's math mode
 ttdft_status panel_step(ttdft_h_s* h, double al, double ga, double be, const double* S, int64_t lds, const double* Z, int64_t ldz,
                         double* O, int64_t ldo, int64_t wc, const I8Work* i8, int k, int m, cudaStream_t st) {
-  if (i8)   // column maxima of iterate k-1 live in cmax[(k-1)&1]; the epilogue leaves those of iterate k in the other
-    return launch_step_i8(h, al, ga, be, S, lds, Z, ldz, O, ldo, wc, *i8, (k - 1) & 1, k > 1, k < m, st);
+  if (i8)   // digits, maxima and flags of iterate k-1 live in slot (k-1)&1; the epilogue leaves those of iterate k in the other
+    return launch_step_i8(h, al, ga, be, S, lds, Z, ldz, O, ldo, wc, *i8, (k - 1) & 1, k > 1, k > 1, k < m, st);
   return launch_step(h, al, ga, be, S, lds, Z, ldz, O, ldo, wc, st);
 }
 
@@ -991,9 +1032,9 @@ ttdft_status gram_run(const GramPlan& g, const double* X, int64_t ldx, const dou
       attr_mark(attr_seen);
     }
     { TimedLaunch tl(4, st);
-      ttdft::y_digits_kernel<S><<<dim3((unsigned)g.nbk, (unsigned)g.nctX), 256, smem, st>>>(X, ldx, 128, g.M, g.ncols, cmX, DX, nullptr); }
+      ttdft::y_digits_kernel<S><<<dim3((unsigned)g.nbk, (unsigned)g.nctX), 256, smem, st>>>(X, ldx, 128, g.M, g.ncols, cmX, DX, nullptr, nullptr); }
     { TimedLaunch tl(4, st);
-      ttdft::y_digits_kernel<S><<<dim3((unsigned)g.nbk, (unsigned)g.nctW), 256, smem, st>>>(W, ldw, 128, g.M, g.ncols, cmW, DW, nullptr); }
+      ttdft::y_digits_kernel<S><<<dim3((unsigned)g.nbk, (unsigned)g.nctW), 256, smem, st>>>(W, ldw, 128, g.M, g.ncols, cmW, DW, nullptr, nullptr); }
     CUDA_TRY(cudaGetLastError());
     g_launches.fetch_add(2);
   }
@@ -1054,7 +1095,7 @@ ttdft_status rotate_plan(int64_t M, int64_t K, int64_t N, RotatePlan* r) {
   r->dx = align_up((size_t)r->nbm * r->nkb * GRAM_S * 128 * 128, 1024);
   r->ex = align_up((size_t)r->nbm * 128 * 4, 1024);
   r->dq = align_up((size_t)r->nkb * r->nct * GRAM_S * 64 * 128, 1024);
-  r->cm = align_up((size_t)N * 4, 1024);
+  r->cm = 2 * align_up((size_t)N * 4, 1024);       // column maxima | column exponents
   r->idx = align_up(((size_t)r->nbm + 1) * 4, 1024) + align_up((size_t)r->nbm * r->nkb * 4 + 4, 1024);
   r->total = r->dx + r->ex + r->dq + r->cm + r->idx;
   return TTDFT_OK;
@@ -1071,6 +1112,7 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
   int32_t* eX = reinterpret_cast<int32_t*>(wb + r.dx);
   int8_t* DQ = reinterpret_cast<int8_t*>(wb + r.dx + r.ex);
   uint32_t* cmQ = reinterpret_cast<uint32_t*>(wb + r.dx + r.ex + r.dq);
+  int32_t* eQ = reinterpret_cast<int32_t*>(wb + r.dx + r.ex + r.dq + r.cm / 2);      // exponents of Q's columns, from cmQ
   int32_t* brow = reinterpret_cast<int32_t*>(wb + r.dx + r.ex + r.dq + r.cm);
   int32_t* bcol = reinterpret_cast<int32_t*>(wb + r.dx + r.ex + r.dq + r.cm + align_up(((size_t)r.nbm + 1) * 4, 1024));
   const int64_t Mpad = (int64_t)r.nbm * 128;
@@ -1080,7 +1122,7 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
   const int64_t nidx = std::max<int64_t>((int64_t)r.nbm * r.nkb, (int64_t)r.nbm + 1);
   ttdft::dense_tile_index_kernel<<<(unsigned)((nidx + 255) / 256), 256, 0, st>>>(r.nbm, r.nkb, brow, bcol);
   // B operand: column maxima and digit tiles of Q (its k rows in blocks of 128, ragged tail read as zero)
-  CUDA_TRY(cudaMemsetAsync(cmQ, 0, r.cm, st));
+  CUDA_TRY(cudaMemsetAsync(cmQ, 0, r.cm / 2, st));
   ttdft::colmax_kernel<<<dim3((unsigned)r.nct, (unsigned)((r.K + 2047) / 2048)), 256, 0, st>>>(Q, ldq, r.K, r.N, cmQ);
   {
     static std::atomic<uint64_t> attr_seen{0};
@@ -1089,7 +1131,7 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
       CUDA_TRY(cudaFuncSetAttribute(ttdft::y_digits_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
       attr_mark(attr_seen);
     }
-    ttdft::y_digits_kernel<S><<<dim3((unsigned)r.nkb, (unsigned)r.nct), 256, smem, st>>>(Q, ldq, 128, r.K, r.N, cmQ, DQ, nullptr);
+    ttdft::y_digits_kernel<S><<<dim3((unsigned)r.nkb, (unsigned)r.nct), 256, smem, st>>>(Q, ldq, 128, r.K, r.N, cmQ, DQ, nullptr, eQ);
   }
   CUDA_TRY(cudaGetLastError());
   g_launches.fetch_add(5);
@@ -1111,7 +1153,7 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
   p.nb = r.nbm; p.b = 128; p.nct = r.nct; p.hplanes = S; p.ncols = r.N;
   p.alpha = 1.0; p.gamma = 0.0; p.beta = 0.0;
   p.S = nullptr; p.lds = 0; p.Z = Y; p.ldz = ldy; p.O = Y; p.ldo = ldy;
-  p.eH = eX; p.hdiag = nullptr; p.cmaxS = cmQ; p.cmaxO = nullptr;
+  p.eH = eX; p.hdiag = nullptr; p.eS = eQ; p.cmaxO = nullptr;
   p.vec = 0; p.l2hints = env.k3_l2hints; p.mrows = r.M;
   auto launch_range = [&](int32_t c0, int32_t n, int32_t jlimit) -> ttdft_status {
     p.jlimit = jlimit;
@@ -1617,6 +1659,7 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     const EnvSwitches env = read_env();
     h->k3_cluster = env.k3_cluster;
     h->k3_l2hints = env.k3_l2hints;
+    h->k3_predict_bias = env.k3_predict_bias;
     h->debug = env.debug;
     h->i8_S = I8_S; h->Hd = Hd; h->eH = eH; h->hdiag = hdiag;
     int dev = 0, nsm = 0;
@@ -1697,7 +1740,7 @@ ttdft_status ttdft_cheb_step(ttdft_h_t h, double alpha, double c, double beta, c
 static size_t step_work_need(const ttdft_h_s* h, int64_t ncols, size_t* panel_bytes) {
   const int64_t ldp = ncols + (ncols & 1);
   *panel_bytes = h->perm ? align_up((size_t)h->M * (size_t)ldp * 8, 1024) : 0;
-  return 2 * *panel_bytes + (want_i8(h) ? i8_work_bytes(h, ncols) : 0);
+  return 2 * *panel_bytes + (want_i8(h) ? i8_work_bytes(h, ncols, 1) : 0);
 }
 
 ttdft_status ttdft_step_work_bytes(ttdft_h_t h, int64_t ncols, size_t* bytes) {
@@ -1719,8 +1762,8 @@ static ttdft_status step_ws(ttdft_h_t h, double alpha, double gamma, double beta
   if (!work || (reinterpret_cast<uintptr_t>(work) & 15)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 16-byte aligned device pointer");
   uint8_t* wb = reinterpret_cast<uint8_t*>(work);
   I8Work k3;
-  if (want_i8(h)) k3 = carve_i8_work(h, wb + 2 * pb, ncols);
-  if (!h->perm) return launch_step_i8(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, k3, 0, false, false, st);
+  if (want_i8(h)) k3 = carve_i8_work(h, wb + 2 * pb, ncols, 1);
+  if (!h->perm) return launch_step_i8(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, k3, 0, false, false, false, st);
   // reordered rows: gather the operands into tile order, step there, scatter the result back
   const int64_t ldp = ncols + (ncols & 1);
   double* Xt = reinterpret_cast<double*>(wb);
@@ -1730,7 +1773,7 @@ static ttdft_status step_ws(ttdft_h_t h, double alpha, double gamma, double beta
   const bool use_z = (beta != 0.0) && Z;
   if (use_z && (s = launch_permute(Z, ldz, Ot, ldp, h->M, ncols, h->perm, 0, st)) != TTDFT_OK) return s;
   if (want_i8(h))
-    s = launch_step_i8(h, alpha, gamma, use_z ? beta : 0.0, Xt, ldp, use_z ? Ot : nullptr, ldp, Ot, ldp, ncols, k3, 0, false, false, st);
+    s = launch_step_i8(h, alpha, gamma, use_z ? beta : 0.0, Xt, ldp, use_z ? Ot : nullptr, ldp, Ot, ldp, ncols, k3, 0, false, false, false, st);
   else
     s = launch_step(h, alpha, gamma, use_z ? beta : 0.0, Xt, ldp, use_z ? Ot : nullptr, ldp, Ot, ldp, ncols, st);
   if (s != TTDFT_OK) return s;
@@ -1790,7 +1833,7 @@ ttdft_status ttdft_cheb_filter_work_bytes(ttdft_h_t h, int64_t ncols, int64_t pa
   int64_t w = panel_cols ? std::min(panel_cols, ncols) : default_panel(ncols);
   w += (w & 1);   // even leading dimension keeps the scratch panel TMA / 128-bit friendly
   *bytes = (size_t)h->M * (size_t)w * 8;
-  if (want_i8(h)) *bytes = align_up(*bytes, 1024) + i8_work_bytes(h, w);   // + digit planes of one iterate
+  if (want_i8(h)) *bytes = align_up(*bytes, 1024) + i8_work_bytes(h, w, 2);   // + digit planes of two iterates (read / being written)
   return TTDFT_OK;
 }
 
@@ -1820,7 +1863,7 @@ ttdft_status ttdft_cheb_filter(ttdft_h_t h, const double* X, int64_t ldx, double
   const int64_t w = panel_cols ? std::min(panel_cols, ncols) : default_panel(ncols);
   const int64_t ldw = w + (w & 1);
   I8Work k3;
-  if (i8) k3 = carve_i8_work(h, reinterpret_cast<uint8_t*>(work) + align_up((size_t)h->M * (size_t)ldw * 8, 1024), ldw);
+  if (i8) k3 = carve_i8_work(h, reinterpret_cast<uint8_t*>(work) + align_up((size_t)h->M * (size_t)ldw * 8, 1024), ldw, 2);
   for (int64_t c0 = 0; c0 < ncols; c0 += w) {
     const int64_t wc = std::min(w, ncols - c0);
     s = filter_panel(h, X + c0, ldx, Y + c0, ldy, reinterpret_cast<double*>(work), ldw, wc, m, c, alpha.data(), beta.data(),
@@ -1836,7 +1879,7 @@ ttdft_status ttdft_cheb_filter_host_work_bytes(ttdft_h_t h, int64_t ncols, int64
   int64_t w = panel_cols ? std::min(panel_cols, ncols) : std::min<int64_t>(ncols, 1024);
   w += (w & 1);
   *bytes = 5 * align_up((size_t)h->M * (size_t)w * 8, 1024);   // 2 x (X panel, Y panel) + scratch
-  if (want_i8(h)) *bytes += i8_work_bytes(h, w);
+  if (want_i8(h)) *bytes += i8_work_bytes(h, w, 2);
   return TTDFT_OK;
 }
 
@@ -1865,7 +1908,7 @@ ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* Xh, int64_t ldx, 
   double* dW = reinterpret_cast<double*>(base + 4 * pbytes);
   const bool i8 = want_i8(h) && m >= 1 && h->M > 0;
   I8Work k3;
-  if (i8) k3 = carve_i8_work(h, base + 5 * pbytes, ldw);
+  if (i8) k3 = carve_i8_work(h, base + 5 * pbytes, ldw, 2);
 
   cudaStream_t sc = (cudaStream_t)stream, sin = nullptr, sout = nullptr;
   cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr}, ev_start = nullptr;

@@ -344,3 +344,82 @@ def test_degree20_wide_gap_b128(tt, mode):
         e, w = relerr(got, ref), worst_col_relerr(got, ref)
         print(f"m=20 wide gap b=128 {mode} inplace={inplace}: {e:.2e} worst col {w:.2e}")
         assert e <= TOL_FILTER and w <= 10 * TOL_FILTER
+
+
+def _filter_with_env(tt, H, X, m, a, b, a0, env, mode="i8x7", panel=0):
+    """Build (the handle reads the environment switches) and filter under the given environment."""
+    import os
+    import torch
+    old = {k: os.environ.get(k) for k in env}
+    os.environ.update(env)
+    try:
+        Hd = build_i8(tt, H, mode=mode)
+    finally:
+        for k, v in old.items():
+            if v is None:
+                os.environ.pop(k, None)
+            else:
+                os.environ[k] = v
+    Y = torch.empty(H.M, X.shape[1], dtype=torch.float64, device="cuda")
+    tt.cheb_filter(Hd, dev(X), Y, m, a, b, a0, panel_cols=panel)
+    return Y.cpu().numpy()
+
+
+@pytest.mark.parametrize("G,b,N", [(3, 128, 200), (3, 64, 150), (2, 96, 100)])
+@pytest.mark.parametrize("wide", [False, True])
+def test_epilogue_digits_prediction_and_fallback(tt, G, b, N, wide):
+    """From the second step on K3's epilogue writes the next iterate's digit planes itself with a PREDICTED column exponent
+    (K3 "digits from the epilogue"); tiles whose prediction is outgrown are redone from the fp64 iterate.  The
+    prediction path (default), the all-fallback path (bias -6: every prediction fails, i.e. the true exponents of the former
+    design) and a pessimistic prediction (bias +3: three bits fewer) must all meet the filter tolerance."""
+    H, C, (rp, col, val), (a0, bb) = small_problem(G, b, 0.4, 2400 + b)
+    m = 12
+    a, bb, a0 = bounds_for(a0, bb, N, H.M, wide=wide)
+    X = synth.dense_normal(H.M, N, 97)
+    ref = oracle.cheb_filter(rp, col, val, X, m, a, bb, a0)
+    for bias in ("0", "-6", "3"):
+        got = _filter_with_env(tt, H, X, m, a, bb, a0, {"TTDFT_K3_PREDICT_BIAS": bias}, panel=128)
+        e, w = relerr(got, ref), worst_col_relerr(got, ref)
+        print(f"epilogue digits G={G} b={b} wide={wide} bias={bias}: {e:.2e} worst col {w:.2e}")
+        assert e <= TOL_FILTER and w <= 10 * TOL_FILTER
+        if bias != "3":
+            assert e <= 50 * ACC["i8x7"]                      # no precision lost to the prediction beyond a guard bit or two
+
+
+def test_column_that_grows_past_its_prediction(tt):
+    """A column whose iterate nearly vanishes at step 1 and comes back at step 2 (X_j = e_i for a row i of H that holds only its
+    diagonal entry c: (H - c) e_i = 0 up to rounding, then Y_2 = beta_1 X + ...): the predicted exponent of Y_2 is ~50 binary
+    orders too small, the column's tile must be redone and the result still match the oracle; so must columns next to it."""
+    import copy
+    import torch
+    H0, _, _, (a0, bb) = small_problem(3, 64, 0.3, 2064)
+    N, m = 70, 10                                            # even degree: p_m(c) = +-1 / T_m(t0) != 0
+    a, bb, a0 = bounds_for(a0, bb, N, H0.M)
+    c = 0.5 * (a + bb)
+    rows = [5, 700]                                          # rows that keep only their diagonal entry, set to c
+    vals = H0.values.copy().reshape(H0.nblocks, H0.b, H0.b)
+    tile_row = np.repeat(np.arange(H0.M // H0.b), np.diff(H0.row_ptr))
+    for p in range(H0.nblocks):
+        I, J = int(tile_row[p]), int(H0.col_idx[p])
+        for r in rows:
+            if I == r // H0.b:
+                vals[p][r % H0.b, :] = 0.0
+            if J == r // H0.b:
+                vals[p][:, r % H0.b] = 0.0
+            if I == J == r // H0.b:
+                vals[p][r % H0.b, r % H0.b] = c
+    H = copy.copy(H0)
+    H.values = vals.reshape(H0.values.shape)
+    rp, col, val = oracle.bsr_to_csr(H.b, H.row_ptr, H.col_idx, H.values)
+    X = synth.dense_normal(H.M, N, 99)
+    X[:, 3] = 0.0
+    X[rows[0], 3] = 1.0                                      # column 3 = e_5; column 66 (ragged last tile) = 2 e_700
+    X[:, 66] = 0.0
+    X[rows[1], 66] = 2.0
+    ref = oracle.cheb_filter(rp, col, val, X, m, a, bb, a0)
+    assert abs(ref[rows[0], 3]) > 1e-3                        # the column does come back
+    for mode in ("i8x7", "i8"):
+        got = _filter_with_env(tt, H, X, m, a, bb, a0, {}, mode=mode)
+        e, w = relerr(got, ref), worst_col_relerr(got, ref)
+        print(f"vanishing column {mode}: {e:.2e} worst col {w:.2e}")
+        assert e <= TOL_FILTER and w <= 10 * TOL_FILTER
