@@ -172,14 +172,15 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&r)[8]) {
 // fp64 instructions are scarce while the tensor pipe runs int8 MMAs (ncu: "math pipe throttle" on every DFMA of
 // the epilogue), so three int32 levels are packed EXACTLY into one int64 (|L| < 2^31: L_a*2^16 + L_b*2^8 + L_c
 // < 2^48) before the conversion: ceil(S/3) conversions and ceil(S/3)-1 FMAs per element instead of S and S-1.
-template <int S, int NC>
+// LS: TMEM columns between two levels (the width of a work item's accumulator block).
+template <int S, int NC, int LS = K3_NT>
 __device__ __forceinline__ void k3_drain(uint32_t trow, double (&v)[NC]) {   // trow: TMEM address of the first column
   constexpr int NG = (S + 2) / 3;
 #pragma unroll
   for (int c = 0; c < NC / 8; ++c) {
     uint32_t a[S][8];
 #pragma unroll
-    for (int g = 0; g < S; ++g) tmem_ld8(trow + (uint32_t)(g * K3_NT + c * 8), a[g]);
+    for (int g = 0; g < S; ++g) tmem_ld8(trow + (uint32_t)(g * LS + c * 8), a[g]);
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
     for (int i = 0; i < 8; ++i) {

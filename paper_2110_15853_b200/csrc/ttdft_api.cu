@@ -20,6 +20,7 @@
 #include "../../include/ttdft.h"
 #include "bsr_dmma.cuh"
 #include "bsr_i8.cuh"
+#include "bsr_i8t.cuh"
 #include "generic_spmm.cuh"
 #include "cholesky.cuh"
 #include "gram_i8.cuh"
@@ -145,6 +146,21 @@ ttdft_status make_map_hd(CUtensorMap* map, const void* base, uint64_t rows, uint
   if (r != CUDA_SUCCESS) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled(H digits) failed with CUresult %d", (int)r);
   return TTDFT_OK;
 }
+// H digit planes as a 3-D tensor {128 B, b rows, tiles x stored planes}, box = {128 B, box_rows, box_planes}: one load brings the
+// leading planes of a row half of a tile (kernel K3T)
+ttdft_status make_map_hd3(CUtensorMap* map, const void* base, uint32_t b, uint64_t ntile_planes, uint32_t box_rows, uint32_t box_planes) {
+  encode_tiled_fn enc = get_encode();
+  if (!enc) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  cuuint64_t dims[3] = {128, b, ntile_planes};
+  cuuint64_t strides[2] = {128, 128 * (cuuint64_t)b};
+  cuuint32_t box[3] = {128, box_rows, box_planes};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(TTDFT_ERR_CUDA, "cuTensorMapEncodeTiled(H digits, 3-D) failed with CUresult %d", (int)r);
+  return TTDFT_OK;
+}
 // Y digit tiles: uint8 [nb*nct*S][64 columns][128 k-bytes], box = S x 64 x 128 B, 128B swizzle
 ttdft_status make_map_yd(CUtensorMap* map, const void* base, uint64_t ntile_planes, uint32_t S) {
   encode_tiled_fn enc = get_encode();
@@ -209,6 +225,9 @@ struct ttdft_h_s {
   const int32_t* eH = nullptr;    // [M]
   const double* hdiag = nullptr;  // [M]
   CUtensorMap tmHd[4];      // box rows b, b/2, b/4, b/8: K3 in clusters of 1, 2, 4, 8 CTAs (every CTA fetches b/C rows of a plane)
+  CUtensorMap tmH3[2];      // K3T: 3-D boxes {128 B, b/2 rows, 7 | 6 planes}
+  int32_t k3t = 0;          // 1: the int8 step runs on the transposed kernel K3T (tiles narrower than 128; env TTDFT_K3_T forces 0 / 1)
+  int32_t k3t_max_clusters = 0;
   int32_t nsm = 148;
   int32_t sym_checked = 0;         // TTDFT_CHECK_SYMMETRY passed at build: H == H^T bit for bit
   const int32_t* perm = nullptr;   // rows reordered by subdomain label: row r of the tiles is the caller's row perm[r]
@@ -492,7 +511,7 @@ int env_int(const char* name, int dflt) {
 // ttdft_h_build into the handle, and at the entry of the handle-less calls (ttdft_gram / _rotate / _orthonormalize and
 // ttdft_project's Gram product) -- never inside a launch path.
 struct EnvSwitches {
-  int math, k3_cluster, k3_l2hints, k3_predict_bias, k4_cluster, debug;
+  int math, k3_cluster, k3_l2hints, k3_predict_bias, k3_t, k4_cluster, debug;
 };
 EnvSwitches read_env() {
   EnvSwitches e;
@@ -502,6 +521,7 @@ EnvSwitches read_env() {
   e.k3_l2hints = env_int("TTDFT_K3_L2HINTS", -1);
   e.k3_predict_bias = env_int("TTDFT_K3_PREDICT_BIAS", 0);
   if (e.k3_predict_bias < -64 || e.k3_predict_bias > 8) e.k3_predict_bias = 0;
+  e.k3_t = env_int("TTDFT_K3_T", -1);
   e.k4_cluster = env_int("TTDFT_K4_CLUSTER", 2) == 1 ? 1 : 2;
   e.debug = env_int("TTDFT_DEBUG", 0);
   return e;
@@ -624,19 +644,23 @@ int i8_planes_in_use(const ttdft_h_s* h) {
   return 0;
 }
 bool want_i8(const ttdft_h_s* h) { return i8_planes_in_use(h) > 0; }
-// digit tiles of one iterate: [nb][ceil(w/64)][planes][64][128] bytes
+// 64-column digit tiles of a w-column panel (K3T works on pairs of them: an even count, the last one all zero if need be)
+size_t i8_nct(const ttdft_h_s* h, int64_t w) {
+  if (h->k3t) return 2 * (size_t)((w + ttdft::K3T_NT - 1) / ttdft::K3T_NT);
+  return (size_t)((w + ttdft::K3_NT - 1) / ttdft::K3_NT);
+}
+// digit tiles of one iterate: [nb][tiles][planes][64][128] bytes
 size_t i8_digit_bytes(const ttdft_h_s* h, int64_t w) {
-  const size_t nct = (size_t)((w + ttdft::K3_NT - 1) / ttdft::K3_NT);
-  return align_up((size_t)i8_planes_in_use(h) * nct * ttdft::K3_NT * (size_t)h->nb * 128, 1024);
+  return align_up((size_t)i8_planes_in_use(h) * i8_nct(h, w) * ttdft::K3_NT * (size_t)h->nb * 128, 1024);
 }
 // nbuf = 2 for the filter (K3's epilogue writes the next iterate's digits while the current ones are being read), 1 for a single step
 size_t i8_work_bytes(const ttdft_h_s* h, int64_t w, int nbuf) {
-  const size_t nct = (size_t)((w + ttdft::K3_NT - 1) / ttdft::K3_NT);
+  const size_t nct = i8_nct(h, w);
   return (size_t)nbuf * i8_digit_bytes(h, w) + 4 * align_up((size_t)w * 4, 1024) + 2 * align_up(nct * 4, 1024);
 }
 I8Work carve_i8_work(const ttdft_h_s* h, void* base, int64_t w, int nbuf) {
   I8Work k;
-  const size_t nct = (size_t)((w + ttdft::K3_NT - 1) / ttdft::K3_NT);
+  const size_t nct = i8_nct(h, w);
   uint8_t* p = reinterpret_cast<uint8_t*>(base);
   k.D[0] = reinterpret_cast<int8_t*>(p);
   p += i8_digit_bytes(h, w);
@@ -724,6 +748,44 @@ ttdft_status launch_k3(ttdft_h_s* h, const CUtensorMap& tmYd, ttdft::K3Params p,
   return TTDFT_OK;
 }
 
+// one K3T launch over all 128-column tiles of the panel (p.nct = 64-column digit tiles, even), clusters of 2 CTAs = the two row halves
+template <int S, int HR>
+ttdft_status launch_k3t(ttdft_h_s* h, const CUtensorMap& tmY4, ttdft::K3Params p, cudaStream_t st) {
+  auto kern = ttdft::bsr_i8t_kernel<S, HR>;
+  using Cf = ttdft::K3TCfg<S, HR>;
+  static std::atomic<uint64_t> attr_seen{0};
+  if (!attr_done(attr_seen)) {
+    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cf::TOTAL));
+    attr_mark(attr_seen);
+  }
+  cudaLaunchConfig_t cfg = cudaLaunchConfig_t{};
+  cudaLaunchAttribute at[1];
+  cfg.blockDim = dim3(ttdft::K3_THREADS);
+  cfg.dynamicSmemBytes = Cf::TOTAL;
+  cfg.stream = st;
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  if (h->k3t_max_clusters <= 0) {
+    int q = 0;
+    cfg.gridDim = dim3((unsigned)(h->nsm / 2 * 2));
+    if (cudaOccupancyMaxActiveClusters(&q, kern, &cfg) == cudaSuccess && q > 0) h->k3t_max_clusters = std::min(q, h->nsm / 2);
+    else { (void)cudaGetLastError(); h->k3t_max_clusters = std::max(1, h->nsm / 2); }
+    if (h->debug) fprintf(stderr, "[ttdft] K3T<%d,%d>: %d co-resident clusters on %d SMs\n", S, HR, h->k3t_max_clusters, h->nsm);
+  }
+  p.ct_begin = 0;
+  p.nctg = p.nct / 2;
+  p.cgc = 1;                       // clusters walk consecutive block rows on the same column tile and share Y digit tiles through L2
+  if (p.l2hints < 0) p.l2hints = 1;
+  const int64_t items = (int64_t)h->nb * p.nctg;
+  cfg.gridDim = dim3((unsigned)(std::min<int64_t>(items, h->k3t_max_clusters) * 2));
+  TimedLaunch tl(3, st);
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, h->tmH3[S == 7 ? 0 : 1], tmY4, p));
+  g_launches.fetch_add(1);
+  return TTDFT_OK;
+}
+
 // Cluster size of K3: the widest of {4, 2, 1} whose co-resident clusters still cover at least 98 % of the SMs
 // (b/C rows per CTA must be whole 8-row swizzle atoms).  On B200 only 33 four-CTA clusters are co-resident
 // (132 of 148 SMs: GPCs whose SM count is not a multiple of 4 leave SMs idle), so this picks 2.  Measured on
@@ -749,7 +811,7 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
                               const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, const I8Work& w, int src,
                               bool have_src, bool have_prev, bool want_next, cudaStream_t st) {
   if (h->M == 0) return TTDFT_OK;
-  const unsigned nct = (unsigned)((ncols + ttdft::K3_NT - 1) / ttdft::K3_NT);
+  const unsigned nct = (unsigned)i8_nct(h, ncols);
   uint32_t* cmS = w.cmax[src];
   if (!have_src) {
     CUDA_TRY(cudaMemsetAsync(cmS, 0, (size_t)ncols * 4, st));
@@ -787,7 +849,8 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
     g_launches.fetch_add(1);
   }
   CUtensorMap tmYd;
-  ttdft_status s = make_map_yd(&tmYd, w.D[src], (uint64_t)h->nb * nct * S, (uint32_t)S);
+  ttdft_status s = h->k3t ? make_map_xd4(&tmYd, w.D[src], (uint64_t)h->nb * nct, (uint32_t)S, 64u)
+                          : make_map_yd(&tmYd, w.D[src], (uint64_t)h->nb * nct * S, (uint32_t)S);
   if (s != TTDFT_OK) return s;
   ttdft::K3Params p;
   p.brow_ptr = h->row_ptr; p.bcol = h->col;
@@ -809,6 +872,14 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
   p.mrows = h->M;
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
+  if (h->k3t) {
+    switch (h->b) {
+      case 64: return launch_k3t<S, 32>(h, tmYd, p, st);
+      case 96: return launch_k3t<S, 48>(h, tmYd, p, st);
+      case 128: return launch_k3t<S, 64>(h, tmYd, p, st);
+      default: return fail(TTDFT_ERR_UNSUPPORTED, "K3T: tile size %d", h->b);
+    }
+  }
   // column tiles in clusters of C; a remainder of < C tiles runs as single CTAs
   int C = k3_pick_cluster<S>(h);
   while (C > 1 && (h->b % (8 * C) != 0 || (int)nct < C)) C >>= 1;
@@ -1657,6 +1728,15 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
       if (s != TTDFT_OK) { delete h; return s; }
     }
     const EnvSwitches env = read_env();
+    // the transposed kernel K3T for tiles narrower than the MMA's M = 128 (no padding rows are multiplied there)
+    h->k3t = (env.k3_t == 0 || env.k3_t == 1) ? env.k3_t : (h->b == 96 ? 1 : 0);
+    if (h->b != 64 && h->b != 96 && h->b != 128) h->k3t = 0;
+    if (h->k3t) {
+      for (int si = 0; si < 2; ++si) {
+        s = make_map_hd3(&h->tmH3[si], Hd, (uint32_t)h->b, (uint64_t)h->nblocks * I8_S, (uint32_t)(h->b / 2), (uint32_t)(7 - si));
+        if (s != TTDFT_OK) { delete h; return s; }
+      }
+    }
     h->k3_cluster = env.k3_cluster;
     h->k3_l2hints = env.k3_l2hints;
     h->k3_predict_bias = env.k3_predict_bias;

@@ -423,3 +423,39 @@ def test_column_that_grows_past_its_prediction(tt):
         e, w = relerr(got, ref), worst_col_relerr(got, ref)
         print(f"vanishing column {mode}: {e:.2e} worst col {w:.2e}")
         assert e <= TOL_FILTER and w <= 10 * TOL_FILTER
+
+
+@pytest.mark.parametrize("mode", ["i8x7", "i8"])
+@pytest.mark.parametrize("G,b,N", [(3, 96, 330), (2, 96, 100), (3, 64, 200), (3, 128, 257), (2, 128, 64)])
+def test_transposed_kernel_k3t(tt, G, b, N, mode):
+    """Kernel K3T (the tile's rows on the N axis of the MMA, columns of Y on M: the default for 96-wide tiles, TTDFT_K3_T=1
+    elsewhere) against the oracle and against kernel K3 (TTDFT_K3_T=0): the integer sums and the epilogue arithmetic are the same,
+    so the two kernels must agree bit for bit -- ragged column counts, single steps and whole filters."""
+    import os
+    import torch
+    H, C, (rp, col, val), (a0, bb) = small_problem(G, b, 0.4, 2500 + b)
+    m = 7
+    a, bb, a0 = bounds_for(a0, bb, N, H.M, wide=True)
+    X = synth.dense_normal(H.M, N, 101)
+    Z = synth.dense_normal(H.M, N, 102)
+    ref = oracle.cheb_filter(rp, col, val, X, m, a, bb, a0)
+    ref_step = oracle.cheb_step(rp, col, val, 0.173, 9.5, -0.31, X, Z)
+    out = {}
+    for t in ("0", "1"):
+        os.environ["TTDFT_K3_T"] = t
+        try:
+            Hd = build_i8(tt, H, mode=mode)
+        finally:
+            os.environ.pop("TTDFT_K3_T", None)
+        Y = torch.full((H.M, N + 3), float("nan"), dtype=torch.float64, device="cuda")
+        tt.cheb_filter(Hd, dev(X), Y[:, :N], m, a, bb, a0, panel_cols=256)
+        O = torch.empty(H.M, N, dtype=torch.float64, device="cuda")
+        tt.cheb_step(Hd, 0.173, 9.5, -0.31, dev(X), dev(Z), O, use_work=True)
+        assert torch.isnan(Y[:, N:]).all()                    # nothing written outside the view
+        out[t] = (Y[:, :N].cpu().numpy(), O.cpu().numpy())
+        assert relerr(out[t][0], ref) <= TOL_FILTER and worst_col_relerr(out[t][0], ref) <= 10 * TOL_FILTER
+        assert relerr(out[t][1], ref_step) <= ACC[mode]
+    assert np.array_equal(out["0"][1], out["1"][1])
+    full = N // 64 * 64          # K3 redoes a ragged last 64-column tile with the true exponents, K3T keeps the predicted ones there
+    assert np.array_equal(out["0"][0][:, :full], out["1"][0][:, :full])
+    assert relerr(out["0"][0], out["1"][0]) <= 1e-14
