@@ -191,7 +191,8 @@ def workload_config(cfg, nnz, nblocks, args):
         "M": cfg.M, "N": cfg.N, "m": cfg.m, "block": cfg.b, "nblocks": nblocks, "nnz": nnz,
         "panel_cols": args.panel if args.panel else cfg.panel,
         "l2": "inputs larger than L2 (H %.2f GB, X %.2f GB per rank)" % (nblocks * cfg.b * cfg.b * 8 / 1e9, cfg.M * cfg.N * 8 / 1e9),
-        "parallelism": f"band x{args.gpus} (H replicated, columns sharded, no collective)",
+        "parallelism": f"band x{args.gpus} (H replicated, columns sharded, no collective); "
+                       + ("weak: every rank filters N columns" if getattr(args, "scaling", "weak") == "weak" else "strong: N columns cut into bands"),
     }
 
 
@@ -203,6 +204,9 @@ def main():
     ap.add_argument("--workload", default="si", choices=list(synth.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--panel", type=int, default=0, help="column-panel width (0 = config default)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank filters its own N-column band (total work grows with N); strong = the config's N "
+                         "columns are cut into N bands (e.g. --workload largest: 14,336 columns).  H is replicated either way.")
     ap.add_argument("--ref-cols", type=int, default=0,
                     help="columns in the oracle sample; 0 = 48 for the cpu_baseline leg (about 18 s on 16 host cores) and 16 per step "
                          "for --impl reference (about 6 s per step, so that any --steps/--warmup ends within a few minutes)")
@@ -254,12 +258,18 @@ def main():
     planes = {tt.MATH_I8: 6, tt.MATH_I8X7: 7}.get(info["math"], 0)
     mode_name = {tt.MATH_FP64: "fp64", tt.MATH_I8: "i8", tt.MATH_I8X7: "i8x7"}[info["math"]]
 
-    # this rank's band of wavefunctions: columns [rank*N, (rank+1)*N) of the global block (host, pinned)
-    Xh = torch.empty((cfg.M, cfg.N), dtype=torch.float64).pin_memory()
+    # this rank's band of wavefunctions (host, pinned).  weak: columns [rank*N, (rank+1)*N) of a global block of world*N columns;
+    # strong: the config's own N columns cut into `world` bands (PAPER.md:L258 band parallelism, paper's partition rule L244-248)
     from paper_2110_15853_b200 import bands
-    band0, _ = bands.weak_band(rank, cfg.N)
-    synth.dense_normal(cfg.M, cfg.N, cfg.seed, synth.STREAM_X, col0=band0, out=Xh.numpy())
-    Yh = torch.empty((cfg.M, cfg.N), dtype=torch.float64).pin_memory()
+    if args.scaling == "strong":
+        band0, ncols = bands.band_of(rank, world, cfg.N)
+        total_cols = cfg.N
+    else:
+        band0, ncols = bands.weak_band(rank, cfg.N)
+        total_cols = cfg.N * world
+    Xh = torch.empty((cfg.M, ncols), dtype=torch.float64).pin_memory()
+    synth.dense_normal(cfg.M, ncols, cfg.seed, synth.STREAM_X, col0=band0, out=Xh.numpy())
+    Yh = torch.empty((cfg.M, ncols), dtype=torch.float64).pin_memory()
     Xd = Xh.to(dev, non_blocking=True)
     Yd = torch.empty_like(Xd)
     panel = args.panel if args.panel else cfg.panel
@@ -270,10 +280,10 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    npanels = -(-cfg.N // (panel if panel else min(cfg.N, 4096)))
-    useful = 2.0 * nnz * cfg.N * cfg.m                                   # flops of the method: non-zeros of H only
-    executed = 2.0 * H.nblocks * cfg.b * cfg.b * cfg.N * cfg.m           # what dense tiles multiply (explicit zeros included)
-    alg_bytes = cfg.m * (npanels * 8.0 * nnz + 24.0 * cfg.M * cfg.N) - 8.0 * cfg.M * cfg.N
+    npanels = -(-ncols // (panel if panel else min(ncols, 4096)))
+    useful = 2.0 * nnz * ncols * cfg.m                                   # flops of the method: non-zeros of H only
+    executed = 2.0 * H.nblocks * cfg.b * cfg.b * ncols * cfg.m           # what dense tiles multiply (explicit zeros included)
+    alg_bytes = cfg.m * (npanels * 8.0 * nnz + 24.0 * cfg.M * ncols) - 8.0 * cfg.M * ncols
     hbm_bw, hbm_src = hbm_peak_gbs()
     t_roof = max(alg_bytes / (hbm_bw * 1e9), useful / (FP64_PEAK_TFLOPS * 1e12))   # SURVEY.md 8(d) (iv), whole filter
     binds = "fp64" if useful / (FP64_PEAK_TFLOPS * 1e12) >= alg_bytes / (hbm_bw * 1e9) else "hbm"
@@ -282,7 +292,7 @@ def main():
         """W warm-up + K timed ttdft_cheb_filter calls in one math mode: device time (max over ranks), the library's own CUDA
         event pairs per kernel, clocks sampled during the timed region, kernel launches counted by the library."""
         Hd.set_math_mode(mode)
-        work = torch.empty(tt.cheb_filter_work_bytes(Hd, cfg.N, panel) + 16, dtype=torch.uint8, device=dev)
+        work = torch.empty(tt.cheb_filter_work_bytes(Hd, ncols, panel) + 16, dtype=torch.uint8, device=dev)
 
         def step():
             tt.cheb_filter(Hd, Xd, Yd, cfg.m, a, b, a0, panel_cols=panel, work=work)
@@ -334,8 +344,8 @@ def main():
             # Algorithmic ops per launch = 2 * pairs * nnz * N (non-zeros only); executed = dense tiles, padded to the MMA shape.
             pairs = planes * (planes + 1) // 2
             peak, peak_src = int8_peak_tops()
-            ops_launch = 2.0 * pairs * nnz * cfg.N / npanels
-            ops_exec = 2.0 * pairs * H.nblocks * 128 * cfg.b * (-(-cfg.N // 64) * 64) / npanels
+            ops_launch = 2.0 * pairs * nnz * ncols / npanels
+            ops_exec = 2.0 * pairs * H.nblocks * 128 * cfg.b * (-(-ncols // 64) * 64) / npanels
             roof = {"bound": "tensor", "achieved": ops_launch / t_launch / 1e12, "peak": peak, "unit": "TFLOP/s",
                     "frac": ops_launch / t_launch / 1e12 / peak, "kernel": "ttdft::bsr_i8_kernel", "peak_source": peak_src,
                     "ops": f"int8 multiply-add = 2 ops; {pairs} digit-plane products per fp64 product ({planes} planes per operand: "
@@ -365,14 +375,14 @@ def main():
         roof["peak_measured_dmma"] = tt.probe_fp64_peak(1, 300)
     except Exception:
         pass
-    cols_d = torch.from_numpy(synth.column_sample(cfg.N, cfg.panel, args.ref_cols, cfg.seed)).to(dev)
+    cols_d = torch.from_numpy(synth.column_sample(ncols, cfg.panel, args.ref_cols, cfg.seed)).to(dev)
     samples = {mode_name: Yd[:, cols_d].clone()}
     Yd_headline = Yd.clone() if not args.no_e2e else None
 
     line = {
-        "metric": "ChFSI filter useful fp64 GFLOP/s", "value": useful * world / t_step / 1e9, "unit": "GFLOP/s",
+        "metric": "ChFSI filter useful fp64 GFLOP/s", "value": 2.0 * nnz * total_cols * cfg.m / t_step / 1e9, "unit": "GFLOP/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_step * 1e3,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": DTYPE[mode_name], "data": "synthetic",
+        "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None, "dtype": DTYPE[mode_name], "data": "synthetic",
         "config": workload_config(cfg, nnz, H.nblocks, args),      # the same object the reference arm prints
         "math": (f"{mode_name}: exact int8 digit planes on tcgen05 ({planes} x 8 bit per fp64 operand = "
                  f"{8 * planes - 1} bits below the row/column maximum, exact int32 accumulation, fp64 "
@@ -388,7 +398,7 @@ def main():
         samples["fp64"] = Yd[:, cols_d].clone()
         line["fp64_native"] = {
             "what": "the same filter in TTDFT_MATH_FP64: every product on the fp64 tensor-core pipe (DMMA), no digit planes",
-            "metric": line["metric"], "value": useful * world / r64["t_step"] / 1e9, "unit": "GFLOP/s", "dtype": DTYPE["fp64"],
+            "metric": line["metric"], "value": 2.0 * nnz * total_cols * cfg.m / r64["t_step"] / 1e9, "unit": "GFLOP/s", "dtype": DTYPE["fp64"],
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": r64["t_step"] * 1e3, "clocks": r64["clocks"],
             "gpu_launches": r64["launches"], "roofline": mode_report(r64, False, 0)}
         others["fp64"] = line["fp64_native"]
@@ -396,7 +406,7 @@ def main():
     # ---- end to end through the C-ABI host-buffer call: H2D of X and D2H of Y inside the timed region
     if not args.no_e2e:
         Hd.set_math_mode(MODES[args.math])
-        hwork = torch.empty(tt.cheb_filter_host_work_bytes(Hd, cfg.N, 1024) + 1024, dtype=torch.uint8, device=dev)
+        hwork = torch.empty(tt.cheb_filter_host_work_bytes(Hd, ncols, 1024) + 1024, dtype=torch.uint8, device=dev)
         tt.cheb_filter_host(Hd, Xh, Yh, cfg.m, a, b, a0, panel_cols=1024, work=hwork)   # warm-up
         barrier()
         t0 = time.perf_counter()
@@ -409,8 +419,8 @@ def main():
             tm = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
             dist.all_reduce(tm, op=dist.ReduceOp.MAX)
             t_e2e = float(tm.item())
-        line["e2e"] = {"value": 2.0 * nnz * cfg.N * cfg.m * world / t_e2e / 1e9, "unit": "GFLOP/s",
-                       "h2d_bytes_per_step": cfg.M * cfg.N * 8, "d2h_bytes_per_step": cfg.M * cfg.N * 8,
+        line["e2e"] = {"value": 2.0 * nnz * total_cols * cfg.m / t_e2e / 1e9, "unit": "GFLOP/s",
+                       "h2d_bytes_per_step": cfg.M * ncols * 8, "d2h_bytes_per_step": cfg.M * ncols * 8,
                        "ms_per_step": t_e2e * 1e3, "api": "ttdft_cheb_filter_host (pinned host X, Y; 1024-column panels)",
                        # sanity: the host path and the device path agree bit for bit on this rank's band
                        "matches_device_path": bool(torch.equal(Yh.to(dev), Yd_headline))}
@@ -422,7 +432,7 @@ def main():
             if name == mode_name or not info["i8_planes"]:
                 continue
             Hd.set_math_mode(MODES[name])
-            w2 = torch.empty(tt.cheb_filter_work_bytes(Hd, cfg.N, panel) + 16, dtype=torch.uint8, device=dev)
+            w2 = torch.empty(tt.cheb_filter_work_bytes(Hd, ncols, panel) + 16, dtype=torch.uint8, device=dev)
             tt.cheb_filter(Hd, Xd, Yd, cfg.m, a, b, a0, panel_cols=panel, work=w2)
             torch.cuda.synchronize()
             f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

@@ -92,3 +92,42 @@ def test_row_sharded_filter_lockstep_emulation(tt):
     Yf = torch.empty_like(Xd)
     tt.cheb_filter(Hf, Xd, Yf, m, a, bq, a0q)
     assert relerr(Y.cpu().numpy(), Yf.cpu().numpy()) <= 1e-13
+
+
+@pytest.mark.parametrize("G,b,world,mode", [(4, 32, 2, "fp64"), (4, 64, 2, "fp64"), (4, 64, 2, "i8x7")])
+def test_interior_and_boundary_handles(tt, G, b, world, mode):
+    """The overlapped row partition runs two handles per rank: interior block rows (tiles only inside the slab) and boundary ones.
+    Their steps fill disjoint rows and together equal the full handle's step bit for bit; the interior step of the fp64 kernel reads
+    no row outside the slab (remote rows poisoned with NaN).  The int8 modes scale by whole-column maxima, i.e. they need the
+    complete iterate and are not eligible for the overlap -- they are only checked on complete data here."""
+    import torch
+    H, C, _, _ = small_problem(G, b, 0.3, 9300 + b)
+    nb = H.M // H.b
+    MODE = {"fp64": tt.MATH_FP64, "i8x7": tt.MATH_I8X7}[mode]
+    Hf = tt.h_build_bsr(H.M, H.b, dev(H.row_ptr), dev(H.col_idx), dev(H.values)).set_math_mode(MODE)
+    N = 40
+    Yk, Ykm1 = dev(synth.dense_normal(H.M, N, 94)), dev(synth.dense_normal(H.M, N, 95))
+    alpha, c, beta = 0.37, 9.5, -0.81
+    full = torch.empty_like(Yk)
+    tt.cheb_step(Hf, alpha, c, beta, Yk, Ykm1, full, use_work=True)
+    got = torch.full_like(Yk, float("nan"))
+    for r in range(world):
+        I0, n = rows.slab_of(r, world, nb)
+        (rpi, cii, vai), (rpb, cib, vab), mask = rows.split_slab(H.row_ptr, H.col_idx, H.values, I0, n)
+        assert 0 < mask.sum() < n
+        Hi = tt.h_build_bsr(H.M, H.b, dev(rpi), dev(cii), dev(vai)).set_math_mode(MODE)
+        Hb = tt.h_build_bsr(H.M, H.b, dev(rpb), dev(cib), dev(vab)).set_math_mode(MODE)
+        rows_i = torch.zeros(H.M, dtype=torch.bool, device="cuda")
+        rows_i[I0 * b:(I0 + n) * b] = dev(np.repeat(mask, b))
+        rows_b = torch.zeros(H.M, dtype=torch.bool, device="cuda")
+        rows_b[I0 * b:(I0 + n) * b] = dev(np.repeat(~mask, b))
+        Yin = Yk.clone()
+        if mode == "fp64":
+            Yin[:I0 * b] = float("nan")
+            Yin[(I0 + n) * b:] = float("nan")
+        part = torch.empty_like(Yk)
+        tt.cheb_step(Hi, alpha, c, beta, Yin, Ykm1, part, use_work=True)
+        got[rows_i] = part[rows_i]
+        tt.cheb_step(Hb, alpha, c, beta, Yk, Ykm1, part, use_work=True)
+        got[rows_b] = part[rows_b]
+    assert torch.equal(got, full)

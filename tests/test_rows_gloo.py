@@ -71,6 +71,36 @@ def _scalars(m, a, b, a0):
     return c, alpha, beta
 
 
+def test_interior_boundary_split():
+    """The interior block rows of a slab (every tile's block column inside the slab) and the boundary ones partition the slab;
+    the two matrices built from them add up to the slab's matrix bit for bit."""
+    H = synth.hamiltonian_bsr(4, 8, 0.3, 79)                              # 64 block rows, 16 per z-layer of the 4 x 4 x 4 grid
+    nb = H.M // H.b
+    X = synth.dense_normal(H.M, 3, 80)
+    for world in (2, 3, 4):
+        total_interior = 0
+        for r in range(world):
+            I0, n = rows.slab_of(r, world, nb)
+            (rpi, cii, vai), (rpb, cib, vab), mask = rows.split_slab(H.row_ptr, H.col_idx, H.values, I0, n)
+            rp, ci, va = rows.slab_bsr(H.row_ptr, H.col_idx, H.values, I0, n)
+            assert mask.shape == (n,) and len(cii) + len(cib) == len(ci)
+            slab = oracle.spmm(*oracle.bsr_to_csr(H.b, rp, ci, va), 1.0, X)
+            inner = oracle.spmm(*oracle.bsr_to_csr(H.b, rpi, cii, vai), 1.0, X)
+            outer = oracle.spmm(*oracle.bsr_to_csr(H.b, rpb, cib, vab), 1.0, X)
+            rows_i = np.repeat(mask, H.b)
+            assert np.array_equal(inner[I0 * H.b:(I0 + n) * H.b][rows_i], slab[I0 * H.b:(I0 + n) * H.b][rows_i])
+            assert np.array_equal(outer[I0 * H.b:(I0 + n) * H.b][~rows_i], slab[I0 * H.b:(I0 + n) * H.b][~rows_i])
+            assert not inner[I0 * H.b:(I0 + n) * H.b][~rows_i].any() and not outer[I0 * H.b:(I0 + n) * H.b][rows_i].any()
+            # interior rows reference only columns inside the slab
+            for i in np.nonzero(mask)[0]:
+                cols = H.col_idx[H.row_ptr[I0 + i]:H.row_ptr[I0 + i + 1]]
+                assert cols.min() >= I0 and cols.max() < I0 + n
+            total_interior += int(mask.sum())
+        assert total_interior < nb
+        if world == 2:
+            assert total_interior == 32                                   # slabs of two x-layers: the outer layer of each is interior
+
+
 def _worker(rank, world, port, out_dir):
     import torch
     import torch.distributed as dist
@@ -93,6 +123,39 @@ def _worker(rank, world, port, out_dir):
         c, alpha, beta = _scalars(DEG, A, B, A0)
         Y = rows.cheb_filter_rows(step, torch.from_numpy(X.copy()), DEG, c, alpha, beta, H.b, (H.M // H.b))
         np.save(os.path.join(out_dir, f"Y{rank}.npy"), Y.numpy())
+
+        # the overlapped form: interior block rows step while the previous exchange is in flight, boundary rows after it.  The
+        # remote rows of every new iterate are poisoned until the exchange delivers them, so an interior step that touched them
+        # (or a boundary step that ran too early) would leave NaNs behind.
+        H = synth.hamiltonian_bsr(4, 8, 0.3, 4244)                        # 64 block rows: slabs of two x-layers, one of them interior
+        I0, n = rows.slab_of(rank, world, (H.M // H.b))
+        X = synth.dense_normal(H.M, NCOLS, 4245)
+        (rpi, cii, vai), (rpb, cib, vab), mask = rows.split_slab(H.row_ptr, H.col_idx, H.values, I0, n)
+        assert mask.sum() == 16
+        Ci, Cb = oracle.bsr_to_csr(H.b, rpi, cii, vai), oracle.bsr_to_csr(H.b, rpb, cib, vab)
+        rows_i = np.zeros(H.M, bool)
+        rows_i[I0 * H.b:(I0 + n) * H.b] = np.repeat(mask, H.b)
+        rows_b = np.zeros(H.M, bool)
+        rows_b[I0 * H.b:(I0 + n) * H.b] = np.repeat(~mask, H.b)
+
+        def make_step(Cx, sel, poison):
+            def f(alpha, c, beta, Yk, Ykm1, Yout):
+                yk = Yk.numpy().copy()
+                if poison:                                                # interior rows must not read another rank's rows
+                    yk[:I0 * H.b] = float("nan")
+                    yk[(I0 + n) * H.b:] = float("nan")
+                    yk[np.isnan(yk)] = 1e300                              # 0 * NaN would survive in the oracle's sums: use a huge value
+                res = oracle.cheb_step(*Cx, alpha, c, beta, yk, None if Ykm1 is None else Ykm1.numpy())
+                out = Yout.numpy()
+                out[sel] = res[sel]
+                if poison:
+                    out[:I0 * H.b] = float("nan")
+                    out[(I0 + n) * H.b:] = float("nan")
+            return f
+
+        Y2 = rows.cheb_filter_rows(make_step(Ci, rows_i, True), torch.from_numpy(X.copy()), DEG, c, alpha, beta, H.b, (H.M // H.b),
+                                   step_boundary=make_step(Cb, rows_b, False))
+        np.save(os.path.join(out_dir, f"Z{rank}.npy"), Y2.numpy())
     finally:
         dist.destroy_process_group()
 
@@ -107,3 +170,7 @@ def test_two_rank_row_sharded_filter_equals_single_process(tmp_path):
     ref = oracle.cheb_filter(*full, X, DEG, A, B, A0)
     for r in range(world):
         assert np.array_equal(np.load(tmp_path / f"Y{r}.npy"), ref)       # every rank holds the whole filtered block, bit for bit
+    H = synth.hamiltonian_bsr(4, 8, 0.3, 4244)
+    ref = oracle.cheb_filter(*oracle.bsr_to_csr(H.b, H.row_ptr, H.col_idx, H.values), synth.dense_normal(H.M, NCOLS, 4245), DEG, A, B, A0)
+    for r in range(world):
+        assert np.array_equal(np.load(tmp_path / f"Z{r}.npy"), ref)       # ... also with interior steps overlapping the exchange
