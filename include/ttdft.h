@@ -69,6 +69,11 @@ typedef enum { TTDFT_FMT_CSR = 0, TTDFT_FMT_BSR = 1 } ttdft_format;
 #define TTDFT_CHECK_SYMMETRY 2u /* verify H == H^T bit for bit (synchronises; needs sorted columns)      */
 #define TTDFT_FORCE_GENERIC 4u  /* keep the input format and use the generic row-per-warp kernel          */
 #define TTDFT_NO_I8 8u          /* do not build the int8 digit planes (saves 0.875x of the tile bytes)    */
+#define TTDFT_OWNED_ROWS_ONLY 16u /* row-partitioned H: this handle holds only the block rows (CSR: rows)
+                                   * one rank owns; rows without any entry belong to another rank, and ttdft_spmm / ttdft_cheb_step
+                                   * (and their _ws forms) leave those rows of the output UNTOUCHED instead of writing the result
+                                   * for an all-zero row.  Meant for single steps between exchanges (paper_2110_15853_b200/rows.py);
+                                   * ttdft_cheb_filter on such a handle never updates the rows it does not own. */
 
 /*
  * Arithmetic of the block-sparse product (every mode returns fp64 results inside north_star's

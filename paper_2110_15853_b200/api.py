@@ -8,7 +8,7 @@ from ctypes import POINTER, byref, c_char_p, c_double, c_int32, c_int64, c_size_
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_PKG, "libttdft.so")
 
-CHECK_SORTED, CHECK_SYMMETRY, FORCE_GENERIC, NO_I8 = 1, 2, 4, 8
+CHECK_SORTED, CHECK_SYMMETRY, FORCE_GENERIC, NO_I8, OWNED_ROWS_ONLY = 1, 2, 4, 8, 16
 MATH_AUTO, MATH_FP64, MATH_I8, MATH_I8X7 = 0, 1, 2, 3
 FMT_CSR, FMT_BSR = 0, 1
 _STATUS = {0: "OK", 1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "NOT_SYMMETRIC", 5: "CUDA", 6: "BREAKDOWN"}

@@ -31,6 +31,7 @@ struct K1Params {
   int32_t nct;         // column tiles = ceil(ncols/TN)
   int32_t cg;          // column tiles per scheduling group (L2 reuse of Y_k across block rows)
   int32_t vec;         // 1: S, Z, O are 16-byte aligned with even leading dimensions
+  int32_t skip_empty = 0;   // 1: block rows without tiles are not this handle's: their output rows are left untouched
   int64_t ncols;
   double alpha, gamma, beta;
   const double* S;     // shift source (Y_k), read at the output position; unused if gamma == 0
@@ -128,6 +129,7 @@ bsr_dmma_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
   }
   constexpr int32_t B = BR * RS;   // tile size of H
   const int32_t p_begin = prm.brow_ptr[I], p_end = prm.brow_ptr[I + 1];
+  if (prm.skip_empty && p_begin == p_end) return;      // CTA-uniform, before any barrier
   const int32_t col0 = ct * K1_TN;
   const int32_t ngrp_valid = min(K1_NGRP, (int32_t)((prm.ncols - col0 + 15) / 16));
 

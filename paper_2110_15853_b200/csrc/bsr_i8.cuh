@@ -58,6 +58,7 @@ struct K3Params {
   int8_t* dO = nullptr;
   const int32_t* ePredO = nullptr;
   uint32_t* flagsO = nullptr;
+  int32_t skip_empty = 0;          // 1: block rows without tiles are not this handle's: their output rows are left untouched
   int64_t mrows;                   // valid rows (= nb*b for a Hamiltonian; < nb*b for the ragged last block of ttdft_rotate)
   int32_t l2hints;                 // 1: evict-first H planes, evict-last Y digit tiles; 2: only the latter; 0: none (< 0 on the host: chosen per launch)
   int32_t jlimit = 0;              // > 0: only the first jlimit tiles of every block row are multiplied; < 0: the right factor is
@@ -451,6 +452,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       k3_decode(prm, u, I, ctg);
       const int32_t ct = prm.ct_begin + ctg * C + crank;
       const int32_t nJ = prm.brow_ptr[I + 1] - prm.brow_ptr[I];
+      if (prm.skip_empty && nJ == 0) continue;           // uniform over the epilogue warps
       const int64_t col0 = (int64_t)ct * K3_NT;          // first column of the item
       const int64_t colw = col0 + half * NCW;            // first column of this warp
       const int64_t row = (int64_t)I * b + r;

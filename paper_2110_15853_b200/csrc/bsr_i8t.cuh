@@ -204,6 +204,7 @@ bsr_i8t_kernel(const __grid_constant__ CUtensorMap tmH3, const __grid_constant__
       k3_decode(prm, u, I, ctg);
       const int32_t ct = prm.ct_begin + ctg;
       const int32_t nJ = prm.brow_ptr[I + 1] - prm.brow_ptr[I];
+      if (prm.skip_empty && nJ == 0) continue;           // uniform over the epilogue warps
       const int64_t col = (int64_t)ct * K3T_NT + cl;
       const bool col_ok = col < prm.ncols;
       const int64_t row0 = (int64_t)I * b + crank * HR;        // first row of this CTA

@@ -24,6 +24,7 @@ struct K2Params {
   const double* Z; int64_t ldz;     // Y_{k-1} / Y, read at the output position if beta != 0
   double* O; int64_t ldo;
   const int32_t* perm;      // BSR handles built from permuted subdomain labels: row r of H is row perm[r] of X/Z/O (else NULL)
+  int32_t skip_empty = 0;   // 1: (block) rows without entries are not this handle's: their output rows are left untouched
 };
 
 template <bool BSR>
@@ -31,6 +32,10 @@ __global__ void __launch_bounds__(32 * K2_ROWS) generic_step_kernel(const K2Para
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t row = (int64_t)blockIdx.x * K2_ROWS + warp;
   if (row >= p.M) return;
+  if (p.skip_empty) {
+    const int64_t ir = BSR ? row / p.b : row;
+    if (p.row_ptr[ir] == p.row_ptr[ir + 1]) return;
+  }
   const int64_t urow = (BSR && p.perm) ? p.perm[row] : row;   // the caller's row
   const int64_t c0 = (int64_t)blockIdx.y * K2_TN + lane;
   double acc[K2_CPL];

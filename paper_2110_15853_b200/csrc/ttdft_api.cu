@@ -230,6 +230,7 @@ struct ttdft_h_s {
   int32_t k3t_max_clusters = 0;
   int32_t nsm = 148;
   int32_t sym_checked = 0;         // TTDFT_CHECK_SYMMETRY passed at build: H == H^T bit for bit
+  int32_t skip_empty = 0;          // TTDFT_OWNED_ROWS_ONLY: (block) rows without entries are left untouched by the step calls
   const int32_t* perm = nullptr;   // rows reordered by subdomain label: row r of the tiles is the caller's row perm[r]
   int32_t k3_cluster = 0;   // 0: choose per launch; 1, 2, 4, 8: forced (env TTDFT_K3_CLUSTER at h_build)
   int32_t k3_l2hints = -1;  // < 0: chosen per launch; 0 / 1 / 2: forced (env TTDFT_K3_L2HINTS at h_build)
@@ -552,6 +553,7 @@ ttdft_status launch_k1(const ttdft_h_s* h, const CUtensorMap& tmH, double alpha,
   p.S = X; p.lds = ldx;
   p.Z = Z; p.ldz = ldz;
   p.O = O; p.ldo = ldo;
+  p.skip_empty = h->skip_empty;
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
   const int64_t tiles = (int64_t)p.nb * p.rs * p.nct;
@@ -613,6 +615,7 @@ ttdft_status launch_step(const ttdft_h_s* h, double alpha, double gamma, double 
   p.alpha = alpha; p.gamma = gamma; p.beta = beta;
   p.X = X; p.ldx = ldx; p.Z = Z; p.ldz = ldz; p.O = O; p.ldo = ldo;
   p.perm = perm;
+  p.skip_empty = h->skip_empty;
   dim3 grid((unsigned)((h->M + ttdft::K2_ROWS - 1) / ttdft::K2_ROWS), (unsigned)((ncols + ttdft::K2_TN - 1) / ttdft::K2_TN));
   if (grid.y > 65535) return fail(TTDFT_ERR_UNSUPPORTED, "ncols too large for the generic kernel");
   TimedLaunch tl(2, st);
@@ -870,6 +873,7 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
 #endif
   p.l2hints = h->k3_l2hints;
   p.mrows = h->M;
+  p.skip_empty = h->skip_empty;
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
   if (h->k3t) {
@@ -1630,6 +1634,7 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
   if (!h) return fail(TTDFT_ERR_CUDA, "out of host memory");
   h->M = d->M;
   h->sym_checked = (d->M > 0 && (d->flags & TTDFT_CHECK_SYMMETRY)) ? 1 : 0;   // reached only if the check passed
+  h->skip_empty = (d->flags & TTDFT_OWNED_ROWS_ONLY) ? 1 : 0;
   h->storage_bytes = need + need_i8;
   uint8_t* base = reinterpret_cast<uint8_t*>(dev_storage);
 

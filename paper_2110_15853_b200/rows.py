@@ -5,12 +5,15 @@ collective-free column bands of bands.py.
 
 Rank k owns a contiguous slab of block rows [I0, I0 + nI) of the tile format (whole subdomains, so every tile belongs to exactly one
 rank) and builds its handle(s) from the M x M matrix that holds only those block rows.  One recurrence step is then
-    Y_{k+1}[rows of rank r] = fused step of rank r's handle on the full iterates           (the library's kernels, unchanged)
+    Y_{k+1}[rows of rank r] = fused step of rank r's handle on the full iterates           (the library's kernels; a handle built
+                              with TTDFT_OWNED_ROWS_ONLY writes only the rows of its own block rows)
     all-gather of the row slabs                                                              (the collective over X' of L258)
 as ONE collective per step (all_gather_into_tensor: in place on the iterate when the slabs are equal, through one padded staging
 buffer when they differ by a block row), issued asynchronously so that it overlaps the next step's INTERIOR block rows -- those
 whose tiles multiply only rows this rank computed itself; the BOUNDARY block rows (a tile reaches into another rank's slab) wait
 for it.  On a 3-D grid of subdomains cut into slabs the boundary is two layers of G^2 block rows per rank, the interior the rest.
+The overlap is for TTDFT_MATH_FP64 handles: the int8 modes scale every column of the iterate by its maximum over ALL rows, so their
+step needs the complete iterate (pass one handle and no step_boundary there).
 
 Why an all-gather and not the paper's reduction.  The paper sums transposed slab products, Y = sum_k (H_k)^T X_k (Eq. 22),
 and all-reduces the M x N result through the host.  That moves the same M x N x 8 bytes per rank and step, but the sum must be

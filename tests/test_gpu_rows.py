@@ -94,12 +94,13 @@ def test_row_sharded_filter_lockstep_emulation(tt):
     assert relerr(Y.cpu().numpy(), Yf.cpu().numpy()) <= 1e-13
 
 
-@pytest.mark.parametrize("G,b,world,mode", [(4, 32, 2, "fp64"), (4, 64, 2, "fp64"), (4, 64, 2, "i8x7")])
+@pytest.mark.parametrize("G,b,world,mode", [(4, 32, 2, "fp64"), (4, 64, 2, "fp64"), (4, 64, 2, "i8x7"), (4, 96, 2, "i8x7")])
 def test_interior_and_boundary_handles(tt, G, b, world, mode):
-    """The overlapped row partition runs two handles per rank: interior block rows (tiles only inside the slab) and boundary ones.
-    Their steps fill disjoint rows and together equal the full handle's step bit for bit; the interior step of the fp64 kernel reads
-    no row outside the slab (remote rows poisoned with NaN).  The int8 modes scale by whole-column maxima, i.e. they need the
-    complete iterate and are not eligible for the overlap -- they are only checked on complete data here."""
+    """The overlapped row partition runs two handles per rank, built with TTDFT_OWNED_ROWS_ONLY: interior block rows (tiles only
+    inside the slab) and boundary ones.  Each step writes ONLY the rows of its own block rows, so both go into the same output:
+    together they equal the full handle's step bit for bit on the slab and leave every other row untouched; the interior step of
+    the fp64 kernel reads no row outside the slab (remote rows poisoned with NaN).  The int8 modes scale by whole-column maxima,
+    i.e. they need the complete iterate and are not eligible for the overlap -- they are only checked on complete data here."""
     import torch
     H, C, _, _ = small_problem(G, b, 0.3, 9300 + b)
     nb = H.M // H.b
@@ -110,24 +111,35 @@ def test_interior_and_boundary_handles(tt, G, b, world, mode):
     alpha, c, beta = 0.37, 9.5, -0.81
     full = torch.empty_like(Yk)
     tt.cheb_step(Hf, alpha, c, beta, Yk, Ykm1, full, use_work=True)
-    got = torch.full_like(Yk, float("nan"))
     for r in range(world):
         I0, n = rows.slab_of(r, world, nb)
         (rpi, cii, vai), (rpb, cib, vab), mask = rows.split_slab(H.row_ptr, H.col_idx, H.values, I0, n)
         assert 0 < mask.sum() < n
-        Hi = tt.h_build_bsr(H.M, H.b, dev(rpi), dev(cii), dev(vai)).set_math_mode(MODE)
-        Hb = tt.h_build_bsr(H.M, H.b, dev(rpb), dev(cib), dev(vab)).set_math_mode(MODE)
-        rows_i = torch.zeros(H.M, dtype=torch.bool, device="cuda")
-        rows_i[I0 * b:(I0 + n) * b] = dev(np.repeat(mask, b))
-        rows_b = torch.zeros(H.M, dtype=torch.bool, device="cuda")
-        rows_b[I0 * b:(I0 + n) * b] = dev(np.repeat(~mask, b))
+        Hi = tt.h_build_bsr(H.M, H.b, dev(rpi), dev(cii), dev(vai), flags=tt.OWNED_ROWS_ONLY).set_math_mode(MODE)
+        Hb = tt.h_build_bsr(H.M, H.b, dev(rpb), dev(cib), dev(vab), flags=tt.OWNED_ROWS_ONLY).set_math_mode(MODE)
         Yin = Yk.clone()
         if mode == "fp64":
             Yin[:I0 * b] = float("nan")
             Yin[(I0 + n) * b:] = float("nan")
-        part = torch.empty_like(Yk)
-        tt.cheb_step(Hi, alpha, c, beta, Yin, Ykm1, part, use_work=True)
-        got[rows_i] = part[rows_i]
-        tt.cheb_step(Hb, alpha, c, beta, Yk, Ykm1, part, use_work=True)
-        got[rows_b] = part[rows_b]
-    assert torch.equal(got, full)
+        for use_work in ([True, False] if mode == "fp64" else [True]):
+            out = torch.full_like(Yk, float("nan"))
+            tt.cheb_step(Hi, alpha, c, beta, Yin, Ykm1, out, use_work=use_work)
+            rows_i = torch.zeros(H.M, dtype=torch.bool, device="cuda")
+            rows_i[I0 * b:(I0 + n) * b] = dev(np.repeat(mask, b))
+            assert torch.equal(out[rows_i], full[rows_i]) and torch.isnan(out[~rows_i]).all()
+            tt.cheb_step(Hb, alpha, c, beta, Yk, Ykm1, out, use_work=use_work)
+            assert torch.equal(out[I0 * b:(I0 + n) * b], full[I0 * b:(I0 + n) * b])
+            assert torch.isnan(out[:I0 * b]).all() and torch.isnan(out[(I0 + n) * b:]).all()
+    # the generic kernel (CSR) honours the flag per row
+    Cs = synth.bsr_to_csr_nonzeros(H)
+    keep = np.zeros(H.M, bool)
+    keep[: H.M // 3] = True
+    counts = np.where(keep, np.diff(Cs.row_ptr), 0)
+    rp = np.zeros(H.M + 1, np.int32)
+    np.cumsum(counts, out=rp[1:])
+    nk = int(rp[-1])
+    Hc = tt.h_build_csr(H.M, dev(rp), dev(Cs.col_idx[:nk]), dev(Cs.values[:nk]), flags=tt.OWNED_ROWS_ONLY)
+    out = torch.full_like(Yk, float("nan"))
+    tt.cheb_step(Hc, alpha, c, beta, Yk, Ykm1, out)
+    ref = oracle.cheb_step(Cs.row_ptr, Cs.col_idx, Cs.values, alpha, c, beta, Yk.cpu().numpy(), Ykm1.cpu().numpy())
+    assert relerr(out[: H.M // 3].cpu().numpy(), ref[: H.M // 3]) <= 1e-12 and torch.isnan(out[H.M // 3:]).all()
