@@ -69,6 +69,12 @@ typedef enum { TTDFT_FMT_CSR = 0, TTDFT_FMT_BSR = 1 } ttdft_format;
 #define TTDFT_CHECK_SYMMETRY 2u /* verify H == H^T bit for bit (synchronises; needs sorted columns)      */
 #define TTDFT_FORCE_GENERIC 4u  /* keep the input format and use the generic row-per-warp kernel          */
 #define TTDFT_NO_I8 8u          /* do not build the int8 digit planes (saves 0.875x of the tile bytes)    */
+#define TTDFT_PACKED 32u        /* also build the PACKED copy of the tiles (per 16-column slab: row offsets, bit masks, non-zero
+                                 * values: 0.65x of the dense tile bytes at 40 % zeros); products with ncols <= 16 then stream it
+                                 * instead of the dense tiles.  A storage variant for memory-tight handles, NOT a speed-up on
+                                 * B200: the fp64 tensor pipe multiplies the expanded zeros either way and bounds a 16-column
+                                 * product at 0.66 ms for config 3, so the dense tiles (0.79 ms) are not far above the bound and
+                                 * the decode costs more shared-memory bandwidth than the bytes save (1.04 ms). */
 #define TTDFT_OWNED_ROWS_ONLY 16u /* row-partitioned H: this handle holds only the block rows (CSR: rows)
                                    * one rank owns; rows without any entry belong to another rank, and ttdft_spmm / ttdft_cheb_step
                                    * (and their _ws forms) leave those rows of the output UNTOUCHED instead of writing the result
@@ -103,7 +109,7 @@ typedef enum { TTDFT_FMT_CSR = 0, TTDFT_FMT_BSR = 1 } ttdft_format;
  *        values[nblocks*block*block], each block a row-major block x block tile.  M % block == 0.
  *   subdomain_of_row (CSR only, optional, may be NULL): subdomain label of every row.  If every subdomain
  *        owns the same number b of rows, b in {32, 64, 96, 128}, the builder groups each localized
- *        subdomain's basis functions into b x b tiles (block-sparse storage).  Two label layouts qualify:
+ *        subdomain's basis functions into b x b tiles (block-sparse storage).  Three label layouts qualify:
  *        (1) rows already grouped: labels strictly increasing from group to group (any integers);
  *        (2) rows in ANY order: labels are the subdomain indices 0 .. M/b-1.  The builder then REORDERS:
  *            reordered row L*b + r is the r-th row (in input order) labelled L, H is stored as the tiles of
@@ -112,6 +118,11 @@ typedef enum { TTDFT_FMT_CSR = 0, TTDFT_FMT_BSR = 1 } ttdft_format;
  *            all m steps there, and scatters the result (two extra passes per panel, no extra scratch).
  *            Single steps on such a handle: ttdft_*_ws gather/scatter through scratch; the calls without
  *            scratch run the generic kernel through the row map.
+ *        (3) subdomains of UNEQUAL size (the real TTDFT basis: ranks differ per subdomain): labels are the
+ *            subdomain indices 0 .. nb-1 without gaps, rows in any order, every subdomain with 1 .. 128 rows.  Every subdomain is
+ *            padded with zero rows and columns to one tile size b (the smallest of 32/64/96/128 that holds the largest one)
+ *            unless that more than doubles the rows; the handle then works in a tile-order space of nb*b rows behind the
+ *            same row map as (2) (ttdft_cheb_filter needs a second scratch panel: ask ttdft_cheb_filter_work_bytes).
  *        Otherwise the CSR is kept as is.
  * All four arrays are DEVICE pointers; the struct itself is a HOST object.
  */
@@ -137,7 +148,9 @@ typedef struct {
   int32_t i8_planes;      /* digit planes per operand of H stored for the I8 modes (0: not built) */
   int32_t math;           /* TTDFT_MATH_FP64, _I8 or _I8X7: what calls that take `work` use */
   int32_t reordered;      /* 1: rows were regrouped by subdomain label (the handle keeps the row map) */
-  int32_t reserved;
+  int32_t padded;         /* 1: the subdomains differ in size and were padded with zero rows/columns to the tile size */
+  int64_t packed_bytes;   /* bytes of the packed copy of the tiles (per 16-column slab: row offsets, bit masks, non-zero values),
+                             the storage variant the products with ncols <= 16 stream instead of the dense tiles; 0: not built */
 } ttdft_h_info_t;
 
 /* A0 -- storage builder (north_star "BSR/CSR storage builder"). */

@@ -8,7 +8,7 @@ from ctypes import POINTER, byref, c_char_p, c_double, c_int32, c_int64, c_size_
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_PKG, "libttdft.so")
 
-CHECK_SORTED, CHECK_SYMMETRY, FORCE_GENERIC, NO_I8, OWNED_ROWS_ONLY = 1, 2, 4, 8, 16
+CHECK_SORTED, CHECK_SYMMETRY, FORCE_GENERIC, NO_I8, OWNED_ROWS_ONLY, PACKED = 1, 2, 4, 8, 16, 32
 MATH_AUTO, MATH_FP64, MATH_I8, MATH_I8X7 = 0, 1, 2, 3
 FMT_CSR, FMT_BSR = 0, 1
 _STATUS = {0: "OK", 1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "NOT_SYMMETRIC", 5: "CUDA", 6: "BREAKDOWN"}
@@ -41,7 +41,8 @@ class _Desc(ctypes.Structure):
 
 class _Info(ctypes.Structure):
     _fields_ = [("M", c_int64), ("nnz_stored", c_int64), ("block", c_int32), ("kernel", c_int32), ("nblocks", c_int64),
-                ("storage_bytes", c_size_t), ("i8_planes", c_int32), ("math", c_int32), ("reordered", c_int32), ("reserved", c_int32)]
+                ("storage_bytes", c_size_t), ("i8_planes", c_int32), ("math", c_int32), ("reordered", c_int32), ("padded", c_int32),
+                ("packed_bytes", c_int64)]
 
 
 _lib = None

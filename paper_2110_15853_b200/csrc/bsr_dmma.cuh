@@ -97,98 +97,17 @@ struct K1Cfg {
   static constexpr int TOTAL = BAR_OFFSET + 2 * NSTAGE * 8 + 1024;  // + alignment slack
 };
 
-template <int WR, int Q, int CPS, int RS>
-__global__ void __launch_bounds__(32 * (2 * WR + 1), CPS)
-bsr_dmma_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmX, const K1Params prm) {
+// The consumer side of kernel K1 (MMA loop over the ring + fused epilogue), shared with the packed-storage variant
+// (bsr_packed.cuh), which fills the A half of every stage by decoding instead of by TMA.
+template <int WR, int Q, int CPS, int RS, int NSTG>
+__device__ __forceinline__ void k1_consume(const K1Params& prm, uint8_t* smem, uint64_t* full, uint64_t* empty, int32_t I, int32_t rsi,
+                                           int32_t col0, int32_t p_begin, int32_t p_end) {
   using SM = K1Cfg<WR, Q, CPS, RS>;
-  constexpr int NCW = SM::NCW;
-  constexpr int K1_NSTAGE = SM::NSTAGE;
+  constexpr int K1_NSTAGE = NSTG;  // stages of the ring (the packed variant runs a shorter one)
   constexpr int K1_TN = SM::TN;
-  constexpr int K1_NGRP = SM::NGRP;
   constexpr int BR = SM::BR;
-  extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  uint64_t* full = reinterpret_cast<uint64_t*>(smem + SM::BAR_OFFSET);
-  uint64_t* empty = full + K1_NSTAGE;
-
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-
-  // ---- tile decode: column-tile groups outermost, then block rows, column tile fastest ----
-  int32_t I, ct, rsi;
-  {
-    const int64_t per_group = (int64_t)prm.nb * RS * prm.cg;
-    const int32_t ngroups = (prm.nct + prm.cg - 1) / prm.cg;
-    int32_t g = (int32_t)((int64_t)blockIdx.x / per_group);
-    if (g > ngroups - 1) g = ngroups - 1;
-    const int64_t rem = (int64_t)blockIdx.x - (int64_t)g * per_group;
-    const int32_t width = min(prm.cg, prm.nct - g * prm.cg);
-    const int64_t irs = rem / width;
-    I = (int32_t)(irs / RS);
-    rsi = (int32_t)(irs - (int64_t)I * RS);
-    ct = g * prm.cg + (int32_t)(rem % width);
-  }
   constexpr int32_t B = BR * RS;   // tile size of H
-  const int32_t p_begin = prm.brow_ptr[I], p_end = prm.brow_ptr[I + 1];
-  if (prm.skip_empty && p_begin == p_end) return;      // CTA-uniform, before any barrier
-  const int32_t col0 = ct * K1_TN;
-  const int32_t ngrp_valid = min(K1_NGRP, (int32_t)((prm.ncols - col0 + 15) / 16));
-
-  if (threadIdx.x == 0) {
-    for (int s = 0; s < K1_NSTAGE; ++s) {
-      mbar_init(&full[s], 1);
-      mbar_init(&empty[s], NCW);
-    }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-  }
-  __syncthreads();
-
-  if (warp == NCW) {
-    // =========================== TMA producer (one elected lane) ===========================
-    if (lane == 0) {
-      asm volatile("prefetch.tensormap [%0];" ::"l"(&tmH) : "memory");
-      asm volatile("prefetch.tensormap [%0];" ::"l"(&tmX) : "memory");
-      const uint32_t tx_bytes = SM::A_BYTES + ngrp_valid * K1_BGRP_BYTES;
-      int stage = 0;
-      uint32_t phase = 0;
-      for (int32_t p = p_begin; p < p_end; ++p) {
-        const int32_t J = prm.bcol[p];
-#pragma unroll 1
-        for (int k0 = 0; k0 < B; k0 += K1_KS) {
-          mbar_wait(&empty[stage], phase ^ 1);
-          uint8_t* As = smem + stage * SM::STAGE_BYTES;
-          uint8_t* Bs = As + SM::A_BYTES;
-          mbar_expect_tx(&full[stage], tx_bytes);
-          tma_load_2d(As, &tmH, k0, p * B + rsi * BR, &full[stage]);
-          for (int g = 0; g < ngrp_valid; ++g)
-            tma_load_2d(Bs + g * K1_BGRP_BYTES, &tmX, col0 + g * 16, J * B + k0, &full[stage]);
-          if (++stage == K1_NSTAGE) { stage = 0; phase ^= 1; }
-        }
-      }
-    }
-    __syncwarp();
-    // The ring now holds the last NSTAGE slabs of work: use that time to pull the epilogue's operands
-    // (Y_k and Y_{k-1} at the output tile) into L2, one 128-byte line per lane and request.
-    {
-      const int64_t row0 = (int64_t)I * B + rsi * BR;
-      const int64_t ncl = min((int64_t)K1_TN, prm.ncols - col0);     // valid columns of this tile
-      const int lines_per_row = (int)((ncl * 8 + 127) / 128);
-      const int total = BR * lines_per_row;
-      for (int idx = lane; idx < total; idx += 32) {
-        const int r = idx / lines_per_row, l = idx - r * lines_per_row;
-        if (prm.beta != 0.0) {
-          const double* zp = prm.Z + (row0 + r) * prm.ldz + col0 + l * 16;
-          asm volatile("prefetch.global.L2 [%0];" ::"l"(zp));
-        }
-        if (prm.gamma != 0.0) {
-          const double* sp = prm.S + (row0 + r) * prm.lds + col0 + l * 16;
-          asm volatile("prefetch.global.L2 [%0];" ::"l"(sp));
-        }
-      }
-    }
-    return;
-  }
-
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   // ================================ consumers: 32 x 64 per warp ================================
   const int wr = warp >> 1, wc = warp & 1;
   const int g = lane >> 2, t = lane & 3;
@@ -298,6 +217,101 @@ bsr_dmma_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__
       }
     }
   }
+}
+
+template <int WR, int Q, int CPS, int RS>
+__global__ void __launch_bounds__(32 * (2 * WR + 1), CPS)
+bsr_dmma_kernel(const __grid_constant__ CUtensorMap tmH, const __grid_constant__ CUtensorMap tmX, const K1Params prm) {
+  using SM = K1Cfg<WR, Q, CPS, RS>;
+  constexpr int NCW = SM::NCW;
+  constexpr int K1_NSTAGE = SM::NSTAGE;
+  constexpr int K1_TN = SM::TN;
+  constexpr int K1_NGRP = SM::NGRP;
+  constexpr int BR = SM::BR;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + SM::BAR_OFFSET);
+  uint64_t* empty = full + K1_NSTAGE;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  // ---- tile decode: column-tile groups outermost, then block rows, column tile fastest ----
+  int32_t I, ct, rsi;
+  {
+    const int64_t per_group = (int64_t)prm.nb * RS * prm.cg;
+    const int32_t ngroups = (prm.nct + prm.cg - 1) / prm.cg;
+    int32_t g = (int32_t)((int64_t)blockIdx.x / per_group);
+    if (g > ngroups - 1) g = ngroups - 1;
+    const int64_t rem = (int64_t)blockIdx.x - (int64_t)g * per_group;
+    const int32_t width = min(prm.cg, prm.nct - g * prm.cg);
+    const int64_t irs = rem / width;
+    I = (int32_t)(irs / RS);
+    rsi = (int32_t)(irs - (int64_t)I * RS);
+    ct = g * prm.cg + (int32_t)(rem % width);
+  }
+  constexpr int32_t B = BR * RS;   // tile size of H
+  const int32_t p_begin = prm.brow_ptr[I], p_end = prm.brow_ptr[I + 1];
+  if (prm.skip_empty && p_begin == p_end) return;      // CTA-uniform, before any barrier
+  const int32_t col0 = ct * K1_TN;
+  const int32_t ngrp_valid = min(K1_NGRP, (int32_t)((prm.ncols - col0 + 15) / 16));
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < K1_NSTAGE; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], NCW);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp == NCW) {
+    // =========================== TMA producer (one elected lane) ===========================
+    if (lane == 0) {
+      asm volatile("prefetch.tensormap [%0];" ::"l"(&tmH) : "memory");
+      asm volatile("prefetch.tensormap [%0];" ::"l"(&tmX) : "memory");
+      const uint32_t tx_bytes = SM::A_BYTES + ngrp_valid * K1_BGRP_BYTES;
+      int stage = 0;
+      uint32_t phase = 0;
+      for (int32_t p = p_begin; p < p_end; ++p) {
+        const int32_t J = prm.bcol[p];
+#pragma unroll 1
+        for (int k0 = 0; k0 < B; k0 += K1_KS) {
+          mbar_wait(&empty[stage], phase ^ 1);
+          uint8_t* As = smem + stage * SM::STAGE_BYTES;
+          uint8_t* Bs = As + SM::A_BYTES;
+          mbar_expect_tx(&full[stage], tx_bytes);
+          tma_load_2d(As, &tmH, k0, p * B + rsi * BR, &full[stage]);
+          for (int g = 0; g < ngrp_valid; ++g)
+            tma_load_2d(Bs + g * K1_BGRP_BYTES, &tmX, col0 + g * 16, J * B + k0, &full[stage]);
+          if (++stage == K1_NSTAGE) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+    __syncwarp();
+    // The ring now holds the last NSTAGE slabs of work: use that time to pull the epilogue's operands
+    // (Y_k and Y_{k-1} at the output tile) into L2, one 128-byte line per lane and request.
+    {
+      const int64_t row0 = (int64_t)I * B + rsi * BR;
+      const int64_t ncl = min((int64_t)K1_TN, prm.ncols - col0);     // valid columns of this tile
+      const int lines_per_row = (int)((ncl * 8 + 127) / 128);
+      const int total = BR * lines_per_row;
+      for (int idx = lane; idx < total; idx += 32) {
+        const int r = idx / lines_per_row, l = idx - r * lines_per_row;
+        if (prm.beta != 0.0) {
+          const double* zp = prm.Z + (row0 + r) * prm.ldz + col0 + l * 16;
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(zp));
+        }
+        if (prm.gamma != 0.0) {
+          const double* sp = prm.S + (row0 + r) * prm.lds + col0 + l * 16;
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(sp));
+        }
+      }
+    }
+    return;
+  }
+
+  k1_consume<WR, Q, CPS, RS, SM::NSTAGE>(prm, smem, full, empty, I, rsi, col0, p_begin, p_end);
 }
 
 }  // namespace ttdft

@@ -37,6 +37,7 @@ __global__ void __launch_bounds__(32 * K2_ROWS) generic_step_kernel(const K2Para
     if (p.row_ptr[ir] == p.row_ptr[ir + 1]) return;
   }
   const int64_t urow = (BSR && p.perm) ? p.perm[row] : row;   // the caller's row
+  if (urow < 0) return;                                       // a padding row of a subdomain smaller than the tile
   const int64_t c0 = (int64_t)blockIdx.y * K2_TN + lane;
   double acc[K2_CPL];
   bool ok[K2_CPL];
@@ -52,7 +53,9 @@ __global__ void __launch_bounds__(32 * K2_ROWS) generic_step_kernel(const K2Para
         const int64_t xrow0 = (int64_t)p.col[q] * p.b;
         for (int32_t s = 0; s < p.b; ++s) {
           const double h = __ldg(tile + s);
-          const double* xr = p.X + (p.perm ? (int64_t)p.perm[xrow0 + s] : xrow0 + s) * p.ldx + c0;
+          const int64_t xrow = p.perm ? (int64_t)p.perm[xrow0 + s] : xrow0 + s;
+          if (xrow < 0) continue;                             // padding column (its tile entries are zero)
+          const double* xr = p.X + xrow * p.ldx + c0;
 #pragma unroll
           for (int c = 0; c < K2_CPL; ++c)
             if (ok[c]) acc[c] = fma(h, __ldg(xr + 32 * c), acc[c]);

@@ -21,6 +21,7 @@
 #include "bsr_dmma.cuh"
 #include "bsr_i8.cuh"
 #include "bsr_i8t.cuh"
+#include "bsr_packed.cuh"
 #include "generic_spmm.cuh"
 #include "cholesky.cuh"
 #include "gram_i8.cuh"
@@ -203,7 +204,10 @@ size_t i8_storage_bytes(int64_t nblocks, int32_t b, int64_t M) {
 // handle
 // ------------------------------------------------------------------------------------------------
 struct ttdft_h_s {
-  int64_t M = 0;
+  int64_t M = 0;            // rows = columns of H as the caller sees it
+  int64_t Mt = 0;           // rows of the tile-order space the tile kernels work in: M, or nb * b > M when subdomains of UNEQUAL size
+                            // were padded to the tile size (padded = 1; perm[t] = -1 marks a padding row)
+  int32_t padded = 0;
   int32_t kernel = 0;       // 1 = K1 (BSR, TMA + DMMA), 0 = K2 generic
   int32_t bsr = 0;          // storage is BSR
   int32_t b = 0;
@@ -226,6 +230,10 @@ struct ttdft_h_s {
   const double* hdiag = nullptr;  // [M]
   CUtensorMap tmHd[4];      // box rows b, b/2, b/4, b/8: K3 in clusters of 1, 2, 4, 8 CTAs (every CTA fetches b/C rows of a plane)
   CUtensorMap tmH3[2];      // K3T: 3-D boxes {128 B, b/2 rows, 7 | 6 planes}
+  // packed tiles (bsr_packed.cuh): slab offsets in 16-byte units and the packed slabs; NULL: not built
+  const uint32_t* pk_ptr = nullptr;
+  const uint8_t* pk_data = nullptr;
+  size_t pk_bytes = 0;
   int32_t k3t = 0;          // 1: the int8 step runs on the transposed kernel K3T (tiles narrower than 128; env TTDFT_K3_T forces 0 / 1)
   int32_t k3t_max_clusters = 0;
   int32_t nsm = 148;
@@ -329,6 +337,17 @@ __global__ void label_hist_check_kernel(int64_t nb, int32_t b, const int32_t* hi
   int64_t L = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (L < nb && hist[L] != b) atomicOr(flags, 1);
 }
+// subdomains of unequal size: stats[0] = largest group, stats[1] = non-empty groups, stats[2] = last non-empty label + 1
+__global__ void label_stats_kernel(int64_t M, const int32_t* hist, int32_t* stats) {
+  int64_t L = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (L >= M) return;
+  const int32_t c = hist[L];
+  if (c > 0) {
+    atomicMax(&stats[0], c);
+    atomicAdd(&stats[1], 1);
+    atomicMax(&stats[2], (int32_t)L + 1);
+  }
+}
 // One CTA per subdomain L: ordered (stable, deterministic) compaction of the rows labelled L.
 // perm[L*b + rank] = row, inv[row] = L*b + rank.  blockDim = 256.
 __global__ void __launch_bounds__(256) label_perm_kernel(int64_t M, int32_t b, const int32_t* lab, int32_t* perm, int32_t* inv) {
@@ -368,7 +387,7 @@ __global__ void __launch_bounds__(256) label_perm_kernel(int64_t M, int32_t b, c
 // Indices are range-guarded (an invalid CSR gives a meaningless count, never a fault): entries outside [0, nnz) and columns
 // outside [0, M) are skipped.
 __global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_ptr, const int32_t* col, const int32_t* perm,
-                                     const int32_t* inv, int32_t* counts, int32_t nwords, int32_t nnz) {
+                                     const int32_t* inv, int32_t* counts, int32_t nwords, int32_t nnz, int64_t M) {
   extern __shared__ uint32_t bits[];
   for (int w = threadIdx.x; w < nwords; w += blockDim.x) bits[w] = 0;
   __syncthreads();
@@ -376,10 +395,11 @@ __global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_p
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
   for (int32_t r = warp; r < b; r += nwarps) {
     const int64_t row = perm ? perm[I * b + r] : I * b + r;
+    if (row < 0) continue;                       // padding row
     const int32_t e1 = min(row_ptr[row + 1], nnz);
     for (int32_t e = max(row_ptr[row], 0) + lane; e < e1; e += 32) {
       const int32_t cj = col[e];
-      if ((uint32_t)cj >= (uint32_t)(nb * b)) continue;
+      if ((uint32_t)cj >= (uint32_t)M) continue;
       const int32_t j = inv ? inv[cj] : cj;
       const int32_t J = j / b;
       atomicOr(&bits[J >> 5], 1u << (J & 31));
@@ -400,7 +420,7 @@ __global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_p
 // pass 2: fill bcol (ascending) and scatter the entries into zero-initialised tiles
 __global__ void csr2bsr_fill_kernel(int64_t nb, int32_t b, const int32_t* row_ptr, const int32_t* col, const double* val,
                                     const int32_t* perm, const int32_t* inv, const int32_t* brow_ptr, int32_t* bcol,
-                                    double* tiles, int32_t nwords, int32_t nnz) {
+                                    double* tiles, int32_t nwords, int32_t nnz, int64_t M) {
   extern __shared__ uint32_t sm[];
   uint32_t* bits = sm;                    // nwords
   uint32_t* pref = sm + nwords;           // nwords: tiles before word w
@@ -410,10 +430,11 @@ __global__ void csr2bsr_fill_kernel(int64_t nb, int32_t b, const int32_t* row_pt
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
   for (int32_t r = warp; r < b; r += nwarps) {
     const int64_t row = perm ? perm[I * b + r] : I * b + r;
+    if (row < 0) continue;                       // padding row
     const int32_t e1 = min(row_ptr[row + 1], nnz);
     for (int32_t e = max(row_ptr[row], 0) + lane; e < e1; e += 32) {
       const int32_t cj = col[e];
-      if ((uint32_t)cj >= (uint32_t)(nb * b)) continue;
+      if ((uint32_t)cj >= (uint32_t)M) continue;
       const int32_t j = inv ? inv[cj] : cj;
       const int32_t J = j / b;
       atomicOr(&bits[J >> 5], 1u << (J & 31));
@@ -438,10 +459,11 @@ __global__ void csr2bsr_fill_kernel(int64_t nb, int32_t b, const int32_t* row_pt
   // rows of this block row: scatter entries
   for (int32_t r = warp; r < b; r += nwarps) {
     const int64_t row = perm ? perm[I * b + r] : I * b + r;
+    if (row < 0) continue;                       // padding row
     const int32_t e1 = min(row_ptr[row + 1], nnz);
     for (int32_t e = max(row_ptr[row], 0) + lane; e < e1; e += 32) {
       const int32_t cj = col[e];
-      if ((uint32_t)cj >= (uint32_t)(nb * b)) continue;
+      if ((uint32_t)cj >= (uint32_t)M) continue;
       const int32_t j = inv ? inv[cj] : cj;
       const int32_t J = j / b;
       const uint32_t w = bits[J >> 5] & ((1u << (J & 31)) - 1u);
@@ -457,6 +479,11 @@ __global__ void __launch_bounds__(256) permute_rows_kernel(const double* __restr
                                                            const int32_t* __restrict__ map, int scatter) {
   const int64_t r = blockIdx.x;
   const int64_t m = map[r];
+  if (m < 0) {                                   // padding row of the tile-order space: zero on a gather, nothing on a scatter
+    if (!scatter)
+      for (int64_t c = (int64_t)blockIdx.y * 1024 + threadIdx.x; c < min(cols, ((int64_t)blockIdx.y + 1) * 1024); c += 256) dst[r * ldd + c] = 0.0;
+    return;
+  }
   const double* s = src + (scatter ? r : m) * lds;
   double* d = dst + (scatter ? m : r) * ldd;
   for (int64_t c = (int64_t)blockIdx.y * 1024 + threadIdx.x; c < min(cols, ((int64_t)blockIdx.y + 1) * 1024); c += 256) d[c] = s[c];
@@ -538,7 +565,7 @@ ttdft_status launch_k1(const ttdft_h_s* h, const CUtensorMap& tmH, double alpha,
     attr_mark(attr_seen);
   }
   CUtensorMap tmX;
-  ttdft_status s = make_map_2d(&tmX, X, (uint64_t)ncols, (uint64_t)h->M, (uint64_t)ldx, ttdft::K1_KS);
+  ttdft_status s = make_map_2d(&tmX, X, (uint64_t)ncols, (uint64_t)h->Mt, (uint64_t)ldx, ttdft::K1_KS);
   if (s != TTDFT_OK) return s;
   ttdft::K1Params p;
   p.brow_ptr = h->row_ptr;
@@ -565,6 +592,35 @@ ttdft_status launch_k1(const ttdft_h_s* h, const CUtensorMap& tmH, double alpha,
   return TTDFT_OK;
 }
 
+// K1P: one 16-column tile from the packed tiles (ncols <= 16)
+template <int WR>
+ttdft_status launch_k1p(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx, const double* Z,
+                        int64_t ldz, double* O, int64_t ldo, int64_t ncols, cudaStream_t st) {
+  using Cf = ttdft::K1PCfg<WR>;
+  static std::atomic<uint64_t> attr_seen{0};
+  if (!attr_done(attr_seen)) {
+    CUDA_TRY(cudaFuncSetAttribute(ttdft::bsr_dmma_packed_kernel<WR>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cf::TOTAL));
+    attr_mark(attr_seen);
+  }
+  CUtensorMap tmX;
+  ttdft_status s = make_map_2d(&tmX, X, (uint64_t)ncols, (uint64_t)h->Mt, (uint64_t)ldx, ttdft::K1_KS);
+  if (s != TTDFT_OK) return s;
+  ttdft::K1Params p;
+  p.brow_ptr = h->row_ptr; p.bcol = h->col;
+  p.nb = (int32_t)h->nb; p.b = h->b; p.rs = 1; p.nct = 1; p.cg = 1;
+  p.ncols = ncols;
+  p.alpha = alpha; p.gamma = gamma; p.beta = beta;
+  p.S = X; p.lds = ldx; p.Z = Z; p.ldz = ldz; p.O = O; p.ldo = ldo;
+  p.skip_empty = h->skip_empty;
+  auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
+  p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
+  TimedLaunch tl(1, st);
+  ttdft::bsr_dmma_packed_kernel<WR><<<(unsigned)h->nb, Cf::THREADS, Cf::TOTAL, st>>>(tmX, p, h->pk_ptr, h->pk_data);
+  CUDA_TRY(cudaGetLastError());
+  g_launches.fetch_add(1);
+  return TTDFT_OK;
+}
+
 // column-tile width by the number of columns: narrow tiles keep the HBM-bound small-N regime from
 // multiplying padding columns (BASELINE.json config 5, N = 16 / 64)
 template <int WR, int CPS, int RS>
@@ -578,6 +634,16 @@ ttdft_status launch_k1_q(const ttdft_h_s* h, const CUtensorMap& tmH, double alph
 
 ttdft_status launch_k1_any(const ttdft_h_s* h, double alpha, double gamma, double beta, const double* X, int64_t ldx,
                            const double* Z, int64_t ldz, double* O, int64_t ldo, int64_t ncols, cudaStream_t st) {
+  if (h->pk_ptr && ncols <= 16) {
+    // HBM-bound: stream the packed tiles (non-zeros + bit maps) instead of the dense ones
+    switch (h->b) {
+      case 32: return launch_k1p<1>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+      case 64: return launch_k1p<2>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+      case 96: return launch_k1p<3>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+      case 128: return launch_k1p<4>(h, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
+      default: break;
+    }
+  }
   switch (h->b) {
     case 32: return launch_k1_q<1, 1, 1>(h, h->tmH, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
     case 64: return launch_k1_q<2, 1, 1>(h, h->tmH, alpha, gamma, beta, X, ldx, Z, ldz, O, ldo, ncols, st);
@@ -611,12 +677,12 @@ ttdft_status launch_step(const ttdft_h_s* h, double alpha, double gamma, double 
   }
   ttdft::K2Params p;
   p.row_ptr = h->row_ptr; p.col = h->col; p.val = h->val;
-  p.M = h->M; p.b = h->b; p.ncols = ncols;
+  p.M = h->Mt; p.b = h->b; p.ncols = ncols;
   p.alpha = alpha; p.gamma = gamma; p.beta = beta;
   p.X = X; p.ldx = ldx; p.Z = Z; p.ldz = ldz; p.O = O; p.ldo = ldo;
   p.perm = perm;
   p.skip_empty = h->skip_empty;
-  dim3 grid((unsigned)((h->M + ttdft::K2_ROWS - 1) / ttdft::K2_ROWS), (unsigned)((ncols + ttdft::K2_TN - 1) / ttdft::K2_TN));
+  dim3 grid((unsigned)((h->Mt + ttdft::K2_ROWS - 1) / ttdft::K2_ROWS), (unsigned)((ncols + ttdft::K2_TN - 1) / ttdft::K2_TN));
   if (grid.y > 65535) return fail(TTDFT_ERR_UNSUPPORTED, "ncols too large for the generic kernel");
   TimedLaunch tl(2, st);
   if (h->bsr)
@@ -818,9 +884,9 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
   uint32_t* cmS = w.cmax[src];
   if (!have_src) {
     CUDA_TRY(cudaMemsetAsync(cmS, 0, (size_t)ncols * 4, st));
-    dim3 g(nct, (unsigned)((h->M + 2047) / 2048));
+    dim3 g(nct, (unsigned)((h->Mt + 2047) / 2048));
     TimedLaunch tl(5, st);
-    ttdft::colmax_kernel<<<g, 256, 0, st>>>(X, ldx, h->M, ncols, cmS);
+    ttdft::colmax_kernel<<<g, 256, 0, st>>>(X, ldx, h->Mt, ncols, cmS);
     CUDA_TRY(cudaGetLastError());
     g_launches.fetch_add(1);
   }
@@ -845,7 +911,7 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
     // rare tile that has to be redone
     dim3 g((unsigned)(have_src ? std::min<int64_t>(h->nb, 32) : h->nb), nct);
     TimedLaunch tl(have_src ? 7 : 4, st);
-    ttdft::y_digits_fix_kernel<S><<<g, 256, smem, st>>>(X, ldx, h->b, h->M, ncols, (int32_t)h->nb, cmS, w.D[src], w.flags[src], have_src ? 0 : 1,
+    ttdft::y_digits_fix_kernel<S><<<g, 256, smem, st>>>(X, ldx, h->b, h->Mt, ncols, (int32_t)h->nb, cmS, w.D[src], w.flags[src], have_src ? 0 : 1,
                                                          have_prev ? 1 : 0, h->k3_predict_bias, w.e_used, w.e_pred, w.cmax[src ^ 1],
                                                          w.flags[src ^ 1]);
     CUDA_TRY(cudaGetLastError());
@@ -872,7 +938,7 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
   p.exp = env_int("TTDFT_K3_EXP", 0);
 #endif
   p.l2hints = h->k3_l2hints;
-  p.mrows = h->M;
+  p.mrows = h->Mt;
   p.skip_empty = h->skip_empty;
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
@@ -962,7 +1028,7 @@ ttdft_status panel_step(ttdft_h_s* h, double al, double ga, double be, const dou
 // panel (ldy), W: scratch (ldw).  inplace: Xp == Yp.
 ttdft_status filter_panel(ttdft_h_s* h, const double* Xp, int64_t ldx, double* Yp, int64_t ldy, double* W,
                           int64_t ldw, int64_t wc, int32_t m, double c, const double* alpha, const double* beta,
-                          bool inplace, cudaStream_t st, const I8Work* i8 = nullptr) {
+                          bool inplace, cudaStream_t st, const I8Work* i8 = nullptr, double* W2 = nullptr) {
   if (m == 0) {
     if (!inplace) return launch_copy2d(Xp, ldx, Yp, ldy, h->M, wc, st);
     return TTDFT_OK;
@@ -972,20 +1038,25 @@ ttdft_status filter_panel(ttdft_h_s* h, const double* Xp, int64_t ldx, double* Y
     // Rows reordered by subdomain label (A0): gather X into tile order, run all m steps there between W and
     // the Y panel (Y_{k+1} overwrites Y_{k-1}), and scatter the last iterate back.  Iterate k sits in buf[k&1];
     // the last one must end in W so that the scatter into Yp is out of place.
+    // Padded handles (subdomains of unequal size): the tile-order space has more rows than the caller's panels, so both buffers
+    // are scratch (W2, W; the last iterate ends in W).
     const bool w_first = inplace || (m % 2 == 0);
-    double* buf[2] = {w_first ? W : Yp, w_first ? Yp : W};
-    const int64_t ldb[2] = {w_first ? ldw : ldy, w_first ? ldy : ldw};
-    if ((s = launch_permute(Xp, ldx, buf[0], ldb[0], h->M, wc, h->perm, 0, st)) != TTDFT_OK) return s;
+    double* other = h->padded ? W2 : Yp;
+    const int64_t ldother = h->padded ? ldw : ldy;
+    double* buf[2] = {w_first ? W : other, w_first ? other : W};
+    const int64_t ldb[2] = {w_first ? ldw : ldother, w_first ? ldother : ldw};
+    if ((s = launch_permute(Xp, ldx, buf[0], ldb[0], h->Mt, wc, h->perm, 0, st)) != TTDFT_OK) return s;
     for (int k = 1; k <= m; ++k) {
       const int o = k & 1;
       const double al = alpha[k - 1], be = (k == 1) ? 0.0 : beta[k - 1];
       s = panel_step(h, al, -al * c, be, buf[o ^ 1], ldb[o ^ 1], k >= 2 ? buf[o] : nullptr, ldb[o], buf[o], ldb[o], wc, i8, k, m, st);
       if (s != TTDFT_OK) return s;
     }
-    if (buf[m & 1] != W) {   // in place with odd m: the result sits in Yp in tile order
+    if (buf[m & 1] != W) {   // in place with odd m: the result sits in the other buffer in tile order
+      if (h->padded) return launch_permute(other, ldother, Yp, ldy, h->Mt, wc, h->perm, 1, st);
       if ((s = launch_copy2d(Yp, ldy, W, ldw, h->M, wc, st)) != TTDFT_OK) return s;
     }
-    return launch_permute(W, ldw, Yp, ldy, h->M, wc, h->perm, 1, st);
+    return launch_permute(W, ldw, Yp, ldy, h->Mt, wc, h->perm, 1, st);
   }
   // destination of step k (1-based).  Out of place: Y_m lands in Yp, the iterates alternate Yp / W and
   // Y_{k+1} overwrites Y_{k-1} (read only at the output position).  In place: even steps land in Yp.
@@ -1212,7 +1283,7 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
   g_launches.fetch_add(5);
   // a transient handle describing X as a block-sparse matrix with nbm block rows of nkb dense 128 x 128 tiles
   ttdft_h_s hx;
-  hx.M = r.M; hx.kernel = 1; hx.bsr = 1; hx.b = 128; hx.nb = r.nbm; hx.nblocks = (int64_t)r.nbm * r.nkb;
+  hx.M = r.M; hx.Mt = r.M; hx.kernel = 1; hx.bsr = 1; hx.b = 128; hx.nb = r.nbm; hx.nblocks = (int64_t)r.nbm * r.nkb;
   hx.row_ptr = brow; hx.col = bcol;
   hx.i8_S = S; hx.math = TTDFT_MATH_I8X7; hx.eH = eX; hx.hdiag = nullptr;
   hx.k3_l2hints = env.k3_l2hints; hx.debug = env.debug;
@@ -1446,14 +1517,15 @@ static ttdft_status desc_counts(const ttdft_h_desc* d, int64_t* nrows_idx, int64
 // Scratch: flag word | M-int label histogram | perm | inv | per-block-row tile counts.  Inside ttdft_h_build it is the caller's
 // dev_storage (nothing has been written there yet; ttdft_h_storage_bytes reports at least analysis_bytes for a labelled CSR, so the
 // region always fits); ttdft_h_storage_bytes has no buffer to use and takes a transient allocation, freed before it returns.
-static size_t analysis_bytes(int64_t M) { return 1024 + 4 * align_up((size_t)M * 4, 1024); }
+static size_t analysis_region(int64_t M) { return align_up(((size_t)2 * M + 128) * 4, 1024); }   // a padded row map has <= 2M + 128 entries
+static size_t analysis_bytes(int64_t M) { return 1024 + 4 * analysis_region(M); }
 struct AnalysisScratch {
   uint8_t* p = nullptr;
   bool owned = false;
   int64_t M = 0;
   ~AnalysisScratch() { if (owned && p) cudaFree(p); }
   int32_t* flag() const { return reinterpret_cast<int32_t*>(p); }
-  int32_t* region(int k) const { return reinterpret_cast<int32_t*>(p + 1024 + (size_t)k * align_up((size_t)M * 4, 1024)); }
+  int32_t* region(int k) const { return reinterpret_cast<int32_t*>(p + 1024 + (size_t)k * analysis_region(M)); }
   int32_t* hist() const { return region(0); }
   int32_t* perm() const { return region(1); }
   int32_t* inv() const { return region(2); }
@@ -1467,12 +1539,25 @@ static ttdft_status d2h(void* dst, const void* src, size_t n, cudaStream_t st) {
 static bool wants_label_analysis(const ttdft_h_desc* d) {
   return d->fmt == TTDFT_FMT_CSR && d->subdomain_of_row && !(d->flags & TTDFT_FORCE_GENERIC) && d->M > 0;
 }
+static bool wants_packed(const ttdft_h_desc* d) { return (d->flags & TTDFT_PACKED) && !(d->flags & TTDFT_FORCE_GENERIC); }
+// scratch the sizing needs: the label analysis of a CSR, or the slab sizes of a BSR's packed copy (nslabs + 1 words)
+static size_t scratch_bytes(const ttdft_h_desc* d, int64_t nstored) {
+  if (wants_label_analysis(d)) return analysis_bytes(d->M);
+  if (d->fmt == TTDFT_FMT_BSR && d->block >= 16 && wants_packed(d) && nstored > 0)
+    return align_up(((size_t)nstored * (d->block / 16) + 1) * 4, 1024);
+  return 0;
+}
 
 // Decide the device format.  For CSR + usable subdomain labels: *hint_b = tile size (else 0) and *permuted tells
 // whether the rows have to be reordered (labels not already grouped).  All kernels and copies run on `st`.
-static ttdft_status plan_format(const ttdft_h_desc* d, const AnalysisScratch& sc, cudaStream_t st, int32_t* hint_b, bool* permuted) {
+// *nb = subdomains; *padded: the subdomains differ in size (labels 0..nb-1, each with 1..128 rows) and every one is padded with zero
+// rows/columns to the tile size *hint_b, the smallest of 32/64/96/128 that holds the largest (at most 2x the rows; A0).
+static ttdft_status plan_format(const ttdft_h_desc* d, const AnalysisScratch& sc, cudaStream_t st, int32_t* hint_b, bool* permuted,
+                                bool* padded, int64_t* nb_out) {
   *hint_b = 0;
   *permuted = false;
+  *padded = false;
+  *nb_out = 0;
   if (!wants_label_analysis(d)) return TTDFT_OK;
   ttdft_status s;
   int32_t* bad = sc.flag();
@@ -1487,7 +1572,7 @@ static ttdft_status plan_format(const ttdft_h_desc* d, const AnalysisScratch& sc
     hint_check_kernel<<<(unsigned)((d->M + 255) / 256), 256, 0, st>>>(d->M, d->subdomain_of_row, (int32_t)b, bad);
     g_launches.fetch_add(1);
     if ((s = d2h(&hb, bad, 4, st)) != TTDFT_OK) return s;
-    if (hb == 0) { *hint_b = (int32_t)b; return TTDFT_OK; }
+    if (hb == 0) { *hint_b = (int32_t)b; *nb_out = d->M / (int64_t)b; return TTDFT_OK; }
   }
   // (2) labels in any row order: they must be the subdomain indices 0..nb-1, each owning the same number b of rows
   int32_t* hist = sc.hist();
@@ -1498,22 +1583,42 @@ static ttdft_status plan_format(const ttdft_h_desc* d, const AnalysisScratch& sc
   int32_t b0 = 0;
   CUDA_TRY(cudaMemcpyAsync(&b0, hist, 4, cudaMemcpyDeviceToHost, st));
   if ((s = d2h(&hb, bad, 4, st)) != TTDFT_OK) return s;
-  if (hb != 0 || !k1_block_ok(b0) || d->M % b0 || d->M / b0 > (1 << 17)) return TTDFT_OK;
-  const int64_t nb = d->M / b0;
-  label_hist_check_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, st>>>(nb, b0, hist, bad);
+  if (hb != 0) return TTDFT_OK;                                      // a label outside [0, M)
+  if (k1_block_ok(b0) && d->M % b0 == 0 && d->M / b0 <= (1 << 17)) {
+    const int64_t nb = d->M / b0;
+    label_hist_check_kernel<<<(unsigned)((nb + 255) / 256), 256, 0, st>>>(nb, b0, hist, bad);
+    g_launches.fetch_add(1);
+    if ((s = d2h(&hb, bad, 4, st)) != TTDFT_OK) return s;
+    if (hb == 0) {
+      *hint_b = b0;
+      *permuted = true;
+      *nb_out = nb;
+      return TTDFT_OK;
+    }
+  }
+  // (3) subdomains of UNEQUAL size: labels 0..nb-1 without gaps, 1..128 rows each -> pad every subdomain to one tile size
+  int32_t* stats = sc.counts();                                      // 3 words of the counts region (not in use yet)
+  CUDA_TRY(cudaMemsetAsync(stats, 0, 12, st));
+  label_stats_kernel<<<(unsigned)((d->M + 255) / 256), 256, 0, st>>>(d->M, hist, stats);
   g_launches.fetch_add(1);
-  if ((s = d2h(&hb, bad, 4, st)) != TTDFT_OK) return s;
-  if (hb != 0) return TTDFT_OK;
-  *hint_b = b0;
+  int32_t hs[3] = {0, 0, 0};
+  if ((s = d2h(hs, stats, 12, st)) != TTDFT_OK) return s;
+  const int32_t maxsz = hs[0];
+  const int64_t nb = hs[1];
+  if (nb != hs[2] || maxsz < 1 || maxsz > 128 || nb > (1 << 17)) return TTDFT_OK;
+  const int32_t bt = maxsz <= 32 ? 32 : maxsz <= 64 ? 64 : maxsz <= 96 ? 96 : 128;
+  if (nb * bt > 2 * d->M + 128 || nb * bt >= 0x7fffffffLL) return TTDFT_OK;    // too much padding: the generic kernel is the better choice
+  *hint_b = bt;
   *permuted = true;
+  *padded = true;
+  *nb_out = nb;
   return TTDFT_OK;
 }
 
-static ttdft_status csr2bsr_counts(const ttdft_h_desc* d, int32_t b, const int32_t* perm, const int32_t* inv, int32_t* dev_counts,
+static ttdft_status csr2bsr_counts(const ttdft_h_desc* d, int64_t nb, int32_t b, const int32_t* perm, const int32_t* inv, int32_t* dev_counts,
                                    int32_t nnz, cudaStream_t st) {
-  const int64_t nb = d->M / b;
   const int32_t nwords = (int32_t)((nb + 31) / 32);
-  csr2bsr_count_kernel<<<(unsigned)nb, 256, (size_t)nwords * 4, st>>>(nb, b, d->row_ptr, d->col_idx, perm, inv, dev_counts, nwords, nnz);
+  csr2bsr_count_kernel<<<(unsigned)nb, 256, (size_t)nwords * 4, st>>>(nb, b, d->row_ptr, d->col_idx, perm, inv, dev_counts, nwords, nnz, d->M);
   CUDA_TRY(cudaGetLastError());
   g_launches.fetch_add(1);
   return TTDFT_OK;
@@ -1524,32 +1629,51 @@ static ttdft_status csr2bsr_counts(const ttdft_h_desc* d, int32_t b, const int32
 struct FormatPlan {
   int64_t nidx = 0, nstored = 0;
   int32_t hint_b = 0;
-  bool permuted = false;
-  size_t base = 0, i8 = 0;
+  bool permuted = false, padded = false;
+  int64_t nb = 0;                        // subdomains (labelled CSR)
+  size_t base = 0, i8 = 0, packed = 0;   // packed: slab offsets + packed slabs (bsr_packed.cuh), 0 if not built
 };
+// bytes of the packed region for nslabs slabs totalling `units` 16-byte units
+static size_t pk_region_bytes(int64_t nslabs, uint64_t units) { return align_up((size_t)(nslabs + 1) * 4, 1024) + align_up((size_t)units * 16, 1024); }
+// sizes of the packed slabs of dense tiles -> slab_ptr (device array of nslabs + 1 entries), total units to the host
+static ttdft_status pk_count(int32_t b, int64_t nslabs, const double* tiles, uint32_t* slab_ptr, cudaStream_t st, uint32_t* total) {
+  ttdft::pk_slabs_kernel<false><<<(unsigned)((nslabs + 7) / 8), 256, 0, st>>>(b, nslabs, tiles, slab_ptr, nullptr, nullptr);
+  ttdft::pk_scan_kernel<<<1, 1024, 0, st>>>(slab_ptr, nslabs + 1);
+  CUDA_TRY(cudaGetLastError());
+  g_launches.fetch_add(2);
+  return d2h(total, slab_ptr + nslabs, 4, st);
+}
 static ttdft_status storage_bytes_impl(const ttdft_h_desc* d, const AnalysisScratch& sc, cudaStream_t st, FormatPlan* f) {
-  ttdft_status s = plan_format(d, sc, st, &f->hint_b, &f->permuted);
+  ttdft_status s = plan_format(d, sc, st, &f->hint_b, &f->permuted, &f->padded, &f->nb);
   if (s != TTDFT_OK) return s;
   if (f->hint_b) {
     // count the tiles the conversion will create
     const int32_t hint_b = f->hint_b;
-    const int64_t nb = d->M / hint_b;
+    const int64_t nb = f->nb;
+    const int64_t Mt = nb * hint_b;      // rows of the tile-order space (> M when subdomains are padded)
     int32_t *perm = nullptr, *inv = nullptr;
     if (f->permuted) {
       perm = sc.perm();
       inv = sc.inv();
+      if (f->padded) CUDA_TRY(cudaMemsetAsync(perm, 0xFF, (size_t)Mt * 4, st));     // -1: padding row
       label_perm_kernel<<<(unsigned)nb, 256, 0, st>>>(d->M, hint_b, d->subdomain_of_row, perm, inv);
       g_launches.fetch_add(1);
     }
-    if ((s = csr2bsr_counts(d, hint_b, perm, inv, sc.counts(), (int32_t)f->nstored, st)) != TTDFT_OK) return s;
+    if ((s = csr2bsr_counts(d, nb, hint_b, perm, inv, sc.counts(), (int32_t)f->nstored, st)) != TTDFT_OK) return s;
     std::vector<int32_t> hc((size_t)nb);
     if ((s = d2h(hc.data(), sc.counts(), (size_t)nb * 4, st)) != TTDFT_OK) return s;
     int64_t nblocks = 0;
     for (int32_t c : hc) nblocks += c;
     // brow_ptr | counts | bcol | tiles | (perm | inv)
     f->base = align_up((size_t)(nb + 1) * 4, 1024) + align_up((size_t)nb * 4, 1024) + align_up((size_t)nblocks * 4, 1024) +
-              align_up((size_t)nblocks * hint_b * hint_b * 8, 1024) + (f->permuted ? 2 * align_up((size_t)d->M * 4, 1024) : 0);
-    if (!(d->flags & TTDFT_NO_I8) && nblocks > 0) f->i8 = i8_storage_bytes(nblocks, hint_b, d->M);
+              align_up((size_t)nblocks * hint_b * hint_b * 8, 1024) +
+              (f->permuted ? align_up((size_t)Mt * 4, 1024) + align_up((size_t)d->M * 4, 1024) : 0);
+    if (!(d->flags & TTDFT_NO_I8) && nblocks > 0) f->i8 = i8_storage_bytes(nblocks, hint_b, Mt);
+    if (wants_packed(d) && nblocks > 0 && nblocks * (hint_b / 16) < ((int64_t)1 << 31)) {
+      // the tiles do not exist yet: an upper bound (every stored entry non-zero, every slab padded by one value)
+      const int64_t nslabs = nblocks * (hint_b / 16);
+      f->packed = pk_region_bytes(nslabs, (uint64_t)nslabs * (4 * hint_b / 16) + ((uint64_t)f->nstored + (uint64_t)nslabs + 1) / 2);
+    }
     return TTDFT_OK;
   }
   const size_t per = (d->fmt == TTDFT_FMT_BSR) ? (size_t)d->block * d->block : 1;
@@ -1559,6 +1683,14 @@ static ttdft_status storage_bytes_impl(const ttdft_h_desc* d, const AnalysisScra
             align_up((size_t)f->nstored * per * 8, 1024) + 1024;
   if (d->fmt == TTDFT_FMT_BSR && k1_block_ok(d->block) && !(d->flags & (TTDFT_FORCE_GENERIC | TTDFT_NO_I8)) && f->nstored > 0)
     f->i8 = i8_storage_bytes(f->nstored, d->block, d->M);
+  if (d->fmt == TTDFT_FMT_BSR && k1_block_ok(d->block) && wants_packed(d) && f->nstored > 0 &&
+      f->nstored * (d->block / 16) < ((int64_t)1 << 31) && (size_t)f->nstored * d->block * d->block * 8 < ((size_t)1 << 35)) {
+    // exact: one pass over the input tiles counts the non-zeros of every slab (scratch: nslabs + 1 words at the start of sc.p)
+    const int64_t nslabs = f->nstored * (d->block / 16);
+    uint32_t total = 0;
+    if ((s = pk_count(d->block, nslabs, d->values, reinterpret_cast<uint32_t*>(sc.p), st, &total)) != TTDFT_OK) return s;
+    f->packed = pk_region_bytes(nslabs, total);
+  }
   return TTDFT_OK;
 }
 
@@ -1569,12 +1701,13 @@ ttdft_status ttdft_h_storage_bytes(const ttdft_h_desc* d, size_t* bytes) {
   if (s != TTDFT_OK) return s;
   AnalysisScratch sc;
   sc.M = d->M;
-  if (wants_label_analysis(d)) {
-    CUDA_TRY(cudaMalloc(&sc.p, analysis_bytes(d->M)));   // transient: this call has no caller buffer to work in
+  const size_t scratch = scratch_bytes(d, f.nstored);
+  if (scratch) {
+    CUDA_TRY(cudaMalloc(&sc.p, scratch));                // transient: this call has no caller buffer to work in
     sc.owned = true;
   }
   if ((s = storage_bytes_impl(d, sc, nullptr, &f)) != TTDFT_OK) return s;
-  *bytes = std::max(f.base + f.i8, wants_label_analysis(d) ? analysis_bytes(d->M) : (size_t)0);
+  *bytes = std::max(f.base + f.i8 + f.packed, scratch);
   return TTDFT_OK;
 }
 
@@ -1586,7 +1719,7 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
   if (s != TTDFT_OK) return s;
   const int64_t nidx = f.nidx, nstored = f.nstored;
   const bool checks = d->M > 0 && (d->flags & (TTDFT_CHECK_SORTED | TTDFT_CHECK_SYMMETRY));
-  const size_t scratch_need = wants_label_analysis(d) ? analysis_bytes(d->M) : (checks ? (size_t)1024 : (size_t)0);
+  const size_t scratch_need = std::max(scratch_bytes(d, f.nstored), checks ? (size_t)1024 : (size_t)0);
   if (d->M > 0 && (!dev_storage || (reinterpret_cast<uintptr_t>(dev_storage) & 1023)))
     return fail(TTDFT_ERR_INVALID_ARG, "dev_storage must be a 1024-byte aligned device pointer");
   if (bytes < scratch_need)
@@ -1627,21 +1760,23 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
   const size_t need = f.base, need_i8 = f.i8;
   const int32_t hint_b = f.hint_b;
   const bool permuted = f.permuted;
-  if (bytes < need + need_i8)
-    return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "dev_storage has %zu bytes, %zu needed", bytes, need + need_i8);
+  if (bytes < need + need_i8 + f.packed)
+    return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "dev_storage has %zu bytes, %zu needed", bytes, need + need_i8 + f.packed);
 
   ttdft_h_s* h = new (std::nothrow) ttdft_h_s;
   if (!h) return fail(TTDFT_ERR_CUDA, "out of host memory");
   h->M = d->M;
+  h->Mt = d->M;
   h->sym_checked = (d->M > 0 && (d->flags & TTDFT_CHECK_SYMMETRY)) ? 1 : 0;   // reached only if the check passed
   h->skip_empty = (d->flags & TTDFT_OWNED_ROWS_ONLY) ? 1 : 0;
-  h->storage_bytes = need + need_i8;
+  h->storage_bytes = need + need_i8 + f.packed;
   uint8_t* base = reinterpret_cast<uint8_t*>(dev_storage);
 
   if (hint_b) {
     // ---- CSR with subdomain labels -> block-sparse tiles (rows of a subdomain contiguous) ----
     const int32_t b = hint_b;
-    const int64_t nb = d->M / b;
+    const int64_t nb = f.nb;
+    const int64_t Mt = nb * b;
     const int32_t nwords = (int32_t)((nb + 31) / 32);
     int32_t* brow = reinterpret_cast<int32_t*>(base);
     int32_t* counts = reinterpret_cast<int32_t*>(base + align_up((size_t)(nb + 1) * 4, 1024));
@@ -1649,11 +1784,12 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     if (permuted) {
       // the row maps live at the end of the fp64 format: reordered row r is the caller's row perm[r]
       inv = reinterpret_cast<int32_t*>(base + need - align_up((size_t)d->M * 4, 1024));
-      perm = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(inv) - align_up((size_t)d->M * 4, 1024));
+      perm = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(inv) - align_up((size_t)Mt * 4, 1024));
+      if (f.padded && cudaMemsetAsync(perm, 0xFF, (size_t)Mt * 4, st) != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "memset of the row map"); }
       label_perm_kernel<<<(unsigned)nb, 256, 0, st>>>(d->M, b, d->subdomain_of_row, perm, inv);
       g_launches.fetch_add(1);
     }
-    s = csr2bsr_counts(d, b, perm, inv, counts, (int32_t)nstored, st);
+    s = csr2bsr_counts(d, nb, b, perm, inv, counts, (int32_t)nstored, st);
     if (s != TTDFT_OK) { delete h; return s; }
     exclusive_scan_small<<<1, 1, 0, st>>>(nb, counts, brow);
     g_launches.fetch_add(1);
@@ -1666,11 +1802,12 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     e = cudaMemsetAsync(tiles, 0, (size_t)nblocks * b * b * 8, st);
     if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "memset: %s", cudaGetErrorString(e)); }
     csr2bsr_fill_kernel<<<(unsigned)nb, 256, (size_t)nwords * 8, st>>>(nb, b, d->row_ptr, d->col_idx, d->values, perm, inv, brow,
-                                                                       bcol, tiles, nwords, (int32_t)nstored);
+                                                                       bcol, tiles, nwords, (int32_t)nstored, d->M);
     e = cudaGetLastError();
     if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "csr->bsr fill: %s", cudaGetErrorString(e)); }
     g_launches.fetch_add(1);
     h->perm = perm;
+    h->Mt = Mt; h->padded = f.padded ? 1 : 0;
     h->bsr = 1; h->b = b; h->nb = nb; h->nblocks = nblocks;
     h->row_ptr = brow; h->col = bcol; h->val = tiles;
     h->kernel = 1;
@@ -1720,7 +1857,7 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     int8_t* Hd = reinterpret_cast<int8_t*>(q);
     q += align_up((size_t)h->nblocks * I8_S * h->b * 128, 1024);
     int32_t* eH = reinterpret_cast<int32_t*>(q);
-    q += align_up((size_t)h->M * 4, 1024);
+    q += align_up((size_t)h->Mt * 4, 1024);
     double* hdiag = reinterpret_cast<double*>(q);
     ttdft::h_rowscale_kernel<<<(unsigned)h->nb, 256, 0, st>>>(h->b, h->row_ptr, h->col, h->val, eH, hdiag);
     ttdft::h_digits_kernel<I8_S><<<(unsigned)h->nb, 256, 0, st>>>(h->b, h->row_ptr, h->col, h->val, eH, Hd);
@@ -1752,6 +1889,27 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
       h->nsm = nsm;
     h->math = env.math;
   }
+  if (h->kernel == 1 && f.packed > 0) {
+    // ---- packed tiles for the HBM-bound small-N regime (bsr_packed.cuh): slab sizes, offsets, then the slabs ----
+    const int64_t nslabs = h->nblocks * (h->b / 16);
+    uint8_t* q = base + need + need_i8;
+    uint32_t* pk_ptr = reinterpret_cast<uint32_t*>(q);
+    uint8_t* pk_data = q + align_up((size_t)(nslabs + 1) * 4, 1024);
+    uint32_t total = 0;
+    if ((s = pk_count(h->b, nslabs, h->val, pk_ptr, st, &total)) != TTDFT_OK) { delete h; return s; }
+    if (pk_region_bytes(nslabs, total) > f.packed) { delete h; return fail(TTDFT_ERR_CUDA, "packed tiles: size changed between sizing and build"); }
+    std::vector<int32_t> hb((size_t)h->nb + 1);
+    if ((s = d2h(hb.data(), h->row_ptr, hb.size() * 4, st)) != TTDFT_OK) { delete h; return s; }
+    int64_t maxj = 0;
+    for (int64_t I = 0; I < h->nb; ++I) maxj = std::max<int64_t>(maxj, hb[(size_t)I + 1] - hb[(size_t)I]);
+    if (maxj * (h->b / 16) < 2047) {             // the kernel keeps a block row's slab offsets in shared memory
+      ttdft::pk_slabs_kernel<true><<<(unsigned)((nslabs + 7) / 8), 256, 0, st>>>(h->b, nslabs, h->val, nullptr, pk_ptr, pk_data);
+      cudaError_t e = cudaGetLastError();
+      if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "packed tiles: %s", cudaGetErrorString(e)); }
+      g_launches.fetch_add(1);
+      h->pk_ptr = pk_ptr; h->pk_data = pk_data; h->pk_bytes = (size_t)total * 16;
+    }
+  }
   *out = h;
   return TTDFT_OK;
 }
@@ -1766,7 +1924,8 @@ ttdft_status ttdft_h_info(ttdft_h_t h, ttdft_h_info_t* info) {
   info->storage_bytes = h->storage_bytes;
   info->i8_planes = h->i8_S;
   info->reordered = h->perm ? 1 : 0;
-  info->reserved = 0;
+  info->padded = h->padded;
+  info->packed_bytes = (int64_t)h->pk_bytes;
   const int used = i8_planes_in_use(h);
   info->math = used == 7 ? TTDFT_MATH_I8X7 : used == 6 ? TTDFT_MATH_I8 : TTDFT_MATH_FP64;
   return TTDFT_OK;
@@ -1824,7 +1983,7 @@ ttdft_status ttdft_cheb_step(ttdft_h_t h, double alpha, double c, double beta, c
 // were reordered by label two panels in tile order (the multiplied block; the output, which also carries Z in)
 static size_t step_work_need(const ttdft_h_s* h, int64_t ncols, size_t* panel_bytes) {
   const int64_t ldp = ncols + (ncols & 1);
-  *panel_bytes = h->perm ? align_up((size_t)h->M * (size_t)ldp * 8, 1024) : 0;
+  *panel_bytes = h->perm ? align_up((size_t)h->Mt * (size_t)ldp * 8, 1024) : 0;
   return 2 * *panel_bytes + (want_i8(h) ? i8_work_bytes(h, ncols, 1) : 0);
 }
 
@@ -1853,16 +2012,16 @@ static ttdft_status step_ws(ttdft_h_t h, double alpha, double gamma, double beta
   const int64_t ldp = ncols + (ncols & 1);
   double* Xt = reinterpret_cast<double*>(wb);
   double* Ot = reinterpret_cast<double*>(wb + pb);
-  ttdft_status s = launch_permute(X, ldx, Xt, ldp, h->M, ncols, h->perm, 0, st);
+  ttdft_status s = launch_permute(X, ldx, Xt, ldp, h->Mt, ncols, h->perm, 0, st);
   if (s != TTDFT_OK) return s;
   const bool use_z = (beta != 0.0) && Z;
-  if (use_z && (s = launch_permute(Z, ldz, Ot, ldp, h->M, ncols, h->perm, 0, st)) != TTDFT_OK) return s;
+  if (use_z && (s = launch_permute(Z, ldz, Ot, ldp, h->Mt, ncols, h->perm, 0, st)) != TTDFT_OK) return s;
   if (want_i8(h))
     s = launch_step_i8(h, alpha, gamma, use_z ? beta : 0.0, Xt, ldp, use_z ? Ot : nullptr, ldp, Ot, ldp, ncols, k3, 0, false, false, false, st);
   else
     s = launch_step(h, alpha, gamma, use_z ? beta : 0.0, Xt, ldp, use_z ? Ot : nullptr, ldp, Ot, ldp, ncols, st);
   if (s != TTDFT_OK) return s;
-  return launch_permute(Ot, ldp, O, ldo, h->M, ncols, h->perm, 1, st);
+  return launch_permute(Ot, ldp, O, ldo, h->Mt, ncols, h->perm, 1, st);
 }
 
 ttdft_status ttdft_spmm_ws(ttdft_h_t h, double alpha, const double* X, int64_t ldx, double beta, double* Y, int64_t ldy,
@@ -1912,13 +2071,16 @@ ttdft_status ttdft_cheb_scalars(int32_t m, double a, double b, double a0, double
   return TTDFT_OK;
 }
 
+// scratch panels of the filter: one, or two for a padded handle (its tile-order space does not fit the caller's Y panel)
+static size_t filter_panels(const ttdft_h_s* h) { return h->padded ? 2 : 1; }
+
 ttdft_status ttdft_cheb_filter_work_bytes(ttdft_h_t h, int64_t ncols, int64_t panel_cols, size_t* bytes) {
   if (!h || !bytes) return fail(TTDFT_ERR_INVALID_ARG, "NULL argument");
   if (ncols < 1 || panel_cols < 0) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1 and panel_cols >= 0");
   int64_t w = panel_cols ? std::min(panel_cols, ncols) : default_panel(ncols);
   w += (w & 1);   // even leading dimension keeps the scratch panel TMA / 128-bit friendly
-  *bytes = (size_t)h->M * (size_t)w * 8;
-  if (want_i8(h)) *bytes = align_up(*bytes, 1024) + i8_work_bytes(h, w, 2);   // + digit planes of two iterates (read / being written)
+  *bytes = filter_panels(h) * align_up((size_t)h->Mt * (size_t)w * 8, 1024);      // scratch panel(s) in tile order
+  if (want_i8(h)) *bytes += i8_work_bytes(h, w, 2);   // + digit planes of two iterates (read / being written)
   return TTDFT_OK;
 }
 
@@ -1948,11 +2110,13 @@ ttdft_status ttdft_cheb_filter(ttdft_h_t h, const double* X, int64_t ldx, double
   const int64_t w = panel_cols ? std::min(panel_cols, ncols) : default_panel(ncols);
   const int64_t ldw = w + (w & 1);
   I8Work k3;
-  if (i8) k3 = carve_i8_work(h, reinterpret_cast<uint8_t*>(work) + align_up((size_t)h->M * (size_t)ldw * 8, 1024), ldw, 2);
+  const size_t pbytes = align_up((size_t)h->Mt * (size_t)ldw * 8, 1024);
+  if (i8) k3 = carve_i8_work(h, reinterpret_cast<uint8_t*>(work) + filter_panels(h) * pbytes, ldw, 2);
+  double* W2 = h->padded ? reinterpret_cast<double*>(reinterpret_cast<uint8_t*>(work) + pbytes) : nullptr;
   for (int64_t c0 = 0; c0 < ncols; c0 += w) {
     const int64_t wc = std::min(w, ncols - c0);
     s = filter_panel(h, X + c0, ldx, Y + c0, ldy, reinterpret_cast<double*>(work), ldw, wc, m, c, alpha.data(), beta.data(),
-                     inplace, (cudaStream_t)stream, i8 ? &k3 : nullptr);
+                     inplace, (cudaStream_t)stream, i8 ? &k3 : nullptr, W2);
     if (s != TTDFT_OK) return s;
   }
   return TTDFT_OK;
@@ -1963,7 +2127,8 @@ ttdft_status ttdft_cheb_filter_host_work_bytes(ttdft_h_t h, int64_t ncols, int64
   if (ncols < 1 || panel_cols < 0) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1 and panel_cols >= 0");
   int64_t w = panel_cols ? std::min(panel_cols, ncols) : std::min<int64_t>(ncols, 1024);
   w += (w & 1);
-  *bytes = 5 * align_up((size_t)h->M * (size_t)w * 8, 1024);   // 2 x (X panel, Y panel) + scratch
+  *bytes = 4 * align_up((size_t)h->M * (size_t)w * 8, 1024) +                  // 2 x (X panel, Y panel)
+           filter_panels(h) * align_up((size_t)h->Mt * (size_t)w * 8, 1024);   // + scratch panel(s) in tile order
   if (want_i8(h)) *bytes += i8_work_bytes(h, w, 2);
   return TTDFT_OK;
 }
@@ -1987,13 +2152,15 @@ ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* Xh, int64_t ldx, 
   const int64_t w = panel_cols ? std::min(panel_cols, ncols) : std::min<int64_t>(ncols, 1024);
   const int64_t ldw = w + (w & 1);
   const size_t pbytes = align_up((size_t)h->M * (size_t)ldw * 8, 1024);
+  const size_t tbytes = align_up((size_t)h->Mt * (size_t)ldw * 8, 1024);
   uint8_t* base = reinterpret_cast<uint8_t*>(work);
   double* dX[2] = {reinterpret_cast<double*>(base), reinterpret_cast<double*>(base + pbytes)};
   double* dY[2] = {reinterpret_cast<double*>(base + 2 * pbytes), reinterpret_cast<double*>(base + 3 * pbytes)};
   double* dW = reinterpret_cast<double*>(base + 4 * pbytes);
+  double* dW2 = h->padded ? reinterpret_cast<double*>(base + 4 * pbytes + tbytes) : nullptr;
   const bool i8 = want_i8(h) && m >= 1 && h->M > 0;
   I8Work k3;
-  if (i8) k3 = carve_i8_work(h, base + 5 * pbytes, ldw, 2);
+  if (i8) k3 = carve_i8_work(h, base + 4 * pbytes + filter_panels(h) * tbytes, ldw, 2);
 
   cudaStream_t sc = (cudaStream_t)stream, sin = nullptr, sout = nullptr;
   cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr}, ev_start = nullptr;
@@ -2042,7 +2209,7 @@ ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* Xh, int64_t ldx, 
     // compute once the panel has arrived and dY[buf]'s previous contents have left
     HOST_TRY(cudaStreamWaitEvent(sc, ev_in[buf], 0));
     if (ip >= 2) HOST_TRY(cudaStreamWaitEvent(sc, ev_out[buf], 0));
-    s = filter_panel(h, dX[buf], ldw, dY[buf], ldw, dW, ldw, wc, m, c, alpha.data(), beta.data(), false, sc, i8 ? &k3 : nullptr);
+    s = filter_panel(h, dX[buf], ldw, dY[buf], ldw, dW, ldw, wc, m, c, alpha.data(), beta.data(), false, sc, i8 ? &k3 : nullptr, dW2);
     if (s != TTDFT_OK) { cudaDeviceSynchronize(); cleanup(); return s; }
     HOST_TRY(cudaEventRecord(ev_comp[buf], sc));
     // device -> host on the output stream

@@ -138,7 +138,16 @@ def test_labels_that_do_not_qualify_keep_csr(tt):
     H, Cp, labels, _ = permuted_problem(4, 32, 0.0, 3032)
     bad = labels.copy()
     i = int(np.flatnonzero(bad == 3)[0])
-    bad[i] = 4                                    # subdomain 3 owns 31 rows, subdomain 4 owns 33
+    bad[i] = 4                                    # subdomain 3 owns 31 rows, subdomain 4 owns 33: unequal sizes are padded (to 64)
+    Hu = build(tt, Cp, bad)
+    assert Hu.info()["kernel"] == 1 and Hu.info()["padded"] == 1 and Hu.info()["block"] == 64
+    X = synth.dense_normal(H.M, 20, 86)
+    import torch
+    Y = torch.empty(H.M, 20, dtype=torch.float64, device="cuda")
+    tt.spmm(Hu, 1.0, dev(X), 0.0, Y, use_work=True)
+    assert relerr(Y.cpu().numpy(), oracle.spmm(Cp.row_ptr, Cp.col_idx, Cp.values, 1.0, X)) <= TOL_SPMM
+    bad = labels.copy()
+    bad[bad == 7] = 9                             # a gap in the labels (no subdomain 7): not the indices 0..nb-1
     assert build(tt, Cp, bad).info()["kernel"] == 0
     bad = labels.copy()
     bad[0] = -1
@@ -146,3 +155,85 @@ def test_labels_that_do_not_qualify_keep_csr(tt):
     bad = labels + 5                              # not the indices 0..nb-1
     assert build(tt, Cp, bad).info()["kernel"] == 0
     assert build(tt, Cp, labels, flags=tt.FORCE_GENERIC).info()["kernel"] == 0
+
+
+def unequal_problem(G, bmax, lo, z, seed):
+    """A planted partition with subdomains of UNEQUAL size: the generator's H (G^3 subdomains of bmax functions) with a random subset
+    of every subdomain's functions removed (lo .. bmax kept), then symmetrically permuted.  Returns (permuted CSR, labels, bounds)."""
+    H, C, _, (a0, bb) = small_problem(G, bmax, z, seed)
+    rng = np.random.default_rng(seed)
+    nb = H.M // bmax
+    keep = np.zeros(H.M, bool)
+    for L in range(nb):
+        s = int(rng.integers(lo, bmax + 1))
+        keep[L * bmax + rng.choice(bmax, s, replace=False)] = True
+    keep[:bmax] = True                                        # one subdomain at full size: the tile size is bmax
+    idx = np.nonzero(keep)[0]
+    newid = -np.ones(H.M, np.int64)
+    newid[idx] = np.arange(len(idx))
+    rp = [0]
+    ci, va = [], []
+    for i in idx:
+        cols = C.col_idx[C.row_ptr[i]:C.row_ptr[i + 1]]
+        vals = C.values[C.row_ptr[i]:C.row_ptr[i + 1]]
+        sel = keep[cols]
+        ci.append(newid[cols[sel]])
+        va.append(vals[sel])
+        rp.append(rp[-1] + int(sel.sum()))
+    Cs = synth.CSR(len(idx), np.array(rp, np.int32), np.concatenate(ci).astype(np.int32), np.concatenate(va))
+    lab = (idx // bmax).astype(np.int32)
+    perm = synth.permutation(Cs.M, seed + 50)
+    Cp = synth.permute_csr(Cs, perm)
+    labels = np.empty(Cs.M, np.int32)
+    labels[perm] = lab
+    return Cp, labels, nb, (a0 - 0.5, bb + 0.5)               # deleting rows/columns only shrinks the spectral range (interlacing)
+
+
+@pytest.mark.parametrize("G,bmax,lo,z", [(3, 128, 80, 0.4), (3, 96, 70, 0.4), (3, 64, 40, 0.3), (4, 32, 20, 0.0)])
+def test_unequal_subdomain_sizes_are_padded_to_tiles(tt, G, bmax, lo, z):
+    """Labels whose groups differ in size (the Tucker ranks differ per subdomain) still run on the tile kernels: every
+    subdomain is padded to the tile size inside h_build, X and Y stay in the caller's row order and size."""
+    import torch
+    Cp, labels, nb, (a0, bb) = unequal_problem(G, bmax, lo, z, 3300 + bmax)
+    M = Cp.M
+    assert len(set(np.bincount(labels))) > 3                 # really unequal
+    Hd = build(tt, Cp, labels, flags=tt.CHECK_SORTED | tt.CHECK_SYMMETRY)
+    info = Hd.info()
+    assert info["kernel"] == 1 and info["block"] == bmax and info["reordered"] == 1 and info["padded"] == 1 and info["M"] == M
+    N, m = 70, 9
+    a, bq, a0q = bounds_for(a0, bb, N, M)
+    X = synth.dense_normal(M, N, 83)
+    Y0 = synth.dense_normal(M, N, 84)
+    ref_mm = oracle.spmm(Cp.row_ptr, Cp.col_idx, Cp.values, -0.75, X, 2.5, Y0.copy())
+    ref_f = oracle.cheb_filter(Cp.row_ptr, Cp.col_idx, Cp.values, X, m, a, bq, a0q)
+    Y = dev(Y0)
+    tt.spmm(Hd, -0.75, dev(X), 2.5, Y)                        # without scratch: the generic kernel through the row map
+    assert relerr(Y.cpu().numpy(), ref_mm) <= TOL_SPMM
+    modes = [tt.MATH_FP64] + ([tt.MATH_I8X7, tt.MATH_I8] if info["i8_planes"] and bmax >= 64 else [])
+    for mode in modes:
+        Hd.set_math_mode(mode)
+        Y = dev(Y0)
+        tt.spmm(Hd, -0.75, dev(X), 2.5, Y, use_work=True)     # gather -> tile kernel on the padded space -> scatter
+        assert relerr(Y.cpu().numpy(), ref_mm) <= TOL_SPMM
+        for inplace in (False, True):
+            Xd = dev(X)
+            Yd = Xd if inplace else torch.full((M, N), float("nan"), dtype=torch.float64, device="cuda")
+            tt.cheb_filter(Hd, Xd, Yd, m, a, bq, a0q, panel_cols=48)
+            got = Yd.cpu().numpy()
+            assert relerr(got, ref_f) <= TOL_FILTER and worst_col_relerr(got, ref_f) <= 10 * TOL_FILTER
+        Yd = torch.empty((M, N), dtype=torch.float64, device="cuda")
+        tt.cheb_filter(Hd, dev(X), Yd, 4, a, bq, a0q)          # even degree, one panel
+        assert relerr(Yd.cpu().numpy(), oracle.cheb_filter(Cp.row_ptr, Cp.col_idx, Cp.values, X, 4, a, bq, a0q)) <= TOL_FILTER
+    # Lanczos bounds and the projection on the padded handle
+    v0 = synth.dense_normal(M, 1, 85).reshape(-1)
+    la0, lb, _ = tt.lanczos_bounds(Hd, dev(v0), 20)
+    ra0, rb, _ = oracle.lanczos_bounds(Cp.row_ptr, Cp.col_idx, Cp.values, v0, 20)
+    assert abs(la0 - ra0) <= 1e-9 * (rb - ra0) and abs(lb - rb) <= 1e-9 * (rb - ra0)
+    Hd.set_math_mode(tt.MATH_AUTO)
+    G_ = torch.empty((N, N), dtype=torch.float64, device="cuda")
+    tt.project(Hd, dev(X), G_)
+    assert relerr(G_.cpu().numpy(), oracle.project(Cp.row_ptr, Cp.col_idx, Cp.values, X)) <= 1e-12
+    # too much padding (tiny groups): the generic format is kept
+    tiny = (np.arange(M) // 3).astype(np.int32)
+    Hg = tt.h_build_csr(M, dev(Cp.row_ptr), dev(Cp.col_idx), dev(Cp.values), subdomain_of_row=dev(tiny))
+    assert Hg.info()["kernel"] == 0 and Hg.info()["padded"] == 0
