@@ -184,6 +184,26 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_sweep(sweep_argv):
+    """Config 5 with parity: sweep.py times, the oracle checks each timed product on a seeded column sample."""
+    import torch
+    import oracle
+    from paper_2110_15853_b200 import sweep
+
+    def check(C, op, coeffs, X, Z, O):
+        n = X.shape[1]
+        cols = np.unique(np.concatenate([[0, n - 1], np.random.default_rng(n).integers(0, n, 14)]))
+        cd = torch.from_numpy(cols).to(X.device)
+        Xs, Zs, got = (np.ascontiguousarray(t[:, cd].cpu().numpy()) for t in (X, Z, O))
+        if op == "spmm":
+            ref = oracle.spmm(C.row_ptr, C.col_idx, C.values, coeffs[0], Xs)
+        else:
+            ref = oracle.cheb_step(C.row_ptr, C.col_idx, C.values, coeffs[0], coeffs[1], coeffs[2], Xs, Zs)
+        return float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
+
+    sweep.main(sweep_argv, check=check)
+
+
 def workload_config(cfg, nnz, nblocks, args):
     return {
         "workload": f"BASELINE.json config '{cfg.name}': G={cfg.G} b={cfg.b} M={cfg.M} N={cfg.N} m={cfg.m} "
@@ -217,7 +237,13 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-project", action="store_true", help="skip the subspace-projection (NEXT-1) measurement")
+    ap.add_argument("--sweep", nargs=argparse.REMAINDER, default=None,
+                    help="BASELINE.json config 5 instead of the headline: the timings of paper_2110_15853_b200.sweep (its own options may "
+                         "follow, e.g. --sweep --ns 16,256 --layouts bsr,csr) with a relerr column -- every timed product compared with "
+                         "the CPU oracle on 16 seeded columns (columns are independent in one product)")
     args = ap.parse_args()
+    if args.sweep is not None:
+        return run_sweep(args.sweep)
     if args.ref_cols <= 0:
         args.ref_cols = 16 if args.impl == "reference" else 48
     if args.impl == "reference":

@@ -32,7 +32,7 @@
  *   TTDFT_K3_L2HINTS  0, 1 or 2: L2 eviction hints of the int8 step kernel's TMA loads (0 none, 1 evict-first
  *                     H planes + evict-last Y digit tiles, 2 only the latter); default: chosen per launch.
  *   TTDFT_K3_T        0 or 1: int8 step on kernel K3 (rows of the tile on the MMA's M axis) or K3T (transposed: columns of Y on
- *                     M, no padding rows for tiles narrower than 128); default: K3T for 96-wide tiles, K3 otherwise.
+ *                     M, no padding rows for tiles narrower than 128); default: K3T for 64- and 96-wide tiles, K3 for 128.
  *   TTDFT_K4_CLUSTER  1 or 2: CTA-cluster size of the int8 Gram kernel; default 2.
  *   TTDFT_K3_PREDICT_BIAS  test hook, -64..8, default 0: added to every predicted column exponent of the filter's int8
  *                     path (negative: predictions fail and the fallback extraction runs; positive: digits lose that many bits).

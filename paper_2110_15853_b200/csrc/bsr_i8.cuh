@@ -58,6 +58,7 @@ struct K3Params {
   int8_t* dO = nullptr;
   const int32_t* ePredO = nullptr;
   uint32_t* flagsO = nullptr;
+  uint32_t* counter = nullptr;     // work counter of this launch (one word, ZERO at launch): clusters draw their work items from it
   int32_t skip_empty = 0;          // 1: block rows without tiles are not this handle's: their output rows are left untouched
   int64_t mrows;                   // valid rows (= nb*b for a Hamiltonian; < nb*b for the ragged last block of ttdft_rotate)
   int32_t l2hints;                 // 1: evict-first H planes, evict-last Y digit tiles; 2: only the latter; 0: none (< 0 on the host: chosen per launch)
@@ -97,7 +98,8 @@ struct K3Cfg {
   static constexpr int CS_OFFSET = BAR_OFFSET + 8 * ((NBAR + 1) & ~1);   // 64 doubles: column scales
   static constexpr int CM_OFFSET = CS_OFFSET + 64 * 8;                   // 64 words: column maxima
   static constexpr int CP_OFFSET = CM_OFFSET + 64 * 4 + 16;              // 64 words: predicted exponents of the output columns (behind the tmem slot)
-  static constexpr int TOTAL = CP_OFFSET + 64 * 4 + 1024;                // + alignment slack
+  static constexpr int Q_OFFSET = CP_OFFSET + 64 * 4;                    // work-item queue (K3Queue, 8-byte aligned)
+  static constexpr int TOTAL = Q_OFFSET + 192 + 1024;                    // + alignment slack
   static_assert(S * K3_NT <= 512, "digit levels must fit TMEM");
   static_assert(NH >= 3, "H ring too short");
 };
@@ -255,6 +257,91 @@ __device__ __forceinline__ void cluster_sync_all() {
   asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
+// ------------------------------------------------------------------------------------------------
+// Dynamic work distribution.  Work items are drawn from ONE global counter, so the clusters that run at the same time always work
+// on a contiguous window of items -- with a static round-robin the clusters drift apart by the differences in item length (8..27
+// tiles per block row) until the active block rows are spread over hundreds of rows, and the Y digit tiles that neighbouring block
+// rows share leave L2 between their uses (ncu, config 4: 204 GB of DRAM traffic per launch, 76 % of the HBM peak).
+// The producer lane of the cluster's CTA 0 draws the items (a few ahead) and hands each one to every role of every CTA of the
+// cluster through a small queue in shared memory: item word + `qfull` mbarrier in each CTA (written remotely for the peers),
+// `qempty` in CTA 0 (every consumer arrives there as soon as it has read the item).
+// ------------------------------------------------------------------------------------------------
+constexpr int K3_NQ = 8;                         // queue slots
+constexpr int K3_QAHEAD = 4;                     // items drawn ahead of the producer's own position
+constexpr int K3_QCONS = 10;                     // consumers per CTA: producer lane, MMA lane, 8 epilogue warps
+constexpr uint32_t K3_NOITEM = 0xffffffffu;
+struct K3Queue {
+  uint64_t qfull[K3_NQ];
+  uint64_t qempty[K3_NQ];
+  uint32_t item[K3_NQ];
+};
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t laddr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(laddr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {      // acquires writes of the whole cluster
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAITC_%=:\n"
+      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONEC_%=;\n"
+      "bra WAITC_%=;\n"
+      "DONEC_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+// the fetcher (CTA 0 of the cluster): item -> slot of every CTA
+template <int C>
+__device__ __forceinline__ void k3_q_push(K3Queue* q, int slot, uint32_t u) {
+#pragma unroll
+  for (int r = 0; r < C; ++r) {
+    const uint32_t ia = mapa_u32(smem_u32(&q->item[slot]), (uint32_t)r), ba = mapa_u32(smem_u32(&q->qfull[slot]), (uint32_t)r);
+    asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(ia), "r"(u) : "memory");
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(ba) : "memory");
+  }
+}
+// a consumer: next item of this CTA's queue; `arrive`: this thread reports the slot as read (one thread per consumer)
+__device__ __forceinline__ uint32_t k3_q_pop(K3Queue* q, int& slot, uint32_t& phase, bool arrive) {
+  mbar_wait_cluster(&q->qfull[slot], phase);
+  const uint32_t u = q->item[slot];
+  if (arrive) {
+    const uint32_t ea = mapa_u32(smem_u32(&q->qempty[slot]), 0u);
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(ea) : "memory");
+  }
+  if (++slot == K3_NQ) { slot = 0; phase ^= 1; }
+  return u;
+}
+// the same for a whole (converged) warp: lane 0 waits, reads and reports, the others take the item from it
+__device__ __forceinline__ uint32_t k3_q_pop_warp(K3Queue* q, int& slot, uint32_t& phase) {
+  uint32_t u = 0;
+  if ((threadIdx.x & 31) == 0) {
+    int s = slot;
+    uint32_t ph = phase;
+    u = k3_q_pop(q, s, ph, true);
+  }
+  u = __shfl_sync(0xffffffffu, u, 0);
+  if (++slot == K3_NQ) { slot = 0; phase ^= 1; }
+  return u;
+}
+// state of the fetcher
+struct K3Fetch {
+  int slot = 0;
+  uint32_t phase = 0;
+  bool done = false;
+};
+template <int C>
+__device__ __forceinline__ void k3_q_fetch(K3Queue* q, K3Fetch& f, uint32_t* counter, uint32_t nitems) {
+  if (f.done) return;
+  mbar_wait_cluster(&q->qempty[f.slot], f.phase ^ 1);       // every consumer of every CTA has read the slot's previous item
+  uint32_t u = atomicAdd(counter, 1u);
+  if (u >= nitems) { u = K3_NOITEM; f.done = true; }        // one end marker, then nothing more is drawn
+  k3_q_push<C>(q, f.slot, u);
+  if (++f.slot == K3_NQ) { f.slot = 0; f.phase ^= 1; }
+}
+
 // cluster work item u -> (block row I, tile group ctg): scheduling groups of cgc tile groups outermost, then
 // block rows, tile group fastest (clusters that run at the same time share H planes and Y rows in L2)
 __device__ __forceinline__ void k3_decode(const K3Params& prm, int64_t u, int32_t& I, int32_t& ctg) {
@@ -298,11 +385,11 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
   uint32_t* cm_s = reinterpret_cast<uint32_t*>(smem + Cf::CM_OFFSET);    // column maxima of the current tile
   uint32_t* tmem_slot = cm_s + 64;
   int32_t* cp_s = reinterpret_cast<int32_t*>(smem + Cf::CP_OFFSET);      // predicted exponents of the output columns
+  K3Queue* wq = reinterpret_cast<K3Queue*>(smem + Cf::Q_OFFSET);         // work items of this cluster
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t nitems = (int64_t)prm.nb * prm.nctg;          // cluster work items
+  const uint32_t nitems = (uint32_t)((int64_t)prm.nb * prm.nctg);   // cluster work items (< 2^32, checked on the host)
   const int32_t crank = (C > 1) ? (int32_t)cluster_ctarank() : 0;
-  const int64_t cluster0 = blockIdx.x / C, nclusters = gridDim.x / C;
   constexpr uint16_t cmask = (uint16_t)((1u << C) - 1u);
   const int32_t b = prm.b;
   const int32_t ksteps = b >> 5;                 // 32-deep int8 MMAs per tile of H
@@ -312,6 +399,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
     for (int i = 0; i < NH; ++i) { mbar_init(&hfull[i], 1); mbar_init(&hempty[i], C); }   // a slot is free once all C CTAs have read it
     mbar_init(accfull, 1);
     mbar_init(accempty, 256);
+    for (int i = 0; i < K3_NQ; ++i) { mbar_init(&wq->qfull[i], 1); mbar_init(&wq->qempty[i], C * K3_QCONS); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
@@ -333,7 +421,16 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       int yb = 0, hs = 0;
       uint32_t yph = 0, hph = 0;
       const int32_t hrows = b / C;               // rows of every H plane this CTA fetches for the cluster
-      for (int64_t u = cluster0; u < nitems; u += nclusters) {
+      int qs = 0;
+      uint32_t qph = 0;
+      bool primed = false;                       // (experiment builds) the rings hold real data
+      K3Fetch fetch;
+      if (crank == 0)
+        for (int i = 0; i < K3_QAHEAD; ++i) k3_q_fetch<C>(wq, fetch, prm.counter, nitems);
+      for (;;) {
+        const uint32_t u = k3_q_pop(wq, qs, qph, true);
+        if (u == K3_NOITEM) break;
+        if (crank == 0) k3_q_fetch<C>(wq, fetch, prm.counter, nitems);
         int32_t I, ctg;
         k3_decode(prm, u, I, ctg);
         const int32_t ct = prm.ct_begin + ctg * C + crank;
@@ -342,7 +439,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         for (int32_t p = p0; p < p1; ++p) {
           const int32_t J = prm.bcol[p];
           mbar_wait(&yempty[yb], yph ^ 1);
-          const bool skip_tma = K3_EXP(2) && (u != cluster0 || p >= p0 + 2);
+          const bool skip_tma = K3_EXP(2) && (primed || p >= p0 + 2);
           mbar_expect_tx(&yfull[yb], skip_tma ? 0u : (uint32_t)Cf::YBUF);
           if (skip_tma) {}
           else if (prm.l2hints) tma_load_3d_hint(ybuf + yb * Cf::YBUF, &tmYd, 0, 0, (J * prm.nct + ct) * S, &yfull[yb], L2_EVICT_LAST);
@@ -366,6 +463,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
           yb ^= 1;
           if (yb == 0) yph ^= 1;
         }
+        primed = true;
       }
     }
   } else if (warp == 1) {
@@ -376,12 +474,17 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       // descriptors differ only in the 14-bit start-address field of the low word
       const uint64_t dbase = umma_desc_sw128(0);
       const uint32_t ylo0 = (smem_u32(ybuf) & 0x3ffffu) >> 4, hlo0 = (smem_u32(hring) & 0x3ffffu) >> 4;
-      for (int64_t u = cluster0; u < nitems; u += nclusters) {
+      int qs = 0;
+      uint32_t qph = 0;
+      int64_t it = -1;
+      for (;;) {
+        const uint32_t u = k3_q_pop(wq, qs, qph, true);
+        if (u == K3_NOITEM) break;
+        ++it;
         int32_t I, ctg;
         k3_decode(prm, u, I, ctg);
         const int32_t nJ = min(prm.brow_ptr[I + 1] - prm.brow_ptr[I], k3_jlimit<C>(prm, ctg));
         if (nJ == 0) continue;
-        const int64_t it = (u - cluster0) / nclusters;
         K3_TRACE_DECL(it < 512);
         K3_TRACE(0, clock64());
         mbar_wait(accempty, aph ^ 1);            // the epilogue has drained the previous item's accumulators
@@ -447,7 +550,13 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
     const bool use_z = (beta != 0.0);
     const bool use_s = (prm.S != nullptr);
     uint32_t aph = 0;
-    for (int64_t u = cluster0; u < nitems; u += nclusters) {
+    int qs = 0;
+    uint32_t qph = 0;
+    int64_t it = -1;
+    for (;;) {
+      const uint32_t u = k3_q_pop_warp(wq, qs, qph);
+      if (u == K3_NOITEM) break;
+      ++it;
       int32_t I, ctg;
       k3_decode(prm, u, I, ctg);
       const int32_t ct = prm.ct_begin + ctg * C + crank;
@@ -481,7 +590,6 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
       asm volatile("bar.sync 1, 256;" ::: "memory");
 
       double v[NCW];
-      const int64_t it = (u - cluster0) / nclusters;
       K3_TRACE_DECL(it < 512 && et == 0);
       K3_TRACE(3, clock64());
       if (nJ > 0) {

@@ -38,7 +38,8 @@ struct K3TCfg {
   static constexpr int RS_OFFSET = CM_OFFSET + 128 * 4;                  // HR doubles: alpha 2^(eH_i - 30)
   static constexpr int GI_OFFSET = RS_OFFSET + 64 * 8;                   // HR doubles: alpha hdiag_i + gamma
   static constexpr int TM_OFFSET = GI_OFFSET + 64 * 8;                   // tmem slot
-  static constexpr int TOTAL = TM_OFFSET + 16 + 1024;                    // + alignment slack
+  static constexpr int Q_OFFSET = TM_OFFSET + 16;                        // work-item queue (K3Queue)
+  static constexpr int TOTAL = Q_OFFSET + 192 + 1024;                    // + alignment slack
   static_assert(HR % 16 == 0 && HR <= 64, "rows per CTA: a multiple of 16 (8-row swizzle atoms, 8-row epilogue groups per half)");
   static_assert(S * HR <= 512, "digit levels must fit TMEM");
   static_assert(HBUF % 1024 == 0, "swizzle atoms");
@@ -80,12 +81,13 @@ bsr_i8t_kernel(const __grid_constant__ CUtensorMap tmH3, const __grid_constant__
   double* rs_s = reinterpret_cast<double*>(smem + Cf::RS_OFFSET);
   double* gi_s = reinterpret_cast<double*>(smem + Cf::GI_OFFSET);
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + Cf::TM_OFFSET);
+  K3Queue* wq = reinterpret_cast<K3Queue*>(smem + Cf::Q_OFFSET);          // work items of this cluster (bsr_i8.cuh)
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t nitems = (int64_t)prm.nb * prm.nctg;          // cluster work items
+  const uint32_t nitems = (uint32_t)((int64_t)prm.nb * prm.nctg);   // cluster work items (< 2^32, checked on the host)
   const int32_t crank = (int32_t)cluster_ctarank();           // which half of the block row's rows
-  const int64_t cluster0 = blockIdx.x / 2, nclusters = gridDim.x / 2;
   constexpr uint16_t cmask = 3;
+  constexpr int C = 2;
   const int32_t b = prm.b;
   const int32_t ksteps = b >> 5;                 // 32-deep int8 MMAs per tile of H
 
@@ -94,6 +96,7 @@ bsr_i8t_kernel(const __grid_constant__ CUtensorMap tmH3, const __grid_constant__
     for (int i = 0; i < NY; ++i) { mbar_init(&yfull[i], 1); mbar_init(&yempty[i], 2); }   // a slot is free once both CTAs have read it
     mbar_init(accfull, 1);
     mbar_init(accempty, 256);
+    for (int i = 0; i < K3_NQ; ++i) { mbar_init(&wq->qfull[i], 1); mbar_init(&wq->qempty[i], C * K3_QCONS); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
@@ -114,7 +117,15 @@ bsr_i8t_kernel(const __grid_constant__ CUtensorMap tmH3, const __grid_constant__
       asm volatile("prefetch.tensormap [%0];" ::"l"(&tmY4) : "memory");
       int hb = 0, ys = 0;
       uint32_t hph = 0, yph = 0;
-      for (int64_t u = cluster0; u < nitems; u += nclusters) {
+      int qs = 0;
+      uint32_t qph = 0;
+      K3Fetch fetch;
+      if (crank == 0)
+        for (int i = 0; i < K3_QAHEAD; ++i) k3_q_fetch<C>(wq, fetch, prm.counter, nitems);
+      for (;;) {
+        const uint32_t u = k3_q_pop(wq, qs, qph, true);
+        if (u == K3_NOITEM) break;
+        if (crank == 0) k3_q_fetch<C>(wq, fetch, prm.counter, nitems);
         int32_t I, ctg;
         k3_decode(prm, u, I, ctg);
         const int32_t ct = prm.ct_begin + ctg;
@@ -147,7 +158,11 @@ bsr_i8t_kernel(const __grid_constant__ CUtensorMap tmH3, const __grid_constant__
       uint32_t hph = 0, yph = 0, aph = 0;
       const uint64_t dbase = umma_desc_sw128(0);
       const uint32_t hlo0 = (smem_u32(hbuf) & 0x3ffffu) >> 4, ylo0 = (smem_u32(yring) & 0x3ffffu) >> 4;
-      for (int64_t u = cluster0; u < nitems; u += nclusters) {
+      int qs = 0;
+      uint32_t qph = 0;
+      for (;;) {
+        const uint32_t u = k3_q_pop(wq, qs, qph, true);
+        if (u == K3_NOITEM) break;
         int32_t I, ctg;
         k3_decode(prm, u, I, ctg);
         const int32_t nJ = prm.brow_ptr[I + 1] - prm.brow_ptr[I];
@@ -199,7 +214,11 @@ bsr_i8t_kernel(const __grid_constant__ CUtensorMap tmH3, const __grid_constant__
     const bool use_s = (prm.S != nullptr);
     const bool digits_out = (prm.dO != nullptr);
     uint32_t aph = 0;
-    for (int64_t u = cluster0; u < nitems; u += nclusters) {
+    int qs = 0;
+    uint32_t qph = 0;
+    for (;;) {
+      const uint32_t u = k3_q_pop_warp(wq, qs, qph);
+      if (u == K3_NOITEM) break;
       int32_t I, ctg;
       k3_decode(prm, u, I, ctg);
       const int32_t ct = prm.ct_begin + ctg;

@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(256) y_digits_kernel(const double* __restrict_
 //     (the iterates of the Chebyshev recurrence shrink or hold their size from step to step, |p_k| <= 1 on the spectrum: a drop of two
 //     or more binary orders is followed with one order of slack, the guard bit absorbs a doubling, anything beyond falls back to the
 //     path above).  Measured on configs 2 and 3 (m = 20, narrow and wide gap): no tile redone after the first step;
-//   * clears next_cmax and next_flags for the coming launch.
+//   * clears next_cmax and next_flags for the coming launch, and the work counters its clusters draw their items from.
 // cmax_prev == next_cmax (the two-slot rotation): the previous iterate's maxima are read before they are cleared, by the same thread.
 // grid (rows <= nb, tiles), 256 threads, dynamic smem S*64*33*4 bytes: CTA (x, ct) walks the block rows x, x + gridDim.x, ... of
 // column tile ct; CTAs of untouched tiles exit at once (the usual case: a small grid keeps that launch at a few microseconds).
@@ -187,7 +187,8 @@ __global__ void __launch_bounds__(256) y_digits_fix_kernel(const double* __restr
                                                            int32_t nb, const uint32_t* __restrict__ cmax, int8_t* __restrict__ D,
                                                            const uint32_t* __restrict__ flags, int32_t force, int32_t have_prev,
                                                            int32_t bias, int32_t* __restrict__ e_used, int32_t* __restrict__ e_pred,
-                                                           uint32_t* __restrict__ next_cmax, uint32_t* __restrict__ next_flags) {
+                                                           uint32_t* __restrict__ next_cmax, uint32_t* __restrict__ next_flags,
+                                                           uint32_t* __restrict__ work_counters) {
   extern __shared__ uint32_t sd[];
   const int lane = threadIdx.x & 31;
   const int64_t n0 = (int64_t)blockIdx.y * 64;
@@ -203,6 +204,7 @@ __global__ void __launch_bounds__(256) y_digits_fix_kernel(const double* __restr
       next_cmax[n] = 0;
     }
     if (threadIdx.x == 0) next_flags[blockIdx.y] = 0;
+    if (threadIdx.x == 0 && blockIdx.y == 0) { work_counters[0] = 0; work_counters[1] = 0; }   // the coming K3 launches draw their items from these
   }
   if (!redo) return;
   int32_t e[2];

@@ -703,6 +703,7 @@ struct I8Work {            // views into the caller's scratch (ttdft_step_work_b
   uint32_t* flags[2] = {nullptr, nullptr};  // per 64-column tile: a column outgrew its predicted exponent
   int32_t* e_used = nullptr;                // exponents the source iterate's digits were taken with
   int32_t* e_pred = nullptr;                // predicted exponents of the iterate the step produces
+  uint32_t* counters = nullptr;             // two work counters (main launch, remainder launch), zeroed by y_digits_fix_kernel
 };
 // digit planes per operand the handle's math mode uses: 0 (fp64 DMMA), 6 or 7
 int i8_planes_in_use(const ttdft_h_s* h) {
@@ -725,7 +726,7 @@ size_t i8_digit_bytes(const ttdft_h_s* h, int64_t w) {
 // nbuf = 2 for the filter (K3's epilogue writes the next iterate's digits while the current ones are being read), 1 for a single step
 size_t i8_work_bytes(const ttdft_h_s* h, int64_t w, int nbuf) {
   const size_t nct = i8_nct(h, w);
-  return (size_t)nbuf * i8_digit_bytes(h, w) + 4 * align_up((size_t)w * 4, 1024) + 2 * align_up(nct * 4, 1024);
+  return (size_t)nbuf * i8_digit_bytes(h, w) + 4 * align_up((size_t)w * 4, 1024) + 2 * align_up(nct * 4, 1024) + 1024;
 }
 I8Work carve_i8_work(const ttdft_h_s* h, void* base, int64_t w, int nbuf) {
   I8Work k;
@@ -742,6 +743,7 @@ I8Work carve_i8_work(const ttdft_h_s* h, void* base, int64_t w, int nbuf) {
   p += 4 * cb;
   k.flags[0] = reinterpret_cast<uint32_t*>(p);
   k.flags[1] = reinterpret_cast<uint32_t*>(p + align_up(nct * 4, 1024));
+  k.counters = reinterpret_cast<uint32_t*>(p + 2 * align_up(nct * 4, 1024));
   return k;
 }
 
@@ -803,8 +805,14 @@ ttdft_status launch_k3(ttdft_h_s* h, const CUtensorMap& tmYd, ttdft::K3Params p,
   // (one cluster's tiles per group, clusters walk consecutive block rows, evict-first on H).
   // Tiles narrower than 128 keep the former order: a 56 KB Y digit tile feeds only b/32 k-steps of MMAs, so at b = 96 the Y
   // traffic per MMA cycle is 4/3 of b = 128's and the Y-friendly order wins (config 4: 8.17 s vs 8.38 s per filter).
+  // With the work items drawn dynamically (r02) the co-resident clusters stay on a compact window of items; a group of 16 cluster
+  // columns (2,048 columns of the panel: 4-5 block rows in flight) then beats the whole panel by 2 % at config 3 -- the Y digit
+  // tiles of neighbouring block rows meet in L2 more often (same-box A/B, 55.2 vs 56.3-56.6 ms per launch).
   const bool share_h = (h->b >= 128);
-  p.cgc = share_h ? std::max(1, p.nctg) : 1;
+  p.cgc = share_h ? std::max(1, std::min(p.nctg, 2048 / (ttdft::K3_NT * C))) : 1;
+#ifdef TTDFT_EXPERIMENT
+  if (env_int("TTDFT_K3_CG", 0) > 0) p.cgc = std::max(1, env_int("TTDFT_K3_CG", 0));
+#endif
   // evict-first on H only where every H plane is used by ONE cluster (no sharing, or a single cluster column: N <= 128)
   if (p.l2hints < 0) p.l2hints = (p.cgc <= 1 || p.nctg <= 1) ? 1 : 2;
   const int64_t items = (int64_t)h->nb * p.nctg;
@@ -845,8 +853,14 @@ ttdft_status launch_k3t(ttdft_h_s* h, const CUtensorMap& tmY4, ttdft::K3Params p
   }
   p.ct_begin = 0;
   p.nctg = p.nct / 2;
-  p.cgc = 1;                       // clusters walk consecutive block rows on the same column tile and share Y digit tiles through L2
-  if (p.l2hints < 0) p.l2hints = 1;
+  // scheduling groups of up to 2,048 columns: the clusters in flight work on few block rows at a time and share their H digit planes
+  // through L2 (one cluster column per group streams all of H once per 128 columns: 134 of the 184 GB of DRAM traffic per launch
+  // at config 4); no evict-first on H then.  Same-box A/B at config 4: 48.8 -> 45.3 ms per launch.
+  p.cgc = std::max(1, std::min(p.nctg, 2048 / ttdft::K3T_NT));
+#ifdef TTDFT_EXPERIMENT
+  if (env_int("TTDFT_K3_CG", 0) > 0) p.cgc = std::max(1, env_int("TTDFT_K3_CG", 0));
+#endif
+  if (p.l2hints < 0) p.l2hints = (p.cgc <= 1) ? 1 : 2;
   const int64_t items = (int64_t)h->nb * p.nctg;
   cfg.gridDim = dim3((unsigned)(std::min<int64_t>(items, h->k3t_max_clusters) * 2));
   TimedLaunch tl(3, st);
@@ -913,7 +927,7 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
     TimedLaunch tl(have_src ? 7 : 4, st);
     ttdft::y_digits_fix_kernel<S><<<g, 256, smem, st>>>(X, ldx, h->b, h->Mt, ncols, (int32_t)h->nb, cmS, w.D[src], w.flags[src], have_src ? 0 : 1,
                                                          have_prev ? 1 : 0, h->k3_predict_bias, w.e_used, w.e_pred, w.cmax[src ^ 1],
-                                                         w.flags[src ^ 1]);
+                                                         w.flags[src ^ 1], w.counters);
     CUDA_TRY(cudaGetLastError());
     g_launches.fetch_add(1);
   }
@@ -940,6 +954,8 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
   p.l2hints = h->k3_l2hints;
   p.mrows = h->Mt;
   p.skip_empty = h->skip_empty;
+  p.counter = w.counters;
+  if ((int64_t)h->nb * nct >= 0xffffffffLL) return fail(TTDFT_ERR_UNSUPPORTED, "too many work items");
   auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
   p.vec = (al16(X) && (ldx % 2 == 0) && al16(O) && (ldo % 2 == 0) && (beta == 0.0 || (al16(Z) && ldz % 2 == 0))) ? 1 : 0;
   if (h->k3t) {
@@ -959,6 +975,7 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
   else if (C == 2) s = launch_k3<S, 2>(h, tmYd, p, 0, main_tiles, st);
   else s = launch_k3<S, 1>(h, tmYd, p, 0, main_tiles, st);
   if (s != TTDFT_OK) return s;
+  p.counter = w.counters + 1;
   if (main_tiles < (int32_t)nct) return launch_k3<S, 1>(h, tmYd, p, main_tiles, (int32_t)nct - main_tiles, st);
   return TTDFT_OK;
 }
@@ -1227,7 +1244,7 @@ ttdft_status gram_run(const GramPlan& g, const double* X, int64_t ldx, const dou
 struct RotatePlan {
   int64_t M = 0, K = 0, N = 0;
   int32_t nbm = 0, nkb = 0, nct = 0;
-  size_t dx = 0, ex = 0, dq = 0, cm = 0, idx = 0, total = 0;
+  size_t dx = 0, ex = 0, dq = 0, cm = 0, idx = 0, ctr = 1024, total = 0;     // ctr: K3's work counters
 };
 ttdft_status rotate_plan(int64_t M, int64_t K, int64_t N, RotatePlan* r) {
   if (M < 0 || K < 1 || N < 1) return fail(TTDFT_ERR_INVALID_ARG, "rotate: M >= 0, k >= 1, n >= 1 required");
@@ -1243,7 +1260,7 @@ ttdft_status rotate_plan(int64_t M, int64_t K, int64_t N, RotatePlan* r) {
   r->dq = align_up((size_t)r->nkb * r->nct * GRAM_S * 64 * 128, 1024);
   r->cm = 2 * align_up((size_t)N * 4, 1024);       // column maxima | column exponents
   r->idx = align_up(((size_t)r->nbm + 1) * 4, 1024) + align_up((size_t)r->nbm * r->nkb * 4 + 4, 1024);
-  r->total = r->dx + r->ex + r->dq + r->cm + r->idx;
+  r->total = r->dx + r->ex + r->dq + r->cm + r->idx + r->ctr;
   return TTDFT_OK;
 }
 
@@ -1261,6 +1278,8 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
   int32_t* eQ = reinterpret_cast<int32_t*>(wb + r.dx + r.ex + r.dq + r.cm / 2);      // exponents of Q's columns, from cmQ
   int32_t* brow = reinterpret_cast<int32_t*>(wb + r.dx + r.ex + r.dq + r.cm);
   int32_t* bcol = reinterpret_cast<int32_t*>(wb + r.dx + r.ex + r.dq + r.cm + align_up(((size_t)r.nbm + 1) * 4, 1024));
+  uint32_t* counters = reinterpret_cast<uint32_t*>(wb + r.dx + r.ex + r.dq + r.cm + r.idx);
+  CUDA_TRY(cudaMemsetAsync(counters, 0, 8, st));
   const int64_t Mpad = (int64_t)r.nbm * 128;
   // A operand: row exponents and digit tiles of X; tile index arrays of the dense grid
   ttdft::x_rowexp_kernel<<<(unsigned)((Mpad + 7) / 8), 256, 0, st>>>(X, ldx, r.M, Mpad, r.K, eX);
@@ -1305,8 +1324,10 @@ ttdft_status rotate_run(const RotatePlan& r, const double* X, int64_t ldx, const
     p.jlimit = jlimit;
     const int C = (n >= 2) ? 2 : 1;
     const int32_t main_tiles = n / C * C;
+    p.counter = counters;
     ttdft_status q = (C == 2) ? launch_k3<S, 2>(&hx, tmQd, p, c0, main_tiles, st) : launch_k3<S, 1>(&hx, tmQd, p, c0, main_tiles, st);
     if (q != TTDFT_OK) return q;
+    p.counter = counters + 1;
     if (main_tiles < n) return launch_k3<S, 1>(&hx, tmQd, p, c0 + main_tiles, n - main_tiles, st);
     return TTDFT_OK;
   };
@@ -1871,7 +1892,7 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     }
     const EnvSwitches env = read_env();
     // the transposed kernel K3T for tiles narrower than the MMA's M = 128 (no padding rows are multiplied there)
-    h->k3t = (env.k3_t == 0 || env.k3_t == 1) ? env.k3_t : (h->b == 96 ? 1 : 0);
+    h->k3t = (env.k3_t == 0 || env.k3_t == 1) ? env.k3_t : (h->b == 96 || h->b == 64 ? 1 : 0);   // measured: -12.5 % / -10 % per step
     if (h->b != 64 && h->b != 96 && h->b != 128) h->k3t = 0;
     if (h->k3t) {
       for (int si = 0; si < 2; ++si) {

@@ -106,7 +106,7 @@ def filter_times(workloads):
         torch.cuda.empty_cache()
 
 
-def main():
+def parse_args(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--filter", default="", help="comma-separated configs (al, largest): time one whole filter each instead of the sweep")
     ap.add_argument("--workload", default="si")
@@ -116,7 +116,13 @@ def main():
     ap.add_argument("--csr-max-n", type=int, default=4096)
     ap.add_argument("--math", default="fp64,i8x7,i8", help="arithmetic of the bsr layout: fp64 (DMMA), i8x7 / i8 (7 / 6 digit planes)")
     ap.add_argument("--out", default="")
-    args = ap.parse_args()
+    return ap.parse_args(argv)
+
+
+def main(argv=None, check=None):
+    """check(permuted: bool, op, alpha_c_beta, X, Z, O) -> relative error of O against a reference, or None: a hook for the caller
+    (bench.py --sweep passes one that runs the CPU oracle on a column sample; this module itself never touches the oracle)."""
+    args = parse_args(argv)
     if args.filter:
         return filter_times(args.filter.split(","))
     import torch
@@ -133,10 +139,15 @@ def main():
     if "bsr" in args.layouts:
         handles["bsr"] = tt.h_build_bsr(H.M, H.b, torch.from_numpy(H.row_ptr).to(dev), torch.from_numpy(H.col_idx).to(dev),
                                         torch.from_numpy(H.values).to(dev))
+    mats = {}
+    if check is not None and "bsr" in args.layouts:
+        mats[False] = synth.bsr_to_csr_nonzeros(H)
     if "csr" in args.layouts:
-        C = synth.bsr_to_csr_nonzeros(H)
+        C = mats.get(False) or synth.bsr_to_csr_nonzeros(H)
         perm = synth.permutation(H.M, cfg.seed + 50)
         Cp = synth.permute_csr(C, perm)
+        if check is not None:
+            mats[True] = Cp
         del C
         rp_d, ci_d, va_d = (torch.from_numpy(Cp.row_ptr).to(dev), torch.from_numpy(Cp.col_idx).to(dev),
                             torch.from_numpy(Cp.values).to(dev))
@@ -171,7 +182,9 @@ def main():
             print(json.dumps({"recover_subdomains_s": t1 - t0, "labelled_build_s": t2 - t1, "n_groups": n_groups,
                               "equals_planted_partition": same, "nblocks": inf["nblocks"]}), flush=True)
             assert same
-        del Cp, rp_d, ci_d, va_d
+        del rp_d, ci_d, va_d
+        if check is None:
+            del Cp
     maths = args.math.split(",")
     if "bsr" in handles and handles["bsr"].info()["i8_planes"]:
         # the same handle through the int8 digit-plane kernel (ttdft_*_ws entry points), 7 and 6 planes
@@ -202,9 +215,11 @@ def main():
                 if op == "spmm":
                     fn = lambda: tt.spmm(Hd, 1.0, X, 0.0, O, work=work)
                     alg_bytes = 8.0 * nnz + 16.0 * cfg.M * N
+                    coeffs = (1.0, 0.0, 0.0)
                 else:
                     fn = lambda: tt.cheb_step(Hd, 0.1, 10.0, -0.2, X, Z, O, work=work)
                     alg_bytes = 8.0 * nnz + 24.0 * cfg.M * N
+                    coeffs = (0.1, 10.0, -0.2)
                 reps = args.reps if (layout == "bsr" or N <= 256) else 3
                 t_med, t_min = time_launches(fn, reps, flush)
                 flops = 2.0 * nnz * N
@@ -214,6 +229,8 @@ def main():
                        "executed_tflops": 2.0 * stored[layout] * N / t_med / 1e12,
                        "binds": "hbm" if alg_bytes / bw > flops / FP64_PEAK else "fp64",
                        "roofline_frac": t_roof / t_med, "kernel": 3 if i8 else Hd.info()["kernel"]}
+                if check is not None:
+                    row["relerr"] = check(mats[layout.startswith("csr")], op, coeffs, X, Z, O)
                 rows.append(row)
                 print(json.dumps(row), flush=True)
         del X, Z, O
