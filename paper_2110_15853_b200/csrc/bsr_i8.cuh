@@ -147,12 +147,31 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
 __device__ __forceinline__ uint32_t umma_idesc_i8(uint32_t n) {
   return (2u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((128u >> 4) << 24);
 }
+// COLL: what the tensor pipe's A collector does with this instruction's A operand -- 0: read from shared memory and dropped (the
+// default), 1 (collector::a::fill): read and KEPT, 2 (collector::a::lastuse): TAKEN from the collector (same descriptor as the
+// fill just before it) and dropped.  A product wider than one instruction (N > 256) goes as a fill + lastuse pair, so its 4 KB of A
+// are read once: the MMA loop is bound by operand reads (~101 B per clock and SM sustained, measured on both K3 and K3T), and A
+// re-reads were 12 % of them.
+template <int COLL = 0>
 __device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
-  asm volatile(
-      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
-      "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n}\n" ::"r"(tmem_d),
-      "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
-      : "memory");
+  if constexpr (COLL == 1)
+    asm volatile(
+        "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::i8.collector::a::fill [%0], %1, %2, %3, p;\n}\n" ::"r"(tmem_d),
+        "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+        : "memory");
+  else if constexpr (COLL == 2)
+    asm volatile(
+        "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::i8.collector::a::lastuse [%0], %1, %2, %3, p;\n}\n" ::"r"(tmem_d),
+        "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+        : "memory");
+  else
+    asm volatile(
+        "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n}\n" ::"r"(tmem_d),
+        "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+        : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -512,8 +531,8 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
                 // ((4 KB of A + 32 N B) / 128 B per clock > N / 2 clocks for N < 128); -1.5 % cycles per tile measured
                 if (ntot > 256) {
                   const int nh = ntot / 2;            // a multiple of 32 for every S - p
-                  umma_i8(tmem_base + (uint32_t)(p * K3_NT), da, dbase | (uint64_t)(ylo + kk * 2), umma_idesc_i8(nh), acc);
-                  umma_i8(tmem_base + (uint32_t)(p * K3_NT + nh), da, dbase | (uint64_t)(ylo + nh * 8 + kk * 2), umma_idesc_i8(nh), acc);
+                  umma_i8<1>(tmem_base + (uint32_t)(p * K3_NT), da, dbase | (uint64_t)(ylo + kk * 2), umma_idesc_i8(nh), acc);
+                  umma_i8<2>(tmem_base + (uint32_t)(p * K3_NT + nh), da, dbase | (uint64_t)(ylo + nh * 8 + kk * 2), umma_idesc_i8(nh), acc);
                 } else {
                   umma_i8(tmem_base + (uint32_t)(p * K3_NT), da, dbase | (uint64_t)(ylo + kk * 2), umma_idesc_i8(ntot), acc);
                 }

@@ -185,9 +185,12 @@ bsr_i8t_kernel(const __grid_constant__ CUtensorMap tmH3, const __grid_constant__
                 const uint64_t da = dbase | (uint64_t)(ylo + kk * 2);    // A: Y plane q, 128 columns of Y x 32 k-bytes
                 // plane 0 comes first and spans every level: its first MMA of a work item overwrites the accumulators
                 const uint32_t acc = (q > 0 || kk > 0) ? 1u : (j > 0 ? 1u : 0u);
-                umma_i8(tmem_base + (uint32_t)(q * HR), da, dbase | (uint64_t)(hlo + kk * 2), umma_idesc_i8(n1), acc);
-                if (n1 < ntot)
-                  umma_i8(tmem_base + (uint32_t)(q * HR + n1), da, dbase | (uint64_t)(hlo + n1 * 8 + kk * 2), umma_idesc_i8(ntot - n1), acc);
+                if (n1 < ntot) {                    // two instructions, A read once (collector fill + lastuse)
+                  umma_i8<1>(tmem_base + (uint32_t)(q * HR), da, dbase | (uint64_t)(hlo + kk * 2), umma_idesc_i8(n1), acc);
+                  umma_i8<2>(tmem_base + (uint32_t)(q * HR + n1), da, dbase | (uint64_t)(hlo + n1 * 8 + kk * 2), umma_idesc_i8(ntot - n1), acc);
+                } else {
+                  umma_i8(tmem_base + (uint32_t)(q * HR), da, dbase | (uint64_t)(hlo + kk * 2), umma_idesc_i8(n1), acc);
+                }
               }
             }
             umma_commit_mc(&yempty[ys], cmask);     // slot free (in both CTAs) once these MMAs have read it
@@ -266,8 +269,15 @@ bsr_i8t_kernel(const __grid_constant__ CUtensorMap tmH3, const __grid_constant__
                                         ((quarter & 1) * 32 + lane) * 128 + crank * HR + rh * NR
                                   : nullptr;
       uint32_t cmx = 0;                           // column maximum (upper word) this lane has seen
+      // digit words of this lane's column are collected over CH rows (plane q, rows c0 + 4 w .. c0 + 4 w + 3) and stored as few
+      // and as wide as the alignment allows: a lane's row is 128 bytes from its neighbour's, so every store instruction costs 32
+      // sectors whatever its width
+      constexpr int CH = (NR % 16 == 0) ? 16 : NR;
+      uint32_t dwd[S][CH / 4];
 #pragma unroll
-      for (int r0 = 0; r0 < NR; r0 += 8) {
+      for (int c0 = 0; c0 < NR; c0 += CH) {
+#pragma unroll
+      for (int r0 = c0; r0 < c0 + CH; r0 += 8) {
         double y[8], z[8], ov[8];
         if (use_s) {
 #pragma unroll
@@ -295,8 +305,30 @@ bsr_i8t_kernel(const __grid_constant__ CUtensorMap tmH3, const __grid_constant__
           digits4<S>(x0, dscale, w0);
           digits4<S>(x1, dscale, w1);
 #pragma unroll
-          for (int q = 0; q < S; ++q) *reinterpret_cast<uint2*>(dtile + q * (K3_NT * 128) + r0) = make_uint2(w0[q], w1[q]);
+          for (int q = 0; q < S; ++q) { dwd[q][(r0 - c0) / 4] = w0[q]; dwd[q][(r0 - c0) / 4 + 1] = w1[q]; }
         }
+      }
+      if (digits_out) {
+        const bool lead8 = ((crank * HR + rh * NR + c0) & 8) != 0;   // warp-uniform: the piece starts 8 bytes into a 16-byte unit
+#pragma unroll
+        for (int q = 0; q < S; ++q) {
+          uint8_t* dq = dtile + q * (K3_NT * 128) + c0;
+          if (lead8) {
+            *reinterpret_cast<uint2*>(dq) = make_uint2(dwd[q][0], dwd[q][1]);
+#pragma unroll
+            for (int w = 2; w + 4 <= CH / 4; w += 4)
+              *reinterpret_cast<uint4*>(dq + 4 * w) = make_uint4(dwd[q][w], dwd[q][w + 1], dwd[q][w + 2], dwd[q][w + 3]);
+            if ((CH / 4 - 2) % 4 != 0)
+              *reinterpret_cast<uint2*>(dq + CH - 8) = make_uint2(dwd[q][CH / 4 - 2], dwd[q][CH / 4 - 1]);
+          } else {
+#pragma unroll
+            for (int w = 0; w + 4 <= CH / 4; w += 4)
+              *reinterpret_cast<uint4*>(dq + 4 * w) = make_uint4(dwd[q][w], dwd[q][w + 1], dwd[q][w + 2], dwd[q][w + 3]);
+            if ((CH / 4) % 4 != 0)
+              *reinterpret_cast<uint2*>(dq + CH - 8) = make_uint2(dwd[q][CH / 4 - 2], dwd[q][CH / 4 - 1]);
+          }
+        }
+      }
       }
       if (digits_out) {
         // the k bytes beyond the tile's rows (b < 128) stay zero: written by the warp that owns the last rows

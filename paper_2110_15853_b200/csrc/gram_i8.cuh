@@ -201,10 +201,12 @@ gram_i8_kernel(const __grid_constant__ CUtensorMap tmXd, const __grid_constant__
             for (int kk = 0; kk < 4; ++kk) {
               const uint64_t da = dbase | (uint64_t)(hlo + kk * 2);
               const uint32_t acc = (ip > 0 || kk > 0) ? 1u : (j > 0 ? 1u : 0u);
-#pragma unroll
-              for (int n0 = 0; n0 < ntot; n0 += 256) {
-                const int n = (ntot - n0) < 256 ? (ntot - n0) : 256;
-                umma_i8(tmem_base + (uint32_t)(p * K3_NT + n0), da, dbase | (uint64_t)(ylo + n0 * 8 + kk * 2), umma_idesc_i8(n), acc);
+              if (ntot > 256) {                  // two instructions, A read once (collector fill + lastuse, bsr_i8.cuh)
+                umma_i8<1>(tmem_base + (uint32_t)(p * K3_NT), da, dbase | (uint64_t)(ylo + kk * 2), umma_idesc_i8(256), acc);
+                umma_i8<2>(tmem_base + (uint32_t)(p * K3_NT + 256), da, dbase | (uint64_t)(ylo + 256 * 8 + kk * 2),
+                           umma_idesc_i8(ntot - 256), acc);
+              } else {
+                umma_i8(tmem_base + (uint32_t)(p * K3_NT), da, dbase | (uint64_t)(ylo + kk * 2), umma_idesc_i8(ntot), acc);
               }
             }
             if (C > 1) umma_commit_mc(&hempty[hs], cmask);

@@ -947,6 +947,7 @@ ttdft_status launch_step_i8_t(ttdft_h_s* h, double alpha, double gamma, double b
   if (want_next && w.D[src ^ 1]) { p.dO = w.D[src ^ 1]; p.ePredO = w.e_pred; p.flagsO = w.flags[src ^ 1]; }
 #ifdef TTDFT_DEBUG_TRACE
   p.trace = g_k3_trace;
+  if (g_k3_trace && env_int("TTDFT_TRACE_ADVANCE", 0)) g_k3_trace += 512 * 8;   // one trace block per launch
 #endif
 #ifdef TTDFT_EXPERIMENT
   p.exp = env_int("TTDFT_K3_EXP", 0);
