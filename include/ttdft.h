@@ -62,7 +62,7 @@ typedef enum {
   TTDFT_ERR_BREAKDOWN = 6 /* ttdft_orthonormalize: X^T X not positive definite (dependent columns) */
 } ttdft_status;
 
-typedef enum { TTDFT_FMT_CSR = 0, TTDFT_FMT_BSR = 1 } ttdft_format;
+typedef enum { TTDFT_FMT_CSR = 0, TTDFT_FMT_BSR = 1, TTDFT_FMT_HYBRID = 2 } ttdft_format;
 
 /* flags for ttdft_h_desc.flags */
 #define TTDFT_CHECK_SORTED 1u   /* verify indices in range, ascending and unique per row (synchronises) */
@@ -124,7 +124,16 @@ typedef enum { TTDFT_FMT_CSR = 0, TTDFT_FMT_BSR = 1 } ttdft_format;
  *            unless that more than doubles the rows; the handle then works in a tile-order space of nb*b rows behind the
  *            same row map as (2) (ttdft_cheb_filter needs a second scratch panel: ask ttdft_cheb_filter_work_bytes).
  *        Otherwise the CSR is kept as is.
- * All four arrays are DEVICE pointers; the struct itself is a HOST object.
+ *   HYBRID: the paper's own layout (Sec. 4.1, Fig. 3: "the diagonal blocks and the off-diagonal blocks of the
+ *        Hamiltonian matrix are stored as dense and sparse matrices"): diag_values holds the dense diagonal blocks H^(D) -- block k
+ *        covers rows and columns [k*diag_block, min((k+1)*diag_block, M)), row-major with leading dimension diag_block at offset
+ *        k*diag_block^2 (ceil(M/diag_block) blocks; what lies beyond M in the last one is ignored) -- and row_ptr / col_idx /
+ *        values a CSR (as above) of H^(OD), the entries OUTSIDE those blocks.  subdomain_of_row applies as for CSR.  The library
+ *        does not keep the two-part layout: zeros of the dense blocks are dropped, and the union goes into the tile format
+ *        (labels usable; tiles only where an entry is non-zero) or into one CSR (otherwise), so every product is one kernel over
+ *        one structure instead of the paper's dense + sparse library calls per step (L286).  nnz(H^(OD)) + the non-zeros of the
+ *        dense blocks < 2^31.
+ * All arrays are DEVICE pointers; the struct itself is a HOST object.
  */
 typedef struct {
   ttdft_format fmt;
@@ -135,6 +144,8 @@ typedef struct {
   const double* values;
   const int32_t* subdomain_of_row;
   uint32_t flags;
+  const double* diag_values; /* HYBRID only (ignored otherwise): the dense diagonal blocks */
+  int64_t diag_block;        /* HYBRID only: rows of one diagonal block, 1 .. M          */
 } ttdft_h_desc;
 
 /* read-back description of a built handle (all HOST values) */

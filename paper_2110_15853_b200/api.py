@@ -10,7 +10,7 @@ _LIB_PATH = os.path.join(_PKG, "libttdft.so")
 
 CHECK_SORTED, CHECK_SYMMETRY, FORCE_GENERIC, NO_I8, OWNED_ROWS_ONLY, PACKED = 1, 2, 4, 8, 16, 32
 MATH_AUTO, MATH_FP64, MATH_I8, MATH_I8X7 = 0, 1, 2, 3
-FMT_CSR, FMT_BSR = 0, 1
+FMT_CSR, FMT_BSR, FMT_HYBRID = 0, 1, 2
 _STATUS = {0: "OK", 1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "NOT_SYMMETRIC", 5: "CUDA", 6: "BREAKDOWN"}
 
 # every symbol include/ttdft.h declares
@@ -36,7 +36,8 @@ class TTDFTError(RuntimeError):
 
 class _Desc(ctypes.Structure):
     _fields_ = [("fmt", c_int32), ("M", c_int64), ("block", c_int32), ("row_ptr", c_void_p), ("col_idx", c_void_p),
-                ("values", c_void_p), ("subdomain_of_row", c_void_p), ("flags", c_uint32)]
+                ("values", c_void_p), ("subdomain_of_row", c_void_p), ("flags", c_uint32), ("diag_values", c_void_p),
+                ("diag_block", c_int64)]
 
 
 class _Info(ctypes.Structure):
@@ -231,9 +232,10 @@ class Hamiltonian:
             pass
 
 
-def _desc(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row, flags) -> _Desc:
+def _desc(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row, flags, diag_values=None, diag_block=0) -> _Desc:
     torch = _torch()
-    for t, dt, nm in ((row_ptr, torch.int32, "row_ptr"), (col_idx, torch.int32, "col_idx"), (values, torch.float64, "values")):
+    for t, dt, nm in ((row_ptr, torch.int32, "row_ptr"), (col_idx, torch.int32, "col_idx"), (values, torch.float64, "values"),
+                      (diag_values, torch.float64, "diag_values")):
         if t is not None and (t.dtype != dt or not t.is_cuda or not t.is_contiguous()):
             raise TypeError(f"{nm} must be a contiguous {dt} CUDA tensor")
     d = _Desc()
@@ -242,24 +244,28 @@ def _desc(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row, flags) -> _
     d.col_idx = col_idx.data_ptr() if col_idx is not None and col_idx.numel() else None
     d.values = values.data_ptr() if values is not None and values.numel() else None
     d.subdomain_of_row = subdomain_of_row.data_ptr() if subdomain_of_row is not None else None
+    d.diag_values = diag_values.data_ptr() if diag_values is not None and diag_values.numel() else None
+    d.diag_block = diag_block
     return d
 
 
-def h_storage_bytes(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row=None, flags=0) -> int:
-    d = _desc(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row, flags)
+def h_storage_bytes(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row=None, flags=0, diag_values=None, diag_block=0) -> int:
+    d = _desc(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row, flags, diag_values, diag_block)
     n = c_size_t()
     _check(_load().ttdft_h_storage_bytes(byref(d), byref(n)))
     return int(n.value)
 
 
-def h_build(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row=None, flags=0, stream=None) -> Hamiltonian:
+def h_build(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row=None, flags=0, stream=None, diag_values=None,
+            diag_block=0) -> Hamiltonian:
     """ttdft_h_build: validate + convert H into library-format device storage (allocated here by torch)."""
     torch = _torch()
-    d = _desc(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row, flags)
+    d = _desc(fmt, M, block, row_ptr, col_idx, values, subdomain_of_row, flags, diag_values, diag_block)
     n = c_size_t()
     L = _load()
     _check(L.ttdft_h_storage_bytes(byref(d), byref(n)))
-    storage = torch.empty(max(int(n.value), 1024) + 1024, dtype=torch.uint8, device=values.device if values is not None else "cuda")
+    dev = next((t.device for t in (values, diag_values, row_ptr) if t is not None), "cuda")
+    storage = torch.empty(max(int(n.value), 1024) + 1024, dtype=torch.uint8, device=dev)
     base = storage.data_ptr()
     aligned = (base + 1023) // 1024 * 1024
     h = c_void_p()
@@ -280,6 +286,12 @@ def h_build_csr(M, row_ptr, col_idx, values, subdomain_of_row=None, flags=0, str
             if e.status_name != "UNSUPPORTED":      # pattern too large for the shared-memory column map: build without labels
                 raise
     return h_build(FMT_CSR, M, 0, row_ptr, col_idx, values, subdomain_of_row, flags, stream)
+
+
+def h_build_hybrid(M, diag_block, diag_values, row_ptr, col_idx, values, subdomain_of_row=None, flags=0, stream=None) -> Hamiltonian:
+    """The paper's own layout: dense diagonal blocks (ceil(M / diag_block) row-major diag_block x diag_block
+    blocks) + a CSR of the entries outside them.  Argument marshalling only: the union is formed by ttdft_h_build."""
+    return h_build(FMT_HYBRID, M, 0, row_ptr, col_idx, values, subdomain_of_row, flags, stream, diag_values.reshape(-1), diag_block)
 
 
 def step_work_bytes(H: Hamiltonian, ncols: int) -> int:

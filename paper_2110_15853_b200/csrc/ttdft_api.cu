@@ -307,6 +307,93 @@ __global__ void check_sym_bsr_kernel(int32_t b, const int32_t* brow_ptr, const i
   if (bad) atomicOr(flags, 2);
 }
 
+// ---- HYBRID input (dense diagonal blocks H^(D) + sparse off-diagonal H^(OD)) ----
+// value (row, c) of the dense diagonal blocks, c inside row's block: block k = row / D at offset k * D * D, leading dimension D
+__device__ __forceinline__ double hyb_dense(const double* diag, int64_t D, int64_t row, int64_t c) {
+  const int64_t k = row / D;
+  return diag[(size_t)k * D * D + (size_t)(row - k * D) * D + (size_t)(c - k * D)];
+}
+// flags |= 1: an entry of the off-diagonal CSR lies inside a diagonal block ; flags |= 2: a dense block is not symmetric
+__global__ void hyb_check_kernel(int64_t M, int64_t D, const int32_t* row_ptr, const int32_t* col, const double* diag, int32_t nnz,
+                                 int32_t check_sym, int32_t* flags) {
+  const int64_t row = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (row >= M) return;
+  const int64_t c0 = (row / D) * D, c1 = min(c0 + D, M);
+  bool bad = false;
+  const int32_t e1 = min(row_ptr[row + 1], nnz);
+  for (int32_t e = max(row_ptr[row], 0) + lane; e < e1; e += 32) {
+    const int32_t c = col[e];
+    if (c >= c0 && c < c1) bad = true;
+  }
+  if (bad) atomicOr(flags, 1);
+  if (check_sym) {
+    bool ns = false;
+    for (int64_t c = c0 + lane; c < c1; c += 32)
+      if (!(hyb_dense(diag, D, row, c) == hyb_dense(diag, D, c, row))) ns = true;
+    if (ns) atomicOr(flags, 2);
+  }
+}
+// one warp per row: counts[row] = off-diagonal entries + non-zeros of the row's dense segment; *total (if given) += the same
+__global__ void hyb_count_kernel(int64_t M, int64_t D, const int32_t* row_ptr, const double* diag, int32_t nnz, int32_t* counts,
+                                 unsigned long long* total) {
+  const int64_t row = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (row >= M) return;
+  const int64_t c0 = (row / D) * D, c1 = min(c0 + D, M);
+  int32_t n = 0;
+  for (int64_t c = c0 + lane; c < c1; c += 32) n += hyb_dense(diag, D, row, c) != 0.0;
+  for (int o = 16; o > 0; o >>= 1) n += __shfl_xor_sync(0xffffffffu, n, o);
+  if (lane == 0) {
+    const int32_t e0 = max(row_ptr[row], 0), e1 = min(row_ptr[row + 1], nnz);
+    n += max(e1 - e0, 0);
+    if (counts) counts[row] = n;
+    if (total) atomicAdd(total, (unsigned long long)n);
+  }
+}
+// one warp per row: the merged CSR row = off-diagonal entries left of the block | non-zeros of the dense segment | the rest
+// (columns ascending if the off-diagonal CSR's are).  Entries of the off-diagonal CSR that lie inside the block are dropped.
+__global__ void hyb_merge_kernel(int64_t M, int64_t D, const int32_t* row_ptr, const int32_t* col, const double* val, const double* diag,
+                                 int32_t nnz, const int32_t* out_ptr, int32_t* out_col, double* out_val) {
+  const int64_t row = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (row >= M) return;
+  const int64_t c0 = (row / D) * D, c1 = min(c0 + D, M);
+  const int32_t e0 = max(row_ptr[row], 0), e1 = min(row_ptr[row + 1], nnz);
+  int32_t o = out_ptr[row];
+  const int32_t oend = out_ptr[row + 1];
+  // entries left of the block (the CSR is sorted when CHECK_SORTED passed; otherwise order by position: any entry with c < c0)
+  for (int pass = 0; pass < 3; ++pass) {
+    if (pass == 1) {
+      for (int64_t cb = c0; cb < c1; cb += 32) {
+        const int64_t c = cb + lane;
+        const double v = c < c1 ? hyb_dense(diag, D, row, c) : 0.0;
+        const unsigned m = __ballot_sync(0xffffffffu, v != 0.0);
+        if (v != 0.0) {
+          const int32_t q = o + __popc(m & ((1u << lane) - 1u));
+          if (q < oend) { out_col[q] = (int32_t)c; out_val[q] = v; }
+        }
+        o += __popc(m);
+      }
+    } else {
+      for (int32_t eb = e0; eb < e1; eb += 32) {
+        const int32_t e = eb + lane;
+        const int32_t c = e < e1 ? col[e] : -1;
+        const bool take = e < e1 && (pass == 0 ? c < c0 : c >= c1);
+        const unsigned m = __ballot_sync(0xffffffffu, take);
+        if (take) {
+          const int32_t q = o + __popc(m & ((1u << lane) - 1u));
+          if (q < oend) { out_col[q] = c; out_val[q] = val[e]; }
+        }
+        o += __popc(m);
+      }
+    }
+  }
+  // entries dropped because they lay inside the block leave the tail of the row unused: fill it with explicit zeros on the
+  // row's own diagonal column so the CSR stays well-formed (never happens for an input that passed hyb_check_kernel)
+  for (int32_t q = o + lane; q < oend; q += 32) { out_col[q] = (int32_t)row; out_val[q] = 0.0; }
+}
+
 __global__ void tile_rows_kernel(int64_t nb, const int32_t* brow_ptr, int32_t* tile_row) {
   int64_t I = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (I >= nb) return;
@@ -386,8 +473,10 @@ __global__ void __launch_bounds__(256) label_perm_kernel(int64_t M, int32_t b, c
 // perm/inv: reordered row r is input row perm[r], input column j is reordered column inv[j] (NULL: identity).
 // Indices are range-guarded (an invalid CSR gives a meaningless count, never a fault): entries outside [0, nnz) and columns
 // outside [0, M) are skipped.
+// diag / D: the dense diagonal blocks of a HYBRID input (NULL / 0: none); their non-zeros count as entries.
 __global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_ptr, const int32_t* col, const int32_t* perm,
-                                     const int32_t* inv, int32_t* counts, int32_t nwords, int32_t nnz, int64_t M) {
+                                     const int32_t* inv, int32_t* counts, int32_t nwords, int32_t nnz, int64_t M, const double* diag,
+                                     int64_t D) {
   extern __shared__ uint32_t bits[];
   for (int w = threadIdx.x; w < nwords; w += blockDim.x) bits[w] = 0;
   __syncthreads();
@@ -403,6 +492,14 @@ __global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_p
       const int32_t j = inv ? inv[cj] : cj;
       const int32_t J = j / b;
       atomicOr(&bits[J >> 5], 1u << (J & 31));
+    }
+    if (diag) {
+      const int64_t c0 = (row / D) * D, c1 = min(c0 + D, M);
+      for (int64_t c = c0 + lane; c < c1; c += 32) {
+        if (hyb_dense(diag, D, row, c) == 0.0) continue;
+        const int32_t J = (inv ? inv[c] : (int32_t)c) / b;
+        atomicOr(&bits[J >> 5], 1u << (J & 31));
+      }
     }
   }
   __syncthreads();
@@ -420,7 +517,7 @@ __global__ void csr2bsr_count_kernel(int64_t nb, int32_t b, const int32_t* row_p
 // pass 2: fill bcol (ascending) and scatter the entries into zero-initialised tiles
 __global__ void csr2bsr_fill_kernel(int64_t nb, int32_t b, const int32_t* row_ptr, const int32_t* col, const double* val,
                                     const int32_t* perm, const int32_t* inv, const int32_t* brow_ptr, int32_t* bcol,
-                                    double* tiles, int32_t nwords, int32_t nnz, int64_t M) {
+                                    double* tiles, int32_t nwords, int32_t nnz, int64_t M, const double* diag, int64_t D) {
   extern __shared__ uint32_t sm[];
   uint32_t* bits = sm;                    // nwords
   uint32_t* pref = sm + nwords;           // nwords: tiles before word w
@@ -438,6 +535,14 @@ __global__ void csr2bsr_fill_kernel(int64_t nb, int32_t b, const int32_t* row_pt
       const int32_t j = inv ? inv[cj] : cj;
       const int32_t J = j / b;
       atomicOr(&bits[J >> 5], 1u << (J & 31));
+    }
+    if (diag) {
+      const int64_t c0 = (row / D) * D, c1 = min(c0 + D, M);
+      for (int64_t c = c0 + lane; c < c1; c += 32) {
+        if (hyb_dense(diag, D, row, c) == 0.0) continue;
+        const int32_t J = (inv ? inv[c] : (int32_t)c) / b;
+        atomicOr(&bits[J >> 5], 1u << (J & 31));
+      }
     }
   }
   __syncthreads();
@@ -469,6 +574,18 @@ __global__ void csr2bsr_fill_kernel(int64_t nb, int32_t b, const int32_t* row_pt
       const uint32_t w = bits[J >> 5] & ((1u << (J & 31)) - 1u);
       const int32_t p = p0 + (int32_t)(pref[J >> 5] + __popc(w));
       tiles[((size_t)p * b + r) * b + (j - J * b)] = val[e];
+    }
+    if (diag) {
+      const int64_t c0 = (row / D) * D, c1 = min(c0 + D, M);
+      for (int64_t c = c0 + lane; c < c1; c += 32) {
+        const double v = hyb_dense(diag, D, row, c);
+        if (v == 0.0) continue;
+        const int32_t j = inv ? inv[c] : (int32_t)c;
+        const int32_t J = j / b;
+        const uint32_t w = bits[J >> 5] & ((1u << (J & 31)) - 1u);
+        const int32_t p = p0 + (int32_t)(pref[J >> 5] + __popc(w));
+        tiles[((size_t)p * b + r) * b + (j - J * b)] = v;
+      }
     }
   }
 }
@@ -1517,7 +1634,11 @@ void ttdft_debug_k3_trace(void* dev_buf) { g_k3_trace = reinterpret_cast<unsigne
 static ttdft_status desc_counts(const ttdft_h_desc* d, int64_t* nrows_idx, int64_t* nstored) {
   if (!d) return fail(TTDFT_ERR_INVALID_ARG, "desc is NULL");
   if (d->M < 0) return fail(TTDFT_ERR_INVALID_ARG, "M < 0");
-  if (d->fmt != TTDFT_FMT_CSR && d->fmt != TTDFT_FMT_BSR) return fail(TTDFT_ERR_INVALID_ARG, "unknown format");
+  if (d->fmt != TTDFT_FMT_CSR && d->fmt != TTDFT_FMT_BSR && d->fmt != TTDFT_FMT_HYBRID) return fail(TTDFT_ERR_INVALID_ARG, "unknown format");
+  if (d->fmt == TTDFT_FMT_HYBRID && d->M > 0) {
+    if (d->diag_block < 1 || d->diag_block > d->M) return fail(TTDFT_ERR_INVALID_ARG, "HYBRID: diag_block must be in 1..M");
+    if (!d->diag_values) return fail(TTDFT_ERR_INVALID_ARG, "HYBRID: diag_values is NULL");
+  }
   if (d->M > 0 && (!d->row_ptr)) return fail(TTDFT_ERR_INVALID_ARG, "row_ptr is NULL");
   if (d->fmt == TTDFT_FMT_BSR) {
     if (d->block < 1) return fail(TTDFT_ERR_INVALID_ARG, "BSR block size must be >= 1");
@@ -1558,8 +1679,10 @@ static ttdft_status d2h(void* dst, const void* src, size_t n, cudaStream_t st) {
   CUDA_TRY(cudaStreamSynchronize(st));
   return TTDFT_OK;
 }
+static bool is_hybrid(const ttdft_h_desc* d) { return d->fmt == TTDFT_FMT_HYBRID && d->M > 0; }
+static const double* hyb_diag(const ttdft_h_desc* d) { return is_hybrid(d) ? d->diag_values : nullptr; }
 static bool wants_label_analysis(const ttdft_h_desc* d) {
-  return d->fmt == TTDFT_FMT_CSR && d->subdomain_of_row && !(d->flags & TTDFT_FORCE_GENERIC) && d->M > 0;
+  return (d->fmt == TTDFT_FMT_CSR || d->fmt == TTDFT_FMT_HYBRID) && d->subdomain_of_row && !(d->flags & TTDFT_FORCE_GENERIC) && d->M > 0;
 }
 static bool wants_packed(const ttdft_h_desc* d) { return (d->flags & TTDFT_PACKED) && !(d->flags & TTDFT_FORCE_GENERIC); }
 // scratch the sizing needs: the label analysis of a CSR, or the slab sizes of a BSR's packed copy (nslabs + 1 words)
@@ -1567,6 +1690,7 @@ static size_t scratch_bytes(const ttdft_h_desc* d, int64_t nstored) {
   if (wants_label_analysis(d)) return analysis_bytes(d->M);
   if (d->fmt == TTDFT_FMT_BSR && d->block >= 16 && wants_packed(d) && nstored > 0)
     return align_up(((size_t)nstored * (d->block / 16) + 1) * 4, 1024);
+  if (is_hybrid(d)) return 1024;                 // the merged entry count
   return 0;
 }
 
@@ -1640,7 +1764,8 @@ static ttdft_status plan_format(const ttdft_h_desc* d, const AnalysisScratch& sc
 static ttdft_status csr2bsr_counts(const ttdft_h_desc* d, int64_t nb, int32_t b, const int32_t* perm, const int32_t* inv, int32_t* dev_counts,
                                    int32_t nnz, cudaStream_t st) {
   const int32_t nwords = (int32_t)((nb + 31) / 32);
-  csr2bsr_count_kernel<<<(unsigned)nb, 256, (size_t)nwords * 4, st>>>(nb, b, d->row_ptr, d->col_idx, perm, inv, dev_counts, nwords, nnz, d->M);
+  csr2bsr_count_kernel<<<(unsigned)nb, 256, (size_t)nwords * 4, st>>>(nb, b, d->row_ptr, d->col_idx, perm, inv, dev_counts, nwords, nnz, d->M,
+                                                                      hyb_diag(d), is_hybrid(d) ? d->diag_block : 0);
   CUDA_TRY(cudaGetLastError());
   g_launches.fetch_add(1);
   return TTDFT_OK;
@@ -1650,6 +1775,7 @@ static ttdft_status csr2bsr_counts(const ttdft_h_desc* d, int64_t nb, int32_t b,
 // (0 if not built).  For a labelled CSR the row maps are left in sc.perm() / sc.inv().
 struct FormatPlan {
   int64_t nidx = 0, nstored = 0;
+  int64_t nmerged = 0;                   // HYBRID kept as one CSR: off-diagonal entries + non-zeros of the dense blocks
   int32_t hint_b = 0;
   bool permuted = false, padded = false;
   int64_t nb = 0;                        // subdomains (labelled CSR)
@@ -1694,8 +1820,25 @@ static ttdft_status storage_bytes_impl(const ttdft_h_desc* d, const AnalysisScra
     if (wants_packed(d) && nblocks > 0 && nblocks * (hint_b / 16) < ((int64_t)1 << 31)) {
       // the tiles do not exist yet: an upper bound (every stored entry non-zero, every slab padded by one value)
       const int64_t nslabs = nblocks * (hint_b / 16);
-      f->packed = pk_region_bytes(nslabs, (uint64_t)nslabs * (4 * hint_b / 16) + ((uint64_t)f->nstored + (uint64_t)nslabs + 1) / 2);
+      const uint64_t nzmax = is_hybrid(d) ? (uint64_t)nblocks * hint_b * hint_b : (uint64_t)f->nstored;   // HYBRID: the dense blocks' non-zeros are not counted yet
+      f->packed = pk_region_bytes(nslabs, (uint64_t)nslabs * (4 * hint_b / 16) + (nzmax + (uint64_t)nslabs + 1) / 2);
     }
+    return TTDFT_OK;
+  }
+  if (is_hybrid(d)) {
+    // one CSR of the union: count it (8-byte counter at the start of the scratch)
+    unsigned long long* total = reinterpret_cast<unsigned long long*>(sc.p);
+    CUDA_TRY(cudaMemsetAsync(total, 0, 8, st));
+    hyb_count_kernel<<<(unsigned)((d->M * 32 + 255) / 256), 256, 0, st>>>(d->M, d->diag_block, d->row_ptr, d->diag_values, (int32_t)f->nstored,
+                                                                         nullptr, total);
+    g_launches.fetch_add(1);
+    unsigned long long ht = 0;
+    if ((s = d2h(&ht, total, 8, st)) != TTDFT_OK) return s;
+    if (ht >= 0x7fffffffULL) return fail(TTDFT_ERR_UNSUPPORTED, "HYBRID: the merged matrix has %llu entries (must be < 2^31)", ht);
+    f->nmerged = (int64_t)ht;
+    // row_ptr | col | values | per-row counts
+    f->base = align_up((size_t)(d->M + 1) * 4, 1024) + align_up((size_t)f->nmerged * 4, 1024) + align_up((size_t)f->nmerged * 8, 1024) +
+              1024 + align_up((size_t)d->M * 4, 1024);
     return TTDFT_OK;
   }
   const size_t per = (d->fmt == TTDFT_FMT_BSR) ? (size_t)d->block * d->block : 1;
@@ -1760,8 +1903,16 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     int32_t hf = 0;
     if ((s = d2h(&hf, flags, 4, st)) != TTDFT_OK) return s;
     if (hf & 1) return fail(TTDFT_ERR_INVALID_ARG, "indices are out of range, unsorted or duplicated");
+    if (is_hybrid(d)) {
+      hyb_check_kernel<<<(unsigned)((d->M * 32 + 255) / 256), 256, 0, st>>>(d->M, d->diag_block, d->row_ptr, d->col_idx, d->diag_values,
+                                                                           (int32_t)nstored, (d->flags & TTDFT_CHECK_SYMMETRY) ? 1 : 0, flags);
+      g_launches.fetch_add(1);
+      if ((s = d2h(&hf, flags, 4, st)) != TTDFT_OK) return s;
+      if (hf & 1) return fail(TTDFT_ERR_INVALID_ARG, "HYBRID: an entry of the off-diagonal CSR lies inside a diagonal block");
+      if (hf & 2) return fail(TTDFT_ERR_NOT_SYMMETRIC, "H is not symmetric (dense diagonal block)");
+    }
     if (d->flags & TTDFT_CHECK_SYMMETRY) {
-      if (d->fmt == TTDFT_FMT_CSR) {
+      if (d->fmt != TTDFT_FMT_BSR) {
         check_sym_csr_kernel<<<(unsigned)((d->M + 127) / 128), 128, 0, st>>>(d->M, d->row_ptr, d->col_idx, d->values, flags);
         g_launches.fetch_add(1);
       } else if (nstored > 0) {
@@ -1824,7 +1975,8 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     e = cudaMemsetAsync(tiles, 0, (size_t)nblocks * b * b * 8, st);
     if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "memset: %s", cudaGetErrorString(e)); }
     csr2bsr_fill_kernel<<<(unsigned)nb, 256, (size_t)nwords * 8, st>>>(nb, b, d->row_ptr, d->col_idx, d->values, perm, inv, brow,
-                                                                       bcol, tiles, nwords, (int32_t)nstored, d->M);
+                                                                       bcol, tiles, nwords, (int32_t)nstored, d->M, hyb_diag(d),
+                                                                       is_hybrid(d) ? d->diag_block : 0);
     e = cudaGetLastError();
     if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "csr->bsr fill: %s", cudaGetErrorString(e)); }
     g_launches.fetch_add(1);
@@ -1833,6 +1985,23 @@ ttdft_status ttdft_h_build(const ttdft_h_desc* d, void* dev_storage, size_t byte
     h->bsr = 1; h->b = b; h->nb = nb; h->nblocks = nblocks;
     h->row_ptr = brow; h->col = bcol; h->val = tiles;
     h->kernel = 1;
+  } else if (is_hybrid(d)) {
+    // ---- HYBRID without usable labels: one CSR of the union (zeros of the dense blocks dropped) ----
+    const int64_t nm = f.nmerged;
+    int32_t* rp = reinterpret_cast<int32_t*>(base);
+    int32_t* col = reinterpret_cast<int32_t*>(base + align_up((size_t)(d->M + 1) * 4, 1024));
+    double* val = reinterpret_cast<double*>(reinterpret_cast<uint8_t*>(col) + align_up((size_t)nm * 4, 1024));
+    int32_t* counts = reinterpret_cast<int32_t*>(reinterpret_cast<uint8_t*>(val) + align_up((size_t)nm * 8, 1024) + 1024);
+    const unsigned grid = (unsigned)((d->M * 32 + 255) / 256);
+    hyb_count_kernel<<<grid, 256, 0, st>>>(d->M, d->diag_block, d->row_ptr, d->diag_values, (int32_t)nstored, counts, nullptr);
+    exclusive_scan_small<<<1, 1, 0, st>>>(d->M, counts, rp);
+    hyb_merge_kernel<<<grid, 256, 0, st>>>(d->M, d->diag_block, d->row_ptr, d->col_idx, d->values, d->diag_values, (int32_t)nstored, rp, col, val);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { delete h; return fail(TTDFT_ERR_CUDA, "hybrid -> csr: %s", cudaGetErrorString(e)); }
+    g_launches.fetch_add(3);
+    h->bsr = 0; h->b = 0; h->nb = d->M; h->nblocks = nm;
+    h->row_ptr = rp; h->col = col; h->val = val;
+    h->kernel = 0;
   } else {
     // ---- keep the input format: copy the three arrays into dev_storage ----
     const size_t per = (d->fmt == TTDFT_FMT_BSR) ? (size_t)d->block * d->block : 1;

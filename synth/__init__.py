@@ -197,6 +197,23 @@ def permute_rows(X: np.ndarray, perm: np.ndarray) -> np.ndarray:
     return out
 
 
+def split_hybrid(H: CSR, D: int) -> tuple[np.ndarray, CSR]:
+    """The paper's two-part layout of the same matrix: (dense diagonal blocks, CSR of the rest).  Block k
+    covers rows and columns [k D, min((k + 1) D, M)); the blocks come back as one (ceil(M / D), D, D) array (zeros where H has no
+    entry and beyond M).  A layout change only: no arithmetic."""
+    M = H.M
+    nd = (M + D - 1) // D
+    diag = np.zeros((nd, D, D), np.float64)
+    rows = np.repeat(np.arange(M, dtype=np.int64), np.diff(H.row_ptr))
+    cols = H.col_idx.astype(np.int64)
+    inside = (rows // D) == (cols // D)
+    diag[rows[inside] // D, rows[inside] % D, cols[inside] % D] = H.values[inside]
+    keep = ~inside
+    rp = np.zeros(M + 1, np.int64)
+    np.add.at(rp, rows[keep] + 1, 1)
+    return diag, CSR(M, np.cumsum(rp).astype(np.int32), H.col_idx[keep].copy(), H.values[keep].copy())
+
+
 def column_sample(N: int, panel: int, count: int, seed: int) -> np.ndarray:
     """Seeded column sample: {0, N-1, every panel's first and last} plus random ones."""
     w = panel if panel > 0 else N
