@@ -456,7 +456,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
         const int32_t p0 = prm.brow_ptr[I];
         const int32_t p1 = p0 + min(prm.brow_ptr[I + 1] - p0, k3_jlimit<C>(prm, ctg));
         for (int32_t p = p0; p < p1; ++p) {
-          const int32_t J = prm.bcol[p];
+          const int32_t J = K3_EXP(16) ? 0 : prm.bcol[p];       // experiment builds: every Y load hits the same tiles (no DRAM traffic for Y)
           mbar_wait(&yempty[yb], yph ^ 1);
           const bool skip_tma = K3_EXP(2) && (primed || p >= p0 + 2);
           mbar_expect_tx(&yfull[yb], skip_tma ? 0u : (uint32_t)Cf::YBUF);
@@ -469,7 +469,7 @@ bsr_i8_kernel(const __grid_constant__ CUtensorMap tmHd, const __grid_constant__ 
             mbar_expect_tx(&hfull[hs], skip_tma ? 0u : (uint32_t)b * 128u);
             if (skip_tma) { if (++hs == NH) { hs = 0; hph ^= 1; } continue; }
             uint8_t* hdst = hring + hs * Cf::HSLOT + (C > 1 ? crank * hrows * 128 : 0);
-            const int32_t hrow = (p * prm.hplanes + k3_plane<S>(q)) * b + (C > 1 ? crank * hrows : 0);
+            const int32_t hrow = ((K3_EXP(32) ? 0 : p) * prm.hplanes + k3_plane<S>(q)) * b + (C > 1 ? crank * hrows : 0);   // (32: none for H)
             if (C > 1) {
               if (prm.l2hints == 1) tma_load_2d_mc_hint(hdst, &tmHd, 0, hrow, &hfull[hs], cmask, L2_EVICT_FIRST);
               else tma_load_2d_mc(hdst, &tmHd, 0, hrow, &hfull[hs], cmask);
