@@ -804,6 +804,10 @@ ttdft_status launch_step(const ttdft_h_s* h, double alpha, double gamma, double 
   TimedLaunch tl(2, st);
   if (h->bsr)
     ttdft::generic_step_kernel<true><<<grid, 32 * ttdft::K2_ROWS, 0, st>>>(p);
+  else if (ncols <= 32)
+    ttdft::generic_csr_narrow_kernel<4><<<grid.x, 32 * ttdft::K2_ROWS, 0, st>>>(p);
+  else if (ncols <= 64)
+    ttdft::generic_csr_narrow_kernel<2><<<grid.x, 32 * ttdft::K2_ROWS, 0, st>>>(p);
   else
     ttdft::generic_step_kernel<false><<<grid, 32 * ttdft::K2_ROWS, 0, st>>>(p);
   CUDA_TRY(cudaGetLastError());

@@ -195,6 +195,41 @@ def test_csr_generic_and_permuted(tt):
     assert relerr(Y.cpu().numpy(), oracle.spmm(Cp.row_ptr, Cp.col_idx, Cp.values, 1.0, Xp)) <= TOL_SPMM
 
 
+@pytest.mark.parametrize("N,ld", [(1, 1), (7, 9), (16, 16), (31, 40), (32, 32), (33, 34), (50, 64), (64, 64)])
+def test_csr_narrow_panels(tt, N, ld):
+    """Panels of <= 64 columns on a CSR run K2's narrow variants (four / two entries of a row per warp step): every width, padded leading
+    dimensions, the fused step with all three terms, rows whose length is not a multiple of 4 or 32 (z = 0.5), an empty row."""
+    import torch
+    H, C, _, _ = small_problem(3, 32, 0.5, 1007)
+    perm = synth.permutation(H.M, 9)
+    Cp = synth.permute_csr(C, perm)
+    Hp = build_csr(tt, Cp)
+    assert Hp.info()["kernel"] == 0
+    X = synth.dense_normal(H.M, N, 63)
+    Z = synth.dense_normal(H.M, N, 64)
+    Xd = torch.full((H.M, ld), float("nan"), dtype=torch.float64, device="cuda")
+    Zd = torch.full((H.M, ld), float("nan"), dtype=torch.float64, device="cuda")
+    Od = torch.full((H.M, ld), float("nan"), dtype=torch.float64, device="cuda")
+    Xd[:, :N] = dev(X)
+    Zd[:, :N] = dev(Z)
+    tt.cheb_step(Hp, 0.7, -1.3, -0.4, Xd[:, :N], Zd[:, :N], Od[:, :N])
+    ref = oracle.cheb_step(Cp.row_ptr, Cp.col_idx, Cp.values, 0.7, -1.3, -0.4, X, Z)
+    assert relerr(Od[:, :N].cpu().numpy(), ref) <= TOL_SPMM
+    assert bool(torch.isnan(Od[:, N:]).all())                     # nothing written outside the view
+    Y = dev(Z)
+    tt.spmm(Hp, 2.0, dev(X), 0.5, Y)
+    assert relerr(Y.cpu().numpy(), oracle.spmm(Cp.row_ptr, Cp.col_idx, Cp.values, 2.0, X, 0.5, Z.copy())) <= TOL_SPMM
+    # a matrix with an empty row: row 5 and column 5 removed
+    keep = (np.repeat(np.arange(Cp.M), np.diff(Cp.row_ptr)) != 5) & (Cp.col_idx != 5)
+    rp = np.zeros(Cp.M + 1, np.int64)
+    np.add.at(rp, np.repeat(np.arange(Cp.M), np.diff(Cp.row_ptr))[keep] + 1, 1)
+    E = synth.CSR(Cp.M, np.cumsum(rp).astype(np.int32), Cp.col_idx[keep].copy(), Cp.values[keep].copy())
+    He = build_csr(tt, E)
+    Y = dev(Z)
+    tt.spmm(He, 1.0, dev(X), -1.0, Y)
+    assert relerr(Y.cpu().numpy(), oracle.spmm(E.row_ptr, E.col_idx, E.values, 1.0, X, -1.0, Z.copy())) <= TOL_SPMM
+
+
 def test_csr_with_subdomain_hint_builds_tiles(tt):
     import torch
     H, C, (rp, col, val), (a0, b) = small_problem(4, 32, 0.0, 1001)
