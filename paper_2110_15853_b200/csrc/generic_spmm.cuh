@@ -109,8 +109,9 @@ __global__ void __launch_bounds__(32 * K2_ROWS) generic_csr_narrow_kernel(const 
   const int g = lane / LPG, l = lane % LPG;
   double acc[4] = {0.0, 0.0, 0.0, 0.0};
   bool ok[4];
+  const int64_t cb = (int64_t)blockIdx.y * (4 * LPG);     // first column of this CTA's column tile
 #pragma unroll
-  for (int c = 0; c < 4; ++c) ok[c] = (l + LPG * c) < p.ncols;
+  for (int c = 0; c < 4; ++c) ok[c] = (cb + l + LPG * c) < p.ncols;
   if (p.alpha != 0.0) {
     for (int32_t base = e0; base < e1; base += 32) {
       const int32_t e = base + lane;
@@ -122,7 +123,7 @@ __global__ void __launch_bounds__(32 * K2_ROWS) generic_csr_narrow_kernel(const 
         const int32_t j = __shfl_sync(0xffffffffu, jc, k + g);
         const double h = __shfl_sync(0xffffffffu, hv, k + g);
         if (k + g < n) {
-          const double* xr = p.X + (int64_t)j * p.ldx + l;
+          const double* xr = p.X + (int64_t)j * p.ldx + cb + l;
 #pragma unroll
           for (int c = 0; c < 4; ++c)
             if (ok[c]) acc[c] = fma(h, __ldg(xr + LPG * c), acc[c]);
@@ -140,7 +141,7 @@ __global__ void __launch_bounds__(32 * K2_ROWS) generic_csr_narrow_kernel(const 
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     if (!ok[c]) continue;
-    const int64_t col = l + LPG * c;
+    const int64_t col = cb + l + LPG * c;
     double v = p.alpha * acc[c];
     if (use_s) v = fma(p.gamma, p.X[row * p.ldx + col], v);
     if (use_z) v = fma(p.beta, p.Z[row * p.ldz + col], v);
