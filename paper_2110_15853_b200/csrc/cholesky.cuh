@@ -3,7 +3,7 @@
 //   G = X^T X  (ttdft_gram)  ->  G = L L^T  (potf2/panel/syrk below)  ->  R^-1 = L^-T  (level/transpose below)  ->  X_F = X R^-1  (ttdft_rotate)
 // For full-rank X the Q of Cholesky-QR is the Q of Gram-Schmidt (R is the unique upper-triangular factor with a
 // positive diagonal); the O(M n^2) work runs on the tensor cores, what is left here is O(n^3) on an n x n matrix
-// (23 GFLOP at n = 4,096) and is written for clarity, not speed: right-looking blocked Cholesky with 64-wide panels.
+// (23 GFLOP at n = 4,096) right-looking blocked Cholesky with 64-wide panels, the block products on the fp64 tensor cores.
 // Row-major, lower triangle referenced and overwritten; the strict upper triangle is never touched.
 #pragma once
 #include <cuda_runtime.h>
@@ -14,6 +14,34 @@ namespace ttdft {
 constexpr int CH_NB = 64;
 constexpr int CH_TILE_BYTES = CH_NB * (CH_NB + 1) * 8;   // one padded 64 x 64 fp64 tile in (dynamic) shared memory
 typedef double ch_tile_t[CH_NB][CH_NB + 1];
+// The three block products (panel, trailing update, inverse levels) run on the fp64 tensor cores (mma.sync m8n8k4 -> DMMA): one
+// 64 x 64 x 64 product per CTA, 8 warps x (16 rows x 32 columns), operands in shared-memory tiles of row stride 68 doubles
+// (fragment loads -- lane l reads [l / 4][l % 4] of an 8 x 4 block, or its transpose -- are then bank-conflict free).
+// Before: 4 x 4 register tiles on the fp64 ALUs, bound by their shared-memory reads (one load per two FMAs): 5.6 TFLOP/s.
+constexpr int CH_LD = CH_NB + 4;
+constexpr int CH_GEMM_SMEM = 2 * CH_NB * CH_LD * 8;      // two operand tiles
+typedef double ch_gtile_t[CH_NB][CH_LD];
+__device__ __forceinline__ void ch_dmma(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+// acc += A[wr.., 0..kmax) * B, for this warp's 16 x 32 piece at (wr, wc); BT: B(k, j) = Bs[j][k], else Bs[k][j].  kmax % 4 == 0.
+// acc[mi][ni][e]: row wr + 8 mi + lane / 4, column wc + 8 ni + 2 (lane % 4) + e.
+template <bool BT>
+__device__ __forceinline__ void ch_warp_mma(const ch_gtile_t& As, const ch_gtile_t& Bs, int kmax, int wr, int wc, int lane,
+                                            double (&acc)[2][4][2]) {
+  const int lr = lane >> 2, lc = lane & 3;
+  for (int k = 0; k < kmax; k += 4) {
+    double a[2], b[4];
+#pragma unroll
+    for (int mi = 0; mi < 2; ++mi) a[mi] = As[wr + 8 * mi + lr][k + lc];
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni) b[ni] = BT ? Bs[wc + 8 * ni + lr][k + lc] : Bs[k + lc][wc + 8 * ni + lr];
+#pragma unroll
+    for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+      for (int ni = 0; ni < 4; ++ni) ch_dmma(acc[mi][ni][0], acc[mi][ni][1], a[mi], b[ni]);
+  }
+}
 
 // Diagonal block: A[k0:k0+nbk, k0:k0+nbk] = L_kk L_kk^T, unblocked, one CTA of 256 threads.
 // flag[0] = 1 + (index of the first non-positive pivot) if the matrix is not positive definite.
@@ -72,12 +100,12 @@ __global__ void __launch_bounds__(256) ch_potf2_kernel(double* __restrict__ A, i
 }
 
 // Panel below the diagonal block: A[i, k0:k0+nbk] <- A[i, k0:k0+nbk] L_kk^-T = A[i, :] W_kk^T for rows i >= k0+nbk.
-// One CTA (256 threads, 4 x 4 register tiles) per 64 rows; dynamic smem 2 tiles.
+// One CTA (256 threads, DMMA) per 64 rows; dynamic smem CH_GEMM_SMEM.
 __global__ void __launch_bounds__(256) ch_panel_kernel(double* __restrict__ A, int64_t ld, int32_t n, int32_t k0, int32_t nbk,
                                                        const double* __restrict__ W, int64_t ldw) {
   extern __shared__ double ch_smem[];
-  ch_tile_t& As = *reinterpret_cast<ch_tile_t*>(ch_smem);
-  ch_tile_t& Ws = *reinterpret_cast<ch_tile_t*>(ch_smem + CH_NB * (CH_NB + 1));
+  ch_gtile_t& As = *reinterpret_cast<ch_gtile_t*>(ch_smem);
+  ch_gtile_t& Ws = *reinterpret_cast<ch_gtile_t*>(ch_smem + CH_NB * CH_LD);
   const int64_t i0 = (int64_t)k0 + nbk + (int64_t)blockIdx.x * 64;
   for (int e = threadIdx.x; e < CH_NB * CH_NB; e += 256) {
     const int r = e / CH_NB, c = e % CH_NB;
@@ -85,57 +113,48 @@ __global__ void __launch_bounds__(256) ch_panel_kernel(double* __restrict__ A, i
     Ws[r][c] = (r < nbk && c <= r) ? W[(int64_t)(k0 + r) * ldw + k0 + c] : 0.0;      // W_kk[r][c], lower triangular
   }
   __syncthreads();
-  const int tr = (threadIdx.x >> 4) * 4, tc = (threadIdx.x & 15) * 4;
-  double acc[4][4] = {};
-  for (int t = 0; t < nbk; ++t) {            // P[i][c] = sum_t A[i][t] W_kk[c][t]
-    double a[4], b[4];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wr = (warp >> 1) * 16, wc = (warp & 1) * 32;
+  double acc[2][4][2] = {};
+  ch_warp_mma<true>(As, Ws, CH_NB, wr, wc, lane, acc);       // P[i][c] = sum_t A[i][t] W_kk[c][t]
 #pragma unroll
-    for (int u = 0; u < 4; ++u) { a[u] = As[tr + u][t]; b[u] = Ws[tc + u][t]; }
+  for (int mi = 0; mi < 2; ++mi)
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
+    for (int ni = 0; ni < 4; ++ni)
 #pragma unroll
-      for (int w = 0; w < 4; ++w) acc[u][w] = fma(a[u], b[w], acc[u][w]);
-  }
-#pragma unroll
-  for (int u = 0; u < 4; ++u)
-#pragma unroll
-    for (int w = 0; w < 4; ++w)
-      if (i0 + tr + u < n && tc + w < nbk) A[(i0 + tr + u) * ld + k0 + tc + w] = acc[u][w];
+      for (int e = 0; e < 2; ++e) {
+        const int64_t i = i0 + wr + 8 * mi + (lane >> 2);
+        const int c = wc + 8 * ni + 2 * (lane & 3) + e;
+        if (i < n && c < nbk) A[i * ld + k0 + c] = acc[mi][ni][e];
+      }
 }
 
 // Trailing update: A[i, j] -= sum_t P[i, t] P[j, t] for k1 <= j <= i < n (lower triangle), P = A[:, k0:k0+nbk], k1 = k0+nbk.
-// grid (tiles, tiles) of 64 x 64 output tiles (upper tiles exit), 256 threads, each a 4 x 4 register tile.
+// grid (tiles, tiles) of 64 x 64 output tiles (upper tiles exit), 256 threads, DMMA (ch_warp_mma).
 __global__ void __launch_bounds__(256) ch_syrk_kernel(double* __restrict__ A, int64_t ld, int32_t n, int32_t k0, int32_t nbk) {
   if (blockIdx.y > blockIdx.x) return;                       // tile column > tile row: strictly upper
-  extern __shared__ double ch_smem[];                        // 2 tiles (dynamic: 2 * CH_TILE_BYTES)
-  ch_tile_t& Pi = *reinterpret_cast<ch_tile_t*>(ch_smem);
-  ch_tile_t& Pj = *reinterpret_cast<ch_tile_t*>(ch_smem + CH_NB * (CH_NB + 1));
+  extern __shared__ double ch_smem[];                        // 2 tiles (dynamic: CH_GEMM_SMEM)
+  ch_gtile_t& Pi = *reinterpret_cast<ch_gtile_t*>(ch_smem);
+  ch_gtile_t& Pj = *reinterpret_cast<ch_gtile_t*>(ch_smem + CH_NB * CH_LD);
   const int32_t k1 = k0 + nbk;
   const int64_t i0 = (int64_t)k1 + (int64_t)blockIdx.x * 64, j0 = (int64_t)k1 + (int64_t)blockIdx.y * 64;
-  for (int e = threadIdx.x; e < 64 * nbk; e += 256) {
-    const int r = e / nbk, t = e % nbk;
-    Pi[r][t] = (i0 + r < n) ? A[(i0 + r) * ld + k0 + t] : 0.0;
-    Pj[r][t] = (j0 + r < n) ? A[(j0 + r) * ld + k0 + t] : 0.0;
+  for (int e = threadIdx.x; e < CH_NB * CH_NB; e += 256) {
+    const int r = e / CH_NB, t = e % CH_NB;
+    Pi[r][t] = (i0 + r < n && t < nbk) ? A[(i0 + r) * ld + k0 + t] : 0.0;
+    Pj[r][t] = (j0 + r < n && t < nbk) ? A[(j0 + r) * ld + k0 + t] : 0.0;
   }
   __syncthreads();
-  const int tr = (threadIdx.x >> 4) * 4, tc = (threadIdx.x & 15) * 4;
-  double acc[4][4] = {};
-  for (int t = 0; t < nbk; ++t) {
-    double a[4], b[4];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wr = (warp >> 1) * 16, wc = (warp & 1) * 32;
+  double acc[2][4][2] = {};
+  ch_warp_mma<true>(Pi, Pj, (nbk + 3) & ~3, wr, wc, lane, acc);
 #pragma unroll
-    for (int u = 0; u < 4; ++u) { a[u] = Pi[tr + u][t]; b[u] = Pj[tc + u][t]; }
+  for (int mi = 0; mi < 2; ++mi)
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
+    for (int ni = 0; ni < 4; ++ni)
 #pragma unroll
-      for (int w = 0; w < 4; ++w) acc[u][w] = fma(a[u], b[w], acc[u][w]);
-  }
-#pragma unroll
-  for (int u = 0; u < 4; ++u)
-#pragma unroll
-    for (int w = 0; w < 4; ++w) {
-      const int64_t i = i0 + tr + u, j = j0 + tc + w;
-      if (i < n && j < n && j <= i) A[i * ld + j] -= acc[u][w];
-    }
+      for (int e = 0; e < 2; ++e) {
+        const int64_t i = i0 + wr + 8 * mi + (lane >> 2), j = j0 + wc + 8 * ni + 2 * (lane & 3) + e;
+        if (i < n && j < n && j <= i) A[i * ld + j] -= acc[mi][ni][e];
+      }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -146,22 +165,22 @@ __global__ void __launch_bounds__(256) ch_syrk_kernel(double* __restrict__ A, in
 // The dependency chain is 2 (1 + 2 + ... + nb/2) block products instead of nb^2 / 2 for a column-by-column substitution,
 // and every level keeps all SMs busy.  Triangular operands are not multiplied through their zero blocks.
 // ------------------------------------------------------------------------------------------------
-// One level of the recursion, one 64 x 64 output tile per CTA (256 threads, 4 x 4 register tiles), dynamic smem 2 tiles.
+// One level of the recursion, one 64 x 64 output tile per CTA (256 threads, DMMA), dynamic smem CH_GEMM_SMEM.
 //   mode 1:  T[bi, bj] =   sum_{t in first half, t >= bj} L[bi, t] W[t, bj]       (W11 is lower triangular)
 //   mode 2:  W[bi, bj] = - sum_{t in second half, t <= bi} W[bi, t] T[t, bj]      (W22 is lower triangular)
 // for bi in the second half of the pair, bj in the first half.  grid (sb, sb, pairs).
 __global__ void __launch_bounds__(256) ch_level_kernel(const double* __restrict__ A, int64_t lda, const double* __restrict__ B, int64_t ldb,
                                                        double* __restrict__ C, int64_t ldc, int32_t n, int32_t sb, int32_t mode) {
   extern __shared__ double ch_smem[];
-  ch_tile_t& As = *reinterpret_cast<ch_tile_t*>(ch_smem);
-  ch_tile_t& Bs = *reinterpret_cast<ch_tile_t*>(ch_smem + CH_NB * (CH_NB + 1));
+  ch_gtile_t& As = *reinterpret_cast<ch_gtile_t*>(ch_smem);
+  ch_gtile_t& Bs = *reinterpret_cast<ch_gtile_t*>(ch_smem + CH_NB * CH_LD);
   const int32_t nb = (n + CH_NB - 1) / CH_NB;
   const int32_t f0 = blockIdx.z * 2 * sb, s0 = f0 + sb, s1 = min(s0 + sb, nb);       // first half [f0, s0), second [s0, s1)
   const int32_t bi = s0 + blockIdx.y, bj = f0 + blockIdx.x;
   if (bi >= s1) return;
   const int32_t tlo = (mode == 1) ? bj : s0, thi = (mode == 1) ? s0 : bi + 1;
-  const int tid = threadIdx.x, tr = (tid >> 4) * 4, tc = (tid & 15) * 4;
-  double acc[4][4] = {};
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, wr = (warp >> 1) * 16, wc = (warp & 1) * 32;
+  double acc[2][4][2] = {};
   for (int32_t t = tlo; t < thi; ++t) {
     __syncthreads();
     for (int e = tid; e < CH_NB * CH_NB; e += 256) {
@@ -174,24 +193,18 @@ __global__ void __launch_bounds__(256) ch_level_kernel(const double* __restrict_
       Bs[r][c] = b_ok ? B[br * ldb + bc] : 0.0;
     }
     __syncthreads();
-    for (int k = 0; k < CH_NB; ++k) {
-      double a[4], b[4];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) { a[u] = As[tr + u][k]; b[u] = Bs[k][tc + u]; }
-#pragma unroll
-      for (int u = 0; u < 4; ++u)
-#pragma unroll
-        for (int w = 0; w < 4; ++w) acc[u][w] = fma(a[u], b[w], acc[u][w]);
-    }
+    ch_warp_mma<false>(As, Bs, CH_NB, wr, wc, lane, acc);
   }
   const double sgn = (mode == 2) ? -1.0 : 1.0;
 #pragma unroll
-  for (int u = 0; u < 4; ++u)
+  for (int mi = 0; mi < 2; ++mi)
 #pragma unroll
-    for (int w = 0; w < 4; ++w) {
-      const int64_t i = (int64_t)bi * CH_NB + tr + u, j = (int64_t)bj * CH_NB + tc + w;
-      if (i < n && j < n) C[i * ldc + j] = sgn * acc[u][w];
-    }
+    for (int ni = 0; ni < 4; ++ni)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int64_t i = (int64_t)bi * CH_NB + wr + 8 * mi + (lane >> 2), j = (int64_t)bj * CH_NB + wc + 8 * ni + 2 * (lane & 3) + e;
+        if (i < n && j < n) C[i * ldc + j] = sgn * acc[mi][ni][e];
+      }
 }
 
 // Rinv = W^T (upper triangular, zero below the diagonal); 32 x 32 tiles through shared memory

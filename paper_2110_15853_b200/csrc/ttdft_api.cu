@@ -1487,9 +1487,9 @@ ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Wm, double*
                           cudaStream_t st) {
   static std::atomic<uint64_t> attr_seen{0};
   if (!attr_done(attr_seen)) {
-    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
-    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_level_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
-    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
+    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ttdft::CH_GEMM_SMEM));
+    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_level_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ttdft::CH_GEMM_SMEM));
+    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ttdft::CH_GEMM_SMEM));
     CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_potf2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
     attr_mark(attr_seen);
   }
@@ -1500,8 +1500,8 @@ ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Wm, double*
     const int32_t rem = n - k0 - nbk;
     if (rem > 0) {
       const unsigned tiles = (unsigned)((rem + 63) / 64);
-      ttdft::ch_panel_kernel<<<tiles, 256, 2 * ttdft::CH_TILE_BYTES, st>>>(G, ldg, n, k0, nbk, Wm, ldr);
-      ttdft::ch_syrk_kernel<<<dim3(tiles, tiles), 256, 2 * ttdft::CH_TILE_BYTES, st>>>(G, ldg, n, k0, nbk);
+      ttdft::ch_panel_kernel<<<tiles, 256, ttdft::CH_GEMM_SMEM, st>>>(G, ldg, n, k0, nbk, Wm, ldr);
+      ttdft::ch_syrk_kernel<<<dim3(tiles, tiles), 256, ttdft::CH_GEMM_SMEM, st>>>(G, ldg, n, k0, nbk);
       g_launches.fetch_add(2);
     }
     g_launches.fetch_add(1);
@@ -1515,8 +1515,8 @@ ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Wm, double*
   for (int32_t sb = 1; sb < nb; sb *= 2) {
     const unsigned pairs = (unsigned)((nb + 2 * sb - 1) / (2 * sb));
     const dim3 grid((unsigned)sb, (unsigned)sb, pairs);
-    ttdft::ch_level_kernel<<<grid, 256, 2 * ttdft::CH_TILE_BYTES, st>>>(G, ldg, Wm, ldr, Rinv, ldr, n, sb, 1);    // T = L21 W11
-    ttdft::ch_level_kernel<<<grid, 256, 2 * ttdft::CH_TILE_BYTES, st>>>(Wm, ldr, Rinv, ldr, Wm, ldr, n, sb, 2);   // W21 = -W22 T
+    ttdft::ch_level_kernel<<<grid, 256, ttdft::CH_GEMM_SMEM, st>>>(G, ldg, Wm, ldr, Rinv, ldr, n, sb, 1);    // T = L21 W11
+    ttdft::ch_level_kernel<<<grid, 256, ttdft::CH_GEMM_SMEM, st>>>(Wm, ldr, Rinv, ldr, Wm, ldr, n, sb, 2);   // W21 = -W22 T
     g_launches.fetch_add(2);
   }
   ttdft::ch_transpose_upper_kernel<<<dim3((unsigned)((n + 31) / 32), (unsigned)((n + 31) / 32)), 256, 0, st>>>(Wm, ldr, n, Rinv, ldr);
