@@ -228,6 +228,24 @@ ttdft_status ttdft_cheb_step_ws(ttdft_h_t h, double alpha, double c, double beta
                                 void* work, size_t work_bytes, void* stream);
 
 /*
+ * ttdft_cheb_step_ws for callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): the same fused step in the handle's math mode, with the scratch taken from a
+ * static device array INSIDE the library instead of from the caller.  Arguments and overlap rules as ttdft_cheb_step_ws.
+ *   - The array holds TTDFT_STATIC_SCRATCH_BYTES (32 MiB); every GPU that loads the library keeps it until the process exits.
+ *     A step whose ttdft_step_work_bytes(h, ncols) exceeds it is rejected with TTDFT_ERR_WORKSPACE_TOO_SMALL (nothing is
+ *     launched): use ttdft_cheb_step_ws there.  32 MiB covers about M x ncols <= 4.5e6 in the int8 modes (e.g. M = 8,192 with
+ *     512 columns); TTDFT_MATH_FP64 steps on a handle that was not reordered need no scratch at all.
+ *   - The call allocates and frees no device memory: no cudaMalloc / cudaFree, no allocating library routine.  The first call
+ *     on a device looks the array's device address up (cudaGetSymbolAddress, with that device current) and keeps it.
+ *   - ALL calls on one device share the array, and it keeps the last call's contents (the step clears what it needs zeroed).
+ *     Calls that overlap on the GPU -- different streams, or graphs replayed concurrently -- RACE on it: keep such calls on one
+ *     stream, or order them with events.  Calls on one stream, and calls mixed with ttdft_*_ws on caller scratch, are safe.
+ */
+#define TTDFT_STATIC_SCRATCH_BYTES (32u << 20)
+ttdft_status ttdft_cheb_step_static(ttdft_h_t h, double alpha, double c, double beta, const double* Yk, int64_t ldk,
+                                    const double* Ykm1, int64_t ldm, double* Yout, int64_t ldo, int64_t ncols, void* stream);
+
+/*
  * A1 -- the scalars of Algorithm 1, HOST arrays of length m:
  *   e = (b-a)/2, c = (b+a)/2, sigma_1 = e/(a0-c), gamma = 2/sigma_1, sigma_{k+1} = 1/(gamma-sigma_k)
  *   alpha[0] = sigma_1/e, beta[0] = 0;   alpha[k] = 2*sigma_{k+1}/e, beta[k] = -sigma_k*sigma_{k+1}

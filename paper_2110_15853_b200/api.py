@@ -18,7 +18,7 @@ exported_symbols = [
     "ttdft_h_storage_bytes", "ttdft_h_build", "ttdft_h_info", "ttdft_h_destroy", "ttdft_spmm", "ttdft_cheb_step",
     "ttdft_cheb_scalars", "ttdft_cheb_filter_work_bytes", "ttdft_cheb_filter", "ttdft_cheb_filter_host_work_bytes",
     "ttdft_cheb_filter_host", "ttdft_probe_fp64_peak", "ttdft_launch_count", "ttdft_last_error",
-    "ttdft_h_set_math_mode", "ttdft_step_work_bytes", "ttdft_spmm_ws", "ttdft_cheb_step_ws",
+    "ttdft_h_set_math_mode", "ttdft_step_work_bytes", "ttdft_spmm_ws", "ttdft_cheb_step_ws", "ttdft_cheb_step_static",
     "ttdft_timing_enable", "ttdft_timing_read",
     "ttdft_gram_work_bytes", "ttdft_gram", "ttdft_project_work_bytes", "ttdft_project",
     "ttdft_rotate_work_bytes", "ttdft_rotate", "ttdft_orthonormalize_work_bytes", "ttdft_orthonormalize",
@@ -75,6 +75,8 @@ def _load() -> ctypes.CDLL:
     L.ttdft_cheb_step.restype = st
     L.ttdft_cheb_step.argtypes = [c_void_p, c_double, c_double, c_double, c_void_p, c_int64, c_void_p, c_int64, c_void_p,
                                   c_int64, c_int64, c_void_p]
+    L.ttdft_cheb_step_static.restype = st
+    L.ttdft_cheb_step_static.argtypes = list(L.ttdft_cheb_step.argtypes)
     L.ttdft_h_set_math_mode.restype = st
     L.ttdft_h_set_math_mode.argtypes = [c_void_p, c_int32]
     L.ttdft_step_work_bytes.restype = st
@@ -338,6 +340,22 @@ def cheb_step(H: Hamiltonian, alpha: float, c: float, beta: float, Yk, Ykm1, You
         _keep(keep, stream)
         return Yout
     _check(_load().ttdft_cheb_step(H.handle, alpha, c, beta, kp, ldk, mp, ldm, op, ldo, Yk.shape[1], _stream(stream)))
+    return Yout
+
+
+STATIC_SCRATCH_BYTES = 32 << 20
+
+
+def cheb_step_static(H: Hamiltonian, alpha: float, c: float, beta: float, Yk, Ykm1, Yout, stream=None):
+    """ttdft_cheb_step_static: the fused step in the handle's math mode with the library's own static device scratch (no device
+    allocation by the library or by this binding; steps that need more than STATIC_SCRATCH_BYTES are rejected; calls that
+    overlap on the GPU race on the shared scratch).  Argument marshalling only."""
+    kp, ldk = _mat(Yk, "Yk")
+    op, ldo = _mat(Yout, "Yout")
+    mp, ldm = (None, 0) if Ykm1 is None else _mat(Ykm1, "Ykm1")
+    if Yk.shape != Yout.shape or Yk.shape[0] != H.M or (Ykm1 is not None and Ykm1.shape != Yk.shape):
+        raise ValueError("shape mismatch")
+    _check(_load().ttdft_cheb_step_static(H.handle, alpha, c, beta, kp, ldk, mp, ldm, op, ldo, Yk.shape[1], _stream(stream)))
     return Yout
 
 

@@ -2246,6 +2246,45 @@ ttdft_status ttdft_cheb_step_ws(ttdft_h_t h, double alpha, double c, double beta
   return step_ws(h, alpha, -alpha * c, be, Yk, ldk, Ykm1, ldm, Yout, ldo, ncols, work, work_bytes, (cudaStream_t)stream);
 }
 
+// ---- the step without caller scratch: a static device array inside the library (include/ttdft.h, ttdft_cheb_step_static) ----
+// Its name is a HOST-side stand-in in host code, not a device address: the address comes from cudaGetSymbolAddress, looked up once
+// per device with that device current.  Every call on a device shares the array (calls that overlap on the GPU race).
+static __device__ __align__(256) unsigned char g_static_scratch[TTDFT_STATIC_SCRATCH_BYTES];
+
+static ttdft_status static_scratch_ptr(void** out) {
+  constexpr int MAXDEV = 64;
+  static std::mutex mu;
+  static void* ptrs[MAXDEV] = {};
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= MAXDEV) return fail(TTDFT_ERR_UNSUPPORTED, "static scratch: device ordinal %d outside 0..%d", dev, MAXDEV - 1);
+  std::lock_guard<std::mutex> lk(mu);
+  if (!ptrs[dev]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess || !p) return fail(TTDFT_ERR_CUDA, "static scratch: cudaGetSymbolAddress on device %d: %s", dev, cudaGetErrorString(e));
+    ptrs[dev] = p;
+  }
+  *out = ptrs[dev];
+  return TTDFT_OK;
+}
+
+ttdft_status ttdft_cheb_step_static(ttdft_h_t h, double alpha, double c, double beta, const double* Yk, int64_t ldk,
+                                    const double* Ykm1, int64_t ldm, double* Yout, int64_t ldo, int64_t ncols, void* stream) {
+  if (!h) return fail(TTDFT_ERR_INVALID_ARG, "handle is NULL");
+  if (ncols < 1) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1");
+  size_t pb;
+  const size_t need = step_work_need(h, ncols, &pb);
+  if (need > (size_t)TTDFT_STATIC_SCRATCH_BYTES)
+    return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL,
+                "this step needs %zu bytes of scratch, the library's static scratch holds %zu: use ttdft_cheb_step_ws with caller scratch",
+                need, (size_t)TTDFT_STATIC_SCRATCH_BYTES);
+  void* work = nullptr;
+  ttdft_status s = static_scratch_ptr(&work);
+  if (s != TTDFT_OK) return s;
+  return ttdft_cheb_step_ws(h, alpha, c, beta, Yk, ldk, Ykm1, ldm, Yout, ldo, ncols, work, (size_t)TTDFT_STATIC_SCRATCH_BYTES, stream);
+}
+
 ttdft_status ttdft_cheb_scalars(int32_t m, double a, double b, double a0, double* c_out, double* alpha, double* beta) {
   ttdft_status s = check_scalars(m, a, b, a0);
   if (s != TTDFT_OK) return s;
