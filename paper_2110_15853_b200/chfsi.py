@@ -27,8 +27,7 @@ def chfsi_iteration(H: "api.Hamiltonian", X, m: int, a: float, b: float, a0: flo
     del Xf
     HF = torch.empty((n, n), dtype=torch.float64, device=X.device)
     api.project(H, Xo, HF)                                                 # step 3
-    HF = 0.5 * (HF + HF.T)
-    lam, Q = torch.linalg.eigh(HF)                                         # step 4 (library)
+    lam, Q = torch.linalg.eigh(HF)                                         # step 4 (library; reads the lower triangle of H_F only)
     Psi = torch.empty_like(X)
     api.rotate(Xo, Q.contiguous(), Psi)                                    # step 5
     return Psi, lam
