@@ -277,6 +277,11 @@ ttdft_status ttdft_cheb_filter(ttdft_h_t h, const double* X, int64_t ldx, double
  * host->device, filtered, and copied device->host, the copies of neighbouring panels overlapping
  * the arithmetic.  `work` is DEVICE scratch of at least ttdft_cheb_filter_host_work_bytes.  The call
  * returns after the last panel has reached Y (it synchronises).
+ * panel_cols > 0: every panel has that width (the last one what is left).  panel_cols == 0: a ramp of panel widths, 256, 768, then
+ * up to 2,048 columns, mirrored at the end (4,096 columns: 256 | 768 | 2,048 | 768 | 256) -- the copy of the first panel in and of
+ * the last panel out are the only transfers no arithmetic can hide, so those panels are narrow, and each panel's arithmetic
+ * covers the copy of the wider next one.  The scratch is sized for the widest panel (ask ttdft_cheb_filter_host_work_bytes with
+ * the same panel_cols).  The result of every column is independent of the panel schedule (bit for bit).
  */
 ttdft_status ttdft_cheb_filter_host_work_bytes(ttdft_h_t h, int64_t ncols, int64_t panel_cols, size_t* bytes);
 ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* X_host, int64_t ldx, double* Y_host, int64_t ldy,

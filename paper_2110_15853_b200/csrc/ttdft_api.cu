@@ -2356,10 +2356,36 @@ ttdft_status ttdft_cheb_filter(ttdft_h_t h, const double* X, int64_t ldx, double
   return TTDFT_OK;
 }
 
+// Panel widths of the host-buffer filter.  panel_cols > 0: uniform.  0: a ramp -- 256, 768, then up to HOST_WMAX = 2,048 columns, and
+// the mirror image at the end (4,096 columns: 256 | 768 | 2,048 | 768 | 256).  The copy of the first panel in and of the last panel
+// out are the only transfers no arithmetic overlaps, so those panels are narrow; each panel's arithmetic then covers the copy of
+// the (three times wider) next one, and wide panels in the middle keep the step kernel at its whole-panel rate.
+constexpr int64_t HOST_WMAX = 2048;
+static std::vector<int64_t> host_panel_widths(int64_t ncols, int64_t panel_cols) {
+  std::vector<int64_t> head, tail;
+  if (panel_cols > 0) {
+    for (int64_t c0 = 0; c0 < ncols; c0 += panel_cols) head.push_back(std::min(panel_cols, ncols - c0));
+    return head;
+  }
+  const int64_t lead = std::min<int64_t>(256, (ncols / 4) / 64 * 64);
+  if (lead < 64) { head.push_back(ncols); return head; }       // too narrow to cut (ncols < 256)
+  int64_t left = ncols, wh = lead, wt = lead;
+  for (bool from_head = true; left > 0; from_head = !from_head) {
+    int64_t& wn = from_head ? wh : wt;
+    int64_t c = std::min(wn, left);
+    if (left - c < lead && left <= HOST_WMAX) c = left;           // no sliver at the end of the middle
+    (from_head ? head : tail).push_back(c);
+    left -= c;
+    wn = std::min(HOST_WMAX, 3 * wn);
+  }
+  head.insert(head.end(), tail.rbegin(), tail.rend());
+  return head;
+}
+
 ttdft_status ttdft_cheb_filter_host_work_bytes(ttdft_h_t h, int64_t ncols, int64_t panel_cols, size_t* bytes) {
   if (!h || !bytes) return fail(TTDFT_ERR_INVALID_ARG, "NULL argument");
   if (ncols < 1 || panel_cols < 0) return fail(TTDFT_ERR_INVALID_ARG, "ncols must be >= 1 and panel_cols >= 0");
-  int64_t w = panel_cols ? std::min(panel_cols, ncols) : std::min<int64_t>(ncols, 1024);
+  int64_t w = panel_cols ? std::min(panel_cols, ncols) : std::min<int64_t>(ncols, HOST_WMAX);
   w += (w & 1);
   *bytes = 4 * align_up((size_t)h->M * (size_t)w * 8, 1024) +                  // 2 x (X panel, Y panel)
            filter_panels(h) * align_up((size_t)h->Mt * (size_t)w * 8, 1024);   // + scratch panel(s) in tile order
@@ -2383,7 +2409,7 @@ ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* Xh, int64_t ldx, 
   std::vector<double> alpha((size_t)std::max(m, 1)), beta((size_t)std::max(m, 1));
   double c;
   if ((s = ttdft_cheb_scalars(m, a, b, a0, &c, alpha.data(), beta.data())) != TTDFT_OK) return s;
-  const int64_t w = panel_cols ? std::min(panel_cols, ncols) : std::min<int64_t>(ncols, 1024);
+  const int64_t w = panel_cols ? std::min(panel_cols, ncols) : std::min<int64_t>(ncols, HOST_WMAX);
   const int64_t ldw = w + (w & 1);
   const size_t pbytes = align_up((size_t)h->M * (size_t)ldw * 8, 1024);
   const size_t tbytes = align_up((size_t)h->Mt * (size_t)ldw * 8, 1024);
@@ -2431,10 +2457,11 @@ ttdft_status ttdft_cheb_filter_host(ttdft_h_t h, const double* Xh, int64_t ldx, 
   HOST_TRY(cudaEventRecord(ev_start, sc));
   HOST_TRY(cudaStreamWaitEvent(sin, ev_start, 0));
   HOST_TRY(cudaStreamWaitEvent(sout, ev_start, 0));
-  int64_t ip = 0;
-  for (int64_t c0 = 0; c0 < ncols; c0 += w, ++ip) {
+  const std::vector<int64_t> widths = host_panel_widths(ncols, panel_cols);    // every entry <= w
+  int64_t c0 = 0;
+  for (size_t ip = 0; ip < widths.size(); c0 += widths[ip], ++ip) {
     const int buf = (int)(ip & 1);
-    const int64_t wc = std::min(w, ncols - c0);
+    const int64_t wc = widths[ip];
     // host -> device on the input stream once the compute that last read dX[buf] is done
     if (ip >= 2) HOST_TRY(cudaStreamWaitEvent(sin, ev_comp[buf], 0));
     HOST_TRY(cudaMemcpy2DAsync(dX[buf], (size_t)ldw * 8, Xh + c0, (size_t)ldx * 8, (size_t)wc * 8, (size_t)h->M,

@@ -150,6 +150,28 @@ def test_filter_host_buffers(tt):
     assert relerr(Yh.numpy(), ref) <= TOL_FILTER
 
 
+@pytest.mark.parametrize("G,b,N,mode", [(4, 32, 700, "FP64"), (3, 64, 2500, "I8X7"), (3, 64, 200, "I8X7")])
+def test_filter_host_default_panel_schedule(tt, G, b, N, mode):
+    """panel_cols = 0 on host buffers: a ramp of panel widths, narrow first and last (N = 700: 128 | 444 | 128,
+    N = 2,500: 256 | 768 | 452 | 768 | 256, N = 200: one panel).  Every column equals the device-resident filter's bit for bit (the
+    result of a column does not depend on the panels), and sampled columns the oracle's."""
+    import torch
+    H, C, _, (a0, bb) = small_problem(G, b, 0.3, 1300 + b)
+    a, bb, a0 = bounds_for(a0, bb, 64, H.M)
+    Hd = build_bsr(tt, H)
+    Hd.set_math_mode(getattr(tt, "MATH_" + mode))
+    X = synth.dense_normal(H.M, N, 43)
+    Xh = torch.from_numpy(X).pin_memory()
+    Yh = torch.full((H.M, N), float("nan"), dtype=torch.float64).pin_memory()
+    tt.cheb_filter_host(Hd, Xh, Yh, 9, a, bb, a0, panel_cols=0)
+    Yd = torch.empty(H.M, N, dtype=torch.float64, device="cuda")
+    tt.cheb_filter(Hd, dev(X), Yd, 9, a, bb, a0)
+    assert torch.equal(Yh, Yd.cpu())
+    cols = sorted({0, 63, 64, 127, 128, 255, 256, N // 2, N - 129, N - 128, N - 1} & set(range(N)))
+    ref = oracle.cheb_filter(C.row_ptr, C.col_idx, C.values, np.ascontiguousarray(X[:, cols]), 9, a, bb, a0)
+    assert worst_col_relerr(Yh.numpy()[:, cols], ref) <= TOL_FILTER
+
+
 # ---------------------------------------------------------------- other tile sizes (several tiles + ragged tail)
 @pytest.mark.parametrize("G,b,z,N", [(3, 64, 0.3, 200), (2, 96, 0.4, 130), (3, 128, 0.4, 300)])
 def test_filter_other_block_sizes(tt, G, b, z, N):
