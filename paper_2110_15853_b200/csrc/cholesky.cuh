@@ -46,57 +46,106 @@ __device__ __forceinline__ void ch_warp_mma(const ch_gtile_t& As, const ch_gtile
 // Diagonal block: A[k0:k0+nbk, k0:k0+nbk] = L_kk L_kk^T, unblocked, one CTA of 256 threads.
 // flag[0] = 1 + (index of the first non-positive pivot) if the matrix is not positive definite.
 // Also W[k0.., k0..] = L_kk^-1 (lower triangular), which turns the panel solve into a product and seeds the inverse.
+// The block lives in REGISTERS: thread (ty, tx) of 16 x 16 holds rows ty + 16 u, columns tx + 16 w (u, w < 4) of A and of the
+// right-hand side B of L W = I (B = I at the start).  Step j takes the pivot, column j of A and row j of B from a small
+// double-buffered shared-memory exchange, scales them by 1 / sqrt(pivot) and applies both rank-1 updates (A -= l l^T,
+// B -= l w_j) in registers; the owners of column j + 1 / row j + 1 then publish them: ONE barrier and ~45 instructions per
+// column (before: two barriers, a division loop and a shared-memory update of the trailing block per column, then a serial
+// forward substitution: 72 -> 12 us per block, and the chain of 64 blocks is serial).
 __global__ void __launch_bounds__(256) ch_potf2_kernel(double* __restrict__ A, int64_t ld, int32_t k0, int32_t nbk, int32_t* __restrict__ flag,
                                                        double* __restrict__ W, int64_t ldw) {
-  extern __shared__ double ch_smem[];                        // 2 tiles (dynamic: 2 * CH_TILE_BYTES): L_kk and its inverse
-  ch_tile_t& s = *reinterpret_cast<ch_tile_t*>(ch_smem);
-  ch_tile_t& w = *reinterpret_cast<ch_tile_t*>(ch_smem + CH_NB * (CH_NB + 1));
-  const int tid = threadIdx.x;
-  const int tx = tid & 15, ty = tid >> 4;                    // 16 x 16 threads over the tile (no integer divisions in the loops)
-  __shared__ double dg[CH_NB];                               // the diagonal of L_kk
-  for (int r = ty; r < nbk; r += 16)
-    for (int c = tx; c < nbk; c += 16) s[r][c] = (c <= r) ? A[(int64_t)(k0 + r) * ld + k0 + c] : 0.0;
-  __syncthreads();
-  for (int j = 0; j < nbk; ++j) {
-    // column j: every thread takes the pivot from s[j][j] (not written in this phase), one of them records it
-    const double d = s[j][j];
-    const bool ok = d > 0.0;
-    const double ljj = ok ? sqrt(d) : 1.0;
-    if (tid == 0) {
-      dg[j] = ljj;
-      if (!ok && flag[0] == 0) flag[0] = 1 + k0 + j;
+  __shared__ double colraw[2][CH_NB], brow[2][CH_NB], piv[2];
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  double a[4][4], bb[4][4];
+#pragma unroll
+  for (int u = 0; u < 4; ++u)
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const int row = ty + 16 * u, col = tx + 16 * w;
+      // only the lower triangle is ever read; rows / columns beyond nbk behave as an identity block
+      a[u][w] = (row < nbk && col <= row) ? A[(int64_t)(k0 + row) * ld + k0 + col] : (row == col ? 1.0 : 0.0);
+      bb[u][w] = (row == col) ? 1.0 : 0.0;
     }
-    for (int r = j + 1 + tid; r < nbk; r += 256) s[r][j] /= ljj;
-    __syncthreads();
-    // trailing update of the lower triangle: s[r][c] -= s[r][j] * s[c][j], j < c <= r
-    for (int r = j + 1 + ty; r < nbk; r += 16) {
-      const double lrj = s[r][j];
-      for (int c = j + 1 + tx; c <= r; c += 16) s[r][c] -= lrj * s[c][j];
-    }
-    __syncthreads();
+  if (tx == 0) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) colraw[0][ty + 16 * u] = a[u][0];
   }
-  if (tid < nbk) s[tid][tid] = dg[tid];
+  if (ty == 0) {
+#pragma unroll
+    for (int w = 0; w < 4; ++w) brow[0][tx + 16 * w] = bb[0][w];
+  }
+  if (tid == 0) piv[0] = a[0][0];
   __syncthreads();
-  for (int r = ty; r < nbk; r += 16)
-    for (int c = tx; c <= r && c < nbk; c += 16) A[(int64_t)(k0 + r) * ld + k0 + c] = s[r][c];
-  // W_kk = L_kk^-1: forward substitution on the identity, four threads per column (partial sums over t = q mod 4, combined by
-  // two shuffles; the four threads of a column sit in one warp, so a warp barrier orders the row just written), then stored
-  {
-    const int c = tid >> 2, q = tid & 3;                     // 256 threads = 64 columns x 4
-    for (int r = 0; r < nbk; ++r) {
-      const bool on = (c < nbk && r >= c);
-      double v = 0.0;
-      if (on)
-        for (int t = c + q; t < r; t += 4) v -= s[r][t] * w[t][c];
-      v += __shfl_xor_sync(0xffffffffu, v, 1);               // all lanes take part, whatever their column
-      v += __shfl_xor_sync(0xffffffffu, v, 2);
-      if (on && q == 0) w[r][c] = (v + ((r == c) ? 1.0 : 0.0)) / s[r][r];
-      __syncwarp();
+#pragma unroll
+  for (int jb = 0; jb < 4; ++jb) {
+#pragma unroll 1
+    for (int j16 = 0; j16 < 16; ++j16) {
+      const int j = jb * 16 + j16, p = j & 1, q = p ^ 1;
+      double d = piv[p];
+      if (!(d > 0.0)) {                                      // not positive definite (or NaN): record, go on with a harmless pivot
+        if (tid == 0 && j < nbk && flag[0] == 0) flag[0] = 1 + k0 + j;
+        d = 1.0;
+      }
+      const double r = rsqrt(d);
+      double ljj = d * r;
+      ljj = fma(fma(-ljj, ljj, d), 0.5 * r, ljj);            // one Newton step: sqrt(d) to the last bit or two
+      double lr[4], lc[4], wr[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) lr[u] = colraw[p][ty + 16 * u] * r;          // l_rj of this thread's rows
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        lc[w] = colraw[p][tx + 16 * w] * r;                                    // l_cj of this thread's columns
+        wr[w] = brow[p][tx + 16 * w] * r;                                      // row j of W = row j of B / l_jj
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+          a[u][w] = fma(-lr[u], lc[w], a[u][w]);             // rows / columns <= j are finished and never read again
+          bb[u][w] = fma(-lr[u], wr[w], bb[u][w]);
+        }
+      if (j < nbk) {
+        if (tx == j16) {                                     // column j of L
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int row = ty + 16 * u;
+            if (row < nbk && row >= j) A[(int64_t)(k0 + row) * ld + k0 + j] = (row == j) ? ljj : lr[u];
+          }
+        }
+        if (ty == j16) {                                     // row j of W (zero right of the diagonal: not stored)
+#pragma unroll
+          for (int w = 0; w < 4; ++w) {
+            const int col = tx + 16 * w;
+            if (col <= j) W[(int64_t)(k0 + j) * ldw + k0 + col] = wr[w];
+          }
+        }
+      }
+      // publish column j + 1 of A, row j + 1 of B and the next pivot
+      if (j16 < 15) {
+        if (tx == j16 + 1) {
+#pragma unroll
+          for (int u = 0; u < 4; ++u) colraw[q][ty + 16 * u] = a[u][jb];
+        }
+        if (ty == j16 + 1) {
+#pragma unroll
+          for (int w = 0; w < 4; ++w) brow[q][tx + 16 * w] = bb[jb][w];
+          if (tx == j16 + 1) piv[q] = a[jb][jb];
+        }
+      } else if (jb < 3) {
+        const int jn = jb < 3 ? jb + 1 : 3;
+        if (tx == 0) {
+#pragma unroll
+          for (int u = 0; u < 4; ++u) colraw[q][ty + 16 * u] = a[u][jn];
+        }
+        if (ty == 0) {
+#pragma unroll
+          for (int w = 0; w < 4; ++w) brow[q][tx + 16 * w] = bb[jn][w];
+          if (tx == 0) piv[q] = a[jn][jn];
+        }
+      }
+      __syncthreads();
     }
   }
-  __syncthreads();
-  for (int r = ty; r < nbk; r += 16)
-    for (int c = tx; c <= r && c < nbk; c += 16) W[(int64_t)(k0 + r) * ldw + k0 + c] = w[r][c];
 }
 
 // Panel below the diagonal block: A[i, k0:k0+nbk] <- A[i, k0:k0+nbk] L_kk^-T = A[i, :] W_kk^T for rows i >= k0+nbk.
@@ -137,13 +186,25 @@ __global__ void __launch_bounds__(256) ch_syrk_kernel(double* __restrict__ A, in
   ch_gtile_t& Pj = *reinterpret_cast<ch_gtile_t*>(ch_smem + CH_NB * CH_LD);
   const int32_t k1 = k0 + nbk;
   const int64_t i0 = (int64_t)k1 + (int64_t)blockIdx.x * 64, j0 = (int64_t)k1 + (int64_t)blockIdx.y * 64;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wr = (warp >> 1) * 16, wc = (warp & 1) * 32;
+  // the output tile is read FIRST, so that its latency runs under the panel loads and the product (the kernel is bound by
+  // memory latency: a tile is 0.5 MFLOP; with the read-modify-write at the end three quarters of the stalls sat on these loads)
+  double cv[2][4][2];
+#pragma unroll
+  for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int64_t i = i0 + wr + 8 * mi + (lane >> 2), j = j0 + wc + 8 * ni + 2 * (lane & 3) + e;
+        cv[mi][ni][e] = (i < n && j < n && j <= i) ? A[i * ld + j] : 0.0;
+      }
   for (int e = threadIdx.x; e < CH_NB * CH_NB; e += 256) {
     const int r = e / CH_NB, t = e % CH_NB;
     Pi[r][t] = (i0 + r < n && t < nbk) ? A[(i0 + r) * ld + k0 + t] : 0.0;
     Pj[r][t] = (j0 + r < n && t < nbk) ? A[(j0 + r) * ld + k0 + t] : 0.0;
   }
   __syncthreads();
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wr = (warp >> 1) * 16, wc = (warp & 1) * 32;
   double acc[2][4][2] = {};
   ch_warp_mma<true>(Pi, Pj, (nbk + 3) & ~3, wr, wc, lane, acc);
 #pragma unroll
@@ -153,7 +214,7 @@ __global__ void __launch_bounds__(256) ch_syrk_kernel(double* __restrict__ A, in
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         const int64_t i = i0 + wr + 8 * mi + (lane >> 2), j = j0 + wc + 8 * ni + 2 * (lane & 3) + e;
-        if (i < n && j < n && j <= i) A[i * ld + j] -= acc[mi][ni][e];
+        if (i < n && j < n && j <= i) A[i * ld + j] = cv[mi][ni][e] - acc[mi][ni][e];
       }
 }
 
@@ -181,18 +242,30 @@ __global__ void __launch_bounds__(256) ch_level_kernel(const double* __restrict_
   const int32_t tlo = (mode == 1) ? bj : s0, thi = (mode == 1) ? s0 : bi + 1;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, wr = (warp >> 1) * 16, wc = (warp & 1) * 32;
   double acc[2][4][2] = {};
-  for (int32_t t = tlo; t < thi; ++t) {
-    __syncthreads();
-    for (int e = tid; e < CH_NB * CH_NB; e += 256) {
-      const int r = e / CH_NB, c = e % CH_NB;
+  double ra[16], rb[16];                                     // this thread's 16 + 16 elements of the next pair of operand tiles
+  auto fetch = [&](int32_t t) {
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+      const int e = tid + 256 * q, r = e / CH_NB, c = e % CH_NB;
       const int64_t ar = (int64_t)bi * CH_NB + r, ac = (int64_t)t * CH_NB + c, br = (int64_t)t * CH_NB + r, bc = (int64_t)bj * CH_NB + c;
       // triangular operands: only the lower part of a diagonal block is defined
       const bool a_ok = ar < n && ac < n && !(mode == 2 && t == bi && c > r);
       const bool b_ok = br < n && bc < n && !(mode == 1 && t == bj && c > r);
-      As[r][c] = a_ok ? A[ar * lda + ac] : 0.0;
-      Bs[r][c] = b_ok ? B[br * ldb + bc] : 0.0;
+      ra[q] = a_ok ? A[ar * lda + ac] : 0.0;
+      rb[q] = b_ok ? B[br * ldb + bc] : 0.0;
+    }
+  };
+  if (tlo < thi) fetch(tlo);
+  for (int32_t t = tlo; t < thi; ++t) {
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+      const int e = tid + 256 * q, r = e / CH_NB, c = e % CH_NB;
+      As[r][c] = ra[q];
+      Bs[r][c] = rb[q];
     }
     __syncthreads();
+    if (t + 1 < thi) fetch(t + 1);                           // in flight while the tensor cores work on tile t
     ch_warp_mma<false>(As, Bs, CH_NB, wr, wc, lane, acc);
   }
   const double sgn = (mode == 2) ? -1.0 : 1.0;

@@ -1490,13 +1490,12 @@ ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Wm, double*
     CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_syrk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ttdft::CH_GEMM_SMEM));
     CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_level_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ttdft::CH_GEMM_SMEM));
     CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ttdft::CH_GEMM_SMEM));
-    CUDA_TRY(cudaFuncSetAttribute(ttdft::ch_potf2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * ttdft::CH_TILE_BYTES));
     attr_mark(attr_seen);
   }
   CUDA_TRY(cudaMemsetAsync(dflag, 0, 4, st));
   for (int32_t k0 = 0; k0 < n; k0 += ttdft::CH_NB) {
     const int32_t nbk = std::min(ttdft::CH_NB, n - k0);
-    ttdft::ch_potf2_kernel<<<1, 256, 2 * ttdft::CH_TILE_BYTES, st>>>(G, ldg, k0, nbk, dflag, Wm, ldr);
+    ttdft::ch_potf2_kernel<<<1, 256, 0, st>>>(G, ldg, k0, nbk, dflag, Wm, ldr);
     const int32_t rem = n - k0 - nbk;
     if (rem > 0) {
       const unsigned tiles = (unsigned)((rem + 63) / 64);
