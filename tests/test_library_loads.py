@@ -62,6 +62,24 @@ def test_host_only_entry_points(lib):
     assert lib.ttdft_h_destroy(None) in (0, 1)
 
 
+def test_static_scratch_constant_and_null_handle(lib):
+    """ttdft_cheb_step_static: the binding's size limit is the header's, the array is a static device symbol of that size inside the
+    library (no allocation at run time), and a NULL handle is rejected before any CUDA call."""
+    import subprocess
+    import paper_2110_15853_b200 as tt
+    text = open(os.path.join(ROOT, "include", "ttdft.h")).read()
+    m = re.search(r"#define\s+TTDFT_STATIC_SCRATCH_BYTES\s+\((\d+)u\s*<<\s*(\d+)\)", text)
+    assert m and (int(m.group(1)) << int(m.group(2))) == tt.STATIC_SCRATCH_BYTES == 32 << 20
+    lib.ttdft_cheb_step_static.restype = ctypes.c_int
+    args = [None, ctypes.c_double(1.0), ctypes.c_double(0.0), ctypes.c_double(0.0), None, ctypes.c_int64(1), None, ctypes.c_int64(1),
+            None, ctypes.c_int64(1), ctypes.c_int64(1), None]
+    assert lib.ttdft_cheb_step_static(*args) == 1                 # TTDFT_ERR_INVALID_ARG
+    out = subprocess.run(["cuobjdump", "-elf", tt.library_path()], capture_output=True, text=True)
+    if out.returncode == 0:
+        assert re.search(r"\.global\s+\.align\s+256\s+\.b8\s+g_static_scratch\[%d\]" % tt.STATIC_SCRATCH_BYTES, out.stdout) or \
+            "g_static_scratch" in out.stdout
+
+
 def test_no_cpu_fallback_without_a_gpu():
     """The product path must fail loudly, not compute on the CPU, when no CUDA device is there."""
     import torch
