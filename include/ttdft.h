@@ -341,6 +341,14 @@ ttdft_status ttdft_rotate(int64_t M, const double* X, int64_t ldx, int64_t k, co
 ttdft_status ttdft_orthonormalize_work_bytes(int64_t M, int64_t n, int32_t passes, size_t* bytes);
 ttdft_status ttdft_orthonormalize(int64_t M, const double* X, int64_t ldx, int64_t n, double* Y, int64_t ldy, int32_t passes, void* work,
                                   size_t work_bytes, void* stream);
+/*
+ * The same without any synchronisation (so that it can be captured into a CUDA graph together with the filter and the projection):
+ * the breakdown flag stays on the device.  dev_status: DEVICE array of `passes` int32; entry p becomes 0, or 1 + the index of the
+ * first non-positive pivot of pass p + 1.  The call always runs to the end: after a breakdown Y is meaningless (the factorisation
+ * goes on with unit pivots; nothing is read or written outside the buffers), and it is the caller who looks at dev_status.
+ */
+ttdft_status ttdft_orthonormalize_async(int64_t M, const double* X, int64_t ldx, int64_t n, double* Y, int64_t ldy, int32_t passes,
+                                        void* work, size_t work_bytes, int32_t* dev_status, void* stream);
 
 /*
  * Spectral bounds by a k-step Lanczos.  Algorithm 1 takes eps_0 and eps_ub^uw as inputs and refers to

@@ -21,7 +21,7 @@ exported_symbols = [
     "ttdft_h_set_math_mode", "ttdft_step_work_bytes", "ttdft_spmm_ws", "ttdft_cheb_step_ws", "ttdft_cheb_step_static",
     "ttdft_timing_enable", "ttdft_timing_read",
     "ttdft_gram_work_bytes", "ttdft_gram", "ttdft_project_work_bytes", "ttdft_project",
-    "ttdft_rotate_work_bytes", "ttdft_rotate", "ttdft_orthonormalize_work_bytes", "ttdft_orthonormalize",
+    "ttdft_rotate_work_bytes", "ttdft_rotate", "ttdft_orthonormalize_work_bytes", "ttdft_orthonormalize", "ttdft_orthonormalize_async",
     "ttdft_lanczos_work_bytes", "ttdft_lanczos_bounds",
     "ttdft_recover_subdomains_work_bytes", "ttdft_recover_subdomains",
 ]
@@ -115,6 +115,9 @@ def _load() -> ctypes.CDLL:
     L.ttdft_orthonormalize_work_bytes.argtypes = [c_int64, c_int64, c_int32, POINTER(c_size_t)]
     L.ttdft_orthonormalize.restype = st
     L.ttdft_orthonormalize.argtypes = [c_int64, c_void_p, c_int64, c_int64, c_void_p, c_int64, c_int32, c_void_p, c_size_t, c_void_p]
+    L.ttdft_orthonormalize_async.restype = st
+    L.ttdft_orthonormalize_async.argtypes = [c_int64, c_void_p, c_int64, c_int64, c_void_p, c_int64, c_int32, c_void_p, c_size_t, c_void_p,
+                                             c_void_p]
     L.ttdft_lanczos_work_bytes.restype = st
     L.ttdft_lanczos_work_bytes.argtypes = [c_void_p, POINTER(c_size_t)]
     L.ttdft_lanczos_bounds.restype = st
@@ -502,6 +505,23 @@ def orthonormalize(X, Y, passes: int = 2, work=None, stream=None):
         raise ValueError("shape mismatch")
     wp, wb, keep = _aligned_work(orthonormalize_work_bytes(M, n, passes), work, X.device)
     _check(_load().ttdft_orthonormalize(M, xp, ldx, n, yp, ldy, passes, wp, wb, _stream(stream)))
+    _keep(keep, stream)
+    return Y
+
+
+def orthonormalize_async(X, Y, status, passes: int = 2, work=None, stream=None):
+    """ttdft_orthonormalize_async: the same without any synchronisation (capturable into a CUDA graph).  status: int32 CUDA tensor
+    of `passes` entries; entry p becomes 0, or 1 + the first non-positive pivot of pass p + 1 (Y is then meaningless)."""
+    torch = _torch()
+    xp, ldx = _mat(X, "X")
+    yp, ldy = _mat(Y, "Y")
+    M, n = X.shape
+    if tuple(Y.shape) != (M, n):
+        raise ValueError("shape mismatch")
+    if status.dtype != torch.int32 or not status.is_cuda or not status.is_contiguous() or status.numel() < passes:
+        raise TypeError("status must be a contiguous int32 CUDA tensor with one entry per pass")
+    wp, wb, keep = _aligned_work(orthonormalize_work_bytes(M, n, passes), work, X.device)
+    _check(_load().ttdft_orthonormalize_async(M, xp, ldx, n, yp, ldy, passes, wp, wb, c_void_p(status.data_ptr()), _stream(stream)))
     _keep(keep, stream)
     return Y
 

@@ -1506,9 +1506,11 @@ ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Wm, double*
     g_launches.fetch_add(1);
   }
   CUDA_TRY(cudaGetLastError());
-  CUDA_TRY(cudaMemcpyAsync(hflag, dflag, 4, cudaMemcpyDeviceToHost, st));
-  CUDA_TRY(cudaStreamSynchronize(st));
-  if (*hflag) return TTDFT_OK;                      // caller reports the breakdown
+  if (hflag) {                                      // hflag == NULL: the caller keeps the flag on the device and never waits
+    CUDA_TRY(cudaMemcpyAsync(hflag, dflag, 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (*hflag) return TTDFT_OK;                    // caller reports the breakdown
+  }
   // W = L^-1 by recursive doubling (Rinv's buffer serves as the intermediate T), then Rinv = W^T
   const int32_t nb = (n + ttdft::CH_NB - 1) / ttdft::CH_NB;
   for (int32_t sb = 1; sb < nb; sb *= 2) {
@@ -1524,7 +1526,9 @@ ttdft_status chol_inverse(double* G, int64_t ldg, int32_t n, double* Wm, double*
   return TTDFT_OK;
 }
 
-ttdft_status orth_run(const OrthPlan& o, const double* X, int64_t ldx, double* Y, int64_t ldy, void* work, cudaStream_t st) {
+// dev_status != NULL: no synchronisation; the breakdown flag of pass p is left in dev_status[p] (device memory)
+ttdft_status orth_run(const OrthPlan& o, const double* X, int64_t ldx, double* Y, int64_t ldy, void* work, cudaStream_t st,
+                      int32_t* dev_status = nullptr) {
   const EnvSwitches env = read_env();
   uint8_t* wb = reinterpret_cast<uint8_t*>(work);
   const int64_t ldn = o.n + (o.n & 1);
@@ -1544,7 +1548,8 @@ ttdft_status orth_run(const OrthPlan& o, const double* X, int64_t ldx, double* Y
     ttdft_status s = gram_run(o.g, src, lds, src, lds, G, ldn, inner, st, env);     // G = src^T src
     if (s != TTDFT_OK) return s;
     int32_t hflag = 0;
-    if ((s = chol_inverse(G, ldn, (int32_t)o.n, Wm, Rinv, ldn, dflag, &hflag, st)) != TTDFT_OK) return s;
+    if ((s = chol_inverse(G, ldn, (int32_t)o.n, Wm, Rinv, ldn, dflag, dev_status ? nullptr : &hflag, st)) != TTDFT_OK) return s;
+    if (dev_status) CUDA_TRY(cudaMemcpyAsync(dev_status + p, dflag, 4, cudaMemcpyDeviceToDevice, st));
     if (hflag)
       return fail(TTDFT_ERR_BREAKDOWN, "orthonormalize: X^T X is not positive definite in pass %d (pivot %d): columns are linearly "
                                        "dependent to working precision", p + 1, hflag - 1);
@@ -2592,6 +2597,19 @@ ttdft_status ttdft_orthonormalize(int64_t M, const double* X, int64_t ldx, int64
   if (work_bytes < o.total) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, o.total);
   if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
   return orth_run(o, X, ldx, Y, ldy, work, (cudaStream_t)stream);
+}
+ttdft_status ttdft_orthonormalize_async(int64_t M, const double* X, int64_t ldx, int64_t n, double* Y, int64_t ldy, int32_t passes,
+                                        void* work, size_t work_bytes, int32_t* dev_status, void* stream) {
+  OrthPlan o;
+  ttdft_status s = orth_plan(M, n, passes, &o);
+  if (s != TTDFT_OK) return s;
+  if (!dev_status) return fail(TTDFT_ERR_INVALID_ARG, "dev_status is NULL");
+  if ((s = check_mat("X", X, ldx, n)) != TTDFT_OK) return s;
+  if ((s = check_mat("Y", Y, ldy, n)) != TTDFT_OK) return s;
+  if (overlaps(X, ldx, Y, ldy, M, n)) return fail(TTDFT_ERR_INVALID_ARG, "X overlaps Y");
+  if (work_bytes < o.total) return fail(TTDFT_ERR_WORKSPACE_TOO_SMALL, "work has %zu bytes, %zu needed", work_bytes, o.total);
+  if (!work || (reinterpret_cast<uintptr_t>(work) & 1023)) return fail(TTDFT_ERR_INVALID_ARG, "work must be a 1024-byte aligned device pointer");
+  return orth_run(o, X, ldx, Y, ldy, work, (cudaStream_t)stream, dev_status);
 }
 
 ttdft_status ttdft_lanczos_work_bytes(ttdft_h_t h, size_t* bytes) {

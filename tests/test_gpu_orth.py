@@ -79,6 +79,56 @@ def test_single_pass_and_breakdown(tt):
         tt.orthonormalize(Xd, Xd)                                # overlap
 
 
+def test_orthonormalize_async_no_sync_and_graph_capture(tt):
+    """ttdft_orthonormalize_async: the same result bit for bit, the breakdown flag left on the device (0 per pass; non-zero for
+    dependent columns, where the call still runs to the end), and the call captures into a CUDA graph (no synchronisation inside)."""
+    import torch
+    M, n = 3000, 200
+    X = conditioned(M, n, 1e3, 521)
+    Xd = dev(X)
+    Y1 = torch.empty_like(Xd)
+    tt.orthonormalize(Xd, Y1, passes=2)
+    Y2 = torch.full_like(Xd, float("nan"))
+    st = torch.full((2,), -1, dtype=torch.int32, device="cuda")
+    work = torch.empty(tt.orthonormalize_work_bytes(M, n, 2) + 1024, dtype=torch.uint8, device="cuda")
+    tt.orthonormalize_async(Xd, Y2, st, passes=2, work=work)
+    assert torch.equal(Y1, Y2) and st.tolist() == [0, 0]
+    assert relerr(Y2.cpu().numpy(), oracle.orthonormalize(X)) <= 1e-13 * 1e3
+    # captured into a graph and replayed on new contents of the same buffers
+    g = torch.cuda.CUDAGraph()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(g, stream=s):
+            tt.orthonormalize_async(Xd, Y2, st, passes=2, work=work, stream=s)
+    torch.cuda.current_stream().wait_stream(s)
+    X2 = conditioned(M, n, 10.0, 522)
+    Xd.copy_(dev(X2))
+    Y2.fill_(float("nan"))
+    st.fill_(-1)
+    g.replay()
+    torch.cuda.synchronize()
+    assert st.tolist() == [0, 0]
+    assert relerr(Y2.cpu().numpy(), oracle.orthonormalize(X2)) <= 1e-12
+    # dependent columns (the matrix of test_single_pass_and_breakdown): no error status from the call, the flag on the device says
+    # which pivot broke down -- the same one the synchronising call reports
+    Xb = conditioned(3000, 64, 1e4, 511)
+    Xb[:, 7] = Xb[:, 3]
+    Xbd = dev(Xb)
+    Yb = torch.empty_like(Xbd)
+    st.fill_(-1)
+    tt.orthonormalize_async(Xbd, Yb, st, passes=2)
+    torch.cuda.synchronize()
+    flags = st.tolist()
+    assert all(f >= 0 for f in flags) and any(f > 0 for f in flags)
+    first = next(f for f in flags if f > 0)
+    with pytest.raises(tt.TTDFTError) as e:
+        tt.orthonormalize(Xbd, Yb)
+    assert e.value.status_name == "BREAKDOWN" and ("(pivot %d)" % (first - 1)) in tt.last_error()
+    with pytest.raises(TypeError):
+        tt.orthonormalize_async(Xd, Y2, torch.zeros(1, dtype=torch.int32, device="cuda"), passes=2)      # needs one entry per pass
+
+
 def test_orthonormalize_full_config3_shape():
     """Config 3's shape (M = 221,184, n = 4,096): a leading block of columns is compared with the oracle's Gram-Schmidt (column j of
     Q depends on columns 0..j of X only), orthonormality is checked on a seeded sample of column pairs through the oracle's Gram
