@@ -371,12 +371,16 @@ def main():
             pairs = planes * (planes + 1) // 2
             peak, peak_src = int8_peak_tops()
             ops_launch = 2.0 * pairs * nnz * ncols / npanels
-            ops_exec = 2.0 * pairs * H.nblocks * 128 * cfg.b * (-(-ncols // 64) * 64) / npanels
+            mrows = cfg.b if cfg.b in (64, 96) else 128        # K3T (the default for 64- and 96-wide tiles) multiplies no padding rows
+            ops_exec = 2.0 * pairs * H.nblocks * mrows * cfg.b * (-(-ncols // 64) * 64) / npanels
             roof = {"bound": "tensor", "achieved": ops_launch / t_launch / 1e12, "peak": peak, "unit": "TFLOP/s",
                     "frac": ops_launch / t_launch / 1e12 / peak, "kernel": "ttdft::bsr_i8_kernel", "peak_source": peak_src,
                     "ops": f"int8 multiply-add = 2 ops; {pairs} digit-plane products per fp64 product ({planes} planes per operand: "
                            "the implementation's choice of arithmetic, not the method's work)",
                     "executed_tops": ops_exec / t_launch / 1e12, "executed_frac": ops_exec / t_launch / 1e12 / peak,
+                    # the measured-peak figure above is 2 x a power-limited cuBLAS bf16 rate, which an int8 kernel can exceed
+                    # (fewer joules per op): the nominal dense 8-bit peak (B200_PROFILING.md's fp8 row, 4.5 Pop/s; int8 has the same rate) is the hard ceiling
+                    "peak_nominal": 4500.0, "executed_frac_of_nominal": ops_exec / t_launch / 1e12 / 4500.0,
                     "dense_tile_ceiling": useful / executed,
                     "useful_fp64_tflops_kernel": useful / nl / t_launch / 1e12}
         else:
