@@ -38,7 +38,7 @@ FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # (dram__bytes_read.sum + dram__bytes_write.sum), keyed by (workload, kernel): a number copied from that file, NOT measured
 # in this run -- the line prints the file and the commit the capture was taken at beside it.  Missing key = not captured.
 NCU_TRAFFIC = {("si", "bsr_i8"): (103.514e9 + 14.690e9, "profiles/r02_k3_si_full.txt", "5bdfe72"),
-               ("si", "bsr_dmma"): (88.096e9 + 7.241e9, "profiles/r01_k1_si_full.txt", "92819c1")}
+               ("si", "bsr_dmma"): (88.192e9 + 8.039e9, "profiles/r02_k1_si_full.txt", "228981b")}
 
 
 def ncu_traffic(workload, kname):
