@@ -51,23 +51,68 @@ __device__ __forceinline__ void tma_load_4d_mc(void* dst, const CUtensorMap* map
       : "memory");
 }
 
+// first tile group of row tile ctx that is not entirely below the diagonal of G (symmetric mode; 0 otherwise): group g holds the
+// 64-column tiles ctw_begin + g C ... + C - 1, and is needed iff its last column >= the row tile's first row
+template <int C>
+__device__ __forceinline__ int32_t k4_gmin(const K4Params& prm, int32_t ctx) {
+  if (!prm.sym) return 0;
+  const int64_t t = (int64_t)ctx * 128 - (K3_NT - 1) - (int64_t)K3_NT * (prm.ctw_begin + C - 1);      // need  g * 64 C >= t
+  const int64_t g = t <= 0 ? 0 : (t + K3_NT * C - 1) / (K3_NT * C);
+  return (int32_t)min(g, (int64_t)prm.nctwg);
+}
+// work items of one chunk that are computed at all (symmetric mode skips the groups below the diagonal)
+template <int C>
+__device__ __forceinline__ int64_t k4_valid_per_chunk(const K4Params& prm) {
+  if (!prm.sym) return (int64_t)prm.nctx * prm.nctwg;
+  int64_t n = 0;
+  for (int32_t ctx = 0; ctx < prm.nctx; ++ctx) n += prm.nctwg - k4_gmin<C>(prm, ctx);
+  return n;
+}
 // cluster work item u -> (chunk, row tile ctx, tile group ctwg).  Chunks outermost; inside a chunk the tiles of G are
 // walked in super-tiles of 8 row tiles x 9 tile groups (72 ~ the 74 co-resident 2-CTA clusters), so that the clusters
 // running at the same time walk the same blocks of the contraction on few distinct operand tiles: 8 X tile pairs +
 // 18 W tiles per block instead of 2-3 X pairs + 64 W tiles, i.e. each W tile is fetched from HBM once per 8 row tiles
-// instead of once per row tile.
-__device__ __forceinline__ void k4_decode(const K4Params& prm, int64_t u, int32_t& chunk, int32_t& ctx, int32_t& ctwg) {
+// instead of once per row tile.  In symmetric mode ONLY the computed items are numbered (nvalid per chunk): were the
+// skipped ones numbered too, a cluster that draws one would move on to the next wave at once, the waves would mix and the
+// clusters in flight would no longer share their operand tiles (143 GB of DRAM traffic per launch at config 3's shape).
+template <int C>
+__device__ __forceinline__ void k4_decode(const K4Params& prm, int64_t u, int64_t nvalid, int32_t& chunk, int32_t& ctx, int32_t& ctwg) {
   constexpr int SX = 8, SW = 9;
-  const int64_t per_chunk = (int64_t)prm.nctx * prm.nctwg;
-  chunk = (int32_t)(u / per_chunk);
-  const int32_t rem = (int32_t)(u - (int64_t)chunk * per_chunk);
-  const int32_t sx = rem / (SX * prm.nctwg);
-  const int32_t hx = min(SX, prm.nctx - sx * SX);            // row tiles in this super row
-  const int32_t rem2 = rem - sx * SX * prm.nctwg;
-  const int32_t sw = rem2 / (hx * SW);
-  const int32_t rem3 = rem2 - sw * hx * SW;
-  ctx = sx * SX + rem3 % hx;
-  ctwg = sw * SW + rem3 / hx;
+  chunk = (int32_t)(u / nvalid);
+  int32_t v = (int32_t)(u - (int64_t)chunk * nvalid);
+  if (!prm.sym) {
+    const int32_t sx = v / (SX * prm.nctwg);
+    const int32_t hx = min(SX, prm.nctx - sx * SX);            // row tiles in this super row
+    const int32_t rem2 = v - sx * SX * prm.nctwg;
+    const int32_t sw = rem2 / (hx * SW);
+    const int32_t rem3 = rem2 - sw * hx * SW;
+    ctx = sx * SX + rem3 % hx;
+    ctwg = sw * SW + rem3 / hx;
+    return;
+  }
+  for (int32_t x0 = 0; x0 < prm.nctx; x0 += SX) {
+    const int32_t hx = min(SX, prm.nctx - x0);
+    int32_t gm[SX];
+#pragma unroll
+    for (int i = 0; i < SX; ++i) gm[i] = i < hx ? k4_gmin<C>(prm, x0 + i) : prm.nctwg;
+    for (int32_t g0 = 0; g0 < prm.nctwg; g0 += SW) {
+      const int32_t g1 = min(g0 + SW, prm.nctwg);
+      int32_t cnt = 0;
+#pragma unroll
+      for (int i = 0; i < SX; ++i) cnt += max(0, g1 - max(g0, gm[i]));
+      if (v < cnt) {                                           // in this super-tile: same order as above, valid items only
+        for (int32_t g = g0; g < g1; ++g)
+#pragma unroll
+          for (int i = 0; i < SX; ++i)
+            if (g >= gm[i]) {
+              if (v == 0) { ctx = x0 + i; ctwg = g; return; }
+              --v;
+            }
+      }
+      v -= cnt;
+    }
+  }
+  ctx = 0; ctwg = 0;                                           // not reached for u < nchunks * nvalid
 }
 
 // a work item is skipped in symmetric mode if even its last 64-column tile lies entirely below the diagonal of G
@@ -111,7 +156,8 @@ gram_i8_kernel(const __grid_constant__ CUtensorMap tmXd, const __grid_constant__
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + Cf::CM_OFFSET) + 64;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t nitems = (int64_t)prm.nchunks * prm.nctx * prm.nctwg;
+  const int64_t nvalid = k4_valid_per_chunk<C>(prm);          // computed items per chunk (all of them unless symmetric)
+  const int64_t nitems = (int64_t)prm.nchunks * nvalid;
   const int32_t crank = (C > 1) ? (int32_t)cluster_ctarank() : 0;
   const int64_t cluster0 = blockIdx.x / C, nclusters = gridDim.x / C;
   constexpr uint16_t cmask = (uint16_t)((1u << C) - 1u);
@@ -144,7 +190,7 @@ gram_i8_kernel(const __grid_constant__ CUtensorMap tmXd, const __grid_constant__
       constexpr int ncol = 64 / C;               // columns of each of the two X tiles this CTA fetches per plane
       for (int64_t u = cluster0; u < nitems; u += nclusters) {
         int32_t chunk, ctx, ctwg;
-        k4_decode(prm, u, chunk, ctx, ctwg);
+        k4_decode<C>(prm, u, nvalid, chunk, ctx, ctwg);
         const int32_t ctw = prm.ctw_begin + ctwg * C + crank;
         if (k4_skip(prm, ctx, prm.ctw_begin + ctwg * C + C - 1)) continue;
         const int32_t I0 = chunk * prm.kc, I1 = min(prm.nbk, I0 + prm.kc);
@@ -182,7 +228,7 @@ gram_i8_kernel(const __grid_constant__ CUtensorMap tmXd, const __grid_constant__
       const uint32_t ylo0 = (smem_u32(ybuf) & 0x3ffffu) >> 4, hlo0 = (smem_u32(hring) & 0x3ffffu) >> 4;
       for (int64_t u = cluster0; u < nitems; u += nclusters) {
         int32_t chunk, ctx, ctwg;
-        k4_decode(prm, u, chunk, ctx, ctwg);
+        k4_decode<C>(prm, u, nvalid, chunk, ctx, ctwg);
         if (k4_skip(prm, ctx, prm.ctw_begin + ctwg * C + C - 1)) continue;
         const int32_t nI = min(prm.nbk, chunk * prm.kc + prm.kc) - chunk * prm.kc;
         mbar_wait(accempty, aph ^ 1);
@@ -229,7 +275,7 @@ gram_i8_kernel(const __grid_constant__ CUtensorMap tmXd, const __grid_constant__
     uint32_t aph = 0;
     for (int64_t u = cluster0; u < nitems; u += nclusters) {
       int32_t chunk, ctx, ctwg;
-      k4_decode(prm, u, chunk, ctx, ctwg);
+      k4_decode<C>(prm, u, nvalid, chunk, ctx, ctwg);
       const int32_t ctw = prm.ctw_begin + ctwg * C + crank;
       if (k4_skip(prm, ctx, prm.ctw_begin + ctwg * C + C - 1)) continue;
       const int64_t lcol0 = (int64_t)ctw * K3_NT;            // column inside the panel
