@@ -22,7 +22,8 @@ namespace ttdft {
 
 struct K4Params {
   int32_t nbk;                 // 128-row blocks of the contraction = ceil(M / 128)
-  int32_t kc, nchunks;         // blocks per chunk, chunks
+  int32_t kc, nchunks;         // blocks per chunk, chunks of THIS launch
+  int32_t chunk0 = 0;          // first chunk of this launch (a product is launched in groups of a few chunks)
   int32_t nctx;                // 128-column tiles of X (row tiles of G)
   int32_t nctX, nctW;          // 64-column tiles per block in the digit arrays of X (even) and W
   int32_t ctw_begin, nctwg;    // this launch: first 64-column tile of W, groups of C tiles
@@ -78,8 +79,9 @@ __device__ __forceinline__ int64_t k4_valid_per_chunk(const K4Params& prm) {
 template <int C>
 __device__ __forceinline__ void k4_decode(const K4Params& prm, int64_t u, int64_t nvalid, int32_t& chunk, int32_t& ctx, int32_t& ctwg) {
   constexpr int SX = 8, SW = 9;
-  chunk = (int32_t)(u / nvalid);
-  int32_t v = (int32_t)(u - (int64_t)chunk * nvalid);
+  const int32_t lc = (int32_t)(u / nvalid);                    // chunk inside this launch
+  chunk = prm.chunk0 + lc;
+  int32_t v = (int32_t)(u - (int64_t)lc * nvalid);
   if (!prm.sym) {
     const int32_t sx = v / (SX * prm.nctwg);
     const int32_t hx = min(SX, prm.nctx - sx * SX);            // row tiles in this super row
