@@ -510,7 +510,8 @@ def main():
         tt.timing_enable(False)
         pk = {k: tt.timing_read(k) for k in tt.KERNEL_IDS}
         t_p = g0.elapsed_time(g1) * 1e-3 / 2
-        gram_ms = pk["gram_i8"][0] / max(pk["gram_i8"][1], 1)
+        gram_ms = pk["gram_i8"][0] / 2                 # K4's time per ttdft_project call (the product runs as several launches)
+        gram_launches = pk["gram_i8"][1] // 2
         # The handle was built with TTDFT_CHECK_SYMMETRY, so H_F = H_F^T is known and ttdft_project computes only the entries on and
         # above the diagonal (the method's own work: N(N+1)/2 entries of 2M flops), as whole 128 x 128 tile groups (executed work).
         n128 = -(-cfg.N // 128)
@@ -526,6 +527,7 @@ def main():
             "kernels_ms_each": {k: v[0] / v[1] for k, v in pk.items() if v[1]},
             "gram_roofline": {"bound": "tensor", "achieved": 28.0 * fl_gram / (gram_ms * 1e-3) / 1e12, "peak": peak8, "unit": "TFLOP/s",
                               "frac": 28.0 * fl_gram / (gram_ms * 1e-3) / 1e12 / peak8, "peak_source": peak8_src, "launch_ms": gram_ms,
+                              "launches": gram_launches,       # launch_ms is their sum: the whole Gram product
                               "ops": "method's own work: N(N+1)/2 entries x 2M flops x 28 digit-plane products",
                               "executed_tops": 28.0 * fl_gram_exec / (gram_ms * 1e-3) / 1e12,
                               "executed_frac": 28.0 * fl_gram_exec / (gram_ms * 1e-3) / 1e12 / peak8,
